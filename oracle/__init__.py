@@ -1,0 +1,157 @@
+"""ORACLE — TEST INFRASTRUCTURE ONLY (see bg_oracle.cpp header).
+
+ctypes front end to ``libbgoracle.so`` (plain C++ written from PAPER.md).  Only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may import this.
+It imports nothing from ``paper_2106_06507_b200``.
+
+Arrays are AoS: ``mom[N][n][4]`` float64 (E,px,py,pz; all-outgoing), ``hel[N][n]`` int8 (+1/-1),
+``col[N][n][2]`` int8 in {1,2,3}.  ``prec``: ``"double"`` or ``"long double"`` (x87 80-bit, the round-off truth).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "bg_oracle.cpp")
+_LIB = os.path.join(_HERE, "libbgoracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fopenmp", "-shared", "-fPIC", _SRC, "-o", _LIB])
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        for name in ("bgo_polarisation", "bgo_cobg_amp_ext", "bgo_cobg_amp", "bgo_colour_matrix",
+                     "bgo_cobg_full_colour", "bgo_cdbg", "bgo_colour_flow", "bgo_max_threads"):
+            getattr(_lib, name).restype = ctypes.c_int
+    return _lib
+
+
+def _prec(prec: str) -> int:
+    return {"double": 0, "long double": 1}[prec]
+
+
+def _p(a):
+    return None if a is None else ctypes.c_void_p(a.ctypes.data)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i8(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.int8)
+
+
+def max_threads() -> int:
+    return int(_load().bgo_max_threads())
+
+
+def polarisation(p, lam: int) -> np.ndarray:
+    """eps^lam(p) as a complex 4-vector (upper index)."""
+    p = _f64(p)
+    out = np.empty((4, 2))
+    _load().bgo_polarisation(_p(p), ctypes.c_int(int(lam)), _p(out))
+    return out[:, 0] + 1j * out[:, 1]
+
+
+def cobg_amp_ext(mom, ext, tensor_form: bool = False, prec: str = "double") -> complex:
+    """Colour-ordered amplitude (Eq. 20/22) for explicit external currents ext[n][4] complex; legs in order."""
+    mom = _f64(mom)
+    n = mom.shape[0]
+    e = np.ascontiguousarray(np.stack([np.real(ext), np.imag(ext)], axis=-1), dtype=np.float64)
+    out = np.empty(2)
+    rc = _load().bgo_cobg_amp_ext(n, _p(mom), _p(e), int(tensor_form), _prec(prec), _p(out))
+    assert rc == 0
+    return complex(out[0], out[1])
+
+
+def cobg_amp(mom, hel, order, tensor_form: bool = False, prec: str = "double") -> complex:
+    """A(order[0],..,order[n-1]) for one event; order holds 0-based gluon labels."""
+    mom = _f64(mom)
+    n = mom.shape[0]
+    hel = _i8(hel)
+    order = np.ascontiguousarray(order, dtype=np.int32)
+    assert order.shape[0] == n
+    out = np.empty(2)
+    rc = _load().bgo_cobg_amp(n, _p(mom), _p(hel), _p(order), int(tensor_form), _prec(prec), _p(out))
+    assert rc == 0
+    return complex(out[0], out[1])
+
+
+_cm_cache: dict[int, np.ndarray] = {}
+
+
+def colour_matrix(n: int) -> np.ndarray:
+    """Eq. 17 from its definition; sigma over permutations of gluons 2..n-1 in lexicographic order."""
+    if n not in _cm_cache:
+        import math
+        m = math.factorial(n - 2)
+        C = np.empty((m, m))
+        rc = _load().bgo_colour_matrix(n, _p(C))
+        assert rc == 0
+        # Eq. 17 is integer-valued in this normalisation (a signed sum of powers of N_c); the floating-point
+        # evaluation from Gell-Mann matrices carries ~1e-12 noise, removed here after checking it is noise.
+        Cr = np.rint(C)
+        assert np.max(np.abs(C - Cr)) < 1e-7, "colour matrix not integer-valued"
+        _cm_cache[n] = Cr
+    return _cm_cache[n]
+
+
+def cobg_full_colour(mom, hel=None, C=None, tensor_form: bool = False, prec: str = "double", threads: int = 0,
+                     return_amps: bool = False):
+    """Batched sum_{sigma sigma'} C A A^* (Eq. 16).  hel=None sums all 2^n helicity assignments."""
+    mom = _f64(mom)
+    N, n = mom.shape[0], mom.shape[1]
+    hel = _i8(hel)
+    if C is None:
+        C = colour_matrix(n)
+    C = _f64(C)
+    out = np.empty(N)
+    amps = None
+    if return_amps:
+        assert hel is not None
+        amps = np.empty((N, C.shape[0], 2))
+    rc = _load().bgo_cobg_full_colour(n, ctypes.c_longlong(N), _p(mom), _p(hel), _p(C), int(tensor_form),
+                                      _prec(prec), int(threads), _p(out), _p(amps))
+    assert rc == 0
+    if return_amps:
+        return out, amps[..., 0] + 1j * amps[..., 1]
+    return out
+
+
+def cdbg(mom, hel, col, prec: str = "double", threads: int = 0, return_live: bool = False):
+    """Batched colour-dressed |A|^2 (Eq. 28-32, colour-flow basis, given helicities and colours)."""
+    mom = _f64(mom)
+    N, n = mom.shape[0], mom.shape[1]
+    hel, col = _i8(hel), _i8(col)
+    out = np.empty(N)
+    live = np.empty(N, dtype=np.int64)
+    rc = _load().bgo_cdbg(n, ctypes.c_longlong(N), _p(mom), _p(hel), _p(col), _prec(prec), int(threads), _p(out),
+                          _p(live))
+    assert rc == 0
+    return (out, live) if return_live else out
+
+
+def colour_flow(mom, hel, col, prec: str = "double", threads: int = 0, return_count: bool = False):
+    """Batched Eq. 19 brute force: |sum over colour-connected orderings of COBG amplitudes|^2."""
+    mom = _f64(mom)
+    N, n = mom.shape[0], mom.shape[1]
+    hel, col = _i8(hel), _i8(col)
+    out = np.empty(N)
+    cnt = np.empty(N, dtype=np.int64)
+    rc = _load().bgo_colour_flow(n, ctypes.c_longlong(N), _p(mom), _p(hel), _p(col), _prec(prec), int(threads),
+                                 _p(out), _p(cnt))
+    assert rc == 0
+    return (out, cnt) if return_count else out
