@@ -1,0 +1,311 @@
+#!/usr/bin/env python
+"""bench.py — n-gluon |M|^2 events/s on B200 (BASELINE.json metric), one JSON line on stdout.
+
+A "step" is one pass of the whole hot path (load event, external currents, recursion, closure / colour assembly,
+store) over one batch of synthetic events.  Default workload: BASELINE.json configs[1]
+(n = 6 gluons, colour-dressed recursion with sampled helicities and colour flows, 2^20 RAMBO events).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--n n] [--events N] [--kernel k]
+  python bench.py --impl reference ...      # the CPU oracle on the host cores (bounded sample per step)
+
+Multi-GPU (torchrun): events are independent, so each rank evaluates its own batch of the
+same size with no data-path collective (weak scaling); timing is max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+# Algorithmic FP64 work per event of the colour-dressed recursion with sampled discrete colours (SURVEY.md §8d,
+# mean over sampled colour assignments), and of the colour-ordered configs.
+CDBG_FLOP_PER_EVENT = {4: 2.1e3, 5: 8.4e3, 6: 2.5e4, 7: 7.0e4, 8: 2.2e5, 9: 6.4e5, 10: 1.9e6, 11: 5.1e6, 12: 1.46e7}
+COBG_FLOP_PER_EVENT = {0: 2.6e4, 2: 1.41e6 + 5.8e4}     # config 0 (n=4 helsum), config 2 (n=7 + colour form)
+CONFIG_N = {0: 4, 1: 6, 2: 7, 3: 9}
+CONFIG_EVENTS = {0: 1024, 1: 1 << 20, 2: 1 << 18, 3: 1 << 18, 4: 1 << 16}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--n", type=int, default=None, help="gluon multiplicity for the sweep config 4")
+    ap.add_argument("--events", type=int, default=None, help="override the number of events per step and GPU")
+    ap.add_argument("--kernel", type=int, default=0, help="BG_OPT_KERNEL (0 auto, 1 generic, 2 quad)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload_desc(args):
+    n = CONFIG_N.get(args.config, args.n)
+    if n is None:
+        raise SystemExit("--config 4 needs --n")
+    N = args.events or CONFIG_EVENTS[args.config]
+    if args.config in (0, 2):
+        flop = COBG_FLOP_PER_EVENT[args.config]
+    else:
+        flop = CDBG_FLOP_PER_EVENT[n]
+    names = {0: "C1 n=4 COBG helicity-summed full-colour", 1: "C2 n=6 CDBG sampled helicity+colour",
+             2: "C3 n=7 COBG sampled helicity full-colour (120x120)", 3: "C4 n=9 CDBG sampled helicity+colour",
+             4: f"C5 n={n} CDBG sampled helicity+colour"}
+    return n, N, flop, names[args.config]
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4)}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2)
+        med = int(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def make_events(args, n, N, rank):
+    from paper_2106_06507_b200 import workload as wl
+    return wl.config_events(args.config, N=N, n=n if args.config == 4 else None, first_event=rank * N)
+
+
+def mode_for(config):
+    import paper_2106_06507_b200 as bg
+    return {0: bg.BG_COBG_HELSUM_FULLCOLOR, 2: bg.BG_COBG_HELGIVEN_FULLCOLOR}.get(config, bg.BG_CDBG_GIVEN)
+
+
+def oracle_eval(args, ev, threads=0):
+    import oracle
+    if args.config == 0:
+        return oracle.cobg_full_colour(ev.mom, None, threads=threads)
+    if args.config == 2:
+        return oracle.cobg_full_colour(ev.mom, ev.hel, threads=threads)
+    return oracle.cdbg(ev.mom, ev.hel, ev.col, threads=threads)
+
+
+def cpu_sample_size(args, n, N):
+    """Events per oracle timing sample: about 10-30 s of CPU work (single-core estimates per event)."""
+    per_event = {0: 6e-5, 2: 4e-3}.get(args.config)
+    if per_event is None:
+        per_event = {4: 1.5e-6, 5: 6e-6, 6: 2.0e-5, 7: 6e-5, 8: 1.8e-4, 9: 5e-4, 10: 1.6e-3, 11: 5e-3, 12: 1.5e-2}[n]
+    return int(max(64, min(N, 20.0 / per_event)))
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, on the host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    n, N, flop, name = workload_desc(args)
+    S = cpu_sample_size(args, n, N)
+    S = max(64, S // max(1, args.steps + args.warmup) * 2) if args.steps + args.warmup > 4 else S
+    ev = make_events(args, n, S, 0)
+    cores = oracle.max_threads()
+    for _ in range(max(1, min(args.warmup, 3))):
+        oracle_eval(args, ev.head(max(64, S // 8)))
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_eval(args, ev)
+    dt = time.perf_counter() - t0
+    value = S * args.steps / dt
+    line = {"impl": "reference", "metric": "n-gluon |M|^2 events/sec", "value": value, "unit": "events/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "n": n, "events_per_step": S, "note": "CPU oracle (oracle/bg_oracle.cpp, "
+                       "double, OpenMP), bounded sample of the workload per step"},
+            "cpu_baseline": {"value": value, "unit": "events/s", "cores": cores, "kind": "oracle",
+                             "sample": f"{S} events per step x {args.steps} steps of {name}"},
+            "e2e": {"value": value, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2106_06507_b200 as bg
+    from paper_2106_06507_b200 import workload as wl
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the B200 path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    n, N, flop_per_event, name = workload_desc(args)
+    ev = make_events(args, n, N, rank)
+    mode = mode_for(args.config)
+    mom = wl.to_soa(mom=ev.mom)
+    hel = None if ev.hel is None else wl.to_soa(hel=ev.hel)
+    col = None if ev.col is None else wl.to_soa(col=ev.col)
+    # pinned host copies (end-to-end path) and device-resident copies (kernel path)
+    h_mom = torch.from_numpy(mom).pin_memory()
+    h_hel = None if hel is None else torch.from_numpy(hel).pin_memory()
+    h_col = None if col is None else torch.from_numpy(col).pin_memory()
+    h_out = torch.empty(N, dtype=torch.float64).pin_memory()
+    d_mom = h_mom.to(dev)
+    d_hel = None if h_hel is None else h_hel.to(dev)
+    d_col = None if h_col is None else h_col.to(dev)
+    d_out = torch.empty(N, dtype=torch.float64, device=dev)
+
+    ctx = bg.bg_init(n, mode)
+    if args.kernel:
+        bg.bg_set_option(ctx, bg.BG_OPT_KERNEL, args.kernel)
+    bg.bg_reserve(ctx, N)
+    stream = torch.cuda.current_stream()
+    sh = stream.cuda_stream
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        bg.bg_eval(ctx, sh, N, d_mom, d_hel, d_col, d_out)
+
+    peak_tf = bg.bg_fp64_peak_probe(1 << 14) if rank == 0 else None
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    e0.record(stream)
+    for a, b in evs:
+        a.record(stream)
+        step()
+        b.record(stream)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    total_ms = e0.elapsed_time(e1)
+    launches_per_step = bg.bg_last_launch_count(ctx)
+    kernel_name = bg.bg_last_kernel_name(ctx)
+    kernel_ms = float(np.mean([a.elapsed_time(b) for a, b in evs])) / max(1, launches_per_step)
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    value = N * world * args.steps / (total_ms * 1e-3)
+
+    # end-to-end: host buffers through bg_eval_host (H2D of inputs + D2H of results inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        k2 = max(3, min(args.steps, 10))
+        for _ in range(2):
+            bg.bg_eval_host(ctx, N, h_mom, h_hel, h_col, h_out)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(k2):
+            bg.bg_eval_host(ctx, N, h_mom, h_hel, h_col, h_out)
+        barrier()
+        dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        h2d = mom.nbytes + (0 if hel is None or mode & bg.BG_HEL_SUM else hel.nbytes) + \
+            (0 if col is None or not (mode & bg.BG_COL_GIVEN) else col.nbytes)
+        e2e = {"value": N * world * k2 / float(dt.item()), "unit": "events/s", "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(N * 8), "steps": k2}
+        if rank == 0 and not np.allclose(h_out.numpy(), d_out.cpu().numpy(), rtol=0, atol=0, equal_nan=True):
+            raise SystemExit("bench.py: host path and device path disagree")
+
+    if rank == 0:
+        out_host = d_out.cpu().numpy()
+        if not np.all(np.isfinite(out_host)):
+            raise SystemExit("bench.py: non-finite |M|^2 in the output")
+        achieved_tf = flop_per_event * N / (kernel_ms * 1e-3 * launches_per_step) * 1e-12
+        roofline = {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                    "frac": achieved_tf / peak_tf, "traffic": None, "kernel": kernel_name,
+                    "peak_source": "bg_fp64_peak_probe (DFMA chains, this run); nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2",
+                    "flop_per_event": flop_per_event, "kernel_ms": kernel_ms * launches_per_step}
+        cpu = None
+        if not args.no_cpu_baseline:
+            import oracle
+            S = cpu_sample_size(args, n, N)
+            sample = ev.head(S)
+            oracle_eval(args, sample.head(max(64, S // 16)))
+            t0 = time.perf_counter()
+            ref = oracle_eval(args, sample)
+            dt = time.perf_counter() - t0
+            err = np.abs(out_host[:S] - ref) / np.abs(ref)
+            cpu = {"value": S / dt, "unit": "events/s", "cores": oracle.max_threads(), "kind": "oracle",
+                   "sample": f"first {S} events of the workload, {dt:.2f} s wall",
+                   "median_rel_diff_gpu_vs_oracle": float(np.median(err))}
+        line = {"metric": "n-gluon |M|^2 events/sec (device-timed)", "value": value, "unit": "events/s",
+                "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+                "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": name, "n": n, "events_per_step_per_gpu": N, "mode": hex(mode),
+                           "l2": "inputs larger than L2" if mom.nbytes > 126e6 else "inputs fit L2 (no flush; "
+                           "compute-bound kernel, compulsory traffic 35n+8 B/event)",
+                           "kernel": kernel_name, "current_bytes_per_event": bg.bg_current_bytes_per_event(ctx)},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
+                "roofline": roofline, "cpu_baseline": cpu}
+        print(json.dumps(line), flush=True)
+    bg.bg_destroy(ctx)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,132 @@
+/*
+ * bg.h — C-ABI of the B200-native Berends-Giele engine (all-gluon tree-level |M|^2, FP64).
+ *
+ * Method: arxiv 2106.06507, "Many-gluon tree amplitudes on modern GPUs" (PAPER.md = /root/reference/PAPER.md).
+ * Conventions: n gluons labelled 1..n, ALL-OUTGOING momenta (sum p = 0;
+ * an incoming gluon enters with -p_phys), metric (+,-,-,-), N_c = 3, g_s = 1, Tr(T^a T^b) = delta^ab
+ * (PAPER.md:L187).  No averaging, symmetry factor, coupling or sampling weight is applied to `out`.
+ *
+ * Storage of per-event inputs is event-fastest ("SoA"): element (event e, gluon k, component c) of
+ *     mom : mom[(k*4 + c)*N + e]   c = (E, px, py, pz)          double
+ *     hel : hel[k*N + e]           +1 / -1 (all-outgoing labels) signed char
+ *     col : col[(k*2 + a)*N + e]   a = 0: i_k, a = 1: j_k, values 1..3 (colour-flow indices)
+ *     out : out[e]                                              double
+ * so that consecutive threads read consecutive addresses.
+ *
+ * Ownership: every pointer passed to bg_eval is a DEVICE pointer owned by the caller (for instance the
+ * data_ptr() of a torch tensor); the library neither frees nor keeps it.  bg_eval_host takes HOST pointers.
+ * The context owns the colour matrix and scratch buffers on the device that was current at bg_init.
+ *
+ * Errors: every int-returning call returns BG_OK (0) or a negative code; nothing throws across the ABI and
+ * nothing is printed.  There is no CPU fallback: without a CUDA device bg_init returns BG_ECUDA.
+ */
+#ifndef BG_H
+#define BG_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bg_ctx bg_ctx; /* opaque */
+
+enum {
+    BG_OK = 0,
+    BG_EINVAL = -1,       /* bad argument (n out of range, NULL pointer the mode needs, N < 0, ...) */
+    BG_ENOMEM = -2,       /* host or device allocation failed */
+    BG_ECUDA = -3,        /* CUDA runtime error (no device, launch failure, ...) */
+    BG_EUNSUPPORTED = -4  /* mode / n combination not implemented */
+};
+
+/* mode = recursion | helicity treatment | colour treatment */
+enum {
+    BG_REC_COBG = 0x001,  /* colour-ordered recursion, Eq. 20-22 */
+    BG_REC_CDBG = 0x002,  /* colour-dressed recursion, Eq. 28-32 */
+    BG_HEL_SUM = 0x010,   /* sum over all 2^n helicity assignments, Eq. 4; hel must be NULL */
+    BG_HEL_GIVEN = 0x020, /* one assignment per event in hel */
+    BG_COL_FULL = 0x100,  /* full-colour sum sum_{s,s'} C_{ss'} A_s A_s'^*, Eq. 15-17; col NULL */
+    BG_COL_GIVEN = 0x200, /* one colour-flow assignment (i_k, j_k) per gluon per event in col, Eq. 19 */
+
+    BG_COBG_HELSUM_FULLCOLOR = BG_REC_COBG | BG_HEL_SUM | BG_COL_FULL,     /* BASELINE config 1 */
+    BG_COBG_HELGIVEN_FULLCOLOR = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_FULL, /* BASELINE config 3 */
+    BG_CDBG_GIVEN = BG_REC_CDBG | BG_HEL_GIVEN | BG_COL_GIVEN,             /* BASELINE configs 2, 4, 5 */
+    BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN
+};
+
+/* bg_set_option keys */
+enum {
+    BG_OPT_KERNEL = 1,       /* 0 = automatic choice by n; 1 = generic thread-per-event kernels with currents in
+                                global scratch (any n); 2 = quad kernel, currents in shared memory (CDBG) */
+    BG_OPT_SCRATCH_LIMIT = 2 /* upper bound in bytes for the scratch the generic kernels may use (default 16 GiB) */
+};
+
+/*
+ * Create a context for n gluons (4 <= n <= 12) in the given mode on the current CUDA device.
+ * COBG full-colour modes need n <= 8 ((n-2)!^2 colour-matrix entries); they build the colour
+ * matrix C of Eq. 17 (exact integers, orderings sigma = permutations of gluons 2..n-1 in lexicographic order)
+ * on the host and upload it.  Returns BG_EUNSUPPORTED for other mode combinations.
+ */
+int bg_init(bg_ctx** ctx, int n, int mode);
+
+/*
+ * Evaluate |M|^2 for N events, asynchronously on `cuda_stream` (a cudaStream_t; NULL = default stream).
+ *   COBG + FULL colour : out[e] = sum_{sigma,sigma'} C A_sigma A_sigma'^*  (Eq. 16), A from Eq. 20 + 22, for the
+ *                        helicities in hel, or summed over all 2^n assignments when the mode has BG_HEL_SUM.
+ *   CDBG + GIVEN colour: out[e] = |A_{i1 j1 .. in jn}|^2 from the subset recursion Eq. 29-32 closed with gluon n
+ *                        (Eq. 22); assignments whose amplitude vanishes identically return exactly 0.0.
+ * External currents are the helicity eigenvectors of Eq. 3 in the light-cone gauge of DESIGN.md reading g2.
+ * No host synchronisation and no allocation happen here when bg_reserve was called for >= N events; otherwise
+ * scratch is (re)allocated first, which synchronises.  Inputs are not validated on the device: non-finite or
+ * off-shell momenta give unspecified (possibly NaN) output, never a fault.  N = 0 is a no-op.
+ */
+int bg_eval(bg_ctx* ctx, void* cuda_stream, long long N, const double* mom, const signed char* hel,
+            const signed char* col, double* out);
+
+/*
+ * Same computation with HOST buffers (same layouts): copies inputs to the device, runs bg_eval on an internal
+ * stream, copies `out` back and waits.  Staging buffers are owned by the context (grown by bg_reserve).
+ */
+int bg_eval_host(bg_ctx* ctx, long long N, const double* mom, const signed char* hel, const signed char* col,
+                 double* out);
+
+/* Pre-allocate scratch (and host-path staging) for up to N events per call, so bg_eval never allocates. */
+int bg_reserve(bg_ctx* ctx, long long N);
+
+/* Bytes of device scratch a call with N events uses with the current options (0 for kernels that keep all
+ * currents on chip). */
+size_t bg_scratch_bytes(const bg_ctx* ctx, long long N);
+
+/* Bytes of current storage (vector + tensor currents) one event occupies in the selected kernel. */
+size_t bg_current_bytes_per_event(const bg_ctx* ctx);
+
+int bg_set_option(bg_ctx* ctx, int key, long long value);
+
+/* Copy the (n-2)! x (n-2)! colour matrix (row-major doubles) to a host buffer; BG_EINVAL for CDBG contexts. */
+int bg_colour_matrix(const bg_ctx* ctx, double* C_host);
+
+/* Host-only: build the colour matrix of Eq. 17 for n gluons (4 <= n <= 8) into C_host[(n-2)!^2] without a
+ * context or a device (this is what bg_init uploads). */
+int bg_build_colour_matrix(int n, double* C_host);
+
+/* Number of kernels the most recent bg_eval / bg_eval_host launched. */
+int bg_last_launch_count(const bg_ctx* ctx);
+
+/* Name of the kernel variant the most recent bg_eval used (static string). */
+const char* bg_last_kernel_name(const bg_ctx* ctx);
+
+int bg_destroy(bg_ctx* ctx);
+
+const char* bg_strerror(int code);
+
+/*
+ * Measure the FP64 FMA throughput of the current device with a register-resident DFMA chain benchmark
+ * (all SMs, 8 independent chains per thread).  Writes TFLOP/s (2 flop per FMA) to *tflops.  Used by bench.py
+ * as the "alu" roofline denominator; synchronous.
+ */
+int bg_fp64_peak_probe(int iterations, double* tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BG_H */

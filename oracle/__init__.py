@@ -131,17 +131,23 @@ def cobg_full_colour(mom, hel=None, C=None, tensor_form: bool = False, prec: str
     return out
 
 
-def cdbg(mom, hel, col, prec: str = "double", threads: int = 0, return_live: bool = False):
-    """Batched colour-dressed |A|^2 (Eq. 28-32, colour-flow basis, given helicities and colours)."""
+def cdbg(mom, hel, col, prec: str = "double", threads: int = 0, return_live: bool = False,
+         return_rho: bool = False):
+    """Batched colour-dressed |A|^2 (Eq. 28-32, colour-flow basis, given helicities and colours).
+
+    ``return_rho`` adds the top-level cancellation ratio rho = |A| / sum_terms |eps_n . term| (terms = the
+    ordered-split contributions to the last current), the conditioning measure of DESIGN.md's parity protocol."""
     mom = _f64(mom)
     N, n = mom.shape[0], mom.shape[1]
     hel, col = _i8(hel), _i8(col)
     out = np.empty(N)
     live = np.empty(N, dtype=np.int64)
+    rho = np.empty(N)
     rc = _load().bgo_cdbg(n, ctypes.c_longlong(N), _p(mom), _p(hel), _p(col), _prec(prec), int(threads), _p(out),
-                          _p(live))
+                          _p(live), _p(rho))
     assert rc == 0
-    return (out, live) if return_live else out
+    res = (out,) + ((live,) if return_live else ()) + ((rho,) if return_rho else ())
+    return res if len(res) > 1 else out
 
 
 def colour_flow(mom, hel, col, prec: str = "double", threads: int = 0, return_count: bool = False):

@@ -296,9 +296,12 @@ template <class R> R cobg_full_colour_helsum(int n, const V4r<R>* mom, const dou
 //   A = sum_{hg} (eps_n . J({1..n-1})_{hg}) [g==i_n][h==j_n];  out = |A|^2
 template <class R>
 cx<R> cdbg_amplitude(int n, const V4r<R>* mom, const V4c<R>* ext, const int8_t* col /* [n][2], 1..3 */,
-                     long long* live_splits /* may be null: counts (split, h,k,g) terms evaluated */) {
+                     long long* live_splits /* may be null: counts (split, h,k,g) terms evaluated */,
+                     R* cancel /* may be null: rho = |A| / sum over top-level ordered-split terms |eps_n . term| */) {
     const int m = n - 1;
     const int nsub = 1 << m;
+    const int in = col[2 * (n - 1)] - 1, jn = col[2 * (n - 1) + 1] - 1;
+    R sumabs = 0;
     struct Cur { V4c<R> J[3][3]; T6c<R> T[3][3]; bool nzJ[3][3]; bool nzT[3][3]; V4r<R> P; };
     std::vector<Cur> cur(nsub);
     long long live = 0;
@@ -331,8 +334,9 @@ cx<R> cdbg_amplitude(int n, const V4r<R>* mom, const V4c<R>* ext, const int8_t* 
                         live++;
                         V4c<R> t;
                         V3(c1.P, c2.P, c1.J[h][k], c2.J[k][g], t);
+                        VT_add(c1.J[h][k], c1.T[h][k], c2.J[k][g], c2.T[k][g], t);
                         for (int mu = 0; mu < 4; mu++) c.J[h][g].v[mu] += t.v[mu];
-                        VT_add(c1.J[h][k], c1.T[h][k], c2.J[k][g], c2.T[k][g], c.J[h][g]);
+                        if (pi == nsub - 1 && h == jn && g == in) sumabs += std::abs(mdot(ext[n - 1], t));
                         tensor_build_add(c1.J[h][k], c2.J[k][g], c.T[h][g]);
                         c.nzJ[h][g] = c.nzT[h][g] = true;
                     }
@@ -345,14 +349,19 @@ cx<R> cdbg_amplitude(int n, const V4r<R>* mom, const V4c<R>* ext, const int8_t* 
         }
     }
     if (live_splits) *live_splits = live;
-    const int in = col[2 * (n - 1)] - 1, jn = col[2 * (n - 1) + 1] - 1;
-    return mdot(ext[n - 1], cur[nsub - 1].J[jn][in]);
+    const cx<R> A = mdot(ext[n - 1], cur[nsub - 1].J[jn][in]);
+    if (cancel) *cancel = sumabs > 0 ? std::abs(A) / sumabs : R(1);
+    return A;
 }
 
-template <class R> R cdbg_me2(int n, const V4r<R>* mom, const int8_t* hel, const int8_t* col, long long* live) {
+template <class R>
+R cdbg_me2(int n, const V4r<R>* mom, const int8_t* hel, const int8_t* col, long long* live, double* rho) {
     V4c<R> ex[MAXN];
     for (int k = 0; k < n; k++) polarisation(mom[k], hel[k], ex[k]);
-    return std::norm(cdbg_amplitude(n, mom, ex, col, live));
+    R cancel = 1;
+    const R r = std::norm(cdbg_amplitude(n, mom, ex, col, live, &cancel));
+    if (rho) *rho = (double)cancel;
+    return r;
 }
 
 // ---- Colour-flow decomposition, Eq. 19: the definition CDBG must equal.  Matrix-product
@@ -476,17 +485,17 @@ int bgo_cobg_full_colour(int n, long long N, const double* mom, const signed cha
 
 // Batched colour-dressed |A|^2 (CDBG).  live (may be NULL): [N] number of non-zero (split,h,k,g) terms.
 int bgo_cdbg(int n, long long N, const double* mom, const signed char* hel, const signed char* col, int prec,
-             int threads, double* out, long long* live) {
+             int threads, double* out, long long* live, double* rho /* may be NULL: [N] cancellation ratio */) {
     if (n < 3 || n >= MAXN) return -1;
 #pragma omp parallel for schedule(dynamic, 4) num_threads(threads > 0 ? threads : omp_get_max_threads_wrapper())
     for (long long e = 0; e < N; e++) {
         long long lv = 0;
         if (prec == 0) {
             V4r<double> pm[MAXN]; load_mom(n, mom + (size_t)e * n * 4, pm);
-            out[e] = cdbg_me2(n, pm, (const int8_t*)hel + (size_t)e * n, (const int8_t*)col + (size_t)e * n * 2, &lv);
+            out[e] = cdbg_me2(n, pm, (const int8_t*)hel + (size_t)e * n, (const int8_t*)col + (size_t)e * n * 2, &lv, rho ? rho + e : nullptr);
         } else {
             V4r<long double> pm[MAXN]; load_mom(n, mom + (size_t)e * n * 4, pm);
-            out[e] = (double)cdbg_me2(n, pm, (const int8_t*)hel + (size_t)e * n, (const int8_t*)col + (size_t)e * n * 2, &lv);
+            out[e] = (double)cdbg_me2(n, pm, (const int8_t*)hel + (size_t)e * n, (const int8_t*)col + (size_t)e * n * 2, &lv, rho ? rho + e : nullptr);
         }
         if (live) live[e] = lv;
     }

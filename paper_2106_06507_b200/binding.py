@@ -1,0 +1,163 @@
+"""Thin ctypes binding of libbg.so (include/bg.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of ``csrc/``; there is no CPU or PyTorch fallback.  If the
+shared library is missing or cannot be loaded, every entry point raises :class:`BgError` loudly.
+PyTorch is used by callers for device buffers and streams only; this module accepts either integers (raw
+device pointers) or objects with ``data_ptr()`` (torch tensors) / ``ctypes.data`` (numpy arrays, host calls).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbg.so")
+
+BG_OK, BG_EINVAL, BG_ENOMEM, BG_ECUDA, BG_EUNSUPPORTED = 0, -1, -2, -3, -4
+BG_REC_COBG, BG_REC_CDBG = 0x001, 0x002
+BG_HEL_SUM, BG_HEL_GIVEN = 0x010, 0x020
+BG_COL_FULL, BG_COL_GIVEN = 0x100, 0x200
+BG_COBG_HELSUM_FULLCOLOR = BG_REC_COBG | BG_HEL_SUM | BG_COL_FULL
+BG_COBG_HELGIVEN_FULLCOLOR = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_FULL
+BG_CDBG_GIVEN = BG_REC_CDBG | BG_HEL_GIVEN | BG_COL_GIVEN
+BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN
+BG_OPT_KERNEL, BG_OPT_SCRATCH_LIMIT = 1, 2
+
+EXPORTS = ("bg_init", "bg_eval", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",
+           "bg_set_option", "bg_colour_matrix", "bg_build_colour_matrix", "bg_last_launch_count",
+           "bg_last_kernel_name", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe")
+
+
+class BgError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__(f"{what}: {bg_strerror(code) if _lib is not None else code} (code {code})")
+        self.code = code
+
+
+_lib = None
+
+
+def load():
+    """Load libbg.so (built by ``paper_2106_06507_b200.build``); raises if it is absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2106_06507_b200.build` "
+                               "(there is no fallback path)")
+        lib = ctypes.CDLL(LIB_PATH)
+        vp, ll, i = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int
+        lib.bg_init.argtypes = [ctypes.POINTER(vp), i, i]
+        lib.bg_eval.argtypes = [vp, vp, ll, vp, vp, vp, vp]
+        lib.bg_eval_host.argtypes = [vp, ll, vp, vp, vp, vp]
+        lib.bg_reserve.argtypes = [vp, ll]
+        lib.bg_scratch_bytes.argtypes = [vp, ll]
+        lib.bg_scratch_bytes.restype = ctypes.c_size_t
+        lib.bg_current_bytes_per_event.argtypes = [vp]
+        lib.bg_current_bytes_per_event.restype = ctypes.c_size_t
+        lib.bg_set_option.argtypes = [vp, i, ll]
+        lib.bg_colour_matrix.argtypes = [vp, vp]
+        lib.bg_build_colour_matrix.argtypes = [i, vp]
+        lib.bg_last_launch_count.argtypes = [vp]
+        lib.bg_last_kernel_name.argtypes = [vp]
+        lib.bg_last_kernel_name.restype = ctypes.c_char_p
+        lib.bg_destroy.argtypes = [vp]
+        lib.bg_strerror.argtypes = [i]
+        lib.bg_strerror.restype = ctypes.c_char_p
+        lib.bg_fp64_peak_probe.argtypes = [i, ctypes.POINTER(ctypes.c_double)]
+        for name in ("bg_init", "bg_eval", "bg_eval_host", "bg_reserve", "bg_set_option", "bg_colour_matrix",
+                     "bg_build_colour_matrix", "bg_last_launch_count", "bg_destroy", "bg_fp64_peak_probe"):
+            getattr(lib, name).restype = i
+        _lib = lib
+    return _lib
+
+
+def _ptr(x):
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return ctypes.c_void_p(x)
+    if hasattr(x, "data_ptr"):
+        return ctypes.c_void_p(x.data_ptr())
+    if hasattr(x, "ctypes"):
+        return ctypes.c_void_p(x.ctypes.data)
+    raise TypeError(f"cannot take a pointer from {type(x)}")
+
+
+def _check(rc: int, what: str):
+    if rc != BG_OK:
+        raise BgError(rc, what)
+
+
+def bg_strerror(code: int) -> str:
+    return load().bg_strerror(code).decode()
+
+
+def bg_init(n: int, mode: int):
+    ctx = ctypes.c_void_p()
+    _check(load().bg_init(ctypes.byref(ctx), n, mode), "bg_init")
+    return ctx
+
+
+def bg_eval(ctx, stream, N: int, mom, hel, col, out) -> None:
+    """Device pointers (or torch CUDA tensors); ``stream`` is a cudaStream_t as int (0/None = default stream)."""
+    s = ctypes.c_void_p(int(stream)) if stream else None
+    _check(load().bg_eval(ctx, s, N, _ptr(mom), _ptr(hel), _ptr(col), _ptr(out)), "bg_eval")
+
+
+def bg_eval_host(ctx, N: int, mom, hel, col, out) -> None:
+    """Host buffers (numpy arrays or pinned torch CPU tensors), copies included."""
+    _check(load().bg_eval_host(ctx, N, _ptr(mom), _ptr(hel), _ptr(col), _ptr(out)), "bg_eval_host")
+
+
+def bg_reserve(ctx, N: int) -> None:
+    _check(load().bg_reserve(ctx, N), "bg_reserve")
+
+
+def bg_scratch_bytes(ctx, N: int) -> int:
+    return int(load().bg_scratch_bytes(ctx, N))
+
+
+def bg_current_bytes_per_event(ctx) -> int:
+    return int(load().bg_current_bytes_per_event(ctx))
+
+
+def bg_set_option(ctx, key: int, value: int) -> None:
+    _check(load().bg_set_option(ctx, key, value), "bg_set_option")
+
+
+def bg_colour_matrix(ctx, n: int):
+    import math
+    import numpy as np
+    m = math.factorial(n - 2)
+    C = np.empty((m, m))
+    _check(load().bg_colour_matrix(ctx, _ptr(C)), "bg_colour_matrix")
+    return C
+
+
+def bg_build_colour_matrix(n: int):
+    import math
+    import numpy as np
+    if not 4 <= n <= 8:
+        raise BgError(BG_EINVAL, "bg_build_colour_matrix")
+    m = math.factorial(n - 2)
+    C = np.empty((m, m))
+    _check(load().bg_build_colour_matrix(n, _ptr(C)), "bg_build_colour_matrix")
+    return C
+
+
+def bg_last_launch_count(ctx) -> int:
+    return int(load().bg_last_launch_count(ctx))
+
+
+def bg_last_kernel_name(ctx) -> str:
+    return load().bg_last_kernel_name(ctx).decode()
+
+
+def bg_destroy(ctx) -> None:
+    _check(load().bg_destroy(ctx), "bg_destroy")
+
+
+def bg_fp64_peak_probe(iterations: int = 1 << 16) -> float:
+    v = ctypes.c_double()
+    _check(load().bg_fp64_peak_probe(iterations, ctypes.byref(v)), "bg_fp64_peak_probe")
+    return v.value

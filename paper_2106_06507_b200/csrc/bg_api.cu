@@ -1,0 +1,361 @@
+// C-ABI of libbg.so (declared in include/bg.h): context management, colour-matrix construction, dispatch.
+#include <algorithm>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <numeric>
+#include <vector>
+
+#include "bg_internal.h"
+
+namespace bg {
+
+// ---------------------------------------------------------------------------------------------------------
+// Colour matrix, Eq. 17, as exact integers.  With Tr(T^a T^b) = delta^ab,
+//   (F^{a_2} .. F^{a_{n-1}})_{a_1 a_n} = (-1)^n Tr(T^{a_1} [T^{a_2}, [T^{a_3}, .. [T^{a_{n-1}}, T^{a_n}] .. ]])
+// (the overall sign drops out of C).  Expanding the nested commutator gives 2^{n-2} signed single traces; the sum
+// over all colours of Tr(w) Tr(w')^* follows from the U(N) completeness relation T^a_ij T^a_kl = delta_il delta_kj
+// as N_c^{#index loops} (commutators have no U(1) component, so U(N) and SU(N) sums agree).  Relabelling the
+// summed colours gives C_{sigma sigma'} = C_{id, sigma^-1 sigma'}, so one row is computed and permuted.
+// Orderings sigma: permutations of gluons 2..n-1 in lexicographic order.
+// ---------------------------------------------------------------------------------------------------------
+static void expand_words(const std::vector<int>& order /* n labels, order[0]=first, order[n-1]=last */,
+                         std::vector<std::vector<int>>& words, std::vector<int>& signs) {
+    const int n = (int)order.size();
+    words.assign(1, std::vector<int>{order[n - 1]});
+    signs.assign(1, 1);
+    for (int k = n - 2; k >= 1; k--) {
+        std::vector<std::vector<int>> nw;
+        std::vector<int> ns;
+        for (size_t i = 0; i < words.size(); i++) {
+            std::vector<int> a{order[k]};
+            a.insert(a.end(), words[i].begin(), words[i].end());
+            nw.push_back(a);
+            ns.push_back(signs[i]);
+            std::vector<int> b = words[i];
+            b.push_back(order[k]);
+            nw.push_back(b);
+            ns.push_back(-signs[i]);
+        }
+        words.swap(nw);
+        signs.swap(ns);
+    }
+    for (auto& w : words) w.insert(w.begin(), order[0]);
+}
+
+static int find_root(int* parent, int x) {
+    while (parent[x] != x) x = parent[x] = parent[parent[x]];
+    return x;
+}
+
+// sum over all colour labels of Tr(T^{w1}) Tr(T^{w2})^* = N^(loops)
+static long long trace_pair(const std::vector<int>& w1, const std::vector<int>& w2) {
+    const int n = (int)w1.size();
+    int pos1[16], pos2[16], parent[32];
+    std::vector<int> w2r(w2.rbegin(), w2.rend());   // complex conjugate of a trace = trace of the reversed word
+    for (int p = 0; p < n; p++) { pos1[w1[p]] = p; pos2[w2r[p]] = p; }
+    for (int i = 0; i < 2 * n; i++) parent[i] = i;
+    for (int a = 0; a < n; a++) {
+        const int p = pos1[a], q = pos2[a];
+        // generator a carries (row r_p, col r_{p+1}) in trace 1 and (row s_q, col s_{q+1}) in trace 2
+        int x = find_root(parent, p), y = find_root(parent, n + (q + 1) % n);
+        if (x != y) parent[x] = y;
+        x = find_root(parent, n + q); y = find_root(parent, (p + 1) % n);
+        if (x != y) parent[x] = y;
+    }
+    int loops = 0;
+    for (int i = 0; i < 2 * n; i++) loops += find_root(parent, i) == i;
+    long long r = 1;
+    for (int i = 0; i < loops; i++) r *= 3;
+    return r;
+}
+
+int build_colour_matrix(int n, double* C) {
+    const int m = n - 2;
+    std::vector<std::vector<int>> perms;
+    std::vector<int> p(m);
+    std::iota(p.begin(), p.end(), 1);
+    do perms.push_back(p); while (std::next_permutation(p.begin(), p.end()));
+    const int np = (int)perms.size();
+    // words of the identity ordering and of every ordering
+    auto full_order = [&](const std::vector<int>& s) {
+        std::vector<int> o{0};
+        o.insert(o.end(), s.begin(), s.end());
+        o.push_back(n - 1);
+        return o;
+    };
+    std::vector<std::vector<int>> w0, w1;
+    std::vector<int> s0, s1;
+    expand_words(full_order(perms[0]), w0, s0);
+    std::vector<long long> row(np);
+    for (int t = 0; t < np; t++) {
+        expand_words(full_order(perms[t]), w1, s1);
+        long long acc = 0;
+        for (size_t i = 0; i < w0.size(); i++)
+            for (size_t j = 0; j < w1.size(); j++) acc += (long long)(s0[i] * s1[j]) * trace_pair(w0[i], w1[j]);
+        row[t] = acc;
+    }
+    // C[s][s'] = row[index of s^-1 o s']
+    std::vector<int> inv(n);
+    for (int s = 0; s < np; s++) {
+        for (int i = 0; i < m; i++) inv[perms[s][i]] = i + 1;   // label -> position (as a label 1..m)
+        for (int t = 0; t < np; t++) {
+            // relative permutation rel(i) = inv[perms[t][i]]; its lexicographic index
+            int idx = 0;
+            bool used[16] = {false};
+            for (int i = 0; i < m; i++) {
+                const int v = inv[perms[t][i]];
+                int smaller = 0;
+                for (int u = 1; u < v; u++) smaller += !used[u];
+                used[v] = true;
+                int f = 1;
+                for (int u = 2; u <= m - 1 - i; u++) f *= u;
+                idx += smaller * f;
+            }
+            C[(size_t)s * np + t] = (double)row[idx];
+        }
+    }
+    return np;
+}
+
+}  // namespace bg
+
+// =========================================== ABI ===========================================================
+static bool mode_supported(int n, int mode) {
+    if (n < 4 || n > 12) return false;
+    if (mode == BG_COBG_HELSUM_FULLCOLOR || mode == BG_COBG_HELGIVEN_FULLCOLOR) return n <= 8;
+    if (mode == BG_CDBG_GIVEN || mode == BG_CDBG_HELSUM_COLGIVEN) return true;
+    return false;
+}
+
+extern "C" {
+
+const char* bg_strerror(int code) {
+    switch (code) {
+        case BG_OK: return "ok";
+        case BG_EINVAL: return "invalid argument";
+        case BG_ENOMEM: return "out of memory";
+        case BG_ECUDA: return "CUDA error (no device, or a runtime/launch failure)";
+        case BG_EUNSUPPORTED: return "mode / n combination not supported";
+        default: return "unknown error code";
+    }
+}
+
+int bg_init(bg_ctx** out, int n, int mode) {
+    if (!out) return BG_EINVAL;
+    *out = nullptr;
+    if (n < 4 || n > 12) return BG_EINVAL;
+    if (!mode_supported(n, mode)) return BG_EUNSUPPORTED;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return BG_ECUDA;
+    bg_ctx* c = new (std::nothrow) bg_ctx();
+    if (!c) return BG_ENOMEM;
+    std::memset(c, 0, sizeof(*c));
+    c->n = n;
+    c->mode = mode;
+    c->scratch_limit = (size_t)16 << 30;
+    c->last_kernel = "none";
+    if (cudaGetDevice(&c->device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) {
+        delete c;
+        return BG_ECUDA;
+    }
+    if (mode & BG_REC_COBG) {
+        int np = 1;
+        for (int i = 2; i <= n - 2; i++) np *= i;
+        c->nperm = np;
+        c->hC = (double*)std::malloc(sizeof(double) * np * np);
+        if (!c->hC) { delete c; return BG_ENOMEM; }
+        bg::build_colour_matrix(n, c->hC);
+        if (cudaMalloc(&c->dC, sizeof(double) * np * np) != cudaSuccess) { std::free(c->hC); delete c; return BG_ENOMEM; }
+        if (cudaMemcpy(c->dC, c->hC, sizeof(double) * np * np, cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaFree(c->dC); std::free(c->hC); delete c; return BG_ECUDA;
+        }
+    }
+    if (cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking) != cudaSuccess) {
+        if (c->dC) cudaFree(c->dC);
+        std::free(c->hC);
+        delete c;
+        return BG_ECUDA;
+    }
+    *out = c;
+    return BG_OK;
+}
+
+int bg_destroy(bg_ctx* c) {
+    if (!c) return BG_EINVAL;
+    cudaStreamSynchronize(c->hstream);
+    cudaStreamDestroy(c->hstream);
+    if (c->dC) cudaFree(c->dC);
+    if (c->scratch) cudaFree(c->scratch);
+    if (c->d_mom) cudaFree(c->d_mom);
+    if (c->d_hel) cudaFree(c->d_hel);
+    if (c->d_col) cudaFree(c->d_col);
+    if (c->d_out) cudaFree(c->d_out);
+    std::free(c->hC);
+    delete c;
+    return BG_OK;
+}
+
+static bool use_quad(const bg_ctx* c) {
+    if (!(c->mode & BG_REC_CDBG) || c->mode != BG_CDBG_GIVEN) return false;
+    if (c->kernel_opt == 1) return false;
+    return bg::cdbg_quad_supported(c->n);
+}
+
+// events per generic-CDBG launch under the scratch limit
+static long long generic_chunk(const bg_ctx* c, long long N) {
+    const size_t per = bg::cdbg_generic_scratch_per_event(c->n);
+    long long chunk = (long long)(c->scratch_limit / per);
+    if (chunk < 128) chunk = 128;
+    chunk -= chunk % 128;
+    return std::min(chunk, std::max<long long>(N, 1));
+}
+
+size_t bg_scratch_bytes(const bg_ctx* c, long long N) {
+    if (!c || N <= 0) return 0;
+    if (!(c->mode & BG_REC_CDBG) || use_quad(c)) return 0;
+    return bg::cdbg_generic_scratch_per_event(c->n) * (size_t)generic_chunk(c, N);
+}
+
+size_t bg_current_bytes_per_event(const bg_ctx* c) {
+    if (!c) return 0;
+    if (c->mode & BG_REC_COBG) return (size_t)(c->n - 1) * c->n / 2 * 64;   // one ordering's current table
+    if (use_quad(c)) return bg::cdbg_quad_current_bytes(c->n);
+    return ((size_t)1 << (c->n - 1)) * 3 * 160;
+}
+
+static int ensure_scratch(bg_ctx* c, long long N) {
+    const size_t need = bg_scratch_bytes(c, N);
+    if (need <= c->scratch_bytes) return BG_OK;
+    if (c->scratch) { cudaDeviceSynchronize(); cudaFree(c->scratch); c->scratch = nullptr; c->scratch_bytes = 0; }
+    if (cudaMalloc(&c->scratch, need) != cudaSuccess) { cudaGetLastError(); return BG_ENOMEM; }
+    c->scratch_bytes = need;
+    return BG_OK;
+}
+
+static int ensure_staging(bg_ctx* c, long long N) {
+    if (N <= c->staged_events) return BG_OK;
+    cudaStreamSynchronize(c->hstream);
+    if (c->d_mom) cudaFree(c->d_mom);
+    if (c->d_hel) cudaFree(c->d_hel);
+    if (c->d_col) cudaFree(c->d_col);
+    if (c->d_out) cudaFree(c->d_out);
+    c->d_mom = nullptr; c->d_hel = nullptr; c->d_col = nullptr; c->d_out = nullptr;
+    c->staged_events = 0;
+    const size_t n = (size_t)c->n;
+    if (cudaMalloc(&c->d_mom, sizeof(double) * 4 * n * N) != cudaSuccess ||
+        cudaMalloc(&c->d_hel, n * N) != cudaSuccess || cudaMalloc(&c->d_col, 2 * n * N) != cudaSuccess ||
+        cudaMalloc(&c->d_out, sizeof(double) * N) != cudaSuccess) {
+        cudaGetLastError();
+        return BG_ENOMEM;
+    }
+    c->staged_events = N;
+    return BG_OK;
+}
+
+int bg_reserve(bg_ctx* c, long long N) {
+    if (!c || N < 0) return BG_EINVAL;
+    if (N == 0) return BG_OK;
+    int rc = ensure_scratch(c, N);
+    if (rc != BG_OK) return rc;
+    return ensure_staging(c, N);
+}
+
+int bg_set_option(bg_ctx* c, int key, long long value) {
+    if (!c) return BG_EINVAL;
+    switch (key) {
+        case BG_OPT_KERNEL:
+            if (value < 0 || value > 2) return BG_EINVAL;
+            if (value == 2 && !(c->mode == BG_CDBG_GIVEN && bg::cdbg_quad_supported(c->n))) return BG_EUNSUPPORTED;
+            c->kernel_opt = (int)value;
+            return BG_OK;
+        case BG_OPT_SCRATCH_LIMIT:
+            if (value < (1ll << 20)) return BG_EINVAL;
+            c->scratch_limit = (size_t)value;
+            return BG_OK;
+        default:
+            return BG_EINVAL;
+    }
+}
+
+int bg_colour_matrix(const bg_ctx* c, double* C_host) {
+    if (!c || !C_host || !c->hC) return BG_EINVAL;
+    std::memcpy(C_host, c->hC, sizeof(double) * c->nperm * c->nperm);
+    return BG_OK;
+}
+
+int bg_build_colour_matrix(int n, double* C_host) {
+    if (n < 4 || n > 8 || !C_host) return BG_EINVAL;
+    bg::build_colour_matrix(n, C_host);
+    return BG_OK;
+}
+
+int bg_last_launch_count(const bg_ctx* c) { return c ? c->last_launches : 0; }
+const char* bg_last_kernel_name(const bg_ctx* c) { return c ? c->last_kernel : "none"; }
+
+int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const signed char* hel,
+            const signed char* col, double* out) {
+    if (!c || N < 0) return BG_EINVAL;
+    c->last_launches = 0;
+    if (N == 0) return BG_OK;
+    if (!mom || !out) return BG_EINVAL;
+    const bool helsum = (c->mode & BG_HEL_SUM) != 0;
+    if (!helsum && !hel) return BG_EINVAL;
+    if ((c->mode & BG_COL_GIVEN) && !col) return BG_EINVAL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaError_t err = cudaSuccess;
+    if (c->mode & BG_REC_COBG) {
+        err = bg::cobg_generic_launch(s, c->n, helsum, c->nperm, c->dC, N, mom, hel, out);
+        c->last_launches = 1;
+        c->last_kernel = "cobg_generic_kernel";
+    } else if (use_quad(c)) {
+        err = bg::cdbg_quad_launch(s, c->n, c->sm_count, N, mom, hel, col, out);
+        c->last_launches = 1;
+        c->last_kernel = "cdbg_quad_kernel";
+    } else {
+        int rc = ensure_scratch(c, N);
+        if (rc != BG_OK) return rc;
+        const long long chunk = generic_chunk(c, N);
+        for (long long first = 0; first < N && err == cudaSuccess; first += chunk) {
+            const long long count = std::min(chunk, N - first);
+            err = bg::cdbg_generic_launch(s, c->n, helsum, N, first, count, mom, hel, col, out, c->scratch);
+            c->last_launches++;
+        }
+        c->last_kernel = "cdbg_generic_kernel";
+    }
+    return err == cudaSuccess ? BG_OK : BG_ECUDA;
+}
+
+int bg_eval_host(bg_ctx* c, long long N, const double* mom, const signed char* hel, const signed char* col,
+                 double* out) {
+    if (!c || N < 0) return BG_EINVAL;
+    if (N == 0) { c->last_launches = 0; return BG_OK; }
+    if (!mom || !out) return BG_EINVAL;
+    const bool helsum = (c->mode & BG_HEL_SUM) != 0;
+    if (!helsum && !hel) return BG_EINVAL;
+    if ((c->mode & BG_COL_GIVEN) && !col) return BG_EINVAL;
+    int rc = ensure_staging(c, N);
+    if (rc != BG_OK) return rc;
+    const size_t n = (size_t)c->n;
+    cudaStream_t s = c->hstream;
+    if (cudaMemcpyAsync(c->d_mom, mom, sizeof(double) * 4 * n * N, cudaMemcpyHostToDevice, s) != cudaSuccess) return BG_ECUDA;
+    if (!helsum && cudaMemcpyAsync(c->d_hel, hel, n * N, cudaMemcpyHostToDevice, s) != cudaSuccess) return BG_ECUDA;
+    if ((c->mode & BG_COL_GIVEN) && cudaMemcpyAsync(c->d_col, col, 2 * n * N, cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return BG_ECUDA;
+    rc = bg_eval(c, (void*)s, N, c->d_mom, helsum ? nullptr : c->d_hel, (c->mode & BG_COL_GIVEN) ? c->d_col : nullptr,
+                 c->d_out);
+    if (rc != BG_OK) return rc;
+    if (cudaMemcpyAsync(out, c->d_out, sizeof(double) * N, cudaMemcpyDeviceToHost, s) != cudaSuccess) return BG_ECUDA;
+    if (cudaStreamSynchronize(s) != cudaSuccess) return BG_ECUDA;
+    return BG_OK;
+}
+
+int bg_fp64_peak_probe(int iterations, double* tflops) {
+    if (!tflops || iterations < 1) return BG_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return BG_ECUDA;
+    return bg::fp64_probe(iterations, tflops) == cudaSuccess ? BG_OK : BG_ECUDA;
+}
+
+}  // extern "C"

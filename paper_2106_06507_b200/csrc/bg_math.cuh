@@ -1,0 +1,138 @@
+// Device-side FP64 complex Lorentz arithmetic for the Berends-Giele kernels (sm_100a).
+// Formulas follow PAPER.md Eq. 3 (polarisation vectors), Eq. 21 (three- and four-gluon vertices) and
+// Eq. 23-26 (tensor pseudo-particle) with g_s = 1 and the factors of i multiplied out; the common factor
+// 1/sqrt2 of V3, V_T and of the tensor current is NOT applied here: callers accumulate unscaled sums and
+// multiply once when a current is finalised.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace bg {
+
+constexpr double kInvSqrt2 = 0.70710678118654752440;
+
+struct cx {
+    double re, im;
+};
+
+__device__ __forceinline__ cx mk(double re, double im) { cx r; r.re = re; r.im = im; return r; }
+__device__ __forceinline__ cx operator+(cx a, cx b) { return mk(a.re + b.re, a.im + b.im); }
+__device__ __forceinline__ cx operator-(cx a, cx b) { return mk(a.re - b.re, a.im - b.im); }
+__device__ __forceinline__ cx operator*(cx a, cx b) {
+    return mk(fma(a.re, b.re, -(a.im * b.im)), fma(a.re, b.im, a.im * b.re));
+}
+__device__ __forceinline__ cx operator*(double s, cx a) { return mk(s * a.re, s * a.im); }
+// acc += a*b
+__device__ __forceinline__ void cfma(cx& acc, cx a, cx b) {
+    acc.re = fma(a.re, b.re, acc.re);
+    acc.re = fma(-a.im, b.im, acc.re);
+    acc.im = fma(a.re, b.im, acc.im);
+    acc.im = fma(a.im, b.re, acc.im);
+}
+// acc -= a*b
+__device__ __forceinline__ void cfms(cx& acc, cx a, cx b) {
+    acc.re = fma(-a.re, b.re, acc.re);
+    acc.re = fma(a.im, b.im, acc.re);
+    acc.im = fma(-a.re, b.im, acc.im);
+    acc.im = fma(-a.im, b.re, acc.im);
+}
+// acc += s*a (s real)
+__device__ __forceinline__ void rfma(cx& acc, double s, cx a) {
+    acc.re = fma(s, a.re, acc.re);
+    acc.im = fma(s, a.im, acc.im);
+}
+
+// Minkowski product, no complex conjugation
+__device__ __forceinline__ cx mdot(const cx* a, const cx* b) {
+    cx r = a[0] * b[0];
+    cfms(r, a[1], b[1]);
+    cfms(r, a[2], b[2]);
+    cfms(r, a[3], b[3]);
+    return r;
+}
+__device__ __forceinline__ cx mdot(const double* p, const cx* a) {
+    cx r = mk(p[0] * a[0].re, p[0] * a[0].im);
+    rfma(r, -p[1], a[1]);
+    rfma(r, -p[2], a[2]);
+    rfma(r, -p[3], a[3]);
+    return r;
+}
+__device__ __forceinline__ double mdot(const double* p, const double* q) {
+    return fma(p[0], q[0], -fma(p[1], q[1], fma(p[2], q[2], p[3] * q[3])));
+}
+
+// Helicity eigenvector eps^lambda(p), Eq. 3 in the light-cone gauge k = (q0, -q) of DESIGN.md
+// reading g2/g3 (q = p for outgoing, -p for incoming legs; same lambda).  eps^0 = 0.
+__device__ __forceinline__ void polarisation(const double* p, int lambda, cx* eps) {
+    const double s = p[0] < 0.0 ? -1.0 : 1.0;
+    const double qx = s * p[1], qy = s * p[2], qz = s * p[3];
+    const double qt2 = qx * qx + qy * qy;
+    const double qt = sqrt(qt2), qa = sqrt(qt2 + qz * qz);
+    double e1x, e1y, e1z, e2x, e2y;
+    if (qt < 1e-9 * qa) {
+        e1x = 1.0; e1y = 0.0; e1z = 0.0;
+        e2x = 0.0; e2y = qz < 0.0 ? -1.0 : 1.0;
+    } else {
+        const double inv = 1.0 / (qa * qt), invt = 1.0 / qt;
+        e1x = qx * qz * inv; e1y = qy * qz * inv; e1z = -qt / qa;
+        e2x = -qy * invt; e2y = qx * invt;
+    }
+    const double l = -(double)lambda * kInvSqrt2;
+    eps[0] = mk(0.0, 0.0);
+    eps[1] = mk(l * e1x, -kInvSqrt2 * e2x);
+    eps[2] = mk(l * e1y, -kInvSqrt2 * e2y);
+    eps[3] = mk(l * e1z, 0.0);
+}
+
+// acc += sign * sqrt2 * V3(p,q;a,b)   [Eq. 21 first line: (a.b)(p-q) + ((2q+p).a) b - ((2p+q).b) a]
+__device__ __forceinline__ void v3_acc(cx* acc, const double* p, const double* q, const cx* a, const cx* b,
+                                       double sign) {
+    double tqp[4], tpq[4];
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        tqp[mu] = fma(2.0, q[mu], p[mu]);
+        tpq[mu] = fma(2.0, p[mu], q[mu]);
+    }
+    cx ab = mdot(a, b), qa = mdot(tqp, a), pb = mdot(tpq, b);
+    ab = sign * ab; qa = sign * qa; pb = sign * pb;
+#pragma unroll
+    for (int nu = 0; nu < 4; nu++) {
+        rfma(acc[nu], p[nu] - q[nu], ab);
+        cfma(acc[nu], qa, b[nu]);
+        cfms(acc[nu], pb, a[nu]);
+    }
+}
+
+// Tensor components are stored as T[0..5] = T^{01}, T^{02}, T^{03}, T^{12}, T^{13}, T^{23} (antisymmetric).
+// acc^nu += sign * T^{nu beta} v_beta (index lowered with the metric)
+__device__ __forceinline__ void tcontract_acc(cx* acc, const cx* T, const cx* v, double sign) {
+    const cx v0 = sign * v[0], v1 = sign * v[1], v2 = sign * v[2], v3 = sign * v[3];
+    cfms(acc[0], T[0], v1); cfms(acc[0], T[1], v2); cfms(acc[0], T[2], v3);
+    cfms(acc[1], T[0], v0); cfms(acc[1], T[3], v2); cfms(acc[1], T[4], v3);
+    cfms(acc[2], T[1], v0); cfma(acc[2], T[3], v1); cfms(acc[2], T[5], v3);
+    cfms(acc[3], T[2], v0); cfma(acc[3], T[4], v1); cfma(acc[3], T[5], v2);
+}
+
+// tacc += sign * (a^alpha b^beta - a^beta b^alpha)   [Eq. 25, unscaled]
+__device__ __forceinline__ void tbuild_acc(cx* tacc, const cx* a, const cx* b, double sign) {
+    const cx b0 = sign * b[0], b1 = sign * b[1], b2 = sign * b[2], b3 = sign * b[3];
+    cfma(tacc[0], a[0], b1); cfms(tacc[0], a[1], b0);
+    cfma(tacc[1], a[0], b2); cfms(tacc[1], a[2], b0);
+    cfma(tacc[2], a[0], b3); cfms(tacc[2], a[3], b0);
+    cfma(tacc[3], a[1], b2); cfms(tacc[3], a[2], b1);
+    cfma(tacc[4], a[1], b3); cfms(tacc[4], a[3], b1);
+    cfma(tacc[5], a[2], b3); cfms(tacc[5], a[3], b2);
+}
+
+// acc += sign * 2 * V4(a,b,c)   [Eq. 21 second line: 2(a.c) b - (a.b) c - (b.c) a]
+__device__ __forceinline__ void v4_acc(cx* acc, const cx* a, const cx* b, const cx* c) {
+    cx ac = mdot(a, c), ab = mdot(a, b), bc = mdot(b, c);
+    ac = 2.0 * ac;
+#pragma unroll
+    for (int nu = 0; nu < 4; nu++) {
+        cfma(acc[nu], ac, b[nu]);
+        cfms(acc[nu], ab, c[nu]);
+        cfms(acc[nu], bc, a[nu]);
+    }
+}
+
+}  // namespace bg
