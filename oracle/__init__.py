@@ -150,14 +150,20 @@ def cdbg(mom, hel, col, prec: str = "double", threads: int = 0, return_live: boo
     return res if len(res) > 1 else out
 
 
-def colour_flow(mom, hel, col, prec: str = "double", threads: int = 0, return_count: bool = False):
-    """Batched Eq. 19 brute force: |sum over colour-connected orderings of COBG amplitudes|^2."""
+def colour_flow(mom, hel, col, prec: str = "double", threads: int = 0, return_count: bool = False,
+                return_rho: bool = False):
+    """Batched Eq. 19 brute force: |sum over colour-connected orderings of COBG amplitudes|^2.
+
+    ``return_rho`` adds rho19 = |sum_sigma A_sigma| / sum_sigma |A_sigma|, the cancellation between the colour
+    orderings of Eq. 19 (1 = none)."""
     mom = _f64(mom)
     N, n = mom.shape[0], mom.shape[1]
     hel, col = _i8(hel), _i8(col)
     out = np.empty(N)
     cnt = np.empty(N, dtype=np.int64)
+    rho = np.empty(N)
     rc = _load().bgo_colour_flow(n, ctypes.c_longlong(N), _p(mom), _p(hel), _p(col), _prec(prec), int(threads),
-                                 _p(out), _p(cnt))
+                                 _p(out), _p(cnt), _p(rho))
     assert rc == 0
-    return (out, cnt) if return_count else out
+    res = (out,) + ((cnt,) if return_count else ()) + ((rho,) if return_rho else ())
+    return res if len(res) > 1 else out

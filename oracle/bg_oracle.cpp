@@ -369,12 +369,14 @@ R cdbg_me2(int n, const V4r<R>* mom, const int8_t* hel, const int8_t* col, long 
 // j_{s_1} = i_{s_2}, ..., j_{s_{n-1}} = i_n.  Depth-first search over colour-connected orderings. ----------
 template <class R>
 void colour_flow_dfs(int n, const V4r<R>* mom, const int8_t* hel, const int8_t* col, int depth, int* order,
-                     unsigned used, int last, cx<R>& sum, long long& count) {
+                     unsigned used, int last, cx<R>& sum, R& sumabs, long long& count) {
     const int m = n - 1;
     if (depth == m) {
         if (col[2 * last + 1] != col[2 * (n - 1)]) return;   // j_last = i_n
         order[m] = n - 1;
-        sum += cobg_ordered(n, mom, hel, order, false);
+        const cx<R> a = cobg_ordered(n, mom, hel, order, false);
+        sum += a;
+        sumabs += std::abs(a);
         count++;
         return;
     }
@@ -382,15 +384,18 @@ void colour_flow_dfs(int n, const V4r<R>* mom, const int8_t* hel, const int8_t* 
         if (used >> k & 1) continue;
         if (col[2 * last + 1] != col[2 * k]) continue;       // j_prev = i_k
         order[depth] = k;
-        colour_flow_dfs(n, mom, hel, col, depth + 1, order, used | (1u << k), k, sum, count);
+        colour_flow_dfs(n, mom, hel, col, depth + 1, order, used | (1u << k), k, sum, sumabs, count);
     }
 }
-template <class R> R colour_flow_me2(int n, const V4r<R>* mom, const int8_t* hel, const int8_t* col, long long* cnt) {
+template <class R>
+R colour_flow_me2(int n, const V4r<R>* mom, const int8_t* hel, const int8_t* col, long long* cnt, double* rho) {
     cx<R> sum(0, 0);
+    R sumabs = 0;
     long long count = 0;
     int order[MAXN];
-    colour_flow_dfs(n, mom, hel, col, 0, order, 0u, n - 1, sum, count);
+    colour_flow_dfs(n, mom, hel, col, 0, order, 0u, n - 1, sum, sumabs, count);
     if (cnt) *cnt = count;
+    if (rho) *rho = sumabs > 0 ? (double)(std::abs(sum) / sumabs) : 1.0;   // |sum_s A_s| / sum_s |A_s|
     return std::norm(sum);
 }
 
@@ -504,17 +509,18 @@ int bgo_cdbg(int n, long long N, const double* mom, const signed char* hel, cons
 
 // Batched Eq. 19 brute force.  count (may be NULL): [N] number of colour-connected orderings.
 int bgo_colour_flow(int n, long long N, const double* mom, const signed char* hel, const signed char* col,
-                    int prec, int threads, double* out, long long* count) {
+                    int prec, int threads, double* out, long long* count,
+                    double* rho /* may be NULL: [N] |sum A_sigma| / sum |A_sigma| over connected orderings */) {
     if (n < 3 || n >= MAXN) return -1;
 #pragma omp parallel for schedule(dynamic, 1) num_threads(threads > 0 ? threads : omp_get_max_threads_wrapper())
     for (long long e = 0; e < N; e++) {
         long long c = 0;
         if (prec == 0) {
             V4r<double> pm[MAXN]; load_mom(n, mom + (size_t)e * n * 4, pm);
-            out[e] = colour_flow_me2(n, pm, (const int8_t*)hel + (size_t)e * n, (const int8_t*)col + (size_t)e * n * 2, &c);
+            out[e] = colour_flow_me2(n, pm, (const int8_t*)hel + (size_t)e * n, (const int8_t*)col + (size_t)e * n * 2, &c, rho ? rho + e : nullptr);
         } else {
             V4r<long double> pm[MAXN]; load_mom(n, mom + (size_t)e * n * 4, pm);
-            out[e] = (double)colour_flow_me2(n, pm, (const int8_t*)hel + (size_t)e * n, (const int8_t*)col + (size_t)e * n * 2, &c);
+            out[e] = (double)colour_flow_me2(n, pm, (const int8_t*)hel + (size_t)e * n, (const int8_t*)col + (size_t)e * n * 2, &c, rho ? rho + e : nullptr);
         }
         if (count) count[e] = c;
     }

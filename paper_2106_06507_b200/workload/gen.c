@@ -62,6 +62,23 @@ static void rambo_outgoing(uint64_t seed, uint64_t stream, uint64_t ev, uint64_t
         /* re-project onto the light cone so that p^2 = 0 to rounding */
         p[i][0] = sqrt(p[i][1] * p[i][1] + p[i][2] * p[i][2] + p[i][3] * p[i][3]);
     }
+    /* Polish: sqrt(Q^2) cancels when the q_i are nearly collinear, which leaves sum(p) off by up to ~1e-7 GeV in
+     * rare events.  Two rounds of "remove the residual 3-momentum evenly, re-project, rescale to sqrt_s" bring
+     * momentum conservation and masslessness to rounding level (a relative deformation of the event <= 1e-9). */
+    for (int it = 0; it < 2; it++) {
+        double d[3] = {0, 0, 0};
+        for (int i = 0; i < m; i++)
+            for (int k = 0; k < 3; k++) d[k] += p[i][k + 1];
+        double esum = 0;
+        for (int i = 0; i < m; i++) {
+            for (int k = 0; k < 3; k++) p[i][k + 1] -= d[k] / m;
+            p[i][0] = sqrt(p[i][1] * p[i][1] + p[i][2] * p[i][2] + p[i][3] * p[i][3]);
+            esum += p[i][0];
+        }
+        double sc = sqrt_s / esum;
+        for (int i = 0; i < m; i++)
+            for (int mu = 0; mu < 4; mu++) p[i][mu] *= sc;
+    }
 }
 
 static int pass_cuts(int m, double (*p)[4], double ptmin, double drmin) {

@@ -1,10 +1,13 @@
 """Parity of the CUDA path (through the C-ABI) with the CPU oracle on the same seeded events.
 
-Tolerances: truth = the oracle in long double.  Full-colour COBG configs: relative
-error <= 1e-11 on every event.  Colour-dressed, single colour flow: <= 1e-11 on every event whose top-level
-cancellation ratio rho (computed by the oracle) is >= 0.01, and <= 1e-13 / rho for the ill-conditioned rest
-(near-zeros by cancellation between colour orderings, about 3-4 % of events), where two correct FP64 evaluations
-differ by the same amount."""
+Tolerances: truth = the oracle in long double.  Helicity-summed full colour: relative
+error <= 1e-11 on every event.  Colour-dressed, single colour flow: <= 1e-11 on every event, except where FP64
+arithmetic itself cannot deliver it: single-flow amplitudes have near-zeros by cancellation (gauge cancellations
+between splits, cancellations between colour orderings), where the double-precision oracle misses 1e-11 as well
+(0.13 % of n = 6 events).  For an event over 1e-11 the test measures that event's FP64 noise floor with the
+oracle itself (double precision, gluons relabelled 16 ways: same mathematical value, different summation order)
+and requires e_gpu <= 10 x floor.  The same rule covers the given-helicity full-colour mode, whose kinematic near-zeros
+put 9 of 16384 n = 7 events of the double-precision oracle itself above 1e-11."""
 import numpy as np
 import pytest
 
@@ -20,16 +23,43 @@ def bg():
     return bg
 
 
-def cdbg_tol(rho):
-    return 1e-13 / np.minimum(rho, 0.01)
+def oracle_double(oracle, ev, cdbg):
+    if cdbg:
+        return oracle.cdbg(ev.mom, ev.hel, ev.col)
+    return oracle.cobg_full_colour(ev.mom, ev.hel)
 
 
-def check_cdbg(oracle, ev, got):
-    truth, rho = oracle.cdbg(ev.mom, ev.hel, ev.col, prec="long double", return_rho=True)
+def fp64_noise_floor(oracle, ev, truth, cdbg, reps=16, seed=7):
+    """max over relabelled double-precision oracle evaluations of |cpu - truth| / truth, per event."""
+    rng = np.random.default_rng(seed)
+    floor = rel_err(oracle_double(oracle, ev, cdbg), truth)
+    for _ in range(reps):
+        perm = rng.permutation(ev.n)
+        pe = type(ev)(ev.n, ev.mom[:, perm], ev.hel[:, perm], None if ev.col is None else ev.col[:, perm])
+        floor = np.maximum(floor, rel_err(oracle_double(oracle, pe, cdbg), truth))
+    return floor
+
+
+def check_parity(oracle, ev, got, cdbg, max_tail_frac=0.01):
+    """<= 1e-11 against the long-double truth on every event, except inside the event's own FP64 noise floor."""
+    if cdbg:
+        truth = oracle.cdbg(ev.mom, ev.hel, ev.col, prec="long double")
+    else:
+        truth = oracle.cobg_full_colour(ev.mom, ev.hel, prec="long double")
+    assert np.all(truth > 0)
     err = rel_err(got, truth)
-    bad = err > cdbg_tol(rho)
-    assert not bad.any(), f"{bad.sum()} events off: max err {err[bad].max():.3e}, rho {rho[bad][:5]}"
-    return err, rho
+    tail = np.nonzero(err > 1e-11)[0]
+    assert len(tail) <= max(3, max_tail_frac * ev.N), f"{len(tail)} of {ev.N} events over 1e-11"
+    if len(tail):
+        floor = fp64_noise_floor(oracle, ev.take(tail), truth[tail], cdbg)
+        bad = err[tail] > 10 * floor
+        assert not bad.any(), f"{bad.sum()} events beyond 10x the FP64 noise floor: err {err[tail][bad][:5]}, " \
+                              f"floor {floor[bad][:5]}"
+    return err, tail
+
+
+def check_cdbg(oracle, ev, got, max_tail_frac=0.01):
+    return check_parity(oracle, ev, got, True, max_tail_frac)
 
 
 def test_config1_n4_helsum_closed_form(bg, oracle, wl):
@@ -37,31 +67,34 @@ def test_config1_n4_helsum_closed_form(bg, oracle, wl):
     got, name = gpu_eval(ev, bg.BG_COBG_HELSUM_FULLCOLOR)
     truth = oracle.cobg_full_colour(ev.mom, prec="long double")
     assert rel_err(got, truth).max() <= 1e-11
-    m = ev.mom
+    m = ev.mom.astype(np.longdouble)     # the invariants t, u cancel strongly for forward scattering
 
     def md(a, b):
         return a[:, 0] * b[:, 0] - (a[:, 1:] * b[:, 1:]).sum(1)
     s, t, u = md(m[:, 0] + m[:, 1], m[:, 0] + m[:, 1]), md(m[:, 0] + m[:, 2], m[:, 0] + m[:, 2]), \
         md(m[:, 0] + m[:, 3], m[:, 0] + m[:, 3])
     closed = 1152.0 * (3 - t * u / s ** 2 - s * u / t ** 2 - s * t / u ** 2)
-    assert rel_err(got, closed).max() <= 1e-11
+    # the closed form assumes exactly massless, exactly conserved momenta; the double-precision inputs satisfy
+    # that to ~1e-16 sqrt(s), which is amplified by s/min(|t|,|u|) for forward scattering (no cuts in config 1)
+    amp = (s / np.minimum(np.abs(t), np.abs(u))).astype(np.float64)
+    assert np.all(rel_err(got, closed.astype(np.float64)) <= 1e-11 * np.maximum(1.0, 1e-2 * amp))
+    assert np.mean(amp < 100) > 0.9
 
 
 @pytest.mark.parametrize("n,N", [(5, 300), (6, 200), (7, 333)])
 def test_cobg_given_helicity_full_colour(bg, oracle, wl, n, N):
     ev = wl.config_events(4, N=N, n=n)          # momenta + helicities of the sweep stream; colours ignored
     got, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR)
-    truth = oracle.cobg_full_colour(ev.mom, ev.hel, prec="long double")
-    assert rel_err(got, truth).max() <= 1e-11
+    check_parity(oracle, ev, got, False)
 
 
 def test_config3_n7_full_size_sampled(bg, oracle, wl):
     ev = wl.config_events(2)                      # 2^18 events, the bench launch configuration
     got, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR)
     assert np.all(np.isfinite(got)) and np.all(got > 0)
-    idx = np.arange(0, ev.N, 509)
-    truth = oracle.cobg_full_colour(ev.mom[idx], ev.hel[idx], prec="long double")
-    assert rel_err(got[idx], truth).max() <= 1e-11
+    idx = np.arange(0, ev.N, 127)
+    err, tail = check_parity(oracle, ev.take(idx), got[idx], False, max_tail_frac=0.003)
+    assert np.median(err) < 1e-14
 
 
 @pytest.mark.parametrize("n,N", [(4, 1000), (5, 1000), (6, 4099), (7, 2051), (8, 1031), (9, 515), (10, 259),
@@ -75,9 +108,8 @@ def test_cdbg_sweep_small(bg, oracle, wl, n, N):
 def test_config2_n6_full_size_all_events(bg, oracle, wl):
     ev = wl.config_events(1)                      # 2^20 events
     got, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
-    err, rho = check_cdbg(oracle, ev, got)
-    assert np.median(err) < 1e-14
-    assert (err[rho >= 0.01] <= 1e-11).all()
+    err, tail = check_cdbg(oracle, ev, got, max_tail_frac=0.003)
+    assert np.median(err) < 1e-14 and np.percentile(err, 99) < 2e-12
 
 
 def test_config4_n9_full_size_sampled(bg, oracle, wl):

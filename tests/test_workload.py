@@ -8,11 +8,11 @@ import pytest
 
 def test_rambo_kinematics_and_cuts(wl):
     for n in (4, 6, 9, 12):
-        mom = wl.rambo(n, 200, seed=1, stream=n)
-        assert mom.shape == (200, n, 4)
+        mom = wl.rambo(n, 20000 if n == 4 else 2000, seed=1, stream=n)
+        assert mom.shape[1:] == (n, 4)
         m2 = mom[..., 0] ** 2 - (mom[..., 1:] ** 2).sum(-1)
-        assert np.max(np.abs(m2)) < 1e-9 * wl.SQRT_S ** 2                 # massless
-        assert np.max(np.abs(mom.sum(1))) < 1e-9 * wl.SQRT_S              # momentum conservation, all-outgoing
+        assert np.max(np.abs(m2)) < 1e-13 * wl.SQRT_S ** 2                # massless
+        assert np.max(np.abs(mom.sum(1))) < 1e-13 * wl.SQRT_S             # momentum conservation, all-outgoing
         assert np.all(mom[:, :2, 0] < 0) and np.all(mom[:, 2:, 0] > 0)
         out = mom[:, 2:]
         pt = np.hypot(out[..., 1], out[..., 2])
