@@ -57,8 +57,12 @@ enum {
 /* bg_set_option keys */
 enum {
     BG_OPT_KERNEL = 1,       /* 0 = automatic choice by n; 1 = generic thread-per-event kernels with currents in
-                                global scratch (any n); 2 = quad kernel, currents in shared memory (CDBG) */
-    BG_OPT_SCRATCH_LIMIT = 2 /* upper bound in bytes for the scratch the generic kernels may use (default 16 GiB) */
+                                global scratch (any n); 2 = colour-class program interpreter, currents in shared
+                                memory (BG_CDBG_GIVEN, n <= 8) */
+    BG_OPT_SCRATCH_LIMIT = 2,/* upper bound in bytes for the scratch the generic kernels may use (default 16 GiB) */
+    BG_OPT_LANES = 3,        /* lanes that cooperate on one event in the program interpreter: 1, 2, 4, 8, 16, 32;
+                                0 = automatic.  Rebuilds the class programs (synchronises the device). */
+    BG_OPT_TIMING = 4        /* 1: record CUDA events around the dominant kernel of every bg_eval (bg_last_kernel_ms) */
 };
 
 /*
@@ -111,6 +115,11 @@ int bg_build_colour_matrix(int n, double* C_host);
 
 /* Number of kernels the most recent bg_eval / bg_eval_host launched. */
 int bg_last_launch_count(const bg_ctx* ctx);
+
+/* Device time in milliseconds of the dominant (recursion) kernel of the most recent bg_eval, measured with CUDA
+ * events recorded on the caller's stream around that launch.  Only available after
+ * bg_set_option(ctx, BG_OPT_TIMING, 1); waits for that launch to finish.  BG_EINVAL if timing is off or nothing ran. */
+int bg_last_kernel_ms(bg_ctx* ctx, double* ms);
 
 /* Name of the kernel variant the most recent bg_eval used (static string). */
 const char* bg_last_kernel_name(const bg_ctx* ctx);

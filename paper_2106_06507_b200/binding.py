@@ -21,11 +21,11 @@ BG_COBG_HELSUM_FULLCOLOR = BG_REC_COBG | BG_HEL_SUM | BG_COL_FULL
 BG_COBG_HELGIVEN_FULLCOLOR = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_FULL
 BG_CDBG_GIVEN = BG_REC_CDBG | BG_HEL_GIVEN | BG_COL_GIVEN
 BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN
-BG_OPT_KERNEL, BG_OPT_SCRATCH_LIMIT = 1, 2
+BG_OPT_KERNEL, BG_OPT_SCRATCH_LIMIT, BG_OPT_LANES, BG_OPT_TIMING = 1, 2, 3, 4
 
 EXPORTS = ("bg_init", "bg_eval", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",
            "bg_set_option", "bg_colour_matrix", "bg_build_colour_matrix", "bg_last_launch_count",
-           "bg_last_kernel_name", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe")
+           "bg_last_kernel_name", "bg_last_kernel_ms", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe")
 
 
 class BgError(RuntimeError):
@@ -60,6 +60,8 @@ def load():
         lib.bg_last_launch_count.argtypes = [vp]
         lib.bg_last_kernel_name.argtypes = [vp]
         lib.bg_last_kernel_name.restype = ctypes.c_char_p
+        lib.bg_last_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+        lib.bg_last_kernel_ms.restype = i
         lib.bg_destroy.argtypes = [vp]
         lib.bg_strerror.argtypes = [i]
         lib.bg_strerror.restype = ctypes.c_char_p
@@ -151,6 +153,12 @@ def bg_last_launch_count(ctx) -> int:
 
 def bg_last_kernel_name(ctx) -> str:
     return load().bg_last_kernel_name(ctx).decode()
+
+
+def bg_last_kernel_ms(ctx) -> float:
+    v = ctypes.c_double()
+    _check(load().bg_last_kernel_ms(ctx, ctypes.byref(v)), "bg_last_kernel_ms")
+    return v.value
 
 
 def bg_destroy(ctx) -> None:

@@ -121,6 +121,10 @@ int build_colour_matrix(int n, double* C) {
 }  // namespace bg
 
 // =========================================== ABI ===========================================================
+// largest n whose colour-class programs are tabulated at bg_init, and the default lanes per event
+static const int kProgMaxN = 8;
+static int auto_lanes(int n) { return n <= 5 ? 2 : (n <= 7 ? 4 : 8); }
+
 static bool mode_supported(int n, int mode) {
     if (n < 4 || n > 12) return false;
     if (mode == BG_COBG_HELSUM_FULLCOLOR || mode == BG_COBG_HELGIVEN_FULLCOLOR) return n <= 8;
@@ -172,7 +176,12 @@ int bg_init(bg_ctx** out, int n, int mode) {
             cudaFree(c->dC); std::free(c->hC); delete c; return BG_ECUDA;
         }
     }
+    if (mode == BG_CDBG_GIVEN && n <= kProgMaxN) {
+        const int rc = bg::prog_table_create(n, auto_lanes(n), &c->prog);
+        if (rc != BG_OK) { delete c; return rc; }
+    }
     if (cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking) != cudaSuccess) {
+        bg::prog_table_destroy(c->prog);
         if (c->dC) cudaFree(c->dC);
         std::free(c->hC);
         delete c;
@@ -186,6 +195,9 @@ int bg_destroy(bg_ctx* c) {
     if (!c) return BG_EINVAL;
     cudaStreamSynchronize(c->hstream);
     cudaStreamDestroy(c->hstream);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    bg::prog_table_destroy(c->prog);
     if (c->dC) cudaFree(c->dC);
     if (c->scratch) cudaFree(c->scratch);
     if (c->d_mom) cudaFree(c->d_mom);
@@ -197,10 +209,9 @@ int bg_destroy(bg_ctx* c) {
     return BG_OK;
 }
 
-static bool use_quad(const bg_ctx* c) {
-    if (!(c->mode & BG_REC_CDBG) || c->mode != BG_CDBG_GIVEN) return false;
-    if (c->kernel_opt == 1) return false;
-    return bg::cdbg_quad_supported(c->n);
+static bool use_prog(const bg_ctx* c) {
+    if (c->mode != BG_CDBG_GIVEN || c->kernel_opt == 1) return false;
+    return c->prog != nullptr;
 }
 
 // events per generic-CDBG launch under the scratch limit
@@ -214,14 +225,15 @@ static long long generic_chunk(const bg_ctx* c, long long N) {
 
 size_t bg_scratch_bytes(const bg_ctx* c, long long N) {
     if (!c || N <= 0) return 0;
-    if (!(c->mode & BG_REC_CDBG) || use_quad(c)) return 0;
+    if (!(c->mode & BG_REC_CDBG)) return 0;
+    if (use_prog(c)) return bg::prog_scratch_bytes(c->prog, N);
     return bg::cdbg_generic_scratch_per_event(c->n) * (size_t)generic_chunk(c, N);
 }
 
 size_t bg_current_bytes_per_event(const bg_ctx* c) {
     if (!c) return 0;
     if (c->mode & BG_REC_COBG) return (size_t)(c->n - 1) * c->n / 2 * 64;   // one ordering's current table
-    if (use_quad(c)) return bg::cdbg_quad_current_bytes(c->n);
+    if (use_prog(c)) return bg::prog_state_bytes(c->prog);
     return ((size_t)1 << (c->n - 1)) * 3 * 160;
 }
 
@@ -267,8 +279,30 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
     switch (key) {
         case BG_OPT_KERNEL:
             if (value < 0 || value > 2) return BG_EINVAL;
-            if (value == 2 && !(c->mode == BG_CDBG_GIVEN && bg::cdbg_quad_supported(c->n))) return BG_EUNSUPPORTED;
+            if (value == 2 && !c->prog) return BG_EUNSUPPORTED;
             c->kernel_opt = (int)value;
+            return BG_OK;
+        case BG_OPT_LANES: {
+            if (c->mode != BG_CDBG_GIVEN || c->n > kProgMaxN) return BG_EUNSUPPORTED;
+            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32)
+                return BG_EINVAL;
+            const int G = value ? (int)value : auto_lanes(c->n);
+            if (c->prog && bg::prog_lanes(c->prog) == G) return BG_OK;
+            cudaDeviceSynchronize();
+            bg::ProgTable* t = nullptr;
+            const int rc = bg::prog_table_create(c->n, G, &t);
+            if (rc != BG_OK) return rc;
+            bg::prog_table_destroy(c->prog);
+            c->prog = t;
+            return BG_OK;
+        }
+        case BG_OPT_TIMING:
+            if (value != 0 && value != 1) return BG_EINVAL;
+            if (value && !c->ev0) {
+                if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) return BG_ECUDA;
+            }
+            c->timing = (int)value;
+            c->timed = false;
             return BG_OK;
         case BG_OPT_SCRATCH_LIMIT:
             if (value < (1ll << 20)) return BG_EINVAL;
@@ -292,6 +326,15 @@ int bg_build_colour_matrix(int n, double* C_host) {
 }
 
 int bg_last_launch_count(const bg_ctx* c) { return c ? c->last_launches : 0; }
+
+int bg_last_kernel_ms(bg_ctx* c, double* ms) {
+    if (!c || !ms || !c->timing || !c->timed) return BG_EINVAL;
+    if (cudaEventSynchronize(c->ev1) != cudaSuccess) return BG_ECUDA;
+    float f = 0.f;
+    if (cudaEventElapsedTime(&f, c->ev0, c->ev1) != cudaSuccess) return BG_ECUDA;
+    *ms = (double)f;
+    return BG_OK;
+}
 const char* bg_last_kernel_name(const bg_ctx* c) { return c ? c->last_kernel : "none"; }
 
 int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const signed char* hel,
@@ -305,23 +348,30 @@ int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const 
     if ((c->mode & BG_COL_GIVEN) && !col) return BG_EINVAL;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaError_t err = cudaSuccess;
+    cudaEvent_t ev0 = c->timing ? c->ev0 : nullptr, ev1 = c->timing ? c->ev1 : nullptr;
+    c->timed = c->timing != 0;
     if (c->mode & BG_REC_COBG) {
+        if (ev0) cudaEventRecord(ev0, s);
         err = bg::cobg_generic_launch(s, c->n, helsum, c->nperm, c->dC, N, mom, hel, out);
+        if (ev1) cudaEventRecord(ev1, s);
         c->last_launches = 1;
         c->last_kernel = "cobg_generic_kernel";
-    } else if (use_quad(c)) {
-        err = bg::cdbg_quad_launch(s, c->n, c->sm_count, N, mom, hel, col, out);
-        c->last_launches = 1;
-        c->last_kernel = "cdbg_quad_kernel";
+    } else if (use_prog(c)) {
+        int rc = ensure_scratch(c, N);
+        if (rc != BG_OK) return rc;
+        err = bg::cdbg_prog_launch(s, c->prog, c->sm_count, N, mom, hel, col, out, c->scratch, &c->last_launches, ev0, ev1);
+        c->last_kernel = "cdbg_prog_kernel";
     } else {
         int rc = ensure_scratch(c, N);
         if (rc != BG_OK) return rc;
         const long long chunk = generic_chunk(c, N);
+        if (ev0) cudaEventRecord(ev0, s);
         for (long long first = 0; first < N && err == cudaSuccess; first += chunk) {
             const long long count = std::min(chunk, N - first);
             err = bg::cdbg_generic_launch(s, c->n, helsum, N, first, count, mom, hel, col, out, c->scratch);
             c->last_launches++;
         }
+        if (ev1) cudaEventRecord(ev1, s);
         c->last_kernel = "cdbg_generic_kernel";
     }
     return err == cudaSuccess ? BG_OK : BG_ECUDA;

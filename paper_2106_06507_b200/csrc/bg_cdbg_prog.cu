@@ -1,0 +1,447 @@
+// Colour-class program interpreter: the performance path of the colour-dressed recursion (CDBG, PAPER.md
+// Eq. 28-32, closed with Eq. 22) for discrete colour-flow indices.
+//
+// Pipeline of one bg_eval (all on the caller's stream):
+//   1. cdbg_classify_kernel   one thread per event: colour codes -> canonical gluon order (a relabelling, under
+//                             which |A|^2 is invariant) + colour-class id; histogram of classes
+//   2. cdbg_scan_kernel       exclusive scan of the histogram (classes ordered by program length)
+//   3. cdbg_scatter_kernel    counting sort: event ids grouped by class, so that a warp runs equal programs
+//   4. cdbg_prog_kernel<G>    G lanes per event run the class program (bg_program.h): vertex operations read their
+//                             operands from the event's state block in shared memory, accumulate in registers and
+//                             write each finished current back once.  Levels (popcount of the subset) are separated
+//                             by __syncwarp; the closure amplitude is reduced over the G lanes with shuffles.
+// State layout in shared memory: per warp a slab of [state_cx][EPW] complex doubles (EPW = 32/G events per warp,
+// event index fastest) so that a quarter-warp's LDS.128 touches eight different 16-byte bank groups.
+#include <algorithm>
+#include <cstring>
+#include <new>
+#include <numeric>
+#include <vector>
+
+#include "bg_internal.h"
+#include "bg_math.cuh"
+#include "bg_program.h"
+
+namespace bg {
+
+struct ClassInfo {            // 32 bytes
+    uint32_t op_base;         // first op of the class in the op array (units of ProgOp)
+    uint16_t state_cx;
+    uint8_t closure_code;
+    uint8_t valid;
+    uint16_t level_steps[11];
+    uint16_t pad;
+};
+static_assert(sizeof(ClassInfo) == 32, "ClassInfo layout");
+
+struct ProgTable {
+    int n, G;
+    long long num_classes;
+    int max_state_cx;
+    double mean_steps;
+    ClassInfo* d_info;
+    uint32_t* d_sortkey;      // class id -> position in the order the events are grouped by
+    ProgOp* d_ops;
+    size_t ops_bytes;
+};
+
+__constant__ unsigned c_mscount[kMaxN + 1][kNumCodes];   // multiset_count(r, t) for r <= 12, t <= 8
+
+struct ProgParams {
+    int n;
+    long long N;
+    const double* mom;
+    const signed char* hel;
+    double* out;
+    const ClassInfo* info;
+    const ProgOp* ops;
+    const uint32_t* cls;       // [N] class id per event (0xFFFFFFFF: colour codes out of range)
+    const uint64_t* perm;      // [N] canonical order: nibble k = original index of canonical gluon k
+    const uint32_t* order;     // [N] event ids grouped by class
+    int slab_cx;               // complex doubles of state per event in the slab
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// 1. classification
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+cdbg_classify_kernel(int n, long long N, long long num_classes, const signed char* __restrict__ col,
+                     const ClassInfo* __restrict__ info, const uint32_t* __restrict__ sortkey,
+                     uint32_t* __restrict__ cls, uint64_t* __restrict__ perm, uint32_t* __restrict__ hist) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= N) return;
+    int code[kMaxN], cnt[kNumCodes];
+#pragma unroll
+    for (int c = 0; c < kNumCodes; c++) cnt[c] = 0;
+    bool ok = true;
+    for (int k = 0; k < n; k++) {
+        const int i = col[(size_t)(2 * k) * N + e] - 1, j = col[(size_t)(2 * k + 1) * N + e] - 1;
+        ok = ok && i >= 0 && i < 3 && j >= 0 && j < 3;
+        code[k] = ok ? 3 * i + j : 0;
+    }
+    if (!ok) {
+        cls[e] = 0xFFFFFFFFu;
+        perm[e] = 0;
+        atomicAdd(&hist[num_classes], 1u);
+        return;
+    }
+    for (int k = 0; k < n; k++) {
+#pragma unroll
+        for (int c = 0; c < kNumCodes; c++) cnt[c] += code[k] == c;
+    }
+    unsigned rank = 0;
+    int r = n;
+#pragma unroll
+    for (int t = 0; t < kNumCodes - 1; t++) {
+        for (int c = 0; c < cnt[t]; c++) rank += c_mscount[r - c][kNumCodes - 1 - t];
+        r -= cnt[t];
+    }
+    const ClassInfo ci = info[rank];
+    uint64_t pm = 0;
+    if (ci.valid) {
+        int lastk = 0;
+        for (int k = 0; k < n; k++)
+            if (code[k] == ci.closure_code) lastk = k;
+        int pos = 0;
+        for (int c = 0; c < kNumCodes; c++)
+            for (int k = 0; k < n; k++)
+                if (code[k] == c && k != lastk) pm |= (uint64_t)k << (4 * pos++);
+        pm |= (uint64_t)lastk << (4 * (n - 1));
+    }
+    cls[e] = rank;
+    perm[e] = pm;
+    atomicAdd(&hist[sortkey[rank]], 1u);
+}
+
+// 2. exclusive scan of hist[0..count) in place (one block)
+__global__ void __launch_bounds__(1024) cdbg_scan_kernel(uint32_t* __restrict__ hist, int count) {
+    __shared__ uint32_t warp_tot[32];
+    __shared__ uint32_t carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int base = 0; base < count; base += 1024) {
+        const int i = base + threadIdx.x;
+        const uint32_t v = i < count ? hist[i] : 0u;
+        uint32_t x = v;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, x, d);
+            if (lane >= d) x += y;
+        }
+        if (lane == 31) warp_tot[warp] = x;
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t w = warp_tot[lane];
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, w, d);
+                if (lane >= d) w += y;
+            }
+            warp_tot[lane] = w;
+        }
+        __syncthreads();
+        const uint32_t before = carry + (warp ? warp_tot[warp - 1] : 0u) + (x - v);
+        if (i < count) hist[i] = before;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry = before + v;
+        __syncthreads();
+    }
+}
+
+// 3. scatter event ids into class order
+__global__ void __launch_bounds__(256)
+cdbg_scatter_kernel(long long N, long long num_classes, const uint32_t* __restrict__ cls,
+                    const uint32_t* __restrict__ sortkey, uint32_t* __restrict__ cursor, uint32_t* __restrict__ order) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= N) return;
+    const uint32_t c = cls[e];
+    const uint32_t key = c == 0xFFFFFFFFu ? (uint32_t)num_classes : sortkey[c];
+    order[atomicAdd(&cursor[key], 1u)] = (uint32_t)e;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// 4. interpreter
+// ---------------------------------------------------------------------------------------------------------
+template <int EPW>
+__device__ __forceinline__ cx lds(const double2* S, int o) {
+    const double2 v = S[o * EPW];
+    return mk(v.x, v.y);
+}
+template <int EPW>
+__device__ __forceinline__ void sts(double2* S, int o, cx v) {
+    S[o * EPW] = make_double2(v.re, v.im);
+}
+
+template <int G>
+__global__ void __launch_bounds__(128) cdbg_prog_kernel(const ProgParams p) {
+    constexpr int EPW = 32 / G;
+    extern __shared__ double2 smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int q = lane % EPW, g = lane / EPW;
+    double2* S = smem + (size_t)warp * p.slab_cx * EPW + q;
+    const long long ntasks = (p.N + EPW - 1) / EPW;
+    const int nlev = p.n - 1;
+    const long long N = p.N;
+
+    for (long long task = (long long)blockIdx.x * 4 + warp; task < ntasks; task += (long long)gridDim.x * 4) {
+        const long long idx = task * EPW + q;
+        const bool have = idx < N;
+        const long long e = have ? (long long)p.order[idx] : 0;
+        const uint32_t cls = have ? p.cls[e] : 0xFFFFFFFFu;
+        const ClassInfo* ci = p.info + (cls == 0xFFFFFFFFu ? 0 : cls);
+        const bool valid = cls != 0xFFFFFFFFu && ci->valid;
+        const uint64_t perm = p.perm[e];
+        const ProgOp* ops = p.ops + ci->op_base + g;
+
+        cx amp = mk(0.0, 0.0);
+        cx acc[4], tacc[6];
+        double Pt[4];
+#pragma unroll
+        for (int c = 0; c < 4; c++) { acc[c] = mk(0.0, 0.0); Pt[c] = 0.0; }
+#pragma unroll
+        for (int c = 0; c < 6; c++) tacc[c] = mk(0.0, 0.0);
+
+        for (int lvl = 0; lvl < nlev; lvl++) {
+            const int steps = valid ? (int)ci->level_steps[lvl] : 0;
+            for (int s = 0; s < steps; s++) {
+                const uint4 raw = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s * G));
+                const int offA = raw.x & 0xFFFF, offB = raw.x >> 16;
+                const int offP1 = raw.y & 0xFFFF, offDst = raw.y >> 16;
+                const int offPt = raw.z & 0xFFFF;
+                const unsigned flags = raw.z >> 16;
+                if (flags & OPF_VALID) {
+                    if (flags & OPF_FIRST) {
+#pragma unroll
+                        for (int c = 0; c < 4; c++) acc[c] = mk(0.0, 0.0);
+#pragma unroll
+                        for (int c = 0; c < 6; c++) tacc[c] = mk(0.0, 0.0);
+                        const cx p01 = lds<EPW>(S, offPt), p23 = lds<EPW>(S, offPt + 1);
+                        Pt[0] = p01.re; Pt[1] = p01.im; Pt[2] = p23.re; Pt[3] = p23.im;
+                    }
+                    cx a[4], b[4];
+#pragma unroll
+                    for (int c = 0; c < 4; c++) { a[c] = lds<EPW>(S, offA + c); b[c] = lds<EPW>(S, offB + c); }
+                    double P1[4], P2[4];
+                    {
+                        const cx p01 = lds<EPW>(S, offP1), p23 = lds<EPW>(S, offP1 + 1);
+                        P1[0] = p01.re; P1[1] = p01.im; P1[2] = p23.re; P1[3] = p23.im;
+                    }
+#pragma unroll
+                    for (int c = 0; c < 4; c++) P2[c] = Pt[c] - P1[c];
+                    const double sign = (flags & OPF_NEG) ? -1.0 : 1.0;
+                    v3_acc(acc, P1, P2, a, b, sign);
+                    if (flags & OPF_TENB) {
+                        cx T[6];
+#pragma unroll
+                        for (int c = 0; c < 6; c++) T[c] = lds<EPW>(S, offB + 4 + c);
+                        tcontract_acc(acc, T, a, sign);
+                    }
+                    if (flags & OPF_TENA) {
+                        cx T[6];
+#pragma unroll
+                        for (int c = 0; c < 6; c++) T[c] = lds<EPW>(S, offA + 4 + c);
+                        tcontract_acc(acc, T, b, -sign);
+                    }
+                    if (!(flags & OPF_CLOSURE)) tbuild_acc(tacc, a, b, sign);
+                    if (flags & OPF_LAST) {
+                        if (flags & OPF_CLOSURE) {
+                            cx en[4];
+#pragma unroll
+                            for (int c = 0; c < 4; c++) en[c] = lds<EPW>(S, offDst + c);
+                            const cx d = mdot(en, acc);
+                            amp.re = fma(kInvSqrt2, d.re, amp.re);
+                            amp.im = fma(kInvSqrt2, d.im, amp.im);
+                        } else {
+                            const double f = kInvSqrt2 / mdot(Pt, Pt);
+#pragma unroll
+                            for (int c = 0; c < 4; c++) sts<EPW>(S, offDst + c, f * acc[c]);
+#pragma unroll
+                            for (int c = 0; c < 6; c++) sts<EPW>(S, offDst + 4 + c, kInvSqrt2 * tacc[c]);
+                        }
+                    }
+                } else if (flags & OPF_EXT) {
+                    const int k = (int)raw.w;
+                    const int orig = (int)((perm >> (4 * k)) & 0xF);
+                    double pk[4];
+#pragma unroll
+                    for (int c = 0; c < 4; c++) pk[c] = p.mom[(size_t)(orig * 4 + c) * N + e];
+                    cx eps[4];
+                    polarisation(pk, (int)p.hel[(size_t)orig * N + e], eps);
+#pragma unroll
+                    for (int c = 0; c < 4; c++) sts<EPW>(S, offDst + c, eps[c]);
+                    if (offPt != 0xFFFF) {
+                        sts<EPW>(S, offPt, mk(pk[0], pk[1]));
+                        sts<EPW>(S, offPt + 1, mk(pk[2], pk[3]));
+                    }
+                } else if (flags & OPF_PSUM) {
+                    const unsigned mask = raw.w;
+                    double ps[4] = {0.0, 0.0, 0.0, 0.0};
+                    for (int k = 0; k < p.n - 1; k++) {
+                        if ((mask >> k) & 1u) {
+                            const int orig = (int)((perm >> (4 * k)) & 0xF);
+#pragma unroll
+                            for (int c = 0; c < 4; c++) ps[c] += p.mom[(size_t)(orig * 4 + c) * N + e];
+                        }
+                    }
+                    sts<EPW>(S, offPt, mk(ps[0], ps[1]));
+                    sts<EPW>(S, offPt + 1, mk(ps[2], ps[3]));
+                }
+            }
+            ops += (size_t)steps * G;
+            __syncwarp();
+        }
+        // closure amplitude: sum of the G lanes' partial contractions (Eq. 22), then |A|^2
+#pragma unroll
+        for (int d = EPW; d < 32; d <<= 1) {
+            amp.re += __shfl_xor_sync(0xFFFFFFFFu, amp.re, d);
+            amp.im += __shfl_xor_sync(0xFFFFFFFFu, amp.im, d);
+        }
+        if (g == 0 && have) p.out[e] = valid ? fma(amp.re, amp.re, amp.im * amp.im) : 0.0;
+        __syncwarp();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------------
+static void enumerate_counts(int t, int r, int* counts, std::vector<std::vector<int>>& out) {
+    if (t == kNumCodes - 1) {
+        counts[t] = r;
+        out.emplace_back(counts, counts + kNumCodes);
+        return;
+    }
+    for (int c = 0; c <= r; c++) {
+        counts[t] = c;
+        enumerate_counts(t + 1, r - c, counts, out);
+    }
+}
+
+int prog_table_create(int n, int G, ProgTable** out) {
+    *out = nullptr;
+    if (n < 4 || n > kMaxN || (G != 1 && G != 2 && G != 4 && G != 8 && G != 16 && G != 32)) return BG_EINVAL;
+    std::vector<std::vector<int>> all;
+    int counts[kNumCodes];
+    enumerate_counts(0, n, counts, all);
+    const long long nc = (long long)all.size();
+    if (nc != multiset_count(n, kNumCodes)) return BG_EINVAL;
+    std::vector<ClassInfo> info(nc);
+    std::vector<ProgOp> ops;
+    std::vector<int> steps(nc, 0);
+    int max_state = 0;
+    for (long long r = 0; r < nc; r++) {
+        if (class_rank(n, all[r].data()) != r) return BG_EINVAL;
+        ClassProgram cp;
+        build_class(n, G, all[r].data(), cp);
+        ClassInfo& ci = info[r];
+        std::memset(&ci, 0, sizeof(ci));
+        if (!cp.valid) continue;
+        ci.valid = 1;
+        ci.op_base = (uint32_t)ops.size();
+        ci.state_cx = (uint16_t)cp.state_cx;
+        ci.closure_code = (uint8_t)cp.closure_code;
+        for (int l = 0; l < n - 1; l++) ci.level_steps[l] = cp.level_steps[l];
+        steps[r] = cp.total_steps;
+        max_state = std::max(max_state, cp.state_cx);
+        ops.insert(ops.end(), cp.ops.begin(), cp.ops.end());
+    }
+    // grouping order: longest programs first (the tail of the grid then runs the short ones), invalid last
+    std::vector<uint32_t> by(nc), sortkey(nc);
+    std::iota(by.begin(), by.end(), 0u);
+    std::stable_sort(by.begin(), by.end(), [&](uint32_t a, uint32_t b) { return steps[a] > steps[b]; });
+    for (long long i = 0; i < nc; i++) sortkey[by[i]] = (uint32_t)i;
+
+    ProgTable* t = new (std::nothrow) ProgTable();
+    if (!t) return BG_ENOMEM;
+    std::memset(t, 0, sizeof(*t));
+    t->n = n; t->G = G; t->num_classes = nc; t->max_state_cx = max_state;
+    t->ops_bytes = std::max<size_t>(ops.size(), 1) * sizeof(ProgOp);
+    unsigned ms[kMaxN + 1][kNumCodes];
+    for (int r = 0; r <= kMaxN; r++)
+        for (int tt = 0; tt < kNumCodes; tt++) ms[r][tt] = (unsigned)multiset_count(r, tt);
+    bool ok = cudaMalloc(&t->d_info, sizeof(ClassInfo) * nc) == cudaSuccess &&
+              cudaMalloc(&t->d_sortkey, sizeof(uint32_t) * nc) == cudaSuccess &&
+              cudaMalloc(&t->d_ops, t->ops_bytes) == cudaSuccess;
+    ok = ok && cudaMemcpy(t->d_info, info.data(), sizeof(ClassInfo) * nc, cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(t->d_sortkey, sortkey.data(), sizeof(uint32_t) * nc, cudaMemcpyHostToDevice) == cudaSuccess &&
+         (ops.empty() || cudaMemcpy(t->d_ops, ops.data(), ops.size() * sizeof(ProgOp), cudaMemcpyHostToDevice) == cudaSuccess) &&
+         cudaMemcpyToSymbol(c_mscount, ms, sizeof(ms)) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        prog_table_destroy(t);
+        return BG_ENOMEM;
+    }
+    *out = t;
+    return BG_OK;
+}
+
+void prog_table_destroy(ProgTable* t) {
+    if (!t) return;
+    if (t->d_info) cudaFree(t->d_info);
+    if (t->d_sortkey) cudaFree(t->d_sortkey);
+    if (t->d_ops) cudaFree(t->d_ops);
+    delete t;
+}
+
+size_t prog_state_bytes(const ProgTable* t) { return t ? (size_t)t->max_state_cx * 16 : 0; }
+int prog_lanes(const ProgTable* t) { return t ? t->G : 0; }
+
+// scratch: cls u32[N] | order u32[N] | perm u64[N] | hist u32[num_classes + 1]
+size_t prog_scratch_bytes(const ProgTable* t, long long N) {
+    return (size_t)N * 16 + ((size_t)t->num_classes + 1) * 4 + 256;
+}
+
+template <int G>
+static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p) {
+    constexpr int EPW = 32 / G;
+    const size_t smem = (size_t)4 * EPW * p.slab_cx * 16;
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    if (smem > 227 * 1024) return cudaErrorInvalidValue;
+    int per_sm = (int)std::min<size_t>(16, (227 * 1024) / (smem + 1024));
+    if (per_sm < 1) per_sm = 1;
+    const long long ntasks = (p.N + EPW - 1) / EPW;
+    const long long want = (ntasks + 3) / 4;
+    const unsigned blocks = (unsigned)std::max<long long>(1, std::min<long long>(want, (long long)sm_count * per_sm));
+    cdbg_prog_kernel<G><<<blocks, 128, smem, s>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
+                             const signed char* hel, const signed char* col, double* out, void* scratch,
+                             int* launches, cudaEvent_t ev0, cudaEvent_t ev1) {
+    uint32_t* cls = (uint32_t*)scratch;
+    uint32_t* order = cls + N;
+    uint64_t* perm = (uint64_t*)(order + N + (N & 1));
+    uint32_t* hist = (uint32_t*)(perm + N);
+    const int nbins = (int)t->num_classes + 1;
+    cudaError_t err = cudaMemsetAsync(hist, 0, sizeof(uint32_t) * nbins, s);
+    if (err != cudaSuccess) return err;
+    const unsigned eb = (unsigned)((N + 255) / 256);
+    cdbg_classify_kernel<<<eb, 256, 0, s>>>(t->n, N, t->num_classes, col, t->d_info, t->d_sortkey, cls, perm, hist);
+    cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins);
+    cdbg_scatter_kernel<<<eb, 256, 0, s>>>(N, t->num_classes, cls, t->d_sortkey, hist, order);
+    if ((err = cudaGetLastError()) != cudaSuccess) return err;
+    ProgParams p;
+    p.n = t->n; p.N = N; p.mom = mom; p.hel = hel; p.out = out;
+    p.info = t->d_info; p.ops = t->d_ops; p.cls = cls; p.perm = perm; p.order = order;
+    p.slab_cx = t->max_state_cx;
+    if (ev0) cudaEventRecord(ev0, s);
+    switch (t->G) {
+        case 1: err = launch_interp<1>(s, t, sm_count, p); break;
+        case 2: err = launch_interp<2>(s, t, sm_count, p); break;
+        case 4: err = launch_interp<4>(s, t, sm_count, p); break;
+        case 8: err = launch_interp<8>(s, t, sm_count, p); break;
+        case 16: err = launch_interp<16>(s, t, sm_count, p); break;
+        default: err = launch_interp<32>(s, t, sm_count, p); break;
+    }
+    if (ev1) cudaEventRecord(ev1, s);
+    *launches = 4;
+    return err;
+}
+
+}  // namespace bg

@@ -6,6 +6,8 @@
 
 #include "../../include/bg.h"
 
+namespace bg { struct ProgTable; }
+
 struct bg_ctx {
     int n;
     int mode;
@@ -27,7 +29,13 @@ struct bg_ctx {
     signed char* d_col;
     double* d_out;
     long long staged_events;
+    // colour-class programs (CDBG, given colours)
+    bg::ProgTable* prog;
+    int prog_lanes;            // BG_OPT_LANES (0 = automatic)
     // bookkeeping
+    int timing;                // BG_OPT_TIMING
+    cudaEvent_t ev0, ev1;
+    bool timed;
     int last_launches;
     const char* last_kernel;
 };
@@ -43,11 +51,15 @@ cudaError_t cdbg_generic_launch(cudaStream_t s, int n, bool helsum, long long N,
 cudaError_t cobg_generic_launch(cudaStream_t s, int n, bool helsum, int nperm, const double* dC, long long N,
                                 const double* mom, const signed char* hel, double* out);
 
-// ---- quad kernel (bg_cdbg_quad.cu): four lanes per event, currents in shared memory ----------------------
-bool cdbg_quad_supported(int n);
-size_t cdbg_quad_current_bytes(int n);
-cudaError_t cdbg_quad_launch(cudaStream_t s, int n, int sm_count, long long N, const double* mom,
-                             const signed char* hel, const signed char* col, double* out);
+// ---- colour-class program interpreter (bg_cdbg_prog.cu): G lanes per event, currents in shared memory -------
+int prog_table_create(int n, int G, ProgTable** out);      // BG_* code
+void prog_table_destroy(ProgTable* t);
+size_t prog_state_bytes(const ProgTable* t);               // largest per-event state block
+int prog_lanes(const ProgTable* t);
+size_t prog_scratch_bytes(const ProgTable* t, long long N);
+cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
+                             const signed char* hel, const signed char* col, double* out, void* scratch,
+                             int* launches, cudaEvent_t ev0, cudaEvent_t ev1);
 
 // ---- colour matrix (bg_colour.cpp part of bg_api.cu) ------------------------------------------------------
 int build_colour_matrix(int n, double* C /* (n-2)!^2 */);

@@ -1,0 +1,274 @@
+// Colour-class program generator (see bg_program.h).  Integer bookkeeping only.
+#include "bg_program.h"
+
+#include <algorithm>
+#include <cstring>
+
+namespace bg {
+
+long long multiset_count(int r, int t) {
+    if (r < 0) return 0;
+    if (t == 0) return r == 0 ? 1 : 0;
+    const int k = t - 1, N = r + t - 1;   // C(N, k)
+    long long num = 1;
+    for (int i = 1; i <= k; i++) num = num * (N - k + i) / i;
+    return num;
+}
+
+long long class_rank(int n, const int* m) {
+    long long rank = 0;
+    int r = n;
+    for (int t = 0; t < kNumCodes - 1; t++) {
+        for (int c = 0; c < m[t]; c++) rank += multiset_count(r - c, kNumCodes - 1 - t);
+        r -= m[t];
+    }
+    return rank;
+}
+
+namespace {
+
+// colour type of a subset current: 0x40 dead | 0x80|mask diagonal entries | (h<<2)|g one off-diagonal entry
+inline bool has_entry(unsigned t, int h, int g) {
+    if (t & 0x80u) return h == g && ((t >> h) & 1u);
+    if (t & 0x40u) return false;
+    return t == (unsigned)((h << 2) | g);
+}
+
+struct VOp {
+    int pa, sa, pb, sb;   // subset and slot (0..2) of the two operands; |pa| <= |pb|
+    bool neg;
+};
+
+struct Target {
+    int pi, h, g;
+    std::vector<VOp> ops;
+};
+
+inline int popc(int x) { return __builtin_popcount((unsigned)x); }
+
+}  // namespace
+
+void build_program(int n, int G, const int* code, ClassProgram& out) {
+    out = ClassProgram();
+    const int m = n - 1, nsub = 1 << m, full = nsub - 1;
+    int ci[kMaxN], cj[kMaxN], wk[kMaxN];
+    for (int k = 0; k < n; k++) {
+        ci[k] = code[k] / 3;
+        cj[k] = code[k] % 3;
+        wk[k] = (1 << (8 * ci[k])) - (1 << (8 * cj[k]));
+    }
+    out.closure_code = code[n - 1];
+
+    std::vector<uint8_t> type(nsub, 0x40);
+    std::vector<int> off(nsub * 3, -1), poff(nsub, -1);
+    int next = 0;
+    // external currents (4 cx) and the closure polarisation
+    for (int k = 0; k < m; k++) {
+        const int pi = 1 << k;
+        const bool diag = ci[k] == cj[k];
+        type[pi] = diag ? (uint8_t)(0x80u | (1u << ci[k])) : (uint8_t)((ci[k] << 2) | cj[k]);
+        off[pi * 3 + (diag ? ci[k] : 0)] = next;
+        next += 4;
+    }
+    const int off_epsn = next;
+    next += 4;
+    for (int k = 0; k < m; k++) { poff[1 << k] = next; next += 2; }
+
+    std::vector<std::vector<Target>> levels(m + 1);   // by popcount
+    for (int pi = 3; pi <= full; pi++) {
+        if ((pi & (pi - 1)) == 0) continue;
+        const int low = pi & -pi, rest = pi ^ low;
+        int D = 0;
+        for (int k = 0; k < m; k++)
+            if ((pi >> k) & 1) D += wk[k];
+        int cand_h[3], cand_g[3], ncand = 0;
+        bool diag = false;
+        if (D == 0) {
+            diag = true;
+            for (int h = 0; h < 3; h++) { cand_h[ncand] = h; cand_g[ncand] = h; ncand++; }
+        } else {
+            for (int h = 0; h < 3; h++)
+                for (int g = 0; g < 3; g++)
+                    if (h != g && D == (1 << (8 * h)) - (1 << (8 * g))) { cand_h[0] = h; cand_g[0] = g; ncand = 1; }
+        }
+        if (pi == full) {
+            // closure, Eq. 22: only the entry contracted with X_n = e_{i_n j_n}
+            const int h = cj[n - 1], g = ci[n - 1];
+            bool ok = false;
+            for (int c = 0; c < ncand; c++) ok = ok || (cand_h[c] == h && cand_g[c] == g);
+            ncand = 0;
+            if (ok) { cand_h[0] = h; cand_g[0] = g; ncand = 1; }
+        }
+        unsigned livemask = 0;
+        for (int cd = 0; cd < ncand; cd++) {
+            const int h = cand_h[cd], g = cand_g[cd];
+            Target t;
+            t.pi = pi; t.h = h; t.g = g;
+            for (int sub = (rest - 1) & rest;; sub = (sub - 1) & rest) {
+                const int p1 = low | sub, p2 = pi ^ p1;
+                const unsigned t1 = type[p1], t2 = type[p2];
+                if (!((t1 | t2) & 0x40u)) {
+                    for (int k = 0; k < 3; k++) {
+                        const bool fwd = has_entry(t1, h, k) && has_entry(t2, k, g);
+                        const bool bwd = has_entry(t2, h, k) && has_entry(t1, k, g);
+                        if (fwd && bwd && h == k && k == g) continue;   // +X - X
+                        for (int dir = 0; dir < 2; dir++) {
+                            if (dir == 0 ? !fwd : !bwd) continue;
+                            const int ah = dir == 0 ? h : k, ag = dir == 0 ? k : g;   // entry of pi_1
+                            const int bh = dir == 0 ? k : h, bg_ = dir == 0 ? g : k;  // entry of pi_2
+                            VOp o;
+                            o.pa = p1; o.sa = ah == ag ? ah : 0;
+                            o.pb = p2; o.sb = bh == bg_ ? bh : 0;
+                            o.neg = dir == 1;
+                            if (popc(o.pa) > popc(o.pb)) {   // X(a,b) = -X(b,a): keep the smaller subset as `a`
+                                std::swap(o.pa, o.pb);
+                                std::swap(o.sa, o.sb);
+                                o.neg = !o.neg;
+                            }
+                            t.ops.push_back(o);
+                        }
+                    }
+                }
+                if (sub == 0) break;
+            }
+            if (t.ops.empty()) continue;
+            livemask |= diag ? (1u << h) : 1u;
+            if (pi != full) {
+                off[pi * 3 + (h == g ? h : 0)] = next;
+                next += 10;
+            }
+            levels[popc(pi)].push_back(std::move(t));
+        }
+        if (pi != full) {
+            uint8_t ty = 0x40u;
+            if (livemask) ty = diag ? (uint8_t)(0x80u | livemask) : (uint8_t)((cand_h[0] << 2) | cand_g[0]);
+            type[pi] = ty;
+        }
+        if (livemask) { poff[pi] = next; next += 2; }
+    }
+    if (levels[m].empty()) return;   // no closure: amplitude vanishes identically
+    out.valid = true;
+    out.state_cx = next;
+    out.level_steps.assign(m, 0);
+
+    auto emit_level = [&](int lvl, std::vector<std::vector<ProgOp>>& lanes) {
+        size_t steps = 0;
+        for (auto& l : lanes) steps = std::max(steps, l.size());
+        out.level_steps[lvl] = (uint16_t)steps;
+        ProgOp nop;
+        std::memset(&nop, 0, sizeof(nop));
+        for (size_t s = 0; s < steps; s++)
+            for (int l = 0; l < G; l++) out.ops.push_back(s < lanes[l].size() ? lanes[l][s] : nop);
+        out.total_steps += (int)steps;
+    };
+
+    // level 0: setup ops (external currents, subset momenta), heaviest first on the least loaded lane
+    {
+        std::vector<std::vector<ProgOp>> lanes(G);
+        std::vector<int> load(G, 0);
+        auto least = [&]() { return (int)(std::min_element(load.begin(), load.end()) - load.begin()); };
+        for (int k = 0; k < n; k++) {
+            ProgOp o;
+            std::memset(&o, 0, sizeof(o));
+            o.flags = OPF_EXT;
+            o.extra = (uint32_t)k;
+            if (k < m) {
+                const int pi = 1 << k;
+                o.offDst = (uint16_t)off[pi * 3 + (ci[k] == cj[k] ? ci[k] : 0)];
+                o.offPt = (uint16_t)poff[pi];
+            } else {
+                o.offDst = (uint16_t)off_epsn;
+                o.offPt = 0xFFFF;
+            }
+            const int l = least();
+            lanes[l].push_back(o);
+            load[l] += 8;
+        }
+        for (int pi = 3; pi <= full; pi++) {
+            if ((pi & (pi - 1)) == 0 || poff[pi] < 0) continue;
+            ProgOp o;
+            std::memset(&o, 0, sizeof(o));
+            o.flags = OPF_PSUM;
+            o.extra = (uint32_t)pi;
+            o.offPt = (uint16_t)poff[pi];
+            const int l = least();
+            lanes[l].push_back(o);
+            load[l] += 1;
+        }
+        // EXT ops first in every lane so that a warp runs them together
+        for (auto& l : lanes)
+            std::stable_sort(l.begin(), l.end(), [](const ProgOp& a, const ProgOp& b) {
+                return (a.flags & OPF_EXT) > (b.flags & OPF_EXT);
+            });
+        emit_level(0, lanes);
+    }
+
+    auto make_op = [&](const Target& t, const VOp& v) {
+        ProgOp o;
+        std::memset(&o, 0, sizeof(o));
+        o.offA = (uint16_t)off[v.pa * 3 + v.sa];
+        o.offB = (uint16_t)off[v.pb * 3 + v.sb];
+        o.offP1 = (uint16_t)poff[v.pa];
+        o.offPt = (uint16_t)poff[t.pi];
+        o.offDst = t.pi == full ? (uint16_t)off_epsn : (uint16_t)off[t.pi * 3 + (t.h == t.g ? t.h : 0)];
+        o.flags = OPF_VALID | (v.neg ? OPF_NEG : 0) | (popc(v.pa) >= 2 ? OPF_TENA : 0) |
+                  (popc(v.pb) >= 2 ? OPF_TENB : 0) | (t.pi == full ? OPF_CLOSURE : 0);
+        return o;
+    };
+
+    for (int pc = 2; pc <= m; pc++) {
+        std::vector<std::vector<ProgOp>> lanes(G);
+        auto& tg = levels[pc];
+        if (pc == m) {
+            // closure: one target, its ops dealt round-robin; every lane contracts its partial sum with eps_n
+            const Target& t = tg[0];
+            // ops with both tensors first so that lanes hit the same code path together
+            std::vector<VOp> ops = t.ops;
+            std::stable_sort(ops.begin(), ops.end(), [](const VOp& a, const VOp& b) { return popc(a.pa) > popc(b.pa); });
+            for (size_t i = 0; i < ops.size(); i++) lanes[i % G].push_back(make_op(t, ops[i]));
+        } else {
+            std::vector<int> order(tg.size()), load(G, 0);
+            for (size_t i = 0; i < tg.size(); i++) order[i] = (int)i;
+            std::stable_sort(order.begin(), order.end(),
+                             [&](int a, int b) { return tg[a].ops.size() > tg[b].ops.size(); });
+            for (int idx : order) {
+                const int l = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+                for (auto& v : tg[idx].ops) lanes[l].push_back(make_op(tg[idx], v));
+                load[l] += (int)tg[idx].ops.size();
+            }
+        }
+        // mark first / last op of each target run in every lane
+        for (auto& l : lanes) {
+            for (size_t i = 0; i < l.size(); i++) {
+                const bool first = i == 0 || l[i - 1].offDst != l[i].offDst;
+                const bool last = i + 1 == l.size() || l[i + 1].offDst != l[i].offDst;
+                if (first) l[i].flags |= OPF_FIRST;
+                if (last) l[i].flags |= OPF_LAST;
+                out.n_vertex_ops++;
+            }
+        }
+        emit_level(pc - 1, lanes);
+    }
+}
+
+void build_class(int n, int G, const int* counts, ClassProgram& out) {
+    out = ClassProgram();
+    bool have = false;
+    for (int c = 0; c < kNumCodes; c++) {
+        if (!counts[c]) continue;
+        int code[kMaxN], k = 0;
+        for (int t = 0; t < kNumCodes; t++)
+            for (int r = 0; r < counts[t] - (t == c ? 1 : 0); r++) code[k++] = t;
+        code[k++] = c;
+        ClassProgram p;
+        build_program(n, G, code, p);
+        if (!p.valid) continue;   // validity does not depend on the closure leg, but be safe
+        if (!have || p.total_steps < out.total_steps ||
+            (p.total_steps == out.total_steps && p.state_cx < out.state_cx)) {
+            out = std::move(p);
+            have = true;
+        }
+    }
+}
+
+}  // namespace bg

@@ -1,0 +1,67 @@
+// Host-side generator of "colour-class programs" for the colour-dressed recursion (CDBG, Eq. 28-32,
+// L187-213) with discrete colour-flow indices.
+//
+// For fixed (i_k, j_k) the 3x3 colour matrix of every subset current has at most one off-diagonal or up to three
+// diagonal non-zero entries (a product of elementary matrices e_ij is elementary), so WHICH vertex evaluations of
+// Eq. 29 are non-zero, and where their operands live, depends only on the colour assignment - not on momenta or
+// helicities.  |A|^2 is symmetric under relabelling the gluons (p, lambda, i, j permuted together), so events are
+// brought to a canonical gluon order (sorted by the colour code 3*i+j, then one chosen gluon moved to the last
+// place as the closure leg of Eq. 22) and the structure depends only on the MULTISET of colour codes: the "colour
+// class".  For each class this file emits a straight-line program of vertex operations, already distributed
+// over G cooperating lanes and grouped into popcount levels, that the CUDA interpreter (bg_cdbg_prog.cu) runs
+// for every event of the class.  Nothing here touches floating-point event data.
+#pragma once
+#include <stdint.h>
+
+#include <vector>
+
+namespace bg {
+
+// One interpreter instruction (16 bytes).  Offsets are in units of one complex double (16 B) inside the
+// per-event state block.
+struct alignas(16) ProgOp {
+    uint16_t offA;    // vector current a = entry of pi_1 (4 cx, followed by its 6-cx tensor if |pi_1| >= 2)
+    uint16_t offB;    // vector current b = entry of pi_2
+    uint16_t offP1;   // momentum of pi_1 (4 doubles = 2 cx)
+    uint16_t offDst;  // target entry (LAST) | for setup ops: destination
+    uint16_t offPt;   // momentum of the target subset
+    uint16_t flags;
+    uint32_t extra;   // setup ops: gluon index (EXT) or subset mask (PSUM)
+};
+static_assert(sizeof(ProgOp) == 16, "ProgOp must be 16 bytes");
+
+enum : uint16_t {
+    OPF_VALID = 1,     // a vertex evaluation X(a, b)
+    OPF_NEG = 2,       // contributes with sign -1
+    OPF_TENA = 4,      // pi_1 carries a tensor current
+    OPF_TENB = 8,      // pi_2 carries a tensor current
+    OPF_FIRST = 16,    // first op of a target: clear the accumulators, load P(target)
+    OPF_LAST = 32,     // last op of a target: apply 1/sqrt2 (and 1/P^2), store vector + tensor current
+    OPF_CLOSURE = 64,  // target is the full set: contract with eps_n instead of storing (Eq. 22)
+    OPF_EXT = 128,     // setup: external current of gluon `extra` -> offDst, its momentum -> offPt
+    OPF_PSUM = 256     // setup: momentum of subset mask `extra` -> offPt
+};
+
+constexpr int kMaxN = 12;
+constexpr int kNumCodes = 9;   // colour code c = 3*(i-1) + (j-1)
+
+struct ClassProgram {
+    bool valid = false;          // false: the amplitude vanishes identically for this colour class
+    int closure_code = 0;        // colour code of the gluon placed last (closure leg)
+    int state_cx = 0;            // per-event state size in complex doubles
+    int n_vertex_ops = 0;        // number of OPF_VALID ops
+    int total_steps = 0;         // sum over levels of max-lane op count
+    std::vector<uint16_t> level_steps;   // [n-1]: level 0 = setup, then popcount 2 .. n-1
+    std::vector<ProgOp> ops;             // [total_steps][G]
+};
+
+// number of multisets of size r over t types
+long long multiset_count(int r, int t);
+// rank of a count vector m[0..8] (sum = n) in the fixed enumeration order used by host and device
+long long class_rank(int n, const int* counts);
+// Build the program for canonical colour codes code[0..n-1] (code[n-1] = closure leg), G lanes per event.
+void build_program(int n, int G, const int* code, ClassProgram& out);
+// Build the best program (over the choice of closure leg) for a multiset of colour codes.
+void build_class(int n, int G, const int* counts, ClassProgram& out);
+
+}  // namespace bg

@@ -2,7 +2,7 @@
 import numpy as np
 
 
-def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None):
+def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None, lanes=None):
     """ev: workload.Events (AoS numpy).  Returns out[N] (numpy) and the kernel name used."""
     import torch
     import paper_2106_06507_b200 as bg
@@ -15,6 +15,8 @@ def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None):
     try:
         if kernel:
             bg.bg_set_option(ctx, bg.BG_OPT_KERNEL, kernel)
+        if lanes is not None:
+            bg.bg_set_option(ctx, bg.BG_OPT_LANES, lanes)
         if scratch_limit:
             bg.bg_set_option(ctx, bg.BG_OPT_SCRATCH_LIMIT, scratch_limit)
         if host:

@@ -132,6 +132,16 @@ def test_kernel_variants_agree(bg, oracle, wl, n):
     assert np.array_equal(a, c)
 
 
+@pytest.mark.parametrize("n,N", [(4, 515), (5, 1031), (6, 2051), (7, 1029), (8, 519)])
+@pytest.mark.parametrize("lanes", [1, 2, 4, 8, 32])
+def test_program_interpreter_lane_counts(bg, oracle, wl, n, N, lanes):
+    """The colour-class program interpreter with G lanes per event, sizes with ragged last warps."""
+    ev = wl.config_events(4, N=N, n=n)
+    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=2, lanes=lanes)
+    assert name == "cdbg_prog_kernel"
+    check_cdbg(oracle, ev, got)
+
+
 def test_cdbg_helicity_sum_mode(bg, oracle, wl):
     import itertools
     ev = wl.config_events(4, N=40, n=5)
