@@ -184,7 +184,8 @@ __global__ void __launch_bounds__(128) cdbg_prog_kernel(const ProgParams p) {
     const int nlev = p.n - 1;
     const long long N = p.N;
 
-    for (long long task = (long long)blockIdx.x * 4 + warp; task < ntasks; task += (long long)gridDim.x * 4) {
+    const int wpb = blockDim.x >> 5;
+    for (long long task = (long long)blockIdx.x * wpb + warp; task < ntasks; task += (long long)gridDim.x * wpb) {
         const long long idx = task * EPW + q;
         const bool have = idx < N;
         const long long e = have ? (long long)p.order[idx] : 0;
@@ -202,23 +203,18 @@ __global__ void __launch_bounds__(128) cdbg_prog_kernel(const ProgParams p) {
 #pragma unroll
         for (int c = 0; c < 6; c++) tacc[c] = mk(0.0, 0.0);
 
+        uint4 raw = __ldg(reinterpret_cast<const uint4*>(ops));
         for (int lvl = 0; lvl < nlev; lvl++) {
             const int steps = valid ? (int)ci->level_steps[lvl] : 0;
             for (int s = 0; s < steps; s++) {
-                const uint4 raw = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s * G));
+                ops += G;
+                // the op of the next step (the table ends with one spare row of no-ops)
+                const uint4 nxt = __ldg(reinterpret_cast<const uint4*>(ops));
                 const int offA = raw.x & 0xFFFF, offB = raw.x >> 16;
                 const int offP1 = raw.y & 0xFFFF, offDst = raw.y >> 16;
                 const int offPt = raw.z & 0xFFFF;
                 const unsigned flags = raw.z >> 16;
                 if (flags & OPF_VALID) {
-                    if (flags & OPF_FIRST) {
-#pragma unroll
-                        for (int c = 0; c < 4; c++) acc[c] = mk(0.0, 0.0);
-#pragma unroll
-                        for (int c = 0; c < 6; c++) tacc[c] = mk(0.0, 0.0);
-                        const cx p01 = lds<EPW>(S, offPt), p23 = lds<EPW>(S, offPt + 1);
-                        Pt[0] = p01.re; Pt[1] = p01.im; Pt[2] = p23.re; Pt[3] = p23.im;
-                    }
                     cx a[4], b[4];
 #pragma unroll
                     for (int c = 0; c < 4; c++) { a[c] = lds<EPW>(S, offA + c); b[c] = lds<EPW>(S, offB + c); }
@@ -226,6 +222,15 @@ __global__ void __launch_bounds__(128) cdbg_prog_kernel(const ProgParams p) {
                     {
                         const cx p01 = lds<EPW>(S, offP1), p23 = lds<EPW>(S, offP1 + 1);
                         P1[0] = p01.re; P1[1] = p01.im; P1[2] = p23.re; P1[3] = p23.im;
+                    }
+                    if (flags & OPF_FIRST) {
+#pragma unroll
+                        for (int c = 0; c < 4; c++) acc[c] = mk(0.0, 0.0);
+#pragma unroll
+                        for (int c = 0; c < 6; c++) tacc[c] = mk(0.0, 0.0);
+                        const int offP2 = (int)(raw.w & 0xFFFF);
+                        const cx p01 = lds<EPW>(S, offP2), p23 = lds<EPW>(S, offP2 + 1);
+                        Pt[0] = P1[0] + p01.re; Pt[1] = P1[1] + p01.im; Pt[2] = P1[2] + p23.re; Pt[3] = P1[3] + p23.im;
                     }
 #pragma unroll
                     for (int c = 0; c < 4; c++) P2[c] = Pt[c] - P1[c];
@@ -258,6 +263,10 @@ __global__ void __launch_bounds__(128) cdbg_prog_kernel(const ProgParams p) {
                             for (int c = 0; c < 4; c++) sts<EPW>(S, offDst + c, f * acc[c]);
 #pragma unroll
                             for (int c = 0; c < 6; c++) sts<EPW>(S, offDst + 4 + c, kInvSqrt2 * tacc[c]);
+                            if (flags & OPF_STOREP) {
+                                sts<EPW>(S, offPt, mk(Pt[0], Pt[1]));
+                                sts<EPW>(S, offPt + 1, mk(Pt[2], Pt[3]));
+                            }
                         }
                     }
                 } else if (flags & OPF_EXT) {
@@ -274,21 +283,9 @@ __global__ void __launch_bounds__(128) cdbg_prog_kernel(const ProgParams p) {
                         sts<EPW>(S, offPt, mk(pk[0], pk[1]));
                         sts<EPW>(S, offPt + 1, mk(pk[2], pk[3]));
                     }
-                } else if (flags & OPF_PSUM) {
-                    const unsigned mask = raw.w;
-                    double ps[4] = {0.0, 0.0, 0.0, 0.0};
-                    for (int k = 0; k < p.n - 1; k++) {
-                        if ((mask >> k) & 1u) {
-                            const int orig = (int)((perm >> (4 * k)) & 0xF);
-#pragma unroll
-                            for (int c = 0; c < 4; c++) ps[c] += p.mom[(size_t)(orig * 4 + c) * N + e];
-                        }
-                    }
-                    sts<EPW>(S, offPt, mk(ps[0], ps[1]));
-                    sts<EPW>(S, offPt + 1, mk(ps[2], ps[3]));
                 }
+                raw = nxt;
             }
-            ops += (size_t)steps * G;
             __syncwarp();
         }
         // closure amplitude: sum of the G lanes' partial contractions (Eq. 22), then |A|^2
@@ -351,11 +348,17 @@ int prog_table_create(int n, int G, ProgTable** out) {
     std::stable_sort(by.begin(), by.end(), [&](uint32_t a, uint32_t b) { return steps[a] > steps[b]; });
     for (long long i = 0; i < nc; i++) sortkey[by[i]] = (uint32_t)i;
 
+    if ((size_t)(32 / G) * max_state * 16 > 227 * 1024) return BG_EUNSUPPORTED;   // one warp's slab must fit
     ProgTable* t = new (std::nothrow) ProgTable();
     if (!t) return BG_ENOMEM;
     std::memset(t, 0, sizeof(*t));
     t->n = n; t->G = G; t->num_classes = nc; t->max_state_cx = max_state;
-    t->ops_bytes = std::max<size_t>(ops.size(), 1) * sizeof(ProgOp);
+    {   // one spare row of no-ops: the interpreter prefetches one step ahead
+        ProgOp nop;
+        std::memset(&nop, 0, sizeof(nop));
+        ops.insert(ops.end(), (size_t)G, nop);
+    }
+    t->ops_bytes = ops.size() * sizeof(ProgOp);
     unsigned ms[kMaxN + 1][kNumCodes];
     for (int r = 0; r <= kMaxN; r++)
         for (int tt = 0; tt < kNumCodes; tt++) ms[r][tt] = (unsigned)multiset_count(r, tt);
@@ -394,20 +397,22 @@ size_t prog_scratch_bytes(const ProgTable* t, long long N) {
 template <int G>
 static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p) {
     constexpr int EPW = 32 / G;
-    const size_t smem = (size_t)4 * EPW * p.slab_cx * 16;
+    const size_t per_warp = (size_t)EPW * p.slab_cx * 16;
+    if (per_warp > 227 * 1024) return cudaErrorInvalidValue;
+    const int wpb = (int)std::max<size_t>(1, std::min<size_t>(4, (227 * 1024) / per_warp));
+    const size_t smem = per_warp * wpb;
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    if (smem > 227 * 1024) return cudaErrorInvalidValue;
     int per_sm = (int)std::min<size_t>(16, (227 * 1024) / (smem + 1024));
     if (per_sm < 1) per_sm = 1;
     const long long ntasks = (p.N + EPW - 1) / EPW;
-    const long long want = (ntasks + 3) / 4;
+    const long long want = (ntasks + wpb - 1) / wpb;
     const unsigned blocks = (unsigned)std::max<long long>(1, std::min<long long>(want, (long long)sm_count * per_sm));
-    cdbg_prog_kernel<G><<<blocks, 128, smem, s>>>(p);
+    cdbg_prog_kernel<G><<<blocks, 32 * wpb, smem, s>>>(p);
     return cudaGetLastError();
 }
 
@@ -416,7 +421,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
                              int* launches, cudaEvent_t ev0, cudaEvent_t ev1) {
     uint32_t* cls = (uint32_t*)scratch;
     uint32_t* order = cls + N;
-    uint64_t* perm = (uint64_t*)(order + N + (N & 1));
+    uint64_t* perm = (uint64_t*)(order + N);   // 2N u32 before it: 8-byte aligned
     uint32_t* hist = (uint32_t*)(perm + N);
     const int nbins = (int)t->num_classes + 1;
     cudaError_t err = cudaMemsetAsync(hist, 0, sizeof(uint32_t) * nbins, s);

@@ -41,6 +41,7 @@ struct VOp {
 
 struct Target {
     int pi, h, g;
+    bool store_p;   // first live entry of its subset: its LAST op also stores P(pi)
     std::vector<VOp> ops;
 };
 
@@ -132,6 +133,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
                 if (sub == 0) break;
             }
             if (t.ops.empty()) continue;
+            t.store_p = livemask == 0 && pi != full;
             livemask |= diag ? (1u << h) : 1u;
             if (pi != full) {
                 off[pi * 3 + (h == g ? h : 0)] = next;
@@ -162,7 +164,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
         out.total_steps += (int)steps;
     };
 
-    // level 0: setup ops (external currents, subset momenta), heaviest first on the least loaded lane
+    // level 0: external currents and momenta, dealt over the lanes
     {
         std::vector<std::vector<ProgOp>> lanes(G);
         std::vector<int> load(G, 0);
@@ -184,22 +186,6 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
             lanes[l].push_back(o);
             load[l] += 8;
         }
-        for (int pi = 3; pi <= full; pi++) {
-            if ((pi & (pi - 1)) == 0 || poff[pi] < 0) continue;
-            ProgOp o;
-            std::memset(&o, 0, sizeof(o));
-            o.flags = OPF_PSUM;
-            o.extra = (uint32_t)pi;
-            o.offPt = (uint16_t)poff[pi];
-            const int l = least();
-            lanes[l].push_back(o);
-            load[l] += 1;
-        }
-        // EXT ops first in every lane so that a warp runs them together
-        for (auto& l : lanes)
-            std::stable_sort(l.begin(), l.end(), [](const ProgOp& a, const ProgOp& b) {
-                return (a.flags & OPF_EXT) > (b.flags & OPF_EXT);
-            });
         emit_level(0, lanes);
     }
 
@@ -210,9 +196,10 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
         o.offB = (uint16_t)off[v.pb * 3 + v.sb];
         o.offP1 = (uint16_t)poff[v.pa];
         o.offPt = (uint16_t)poff[t.pi];
+        o.extra = (uint32_t)poff[v.pb];
         o.offDst = t.pi == full ? (uint16_t)off_epsn : (uint16_t)off[t.pi * 3 + (t.h == t.g ? t.h : 0)];
         o.flags = OPF_VALID | (v.neg ? OPF_NEG : 0) | (popc(v.pa) >= 2 ? OPF_TENA : 0) |
-                  (popc(v.pb) >= 2 ? OPF_TENB : 0) | (t.pi == full ? OPF_CLOSURE : 0);
+                  (popc(v.pb) >= 2 ? OPF_TENB : 0) | (t.pi == full ? OPF_CLOSURE : 0) | (t.store_p ? OPF_STOREP : 0);
         return o;
     };
 

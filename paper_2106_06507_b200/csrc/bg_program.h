@@ -24,9 +24,9 @@ struct alignas(16) ProgOp {
     uint16_t offB;    // vector current b = entry of pi_2
     uint16_t offP1;   // momentum of pi_1 (4 doubles = 2 cx)
     uint16_t offDst;  // target entry (LAST) | for setup ops: destination
-    uint16_t offPt;   // momentum of the target subset
+    uint16_t offPt;   // momentum of the target subset (written by the target's LAST op)
     uint16_t flags;
-    uint32_t extra;   // setup ops: gluon index (EXT) or subset mask (PSUM)
+    uint32_t extra;   // vertex ops: offset of the momentum of pi_2; EXT: canonical gluon index
 };
 static_assert(sizeof(ProgOp) == 16, "ProgOp must be 16 bytes");
 
@@ -35,11 +35,11 @@ enum : uint16_t {
     OPF_NEG = 2,       // contributes with sign -1
     OPF_TENA = 4,      // pi_1 carries a tensor current
     OPF_TENB = 8,      // pi_2 carries a tensor current
-    OPF_FIRST = 16,    // first op of a target: clear the accumulators, load P(target)
-    OPF_LAST = 32,     // last op of a target: apply 1/sqrt2 (and 1/P^2), store vector + tensor current
+    OPF_FIRST = 16,    // first op of a target: clear the accumulators, P(target) = P(pi_1) + P(pi_2)
+    OPF_LAST = 32,     // last op of a target: apply 1/sqrt2 (and 1/P^2), store vector + tensor current and P
     OPF_CLOSURE = 64,  // target is the full set: contract with eps_n instead of storing (Eq. 22)
-    OPF_EXT = 128,     // setup: external current of gluon `extra` -> offDst, its momentum -> offPt
-    OPF_PSUM = 256     // setup: momentum of subset mask `extra` -> offPt
+    OPF_STOREP = 256,  // (with LAST) also store P(target) at offPt: set on one entry per subset
+    OPF_EXT = 128      // setup: external current of gluon `extra` -> offDst, its momentum -> offPt
 };
 
 constexpr int kMaxN = 12;

@@ -16,7 +16,13 @@ def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None, lanes=None):
         if kernel:
             bg.bg_set_option(ctx, bg.BG_OPT_KERNEL, kernel)
         if lanes is not None:
-            bg.bg_set_option(ctx, bg.BG_OPT_LANES, lanes)
+            try:
+                bg.bg_set_option(ctx, bg.BG_OPT_LANES, lanes)
+            except bg.BgError as e:
+                if e.code == bg.BG_EUNSUPPORTED:
+                    import pytest
+                    pytest.skip(f"{lanes} lanes per event: one warp's state exceeds shared memory for n={n}")
+                raise
         if scratch_limit:
             bg.bg_set_option(ctx, bg.BG_OPT_SCRATCH_LIMIT, scratch_limit)
         if host:
