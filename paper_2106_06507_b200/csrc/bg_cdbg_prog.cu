@@ -64,53 +64,75 @@ struct ProgParams {
 // ---------------------------------------------------------------------------------------------------------
 // 1. classification
 // ---------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
+// Block-level aggregation: sampled colour assignments fall into few classes (92 distinct ones at n = 6), so the
+// class counters are kept in shared memory per block (kPreEvents events) and flushed once; with BLOCK_HIST false
+// (histogram larger than shared memory) the counters are updated in global memory directly.
+constexpr int kPreThreads = 512, kPrePer = 8, kPreEvents = kPreThreads * kPrePer;
+
+template <bool BLOCK_HIST>
+__global__ void __launch_bounds__(kPreThreads)
 cdbg_classify_kernel(int n, long long N, long long num_classes, const signed char* __restrict__ col,
                      const ClassInfo* __restrict__ info, const uint32_t* __restrict__ sortkey,
                      uint32_t* __restrict__ cls, uint64_t* __restrict__ perm, uint32_t* __restrict__ hist) {
-    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= N) return;
-    int code[kMaxN], cnt[kNumCodes];
+    extern __shared__ uint32_t sh_hist[];
+    const int nbins = (int)num_classes + 1;
+    if (BLOCK_HIST) {
+        for (int i = threadIdx.x; i < nbins; i += kPreThreads) sh_hist[i] = 0;
+        __syncthreads();
+    }
+    uint32_t* const h = BLOCK_HIST ? sh_hist : hist;
+    for (int j = 0; j < kPrePer; j++) {
+        const long long e = (long long)blockIdx.x * kPreEvents + j * kPreThreads + threadIdx.x;
+        if (e >= N) break;
+        int code[kMaxN], cnt[kNumCodes];
 #pragma unroll
-    for (int c = 0; c < kNumCodes; c++) cnt[c] = 0;
-    bool ok = true;
-    for (int k = 0; k < n; k++) {
-        const int i = col[(size_t)(2 * k) * N + e] - 1, j = col[(size_t)(2 * k + 1) * N + e] - 1;
-        ok = ok && i >= 0 && i < 3 && j >= 0 && j < 3;
-        code[k] = ok ? 3 * i + j : 0;
-    }
-    if (!ok) {
-        cls[e] = 0xFFFFFFFFu;
-        perm[e] = 0;
-        atomicAdd(&hist[num_classes], 1u);
-        return;
-    }
-    for (int k = 0; k < n; k++) {
+        for (int c = 0; c < kNumCodes; c++) cnt[c] = 0;
+        bool ok = true;
+        for (int k = 0; k < n; k++) {
+            const int i = col[(size_t)(2 * k) * N + e] - 1, jj = col[(size_t)(2 * k + 1) * N + e] - 1;
+            ok = ok && i >= 0 && i < 3 && jj >= 0 && jj < 3;
+            code[k] = ok ? 3 * i + jj : 0;
+        }
+        if (!ok) {
+            cls[e] = 0xFFFFFFFFu;
+            perm[e] = 0;
+            atomicAdd(&h[num_classes], 1u);
+            continue;
+        }
+        for (int k = 0; k < n; k++) {
 #pragma unroll
-        for (int c = 0; c < kNumCodes; c++) cnt[c] += code[k] == c;
-    }
-    unsigned rank = 0;
-    int r = n;
+            for (int c = 0; c < kNumCodes; c++) cnt[c] += code[k] == c;
+        }
+        unsigned rank = 0;
+        int r = n;
 #pragma unroll
-    for (int t = 0; t < kNumCodes - 1; t++) {
-        for (int c = 0; c < cnt[t]; c++) rank += c_mscount[r - c][kNumCodes - 1 - t];
-        r -= cnt[t];
-    }
-    const ClassInfo ci = info[rank];
-    uint64_t pm = 0;
-    if (ci.valid) {
-        int lastk = 0;
-        for (int k = 0; k < n; k++)
-            if (code[k] == ci.closure_code) lastk = k;
-        int pos = 0;
-        for (int c = 0; c < kNumCodes; c++)
+        for (int t = 0; t < kNumCodes - 1; t++) {
+            for (int c = 0; c < cnt[t]; c++) rank += c_mscount[r - c][kNumCodes - 1 - t];
+            r -= cnt[t];
+        }
+        const ClassInfo ci = info[rank];
+        uint64_t pm = 0;
+        if (ci.valid) {
+            int lastk = 0;
             for (int k = 0; k < n; k++)
-                if (code[k] == c && k != lastk) pm |= (uint64_t)k << (4 * pos++);
-        pm |= (uint64_t)lastk << (4 * (n - 1));
+                if (code[k] == ci.closure_code) lastk = k;
+            int pos = 0;
+            for (int c = 0; c < kNumCodes; c++)
+                for (int k = 0; k < n; k++)
+                    if (code[k] == c && k != lastk) pm |= (uint64_t)k << (4 * pos++);
+            pm |= (uint64_t)lastk << (4 * (n - 1));
+        }
+        cls[e] = rank;
+        perm[e] = pm;
+        atomicAdd(&h[sortkey[rank]], 1u);
     }
-    cls[e] = rank;
-    perm[e] = pm;
-    atomicAdd(&hist[sortkey[rank]], 1u);
+    if (BLOCK_HIST) {
+        __syncthreads();
+        for (int i = threadIdx.x; i < nbins; i += kPreThreads) {
+            const uint32_t c = sh_hist[i];
+            if (c) atomicAdd(&hist[i], c);
+        }
+    }
 }
 
 // 2. exclusive scan of hist[0..count) in place (one block)
@@ -149,15 +171,41 @@ __global__ void __launch_bounds__(1024) cdbg_scan_kernel(uint32_t* __restrict__ 
     }
 }
 
-// 3. scatter event ids into class order
-__global__ void __launch_bounds__(256)
+// 3. scatter event ids into class order (each block reserves one range per class it holds)
+template <bool BLOCK_HIST>
+__global__ void __launch_bounds__(kPreThreads)
 cdbg_scatter_kernel(long long N, long long num_classes, const uint32_t* __restrict__ cls,
                     const uint32_t* __restrict__ sortkey, uint32_t* __restrict__ cursor, uint32_t* __restrict__ order) {
-    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= N) return;
-    const uint32_t c = cls[e];
-    const uint32_t key = c == 0xFFFFFFFFu ? (uint32_t)num_classes : sortkey[c];
-    order[atomicAdd(&cursor[key], 1u)] = (uint32_t)e;
+    extern __shared__ uint32_t sh_hist[];
+    const int nbins = (int)num_classes + 1;
+    uint32_t key[kPrePer], rank[kPrePer];
+    if (BLOCK_HIST) {
+        for (int i = threadIdx.x; i < nbins; i += kPreThreads) sh_hist[i] = 0;
+        __syncthreads();
+    }
+#pragma unroll
+    for (int j = 0; j < kPrePer; j++) {
+        const long long e = (long long)blockIdx.x * kPreEvents + j * kPreThreads + threadIdx.x;
+        key[j] = 0xFFFFFFFFu;
+        if (e < N) {
+            const uint32_t c = cls[e];
+            key[j] = c == 0xFFFFFFFFu ? (uint32_t)num_classes : sortkey[c];
+            if (BLOCK_HIST) rank[j] = atomicAdd(&sh_hist[key[j]], 1u);
+            else order[atomicAdd(&cursor[key[j]], 1u)] = (uint32_t)e;
+        }
+    }
+    if (!BLOCK_HIST) return;
+    __syncthreads();
+    for (int i = threadIdx.x; i < nbins; i += kPreThreads) {
+        const uint32_t c = sh_hist[i];
+        if (c) sh_hist[i] = atomicAdd(&cursor[i], c);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < kPrePer; j++) {
+        const long long e = (long long)blockIdx.x * kPreEvents + j * kPreThreads + threadIdx.x;
+        if (key[j] != 0xFFFFFFFFu) order[sh_hist[key[j]] + rank[j]] = (uint32_t)e;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -260,15 +308,39 @@ __global__ void __launch_bounds__(128) cdbg_prog_kernel(const ProgParams p) {
                         } else {
                             const double f = kInvSqrt2 / mdot(Pt, Pt);
 #pragma unroll
-                            for (int c = 0; c < 4; c++) sts<EPW>(S, offDst + c, f * acc[c]);
+                            for (int c = 0; c < 4; c++) acc[c] = f * acc[c];
 #pragma unroll
-                            for (int c = 0; c < 6; c++) sts<EPW>(S, offDst + 4 + c, kInvSqrt2 * tacc[c]);
+                            for (int c = 0; c < 6; c++) tacc[c] = kInvSqrt2 * tacc[c];
+                            if (!(flags & OPF_NOSTORE)) {
+#pragma unroll
+                                for (int c = 0; c < 4; c++) sts<EPW>(S, offDst + c, acc[c]);
+#pragma unroll
+                                for (int c = 0; c < 6; c++) sts<EPW>(S, offDst + 4 + c, tacc[c]);
+                            }
                             if (flags & OPF_STOREP) {
                                 sts<EPW>(S, offPt, mk(Pt[0], Pt[1]));
                                 sts<EPW>(S, offPt + 1, mk(Pt[2], Pt[3]));
                             }
                         }
                     }
+                } else if (flags & OPF_FUSED) {
+                    // closure vertex X(eps_k, J(pi)) . eps_n with J(pi), T(pi) still in acc / tacc, P(pi) in Pt
+                    cx a[4], x[4], en[4];
+                    double P1[4];
+#pragma unroll
+                    for (int c = 0; c < 4; c++) { a[c] = lds<EPW>(S, offA + c); x[c] = mk(0.0, 0.0); }
+                    {
+                        const cx p01 = lds<EPW>(S, offP1), p23 = lds<EPW>(S, offP1 + 1);
+                        P1[0] = p01.re; P1[1] = p01.im; P1[2] = p23.re; P1[3] = p23.im;
+                    }
+                    const double sign = (flags & OPF_NEG) ? -1.0 : 1.0;
+                    v3_acc(x, P1, Pt, a, acc, sign);
+                    tcontract_acc(x, tacc, a, sign);
+#pragma unroll
+                    for (int c = 0; c < 4; c++) en[c] = lds<EPW>(S, offDst + c);
+                    const cx d = mdot(en, x);
+                    amp.re = fma(kInvSqrt2, d.re, amp.re);
+                    amp.im = fma(kInvSqrt2, d.im, amp.im);
                 } else if (flags & OPF_EXT) {
                     const int k = (int)raw.w;
                     const int orig = (int)((perm >> (4 * k)) & 0xF);
@@ -426,10 +498,25 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     const int nbins = (int)t->num_classes + 1;
     cudaError_t err = cudaMemsetAsync(hist, 0, sizeof(uint32_t) * nbins, s);
     if (err != cudaSuccess) return err;
-    const unsigned eb = (unsigned)((N + 255) / 256);
-    cdbg_classify_kernel<<<eb, 256, 0, s>>>(t->n, N, t->num_classes, col, t->d_info, t->d_sortkey, cls, perm, hist);
-    cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins);
-    cdbg_scatter_kernel<<<eb, 256, 0, s>>>(N, t->num_classes, cls, t->d_sortkey, hist, order);
+    const unsigned eb = (unsigned)((N + kPreEvents - 1) / kPreEvents);
+    const size_t hist_smem = sizeof(uint32_t) * nbins;
+    if (hist_smem <= 160 * 1024) {
+        static bool configured = false;
+        if (!configured) {
+            cudaFuncSetAttribute(cdbg_classify_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+            cudaFuncSetAttribute(cdbg_scatter_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+            configured = true;
+        }
+        cdbg_classify_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
+                                                                      t->d_sortkey, cls, perm, hist);
+        cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins);
+        cdbg_scatter_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(N, t->num_classes, cls, t->d_sortkey, hist, order);
+    } else {
+        cdbg_classify_kernel<false><<<eb, kPreThreads, 0, s>>>(t->n, N, t->num_classes, col, t->d_info, t->d_sortkey,
+                                                               cls, perm, hist);
+        cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins);
+        cdbg_scatter_kernel<false><<<eb, kPreThreads, 0, s>>>(N, t->num_classes, cls, t->d_sortkey, hist, order);
+    }
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     ProgParams p;
     p.n = t->n; p.N = N; p.mom = mom; p.hel = hel; p.out = out;

@@ -41,8 +41,12 @@ struct VOp {
 
 struct Target {
     int pi, h, g;
-    bool store_p;   // first live entry of its subset: its LAST op also stores P(pi)
+    bool store_p = false;   // its LAST op also stores P(pi) (one entry per subset whose momentum is read later)
+    bool used = false;      // read by a later vertex (dead-code elimination)
+    bool fused = false;     // |pi| = n-2: not stored; its closure contribution is taken from registers
+    VOp fuse;               // the closure vertex X(eps_k, this) of a fused target (pb = this entry)
     std::vector<VOp> ops;
+    int slot() const { return h == g ? h : 0; }
 };
 
 inline int popc(int x) { return __builtin_popcount((unsigned)x); }
@@ -60,22 +64,12 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
     }
     out.closure_code = code[n - 1];
 
+    // ---- phase 1: which entries of which subsets are non-zero, and the vertex evaluations that feed them ----
     std::vector<uint8_t> type(nsub, 0x40);
-    std::vector<int> off(nsub * 3, -1), poff(nsub, -1);
-    int next = 0;
-    // external currents (4 cx) and the closure polarisation
-    for (int k = 0; k < m; k++) {
-        const int pi = 1 << k;
-        const bool diag = ci[k] == cj[k];
-        type[pi] = diag ? (uint8_t)(0x80u | (1u << ci[k])) : (uint8_t)((ci[k] << 2) | cj[k]);
-        off[pi * 3 + (diag ? ci[k] : 0)] = next;
-        next += 4;
-    }
-    const int off_epsn = next;
-    next += 4;
-    for (int k = 0; k < m; k++) { poff[1 << k] = next; next += 2; }
-
+    for (int k = 0; k < m; k++)
+        type[1 << k] = ci[k] == cj[k] ? (uint8_t)(0x80u | (1u << ci[k])) : (uint8_t)((ci[k] << 2) | cj[k]);
     std::vector<std::vector<Target>> levels(m + 1);   // by popcount
+    std::vector<int> tindex(nsub * 3, -1);            // (subset, slot) -> index in its level
     for (int pi = 3; pi <= full; pi++) {
         if ((pi & (pi - 1)) == 0) continue;
         const int low = pi & -pi, rest = pi ^ low;
@@ -133,12 +127,8 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
                 if (sub == 0) break;
             }
             if (t.ops.empty()) continue;
-            t.store_p = livemask == 0 && pi != full;
             livemask |= diag ? (1u << h) : 1u;
-            if (pi != full) {
-                off[pi * 3 + (h == g ? h : 0)] = next;
-                next += 10;
-            }
+            tindex[pi * 3 + t.slot()] = (int)levels[popc(pi)].size();
             levels[popc(pi)].push_back(std::move(t));
         }
         if (pi != full) {
@@ -146,13 +136,70 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
             if (livemask) ty = diag ? (uint8_t)(0x80u | livemask) : (uint8_t)((cand_h[0] << 2) | cand_g[0]);
             type[pi] = ty;
         }
-        if (livemask) { poff[pi] = next; next += 2; }
     }
     if (levels[m].empty()) return;   // no closure: amplitude vanishes identically
     out.valid = true;
+    // ---- phase 2: closure vertices X(eps_k, J(pi)) with |pi| = n-2 are evaluated straight from the registers
+    // that hold the just-finished J(pi), T(pi) ("fused": those currents are never stored), and entries that no
+    // later vertex reads are dropped ----
+    {
+        Target& clo = levels[m][0];
+        clo.used = true;
+        if (m - 1 >= 2) {
+            std::vector<VOp> keep;
+            for (auto& v : clo.ops) {
+                if (popc(v.pa) == 1 && popc(v.pb) == m - 1) {
+                    Target& t = levels[m - 1][tindex[v.pb * 3 + v.sb]];
+                    if (!t.fused) {   // at most one closure vertex reads a given entry
+                        t.fused = true;
+                        t.fuse = v;
+                        t.used = true;
+                        continue;
+                    }
+                }
+                keep.push_back(v);
+            }
+            clo.ops.swap(keep);
+        }
+        for (int pc = m; pc >= 2; pc--)
+            for (auto& t : levels[pc]) {
+                if (!t.used) continue;
+                for (auto& v : t.ops) {
+                    if (popc(v.pa) >= 2) levels[popc(v.pa)][tindex[v.pa * 3 + v.sa]].used = true;
+                    if (popc(v.pb) >= 2) levels[popc(v.pb)][tindex[v.pb * 3 + v.sb]].used = true;
+                }
+            }
+        for (int pc = 2; pc < m; pc++) {
+            std::vector<Target> keep;
+            for (auto& t : levels[pc])
+                if (t.used) keep.push_back(std::move(t));
+            levels[pc].swap(keep);
+        }
+    }
+
+    // ---- phase 3: state layout (units of one complex double) ----
+    std::vector<int> off(nsub * 3, -1), poff(nsub, -1);
+    std::vector<char> need_p(nsub, 0);
+    for (int pc = 2; pc <= m; pc++)
+        for (auto& t : levels[pc])
+            for (auto& v : t.ops) { need_p[v.pa] = 1; need_p[v.pb] = 1; }
+    int next = 0;
+    for (int k = 0; k < m; k++) {
+        off[(1 << k) * 3 + (ci[k] == cj[k] ? ci[k] : 0)] = next;
+        next += 4;
+    }
+    const int off_epsn = next;
+    next += 4;
+    for (int k = 0; k < m; k++) { poff[1 << k] = next; next += 2; }
+    for (int pc = 2; pc < m; pc++)
+        for (auto& t : levels[pc]) {
+            if (!t.fused) { off[t.pi * 3 + t.slot()] = next; next += 10; }
+            if (need_p[t.pi] && poff[t.pi] < 0) { poff[t.pi] = next; next += 2; t.store_p = true; }
+        }
     out.state_cx = next;
     out.level_steps.assign(m, 0);
 
+    // ---- phase 4: deal the work of every level over the G lanes and emit ----
     auto emit_level = [&](int lvl, std::vector<std::vector<ProgOp>>& lanes) {
         size_t steps = 0;
         for (auto& l : lanes) steps = std::max(steps, l.size());
@@ -164,11 +211,8 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
         out.total_steps += (int)steps;
     };
 
-    // level 0: external currents and momenta, dealt over the lanes
-    {
+    {   // level 0: external currents and momenta
         std::vector<std::vector<ProgOp>> lanes(G);
-        std::vector<int> load(G, 0);
-        auto least = [&]() { return (int)(std::min_element(load.begin(), load.end()) - load.begin()); };
         for (int k = 0; k < n; k++) {
             ProgOp o;
             std::memset(&o, 0, sizeof(o));
@@ -182,9 +226,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
                 o.offDst = (uint16_t)off_epsn;
                 o.offPt = 0xFFFF;
             }
-            const int l = least();
-            lanes[l].push_back(o);
-            load[l] += 8;
+            lanes[k % G].push_back(o);
         }
         emit_level(0, lanes);
     }
@@ -195,43 +237,57 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
         o.offA = (uint16_t)off[v.pa * 3 + v.sa];
         o.offB = (uint16_t)off[v.pb * 3 + v.sb];
         o.offP1 = (uint16_t)poff[v.pa];
-        o.offPt = (uint16_t)poff[t.pi];
         o.extra = (uint32_t)poff[v.pb];
-        o.offDst = t.pi == full ? (uint16_t)off_epsn : (uint16_t)off[t.pi * 3 + (t.h == t.g ? t.h : 0)];
+        o.offPt = t.store_p ? (uint16_t)poff[t.pi] : (uint16_t)0xFFFF;
+        o.offDst = t.pi == full ? (uint16_t)off_epsn : (t.fused ? (uint16_t)0xFFFF : (uint16_t)off[t.pi * 3 + t.slot()]);
         o.flags = OPF_VALID | (v.neg ? OPF_NEG : 0) | (popc(v.pa) >= 2 ? OPF_TENA : 0) |
-                  (popc(v.pb) >= 2 ? OPF_TENB : 0) | (t.pi == full ? OPF_CLOSURE : 0) | (t.store_p ? OPF_STOREP : 0);
+                  (popc(v.pb) >= 2 ? OPF_TENB : 0) | (t.pi == full ? OPF_CLOSURE : 0);
         return o;
+    };
+    auto push_target = [&](std::vector<ProgOp>& lane, const Target& t) {
+        for (size_t i = 0; i < t.ops.size(); i++) {
+            ProgOp o = make_op(t, t.ops[i]);
+            if (i == 0) o.flags |= OPF_FIRST;
+            if (i + 1 == t.ops.size())
+                o.flags |= OPF_LAST | (t.store_p ? OPF_STOREP : 0) | (t.fused ? OPF_NOSTORE : 0);
+            lane.push_back(o);
+            out.n_vertex_ops++;
+        }
+        if (t.fused) {
+            ProgOp o;
+            std::memset(&o, 0, sizeof(o));
+            o.offA = (uint16_t)off[t.fuse.pa * 3 + t.fuse.sa];
+            o.offP1 = (uint16_t)poff[t.fuse.pa];
+            o.offDst = (uint16_t)off_epsn;
+            o.flags = OPF_FUSED | (t.fuse.neg ? OPF_NEG : 0);
+            lane.push_back(o);
+            out.n_vertex_ops++;
+        }
     };
 
     for (int pc = 2; pc <= m; pc++) {
         std::vector<std::vector<ProgOp>> lanes(G);
         auto& tg = levels[pc];
         if (pc == m) {
-            // closure: one target, its ops dealt round-robin; every lane contracts its partial sum with eps_n
+            // closure: one target, its remaining vertices dealt round-robin; every lane contracts its partial
+            // sum with eps_n and the lanes' amplitudes are added at the end
             const Target& t = tg[0];
-            // ops with both tensors first so that lanes hit the same code path together
             std::vector<VOp> ops = t.ops;
-            std::stable_sort(ops.begin(), ops.end(), [](const VOp& a, const VOp& b) { return popc(a.pa) > popc(b.pa); });
-            for (size_t i = 0; i < ops.size(); i++) lanes[i % G].push_back(make_op(t, ops[i]));
+            for (size_t i = 0; i < ops.size(); i++) {
+                lanes[i % G].push_back(make_op(t, ops[i]));
+                out.n_vertex_ops++;
+            }
+            for (auto& l : lanes)
+                if (!l.empty()) { l.front().flags |= OPF_FIRST; l.back().flags |= OPF_LAST; }
         } else {
             std::vector<int> order(tg.size()), load(G, 0);
             for (size_t i = 0; i < tg.size(); i++) order[i] = (int)i;
-            std::stable_sort(order.begin(), order.end(),
-                             [&](int a, int b) { return tg[a].ops.size() > tg[b].ops.size(); });
+            auto cost = [&](int a) { return (int)tg[a].ops.size() + (tg[a].fused ? 1 : 0); };
+            std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return cost(a) > cost(b); });
             for (int idx : order) {
                 const int l = (int)(std::min_element(load.begin(), load.end()) - load.begin());
-                for (auto& v : tg[idx].ops) lanes[l].push_back(make_op(tg[idx], v));
-                load[l] += (int)tg[idx].ops.size();
-            }
-        }
-        // mark first / last op of each target run in every lane
-        for (auto& l : lanes) {
-            for (size_t i = 0; i < l.size(); i++) {
-                const bool first = i == 0 || l[i - 1].offDst != l[i].offDst;
-                const bool last = i + 1 == l.size() || l[i + 1].offDst != l[i].offDst;
-                if (first) l[i].flags |= OPF_FIRST;
-                if (last) l[i].flags |= OPF_LAST;
-                out.n_vertex_ops++;
+                push_target(lanes[l], tg[idx]);
+                load[l] += cost(idx);
             }
         }
         emit_level(pc - 1, lanes);

@@ -39,6 +39,8 @@ enum : uint16_t {
     OPF_LAST = 32,     // last op of a target: apply 1/sqrt2 (and 1/P^2), store vector + tensor current and P
     OPF_CLOSURE = 64,  // target is the full set: contract with eps_n instead of storing (Eq. 22)
     OPF_STOREP = 256,  // (with LAST) also store P(target) at offPt: set on one entry per subset
+    OPF_FUSED = 512,   // closure vertex X(eps_k at offA, b = the current just finished in registers) . eps_n
+    OPF_NOSTORE = 1024,// (with LAST) the finished current stays in registers only (a FUSED op follows)
     OPF_EXT = 128      // setup: external current of gluon `extra` -> offDst, its momentum -> offPt
 };
 
