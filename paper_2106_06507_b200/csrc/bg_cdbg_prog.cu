@@ -34,10 +34,18 @@ struct ClassInfo {            // 32 bytes
 };
 static_assert(sizeof(ClassInfo) == 32, "ClassInfo layout");
 
+constexpr int kTiers = 4;     // classes are grouped by state size so that small ones get more warps per SM
+
+struct TierInfo {
+    int first_key[kTiers + 1];   // first position (in grouping order) of each tier; [kTiers] = number of classes
+    int slab_cx[kTiers];         // state block (complex doubles per event) the tier's launch reserves
+};
+
 struct ProgTable {
     int n, G;
     long long num_classes;
     int max_state_cx;
+    TierInfo tiers;
     double mean_steps;
     ClassInfo* d_info;
     uint32_t* d_sortkey;      // class id -> position in the order the events are grouped by
@@ -58,6 +66,8 @@ struct ProgParams {
     const uint32_t* cls;       // [N] class id per event (0xFFFFFFFF: colour codes out of range)
     const uint64_t* perm;      // [N] canonical order: nibble k = original index of canonical gluon k
     const uint32_t* order;     // [N] event ids grouped by class
+    const uint32_t* bounds;    // [kTiers + 1] positions in `order` where the tiers start (bounds[kTiers] = N)
+    int tier;
     int slab_cx;               // complex doubles of state per event in the slab
 };
 
@@ -136,7 +146,8 @@ cdbg_classify_kernel(int n, long long N, long long num_classes, const signed cha
 }
 
 // 2. exclusive scan of hist[0..count) in place (one block)
-__global__ void __launch_bounds__(1024) cdbg_scan_kernel(uint32_t* __restrict__ hist, int count) {
+__global__ void __launch_bounds__(1024)
+cdbg_scan_kernel(uint32_t* __restrict__ hist, int count, TierInfo tiers, uint32_t* __restrict__ bounds, uint32_t N) {
     __shared__ uint32_t warp_tot[32];
     __shared__ uint32_t carry;
     if (threadIdx.x == 0) carry = 0;
@@ -169,6 +180,7 @@ __global__ void __launch_bounds__(1024) cdbg_scan_kernel(uint32_t* __restrict__ 
         if (threadIdx.x == 1023) carry = before + v;
         __syncthreads();
     }
+    if (threadIdx.x <= kTiers) bounds[threadIdx.x] = threadIdx.x == kTiers ? N : hist[tiers.first_key[threadIdx.x]];
 }
 
 // 3. scatter event ids into class order (each block reserves one range per class it holds)
@@ -222,20 +234,20 @@ __device__ __forceinline__ void sts(double2* S, int o, cx v) {
 }
 
 template <int G>
-__global__ void __launch_bounds__(128) cdbg_prog_kernel(const ProgParams p) {
+__global__ void __launch_bounds__(32) cdbg_prog_kernel(const ProgParams p) {
     constexpr int EPW = 32 / G;
     extern __shared__ double2 smem[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int lane = threadIdx.x;          // one warp per block
     const int q = lane % EPW, g = lane / EPW;
-    double2* S = smem + (size_t)warp * p.slab_cx * EPW + q;
-    const long long ntasks = (p.N + EPW - 1) / EPW;
+    double2* S = smem + q;
+    const long long first = p.bounds[p.tier], end = p.bounds[p.tier + 1];
+    const long long ntasks = (end - first + EPW - 1) / EPW;
     const int nlev = p.n - 1;
     const long long N = p.N;
 
-    const int wpb = blockDim.x >> 5;
-    for (long long task = (long long)blockIdx.x * wpb + warp; task < ntasks; task += (long long)gridDim.x * wpb) {
-        const long long idx = task * EPW + q;
-        const bool have = idx < N;
+    for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
+        const long long idx = first + task * EPW + q;
+        const bool have = idx < end;
         const long long e = have ? (long long)p.order[idx] : 0;
         const uint32_t cls = have ? p.cls[e] : 0xFFFFFFFFu;
         const ClassInfo* ci = p.info + (cls == 0xFFFFFFFFu ? 0 : cls);
@@ -417,14 +429,30 @@ int prog_table_create(int n, int G, ProgTable** out) {
     // grouping order: longest programs first (the tail of the grid then runs the short ones), invalid last
     std::vector<uint32_t> by(nc), sortkey(nc);
     std::iota(by.begin(), by.end(), 0u);
-    std::stable_sort(by.begin(), by.end(), [&](uint32_t a, uint32_t b) { return steps[a] > steps[b]; });
+    // tiers by state size (tier 0 = the largest blocks); inside a tier the longest programs come first, classes
+    // whose amplitude vanishes (no state, no steps) end up last
+    TierInfo tiers;
+    static const double kTierFrac[kTiers] = {1.0, 0.8, 0.64, 0.5};
+    for (int k = 0; k < kTiers; k++) tiers.slab_cx[k] = std::max(16, (int)(max_state * kTierFrac[k] + 0.999));
+    std::vector<int> tier_of(nc);
+    for (long long r = 0; r < nc; r++) {
+        int k = 0;
+        while (k + 1 < kTiers && (int)info[r].state_cx <= tiers.slab_cx[k + 1]) k++;
+        tier_of[r] = k;
+    }
+    std::stable_sort(by.begin(), by.end(), [&](uint32_t a, uint32_t b) {
+        return tier_of[a] != tier_of[b] ? tier_of[a] < tier_of[b] : steps[a] > steps[b];
+    });
     for (long long i = 0; i < nc; i++) sortkey[by[i]] = (uint32_t)i;
+    for (int k = 0; k <= kTiers; k++) tiers.first_key[k] = (int)nc;
+    for (long long i = nc - 1; i >= 0; i--) tiers.first_key[tier_of[by[i]]] = (int)i;
+    for (int k = kTiers - 1; k >= 0; k--) tiers.first_key[k] = std::min(tiers.first_key[k], tiers.first_key[k + 1]);
 
     if ((size_t)(32 / G) * max_state * 16 > 227 * 1024) return BG_EUNSUPPORTED;   // one warp's slab must fit
     ProgTable* t = new (std::nothrow) ProgTable();
     if (!t) return BG_ENOMEM;
     std::memset(t, 0, sizeof(*t));
-    t->n = n; t->G = G; t->num_classes = nc; t->max_state_cx = max_state;
+    t->n = n; t->G = G; t->num_classes = nc; t->max_state_cx = max_state; t->tiers = tiers;
     {   // one spare row of no-ops: the interpreter prefetches one step ahead
         ProgOp nop;
         std::memset(&nop, 0, sizeof(nop));
@@ -467,24 +495,27 @@ size_t prog_scratch_bytes(const ProgTable* t, long long N) {
 }
 
 template <int G>
-static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p) {
+static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched) {
     constexpr int EPW = 32 / G;
-    const size_t per_warp = (size_t)EPW * p.slab_cx * 16;
-    if (per_warp > 227 * 1024) return cudaErrorInvalidValue;
-    const int wpb = (int)std::max<size_t>(1, std::min<size_t>(4, (227 * 1024) / per_warp));
-    const size_t smem = per_warp * wpb;
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    int per_sm = (int)std::min<size_t>(16, (227 * 1024) / (smem + 1024));
-    if (per_sm < 1) per_sm = 1;
-    const long long ntasks = (p.N + EPW - 1) / EPW;
-    const long long want = (ntasks + wpb - 1) / wpb;
-    const unsigned blocks = (unsigned)std::max<long long>(1, std::min<long long>(want, (long long)sm_count * per_sm));
-    cdbg_prog_kernel<G><<<blocks, 32 * wpb, smem, s>>>(p);
+    const long long max_tasks = (p.N + EPW - 1) / EPW + kTiers;
+    for (int k = 0; k < kTiers; k++) {
+        if (t->tiers.first_key[k] == t->tiers.first_key[k + 1] && k + 1 < kTiers) continue;   // no class in this tier
+        p.tier = k;
+        p.slab_cx = t->tiers.slab_cx[k];
+        const size_t smem = (size_t)EPW * p.slab_cx * 16;     // one warp per block
+        if (smem > 227 * 1024) return cudaErrorInvalidValue;
+        // resident warps per SM: shared memory (1 KB reserved per block), and 65536 / (32 x 152) registers
+        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(13, (228 * 1024) / (smem + 1024)));
+        const unsigned blocks = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
+        cdbg_prog_kernel<G><<<blocks, 32, smem, s>>>(p);
+        ++*launched;
+    }
     return cudaGetLastError();
 }
 
@@ -495,6 +526,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     uint32_t* order = cls + N;
     uint64_t* perm = (uint64_t*)(order + N);   // 2N u32 before it: 8-byte aligned
     uint32_t* hist = (uint32_t*)(perm + N);
+    uint32_t* bounds = hist + ((size_t)t->num_classes + 1);
     const int nbins = (int)t->num_classes + 1;
     cudaError_t err = cudaMemsetAsync(hist, 0, sizeof(uint32_t) * nbins, s);
     if (err != cudaSuccess) return err;
@@ -509,30 +541,32 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         }
         cdbg_classify_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
                                                                       t->d_sortkey, cls, perm, hist);
-        cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins);
+        cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins, t->tiers, bounds, (uint32_t)N);
         cdbg_scatter_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(N, t->num_classes, cls, t->d_sortkey, hist, order);
     } else {
         cdbg_classify_kernel<false><<<eb, kPreThreads, 0, s>>>(t->n, N, t->num_classes, col, t->d_info, t->d_sortkey,
                                                                cls, perm, hist);
-        cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins);
+        cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins, t->tiers, bounds, (uint32_t)N);
         cdbg_scatter_kernel<false><<<eb, kPreThreads, 0, s>>>(N, t->num_classes, cls, t->d_sortkey, hist, order);
     }
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     ProgParams p;
     p.n = t->n; p.N = N; p.mom = mom; p.hel = hel; p.out = out;
     p.info = t->d_info; p.ops = t->d_ops; p.cls = cls; p.perm = perm; p.order = order;
+    p.bounds = bounds;
+    p.tier = 0;
     p.slab_cx = t->max_state_cx;
+    *launches = 3;
     if (ev0) cudaEventRecord(ev0, s);
     switch (t->G) {
-        case 1: err = launch_interp<1>(s, t, sm_count, p); break;
-        case 2: err = launch_interp<2>(s, t, sm_count, p); break;
-        case 4: err = launch_interp<4>(s, t, sm_count, p); break;
-        case 8: err = launch_interp<8>(s, t, sm_count, p); break;
-        case 16: err = launch_interp<16>(s, t, sm_count, p); break;
-        default: err = launch_interp<32>(s, t, sm_count, p); break;
+        case 1: err = launch_interp<1>(s, t, sm_count, p, launches); break;
+        case 2: err = launch_interp<2>(s, t, sm_count, p, launches); break;
+        case 4: err = launch_interp<4>(s, t, sm_count, p, launches); break;
+        case 8: err = launch_interp<8>(s, t, sm_count, p, launches); break;
+        case 16: err = launch_interp<16>(s, t, sm_count, p, launches); break;
+        default: err = launch_interp<32>(s, t, sm_count, p, launches); break;
     }
     if (ev1) cudaEventRecord(ev1, s);
-    *launches = 4;
     return err;
 }
 
