@@ -176,12 +176,17 @@ int bg_init(bg_ctx** out, int n, int mode) {
             cudaFree(c->dC); std::free(c->hC); delete c; return BG_ECUDA;
         }
     }
+    if ((mode & BG_REC_COBG) && bg::cobg_shared_supported(n)) {
+        const int rc = bg::cobg_table_create(n, &c->cobg);
+        if (rc != BG_OK) { cudaFree(c->dC); std::free(c->hC); delete c; return rc; }
+    }
     if (mode == BG_CDBG_GIVEN && n <= kProgMaxN) {
         const int rc = bg::prog_table_create(n, auto_lanes(n), &c->prog);
         if (rc != BG_OK) { delete c; return rc; }
     }
     if (cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking) != cudaSuccess) {
         bg::prog_table_destroy(c->prog);
+        bg::cobg_table_destroy(c->cobg);
         if (c->dC) cudaFree(c->dC);
         std::free(c->hC);
         delete c;
@@ -198,6 +203,7 @@ int bg_destroy(bg_ctx* c) {
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     bg::prog_table_destroy(c->prog);
+    bg::cobg_table_destroy(c->cobg);
     if (c->dC) cudaFree(c->dC);
     if (c->scratch) cudaFree(c->scratch);
     if (c->d_mom) cudaFree(c->d_mom);
@@ -232,6 +238,7 @@ size_t bg_scratch_bytes(const bg_ctx* c, long long N) {
 
 size_t bg_current_bytes_per_event(const bg_ctx* c) {
     if (!c) return 0;
+    if ((c->mode & BG_REC_COBG) && c->cobg && c->kernel_opt != 1) return bg::cobg_shared_current_bytes(c->cobg);
     if (c->mode & BG_REC_COBG) return (size_t)(c->n - 1) * c->n / 2 * 64;   // one ordering's current table
     if (use_prog(c)) return bg::prog_state_bytes(c->prog);
     return ((size_t)1 << (c->n - 1)) * 3 * 160;
@@ -279,7 +286,7 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
     switch (key) {
         case BG_OPT_KERNEL:
             if (value < 0 || value > 2) return BG_EINVAL;
-            if (value == 2 && !c->prog) return BG_EUNSUPPORTED;
+            if (value == 2 && !c->prog && !c->cobg) return BG_EUNSUPPORTED;
             c->kernel_opt = (int)value;
             return BG_OK;
         case BG_OPT_LANES: {
@@ -352,10 +359,15 @@ int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const 
     c->timed = c->timing != 0;
     if (c->mode & BG_REC_COBG) {
         if (ev0) cudaEventRecord(ev0, s);
-        err = bg::cobg_generic_launch(s, c->n, helsum, c->nperm, c->dC, N, mom, hel, out);
+        if (c->cobg && c->kernel_opt != 1) {
+            err = bg::cobg_shared_launch(s, c->cobg, helsum, c->dC, N, mom, hel, out);
+            c->last_kernel = "cobg_shared_kernel";
+        } else {
+            err = bg::cobg_generic_launch(s, c->n, helsum, c->nperm, c->dC, N, mom, hel, out);
+            c->last_kernel = "cobg_generic_kernel";
+        }
         if (ev1) cudaEventRecord(ev1, s);
         c->last_launches = 1;
-        c->last_kernel = "cobg_generic_kernel";
     } else if (use_prog(c)) {
         int rc = ensure_scratch(c, N);
         if (rc != BG_OK) return rc;

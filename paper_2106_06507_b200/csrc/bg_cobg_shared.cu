@@ -1,0 +1,372 @@
+// Colour-ordered recursion (COBG, Eq. 20-22) for all (n-2)! orderings A(1, sigma, n) of one
+// event, followed by the full-colour quadratic form of Eq. 16 (L119-127) - the performance path of BASELINE
+// configs 1 and 3.
+//
+// The (n-2)! orderings of one event share their short sub-currents: J(g_i .. g_j) depends only on the ordered
+// sequence of gluons, not on the ordering it sits in (651 distinct sequences against 120 x 21 = 2520 ranges at
+// n = 7).  A group of TPE threads works on one event:
+//   * "shared" currents - sequences of length <= n-3 - are computed once, one thread per sequence, level by level,
+//     into shared memory (291 x 64 B = 18.2 KB at n = 7);
+//   * the two currents of length n-2 and the final one of length n-1 of every ordering are used by that ordering
+//     only, so thread sigma computes them in registers (13 V3 + 22 V4 at n = 7) from the shared ones and closes
+//     with eps_n (Eq. 22: the last current keeps no propagator);
+//   * A_sigma goes to shared memory and thread sigma takes row sigma of  w = a_r^T C a_r + a_i^T C a_i  (C of
+//     Eq. 17 is real and symmetric, so consecutive threads read consecutive addresses of a column).
+// The amplitudes never leave the SM.  Which sequence lives in which slot is tabulated on the host at bg_init
+// (integer bookkeeping, same for every event).
+#include <algorithm>
+#include <cstring>
+#include <map>
+#include <new>
+#include <numeric>
+#include <vector>
+
+#include "bg_internal.h"
+#include "bg_math.cuh"
+
+namespace bg {
+
+constexpr int kCobgMaxM = 6;   // n - 1 <= 6: n = 4..7
+
+struct CobgTable {
+    int n, np, nslots;
+    int level_begin[kCobgMaxM + 2];   // level L (sequence length) occupies lower[level_begin[L] .. level_begin[L+1])
+    uint16_t* d_slot;                 // [np][m][m] slot of range (i..j) of ordering sigma; 0xFFFF if longer than n-3
+    uint8_t* d_ord;                   // [np][m] gluon at position i of (1, sigma)  (0-based labels, position 0 = gluon 0)
+    uint32_t* d_lower;                // representatives of the shared sequences: sigma << 8 | i << 4 | j
+};
+
+struct CobgParams {
+    int n, np, nslots, helsum;
+    long long N;
+    const double* mom;
+    const signed char* hel;
+    const double* C;
+    double* out;
+    const uint16_t* slot;
+    const uint8_t* ord;
+    const uint32_t* lower;
+    int level_begin[kCobgMaxM + 2];
+};
+
+
+// ---------------------------------------------------------------------------------------------------------
+// device side
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void lds_cur(const double* cur, int slot, cx* v) {
+    const double2* p = reinterpret_cast<const double2*>(cur + (size_t)slot * 8);
+#pragma unroll
+    for (int c = 0; c < 4; c++) { const double2 t = p[c]; v[c] = mk(t.x, t.y); }
+}
+__device__ __forceinline__ void sts_cur(double* cur, int slot, const cx* v) {
+    double2* p = reinterpret_cast<double2*>(cur + (size_t)slot * 8);
+#pragma unroll
+    for (int c = 0; c < 4; c++) p[c] = make_double2(v[c].re, v[c].im);
+}
+
+// Per-ordering view used by the register-resident top of the recursion: sl[i*M+j] = shared slot of range (i..j),
+// pm[k] = OR of the gluon bits at positions 0..k-1, JA / JB = the two currents of length M-1 (positions 1..M-1 and
+// 0..M-2) once they exist.
+template <int NG>
+struct TopView {
+    static constexpr int M = NG - 1, LS = NG - 3;
+    const double* cur;
+    const double* P;
+    uint16_t sl[M * M];
+    unsigned pm[M + 1];
+    cx JA[4], JB[4];
+
+    template <int I, int J>
+    __device__ __forceinline__ void fetch(cx* v) const {
+        if (J - I + 1 <= LS) {
+            lds_cur(cur, sl[I * M + J], v);
+        } else if (I == 0) {
+#pragma unroll
+            for (int c = 0; c < 4; c++) v[c] = JB[c];
+        } else {
+#pragma unroll
+            for (int c = 0; c < 4; c++) v[c] = JA[c];
+        }
+    }
+    template <int I, int J>
+    __device__ __forceinline__ const double* mom() const { return P + 4 * (pm[J + 1] ^ pm[I]); }
+
+    template <int I, int K, int L, int J>
+    __device__ __forceinline__ void v4_inner(cx* s4, const cx* a) const {
+        if constexpr (L < J) {
+            cx b[4], c[4];
+            fetch<K + 1, L>(b);
+            fetch<L + 1, J>(c);
+            v4_acc(s4, a, b, c);
+            v4_inner<I, K, L + 1, J>(s4, a);
+        }
+    }
+    template <int I, int K, int J>
+    __device__ __forceinline__ void splits(cx* s3, cx* s4) const {
+        if constexpr (K < J) {
+            cx a[4], b[4];
+            fetch<I, K>(a);
+            fetch<K + 1, J>(b);
+            v3_acc(s3, mom<I, K>(), mom<K + 1, J>(), a, b, 1.0);
+            v4_inner<I, K, K + 1, J>(s4, a);
+            splits<I, K + 1, J>(s3, s4);
+        }
+    }
+    // Eq. 20 for the range (I..J); PROP = false keeps the inverse propagator (last current, Eq. 22)
+    template <int I, int J, bool PROP>
+    __device__ __forceinline__ void range(cx* out) const {
+        cx s3[4], s4[4];
+#pragma unroll
+        for (int c = 0; c < 4; c++) { s3[c] = mk(0.0, 0.0); s4[c] = mk(0.0, 0.0); }
+        splits<I, I, J>(s3, s4);
+        double f3 = kInvSqrt2, f4 = 0.5;
+        if (PROP) {
+            const double* Pr = mom<I, J>();
+            const double ip2 = 1.0 / mdot(Pr, Pr);
+            f3 *= ip2; f4 *= ip2;
+        }
+#pragma unroll
+        for (int c = 0; c < 4; c++) out[c] = f3 * s3[c] + f4 * s4[c];
+    }
+};
+
+template <int NG, int TPE>
+__global__ void __launch_bounds__(128) cobg_shared_kernel(const CobgParams p) {
+    constexpr int M = NG - 1, LS = NG - 3, EPB = 128 / TPE, NSUB = 1 << M;
+    extern __shared__ double smem_d[];
+    const int evl = threadIdx.x / TPE, t = threadIdx.x % TPE;
+    const int np = p.np;
+    // per-event shared block: currents | subset momenta | eps_n | amplitudes | reduction scratch
+    const int ev_doubles = p.nslots * 8 + NSUB * 4 + 8 + np * 2 + 8;
+    double* cur = smem_d + (size_t)evl * ev_doubles;
+    double* P = cur + p.nslots * 8;
+    double* epsn = P + NSUB * 4;
+    double* A = epsn + 8;
+    double* red = A + np * 2;
+    const long long N = p.N;
+    const long long e_raw = (long long)blockIdx.x * EPB + evl;
+    const bool active = e_raw < N;
+    const long long e = active ? e_raw : 0;
+
+    // subset momenta P[mask] = sum of p_g over the bits of mask (gluons 0..M-1), the same for all helicities
+    for (int mask = t; mask < NSUB; mask += TPE) {
+        double ps[4] = {0.0, 0.0, 0.0, 0.0};
+        for (int g = 0; g < M; g++)
+            if ((mask >> g) & 1) {
+#pragma unroll
+                for (int c = 0; c < 4; c++) ps[c] += p.mom[(size_t)(g * 4 + c) * N + e];
+            }
+#pragma unroll
+        for (int c = 0; c < 4; c++) P[mask * 4 + c] = ps[c];
+    }
+
+    TopView<NG> tv;
+    tv.cur = cur;
+    tv.P = P;
+    const bool top = t < np;
+    {
+        const int sig = top ? t : 0;
+        tv.pm[0] = 0;
+#pragma unroll
+        for (int i = 0; i < M; i++) {
+            tv.pm[i + 1] = tv.pm[i] | (1u << p.ord[sig * M + i]);
+#pragma unroll
+            for (int j = 0; j < M; j++) tv.sl[i * M + j] = p.slot[(sig * M + i) * M + j];
+        }
+    }
+
+    double total = 0.0;
+    const int nhel = p.helsum ? (1 << NG) : 1;
+    for (int hc = 0; hc < nhel; hc++) {
+        __syncthreads();   // previous helicity's reads are done; P is visible
+        // level 1: external currents eps^lambda(p_g), Eq. 3, and eps_n
+        for (int idx = t; idx <= M; idx += TPE) {
+            int g = M, slot = -1;
+            if (idx < M) {
+                const uint32_t rep = p.lower[p.level_begin[1] + idx];
+                const int sig = rep >> 8, i = (rep >> 4) & 0xF;
+                g = p.ord[sig * M + i];
+                slot = p.slot[(sig * M + i) * M + i];
+            }
+            double pg[4];
+#pragma unroll
+            for (int c = 0; c < 4; c++) pg[c] = p.mom[(size_t)(g * 4 + c) * N + e];
+            const int lam = p.helsum ? (((hc >> g) & 1) ? 1 : -1) : (int)p.hel[(size_t)g * N + e];
+            cx eps[4];
+            polarisation(pg, lam, eps);
+            if (slot >= 0) sts_cur(cur, slot, eps);
+            else sts_cur(epsn, 0, eps);
+        }
+        __syncthreads();
+        // shared levels 2 .. n-3: one thread per distinct gluon sequence
+        for (int L = 2; L <= LS; L++) {
+            for (int idx = p.level_begin[L] + t; idx < p.level_begin[L + 1]; idx += TPE) {
+                const uint32_t rep = p.lower[idx];
+                const int sig = rep >> 8, i = (rep >> 4) & 0xF, j = rep & 0xF;
+                const uint16_t* sl = p.slot + (size_t)sig * M * M;
+                const uint8_t* og = p.ord + sig * M;
+                cx s3[4], s4[4];
+#pragma unroll
+                for (int c = 0; c < 4; c++) { s3[c] = mk(0.0, 0.0); s4[c] = mk(0.0, 0.0); }
+                unsigned mall = 0;
+                for (int k = i; k <= j; k++) mall |= 1u << og[k];
+                unsigned ma = 0;
+                for (int k = i; k < j; k++) {
+                    ma |= 1u << og[k];
+                    cx a[4], b[4];
+                    lds_cur(cur, sl[i * M + k], a);
+                    lds_cur(cur, sl[(k + 1) * M + j], b);
+                    v3_acc(s3, P + 4 * ma, P + 4 * (mall ^ ma), a, b, 1.0);
+                    for (int l = k + 1; l < j; l++) {
+                        cx b2[4], c2[4];
+                        lds_cur(cur, sl[(k + 1) * M + l], b2);
+                        lds_cur(cur, sl[(l + 1) * M + j], c2);
+                        v4_acc(s4, a, b2, c2);
+                    }
+                }
+                const double ip2 = 1.0 / mdot(P + 4 * mall, P + 4 * mall);
+                cx J[4];
+#pragma unroll
+                for (int c = 0; c < 4; c++) J[c] = (kInvSqrt2 * ip2) * s3[c] + (0.5 * ip2) * s4[c];
+                sts_cur(cur, sl[i * M + j], J);
+            }
+            __syncthreads();
+        }
+        // register-resident top: thread sigma builds the two (n-2)-gluon currents and the final one of its ordering
+        if (top) {
+            tv.template range<1, M - 1, true>(tv.JA);
+            tv.template range<0, M - 2, true>(tv.JB);
+            cx JF[4], en[4];
+            tv.template range<0, M - 1, false>(JF);
+            lds_cur(epsn, 0, en);
+            const cx amp = mdot(en, JF);
+            A[2 * t] = amp.re;
+            A[2 * t + 1] = amp.im;
+        }
+        __syncthreads();
+        // Eq. 16: row sigma of the real symmetric quadratic form
+        double w = 0.0;
+        if (top) {
+            double tr = 0.0, ti = 0.0;
+            const double* Ccol = p.C + t;
+            for (int s2 = 0; s2 < np; s2++) {
+                const double c = __ldg(Ccol + (size_t)s2 * np);
+                const double2 a2 = *reinterpret_cast<const double2*>(A + 2 * s2);
+                tr = fma(c, a2.x, tr);
+                ti = fma(c, a2.y, ti);
+            }
+            w = fma(A[2 * t], tr, A[2 * t + 1] * ti);
+        }
+#pragma unroll
+        for (int d = 1; d < (TPE < 32 ? TPE : 32); d <<= 1) w += __shfl_xor_sync(0xFFFFFFFFu, w, d);
+        if (TPE > 32) {
+            if ((t & 31) == 0) red[t >> 5] = w;
+            __syncthreads();
+            w = 0.0;
+            for (int i = 0; i < TPE / 32; i++) w += red[i];
+        }
+        total += w;
+    }
+    if (t == 0 && active) p.out[e] = total;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------------------
+bool cobg_shared_supported(int n) { return n >= 4 && n <= 7; }
+
+int cobg_table_create(int n, CobgTable** out) {
+    *out = nullptr;
+    if (!cobg_shared_supported(n)) return BG_EUNSUPPORTED;
+    const int m = n - 1, ls = n - 3;
+    std::vector<int> sigma(n - 2);
+    std::iota(sigma.begin(), sigma.end(), 1);
+    std::vector<std::vector<int>> ords;   // (0, sigma) in lexicographic order of sigma - the order of C's rows
+    do {
+        std::vector<int> o{0};
+        o.insert(o.end(), sigma.begin(), sigma.end());
+        ords.push_back(o);
+    } while (std::next_permutation(sigma.begin(), sigma.end()));
+    const int np = (int)ords.size();
+    std::vector<uint16_t> slot((size_t)np * m * m, 0xFFFF);
+    std::vector<uint8_t> ord((size_t)np * m);
+    std::vector<uint32_t> lower;
+    CobgTable* t = new (std::nothrow) CobgTable();
+    if (!t) return BG_ENOMEM;
+    std::memset(t, 0, sizeof(*t));
+    std::map<std::vector<int>, int> ids;
+    int next = 0;
+    t->level_begin[0] = t->level_begin[1] = 0;
+    for (int L = 1; L <= ls; L++) {
+        t->level_begin[L] = (int)lower.size();
+        for (int s = 0; s < np; s++)
+            for (int i = 0; i + L <= m; i++) {
+                const std::vector<int> seq(ords[s].begin() + i, ords[s].begin() + i + L);
+                auto it = ids.find(seq);
+                if (it == ids.end()) {
+                    it = ids.emplace(seq, next++).first;
+                    lower.push_back((uint32_t)(s << 8 | i << 4 | (i + L - 1)));
+                }
+                slot[((size_t)s * m + i) * m + i + L - 1] = (uint16_t)it->second;
+            }
+    }
+    for (int L = ls + 1; L <= kCobgMaxM + 1; L++) t->level_begin[L] = (int)lower.size();
+    for (int s = 0; s < np; s++)
+        for (int i = 0; i < m; i++) ord[(size_t)s * m + i] = (uint8_t)ords[s][i];
+    t->n = n; t->np = np; t->nslots = next;
+    bool ok = cudaMalloc(&t->d_slot, slot.size() * 2) == cudaSuccess && cudaMalloc(&t->d_ord, ord.size()) == cudaSuccess &&
+              cudaMalloc(&t->d_lower, std::max<size_t>(lower.size(), 1) * 4) == cudaSuccess;
+    ok = ok && cudaMemcpy(t->d_slot, slot.data(), slot.size() * 2, cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(t->d_ord, ord.data(), ord.size(), cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(t->d_lower, lower.data(), lower.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        cobg_table_destroy(t);
+        return BG_ENOMEM;
+    }
+    *out = t;
+    return BG_OK;
+}
+
+void cobg_table_destroy(CobgTable* t) {
+    if (!t) return;
+    if (t->d_slot) cudaFree(t->d_slot);
+    if (t->d_ord) cudaFree(t->d_ord);
+    if (t->d_lower) cudaFree(t->d_lower);
+    delete t;
+}
+
+size_t cobg_shared_current_bytes(const CobgTable* t) { return t ? (size_t)t->nslots * 64 : 0; }
+
+template <int NG, int TPE>
+static cudaError_t launch_cobg(cudaStream_t s, const CobgParams& p) {
+    constexpr int EPB = 128 / TPE, NSUB = 1 << (NG - 1);
+    const size_t smem = (size_t)EPB * (p.nslots * 8 + NSUB * 4 + 8 + p.np * 2 + 8) * sizeof(double);
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(cobg_shared_kernel<NG, TPE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const unsigned blocks = (unsigned)((p.N + EPB - 1) / EPB);
+    cobg_shared_kernel<NG, TPE><<<blocks, 128, smem, s>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, const double* dC, long long N,
+                               const double* mom, const signed char* hel, double* out) {
+    CobgParams p;
+    p.n = t->n; p.np = t->np; p.nslots = t->nslots; p.helsum = helsum ? 1 : 0;
+    p.N = N; p.mom = mom; p.hel = hel; p.C = dC; p.out = out;
+    p.slot = t->d_slot; p.ord = t->d_ord; p.lower = t->d_lower;
+    for (int i = 0; i < kCobgMaxM + 2; i++) p.level_begin[i] = t->level_begin[i];
+    switch (t->n) {
+        case 4: return launch_cobg<4, 8>(s, p);
+        case 5: return launch_cobg<5, 8>(s, p);
+        case 6: return launch_cobg<6, 32>(s, p);
+        case 7: return launch_cobg<7, 128>(s, p);
+        default: return cudaErrorNotSupported;
+    }
+}
+
+}  // namespace bg

@@ -6,7 +6,7 @@
 
 #include "../../include/bg.h"
 
-namespace bg { struct ProgTable; }
+namespace bg { struct ProgTable; struct CobgTable; }
 
 struct bg_ctx {
     int n;
@@ -31,6 +31,7 @@ struct bg_ctx {
     long long staged_events;
     // colour-class programs (CDBG, given colours)
     bg::ProgTable* prog;
+    bg::CobgTable* cobg;       // sequence tables of the shared-current COBG kernel (n <= 7)
     int prog_lanes;            // BG_OPT_LANES (0 = automatic)
     // bookkeeping
     int timing;                // BG_OPT_TIMING
@@ -60,6 +61,14 @@ size_t prog_scratch_bytes(const ProgTable* t, long long N);
 cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
                              const signed char* hel, const signed char* col, double* out, void* scratch,
                              int* launches, cudaEvent_t ev0, cudaEvent_t ev1);
+
+// ---- shared-current COBG kernel (bg_cobg_shared.cu): one thread group per event, n <= 7 -----------------------
+bool cobg_shared_supported(int n);
+int cobg_table_create(int n, CobgTable** out);              // BG_* code
+void cobg_table_destroy(CobgTable* t);
+size_t cobg_shared_current_bytes(const CobgTable* t);
+cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, const double* dC, long long N,
+                               const double* mom, const signed char* hel, double* out);
 
 // ---- colour matrix (bg_colour.cpp part of bg_api.cu) ------------------------------------------------------
 int build_colour_matrix(int n, double* C /* (n-2)!^2 */);
