@@ -94,6 +94,7 @@ struct TopView {
     template <int I, int K, int L, int J>
     __device__ __forceinline__ void v4_inner(cx* s4, const cx* a) const {
         if constexpr (L < J) {
+            asm volatile("" ::: "memory");   // keep the operand loads of later vertices from being hoisted (registers)
             cx b[4], c[4];
             fetch<K + 1, L>(b);
             fetch<L + 1, J>(c);
@@ -104,6 +105,7 @@ struct TopView {
     template <int I, int K, int J>
     __device__ __forceinline__ void splits(cx* s3, cx* s4) const {
         if constexpr (K < J) {
+            asm volatile("" ::: "memory");
             cx a[4], b[4];
             fetch<I, K>(a);
             fetch<K + 1, J>(b);
@@ -131,7 +133,7 @@ struct TopView {
 };
 
 template <int NG, int TPE>
-__global__ void __launch_bounds__(128) cobg_shared_kernel(const CobgParams p) {
+__global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p) {
     constexpr int M = NG - 1, LS = NG - 3, EPB = 128 / TPE, NSUB = 1 << M;
     extern __shared__ double smem_d[];
     const int evl = threadIdx.x / TPE, t = threadIdx.x % TPE;
@@ -247,15 +249,24 @@ __global__ void __launch_bounds__(128) cobg_shared_kernel(const CobgParams p) {
         // Eq. 16: row sigma of the real symmetric quadratic form
         double w = 0.0;
         if (top) {
-            double tr = 0.0, ti = 0.0;
+            double tr[4] = {0.0, 0.0, 0.0, 0.0}, ti[4] = {0.0, 0.0, 0.0, 0.0};
             const double* Ccol = p.C + t;
-            for (int s2 = 0; s2 < np; s2++) {
-                const double c = __ldg(Ccol + (size_t)s2 * np);
-                const double2 a2 = *reinterpret_cast<const double2*>(A + 2 * s2);
-                tr = fma(c, a2.x, tr);
-                ti = fma(c, a2.y, ti);
+            int s2 = 0;
+            for (; s2 + 4 <= np; s2 += 4) {
+#pragma unroll
+                for (int u = 0; u < 4; u++) {
+                    const double c = __ldg(Ccol + (size_t)(s2 + u) * np);
+                    const double2 a2 = *reinterpret_cast<const double2*>(A + 2 * (s2 + u));
+                    tr[u] = fma(c, a2.x, tr[u]);
+                    ti[u] = fma(c, a2.y, ti[u]);
+                }
             }
-            w = fma(A[2 * t], tr, A[2 * t + 1] * ti);
+            for (; s2 < np; s2++) {
+                const double c = __ldg(Ccol + (size_t)s2 * np);
+                tr[0] = fma(c, A[2 * s2], tr[0]);
+                ti[0] = fma(c, A[2 * s2 + 1], ti[0]);
+            }
+            w = fma(A[2 * t], (tr[0] + tr[1]) + (tr[2] + tr[3]), A[2 * t + 1] * ((ti[0] + ti[1]) + (ti[2] + ti[3])));
         }
 #pragma unroll
         for (int d = 1; d < (TPE < 32 ? TPE : 32); d <<= 1) w += __shfl_xor_sync(0xFFFFFFFFu, w, d);
