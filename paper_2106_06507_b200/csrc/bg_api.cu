@@ -122,8 +122,11 @@ int build_colour_matrix(int n, double* C) {
 
 // =========================================== ABI ===========================================================
 // largest n whose colour-class programs are tabulated at bg_init, and the default lanes per event
-static const int kProgMaxN = 8;
-static int auto_lanes(int n) { return n <= 5 ? 2 : (n <= 7 ? 4 : 8); }
+static const int kProgMaxN = 10;
+static int auto_lanes(int n) {
+    static const int lanes[] = {0, 0, 0, 0, 2, 2, 4, 8, 32, 64, 128, 256, 256};
+    return lanes[n];
+}
 
 static bool mode_supported(int n, int mode) {
     if (n < 4 || n > 12) return false;
@@ -291,7 +294,8 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
             return BG_OK;
         case BG_OPT_LANES: {
             if (c->mode != BG_CDBG_GIVEN || c->n > kProgMaxN) return BG_EUNSUPPORTED;
-            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32)
+            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32 &&
+                value != 64 && value != 128 && value != 256)
                 return BG_EINVAL;
             const int G = value ? (int)value : auto_lanes(c->n);
             if (c->prog && bg::prog_lanes(c->prog) == G) return BG_OK;

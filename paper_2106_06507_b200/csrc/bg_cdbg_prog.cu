@@ -24,16 +24,19 @@
 
 namespace bg {
 
-struct ClassInfo {            // 32 bytes
+constexpr int kMaxLevels = 2 * kMaxN - 4;   // setup | (main, combine) per popcount 2..n-2 | closure
+
+struct ClassInfo {            // 64 bytes
     uint32_t op_base;         // first op of the class in the op array (units of ProgOp)
     uint16_t state_cx;
     uint8_t closure_code;
     uint8_t valid;
-    uint16_t level_steps[11];
-    uint16_t pad;
+    uint16_t level_steps[kMaxLevels];
+    uint16_t pad[28 - kMaxLevels];
 };
-static_assert(sizeof(ClassInfo) == 32, "ClassInfo layout");
+static_assert(sizeof(ClassInfo) == 64, "ClassInfo layout");
 
+constexpr size_t kMaxSlabBytes = 226 * 1024;   // dynamic shared memory per block (1 KB left for static use)
 constexpr int kTiers = 4;     // classes are grouped by state size so that small ones get more warps per SM
 
 struct TierInfo {
@@ -234,15 +237,16 @@ __device__ __forceinline__ void sts(double2* S, int o, cx v) {
 }
 
 template <int G>
-__global__ void __launch_bounds__(32) cdbg_prog_kernel(const ProgParams p) {
-    constexpr int EPW = 32 / G;
+__global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgParams p) {
+    // G <= 32: one warp per block, EPW = 32/G events per warp.  G > 32: one event per block of G threads.
+    constexpr int EPW = G >= 32 ? 1 : 32 / G;
     extern __shared__ double2 smem[];
-    const int lane = threadIdx.x;          // one warp per block
+    const int lane = threadIdx.x;
     const int q = lane % EPW, g = lane / EPW;
     double2* S = smem + q;
     const long long first = p.bounds[p.tier], end = p.bounds[p.tier + 1];
     const long long ntasks = (end - first + EPW - 1) / EPW;
-    const int nlev = p.n - 1;
+    const int nlev = 2 * p.n - 4;
     const long long N = p.N;
 
     for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
@@ -309,7 +313,13 @@ __global__ void __launch_bounds__(32) cdbg_prog_kernel(const ProgParams p) {
                         tcontract_acc(acc, T, b, -sign);
                     }
                     if (!(flags & OPF_CLOSURE)) tbuild_acc(tacc, a, b, sign);
-                    if (flags & OPF_LAST) {
+                    if (flags & OPF_PARTIAL) {
+                        // chunk of a split target: raw sums to its scratch slot, finished by a COMBINE op
+#pragma unroll
+                        for (int c = 0; c < 4; c++) sts<EPW>(S, offDst + c, acc[c]);
+#pragma unroll
+                        for (int c = 0; c < 6; c++) sts<EPW>(S, offDst + 4 + c, tacc[c]);
+                    } else if (flags & OPF_LAST) {
                         if (flags & OPF_CLOSURE) {
                             cx en[4];
 #pragma unroll
@@ -353,6 +363,39 @@ __global__ void __launch_bounds__(32) cdbg_prog_kernel(const ProgParams p) {
                     const cx d = mdot(en, x);
                     amp.re = fma(kInvSqrt2, d.re, amp.re);
                     amp.im = fma(kInvSqrt2, d.im, amp.im);
+                } else if (flags & OPF_COMBINE) {
+                    // add the offB partial sums of a split target and finish it like a LAST op
+#pragma unroll
+                    for (int c = 0; c < 4; c++) acc[c] = lds<EPW>(S, offA + c);
+#pragma unroll
+                    for (int c = 0; c < 6; c++) tacc[c] = lds<EPW>(S, offA + 4 + c);
+                    for (int r = 1; r < offB; r++) {
+#pragma unroll
+                        for (int c = 0; c < 4; c++) acc[c] = acc[c] + lds<EPW>(S, offA + 10 * r + c);
+#pragma unroll
+                        for (int c = 0; c < 6; c++) tacc[c] = tacc[c] + lds<EPW>(S, offA + 10 * r + 4 + c);
+                    }
+                    {
+                        const int offP2 = (int)(raw.w & 0xFFFF);
+                        const cx a01 = lds<EPW>(S, offP1), a23 = lds<EPW>(S, offP1 + 1);
+                        const cx b01 = lds<EPW>(S, offP2), b23 = lds<EPW>(S, offP2 + 1);
+                        Pt[0] = a01.re + b01.re; Pt[1] = a01.im + b01.im; Pt[2] = a23.re + b23.re; Pt[3] = a23.im + b23.im;
+                    }
+                    const double f = kInvSqrt2 / mdot(Pt, Pt);
+#pragma unroll
+                    for (int c = 0; c < 4; c++) acc[c] = f * acc[c];
+#pragma unroll
+                    for (int c = 0; c < 6; c++) tacc[c] = kInvSqrt2 * tacc[c];
+                    if (!(flags & OPF_NOSTORE)) {
+#pragma unroll
+                        for (int c = 0; c < 4; c++) sts<EPW>(S, offDst + c, acc[c]);
+#pragma unroll
+                        for (int c = 0; c < 6; c++) sts<EPW>(S, offDst + 4 + c, tacc[c]);
+                    }
+                    if (flags & OPF_STOREP) {
+                        sts<EPW>(S, offPt, mk(Pt[0], Pt[1]));
+                        sts<EPW>(S, offPt + 1, mk(Pt[2], Pt[3]));
+                    }
                 } else if (flags & OPF_EXT) {
                     const int k = (int)raw.w;
                     const int orig = (int)((perm >> (4 * k)) & 0xF);
@@ -370,7 +413,7 @@ __global__ void __launch_bounds__(32) cdbg_prog_kernel(const ProgParams p) {
                 }
                 raw = nxt;
             }
-            __syncwarp();
+            if constexpr (G > 32) __syncthreads(); else __syncwarp();
         }
         // closure amplitude: sum of the G lanes' partial contractions (Eq. 22), then |A|^2
 #pragma unroll
@@ -378,8 +421,17 @@ __global__ void __launch_bounds__(32) cdbg_prog_kernel(const ProgParams p) {
             amp.re += __shfl_xor_sync(0xFFFFFFFFu, amp.re, d);
             amp.im += __shfl_xor_sync(0xFFFFFFFFu, amp.im, d);
         }
+        if constexpr (G > 32) {
+            __shared__ double red_s[2 * (G / 32)];
+            if ((lane & 31) == 0) { red_s[2 * (lane >> 5)] = amp.re; red_s[2 * (lane >> 5) + 1] = amp.im; }
+            __syncthreads();
+            if (lane == 0) {
+                amp = mk(0.0, 0.0);
+                for (int w = 0; w < G / 32; w++) { amp.re += red_s[2 * w]; amp.im += red_s[2 * w + 1]; }
+            }
+        }
         if (g == 0 && have) p.out[e] = valid ? fma(amp.re, amp.re, amp.im * amp.im) : 0.0;
-        __syncwarp();
+        if constexpr (G > 32) __syncthreads(); else __syncwarp();
     }
 }
 
@@ -400,7 +452,7 @@ static void enumerate_counts(int t, int r, int* counts, std::vector<std::vector<
 
 int prog_table_create(int n, int G, ProgTable** out) {
     *out = nullptr;
-    if (n < 4 || n > kMaxN || (G != 1 && G != 2 && G != 4 && G != 8 && G != 16 && G != 32)) return BG_EINVAL;
+    if (n < 4 || n > kMaxN || (G != 1 && G != 2 && G != 4 && G != 8 && G != 16 && G != 32 && G != 64 && G != 128 && G != 256)) return BG_EINVAL;
     std::vector<std::vector<int>> all;
     int counts[kNumCodes];
     enumerate_counts(0, n, counts, all);
@@ -421,7 +473,7 @@ int prog_table_create(int n, int G, ProgTable** out) {
         ci.op_base = (uint32_t)ops.size();
         ci.state_cx = (uint16_t)cp.state_cx;
         ci.closure_code = (uint8_t)cp.closure_code;
-        for (int l = 0; l < n - 1; l++) ci.level_steps[l] = cp.level_steps[l];
+        for (size_t l = 0; l < cp.level_steps.size(); l++) ci.level_steps[l] = cp.level_steps[l];
         steps[r] = cp.total_steps;
         max_state = std::max(max_state, cp.state_cx);
         ops.insert(ops.end(), cp.ops.begin(), cp.ops.end());
@@ -448,7 +500,7 @@ int prog_table_create(int n, int G, ProgTable** out) {
     for (long long i = nc - 1; i >= 0; i--) tiers.first_key[tier_of[by[i]]] = (int)i;
     for (int k = kTiers - 1; k >= 0; k--) tiers.first_key[k] = std::min(tiers.first_key[k], tiers.first_key[k + 1]);
 
-    if ((size_t)(32 / G) * max_state * 16 > 227 * 1024) return BG_EUNSUPPORTED;   // one warp's slab must fit
+    if ((size_t)(G >= 32 ? 1 : 32 / G) * max_state * 16 > kMaxSlabBytes) return BG_EUNSUPPORTED;   // one block's slab must fit
     ProgTable* t = new (std::nothrow) ProgTable();
     if (!t) return BG_ENOMEM;
     std::memset(t, 0, sizeof(*t));
@@ -496,10 +548,10 @@ size_t prog_scratch_bytes(const ProgTable* t, long long N) {
 
 template <int G>
 static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched) {
-    constexpr int EPW = 32 / G;
+    constexpr int EPW = G >= 32 ? 1 : 32 / G, BLOCK = G > 32 ? G : 32;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSlabBytes);
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -508,12 +560,12 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         if (t->tiers.first_key[k] == t->tiers.first_key[k + 1] && k + 1 < kTiers) continue;   // no class in this tier
         p.tier = k;
         p.slab_cx = t->tiers.slab_cx[k];
-        const size_t smem = (size_t)EPW * p.slab_cx * 16;     // one warp per block
-        if (smem > 227 * 1024) return cudaErrorInvalidValue;
-        // resident warps per SM: shared memory (1 KB reserved per block), and 65536 / (32 x 152) registers
-        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(13, (228 * 1024) / (smem + 1024)));
+        const size_t smem = (size_t)EPW * p.slab_cx * 16;
+        if (smem > kMaxSlabBytes) return cudaErrorInvalidValue;
+        // resident blocks per SM: shared memory (1 KB reserved per block), and 65536 / (160 x BLOCK) registers
+        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (160 * BLOCK), (228 * 1024) / (smem + 1024)));
         const unsigned blocks = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
-        cdbg_prog_kernel<G><<<blocks, 32, smem, s>>>(p);
+        cdbg_prog_kernel<G><<<blocks, BLOCK, smem, s>>>(p);
         ++*launched;
     }
     return cudaGetLastError();
@@ -564,7 +616,10 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         case 4: err = launch_interp<4>(s, t, sm_count, p, launches); break;
         case 8: err = launch_interp<8>(s, t, sm_count, p, launches); break;
         case 16: err = launch_interp<16>(s, t, sm_count, p, launches); break;
-        default: err = launch_interp<32>(s, t, sm_count, p, launches); break;
+        case 32: err = launch_interp<32>(s, t, sm_count, p, launches); break;
+        case 64: err = launch_interp<64>(s, t, sm_count, p, launches); break;
+        case 128: err = launch_interp<128>(s, t, sm_count, p, launches); break;
+        default: err = launch_interp<256>(s, t, sm_count, p, launches); break;
     }
     if (ev1) cudaEventRecord(ev1, s);
     return err;

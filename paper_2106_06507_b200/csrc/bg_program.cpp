@@ -196,8 +196,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
             if (!t.fused) { off[t.pi * 3 + t.slot()] = next; next += 10; }
             if (need_p[t.pi] && poff[t.pi] < 0) { poff[t.pi] = next; next += 2; t.store_p = true; }
         }
-    out.state_cx = next;
-    out.level_steps.assign(m, 0);
+    out.level_steps.assign(2 * m - 2, 0);   // setup | (main, combine) per popcount 2..n-2 | closure
 
     // ---- phase 4: deal the work of every level over the G lanes and emit ----
     auto emit_level = [&](int lvl, std::vector<std::vector<ProgOp>>& lanes) {
@@ -265,40 +264,118 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
         }
     };
 
+    // A unit of work is a run of vertices of one target that one lane accumulates in its registers: the whole
+    // target, or - when a level has fewer big targets than lanes - a chunk of it, whose raw partial sums go to
+    // a scratch slot and are added up by one lane in a "combine" sub-level after a barrier.
+    struct Unit { int target, first, count, part; };   // part: -1 = whole target, else index of the scratch slot
+    const int scratch_base = next;
+    int scratch_max = 0;
     for (int pc = 2; pc <= m; pc++) {
-        std::vector<std::vector<ProgOp>> lanes(G);
+        std::vector<std::vector<ProgOp>> lanes(G), clanes(G);
         auto& tg = levels[pc];
         if (pc == m) {
             // closure: one target, its remaining vertices dealt round-robin; every lane contracts its partial
             // sum with eps_n and the lanes' amplitudes are added at the end
             const Target& t = tg[0];
-            std::vector<VOp> ops = t.ops;
-            for (size_t i = 0; i < ops.size(); i++) {
-                lanes[i % G].push_back(make_op(t, ops[i]));
+            for (size_t i = 0; i < t.ops.size(); i++) {
+                lanes[i % G].push_back(make_op(t, t.ops[i]));
                 out.n_vertex_ops++;
             }
             for (auto& l : lanes)
                 if (!l.empty()) { l.front().flags |= OPF_FIRST; l.back().flags |= OPF_LAST; }
-        } else {
-            std::vector<int> order(tg.size()), load(G, 0);
-            for (size_t i = 0; i < tg.size(); i++) order[i] = (int)i;
-            auto cost = [&](int a) { return (int)tg[a].ops.size() + (tg[a].fused ? 1 : 0); };
-            std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return cost(a) > cost(b); });
-            for (int idx : order) {
-                const int l = (int)(std::min_element(load.begin(), load.end()) - load.begin());
-                push_target(lanes[l], tg[idx]);
-                load[l] += cost(idx);
+            emit_level(2 * (pc - 2) + 1, lanes);
+            break;
+        }
+        long long total = 0;
+        for (auto& t : tg) total += (long long)t.ops.size() + (t.fused ? 1 : 0);
+        const int ideal = (int)((total + G - 1) / G);
+        const int chunk_max = std::max(ideal, 2);
+        std::vector<Unit> units;
+        std::vector<int> nparts(tg.size(), 0), part0(tg.size(), -1);
+        int nscratch = 0;
+        for (size_t i = 0; i < tg.size(); i++) {
+            const int c = (int)tg[i].ops.size();
+            if (G == 1 || c + (tg[i].fused ? 1 : 0) <= chunk_max || c < 4) {
+                units.push_back({(int)i, 0, c, -1});
+                continue;
+            }
+            const int r = (c + chunk_max - 1) / chunk_max;
+            nparts[i] = r;
+            part0[i] = nscratch;
+            for (int k = 0; k < r; k++) {
+                const int lo = (int)((long long)c * k / r), hi = (int)((long long)c * (k + 1) / r);
+                units.push_back({(int)i, lo, hi - lo, nscratch++});
             }
         }
-        emit_level(pc - 1, lanes);
+        scratch_max = std::max(scratch_max, nscratch * 10);
+        auto ucost = [&](const Unit& u) { return u.count + (u.part < 0 && tg[u.target].fused ? 1 : 0); };
+        std::stable_sort(units.begin(), units.end(), [&](const Unit& a, const Unit& b) { return ucost(a) > ucost(b); });
+        std::vector<int> load(G, 0);
+        for (auto& u : units) {
+            const int l = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+            load[l] += ucost(u);
+            const Target& t = tg[u.target];
+            if (u.part < 0) {
+                push_target(lanes[l], t);
+                continue;
+            }
+            for (int i = u.first; i < u.first + u.count; i++) {
+                ProgOp o = make_op(t, t.ops[i]);
+                if (i == u.first) o.flags |= OPF_FIRST;
+                if (i + 1 == u.first + u.count) {
+                    o.flags |= OPF_LAST | OPF_PARTIAL;
+                    o.offDst = (uint16_t)(scratch_base + 10 * u.part);
+                }
+                lanes[l].push_back(o);
+                out.n_vertex_ops++;
+            }
+        }
+        // combine sub-level: one lane per split target
+        int cl = 0;
+        for (size_t i = 0; i < tg.size(); i++) {
+            if (!nparts[i]) continue;
+            const Target& t = tg[i];
+            ProgOp o = make_op(t, t.ops[0]);   // offP1 / extra give P(pi) = P(pi_1) + P(pi_2); offDst, offPt as usual
+            o.offA = (uint16_t)(scratch_base + 10 * part0[i]);
+            o.offB = (uint16_t)nparts[i];
+            o.flags = OPF_COMBINE | (t.store_p ? OPF_STOREP : 0) | (t.fused ? OPF_NOSTORE : 0);
+            auto& lane = clanes[cl++ % G];
+            lane.push_back(o);
+            if (t.fused) {
+                ProgOp f;
+                std::memset(&f, 0, sizeof(f));
+                f.offA = (uint16_t)off[t.fuse.pa * 3 + t.fuse.sa];
+                f.offP1 = (uint16_t)poff[t.fuse.pa];
+                f.offDst = (uint16_t)off_epsn;
+                f.flags = OPF_FUSED | (t.fuse.neg ? OPF_NEG : 0);
+                lane.push_back(f);
+                out.n_vertex_ops++;
+            }
+        }
+        emit_level(2 * (pc - 2) + 1, lanes);
+        emit_level(2 * (pc - 2) + 2, clanes);
     }
+    out.state_cx = next + scratch_max;
 }
 
 void build_class(int n, int G, const int* counts, ClassProgram& out) {
     out = ClassProgram();
+    // the colour charges must cancel over all n gluons (as many i = c as j = c for every colour c)
+    for (int c = 0; c < 3; c++) {
+        int ni = 0, nj = 0;
+        for (int t = 0; t < kNumCodes; t++) {
+            if (t / 3 == c) ni += counts[t];
+            if (t % 3 == c) nj += counts[t];
+        }
+        if (ni != nj) return;
+    }
+    // every gluon can serve as the closure leg; the cheapest program among a few choices is kept
+    const int max_trials = n <= 8 ? kNumCodes : (n == 9 ? 4 : 2);
+    int trials = 0;
     bool have = false;
-    for (int c = 0; c < kNumCodes; c++) {
+    for (int c = 0; c < kNumCodes && trials < max_trials; c++) {
         if (!counts[c]) continue;
+        trials++;
         int code[kMaxN], k = 0;
         for (int t = 0; t < kNumCodes; t++)
             for (int r = 0; r < counts[t] - (t == c ? 1 : 0); r++) code[k++] = t;

@@ -41,6 +41,8 @@ enum : uint16_t {
     OPF_STOREP = 256,  // (with LAST) also store P(target) at offPt: set on one entry per subset
     OPF_FUSED = 512,   // closure vertex X(eps_k at offA, b = the current just finished in registers) . eps_n
     OPF_NOSTORE = 1024,// (with LAST) the finished current stays in registers only (a FUSED op follows)
+    OPF_PARTIAL = 2048,// (with LAST) chunk of a split target: raw partial sums -> scratch slot offDst
+    OPF_COMBINE = 4096,// add offB partial slots starting at offA, then finish the target like LAST
     OPF_EXT = 128      // setup: external current of gluon `extra` -> offDst, its momentum -> offPt
 };
 
@@ -53,7 +55,7 @@ struct ClassProgram {
     int state_cx = 0;            // per-event state size in complex doubles
     int n_vertex_ops = 0;        // number of OPF_VALID ops
     int total_steps = 0;         // sum over levels of max-lane op count
-    std::vector<uint16_t> level_steps;   // [n-1]: level 0 = setup, then popcount 2 .. n-1
+    std::vector<uint16_t> level_steps;   // [2n-4]: setup | (main, combine) for popcount 2..n-2 | closure
     std::vector<ProgOp> ops;             // [total_steps][G]
 };
 

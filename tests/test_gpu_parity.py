@@ -142,6 +142,16 @@ def test_program_interpreter_lane_counts(bg, oracle, wl, n, N, lanes):
     check_cdbg(oracle, ev, got)
 
 
+@pytest.mark.parametrize("n,N", [(8, 131), (9, 259), (10, 131)])
+@pytest.mark.parametrize("lanes", [32, 64, 128, 256])
+def test_program_interpreter_block_per_event(bg, oracle, wl, n, N, lanes):
+    """One event per warp / per block of 64..256 threads (split targets, combine sub-levels, block barriers)."""
+    ev = wl.config_events(4, N=N, n=n)
+    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=2, lanes=lanes)
+    assert name == "cdbg_prog_kernel"
+    check_cdbg(oracle, ev, got)
+
+
 def test_cdbg_helicity_sum_mode(bg, oracle, wl):
     import itertools
     ev = wl.config_events(4, N=40, n=5)
