@@ -115,6 +115,16 @@ def make_events(args, n, N, rank):
     return wl.config_events(args.config, N=N, n=n if args.config == 4 else None, first_event=rank * N)
 
 
+def max_over_ranks(value: float, world: int, dev) -> float:
+    """Multi-GPU numbers are the maximum over ranks (the slowest rank defines the step)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def mode_for(config):
     import paper_2106_06507_b200 as bg
     return {0: bg.BG_COBG_HELSUM_FULLCOLOR, 2: bg.BG_COBG_HELGIVEN_FULLCOLOR}.get(config, bg.BG_CDBG_GIVEN)
@@ -243,10 +253,7 @@ def run_b200(args):
     launches_per_step = bg.bg_last_launch_count(ctx)
     kernel_name = bg.bg_last_kernel_name(ctx)
     kernel_ms = float(np.mean(kms))      # per step: all launches of the dominant kernel
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world, dev)
     value = N * world * args.steps / (total_ms * 1e-3)
 
     # end-to-end: host buffers through bg_eval_host (H2D of inputs + D2H of results inside the timed region)
@@ -260,12 +267,10 @@ def run_b200(args):
         for _ in range(k2):
             bg.bg_eval_host(ctx, N, h_mom, h_hel, h_col, h_out)
         barrier()
-        dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        dt = max_over_ranks(time.perf_counter() - t0, world, dev)
         h2d = mom.nbytes + (0 if hel is None or mode & bg.BG_HEL_SUM else hel.nbytes) + \
             (0 if col is None or not (mode & bg.BG_COL_GIVEN) else col.nbytes)
-        e2e = {"value": N * world * k2 / float(dt.item()), "unit": "events/s", "h2d_bytes_per_step": int(h2d),
+        e2e = {"value": N * world * k2 / dt, "unit": "events/s", "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(N * 8), "steps": k2}
         if rank == 0 and not np.allclose(h_out.numpy(), d_out.cpu().numpy(), rtol=0, atol=0, equal_nan=True):
             raise SystemExit("bench.py: host path and device path disagree")

@@ -124,6 +124,15 @@ int bg_last_kernel_ms(bg_ctx* ctx, double* ms);
 /* Name of the kernel variant the most recent bg_eval used (static string). */
 const char* bg_last_kernel_name(const bg_ctx* ctx);
 
+/*
+ * Host-only introspection of the colour-class program generator behind the BG_CDBG_GIVEN interpreter (no device
+ * needed).  counts[9]: how many of the n gluons carry colour code 3*(i-1)+(j-1) = 0..8 (sum = n, 4 <= n <= 12);
+ * lanes as in BG_OPT_LANES.  Writes stats[0] = 1 if the class has a non-vanishing colour structure else 0,
+ * stats[1] = vertex evaluations per event, stats[2] = interpreter steps (max over lanes, summed over levels),
+ * stats[3] = bytes of per-event state, stats[4] = colour code of the gluon chosen as closure leg.
+ */
+int bg_class_program_stats(int n, int lanes, const int* counts, long long* stats);
+
 int bg_destroy(bg_ctx* ctx);
 
 const char* bg_strerror(int code);

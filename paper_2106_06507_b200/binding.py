@@ -25,7 +25,7 @@ BG_OPT_KERNEL, BG_OPT_SCRATCH_LIMIT, BG_OPT_LANES, BG_OPT_TIMING = 1, 2, 3, 4
 
 EXPORTS = ("bg_init", "bg_eval", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",
            "bg_set_option", "bg_colour_matrix", "bg_build_colour_matrix", "bg_last_launch_count",
-           "bg_last_kernel_name", "bg_last_kernel_ms", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe")
+           "bg_last_kernel_name", "bg_last_kernel_ms", "bg_class_program_stats", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe")
 
 
 class BgError(RuntimeError):
@@ -62,6 +62,8 @@ def load():
         lib.bg_last_kernel_name.restype = ctypes.c_char_p
         lib.bg_last_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
         lib.bg_last_kernel_ms.restype = i
+        lib.bg_class_program_stats.argtypes = [i, i, vp, vp]
+        lib.bg_class_program_stats.restype = i
         lib.bg_destroy.argtypes = [vp]
         lib.bg_strerror.argtypes = [i]
         lib.bg_strerror.restype = ctypes.c_char_p
@@ -159,6 +161,15 @@ def bg_last_kernel_ms(ctx) -> float:
     v = ctypes.c_double()
     _check(load().bg_last_kernel_ms(ctx, ctypes.byref(v)), "bg_last_kernel_ms")
     return v.value
+
+
+def bg_class_program_stats(n: int, lanes: int, counts):
+    """Host-only: (valid, vertex_ops, steps, state_bytes, closure_code) of the class program for a colour multiset."""
+    import numpy as np
+    c = np.ascontiguousarray(counts, dtype=np.int32)
+    out = np.zeros(5, dtype=np.int64)
+    _check(load().bg_class_program_stats(n, lanes, _ptr(c), _ptr(out)), "bg_class_program_stats")
+    return tuple(int(x) for x in out)
 
 
 def bg_destroy(ctx) -> None:

@@ -7,6 +7,7 @@
 #include <vector>
 
 #include "bg_internal.h"
+#include "bg_program.h"
 
 namespace bg {
 
@@ -333,6 +334,24 @@ int bg_colour_matrix(const bg_ctx* c, double* C_host) {
 int bg_build_colour_matrix(int n, double* C_host) {
     if (n < 4 || n > 8 || !C_host) return BG_EINVAL;
     bg::build_colour_matrix(n, C_host);
+    return BG_OK;
+}
+
+int bg_class_program_stats(int n, int lanes, const int* counts, long long* stats) {
+    if (n < 4 || n > 12 || !counts || !stats || lanes < 1 || lanes > 256 || (lanes & (lanes - 1))) return BG_EINVAL;
+    int sum = 0;
+    for (int c = 0; c < bg::kNumCodes; c++) {
+        if (counts[c] < 0) return BG_EINVAL;
+        sum += counts[c];
+    }
+    if (sum != n) return BG_EINVAL;
+    bg::ClassProgram p;
+    bg::build_class(n, lanes, counts, p);
+    stats[0] = p.valid ? 1 : 0;
+    stats[1] = p.n_vertex_ops;
+    stats[2] = p.total_steps;
+    stats[3] = (long long)p.state_cx * 16;
+    stats[4] = p.closure_code;
     return BG_OK;
 }
 
