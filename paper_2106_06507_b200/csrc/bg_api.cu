@@ -123,9 +123,9 @@ int build_colour_matrix(int n, double* C) {
 
 // =========================================== ABI ===========================================================
 // largest n whose colour-class programs are tabulated at bg_init, and the default lanes per event
-static const int kProgMaxN = 10;
+static const int kProgMaxN = 12;
 static int auto_lanes(int n) {
-    static const int lanes[] = {0, 0, 0, 0, 2, 2, 4, 8, 32, 64, 128, 256, 256};
+    static const int lanes[] = {0, 0, 0, 0, 2, 4, 4, 8, 32, 64, 128, 128, 256};
     return lanes[n];
 }
 

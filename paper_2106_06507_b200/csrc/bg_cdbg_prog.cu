@@ -15,7 +15,9 @@
 #include <algorithm>
 #include <cstring>
 #include <new>
+#include <atomic>
 #include <numeric>
+#include <thread>
 #include <vector>
 
 #include "bg_internal.h"
@@ -49,7 +51,8 @@ struct ProgTable {
     long long num_classes;
     int max_state_cx;
     TierInfo tiers;
-    double mean_steps;
+    bool spill;               // largest state blocks exceed shared memory: top of the state in global memory
+    int sm_count;
     ClassInfo* d_info;
     uint32_t* d_sortkey;      // class id -> position in the order the events are grouped by
     ProgOp* d_ops;
@@ -71,7 +74,9 @@ struct ProgParams {
     const uint32_t* order;     // [N] event ids grouped by class
     const uint32_t* bounds;    // [kTiers + 1] positions in `order` where the tiers start (bounds[kTiers] = N)
     int tier;
-    int slab_cx;               // complex doubles of state per event in the slab
+    int slab_cx;               // complex doubles of state per event in the shared-memory slab
+    double2* spill;            // SPILL kernels: global slab, spill_cx complex doubles per block
+    int spill_cx;
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -226,24 +231,42 @@ cdbg_scatter_kernel(long long N, long long num_classes, const uint32_t* __restri
 // ---------------------------------------------------------------------------------------------------------
 // 4. interpreter
 // ---------------------------------------------------------------------------------------------------------
-template <int EPW>
-__device__ __forceinline__ cx lds(const double2* S, int o) {
-    const double2 v = S[o * EPW];
-    return mk(v.x, v.y);
-}
-template <int EPW>
-__device__ __forceinline__ void sts(double2* S, int o, cx v) {
-    S[o * EPW] = make_double2(v.re, v.im);
-}
+// Per-event state block: offsets below `cap` live in shared memory ([offset][event], event fastest); with SPILL
+// the rest (the highest popcount levels, which are read least often) lives in an L2-resident global slab owned by
+// the block, accessed with .cg loads/stores (no stale L1 lines).
+template <int EPW, bool SPILL>
+struct StateRef {
+    double2* S;
+    double2* spill;
+    int cap;
+    __device__ __forceinline__ cx ld(int o) const {
+        if (SPILL && o >= cap) {
+            const double2 v = __ldcg(spill + (o - cap));
+            return mk(v.x, v.y);
+        }
+        const double2 v = S[o * EPW];
+        return mk(v.x, v.y);
+    }
+    __device__ __forceinline__ void st(int o, cx v) const {
+        if (SPILL && o >= cap) {
+            __stcg(spill + (o - cap), make_double2(v.re, v.im));
+            return;
+        }
+        S[o * EPW] = make_double2(v.re, v.im);
+    }
+};
 
-template <int G>
+template <int G, bool SPILL>
 __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgParams p) {
     // G <= 32: one warp per block, EPW = 32/G events per warp.  G > 32: one event per block of G threads.
     constexpr int EPW = G >= 32 ? 1 : 32 / G;
     extern __shared__ double2 smem[];
     const int lane = threadIdx.x;
     const int q = lane % EPW, g = lane / EPW;
-    double2* S = smem + q;
+    StateRef<EPW, SPILL> st_;
+    st_.S = smem + q;
+    st_.spill = SPILL ? p.spill + (size_t)blockIdx.x * p.spill_cx : nullptr;
+    st_.cap = p.slab_cx;
     const long long first = p.bounds[p.tier], end = p.bounds[p.tier + 1];
     const long long ntasks = (end - first + EPW - 1) / EPW;
     const int nlev = 2 * p.n - 4;
@@ -281,10 +304,10 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                 if (flags & OPF_VALID) {
                     cx a[4], b[4];
 #pragma unroll
-                    for (int c = 0; c < 4; c++) { a[c] = lds<EPW>(S, offA + c); b[c] = lds<EPW>(S, offB + c); }
+                    for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); b[c] = st_.ld(offB + c); }
                     double P1[4], P2[4];
                     {
-                        const cx p01 = lds<EPW>(S, offP1), p23 = lds<EPW>(S, offP1 + 1);
+                        const cx p01 = st_.ld(offP1), p23 = st_.ld(offP1 + 1);
                         P1[0] = p01.re; P1[1] = p01.im; P1[2] = p23.re; P1[3] = p23.im;
                     }
                     if (flags & OPF_FIRST) {
@@ -293,7 +316,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
 #pragma unroll
                         for (int c = 0; c < 6; c++) tacc[c] = mk(0.0, 0.0);
                         const int offP2 = (int)(raw.w & 0xFFFF);
-                        const cx p01 = lds<EPW>(S, offP2), p23 = lds<EPW>(S, offP2 + 1);
+                        const cx p01 = st_.ld(offP2), p23 = st_.ld(offP2 + 1);
                         Pt[0] = P1[0] + p01.re; Pt[1] = P1[1] + p01.im; Pt[2] = P1[2] + p23.re; Pt[3] = P1[3] + p23.im;
                     }
 #pragma unroll
@@ -303,27 +326,27 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     if (flags & OPF_TENB) {
                         cx T[6];
 #pragma unroll
-                        for (int c = 0; c < 6; c++) T[c] = lds<EPW>(S, offB + 4 + c);
+                        for (int c = 0; c < 6; c++) T[c] = st_.ld(offB + 4 + c);
                         tcontract_acc(acc, T, a, sign);
                     }
                     if (flags & OPF_TENA) {
                         cx T[6];
 #pragma unroll
-                        for (int c = 0; c < 6; c++) T[c] = lds<EPW>(S, offA + 4 + c);
+                        for (int c = 0; c < 6; c++) T[c] = st_.ld(offA + 4 + c);
                         tcontract_acc(acc, T, b, -sign);
                     }
                     if (!(flags & OPF_CLOSURE)) tbuild_acc(tacc, a, b, sign);
                     if (flags & OPF_PARTIAL) {
                         // chunk of a split target: raw sums to its scratch slot, finished by a COMBINE op
 #pragma unroll
-                        for (int c = 0; c < 4; c++) sts<EPW>(S, offDst + c, acc[c]);
+                        for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
 #pragma unroll
-                        for (int c = 0; c < 6; c++) sts<EPW>(S, offDst + 4 + c, tacc[c]);
+                        for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
                     } else if (flags & OPF_LAST) {
                         if (flags & OPF_CLOSURE) {
                             cx en[4];
 #pragma unroll
-                            for (int c = 0; c < 4; c++) en[c] = lds<EPW>(S, offDst + c);
+                            for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
                             const cx d = mdot(en, acc);
                             amp.re = fma(kInvSqrt2, d.re, amp.re);
                             amp.im = fma(kInvSqrt2, d.im, amp.im);
@@ -335,13 +358,13 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                             for (int c = 0; c < 6; c++) tacc[c] = kInvSqrt2 * tacc[c];
                             if (!(flags & OPF_NOSTORE)) {
 #pragma unroll
-                                for (int c = 0; c < 4; c++) sts<EPW>(S, offDst + c, acc[c]);
+                                for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
 #pragma unroll
-                                for (int c = 0; c < 6; c++) sts<EPW>(S, offDst + 4 + c, tacc[c]);
+                                for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
                             }
                             if (flags & OPF_STOREP) {
-                                sts<EPW>(S, offPt, mk(Pt[0], Pt[1]));
-                                sts<EPW>(S, offPt + 1, mk(Pt[2], Pt[3]));
+                                st_.st(offPt, mk(Pt[0], Pt[1]));
+                                st_.st(offPt + 1, mk(Pt[2], Pt[3]));
                             }
                         }
                     }
@@ -350,35 +373,35 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     cx a[4], x[4], en[4];
                     double P1[4];
 #pragma unroll
-                    for (int c = 0; c < 4; c++) { a[c] = lds<EPW>(S, offA + c); x[c] = mk(0.0, 0.0); }
+                    for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); x[c] = mk(0.0, 0.0); }
                     {
-                        const cx p01 = lds<EPW>(S, offP1), p23 = lds<EPW>(S, offP1 + 1);
+                        const cx p01 = st_.ld(offP1), p23 = st_.ld(offP1 + 1);
                         P1[0] = p01.re; P1[1] = p01.im; P1[2] = p23.re; P1[3] = p23.im;
                     }
                     const double sign = (flags & OPF_NEG) ? -1.0 : 1.0;
                     v3_acc(x, P1, Pt, a, acc, sign);
                     tcontract_acc(x, tacc, a, sign);
 #pragma unroll
-                    for (int c = 0; c < 4; c++) en[c] = lds<EPW>(S, offDst + c);
+                    for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
                     const cx d = mdot(en, x);
                     amp.re = fma(kInvSqrt2, d.re, amp.re);
                     amp.im = fma(kInvSqrt2, d.im, amp.im);
                 } else if (flags & OPF_COMBINE) {
                     // add the offB partial sums of a split target and finish it like a LAST op
 #pragma unroll
-                    for (int c = 0; c < 4; c++) acc[c] = lds<EPW>(S, offA + c);
+                    for (int c = 0; c < 4; c++) acc[c] = st_.ld(offA + c);
 #pragma unroll
-                    for (int c = 0; c < 6; c++) tacc[c] = lds<EPW>(S, offA + 4 + c);
+                    for (int c = 0; c < 6; c++) tacc[c] = st_.ld(offA + 4 + c);
                     for (int r = 1; r < offB; r++) {
 #pragma unroll
-                        for (int c = 0; c < 4; c++) acc[c] = acc[c] + lds<EPW>(S, offA + 10 * r + c);
+                        for (int c = 0; c < 4; c++) acc[c] = acc[c] + st_.ld(offA + 10 * r + c);
 #pragma unroll
-                        for (int c = 0; c < 6; c++) tacc[c] = tacc[c] + lds<EPW>(S, offA + 10 * r + 4 + c);
+                        for (int c = 0; c < 6; c++) tacc[c] = tacc[c] + st_.ld(offA + 10 * r + 4 + c);
                     }
                     {
                         const int offP2 = (int)(raw.w & 0xFFFF);
-                        const cx a01 = lds<EPW>(S, offP1), a23 = lds<EPW>(S, offP1 + 1);
-                        const cx b01 = lds<EPW>(S, offP2), b23 = lds<EPW>(S, offP2 + 1);
+                        const cx a01 = st_.ld(offP1), a23 = st_.ld(offP1 + 1);
+                        const cx b01 = st_.ld(offP2), b23 = st_.ld(offP2 + 1);
                         Pt[0] = a01.re + b01.re; Pt[1] = a01.im + b01.im; Pt[2] = a23.re + b23.re; Pt[3] = a23.im + b23.im;
                     }
                     const double f = kInvSqrt2 / mdot(Pt, Pt);
@@ -388,13 +411,13 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     for (int c = 0; c < 6; c++) tacc[c] = kInvSqrt2 * tacc[c];
                     if (!(flags & OPF_NOSTORE)) {
 #pragma unroll
-                        for (int c = 0; c < 4; c++) sts<EPW>(S, offDst + c, acc[c]);
+                        for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
 #pragma unroll
-                        for (int c = 0; c < 6; c++) sts<EPW>(S, offDst + 4 + c, tacc[c]);
+                        for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
                     }
                     if (flags & OPF_STOREP) {
-                        sts<EPW>(S, offPt, mk(Pt[0], Pt[1]));
-                        sts<EPW>(S, offPt + 1, mk(Pt[2], Pt[3]));
+                        st_.st(offPt, mk(Pt[0], Pt[1]));
+                        st_.st(offPt + 1, mk(Pt[2], Pt[3]));
                     }
                 } else if (flags & OPF_EXT) {
                     const int k = (int)raw.w;
@@ -405,10 +428,10 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     cx eps[4];
                     polarisation(pk, (int)p.hel[(size_t)orig * N + e], eps);
 #pragma unroll
-                    for (int c = 0; c < 4; c++) sts<EPW>(S, offDst + c, eps[c]);
+                    for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
                     if (offPt != 0xFFFF) {
-                        sts<EPW>(S, offPt, mk(pk[0], pk[1]));
-                        sts<EPW>(S, offPt + 1, mk(pk[2], pk[3]));
+                        st_.st(offPt, mk(pk[0], pk[1]));
+                        st_.st(offPt + 1, mk(pk[2], pk[3]));
                     }
                 }
                 raw = nxt;
@@ -462,21 +485,40 @@ int prog_table_create(int n, int G, ProgTable** out) {
     std::vector<ProgOp> ops;
     std::vector<int> steps(nc, 0);
     int max_state = 0;
-    for (long long r = 0; r < nc; r++) {
-        if (class_rank(n, all[r].data()) != r) return BG_EINVAL;
-        ClassProgram cp;
-        build_class(n, G, all[r].data(), cp);
-        ClassInfo& ci = info[r];
-        std::memset(&ci, 0, sizeof(ci));
-        if (!cp.valid) continue;
-        ci.valid = 1;
-        ci.op_base = (uint32_t)ops.size();
-        ci.state_cx = (uint16_t)cp.state_cx;
-        ci.closure_code = (uint8_t)cp.closure_code;
-        for (size_t l = 0; l < cp.level_steps.size(); l++) ci.level_steps[l] = cp.level_steps[l];
-        steps[r] = cp.total_steps;
-        max_state = std::max(max_state, cp.state_cx);
-        ops.insert(ops.end(), cp.ops.begin(), cp.ops.end());
+    {
+        // the programs of different classes are independent: build them on all host cores, then concatenate
+        for (long long r = 0; r < nc; r++)
+            if (class_rank(n, all[r].data()) != r) return BG_EINVAL;
+        std::vector<ClassProgram> progs(nc);
+        std::atomic<long long> next_class{0};
+        auto worker = [&]() {
+            for (long long r = next_class.fetch_add(1); r < nc; r = next_class.fetch_add(1))
+                build_class(n, G, all[r].data(), progs[r]);
+        };
+        unsigned nthreads = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
+        if (n <= 8) nthreads = 1;
+        std::vector<std::thread> pool;
+        for (unsigned i = 1; i < nthreads; i++) pool.emplace_back(worker);
+        worker();
+        for (auto& th : pool) th.join();
+        size_t total_ops = 0;
+        for (auto& cp : progs) total_ops += cp.ops.size();
+        ops.reserve(total_ops + G);
+        for (long long r = 0; r < nc; r++) {
+            ClassProgram& cp = progs[r];
+            ClassInfo& ci = info[r];
+            std::memset(&ci, 0, sizeof(ci));
+            if (!cp.valid) continue;
+            ci.valid = 1;
+            ci.op_base = (uint32_t)ops.size();
+            ci.state_cx = (uint16_t)cp.state_cx;
+            ci.closure_code = (uint8_t)cp.closure_code;
+            for (size_t l = 0; l < cp.level_steps.size(); l++) ci.level_steps[l] = cp.level_steps[l];
+            steps[r] = cp.total_steps;
+            max_state = std::max(max_state, cp.state_cx);
+            ops.insert(ops.end(), cp.ops.begin(), cp.ops.end());
+            std::vector<ProgOp>().swap(cp.ops);
+        }
     }
     // grouping order: longest programs first (the tail of the grid then runs the short ones), invalid last
     std::vector<uint32_t> by(nc), sortkey(nc);
@@ -500,11 +542,22 @@ int prog_table_create(int n, int G, ProgTable** out) {
     for (long long i = nc - 1; i >= 0; i--) tiers.first_key[tier_of[by[i]]] = (int)i;
     for (int k = kTiers - 1; k >= 0; k--) tiers.first_key[k] = std::min(tiers.first_key[k], tiers.first_key[k + 1]);
 
-    if ((size_t)(G >= 32 ? 1 : 32 / G) * max_state * 16 > kMaxSlabBytes) return BG_EUNSUPPORTED;   // one block's slab must fit
+    // A block's slab must fit in shared memory; blocks of >= 128 lanes may keep the top of the state (the highest
+    // levels, read least often) in an L2-resident global slab instead ("spill").
+    const bool spill = (size_t)(G >= 32 ? 1 : 32 / G) * max_state * 16 > kMaxSlabBytes;
+    if (spill && G < 128) return BG_EUNSUPPORTED;
+    if (spill)
+        for (int k = 0; k < kTiers; k++) tiers.slab_cx[k] = std::min<int>(tiers.slab_cx[k], (int)(kMaxSlabBytes / 16));
     ProgTable* t = new (std::nothrow) ProgTable();
     if (!t) return BG_ENOMEM;
     std::memset(t, 0, sizeof(*t));
     t->n = n; t->G = G; t->num_classes = nc; t->max_state_cx = max_state; t->tiers = tiers;
+    t->spill = spill;
+    {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    }
     {   // one spare row of no-ops: the interpreter prefetches one step ahead
         ProgOp nop;
         std::memset(&nop, 0, sizeof(nop));
@@ -541,17 +594,22 @@ void prog_table_destroy(ProgTable* t) {
 size_t prog_state_bytes(const ProgTable* t) { return t ? (size_t)t->max_state_cx * 16 : 0; }
 int prog_lanes(const ProgTable* t) { return t ? t->G : 0; }
 
-// scratch: cls u32[N] | order u32[N] | perm u64[N] | hist u32[num_classes + 1]
+// scratch: cls u32[N] | order u32[N] | perm u64[N] | hist u32[num_classes + 1] | tier bounds | spill slabs
+static size_t prog_spill_offset(const ProgTable* t, long long N) {
+    return (((size_t)N * 16 + ((size_t)t->num_classes + 1) * 4 + 256) + 255) / 256 * 256;
+}
 size_t prog_scratch_bytes(const ProgTable* t, long long N) {
-    return (size_t)N * 16 + ((size_t)t->num_classes + 1) * 4 + 256;
+    // spill kernels run one block per SM, each with a slab for the part of the largest state beyond shared memory
+    const size_t spill = t->spill ? (size_t)t->sm_count * t->max_state_cx * 16 : 0;
+    return prog_spill_offset(t, N) + spill;
 }
 
-template <int G>
+template <int G, bool SPILL>
 static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched) {
     constexpr int EPW = G >= 32 ? 1 : 32 / G, BLOCK = G > 32 ? G : 32;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSlabBytes);
+        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSlabBytes);
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -563,9 +621,10 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         const size_t smem = (size_t)EPW * p.slab_cx * 16;
         if (smem > kMaxSlabBytes) return cudaErrorInvalidValue;
         // resident blocks per SM: shared memory (1 KB reserved per block), and 65536 / (160 x BLOCK) registers
-        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (160 * BLOCK), (228 * 1024) / (smem + 1024)));
+        int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * BLOCK), (228 * 1024) / (smem + 1024)));
+        if (SPILL) per_sm = 1;   // one global slab per SM (prog_scratch_bytes)
         const unsigned blocks = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
-        cdbg_prog_kernel<G><<<blocks, BLOCK, smem, s>>>(p);
+        cdbg_prog_kernel<G, SPILL><<<blocks, BLOCK, smem, s>>>(p);
         ++*launched;
     }
     return cudaGetLastError();
@@ -606,20 +665,28 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.n = t->n; p.N = N; p.mom = mom; p.hel = hel; p.out = out;
     p.info = t->d_info; p.ops = t->d_ops; p.cls = cls; p.perm = perm; p.order = order;
     p.bounds = bounds;
+    p.spill = t->spill ? (double2*)((char*)scratch + prog_spill_offset(t, N)) : nullptr;
+    p.spill_cx = t->max_state_cx;
     p.tier = 0;
     p.slab_cx = t->max_state_cx;
     *launches = 3;
     if (ev0) cudaEventRecord(ev0, s);
     switch (t->G) {
-        case 1: err = launch_interp<1>(s, t, sm_count, p, launches); break;
-        case 2: err = launch_interp<2>(s, t, sm_count, p, launches); break;
-        case 4: err = launch_interp<4>(s, t, sm_count, p, launches); break;
-        case 8: err = launch_interp<8>(s, t, sm_count, p, launches); break;
-        case 16: err = launch_interp<16>(s, t, sm_count, p, launches); break;
-        case 32: err = launch_interp<32>(s, t, sm_count, p, launches); break;
-        case 64: err = launch_interp<64>(s, t, sm_count, p, launches); break;
-        case 128: err = launch_interp<128>(s, t, sm_count, p, launches); break;
-        default: err = launch_interp<256>(s, t, sm_count, p, launches); break;
+        case 1: err = launch_interp<1, false>(s, t, sm_count, p, launches); break;
+        case 2: err = launch_interp<2, false>(s, t, sm_count, p, launches); break;
+        case 4: err = launch_interp<4, false>(s, t, sm_count, p, launches); break;
+        case 8: err = launch_interp<8, false>(s, t, sm_count, p, launches); break;
+        case 16: err = launch_interp<16, false>(s, t, sm_count, p, launches); break;
+        case 32: err = launch_interp<32, false>(s, t, sm_count, p, launches); break;
+        case 64: err = launch_interp<64, false>(s, t, sm_count, p, launches); break;
+        case 128:
+            err = t->spill ? launch_interp<128, true>(s, t, sm_count, p, launches)
+                           : launch_interp<128, false>(s, t, sm_count, p, launches);
+            break;
+        default:
+            err = t->spill ? launch_interp<256, true>(s, t, sm_count, p, launches)
+                           : launch_interp<256, false>(s, t, sm_count, p, launches);
+            break;
     }
     if (ev1) cudaEventRecord(ev1, s);
     return err;
