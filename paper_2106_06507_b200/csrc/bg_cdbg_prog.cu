@@ -28,13 +28,22 @@ namespace bg {
 
 constexpr int kMaxLevels = 2 * kMaxN - 4;   // setup | (main, combine) per popcount 2..n-2 | closure
 
-struct ClassInfo {            // 64 bytes
+struct ClassInfo {            // 64 bytes; the interpreter reads the first 16
     uint32_t op_base;         // first op of the class in the op array (units of ProgOp)
     uint16_t state_cx;
     uint8_t closure_code;
     uint8_t valid;
+    uint32_t total_steps;     // interpreter steps of the whole program
+    uint32_t n_sync;          // how many of them end with a barrier (OPF_SYNC)
     uint16_t level_steps[kMaxLevels];
-    uint16_t pad[28 - kMaxLevels];
+    uint16_t pad[24 - kMaxLevels];
+};
+
+// What the interpreter needs to start an event, in grouping order (written by the scatter kernel).
+struct alignas(16) EventHeader {
+    uint32_t event;           // event id
+    uint32_t cls;             // class id (0xFFFFFFFF: colour codes out of range)
+    uint64_t perm;            // canonical order: nibble k = original index of canonical gluon k
 };
 static_assert(sizeof(ClassInfo) == 64, "ClassInfo layout");
 
@@ -69,10 +78,8 @@ struct ProgParams {
     double* out;
     const ClassInfo* info;
     const ProgOp* ops;
-    const uint32_t* cls;       // [N] class id per event (0xFFFFFFFF: colour codes out of range)
-    const uint64_t* perm;      // [N] canonical order: nibble k = original index of canonical gluon k
-    const uint32_t* order;     // [N] event ids grouped by class
-    const uint32_t* bounds;    // [kTiers + 1] positions in `order` where the tiers start (bounds[kTiers] = N)
+    const EventHeader* hdr;    // [N] events grouped by class
+    const uint32_t* bounds;    // [kTiers + 1] positions in `hdr` where the tiers start (bounds[kTiers] = N)
     int tier;
     int slab_cx;               // complex doubles of state per event in the shared-memory slab
     double2* spill;            // SPILL kernels: global slab, spill_cx complex doubles per block
@@ -195,7 +202,8 @@ cdbg_scan_kernel(uint32_t* __restrict__ hist, int count, TierInfo tiers, uint32_
 template <bool BLOCK_HIST>
 __global__ void __launch_bounds__(kPreThreads)
 cdbg_scatter_kernel(long long N, long long num_classes, const uint32_t* __restrict__ cls,
-                    const uint32_t* __restrict__ sortkey, uint32_t* __restrict__ cursor, uint32_t* __restrict__ order) {
+                    const uint64_t* __restrict__ perm, const uint32_t* __restrict__ sortkey,
+                    uint32_t* __restrict__ cursor, EventHeader* __restrict__ hdr) {
     extern __shared__ uint32_t sh_hist[];
     const int nbins = (int)num_classes + 1;
     uint32_t key[kPrePer], rank[kPrePer];
@@ -211,7 +219,11 @@ cdbg_scatter_kernel(long long N, long long num_classes, const uint32_t* __restri
             const uint32_t c = cls[e];
             key[j] = c == 0xFFFFFFFFu ? (uint32_t)num_classes : sortkey[c];
             if (BLOCK_HIST) rank[j] = atomicAdd(&sh_hist[key[j]], 1u);
-            else order[atomicAdd(&cursor[key[j]], 1u)] = (uint32_t)e;
+            else {
+                EventHeader h;
+                h.event = (uint32_t)e; h.cls = c; h.perm = perm[e];
+                hdr[atomicAdd(&cursor[key[j]], 1u)] = h;
+            }
         }
     }
     if (!BLOCK_HIST) return;
@@ -224,7 +236,11 @@ cdbg_scatter_kernel(long long N, long long num_classes, const uint32_t* __restri
 #pragma unroll
     for (int j = 0; j < kPrePer; j++) {
         const long long e = (long long)blockIdx.x * kPreEvents + j * kPreThreads + threadIdx.x;
-        if (key[j] != 0xFFFFFFFFu) order[sh_hist[key[j]] + rank[j]] = (uint32_t)e;
+        if (key[j] != 0xFFFFFFFFu) {
+            EventHeader h;
+            h.event = (uint32_t)e; h.cls = cls[e]; h.perm = perm[e];
+            hdr[sh_hist[key[j]] + rank[j]] = h;
+        }
     }
 }
 
@@ -269,18 +285,39 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     st_.cap = p.slab_cx;
     const long long first = p.bounds[p.tier], end = p.bounds[p.tier + 1];
     const long long ntasks = (end - first + EPW - 1) / EPW;
-    const int nlev = 2 * p.n - 4;
     const long long N = p.N;
+    const int n = p.n;
+    // lanes of one event (same q) run the same program and meet at its barriers; events of different classes in
+    // one warp pass different numbers of barriers, so the barrier names only the event's own lanes
+    unsigned evmask = 0;
+#pragma unroll
+    for (int i = 0; i < (G < 32 ? G : 32); i++) evmask |= 1u << (q + i * EPW);
 
+    // the header of a task is loaded one task ahead; the inputs of the next task are prefetched into L2 while
+    // the current one computes (events come in class order, so their rows are scattered over the input arrays)
+    EventHeader hnext;
+    hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
+    if ((long long)blockIdx.x < ntasks) {
+        const long long idx = first + (long long)blockIdx.x * EPW + q;
+        if (idx < end) hnext = p.hdr[idx];
+    }
     for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
         const long long idx = first + task * EPW + q;
         const bool have = idx < end;
-        const long long e = have ? (long long)p.order[idx] : 0;
-        const uint32_t cls = have ? p.cls[e] : 0xFFFFFFFFu;
-        const ClassInfo* ci = p.info + (cls == 0xFFFFFFFFu ? 0 : cls);
-        const bool valid = cls != 0xFFFFFFFFu && ci->valid;
-        const uint64_t perm = p.perm[e];
-        const ProgOp* ops = p.ops + ci->op_base + g;
+        const EventHeader h = hnext;
+        {
+            const long long idx2 = idx + (long long)gridDim.x * EPW;
+            hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
+            if (task + gridDim.x < ntasks && idx2 < end) hnext = p.hdr[idx2];
+        }
+        const long long e = h.event;
+        const uint32_t cls = have ? h.cls : 0xFFFFFFFFu;
+        const uint4 ci = __ldg(reinterpret_cast<const uint4*>(p.info + (cls == 0xFFFFFFFFu ? 0 : cls)));
+        const bool valid = cls != 0xFFFFFFFFu && ((ci.y >> 24) & 0xFF);
+        const uint64_t perm = h.perm;
+        const ProgOp* ops = p.ops + ci.x + g;
+        const int total = valid ? (int)ci.z : 0;
+        bool prefetched = false;
 
         cx amp = mk(0.0, 0.0);
         cx acc[4], tacc[6];
@@ -291,9 +328,8 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         for (int c = 0; c < 6; c++) tacc[c] = mk(0.0, 0.0);
 
         uint4 raw = __ldg(reinterpret_cast<const uint4*>(ops));
-        for (int lvl = 0; lvl < nlev; lvl++) {
-            const int steps = valid ? (int)ci->level_steps[lvl] : 0;
-            for (int s = 0; s < steps; s++) {
+        {
+            for (int s = 0; s < total; s++) {
                 ops += G;
                 // the op of the next step (the table ends with one spare row of no-ops)
                 const uint4 nxt = __ldg(reinterpret_cast<const uint4*>(ops));
@@ -434,10 +470,25 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                         st_.st(offPt + 1, mk(pk[2], pk[3]));
                     }
                 }
+                if (flags & OPF_SYNC) {
+                    // end of a level: the currents just written become visible to the lanes of the event
+                    if constexpr (G > 32) __syncthreads(); else __syncwarp(evmask);
+                    if (!prefetched) {
+                        prefetched = true;
+                        if (hnext.cls != 0xFFFFFFFFu) {
+                            // the G lanes share the 4n momentum components and n helicities of the next event
+                            for (int k = g; k < 5 * n; k += G) {
+                                const void* ptr = k < 4 * n ? (const void*)(p.mom + (size_t)k * N + hnext.event)
+                                                            : (const void*)(p.hel + (size_t)(k - 4 * n) * N + hnext.event);
+                                asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
+                            }
+                        }
+                    }
+                }
                 raw = nxt;
             }
-            if constexpr (G > 32) __syncthreads(); else __syncwarp();
         }
+
         // closure amplitude: sum of the G lanes' partial contractions (Eq. 22), then |A|^2
 #pragma unroll
         for (int d = EPW; d < 32; d <<= 1) {
@@ -513,6 +564,8 @@ int prog_table_create(int n, int G, ProgTable** out) {
             ci.op_base = (uint32_t)ops.size();
             ci.state_cx = (uint16_t)cp.state_cx;
             ci.closure_code = (uint8_t)cp.closure_code;
+            ci.total_steps = (uint32_t)cp.total_steps;
+            ci.n_sync = (uint32_t)cp.n_sync;
             for (size_t l = 0; l < cp.level_steps.size(); l++) ci.level_steps[l] = cp.level_steps[l];
             steps[r] = cp.total_steps;
             max_state = std::max(max_state, cp.state_cx);
@@ -594,9 +647,9 @@ void prog_table_destroy(ProgTable* t) {
 size_t prog_state_bytes(const ProgTable* t) { return t ? (size_t)t->max_state_cx * 16 : 0; }
 int prog_lanes(const ProgTable* t) { return t ? t->G : 0; }
 
-// scratch: cls u32[N] | order u32[N] | perm u64[N] | hist u32[num_classes + 1] | tier bounds | spill slabs
+// scratch: headers 16 B x N | perm u64[N] | cls u32[N] | hist u32[num_classes + 1] | tier bounds | spill slabs
 static size_t prog_spill_offset(const ProgTable* t, long long N) {
-    return (((size_t)N * 16 + ((size_t)t->num_classes + 1) * 4 + 256) + 255) / 256 * 256;
+    return (((size_t)N * 28 + ((size_t)t->num_classes + 1) * 4 + 256) + 255) / 256 * 256;
 }
 size_t prog_scratch_bytes(const ProgTable* t, long long N) {
     // spill kernels run one block per SM, each with a slab for the part of the largest state beyond shared memory
@@ -633,10 +686,10 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
 cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
                              const signed char* hel, const signed char* col, double* out, void* scratch,
                              int* launches, cudaEvent_t ev0, cudaEvent_t ev1) {
-    uint32_t* cls = (uint32_t*)scratch;
-    uint32_t* order = cls + N;
-    uint64_t* perm = (uint64_t*)(order + N);   // 2N u32 before it: 8-byte aligned
-    uint32_t* hist = (uint32_t*)(perm + N);
+    EventHeader* hdr = (EventHeader*)scratch;
+    uint64_t* perm = (uint64_t*)(hdr + N);
+    uint32_t* cls = (uint32_t*)(perm + N);
+    uint32_t* hist = cls + N;
     uint32_t* bounds = hist + ((size_t)t->num_classes + 1);
     const int nbins = (int)t->num_classes + 1;
     cudaError_t err = cudaMemsetAsync(hist, 0, sizeof(uint32_t) * nbins, s);
@@ -653,17 +706,17 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         cdbg_classify_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
                                                                       t->d_sortkey, cls, perm, hist);
         cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins, t->tiers, bounds, (uint32_t)N);
-        cdbg_scatter_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(N, t->num_classes, cls, t->d_sortkey, hist, order);
+        cdbg_scatter_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(N, t->num_classes, cls, perm, t->d_sortkey, hist, hdr);
     } else {
         cdbg_classify_kernel<false><<<eb, kPreThreads, 0, s>>>(t->n, N, t->num_classes, col, t->d_info, t->d_sortkey,
                                                                cls, perm, hist);
         cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins, t->tiers, bounds, (uint32_t)N);
-        cdbg_scatter_kernel<false><<<eb, kPreThreads, 0, s>>>(N, t->num_classes, cls, t->d_sortkey, hist, order);
+        cdbg_scatter_kernel<false><<<eb, kPreThreads, 0, s>>>(N, t->num_classes, cls, perm, t->d_sortkey, hist, hdr);
     }
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     ProgParams p;
     p.n = t->n; p.N = N; p.mom = mom; p.hel = hel; p.out = out;
-    p.info = t->d_info; p.ops = t->d_ops; p.cls = cls; p.perm = perm; p.order = order;
+    p.info = t->d_info; p.ops = t->d_ops; p.hdr = hdr;
     p.bounds = bounds;
     p.spill = t->spill ? (double2*)((char*)scratch + prog_spill_offset(t, N)) : nullptr;
     p.spill_cx = t->max_state_cx;

@@ -206,8 +206,13 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
         ProgOp nop;
         std::memset(&nop, 0, sizeof(nop));
         for (size_t s = 0; s < steps; s++)
-            for (int l = 0; l < G; l++) out.ops.push_back(s < lanes[l].size() ? lanes[l][s] : nop);
+            for (int l = 0; l < G; l++) {
+                ProgOp o = s < lanes[l].size() ? lanes[l][s] : nop;
+                if (s + 1 == steps) o.flags |= OPF_SYNC;   // every lane's op of a level's last step carries the barrier
+                out.ops.push_back(o);
+            }
         out.total_steps += (int)steps;
+        if (steps) out.n_sync++;
     };
 
     {   // level 0: external currents and momenta

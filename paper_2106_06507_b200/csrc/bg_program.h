@@ -43,6 +43,7 @@ enum : uint16_t {
     OPF_NOSTORE = 1024,// (with LAST) the finished current stays in registers only (a FUSED op follows)
     OPF_PARTIAL = 2048,// (with LAST) chunk of a split target: raw partial sums -> scratch slot offDst
     OPF_COMBINE = 4096,// add offB partial slots starting at offA, then finish the target like LAST
+    OPF_SYNC = 8192,   // barrier among the lanes of the event after this step (end of a level)
     OPF_EXT = 128      // setup: external current of gluon `extra` -> offDst, its momentum -> offPt
 };
 
@@ -55,6 +56,7 @@ struct ClassProgram {
     int state_cx = 0;            // per-event state size in complex doubles
     int n_vertex_ops = 0;        // number of OPF_VALID ops
     int total_steps = 0;         // sum over levels of max-lane op count
+    int n_sync = 0;              // number of steps that end with a barrier (non-empty levels)
     std::vector<uint16_t> level_steps;   // [2n-4]: setup | (main, combine) for popcount 2..n-2 | closure
     std::vector<ProgOp> ops;             // [total_steps][G]
 };
