@@ -272,6 +272,13 @@ struct StateRef {
     }
 };
 
+__device__ __forceinline__ EventHeader ld_header(const EventHeader* h) {
+    const uint4 v = __ldcg(reinterpret_cast<const uint4*>(h));   // streamed once: not through L1
+    EventHeader r;
+    r.event = v.x; r.cls = v.y; r.perm = (uint64_t)v.z | ((uint64_t)v.w << 32);
+    return r;
+}
+
 template <int G, bool SPILL>
 __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgParams p) {
     // G <= 32: one warp per block, EPW = 32/G events per warp.  G > 32: one event per block of G threads.
@@ -299,7 +306,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
     if ((long long)blockIdx.x < ntasks) {
         const long long idx = first + (long long)blockIdx.x * EPW + q;
-        if (idx < end) hnext = p.hdr[idx];
+        if (idx < end) hnext = ld_header(p.hdr + idx);
     }
     for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
         const long long idx = first + task * EPW + q;
@@ -308,7 +315,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         {
             const long long idx2 = idx + (long long)gridDim.x * EPW;
             hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
-            if (task + gridDim.x < ntasks && idx2 < end) hnext = p.hdr[idx2];
+            if (task + gridDim.x < ntasks && idx2 < end) hnext = ld_header(p.hdr + idx2);
         }
         const long long e = h.event;
         const uint32_t cls = have ? h.cls : 0xFFFFFFFFu;
@@ -328,11 +335,12 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         for (int c = 0; c < 6; c++) tacc[c] = mk(0.0, 0.0);
 
         uint4 raw = __ldg(reinterpret_cast<const uint4*>(ops));
+        uint4 nxt = __ldg(reinterpret_cast<const uint4*>(ops + G));
         {
             for (int s = 0; s < total; s++) {
                 ops += G;
-                // the op of the next step (the table ends with one spare row of no-ops)
-                const uint4 nxt = __ldg(reinterpret_cast<const uint4*>(ops));
+                // ops are fetched two steps ahead (the table ends with two spare rows of no-ops)
+                const uint4 nxt2 = __ldg(reinterpret_cast<const uint4*>(ops + G));
                 const int offA = raw.x & 0xFFFF, offB = raw.x >> 16;
                 const int offP1 = raw.y & 0xFFFF, offDst = raw.y >> 16;
                 const int offPt = raw.z & 0xFFFF;
@@ -460,9 +468,9 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     const int orig = (int)((perm >> (4 * k)) & 0xF);
                     double pk[4];
 #pragma unroll
-                    for (int c = 0; c < 4; c++) pk[c] = p.mom[(size_t)(orig * 4 + c) * N + e];
+                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(p.mom + (size_t)(orig * 4 + c) * N + e);   // L1 is kept for the op stream
                     cx eps[4];
-                    polarisation(pk, (int)p.hel[(size_t)orig * N + e], eps);
+                    polarisation(pk, (int)__ldcg(p.hel + (size_t)orig * N + e), eps);
 #pragma unroll
                     for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
                     if (offPt != 0xFFFF) {
@@ -486,6 +494,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     }
                 }
                 raw = nxt;
+                nxt = nxt2;
             }
         }
 
@@ -611,10 +620,10 @@ int prog_table_create(int n, int G, ProgTable** out) {
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
     }
-    {   // one spare row of no-ops: the interpreter prefetches one step ahead
+    {   // two spare rows of no-ops: the interpreter prefetches two steps ahead
         ProgOp nop;
         std::memset(&nop, 0, sizeof(nop));
-        ops.insert(ops.end(), (size_t)G, nop);
+        ops.insert(ops.end(), (size_t)2 * G, nop);
     }
     t->ops_bytes = ops.size() * sizeof(ProgOp);
     unsigned ms[kMaxN + 1][kNumCodes];
