@@ -188,7 +188,11 @@ int bg_init(bg_ctx** out, int n, int mode) {
         const int rc = bg::prog_table_create(n, auto_lanes(n), &c->prog);
         if (rc != BG_OK) { delete c; return rc; }
     }
-    if (cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking) != cudaSuccess) {
+    bool streams_ok = cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking) == cudaSuccess &&
+                      cudaStreamCreateWithFlags(&c->cstream, cudaStreamNonBlocking) == cudaSuccess;
+    for (int k = 0; k < kHostChunks && streams_ok; k++)
+        streams_ok = cudaEventCreateWithFlags(&c->chunk_ev[k], cudaEventDisableTiming) == cudaSuccess;
+    if (!streams_ok) {
         bg::prog_table_destroy(c->prog);
         bg::cobg_table_destroy(c->cobg);
         if (c->dC) cudaFree(c->dC);
@@ -204,6 +208,9 @@ int bg_destroy(bg_ctx* c) {
     if (!c) return BG_EINVAL;
     cudaStreamSynchronize(c->hstream);
     cudaStreamDestroy(c->hstream);
+    if (c->cstream) { cudaStreamSynchronize(c->cstream); cudaStreamDestroy(c->cstream); }
+    for (int k = 0; k < kHostChunks; k++)
+        if (c->chunk_ev[k]) cudaEventDestroy(c->chunk_ev[k]);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     bg::prog_table_destroy(c->prog);
@@ -423,15 +430,37 @@ int bg_eval_host(bg_ctx* c, long long N, const double* mom, const signed char* h
     int rc = ensure_staging(c, N);
     if (rc != BG_OK) return rc;
     const size_t n = (size_t)c->n;
-    cudaStream_t s = c->hstream;
-    if (cudaMemcpyAsync(c->d_mom, mom, sizeof(double) * 4 * n * N, cudaMemcpyHostToDevice, s) != cudaSuccess) return BG_ECUDA;
-    if (!helsum && cudaMemcpyAsync(c->d_hel, hel, n * N, cudaMemcpyHostToDevice, s) != cudaSuccess) return BG_ECUDA;
-    if ((c->mode & BG_COL_GIVEN) && cudaMemcpyAsync(c->d_col, col, 2 * n * N, cudaMemcpyHostToDevice, s) != cudaSuccess)
-        return BG_ECUDA;
-    rc = bg_eval(c, (void*)s, N, c->d_mom, helsum ? nullptr : c->d_hel, (c->mode & BG_COL_GIVEN) ? c->d_col : nullptr,
-                 c->d_out);
-    if (rc != BG_OK) return rc;
-    if (cudaMemcpyAsync(out, c->d_out, sizeof(double) * N, cudaMemcpyDeviceToHost, s) != cudaSuccess) return BG_ECUDA;
+    const bool colgiven = (c->mode & BG_COL_GIVEN) != 0;
+    cudaStream_t s = c->hstream, cs = c->cstream;
+    // Chunked pipeline: the copy stream runs ahead with the host->device copies of chunk k+1 (one strided 2-D copy
+    // per array: the arrays are event-fastest) while the compute stream evaluates chunk k and returns its results.
+    // Every chunk has its own compact region (event stride = its size) inside the staging buffers.
+    int K = (int)std::min<long long>(kHostChunks, N / 32768);
+    if (K < 1) K = 1;
+    long long chunk = (N + K - 1) / K;
+    chunk = (chunk + 255) / 256 * 256;
+    int launches = 0;
+    int k = 0;
+    for (long long first = 0; first < N; first += chunk, k++) {
+        const long long cnt = std::min(chunk, N - first);
+        double* dm = c->d_mom + 4 * n * first;
+        signed char* dh = c->d_hel + n * first;
+        signed char* dc = c->d_col + 2 * n * first;
+        double* dout = c->d_out + first;
+        if (cudaMemcpy2DAsync(dm, cnt * 8, mom + first, (size_t)N * 8, cnt * 8, 4 * n, cudaMemcpyHostToDevice, cs) != cudaSuccess)
+            return BG_ECUDA;
+        if (!helsum && cudaMemcpy2DAsync(dh, cnt, hel + first, (size_t)N, cnt, n, cudaMemcpyHostToDevice, cs) != cudaSuccess)
+            return BG_ECUDA;
+        if (colgiven && cudaMemcpy2DAsync(dc, cnt, col + first, (size_t)N, cnt, 2 * n, cudaMemcpyHostToDevice, cs) != cudaSuccess)
+            return BG_ECUDA;
+        if (cudaEventRecord(c->chunk_ev[k], cs) != cudaSuccess || cudaStreamWaitEvent(s, c->chunk_ev[k], 0) != cudaSuccess)
+            return BG_ECUDA;
+        rc = bg_eval(c, (void*)s, cnt, dm, helsum ? nullptr : dh, colgiven ? dc : nullptr, dout);
+        if (rc != BG_OK) return rc;
+        launches += c->last_launches;
+        if (cudaMemcpyAsync(out + first, dout, sizeof(double) * cnt, cudaMemcpyDeviceToHost, s) != cudaSuccess) return BG_ECUDA;
+    }
+    c->last_launches = launches;
     if (cudaStreamSynchronize(s) != cudaSuccess) return BG_ECUDA;
     return BG_OK;
 }

@@ -8,6 +8,8 @@
 
 namespace bg { struct ProgTable; struct CobgTable; }
 
+constexpr int kHostChunks = 8;   // bg_eval_host pipelines copies and kernels over up to this many chunks
+
 struct bg_ctx {
     int n;
     int mode;
@@ -23,7 +25,9 @@ struct bg_ctx {
     void* scratch;
     size_t scratch_bytes;
     // host path staging
-    cudaStream_t hstream;
+    cudaStream_t hstream;      // compute + device->host stream of bg_eval_host
+    cudaStream_t cstream;      // host->device copy stream of bg_eval_host (runs ahead of hstream)
+    cudaEvent_t chunk_ev[kHostChunks];
     double* d_mom;
     signed char* d_hel;
     signed char* d_col;
