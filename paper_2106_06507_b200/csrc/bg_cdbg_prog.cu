@@ -40,6 +40,8 @@ struct ClassInfo {            // 64 bytes; the interpreter reads the first 16
 };
 
 // What the interpreter needs to start an event, in grouping order (written by the scatter kernel).
+constexpr int kRecHeaderBytes = 32;
+
 struct alignas(16) EventHeader {
     uint32_t event;           // event id
     uint32_t cls;             // class id (0xFFFFFFFF: colour codes out of range)
@@ -78,8 +80,9 @@ struct ProgParams {
     double* out;
     const ClassInfo* info;
     const ProgOp* ops;
-    const EventHeader* hdr;    // [N] events grouped by class
-    const uint32_t* bounds;    // [kTiers + 1] positions in `hdr` where the tiers start (bounds[kTiers] = N)
+    const char* rec;           // [N] event records (header + canonical momenta) grouped by class
+    int rec_bytes;             // 32 + 32 n
+    const uint32_t* bounds;    // [kTiers + 1] record positions where the tiers start (bounds[kTiers] = N)
     int tier;
     int slab_cx;               // complex doubles of state per event in the shared-memory slab
     double2* spill;            // SPILL kernels: global slab, spill_cx complex doubles per block
@@ -92,7 +95,7 @@ struct ProgParams {
 // Block-level aggregation: sampled colour assignments fall into few classes (92 distinct ones at n = 6), so the
 // class counters are kept in shared memory per block (kPreEvents events) and flushed once; with BLOCK_HIST false
 // (histogram larger than shared memory) the counters are updated in global memory directly.
-constexpr int kPreThreads = 512, kPrePer = 8, kPreEvents = kPreThreads * kPrePer;
+constexpr int kPreThreads = 512, kPrePer = 2, kPreEvents = kPreThreads * kPrePer;
 
 template <bool BLOCK_HIST>
 __global__ void __launch_bounds__(kPreThreads)
@@ -198,12 +201,47 @@ cdbg_scan_kernel(uint32_t* __restrict__ hist, int count, TierInfo tiers, uint32_
     if (threadIdx.x <= kTiers) bounds[threadIdx.x] = threadIdx.x == kTiers ? N : hist[tiers.first_key[threadIdx.x]];
 }
 
-// 3. scatter event ids into class order (each block reserves one range per class it holds)
+// 3. scatter the events into class order.  Each event becomes one contiguous record
+//      [EventHeader, padded to 32 B][momenta of the canonical gluons 0..n-1, 4 doubles = one 32-byte sector each]
+// so that the interpreter reads whole sectors; the inputs are read here in their event-fastest layout (coalesced)
+// and the 8-byte stores of one record merge in L2.  Helicities go into bits 48.. of the header's perm word.
+__device__ __forceinline__ void write_record(int n, long long N, long long e, uint32_t c, uint64_t pm,
+                                             const double* __restrict__ mom, const signed char* __restrict__ hel,
+                                             char* __restrict__ rec) {
+    unsigned inv[kMaxN];                       // original gluon -> canonical position
+    for (int k = 0; k < n; k++) inv[(pm >> (4 * k)) & 0xF] = (unsigned)k;
+    double2* m = reinterpret_cast<double2*>(rec + kRecHeaderBytes);   // 32-byte aligned: one sector per gluon
+    // three gluons (12 coalesced loads) in flight per round
+    for (int j0 = 0; j0 < n; j0 += 3) {
+        double v[3][4];
+        signed char hl[3];
+#pragma unroll
+        for (int u = 0; u < 3; u++) {
+            const int j = j0 + u < n ? j0 + u : n - 1;
+            hl[u] = hel ? hel[(size_t)j * N + e] : (signed char)0;
+#pragma unroll
+            for (int cc = 0; cc < 4; cc++) v[u][cc] = mom[(size_t)(j * 4 + cc) * N + e];
+        }
+#pragma unroll
+        for (int u = 0; u < 3; u++) {
+            if (j0 + u >= n) break;
+            const unsigned k = inv[j0 + u];
+            if (hl[u] > 0) pm |= 1ull << (48 + k);
+            m[k * 2] = make_double2(v[u][0], v[u][1]);
+            m[k * 2 + 1] = make_double2(v[u][2], v[u][3]);
+        }
+    }
+    EventHeader h;
+    h.event = (uint32_t)e; h.cls = c; h.perm = pm;
+    *reinterpret_cast<EventHeader*>(rec) = h;
+}
+
 template <bool BLOCK_HIST>
 __global__ void __launch_bounds__(kPreThreads)
-cdbg_scatter_kernel(long long N, long long num_classes, const uint32_t* __restrict__ cls,
+cdbg_scatter_kernel(int n, long long N, long long num_classes, const uint32_t* __restrict__ cls,
                     const uint64_t* __restrict__ perm, const uint32_t* __restrict__ sortkey,
-                    uint32_t* __restrict__ cursor, EventHeader* __restrict__ hdr) {
+                    const double* __restrict__ mom, const signed char* __restrict__ hel,
+                    uint32_t* __restrict__ cursor, char* __restrict__ rec, int rec_bytes) {
     extern __shared__ uint32_t sh_hist[];
     const int nbins = (int)num_classes + 1;
     uint32_t key[kPrePer], rank[kPrePer];
@@ -219,11 +257,7 @@ cdbg_scatter_kernel(long long N, long long num_classes, const uint32_t* __restri
             const uint32_t c = cls[e];
             key[j] = c == 0xFFFFFFFFu ? (uint32_t)num_classes : sortkey[c];
             if (BLOCK_HIST) rank[j] = atomicAdd(&sh_hist[key[j]], 1u);
-            else {
-                EventHeader h;
-                h.event = (uint32_t)e; h.cls = c; h.perm = perm[e];
-                hdr[atomicAdd(&cursor[key[j]], 1u)] = h;
-            }
+            else write_record(n, N, e, c, perm[e], mom, hel, rec + (size_t)atomicAdd(&cursor[key[j]], 1u) * rec_bytes);
         }
     }
     if (!BLOCK_HIST) return;
@@ -233,14 +267,10 @@ cdbg_scatter_kernel(long long N, long long num_classes, const uint32_t* __restri
         if (c) sh_hist[i] = atomicAdd(&cursor[i], c);
     }
     __syncthreads();
-#pragma unroll
     for (int j = 0; j < kPrePer; j++) {
         const long long e = (long long)blockIdx.x * kPreEvents + j * kPreThreads + threadIdx.x;
-        if (key[j] != 0xFFFFFFFFu) {
-            EventHeader h;
-            h.event = (uint32_t)e; h.cls = cls[e]; h.perm = perm[e];
-            hdr[sh_hist[key[j]] + rank[j]] = h;
-        }
+        if (key[j] != 0xFFFFFFFFu)
+            write_record(n, N, e, cls[e], perm[e], mom, hel, rec + (size_t)(sh_hist[key[j]] + rank[j]) * rec_bytes);
     }
 }
 
@@ -272,7 +302,7 @@ struct StateRef {
     }
 };
 
-__device__ __forceinline__ EventHeader ld_header(const EventHeader* h) {
+__device__ __forceinline__ EventHeader ld_header(const char* h) {
     const uint4 v = __ldcg(reinterpret_cast<const uint4*>(h));   // streamed once: not through L1
     EventHeader r;
     r.event = v.x; r.cls = v.y; r.perm = (uint64_t)v.z | ((uint64_t)v.w << 32);
@@ -306,22 +336,25 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
     if ((long long)blockIdx.x < ntasks) {
         const long long idx = first + (long long)blockIdx.x * EPW + q;
-        if (idx < end) hnext = ld_header(p.hdr + idx);
+        if (idx < end) hnext = ld_header(p.rec + (size_t)idx * p.rec_bytes);
     }
     for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
         const long long idx = first + task * EPW + q;
         const bool have = idx < end;
         const EventHeader h = hnext;
+        long long idx_next = 0;
         {
             const long long idx2 = idx + (long long)gridDim.x * EPW;
             hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
-            if (task + gridDim.x < ntasks && idx2 < end) hnext = ld_header(p.hdr + idx2);
+            idx_next = idx2;
+            if (task + gridDim.x < ntasks && idx2 < end) hnext = ld_header(p.rec + (size_t)idx2 * p.rec_bytes);
         }
         const long long e = h.event;
         const uint32_t cls = have ? h.cls : 0xFFFFFFFFu;
         const uint4 ci = __ldg(reinterpret_cast<const uint4*>(p.info + (cls == 0xFFFFFFFFu ? 0 : cls)));
         const bool valid = cls != 0xFFFFFFFFu && ((ci.y >> 24) & 0xFF);
         const uint64_t perm = h.perm;
+        const double* mrec = reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
         const ProgOp* ops = p.ops + ci.x + g;
         const int total = valid ? (int)ci.z : 0;
         bool prefetched = false;
@@ -465,12 +498,11 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     }
                 } else if (flags & OPF_EXT) {
                     const int k = (int)raw.w;
-                    const int orig = (int)((perm >> (4 * k)) & 0xF);
                     double pk[4];
 #pragma unroll
-                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(p.mom + (size_t)(orig * 4 + c) * N + e);   // L1 is kept for the op stream
+                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + k * 4 + c);   // not through L1: it is kept for the ops
                     cx eps[4];
-                    polarisation(pk, (int)__ldcg(p.hel + (size_t)orig * N + e), eps);
+                    polarisation(pk, ((perm >> (48 + k)) & 1) ? 1 : -1, eps);
 #pragma unroll
                     for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
                     if (offPt != 0xFFFF) {
@@ -484,12 +516,9 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     if (!prefetched) {
                         prefetched = true;
                         if (hnext.cls != 0xFFFFFFFFu) {
-                            // the G lanes share the 4n momentum components and n helicities of the next event
-                            for (int k = g; k < 5 * n; k += G) {
-                                const void* ptr = k < 4 * n ? (const void*)(p.mom + (size_t)k * N + hnext.event)
-                                                            : (const void*)(p.hel + (size_t)(k - 4 * n) * N + hnext.event);
-                                asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
-                            }
+                            // the next event's record (a few 128-byte lines) is pulled into L2 meanwhile
+                            for (int k = g * 128; k < p.rec_bytes; k += G * 128)
+                                asm volatile("prefetch.global.L2 [%0];" ::"l"(p.rec + (size_t)idx_next * p.rec_bytes + k));
                         }
                     }
                 }
@@ -656,9 +685,9 @@ void prog_table_destroy(ProgTable* t) {
 size_t prog_state_bytes(const ProgTable* t) { return t ? (size_t)t->max_state_cx * 16 : 0; }
 int prog_lanes(const ProgTable* t) { return t ? t->G : 0; }
 
-// scratch: headers 16 B x N | perm u64[N] | cls u32[N] | hist u32[num_classes + 1] | tier bounds | spill slabs
+// scratch: records (32 + 32 n) B x N | perm u64[N] | cls u32[N] | hist u32[num_classes + 1] | tier bounds | spill slabs
 static size_t prog_spill_offset(const ProgTable* t, long long N) {
-    return (((size_t)N * 28 + ((size_t)t->num_classes + 1) * 4 + 256) + 255) / 256 * 256;
+    return (((size_t)N * (44 + 32 * t->n) + ((size_t)t->num_classes + 1) * 4 + 256) + 255) / 256 * 256;
 }
 size_t prog_scratch_bytes(const ProgTable* t, long long N) {
     // spill kernels run one block per SM, each with a slab for the part of the largest state beyond shared memory
@@ -695,8 +724,9 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
 cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
                              const signed char* hel, const signed char* col, double* out, void* scratch,
                              int* launches, cudaEvent_t ev0, cudaEvent_t ev1) {
-    EventHeader* hdr = (EventHeader*)scratch;
-    uint64_t* perm = (uint64_t*)(hdr + N);
+    const int rec_bytes = kRecHeaderBytes + 32 * t->n;
+    char* rec = (char*)scratch;
+    uint64_t* perm = (uint64_t*)(rec + (size_t)N * rec_bytes);
     uint32_t* cls = (uint32_t*)(perm + N);
     uint32_t* hist = cls + N;
     uint32_t* bounds = hist + ((size_t)t->num_classes + 1);
@@ -715,17 +745,19 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         cdbg_classify_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
                                                                       t->d_sortkey, cls, perm, hist);
         cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins, t->tiers, bounds, (uint32_t)N);
-        cdbg_scatter_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(N, t->num_classes, cls, perm, t->d_sortkey, hist, hdr);
+        cdbg_scatter_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, cls, perm, t->d_sortkey, mom, hel,
+                                                                     hist, rec, rec_bytes);
     } else {
         cdbg_classify_kernel<false><<<eb, kPreThreads, 0, s>>>(t->n, N, t->num_classes, col, t->d_info, t->d_sortkey,
                                                                cls, perm, hist);
         cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins, t->tiers, bounds, (uint32_t)N);
-        cdbg_scatter_kernel<false><<<eb, kPreThreads, 0, s>>>(N, t->num_classes, cls, perm, t->d_sortkey, hist, hdr);
+        cdbg_scatter_kernel<false><<<eb, kPreThreads, 0, s>>>(t->n, N, t->num_classes, cls, perm, t->d_sortkey, mom, hel, hist,
+                                                              rec, rec_bytes);
     }
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     ProgParams p;
     p.n = t->n; p.N = N; p.mom = mom; p.hel = hel; p.out = out;
-    p.info = t->d_info; p.ops = t->d_ops; p.hdr = hdr;
+    p.info = t->d_info; p.ops = t->d_ops; p.rec = rec; p.rec_bytes = rec_bytes;
     p.bounds = bounds;
     p.spill = t->spill ? (double2*)((char*)scratch + prog_spill_offset(t, N)) : nullptr;
     p.spill_cx = t->max_state_cx;
