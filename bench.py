@@ -29,6 +29,9 @@ sys.path.insert(0, ROOT)
 # mean over sampled colour assignments), and of the colour-ordered configs.
 CDBG_FLOP_PER_EVENT = {4: 2.1e3, 5: 8.4e3, 6: 2.5e4, 7: 7.0e4, 8: 2.2e5, 9: 6.4e5, 10: 1.9e6, 11: 5.1e6, 12: 1.46e7}
 COBG_FLOP_PER_EVENT = {0: 2.6e4, 2: 1.41e6 + 5.8e4}     # config 0 (n=4 helsum), config 2 (n=7 + colour form)
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the recursion kernel launches of ONE step, from the
+# `ncu --set full` captures summarised in profiles/r01_ncu_summary.md (same command, default event counts).
+NCU_TRAFFIC_BYTES = {("cdbg_prog_kernel", 6): 236.2e6, ("cobg_shared_kernel", 7): 334.9e6, ("cdbg_prog_kernel", 9): 393.7e6}
 CONFIG_N = {0: 4, 1: 6, 2: 7, 3: 9}
 CONFIG_EVENTS = {0: 1024, 1: 1 << 20, 2: 1 << 18, 3: 1 << 18, 4: 1 << 16}
 
@@ -143,8 +146,8 @@ def cpu_sample_size(args, n, N):
     """Events per oracle timing sample: about 10-30 s of CPU work (single-core estimates per event)."""
     per_event = {0: 6e-5, 2: 4e-3}.get(args.config)
     if per_event is None:
-        per_event = {4: 1.5e-6, 5: 6e-6, 6: 2.0e-5, 7: 6e-5, 8: 1.8e-4, 9: 5e-4, 10: 1.6e-3, 11: 5e-3, 12: 1.5e-2}[n]
-    return int(max(64, min(N, 20.0 / per_event)))
+        per_event = {4: 1.5e-7, 5: 4e-7, 6: 1.2e-6, 7: 4e-6, 8: 1.2e-5, 9: 4e-5, 10: 1.3e-4, 11: 4e-4, 12: 1.3e-3}[n]
+    return int(max(64, min(N, 15.0 / per_event)))
 
 
 def run_reference(args):
@@ -280,8 +283,10 @@ def run_b200(args):
         if not np.all(np.isfinite(out_host)):
             raise SystemExit("bench.py: non-finite |M|^2 in the output")
         achieved_tf = flop_per_event * N / (kernel_ms * 1e-3) * 1e-12
+        traffic = NCU_TRAFFIC_BYTES.get((kernel_name, n)) if N == CONFIG_EVENTS.get(args.config) else None
         roofline = {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                    "frac": achieved_tf / peak_tf, "traffic": None, "kernel": kernel_name,
+                    "frac": achieved_tf / peak_tf, "traffic": traffic, "traffic_unit": "bytes per step (ncu, "
+                    "profiles/r01_ncu_summary.md)", "kernel": kernel_name,
                     "peak_source": "bg_fp64_peak_probe (DFMA chains, this run); nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2",
                     "flop_per_event": flop_per_event, "kernel_ms": kernel_ms,
                     "kernel_share_of_step": kernel_ms / (total_ms / args.steps)}
