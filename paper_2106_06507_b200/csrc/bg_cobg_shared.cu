@@ -53,13 +53,15 @@ struct CobgParams {
 // ---------------------------------------------------------------------------------------------------------
 // device side
 // ---------------------------------------------------------------------------------------------------------
+constexpr int kSlotStride = 5;   // complex doubles between slots: 4 of data + 1 of padding (odd: spreads the bank groups)
+
 __device__ __forceinline__ void lds_cur(const double* cur, int slot, cx* v) {
-    const double2* p = reinterpret_cast<const double2*>(cur + (size_t)slot * 8);
+    const double2* p = reinterpret_cast<const double2*>(cur + (size_t)slot * (2 * kSlotStride));
 #pragma unroll
     for (int c = 0; c < 4; c++) { const double2 t = p[c]; v[c] = mk(t.x, t.y); }
 }
 __device__ __forceinline__ void sts_cur(double* cur, int slot, const cx* v) {
-    double2* p = reinterpret_cast<double2*>(cur + (size_t)slot * 8);
+    double2* p = reinterpret_cast<double2*>(cur + (size_t)slot * (2 * kSlotStride));
 #pragma unroll
     for (int c = 0; c < 4; c++) p[c] = make_double2(v[c].re, v[c].im);
 }
@@ -139,9 +141,9 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
     const int evl = threadIdx.x / TPE, t = threadIdx.x % TPE;
     const int np = p.np;
     // per-event shared block: currents | subset momenta | eps_n | amplitudes | reduction scratch
-    const int ev_doubles = p.nslots * 8 + NSUB * 4 + 8 + np * 2 + 8;
+    const int ev_doubles = p.nslots * 2 * kSlotStride + NSUB * 4 + 8 + np * 2 + 8;
     double* cur = smem_d + (size_t)evl * ev_doubles;
-    double* P = cur + p.nslots * 8;
+    double* P = cur + p.nslots * 2 * kSlotStride;
     double* epsn = P + NSUB * 4;
     double* A = epsn + 8;
     double* red = A + np * 2;
@@ -305,20 +307,30 @@ int cobg_table_create(int n, CobgTable** out) {
     CobgTable* t = new (std::nothrow) CobgTable();
     if (!t) return BG_ENOMEM;
     std::memset(t, 0, sizeof(*t));
-    std::map<std::vector<int>, int> ids;
+    // Slot numbering: inside a level, sequences are ordered by (set of gluons, lexicographic order).  Threads
+    // sigma, sigma+1, .. (orderings in lexicographic order) then read runs of consecutive slots, which fall into
+    // different shared-memory bank groups (slots are kSlotStride complex doubles apart, an odd number).
     int next = 0;
     t->level_begin[0] = t->level_begin[1] = 0;
     for (int L = 1; L <= ls; L++) {
         t->level_begin[L] = (int)lower.size();
+        std::map<std::pair<unsigned, std::vector<int>>, uint32_t> reps;   // (mask, sequence) -> representative range
         for (int s = 0; s < np; s++)
             for (int i = 0; i + L <= m; i++) {
                 const std::vector<int> seq(ords[s].begin() + i, ords[s].begin() + i + L);
-                auto it = ids.find(seq);
-                if (it == ids.end()) {
-                    it = ids.emplace(seq, next++).first;
-                    lower.push_back((uint32_t)(s << 8 | i << 4 | (i + L - 1)));
-                }
-                slot[((size_t)s * m + i) * m + i + L - 1] = (uint16_t)it->second;
+                unsigned mask = 0;
+                for (int g : seq) mask |= 1u << g;
+                reps.emplace(std::make_pair(mask, seq), (uint32_t)(s << 8 | i << 4 | (i + L - 1)));
+            }
+        std::map<std::vector<int>, int> ids;
+        for (auto& kv : reps) {
+            ids.emplace(kv.first.second, next++);
+            lower.push_back(kv.second);
+        }
+        for (int s = 0; s < np; s++)
+            for (int i = 0; i + L <= m; i++) {
+                const std::vector<int> seq(ords[s].begin() + i, ords[s].begin() + i + L);
+                slot[((size_t)s * m + i) * m + i + L - 1] = (uint16_t)ids[seq];
             }
     }
     for (int L = ls + 1; L <= kCobgMaxM + 1; L++) t->level_begin[L] = (int)lower.size();
@@ -347,12 +359,12 @@ void cobg_table_destroy(CobgTable* t) {
     delete t;
 }
 
-size_t cobg_shared_current_bytes(const CobgTable* t) { return t ? (size_t)t->nslots * 64 : 0; }
+size_t cobg_shared_current_bytes(const CobgTable* t) { return t ? (size_t)t->nslots * 16 * kSlotStride : 0; }
 
 template <int NG, int TPE>
 static cudaError_t launch_cobg(cudaStream_t s, const CobgParams& p) {
     constexpr int EPB = 128 / TPE, NSUB = 1 << (NG - 1);
-    const size_t smem = (size_t)EPB * (p.nslots * 8 + NSUB * 4 + 8 + p.np * 2 + 8) * sizeof(double);
+    const size_t smem = (size_t)EPB * (p.nslots * 2 * kSlotStride + NSUB * 4 + 8 + p.np * 2 + 8) * sizeof(double);
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(cobg_shared_kernel<NG, TPE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
