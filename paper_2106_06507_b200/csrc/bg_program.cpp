@@ -199,6 +199,52 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
     out.level_steps.assign(2 * m - 2, 0);   // setup | (main, combine) per popcount 2..n-2 | closure
 
     // ---- phase 4: deal the work of every level over the G lanes and emit ----
+    // Shared-memory bank groups: the state is laid out [offset][event] in 16-byte elements, so the 8 lanes of a
+    // quarter-warp (EPW events x 8/EPW lanes of each) hit distinct bank groups iff the lanes of one event read
+    // offsets that differ modulo 8/EPW.  The order of the vertices inside a unit is free, so every lane picks, step
+    // by step, the remaining vertex of its unit that collides least with what its neighbours read at that step.
+    auto reduce_bank_conflicts = [&](std::vector<std::vector<ProgOp>>& lanes) {
+        const int EPW = G >= 32 ? 1 : 32 / G;
+        const int M = 8 / EPW, group = 8 / EPW;
+        if (M <= 1 || G < group) return;
+        size_t steps = 0;
+        for (auto& l : lanes) steps = std::max(steps, l.size());
+        auto swap_operands = [](ProgOp& x, ProgOp& y) {
+            std::swap(x.offA, y.offA); std::swap(x.offB, y.offB); std::swap(x.offP1, y.offP1); std::swap(x.extra, y.extra);
+            const uint16_t keep = OPF_NEG | OPF_TENA | OPF_TENB;
+            const uint16_t fx = x.flags & keep, fy = y.flags & keep;
+            x.flags = (uint16_t)((x.flags & ~keep) | fy);
+            y.flags = (uint16_t)((y.flags & ~keep) | fx);
+        };
+        for (size_t s = 0; s < steps; s++)
+            for (int g0 = 0; g0 < G; g0 += group)
+                for (int l = g0 + 1; l < std::min(G, g0 + group); l++) {
+                    auto& ln = lanes[l];
+                    if (s >= ln.size() || !(ln[s].flags & OPF_VALID)) continue;
+                    // the unit that contains step s ends at the next LAST flag
+                    size_t last = s;
+                    while (!(ln[last].flags & OPF_LAST)) last++;
+                    auto cost = [&](const ProgOp& o) {
+                        int c = 0;
+                        for (int j = g0; j < l; j++) {
+                            if (s >= lanes[j].size() || !(lanes[j][s].flags & OPF_VALID)) continue;
+                            const ProgOp& r = lanes[j][s];
+                            if (o.offA != r.offA && o.offA % M == r.offA % M) c += 10;
+                            if (o.offB != r.offB && o.offB % M == r.offB % M) c += 10;
+                            if (o.offP1 != r.offP1 && o.offP1 % M == r.offP1 % M) c += 2;
+                        }
+                        return c;
+                    };
+                    size_t best = s;
+                    int best_cost = cost(ln[s]);
+                    for (size_t c = s + 1; c <= last && best_cost > 0; c++) {
+                        const int cc = cost(ln[c]);
+                        if (cc < best_cost) { best_cost = cc; best = c; }
+                    }
+                    if (best != s) swap_operands(ln[s], ln[best]);
+                }
+    };
+
     auto emit_level = [&](int lvl, std::vector<std::vector<ProgOp>>& lanes) {
         size_t steps = 0;
         for (auto& l : lanes) steps = std::max(steps, l.size());
@@ -288,6 +334,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
             }
             for (auto& l : lanes)
                 if (!l.empty()) { l.front().flags |= OPF_FIRST; l.back().flags |= OPF_LAST; }
+            reduce_bank_conflicts(lanes);
             emit_level(2 * (pc - 2) + 1, lanes);
             break;
         }
@@ -357,6 +404,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
                 out.n_vertex_ops++;
             }
         }
+        reduce_bank_conflicts(lanes);
         emit_level(2 * (pc - 2) + 1, lanes);
         emit_level(2 * (pc - 2) + 2, clanes);
     }
