@@ -302,6 +302,12 @@ struct StateRef {
     }
 };
 
+// v or -v: flips the sign bits when m = 0x80000000 (integer pipe)
+__device__ __forceinline__ cx cneg(cx v, int m) {
+    return mk(__hiloint2double(__double2hiint(v.re) ^ m, __double2loint(v.re)),
+              __hiloint2double(__double2hiint(v.im) ^ m, __double2loint(v.im)));
+}
+
 __device__ __forceinline__ EventHeader ld_header(const char* h) {
     const uint4 v = __ldcg(reinterpret_cast<const uint4*>(h));   // streamed once: not through L1
     EventHeader r;
@@ -398,21 +404,25 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     }
 #pragma unroll
                     for (int c = 0; c < 4; c++) P2[c] = Pt[c] - P1[c];
-                    const double sign = (flags & OPF_NEG) ? -1.0 : 1.0;
-                    v3_acc(acc, P1, P2, a, b, sign);
+                    // X(a,b) is linear in the pair (a, T_a): a negative vertex flips the sign bits of that pair
+                    // (integer pipe) instead of multiplying every term by -1 on the FP64 pipe
+                    const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
+#pragma unroll
+                    for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
+                    v3_acc(acc, P1, P2, a, b, 1.0);
                     if (flags & OPF_TENB) {
                         cx T[6];
 #pragma unroll
                         for (int c = 0; c < 6; c++) T[c] = st_.ld(offB + 4 + c);
-                        tcontract_acc(acc, T, a, sign);
+                        tcontract_acc(acc, T, a, 1.0);
                     }
                     if (flags & OPF_TENA) {
                         cx T[6];
 #pragma unroll
-                        for (int c = 0; c < 6; c++) T[c] = st_.ld(offA + 4 + c);
-                        tcontract_acc(acc, T, b, -sign);
+                        for (int c = 0; c < 6; c++) T[c] = cneg(st_.ld(offA + 4 + c), neg);
+                        tcontract_acc(acc, T, b, -1.0);
                     }
-                    if (!(flags & OPF_CLOSURE)) tbuild_acc(tacc, a, b, sign);
+                    if (!(flags & OPF_CLOSURE)) tbuild_acc(tacc, a, b, 1.0);
                     if (flags & OPF_PARTIAL) {
                         // chunk of a split target: raw sums to its scratch slot, finished by a COMBINE op
 #pragma unroll
@@ -455,9 +465,11 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                         const cx p01 = st_.ld(offP1), p23 = st_.ld(offP1 + 1);
                         P1[0] = p01.re; P1[1] = p01.im; P1[2] = p23.re; P1[3] = p23.im;
                     }
-                    const double sign = (flags & OPF_NEG) ? -1.0 : 1.0;
-                    v3_acc(x, P1, Pt, a, acc, sign);
-                    tcontract_acc(x, tacc, a, sign);
+                    const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
+#pragma unroll
+                    for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
+                    v3_acc(x, P1, Pt, a, acc, 1.0);
+                    tcontract_acc(x, tacc, a, 1.0);
 #pragma unroll
                     for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
                     const cx d = mdot(en, x);
