@@ -341,27 +341,50 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
         long long total = 0;
         for (auto& t : tg) total += (long long)t.ops.size() + (t.fused ? 1 : 0);
         const int ideal = (int)((total + G - 1) / G);
-        const int chunk_max = std::max(ideal, 2);
+        auto ucost = [&](const Unit& u) { return u.count + (u.part < 0 && tg[u.target].fused ? 1 : 0); };
+        // Units no larger than chunk_max vertices; the number of steps the level then needs (longest-processing-
+        // time rule).  A chunk size equal to the ideal step count often leaves slightly more units than lanes and costs a
+        // second round, so slightly larger sizes are tried and the one with the fewest steps (then chunks) is kept.
         std::vector<Unit> units;
-        std::vector<int> nparts(tg.size(), 0), part0(tg.size(), -1);
+        std::vector<int> nparts, part0;
         int nscratch = 0;
-        for (size_t i = 0; i < tg.size(); i++) {
-            const int c = (int)tg[i].ops.size();
-            if (G == 1 || c + (tg[i].fused ? 1 : 0) <= chunk_max || c < 4) {
-                units.push_back({(int)i, 0, c, -1});
-                continue;
+        auto plan = [&](int chunk_max) {
+            units.clear();
+            nparts.assign(tg.size(), 0);
+            part0.assign(tg.size(), -1);
+            nscratch = 0;
+            for (size_t i = 0; i < tg.size(); i++) {
+                const int c = (int)tg[i].ops.size();
+                if (G == 1 || c + (tg[i].fused ? 1 : 0) <= chunk_max || c < 4) {
+                    units.push_back({(int)i, 0, c, -1});
+                    continue;
+                }
+                const int r = (c + chunk_max - 1) / chunk_max;
+                nparts[i] = r;
+                part0[i] = nscratch;
+                for (int k = 0; k < r; k++) {
+                    const int lo = (int)((long long)c * k / r), hi = (int)((long long)c * (k + 1) / r);
+                    units.push_back({(int)i, lo, hi - lo, nscratch++});
+                }
             }
-            const int r = (c + chunk_max - 1) / chunk_max;
-            nparts[i] = r;
-            part0[i] = nscratch;
-            for (int k = 0; k < r; k++) {
-                const int lo = (int)((long long)c * k / r), hi = (int)((long long)c * (k + 1) / r);
-                units.push_back({(int)i, lo, hi - lo, nscratch++});
+            std::stable_sort(units.begin(), units.end(), [&](const Unit& a, const Unit& b) { return ucost(a) > ucost(b); });
+            std::vector<int> ld(G, 0);
+            for (auto& u : units) *std::min_element(ld.begin(), ld.end()) += ucost(u);
+            return *std::max_element(ld.begin(), ld.end());
+        };
+        {
+            int best_chunk = std::max(ideal, 2), best_steps = -1, best_scratch = 0;
+            for (int extra = 0; extra <= 3; extra++) {
+                const int chunk = std::max(ideal, 2) + extra;
+                const int steps = plan(chunk);
+                if (best_steps < 0 || steps < best_steps || (steps == best_steps && nscratch < best_scratch)) {
+                    best_steps = steps; best_chunk = chunk; best_scratch = nscratch;
+                }
+                if (G == 1 || steps <= ideal) break;
             }
+            plan(best_chunk);
         }
         scratch_max = std::max(scratch_max, nscratch * 10);
-        auto ucost = [&](const Unit& u) { return u.count + (u.part < 0 && tg[u.target].fused ? 1 : 0); };
-        std::stable_sort(units.begin(), units.end(), [&](const Unit& a, const Unit& b) { return ucost(a) > ucost(b); });
         std::vector<int> load(G, 0);
         for (auto& u : units) {
             const int l = (int)(std::min_element(load.begin(), load.end()) - load.begin());
