@@ -47,6 +47,7 @@ def parse_args():
     ap.add_argument("--events", type=int, default=None, help="override the number of events per step and GPU")
     ap.add_argument("--kernel", type=int, default=0, help="BG_OPT_KERNEL (0 auto, 1 generic, 2 class programs)")
     ap.add_argument("--lanes", type=int, default=None, help="BG_OPT_LANES (lanes per event, class-program kernel)")
+    ap.add_argument("--smem-limit", type=int, default=None, help="BG_OPT_SMEM_LIMIT in bytes (spill threshold)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -217,6 +218,8 @@ def run_b200(args):
         bg.bg_set_option(ctx, bg.BG_OPT_KERNEL, args.kernel)
     if args.lanes is not None:
         bg.bg_set_option(ctx, bg.BG_OPT_LANES, args.lanes)
+    if args.smem_limit is not None:
+        bg.bg_set_option(ctx, bg.BG_OPT_SMEM_LIMIT, args.smem_limit)
     bg.bg_reserve(ctx, N)
     stream = torch.cuda.current_stream()
     sh = stream.cuda_stream

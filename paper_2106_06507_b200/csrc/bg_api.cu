@@ -125,9 +125,12 @@ int build_colour_matrix(int n, double* C) {
 // largest n whose colour-class programs are tabulated at bg_init, and the default lanes per event
 static const int kProgMaxN = 12;
 static int auto_lanes(int n) {
-    static const int lanes[] = {0, 0, 0, 0, 2, 4, 4, 8, 32, 64, 128, 128, 256};
+    static const int lanes[] = {0, 0, 0, 0, 2, 4, 4, 8, 32, 64, 128, 128, 128};
     return lanes[n];
 }
+
+// shared memory one event's state may take before its top levels spill to global memory (0 = all of it)
+static size_t auto_slab_limit(int n) { return n >= 11 ? (size_t)112 * 1024 : 0; }   // two blocks per SM, measured
 
 static bool mode_supported(int n, int mode) {
     if (n < 4 || n > 12) return false;
@@ -185,7 +188,7 @@ int bg_init(bg_ctx** out, int n, int mode) {
         if (rc != BG_OK) { cudaFree(c->dC); std::free(c->hC); delete c; return rc; }
     }
     if (mode == BG_CDBG_GIVEN && n <= kProgMaxN) {
-        const int rc = bg::prog_table_create(n, auto_lanes(n), &c->prog);
+        const int rc = bg::prog_table_create(n, auto_lanes(n), auto_slab_limit(n), &c->prog);
         if (rc != BG_OK) { delete c; return rc; }
     }
     bool streams_ok = cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking) == cudaSuccess &&
@@ -309,10 +312,23 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
             if (c->prog && bg::prog_lanes(c->prog) == G) return BG_OK;
             cudaDeviceSynchronize();
             bg::ProgTable* t = nullptr;
-            const int rc = bg::prog_table_create(c->n, G, &t);
+            const int rc = bg::prog_table_create(c->n, G, c->slab_limit ? c->slab_limit : auto_slab_limit(c->n), &t);
             if (rc != BG_OK) return rc;
             bg::prog_table_destroy(c->prog);
             c->prog = t;
+            c->prog_lanes = G;
+            return BG_OK;
+        }
+        case BG_OPT_SMEM_LIMIT: {
+            if (c->mode != BG_CDBG_GIVEN || c->n > kProgMaxN || !c->prog) return BG_EUNSUPPORTED;
+            if (value != 0 && (value < 16 * 1024 || value > 222 * 1024)) return BG_EINVAL;
+            cudaDeviceSynchronize();
+            bg::ProgTable* t = nullptr;
+            const int rc = bg::prog_table_create(c->n, bg::prog_lanes(c->prog), value ? (size_t)value : auto_slab_limit(c->n), &t);
+            if (rc != BG_OK) return rc;
+            bg::prog_table_destroy(c->prog);
+            c->prog = t;
+            c->slab_limit = (size_t)value;
             return BG_OK;
         }
         case BG_OPT_TIMING:

@@ -62,7 +62,8 @@ struct ProgTable {
     long long num_classes;
     int max_state_cx;
     TierInfo tiers;
-    bool spill;               // largest state blocks exceed shared memory: top of the state in global memory
+    bool spill;               // largest state blocks exceed the slab limit: top of the state in global memory
+    int spill_blocks_per_sm;  // resident blocks per SM of the spill kernels (each owns one global slab)
     int sm_count;
     ClassInfo* d_info;
     uint32_t* d_sortkey;      // class id -> position in the order the events are grouped by
@@ -574,7 +575,8 @@ static void enumerate_counts(int t, int r, int* counts, std::vector<std::vector<
     }
 }
 
-int prog_table_create(int n, int G, ProgTable** out) {
+int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out) {
+    if (slab_limit == 0 || slab_limit > kMaxSlabBytes) slab_limit = kMaxSlabBytes;
     *out = nullptr;
     if (n < 4 || n > kMaxN || (G != 1 && G != 2 && G != 4 && G != 8 && G != 16 && G != 32 && G != 64 && G != 128 && G != 256)) return BG_EINVAL;
     std::vector<std::vector<int>> all;
@@ -647,15 +649,20 @@ int prog_table_create(int n, int G, ProgTable** out) {
 
     // A block's slab must fit in shared memory; blocks of >= 128 lanes may keep the top of the state (the highest
     // levels, read least often) in an L2-resident global slab instead ("spill").
-    const bool spill = (size_t)(G >= 32 ? 1 : 32 / G) * max_state * 16 > kMaxSlabBytes;
+    const bool spill = (size_t)(G >= 32 ? 1 : 32 / G) * max_state * 16 > slab_limit;
     if (spill && G < 128) return BG_EUNSUPPORTED;
     if (spill)
-        for (int k = 0; k < kTiers; k++) tiers.slab_cx[k] = std::min<int>(tiers.slab_cx[k], (int)(kMaxSlabBytes / 16));
+        for (int k = 0; k < kTiers; k++) tiers.slab_cx[k] = std::min<int>(tiers.slab_cx[k], (int)(slab_limit / 16));
     ProgTable* t = new (std::nothrow) ProgTable();
     if (!t) return BG_ENOMEM;
     std::memset(t, 0, sizeof(*t));
     t->n = n; t->G = G; t->num_classes = nc; t->max_state_cx = max_state; t->tiers = tiers;
     t->spill = spill;
+    {   // blocks of the largest tier that fit an SM (shared memory and registers)
+        const size_t smem0 = (size_t)tiers.slab_cx[0] * 16;
+        const int block = G > 32 ? G : 32;
+        t->spill_blocks_per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * block), (228 * 1024) / (smem0 + 1024)));
+    }
     {
         int dev = 0;
         cudaGetDevice(&dev);
@@ -703,7 +710,7 @@ static size_t prog_spill_offset(const ProgTable* t, long long N) {
 }
 size_t prog_scratch_bytes(const ProgTable* t, long long N) {
     // spill kernels run one block per SM, each with a slab for the part of the largest state beyond shared memory
-    const size_t spill = t->spill ? (size_t)t->sm_count * t->max_state_cx * 16 : 0;
+    const size_t spill = t->spill ? (size_t)t->sm_count * t->spill_blocks_per_sm * t->max_state_cx * 16 : 0;
     return prog_spill_offset(t, N) + spill;
 }
 
@@ -725,7 +732,7 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         if (smem > kMaxSlabBytes) return cudaErrorInvalidValue;
         // resident blocks per SM: shared memory (1 KB reserved per block), and 65536 / (160 x BLOCK) registers
         int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * BLOCK), (228 * 1024) / (smem + 1024)));
-        if (SPILL) per_sm = 1;   // one global slab per SM (prog_scratch_bytes)
+        if (SPILL) per_sm = std::min(per_sm, t->spill_blocks_per_sm);   // one global slab per resident block
         const unsigned blocks = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
         cdbg_prog_kernel<G, SPILL><<<blocks, BLOCK, smem, s>>>(p);
         ++*launched;

@@ -37,6 +37,7 @@ struct bg_ctx {
     bg::ProgTable* prog;
     bg::CobgTable* cobg;       // sequence tables of the shared-current COBG kernel (n <= 7)
     int prog_lanes;            // BG_OPT_LANES (0 = automatic)
+    size_t slab_limit;         // BG_OPT_SMEM_LIMIT (0 = all of shared memory)
     // bookkeeping
     int timing;                // BG_OPT_TIMING
     cudaEvent_t ev0, ev1;
@@ -57,7 +58,7 @@ cudaError_t cobg_generic_launch(cudaStream_t s, int n, bool helsum, int nperm, c
                                 const double* mom, const signed char* hel, double* out);
 
 // ---- colour-class program interpreter (bg_cdbg_prog.cu): G lanes per event, currents in shared memory -------
-int prog_table_create(int n, int G, ProgTable** out);      // BG_* code
+int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out);   // BG_* code; slab_limit 0 = all of shared memory
 void prog_table_destroy(ProgTable* t);
 size_t prog_state_bytes(const ProgTable* t);               // largest per-event state block
 int prog_lanes(const ProgTable* t);
