@@ -152,6 +152,31 @@ def test_program_interpreter_block_per_event(bg, oracle, wl, n, N, lanes):
     check_cdbg(oracle, ev, got)
 
 
+@pytest.mark.parametrize("n,N,lanes,limit", [(8, 131, 128, 16384), (10, 67, 128, 57344), (10, 67, 256, 32768),
+                                             (12, 35, 128, 114688), (12, 35, 256, 0)])
+def test_program_interpreter_spill(bg, oracle, wl, n, N, lanes, limit):
+    """State beyond the shared-memory limit lives in the L2-resident global slab (top levels of the recursion)."""
+    ev = wl.config_events(4, N=N, n=n)
+    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=2, lanes=lanes, smem_limit=limit)
+    assert name == "cdbg_prog_kernel"
+    check_cdbg(oracle, ev, got)
+
+
+def test_program_interpreter_is_deterministic(bg, wl):
+    """Events are regrouped with atomics (their order inside a class varies), but every event runs the same
+    program on the same inputs: repeated calls and different batch compositions give identical bits."""
+    ev = wl.config_events(1, N=20000)
+    a, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
+    b, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
+    assert np.array_equal(a, b)
+    c, _ = gpu_eval(ev.take(np.arange(0, 20000, 3)), bg.BG_CDBG_GIVEN)
+    assert np.array_equal(a[::3], c)
+    ev9 = wl.config_events(3, N=600)
+    a, _ = gpu_eval(ev9, bg.BG_CDBG_GIVEN)
+    c, _ = gpu_eval(ev9.take(np.arange(599, -1, -1)), bg.BG_CDBG_GIVEN)
+    assert np.array_equal(a[::-1], c)
+
+
 def test_cdbg_helicity_sum_mode(bg, oracle, wl):
     import itertools
     ev = wl.config_events(4, N=40, n=5)
