@@ -191,9 +191,12 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
     const int off_epsn = next;
     next += 4;
     for (int k = 0; k < m; k++) { poff[1 << k] = next; next += 2; }
+    // With fewer than 8 events per warp the bank group of an element depends on its offset: one element of padding
+    // after every entry makes the entry starts run through all residues (10 + 2 would only ever give multiples of 4).
+    const int pad = G >= 8 ? 1 : 0;
     for (int pc = 2; pc < m; pc++)
         for (auto& t : levels[pc]) {
-            if (!t.fused) { off[t.pi * 3 + t.slot()] = next; next += 10; }
+            if (!t.fused) { off[t.pi * 3 + t.slot()] = next; next += 10 + pad; }
             if (need_p[t.pi] && poff[t.pi] < 0) { poff[t.pi] = next; next += 2; t.store_p = true; }
         }
     out.level_steps.assign(2 * m - 2, 0);   // setup | (main, combine) per popcount 2..n-2 | closure
