@@ -130,7 +130,7 @@ static int auto_lanes(int n) {
 }
 
 // shared memory one event's state may take before its top levels spill to global memory (0 = all of it)
-static size_t auto_slab_limit(int n) { return n >= 11 ? (size_t)112 * 1024 : 0; }   // two blocks per SM, measured
+static size_t auto_slab_limit(int n) { return n >= 11 ? (size_t)104 * 1024 : 0; }   // two blocks per SM (with their op rings), measured
 
 static bool mode_supported(int n, int mode) {
     if (n < 4 || n > 12) return false;

@@ -49,7 +49,7 @@ struct alignas(16) EventHeader {
 };
 static_assert(sizeof(ClassInfo) == 64, "ClassInfo layout");
 
-constexpr size_t kMaxSlabBytes = 226 * 1024;   // dynamic shared memory per block (1 KB left for static use)
+constexpr size_t kMaxSlabBytes = 208 * 1024;   // state slab per block (the rest: op ring up to 16 KB, static use)
 constexpr int kTiers = 4;     // classes are grouped by state size so that small ones get more warps per SM
 
 struct TierInfo {
@@ -303,6 +303,13 @@ struct StateRef {
     }
 };
 
+constexpr int kRing = 4;   // op ring per lane: ops are requested kRing - 1 steps before they run
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(gmem_src) : "memory");
+}
+
 // v or -v: flips the sign bits when m = 0x80000000 (integer pipe)
 __device__ __forceinline__ cx cneg(cx v, int m) {
     return mk(__hiloint2double(__double2hiint(v.re) ^ m, __double2loint(v.re)),
@@ -323,6 +330,9 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     extern __shared__ double2 smem[];
     const int lane = threadIdx.x;
     const int q = lane % EPW, g = lane / EPW;
+    constexpr int kBlock = G > 32 ? G : 32;
+    constexpr bool kUseRing = G >= 8;
+    uint4* const ring = reinterpret_cast<uint4*>(smem + (size_t)p.slab_cx * EPW) + lane;   // [kRing][kBlock] behind the state
     StateRef<EPW, SPILL> st_;
     st_.S = smem + q;
     st_.spill = SPILL ? p.spill + (size_t)blockIdx.x * p.spill_cx : nullptr;
@@ -374,13 +384,35 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
 #pragma unroll
         for (int c = 0; c < 6; c++) tacc[c] = mk(0.0, 0.0);
 
-        uint4 raw = __ldg(reinterpret_cast<const uint4*>(ops));
-        uint4 nxt = __ldg(reinterpret_cast<const uint4*>(ops + G));
+        // The lane's ops travel global -> shared by cp.async, kRing - 1 steps ahead, into a private ring (no
+        // registers are held across the latency and nothing else reads these slots); the table ends with spare rows.
+        // With few lanes per event (G <= 4) the program of a class is small and stays in L1: plain loads, two steps
+        // ahead, are cheaper there.
+        uint4 r0 = make_uint4(0, 0, 0, 0), r1 = r0;
+        if constexpr (kUseRing) {
+            if (total > 0) {
+#pragma unroll
+                for (int i = 0; i < kRing - 1; i++) {
+                    cp_async16(ring + i * kBlock, ops + (size_t)i * G);
+                    asm volatile("cp.async.commit_group;" ::: "memory");
+                }
+            }
+        } else {
+            r0 = __ldg(reinterpret_cast<const uint4*>(ops));
+            r1 = __ldg(reinterpret_cast<const uint4*>(ops + G));
+        }
         {
             for (int s = 0; s < total; s++) {
-                ops += G;
-                // ops are fetched two steps ahead (the table ends with two spare rows of no-ops)
-                const uint4 nxt2 = __ldg(reinterpret_cast<const uint4*>(ops + G));
+                uint4 raw, r2 = r1;
+                if constexpr (kUseRing) {
+                    cp_async16(ring + ((s + kRing - 1) % kRing) * kBlock, ops + (size_t)(s + kRing - 1) * G);
+                    asm volatile("cp.async.commit_group;" ::: "memory");
+                    asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 1) : "memory");
+                    raw = ring[(s % kRing) * kBlock];
+                } else {
+                    raw = r0;
+                    r2 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)(s + 2) * G));
+                }
                 const int offA = raw.x & 0xFFFF, offB = raw.x >> 16;
                 const int offP1 = raw.y & 0xFFFF, offDst = raw.y >> 16;
                 const int offPt = raw.z & 0xFFFF;
@@ -535,9 +567,9 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                         }
                     }
                 }
-                raw = nxt;
-                nxt = nxt2;
+                if constexpr (!kUseRing) { r0 = r1; r1 = r2; }
             }
+            if constexpr (kUseRing) asm volatile("cp.async.wait_group 0;" ::: "memory");
         }
 
         // closure amplitude: sum of the G lanes' partial contractions (Eq. 22), then |A|^2
@@ -668,10 +700,10 @@ int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out) {
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
     }
-    {   // two spare rows of no-ops: the interpreter prefetches two steps ahead
+    {   // spare rows of no-ops: the interpreter requests ops kRing - 1 steps ahead
         ProgOp nop;
         std::memset(&nop, 0, sizeof(nop));
-        ops.insert(ops.end(), (size_t)2 * G, nop);
+        ops.insert(ops.end(), (size_t)kRing * G, nop);
     }
     t->ops_bytes = ops.size() * sizeof(ProgOp);
     unsigned ms[kMaxN + 1][kNumCodes];
@@ -719,7 +751,8 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
     constexpr int EPW = G >= 32 ? 1 : 32 / G, BLOCK = G > 32 ? G : 32;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSlabBytes);
+        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)(kMaxSlabBytes + (size_t)kRing * BLOCK * 16));
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -728,8 +761,9 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         if (t->tiers.first_key[k] == t->tiers.first_key[k + 1] && k + 1 < kTiers) continue;   // no class in this tier
         p.tier = k;
         p.slab_cx = t->tiers.slab_cx[k];
-        const size_t smem = (size_t)EPW * p.slab_cx * 16;
-        if (smem > kMaxSlabBytes) return cudaErrorInvalidValue;
+        const size_t ring_bytes = G >= 8 ? (size_t)kRing * BLOCK * 16 : 0;
+        const size_t smem = (size_t)EPW * p.slab_cx * 16 + ring_bytes;
+        if (smem > kMaxSlabBytes + ring_bytes) return cudaErrorInvalidValue;
         // resident blocks per SM: shared memory (1 KB reserved per block), and 65536 / (160 x BLOCK) registers
         int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * BLOCK), (228 * 1024) / (smem + 1024)));
         if (SPILL) per_sm = std::min(per_sm, t->spill_blocks_per_sm);   // one global slab per resident block
