@@ -306,7 +306,7 @@ def run_b200(args):
             cpu = {"value": S / dt, "unit": "events/s", "cores": oracle.max_threads(), "kind": "oracle",
                    "sample": f"first {S} events of the workload, {dt:.2f} s wall",
                    "median_rel_diff_gpu_vs_oracle": float(np.median(err))}
-        line = {"metric": "n-gluon |M|^2 events/sec (device-timed)", "value": value, "unit": "events/s",
+        line = {"metric": "n-gluon |M|^2 events/sec", "value": value, "unit": "events/s",
                 "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
                 "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",

@@ -148,7 +148,9 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
     double* A = epsn + 8;
     double* red = A + np * 2;
     const long long N = p.N;
-    const long long e_raw = (long long)blockIdx.x * EPB + evl;
+    // given helicities: the EPB thread groups of a block take EPB events.  Summed helicities: the block takes one
+    // event and its groups share the 2^n assignments (group evl takes hc = evl, evl + EPB, ..)
+    const long long e_raw = p.helsum ? (long long)blockIdx.x : (long long)blockIdx.x * EPB + evl;
     const bool active = e_raw < N;
     const long long e = active ? e_raw : 0;
 
@@ -181,7 +183,9 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
 
     double total = 0.0;
     const int nhel = p.helsum ? (1 << NG) : 1;
-    for (int hc = 0; hc < nhel; hc++) {
+    const int hc_step = p.helsum ? EPB : 1;
+    static_assert((1 << NG) % EPB == 0, "every group runs the same number of helicity assignments (block barriers)");
+    for (int hc = p.helsum ? evl : 0; hc < nhel; hc += hc_step) {
         __syncthreads();   // previous helicity's reads are done; P is visible
         // level 1: external currents eps^lambda(p_g), Eq. 3, and eps_n
         for (int idx = t; idx <= M; idx += TPE) {
@@ -280,6 +284,18 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
         }
         total += w;
     }
+    if (p.helsum && EPB > 1) {
+        // add the groups' partial helicity sums in a fixed order
+        __syncthreads();
+        if (t == 0) red[0] = total;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            total = 0.0;
+            for (int i = 0; i < EPB; i++) total += (smem_d + (size_t)i * ev_doubles + p.nslots * 2 * kSlotStride + NSUB * 4 + 8 + np * 2)[0];
+        }
+        if (threadIdx.x == 0 && active) p.out[e] = total;
+        return;
+    }
     if (t == 0 && active) p.out[e] = total;
 }
 
@@ -371,7 +387,7 @@ static cudaError_t launch_cobg(cudaStream_t s, const CobgParams& p) {
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    const unsigned blocks = (unsigned)((p.N + EPB - 1) / EPB);
+    const unsigned blocks = p.helsum ? (unsigned)p.N : (unsigned)((p.N + EPB - 1) / EPB);
     cobg_shared_kernel<NG, TPE><<<blocks, 128, smem, s>>>(p);
     return cudaGetLastError();
 }
