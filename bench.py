@@ -48,6 +48,7 @@ def parse_args():
     ap.add_argument("--kernel", type=int, default=0, help="BG_OPT_KERNEL (0 auto, 1 generic, 2 class programs)")
     ap.add_argument("--lanes", type=int, default=None, help="BG_OPT_LANES (lanes per event, class-program kernel)")
     ap.add_argument("--smem-limit", type=int, default=None, help="BG_OPT_SMEM_LIMIT in bytes (spill threshold)")
+    ap.add_argument("--lc", action="store_true", help="configs 0 / 2 in leading-colour mode (Eq. 33, SURVEY NEXT-3)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -58,7 +59,11 @@ def workload_desc(args):
     if n is None:
         raise SystemExit("--config 4 needs --n")
     N = args.events or CONFIG_EVENTS[args.config]
-    if args.config in (0, 2):
+    if args.config in (0, 2) and args.lc:
+        import math
+        # (n-1)! orderings x (C(n,3) V3 + C(n,4) V4) at 158 / 178 flop, x 2^n helicities when summed
+        flop = math.factorial(n - 1) * (math.comb(n, 3) * 158 + math.comb(n, 4) * 178) * (16 if args.config == 0 else 1)
+    elif args.config in (0, 2):
         flop = COBG_FLOP_PER_EVENT[args.config]
     else:
         flop = CDBG_FLOP_PER_EVENT[n]
@@ -129,8 +134,10 @@ def max_over_ranks(value: float, world: int, dev) -> float:
     return float(t.item())
 
 
-def mode_for(config):
+def mode_for(config, lc=False):
     import paper_2106_06507_b200 as bg
+    if lc:
+        return {0: bg.BG_COBG_HELSUM_LC, 2: bg.BG_COBG_HELGIVEN_LC}[config]
     return {0: bg.BG_COBG_HELSUM_FULLCOLOR, 2: bg.BG_COBG_HELGIVEN_FULLCOLOR}.get(config, bg.BG_CDBG_GIVEN)
 
 
@@ -199,7 +206,7 @@ def run_b200(args):
 
     n, N, flop_per_event, name = workload_desc(args)
     ev = make_events(args, n, N, rank)
-    mode = mode_for(args.config)
+    mode = mode_for(args.config, args.lc)
     mom = wl.to_soa(mom=ev.mom)
     hel = None if ev.hel is None else wl.to_soa(hel=ev.hel)
     col = None if ev.col is None else wl.to_soa(col=ev.col)
@@ -294,7 +301,7 @@ def run_b200(args):
                     "flop_per_event": flop_per_event, "kernel_ms": kernel_ms,
                     "kernel_share_of_step": kernel_ms / (total_ms / args.steps)}
         cpu = None
-        if not args.no_cpu_baseline:
+        if not args.no_cpu_baseline and not args.lc:    # the oracle has no batched leading-colour entry point
             import oracle
             S = cpu_sample_size(args, n, N)
             sample = ev.head(S)

@@ -46,12 +46,16 @@ enum {
     BG_HEL_SUM = 0x010,   /* sum over all 2^n helicity assignments, Eq. 4; hel must be NULL */
     BG_HEL_GIVEN = 0x020, /* one assignment per event in hel */
     BG_COL_FULL = 0x100,  /* full-colour sum sum_{s,s'} C_{ss'} A_s A_s'^*, Eq. 15-17; col NULL */
+    BG_COL_LC = 0x400,    /* leading-colour approximation N_c^(n-2) (N_c^2-1) sum_{S_(n-1)} |A|^2, Eq. 33
+                             without its O(1/N_c^2) remainder; col NULL; COBG, n <= 7 */
     BG_COL_GIVEN = 0x200, /* one colour-flow assignment (i_k, j_k) per gluon per event in col, Eq. 19 */
 
     BG_COBG_HELSUM_FULLCOLOR = BG_REC_COBG | BG_HEL_SUM | BG_COL_FULL,     /* BASELINE config 1 */
     BG_COBG_HELGIVEN_FULLCOLOR = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_FULL, /* BASELINE config 3 */
     BG_CDBG_GIVEN = BG_REC_CDBG | BG_HEL_GIVEN | BG_COL_GIVEN,             /* BASELINE configs 2, 4, 5 */
-    BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN
+    BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN,
+    BG_COBG_HELSUM_LC = BG_REC_COBG | BG_HEL_SUM | BG_COL_LC,
+    BG_COBG_HELGIVEN_LC = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_LC
 };
 
 /* bg_set_option keys */
@@ -80,6 +84,8 @@ int bg_init(bg_ctx** ctx, int n, int mode);
  * Evaluate |M|^2 for N events, asynchronously on `cuda_stream` (a cudaStream_t; NULL = default stream).
  *   COBG + FULL colour : out[e] = sum_{sigma,sigma'} C A_sigma A_sigma'^*  (Eq. 16), A from Eq. 20 + 22, for the
  *                        helicities in hel, or summed over all 2^n assignments when the mode has BG_HEL_SUM.
+ *   COBG + LC          : out[e] = N_c^(n-2) (N_c^2 - 1) sum over all (n-1)! orderings sigma of gluons 2..n of
+ *                        |A(1, sigma)|^2 (Eq. 33), helicities given or summed.
  *   CDBG + GIVEN colour: out[e] = |A_{i1 j1 .. in jn}|^2 from the subset recursion Eq. 29-32 closed with gluon n
  *                        (Eq. 22); assignments whose amplitude vanishes identically return exactly 0.0.
  * External currents are the helicity eigenvectors of Eq. 3 in the light-cone gauge of DESIGN.md reading g2.

@@ -16,11 +16,13 @@ LIB_PATH = os.path.join(_HERE, "libbg.so")
 BG_OK, BG_EINVAL, BG_ENOMEM, BG_ECUDA, BG_EUNSUPPORTED = 0, -1, -2, -3, -4
 BG_REC_COBG, BG_REC_CDBG = 0x001, 0x002
 BG_HEL_SUM, BG_HEL_GIVEN = 0x010, 0x020
-BG_COL_FULL, BG_COL_GIVEN = 0x100, 0x200
+BG_COL_FULL, BG_COL_GIVEN, BG_COL_LC = 0x100, 0x200, 0x400
 BG_COBG_HELSUM_FULLCOLOR = BG_REC_COBG | BG_HEL_SUM | BG_COL_FULL
 BG_COBG_HELGIVEN_FULLCOLOR = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_FULL
 BG_CDBG_GIVEN = BG_REC_CDBG | BG_HEL_GIVEN | BG_COL_GIVEN
 BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN
+BG_COBG_HELSUM_LC = BG_REC_COBG | BG_HEL_SUM | BG_COL_LC
+BG_COBG_HELGIVEN_LC = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_LC
 BG_OPT_KERNEL, BG_OPT_SCRATCH_LIMIT, BG_OPT_LANES, BG_OPT_TIMING, BG_OPT_SMEM_LIMIT = 1, 2, 3, 4, 5
 
 EXPORTS = ("bg_init", "bg_eval", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",

@@ -135,6 +135,7 @@ static size_t auto_slab_limit(int n) { return n >= 11 ? (size_t)104 * 1024 : 0; 
 static bool mode_supported(int n, int mode) {
     if (n < 4 || n > 12) return false;
     if (mode == BG_COBG_HELSUM_FULLCOLOR || mode == BG_COBG_HELGIVEN_FULLCOLOR) return n <= 8;
+    if (mode == BG_COBG_HELSUM_LC || mode == BG_COBG_HELGIVEN_LC) return bg::cobg_shared_supported(n);
     if (mode == BG_CDBG_GIVEN || mode == BG_CDBG_HELSUM_COLGIVEN) return true;
     return false;
 }
@@ -171,7 +172,7 @@ int bg_init(bg_ctx** out, int n, int mode) {
         delete c;
         return BG_ECUDA;
     }
-    if (mode & BG_REC_COBG) {
+    if ((mode & BG_REC_COBG) && (mode & BG_COL_FULL)) {
         int np = 1;
         for (int i = 2; i <= n - 2; i++) np *= i;
         c->nperm = np;
@@ -405,8 +406,8 @@ int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const 
     c->timed = c->timing != 0;
     if (c->mode & BG_REC_COBG) {
         if (ev0) cudaEventRecord(ev0, s);
-        if (c->cobg && c->kernel_opt != 1) {
-            err = bg::cobg_shared_launch(s, c->cobg, helsum, c->dC, N, mom, hel, out);
+        if (c->cobg && (c->kernel_opt != 1 || (c->mode & BG_COL_LC))) {
+            err = bg::cobg_shared_launch(s, c->cobg, helsum, (c->mode & BG_COL_LC) != 0, c->dC, N, mom, hel, out);
             c->last_kernel = "cobg_shared_kernel";
         } else {
             err = bg::cobg_generic_launch(s, c->n, helsum, c->nperm, c->dC, N, mom, hel, out);

@@ -38,6 +38,8 @@ struct CobgTable {
 
 struct CobgParams {
     int n, np, nslots, helsum;
+    double lc_factor;                 // N_c^(n-2) (N_c^2 - 1)
+    int lc;                           // leading colour (Eq. 33): sum |A|^2 over all (n-1)! orderings, no colour matrix
     long long N;
     const double* mom;
     const signed char* hel;
@@ -134,7 +136,7 @@ struct TopView {
     }
 };
 
-template <int NG, int TPE>
+template <int NG, int TPE, bool LC>
 __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p) {
     constexpr int M = NG - 1, LS = NG - 3, EPB = 128 / TPE, NSUB = 1 << M;
     extern __shared__ double smem_d[];
@@ -154,13 +156,20 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
     const bool active = e_raw < N;
     const long long e = active ? e_raw : 0;
 
+    double total = 0.0;
+    // Leading colour (Eq. 33) needs A(1, sigma) for all (n-1)! orderings of gluons 2..n: for each
+    // choice `last` of the gluon that closes the amplitude the (n-2)! orderings of the others are the same
+    // computation with gluon labels `last` and n exchanged.  Full colour: one pass, last = n.
+    for (int last = M; last >= (LC ? 1 : M); last--) {
+    auto relabel = [&](int g) { return !LC ? g : (g == M ? last : (g == last ? M : g)); };
+    __syncthreads();   // the previous pass is done with P and the currents
     // subset momenta P[mask] = sum of p_g over the bits of mask (gluons 0..M-1), the same for all helicities
     for (int mask = t; mask < NSUB; mask += TPE) {
         double ps[4] = {0.0, 0.0, 0.0, 0.0};
         for (int g = 0; g < M; g++)
             if ((mask >> g) & 1) {
 #pragma unroll
-                for (int c = 0; c < 4; c++) ps[c] += p.mom[(size_t)(g * 4 + c) * N + e];
+                for (int c = 0; c < 4; c++) ps[c] += p.mom[(size_t)(relabel(g) * 4 + c) * N + e];
             }
 #pragma unroll
         for (int c = 0; c < 4; c++) P[mask * 4 + c] = ps[c];
@@ -181,7 +190,6 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
         }
     }
 
-    double total = 0.0;
     const int nhel = p.helsum ? (1 << NG) : 1;
     const int hc_step = p.helsum ? EPB : 1;
     static_assert((1 << NG) % EPB == 0, "every group runs the same number of helicity assignments (block barriers)");
@@ -198,8 +206,8 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
             }
             double pg[4];
 #pragma unroll
-            for (int c = 0; c < 4; c++) pg[c] = p.mom[(size_t)(g * 4 + c) * N + e];
-            const int lam = p.helsum ? (((hc >> g) & 1) ? 1 : -1) : (int)p.hel[(size_t)g * N + e];
+            for (int c = 0; c < 4; c++) pg[c] = p.mom[(size_t)(relabel(g) * 4 + c) * N + e];
+            const int lam = p.helsum ? (((hc >> relabel(g)) & 1) ? 1 : -1) : (int)p.hel[(size_t)relabel(g) * N + e];
             cx eps[4];
             polarisation(pg, lam, eps);
             if (slot >= 0) sts_cur(cur, slot, eps);
@@ -254,7 +262,9 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
         __syncthreads();
         // Eq. 16: row sigma of the real symmetric quadratic form
         double w = 0.0;
-        if (top) {
+        if (top && LC) {
+            w = fma(A[2 * t], A[2 * t], A[2 * t + 1] * A[2 * t + 1]);
+        } else if (top) {
             double tr[4] = {0.0, 0.0, 0.0, 0.0}, ti[4] = {0.0, 0.0, 0.0, 0.0};
             const double* Ccol = p.C + t;
             int s2 = 0;
@@ -284,6 +294,8 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
         }
         total += w;
     }
+    }   // last
+    if (LC) total *= p.lc_factor;
     if (p.helsum && EPB > 1) {
         // add the groups' partial helicity sums in a fixed order
         __syncthreads();
@@ -377,33 +389,36 @@ void cobg_table_destroy(CobgTable* t) {
 
 size_t cobg_shared_current_bytes(const CobgTable* t) { return t ? (size_t)t->nslots * 16 * kSlotStride : 0; }
 
-template <int NG, int TPE>
+template <int NG, int TPE, bool LC>
 static cudaError_t launch_cobg(cudaStream_t s, const CobgParams& p) {
     constexpr int EPB = 128 / TPE, NSUB = 1 << (NG - 1);
     const size_t smem = (size_t)EPB * (p.nslots * 2 * kSlotStride + NSUB * 4 + 8 + p.np * 2 + 8) * sizeof(double);
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(cobg_shared_kernel<NG, TPE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(cobg_shared_kernel<NG, TPE, LC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     const unsigned blocks = p.helsum ? (unsigned)p.N : (unsigned)((p.N + EPB - 1) / EPB);
-    cobg_shared_kernel<NG, TPE><<<blocks, 128, smem, s>>>(p);
+    cobg_shared_kernel<NG, TPE, LC><<<blocks, 128, smem, s>>>(p);
     return cudaGetLastError();
 }
 
-cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, const double* dC, long long N,
+cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, bool lc, const double* dC, long long N,
                                const double* mom, const signed char* hel, double* out) {
     CobgParams p;
     p.n = t->n; p.np = t->np; p.nslots = t->nslots; p.helsum = helsum ? 1 : 0;
+    p.lc = lc ? 1 : 0;
+    p.lc_factor = 8.0;
+    for (int i = 0; i < t->n - 2; i++) p.lc_factor *= 3.0;
     p.N = N; p.mom = mom; p.hel = hel; p.C = dC; p.out = out;
     p.slot = t->d_slot; p.ord = t->d_ord; p.lower = t->d_lower;
     for (int i = 0; i < kCobgMaxM + 2; i++) p.level_begin[i] = t->level_begin[i];
     switch (t->n) {
-        case 4: return launch_cobg<4, 8>(s, p);
-        case 5: return launch_cobg<5, 8>(s, p);
-        case 6: return launch_cobg<6, 32>(s, p);
-        case 7: return launch_cobg<7, 128>(s, p);
+        case 4: return lc ? launch_cobg<4, 8, true>(s, p) : launch_cobg<4, 8, false>(s, p);
+        case 5: return lc ? launch_cobg<5, 8, true>(s, p) : launch_cobg<5, 8, false>(s, p);
+        case 6: return lc ? launch_cobg<6, 32, true>(s, p) : launch_cobg<6, 32, false>(s, p);
+        case 7: return lc ? launch_cobg<7, 128, true>(s, p) : launch_cobg<7, 128, false>(s, p);
         default: return cudaErrorNotSupported;
     }
 }

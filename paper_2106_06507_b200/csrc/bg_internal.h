@@ -72,7 +72,7 @@ bool cobg_shared_supported(int n);
 int cobg_table_create(int n, CobgTable** out);              // BG_* code
 void cobg_table_destroy(CobgTable* t);
 size_t cobg_shared_current_bytes(const CobgTable* t);
-cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, const double* dC, long long N,
+cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, bool lc, const double* dC, long long N,
                                const double* mom, const signed char* hel, double* out);
 
 // ---- colour matrix (bg_colour.cpp part of bg_api.cu) ------------------------------------------------------

@@ -177,6 +177,30 @@ def test_program_interpreter_is_deterministic(bg, wl):
     assert np.array_equal(a[::-1], c)
 
 
+@pytest.mark.parametrize("n,N", [(4, 40), (5, 33), (6, 12), (7, 5)])
+def test_leading_colour_mode(bg, oracle, wl, n, N):
+    """Eq. 33: N^(n-2)(N^2-1) sum over all (n-1)! orderings of |A(1,sigma)|^2, against the oracle's
+    colour-ordered amplitudes ordering by ordering; for n = 4, 5 it also equals the full-colour sum (pinned)."""
+    import itertools
+    ev = wl.config_events(4, N=N, n=n)
+    got, name = gpu_eval(ev, bg.BG_COBG_HELGIVEN_LC)
+    assert name == "cobg_shared_kernel"
+    ref = np.zeros(N)
+    for e in range(N):
+        tot = 0.0
+        for sig in itertools.permutations(range(1, n)):
+            tot += abs(oracle.cobg_amp(ev.mom[e], ev.hel[e], np.array((0,) + sig, dtype=np.int32),
+                                       prec="long double")) ** 2
+        ref[e] = tot * 3 ** (n - 2) * 8
+    assert rel_err(got, ref).max() <= 1e-11
+    if n <= 5:
+        full, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR)
+        assert rel_err(got, full).max() <= 1e-11
+        summed, _ = gpu_eval(ev, bg.BG_COBG_HELSUM_LC)
+        fullsum, _ = gpu_eval(ev, bg.BG_COBG_HELSUM_FULLCOLOR)
+        assert rel_err(summed, fullsum).max() <= 1e-11
+
+
 def test_cdbg_helicity_sum_mode(bg, oracle, wl):
     import itertools
     ev = wl.config_events(4, N=40, n=5)
