@@ -3,15 +3,21 @@
 //
 // Pipeline of one bg_eval (all on the caller's stream):
 //   1. cdbg_classify_kernel   one thread per event: colour codes -> canonical gluon order (a relabelling, under
-//                             which |A|^2 is invariant) + colour-class id; histogram of classes
-//   2. cdbg_scan_kernel       exclusive scan of the histogram (classes ordered by program length)
-//   3. cdbg_scatter_kernel    counting sort: event ids grouped by class, so that a warp runs equal programs
-//   4. cdbg_prog_kernel<G>    G lanes per event run the class program (bg_program.h): vertex operations read their
-//                             operands from the event's state block in shared memory, accumulate in registers and
-//                             write each finished current back once.  Levels (popcount of the subset) are separated
-//                             by __syncwarp; the closure amplitude is reduced over the G lanes with shuffles.
-// State layout in shared memory: per warp a slab of [state_cx][EPW] complex doubles (EPW = 32/G events per warp,
-// event index fastest) so that a quarter-warp's LDS.128 touches eight different 16-byte bank groups.
+//                             which |A|^2 is invariant) + colour-class id; block-aggregated histogram of classes
+//   2. cdbg_scan_kernel       exclusive scan of the histogram (classes ordered by state-size tier, then by
+//                             program length); positions where the tiers start
+//   3. cdbg_scatter_kernel    counting sort: every event becomes one contiguous record (header + momenta of the
+//                             canonical gluons) in class order, so that a warp runs equal programs and reads whole
+//                             sectors
+//   4. cdbg_prog_kernel<G,SPILL>, one launch per non-empty tier: G lanes per event run the class program
+//                             (bg_program.h): vertex operations read their operands from the event's state block in
+//                             shared memory, accumulate in registers and write each finished current back once.
+//                             The program is one flat loop over steps; the last step of a level carries a barrier
+//                             among the event's lanes; the closure amplitude is reduced over the G lanes.
+// State layout in shared memory: per block a slab of [state_cx][EPW] complex doubles (EPW = 32/G events per warp
+// for G < 32, one event per block otherwise; event index fastest) so that a quarter-warp's LDS.128 touches eight
+// different 16-byte bank groups when events share a warp.  With SPILL, offsets beyond the slab live in an
+// L2-resident global slab of the block.  For G >= 8 a per-lane ring behind the slab receives the ops by cp.async.
 #include <algorithm>
 #include <cstring>
 #include <new>
@@ -35,7 +41,7 @@ struct ClassInfo {            // 64 bytes; the interpreter reads the first 16
     uint8_t valid;
     uint32_t total_steps;     // interpreter steps of the whole program
     uint32_t n_sync;          // how many of them end with a barrier (OPF_SYNC)
-    uint16_t level_steps[kMaxLevels];
+    uint16_t level_steps[kMaxLevels];   // steps per level (setup | main, combine per popcount | closure): diagnostics
     uint16_t pad[24 - kMaxLevels];
 };
 
@@ -76,8 +82,6 @@ __constant__ unsigned c_mscount[kMaxN + 1][kNumCodes];   // multiset_count(r, t)
 struct ProgParams {
     int n;
     long long N;
-    const double* mom;
-    const signed char* hel;
     double* out;
     const ClassInfo* info;
     const ProgOp* ops;
@@ -809,7 +813,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     }
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     ProgParams p;
-    p.n = t->n; p.N = N; p.mom = mom; p.hel = hel; p.out = out;
+    p.n = t->n; p.N = N; p.out = out;
     p.info = t->d_info; p.ops = t->d_ops; p.rec = rec; p.rec_bytes = rec_bytes;
     p.bounds = bounds;
     p.spill = t->spill ? (double2*)((char*)scratch + prog_spill_offset(t, N)) : nullptr;
