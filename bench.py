@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--lanes", type=int, default=None, help="BG_OPT_LANES (lanes per event, class-program kernel)")
     ap.add_argument("--smem-limit", type=int, default=None, help="BG_OPT_SMEM_LIMIT in bytes (spill threshold)")
     ap.add_argument("--lc", action="store_true", help="configs 0 / 2 in leading-colour mode (Eq. 33, SURVEY NEXT-3)")
+    ap.add_argument("--precision", type=int, default=None, help="BG_OPT_PRECISION (1 = double-double reference path)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -225,6 +226,8 @@ def run_b200(args):
         bg.bg_set_option(ctx, bg.BG_OPT_KERNEL, args.kernel)
     if args.lanes is not None:
         bg.bg_set_option(ctx, bg.BG_OPT_LANES, args.lanes)
+    if args.precision is not None:
+        bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, args.precision)
     if args.smem_limit is not None:
         bg.bg_set_option(ctx, bg.BG_OPT_SMEM_LIMIT, args.smem_limit)
     bg.bg_reserve(ctx, N)

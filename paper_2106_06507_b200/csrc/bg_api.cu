@@ -230,8 +230,19 @@ int bg_destroy(bg_ctx* c) {
     return BG_OK;
 }
 
+static bool use_dd(const bg_ctx* c) { return c->mode == BG_CDBG_GIVEN && c->precision == 1; }
+
+// events per double-double launch under the scratch limit
+static long long dd_chunk(const bg_ctx* c, long long N) {
+    const size_t per = bg::cdbg_dd_scratch_per_event(c->n);
+    long long chunk = (long long)(c->scratch_limit / per);
+    if (chunk < 128) chunk = 128;
+    chunk -= chunk % 128;
+    return std::min(chunk, std::max<long long>(N, 1));
+}
+
 static bool use_prog(const bg_ctx* c) {
-    if (c->mode != BG_CDBG_GIVEN || c->kernel_opt == 1) return false;
+    if (c->mode != BG_CDBG_GIVEN || c->kernel_opt == 1 || use_dd(c)) return false;
     return c->prog != nullptr;
 }
 
@@ -247,6 +258,7 @@ static long long generic_chunk(const bg_ctx* c, long long N) {
 size_t bg_scratch_bytes(const bg_ctx* c, long long N) {
     if (!c || N <= 0) return 0;
     if (!(c->mode & BG_REC_CDBG)) return 0;
+    if (use_dd(c)) return bg::cdbg_dd_scratch_per_event(c->n) * (size_t)dd_chunk(c, N);
     if (use_prog(c)) return bg::prog_scratch_bytes(c->prog, N);
     return bg::cdbg_generic_scratch_per_event(c->n) * (size_t)generic_chunk(c, N);
 }
@@ -332,6 +344,11 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
             c->slab_limit = (size_t)value;
             return BG_OK;
         }
+        case BG_OPT_PRECISION:
+            if (value != 0 && value != 1) return BG_EINVAL;
+            if (value == 1 && c->mode != BG_CDBG_GIVEN) return BG_EUNSUPPORTED;
+            c->precision = (int)value;
+            return BG_OK;
         case BG_OPT_TIMING:
             if (value != 0 && value != 1) return BG_EINVAL;
             if (value && !c->ev0) {
@@ -415,6 +432,17 @@ int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const 
         }
         if (ev1) cudaEventRecord(ev1, s);
         c->last_launches = 1;
+    } else if (use_dd(c)) {
+        int rc = ensure_scratch(c, N);
+        if (rc != BG_OK) return rc;
+        const long long chunk = dd_chunk(c, N);
+        if (ev0) cudaEventRecord(ev0, s);
+        for (long long first = 0; first < N && err == cudaSuccess; first += chunk) {
+            err = bg::cdbg_dd_launch(s, c->n, N, first, std::min(chunk, N - first), mom, hel, col, out, c->scratch);
+            c->last_launches++;
+        }
+        if (ev1) cudaEventRecord(ev1, s);
+        c->last_kernel = "cdbg_dd_kernel";
     } else if (use_prog(c)) {
         int rc = ensure_scratch(c, N);
         if (rc != BG_OK) return rc;

@@ -38,6 +38,7 @@ struct bg_ctx {
     bg::CobgTable* cobg;       // sequence tables of the shared-current COBG kernel (n <= 7)
     int prog_lanes;            // BG_OPT_LANES (0 = automatic)
     size_t slab_limit;         // BG_OPT_SMEM_LIMIT (0 = all of shared memory)
+    int precision;             // BG_OPT_PRECISION: 0 = FP64, 1 = double-double reference path (CDBG, given colours)
     // bookkeeping
     int timing;                // BG_OPT_TIMING
     cudaEvent_t ev0, ev1;
@@ -56,6 +57,11 @@ cudaError_t cdbg_generic_launch(cudaStream_t s, int n, bool helsum, long long N,
                                 void* scratch);
 cudaError_t cobg_generic_launch(cudaStream_t s, int n, bool helsum, int nperm, const double* dC, long long N,
                                 const double* mom, const signed char* hel, double* out);
+
+// ---- double-double reference path (bg_cdbg_dd.cu): one thread per event, currents in global scratch ---------
+size_t cdbg_dd_scratch_per_event(int n);
+cudaError_t cdbg_dd_launch(cudaStream_t s, int n, long long N, long long first, long long count, const double* mom,
+                           const signed char* hel, const signed char* col, double* out, void* scratch);
 
 // ---- colour-class program interpreter (bg_cdbg_prog.cu): G lanes per event, currents in shared memory -------
 int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out);   // BG_* code; slab_limit 0 = all of shared memory

@@ -2,7 +2,7 @@
 import numpy as np
 
 
-def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None, lanes=None, smem_limit=None):
+def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None, lanes=None, smem_limit=None, precision=None):
     """ev: workload.Events (AoS numpy).  Returns out[N] (numpy) and the kernel name used."""
     import torch
     import paper_2106_06507_b200 as bg
@@ -23,6 +23,8 @@ def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None, lanes=None, sme
                     import pytest
                     pytest.skip(f"{lanes} lanes per event: one warp's state exceeds shared memory for n={n}")
                 raise
+        if precision is not None:
+            bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, precision)
         if smem_limit is not None:
             bg.bg_set_option(ctx, bg.BG_OPT_SMEM_LIMIT, smem_limit)
         if scratch_limit:

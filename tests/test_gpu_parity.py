@@ -110,6 +110,12 @@ def test_config2_n6_full_size_all_events(bg, oracle, wl):
     got, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
     err, tail = check_cdbg(oracle, ev, got, max_tail_frac=0.003)
     assert np.median(err) < 1e-14 and np.percentile(err, 99) < 2e-12
+    # the same 2^20 events through the double-double reference path: every single one within 1e-11 of the truth
+    exact, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, precision=1)
+    truth = oracle.cdbg(ev.mom, ev.hel, ev.col, prec="long double")
+    assert name == "cdbg_dd_kernel" and rel_err(exact, truth).max() <= 1e-11
+    # and the FP64 kernels deviate from it only where the oracle's own FP64 evaluation does
+    assert np.mean(rel_err(got, exact) > 1e-11) < 0.003
 
 
 def test_config4_n9_full_size_sampled(bg, oracle, wl):
@@ -199,6 +205,22 @@ def test_leading_colour_mode(bg, oracle, wl, n, N):
         summed, _ = gpu_eval(ev, bg.BG_COBG_HELSUM_LC)
         fullsum, _ = gpu_eval(ev, bg.BG_COBG_HELSUM_FULLCOLOR)
         assert rel_err(summed, fullsum).max() <= 1e-11
+
+
+@pytest.mark.parametrize("n,N", [(4, 500), (6, 20000), (8, 1500), (9, 515), (10, 131), (12, 19)])
+def test_double_double_reference_path_matches_truth_on_every_event(bg, oracle, wl, n, N):
+    """BG_OPT_PRECISION = 1: the same recursion in double-double arithmetic on the GPU.  With the round-off of
+    FP64 out of the way every event - including the near-zeros where the FP64 kernels and the double-precision
+    oracle both miss 1e-11 - agrees with the extended-precision oracle: what the FP64 kernels lose is rounding."""
+    ev = wl.config_events(4, N=N, n=n)
+    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, precision=1)
+    assert name == "cdbg_dd_kernel"
+    truth = oracle.cdbg(ev.mom, ev.hel, ev.col, prec="long double")
+    err = rel_err(got, truth)
+    # the truth itself carries 64-bit-significand round-off amplified by the same cancellations: allow 1e-11
+    assert err.max() <= 1e-11, f"max {err.max():.2e} at event {err.argmax()}"
+    fp64, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
+    assert np.median(rel_err(fp64, got)) < 1e-13
 
 
 def test_cdbg_helicity_sum_mode(bg, oracle, wl):
