@@ -67,8 +67,8 @@ enum {
     BG_OPT_LANES = 3,        /* lanes that cooperate on one event in the program interpreter: 1, 2, 4, ..., 256;
                                 0 = automatic.  Rebuilds the class programs (synchronises the device). */
     BG_OPT_TIMING = 4,       /* 1: record CUDA events around the dominant kernel of every bg_eval (bg_last_kernel_ms) */
-    BG_OPT_PRECISION = 6,    /* BG_CDBG_GIVEN: 0 = FP64 kernels (default); 1 = every event in double-double arithmetic
-                                (one thread per event, global scratch): the precision reference on the GPU, slow */
+    BG_OPT_PRECISION = 6,    /* BG_CDBG_GIVEN and the COBG full-colour modes: 0 = FP64 kernels (default); 1 = every event
+                                in double-double arithmetic: the precision reference on the GPU, slow */
     BG_OPT_SMEM_LIMIT = 5    /* program interpreter, >= 128 lanes per event: bytes of shared memory one event's state may
                                 take (16 KiB .. 222 KiB, 0 = default); the rest spills to an L2-resident slab.
                                 Rebuilds the class programs. */

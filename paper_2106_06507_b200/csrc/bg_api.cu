@@ -231,6 +231,13 @@ int bg_destroy(bg_ctx* c) {
 }
 
 static bool use_dd(const bg_ctx* c) { return c->mode == BG_CDBG_GIVEN && c->precision == 1; }
+static bool use_cobg_dd(const bg_ctx* c) { return (c->mode & BG_REC_COBG) && (c->mode & BG_COL_FULL) && c->precision == 1; }
+static long long cobg_dd_chunk(const bg_ctx* c, long long N) {
+    const size_t per = bg::cobg_dd_scratch_per_event(c->n, (c->mode & BG_HEL_SUM) != 0);
+    long long chunk = (long long)(std::min<size_t>(c->scratch_limit, (size_t)2 << 30) / per);
+    if (chunk < 64) chunk = 64;
+    return std::min(chunk, std::max<long long>(N, 1));
+}
 
 // events per double-double launch under the scratch limit
 static long long dd_chunk(const bg_ctx* c, long long N) {
@@ -257,6 +264,7 @@ static long long generic_chunk(const bg_ctx* c, long long N) {
 
 size_t bg_scratch_bytes(const bg_ctx* c, long long N) {
     if (!c || N <= 0) return 0;
+    if (use_cobg_dd(c)) return bg::cobg_dd_scratch_per_event(c->n, (c->mode & BG_HEL_SUM) != 0) * (size_t)cobg_dd_chunk(c, N);
     if (!(c->mode & BG_REC_CDBG)) return 0;
     if (use_dd(c)) return bg::cdbg_dd_scratch_per_event(c->n) * (size_t)dd_chunk(c, N);
     if (use_prog(c)) return bg::prog_scratch_bytes(c->prog, N);
@@ -346,7 +354,8 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
         }
         case BG_OPT_PRECISION:
             if (value != 0 && value != 1) return BG_EINVAL;
-            if (value == 1 && c->mode != BG_CDBG_GIVEN) return BG_EUNSUPPORTED;
+            if (value == 1 && c->mode != BG_CDBG_GIVEN && !((c->mode & BG_REC_COBG) && (c->mode & BG_COL_FULL)))
+                return BG_EUNSUPPORTED;
             c->precision = (int)value;
             return BG_OK;
         case BG_OPT_TIMING:
@@ -421,7 +430,19 @@ int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const 
     cudaError_t err = cudaSuccess;
     cudaEvent_t ev0 = c->timing ? c->ev0 : nullptr, ev1 = c->timing ? c->ev1 : nullptr;
     c->timed = c->timing != 0;
-    if (c->mode & BG_REC_COBG) {
+    if (use_cobg_dd(c)) {
+        int rc = ensure_scratch(c, N);
+        if (rc != BG_OK) return rc;
+        const long long chunk = cobg_dd_chunk(c, N);
+        if (ev0) cudaEventRecord(ev0, s);
+        for (long long first = 0; first < N && err == cudaSuccess; first += chunk) {
+            err = bg::cobg_dd_launch(s, c->n, helsum, c->nperm, c->dC, N, first, std::min(chunk, N - first), mom, hel, out,
+                                     c->scratch);
+            c->last_launches += 2;
+        }
+        if (ev1) cudaEventRecord(ev1, s);
+        c->last_kernel = "cobg_dd_kernel";
+    } else if (c->mode & BG_REC_COBG) {
         if (ev0) cudaEventRecord(ev0, s);
         if (c->cobg && (c->kernel_opt != 1 || (c->mode & BG_COL_LC))) {
             err = bg::cobg_shared_launch(s, c->cobg, helsum, (c->mode & BG_COL_LC) != 0, c->dC, N, mom, hel, out);

@@ -195,3 +195,123 @@ cudaError_t cdbg_dd_launch(cudaStream_t s, int n, long long N, long long first, 
 }
 
 }  // namespace bg
+
+// ---------------------------------------------------------------------------------------------------------
+// Colour-ordered recursion (Eq. 20-22) and full-colour form (Eq. 16) in double-double:
+// kernel 1 - one thread per (event, helicity assignment, ordering): triangular current table, A_sigma to scratch;
+// kernel 2 - one thread per event: sum over helicity assignments of  sum_{s s'} C_{s s'} A_s A_s'^*.
+// ---------------------------------------------------------------------------------------------------------
+namespace bg {
+
+namespace {
+constexpr int kDdMaxN = 8;
+__device__ __forceinline__ int tri_dd(int i, int j) { return j * (j + 1) / 2 + i; }   // i <= j
+}  // namespace
+
+__global__ void __launch_bounds__(64)
+cobg_dd_amp_kernel(int n, int nhel, int nperm, long long N, long long first, long long count,
+                   const double* __restrict__ mom, const signed char* __restrict__ hel, double2* __restrict__ amps) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= count * nhel * nperm) return;
+    const int s = (int)(idx % nperm);
+    const int hc = (int)((idx / nperm) % nhel);
+    const long long e = first + idx / ((long long)nperm * nhel);
+    const int m = n - 1, mm = n - 2;
+    // s-th permutation of gluons 2..n-1 (0-based labels 1..n-2) in lexicographic order
+    int avail[kDdMaxN], order[kDdMaxN];
+    for (int i = 0; i < mm; i++) avail[i] = i + 1;
+    int rem = s, fact = nperm;
+    order[0] = 0;
+    for (int i = 0; i < mm; i++) {
+        fact /= (mm - i);
+        const int d = rem / fact;
+        rem -= d * fact;
+        order[i + 1] = avail[d];
+        for (int q = d; q < mm - i - 1; q++) avail[q] = avail[q + 1];
+    }
+    order[n - 1] = n - 1;
+    C J[kDdMaxN * (kDdMaxN - 1) / 2][4];
+    dd P[kDdMaxN * (kDdMaxN - 1) / 2][4];
+    C epsn[4];
+    for (int i = 0; i < n; i++) {
+        const int g = order[i];
+        dd p[4];
+        for (int c = 0; c < 4; c++) p[c] = mkdd(mom[(size_t)(g * 4 + c) * N + e]);
+        const int lam = nhel > 1 ? (((hc >> g) & 1) ? 1 : -1) : (int)hel[(size_t)g * N + e];
+        if (i < m) {
+            polarisation_t<dd>(p, lam, J[tri_dd(i, i)]);
+            for (int c = 0; c < 4; c++) P[tri_dd(i, i)][c] = p[c];
+        } else {
+            polarisation_t<dd>(p, lam, epsn);
+        }
+    }
+    const dd inv_sqrt2 = mkdd(1.0) / sqrt(mkdd(2.0)), half = mkdd(0.5), zero = mkdd(0.0), two = mkdd(2.0);
+    for (int len = 2; len <= m; len++)
+        for (int i = 0; i + len <= m; i++) {
+            const int j = i + len - 1;
+            for (int c = 0; c < 4; c++) P[tri_dd(i, j)][c] = P[tri_dd(i, j - 1)][c] + P[tri_dd(j, j)][c];
+            C s3[4], s4[4];
+            for (int c = 0; c < 4; c++) { s3[c] = mkc<dd>(zero, zero); s4[c] = mkc<dd>(zero, zero); }
+            for (int k = i; k < j; k++) {
+                const C* a = J[tri_dd(i, k)];
+                v3_acc_t<dd>(s3, P[tri_dd(i, k)], P[tri_dd(k + 1, j)], a, J[tri_dd(k + 1, j)], false);
+                for (int l = k + 1; l < j; l++) {
+                    // 2 V4(a,b,c) = 2 (a.c) b - (a.b) c - (b.c) a   (Eq. 21, second line)
+                    const C* b = J[tri_dd(k + 1, l)];
+                    const C* c3 = J[tri_dd(l + 1, j)];
+                    const C ac = two * mdot_t<dd>(a, c3), ab = mdot_t<dd>(a, b), bc = mdot_t<dd>(b, c3);
+                    for (int nu = 0; nu < 4; nu++) s4[nu] = s4[nu] + ac * b[nu] - ab * c3[nu] - bc * a[nu];
+                }
+            }
+            dd f3 = inv_sqrt2, f4 = half;
+            if (len < m) {
+                const dd ip2 = mkdd(1.0) / mdot_t<dd>(P[tri_dd(i, j)], P[tri_dd(i, j)]);
+                f3 = f3 * ip2; f4 = f4 * ip2;
+            }
+            for (int c = 0; c < 4; c++) J[tri_dd(i, j)][c] = f3 * s3[c] + f4 * s4[c];
+        }
+    const C A = mdot_t<dd>(epsn, J[tri_dd(0, m - 1)]);
+    double2* o = amps + idx * 2;
+    o[0] = make_double2(A.re.hi, A.re.lo);
+    o[1] = make_double2(A.im.hi, A.im.lo);
+}
+
+__global__ void __launch_bounds__(64)
+cobg_dd_colour_kernel(int nhel, int nperm, long long first, long long count, const double* __restrict__ Cm,
+                      const double2* __restrict__ amps, double* __restrict__ out) {
+    const long long el = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (el >= count) return;
+    dd total = mkdd(0.0);
+    for (int hc = 0; hc < nhel; hc++) {
+        const double2* a = amps + (el * nhel + hc) * (long long)nperm * 2;
+        for (int s = 0; s < nperm; s++) {
+            dd tr = mkdd(0.0), ti = mkdd(0.0);
+            for (int s2 = 0; s2 < nperm; s2++) {
+                const dd c = mkdd(Cm[(size_t)s * nperm + s2]);
+                tr = tr + c * mkdd(a[2 * s2].x, a[2 * s2].y);
+                ti = ti + c * mkdd(a[2 * s2 + 1].x, a[2 * s2 + 1].y);
+            }
+            total = total + mkdd(a[2 * s].x, a[2 * s].y) * tr + mkdd(a[2 * s + 1].x, a[2 * s + 1].y) * ti;
+        }
+    }
+    out[first + el] = to_double(total);
+}
+
+size_t cobg_dd_scratch_per_event(int n, bool helsum) {
+    size_t np = 1;
+    for (int i = 2; i <= n - 2; i++) np *= i;
+    return np * (helsum ? ((size_t)1 << n) : 1) * 2 * sizeof(double2);
+}
+
+cudaError_t cobg_dd_launch(cudaStream_t s, int n, bool helsum, int nperm, const double* dC, long long N, long long first,
+                           long long count, const double* mom, const signed char* hel, double* out, void* scratch) {
+    const int nhel = helsum ? (1 << n) : 1;
+    const long long threads = count * nhel * nperm;
+    cobg_dd_amp_kernel<<<(unsigned)((threads + 63) / 64), 64, 0, s>>>(n, nhel, nperm, N, first, count, mom, hel,
+                                                                      (double2*)scratch);
+    cobg_dd_colour_kernel<<<(unsigned)((count + 63) / 64), 64, 0, s>>>(nhel, nperm, first, count, dC, (const double2*)scratch,
+                                                                       out);
+    return cudaGetLastError();
+}
+
+}  // namespace bg

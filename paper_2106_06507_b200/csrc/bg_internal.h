@@ -63,6 +63,10 @@ size_t cdbg_dd_scratch_per_event(int n);
 cudaError_t cdbg_dd_launch(cudaStream_t s, int n, long long N, long long first, long long count, const double* mom,
                            const signed char* hel, const signed char* col, double* out, void* scratch);
 
+size_t cobg_dd_scratch_per_event(int n, bool helsum);
+cudaError_t cobg_dd_launch(cudaStream_t s, int n, bool helsum, int nperm, const double* dC, long long N, long long first,
+                           long long count, const double* mom, const signed char* hel, double* out, void* scratch);
+
 // ---- colour-class program interpreter (bg_cdbg_prog.cu): G lanes per event, currents in shared memory -------
 int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out);   // BG_* code; slab_limit 0 = all of shared memory
 void prog_table_destroy(ProgTable* t);

@@ -223,6 +223,23 @@ def test_double_double_reference_path_matches_truth_on_every_event(bg, oracle, w
     assert np.median(rel_err(fp64, got)) < 1e-13
 
 
+@pytest.mark.parametrize("n,N", [(5, 1000), (6, 600), (7, 2048)])
+def test_double_double_reference_path_cobg(bg, oracle, wl, n, N):
+    """Full-colour COBG in double-double on the GPU: every event within 1e-11 of the extended-precision oracle,
+    including the kinematic near-zeros where FP64 (oracle and kernels alike) loses more."""
+    ev = wl.config_events(4, N=N, n=n)
+    got, name = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR, precision=1)
+    assert name == "cobg_dd_kernel"
+    truth = oracle.cobg_full_colour(ev.mom, ev.hel, prec="long double")
+    assert rel_err(got, truth).max() <= 1e-11
+    fp64, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR)
+    assert np.median(rel_err(fp64, got)) < 1e-13
+    if n == 5:
+        ev4 = wl.config_events(0, N=300)
+        got, _ = gpu_eval(ev4, bg.BG_COBG_HELSUM_FULLCOLOR, precision=1)
+        assert rel_err(got, oracle.cobg_full_colour(ev4.mom, prec="long double")).max() <= 1e-11
+
+
 def test_cdbg_helicity_sum_mode(bg, oracle, wl):
     import itertools
     ev = wl.config_events(4, N=40, n=5)
