@@ -33,7 +33,7 @@ def _load():
         build()
         _lib = ctypes.CDLL(_LIB)
         for name in ("bgo_polarisation", "bgo_cobg_amp_ext", "bgo_cobg_amp", "bgo_colour_matrix",
-                     "bgo_cobg_full_colour", "bgo_cdbg", "bgo_colour_flow", "bgo_max_threads"):
+                     "bgo_cobg_full_colour", "bgo_cdbg", "bgo_colour_flow", "bgo_max_threads", "bgo_cdbg_general"):
             getattr(_lib, name).restype = ctypes.c_int
     return _lib
 
@@ -148,6 +148,42 @@ def cdbg(mom, hel, col, prec: str = "double", threads: int = 0, return_live: boo
     assert rc == 0
     res = (out,) + ((live,) if return_live else ()) + ((rho,) if return_rho else ())
     return res if len(res) > 1 else out
+
+
+def cdbg_general(mom, ext, X, prec: str = "double", threads: int = 0) -> np.ndarray:
+    """Batched colour-dressed amplitude (complex) for general external states: ext[N][n][4] complex polarisation
+    vectors, X[N][n][3][3] complex colour matrices (Eq. 14 + Eq. 28-32)."""
+    mom = _f64(mom)
+    N, n = mom.shape[0], mom.shape[1]
+    e = np.ascontiguousarray(np.stack([np.real(ext), np.imag(ext)], axis=-1), dtype=np.float64)
+    x = np.ascontiguousarray(np.stack([np.real(X), np.imag(X)], axis=-1), dtype=np.float64)
+    assert e.shape == (N, n, 4, 2) and x.shape == (N, n, 3, 3, 2)
+    amp = np.empty((N, 2))
+    rc = _load().bgo_cdbg_general(n, ctypes.c_longlong(N), _p(mom), _p(e), _p(x), _prec(prec), int(threads), _p(amp))
+    assert rc == 0
+    return amp[:, 0] + 1j * amp[:, 1]
+
+
+def continuous_states(mom, phi, eta):
+    """External states of the continuous sampling (Eq. 7, 9, 12): real polarisation e = cos(phi) e1 + sin(phi) e2
+    with e1 = (eps^- - eps^+)/sqrt2, e2 = i (eps^+ + eps^-)/sqrt2 (the unit vectors of reading g2), and colour matrix
+    X_hg = etabar_h eta_g from eta[..., 0, :] = eta, eta[..., 1, :] = etabar.  Returns (ext, X)."""
+    mom = _f64(mom)
+    N, n = mom.shape[0], mom.shape[1]
+    ext = np.empty((N, n, 4), dtype=complex)
+    for e in range(N):
+        for k in range(n):
+            ep, em = polarisation(mom[e, k], +1), polarisation(mom[e, k], -1)
+            e1, e2 = (em - ep) / np.sqrt(2.0), 1j * (ep + em) / np.sqrt(2.0)
+            ext[e, k] = np.cos(phi[e, k]) * e1 + np.sin(phi[e, k]) * e2
+    X = np.einsum("ekh,ekg->ekhg", eta[:, :, 1, :], eta[:, :, 0, :]).astype(complex)
+    return ext, X
+
+
+def cdbg_continuous(mom, phi, eta, prec: str = "double", threads: int = 0) -> np.ndarray:
+    """|A|^2 of the continuous colour / polarisation sub-amplitude (Eq. 14)."""
+    ext, X = continuous_states(mom, phi, eta)
+    return np.abs(cdbg_general(mom, ext, X, prec=prec, threads=threads)) ** 2
 
 
 def colour_flow(mom, hel, col, prec: str = "double", threads: int = 0, return_count: bool = False,

@@ -15,7 +15,9 @@
 // Pins (tests/test_oracle_pins.py): Parke-Taylor MHV moduli, vanishing all-plus / single-minus amplitudes,
 // cyclicity, reflection, U(1) decoupling, gauge invariance (eps -> eps + z p, eps -> p), V4 form == tensor
 // form, closed-form gg->gg, hand-derivable colour-matrix entries, Eq. 33 exactness at n = 4,5, colour-dressed
-// == Eq. 19 brute force, sum over all 9^n colour flows == A^dagger C A.  Parity unpinned: nothing exported here.
+// == Eq. 19 brute force, sum over all 9^n colour flows == A^dagger C A; general external states (continuous
+// colour / polarisation, Eq. 7-14): elementary X == discrete CDBG, multilinearity in colour and helicity, real
+// inputs give real amplitudes, trace part of X decouples, Monte-Carlo normalisation of Eq. 13.  Parity unpinned: nothing exported here.
 //
 // Build: g++ -O2 -std=c++17 -fopenmp -shared -fPIC bg_oracle.cpp -o libbgoracle.so
 #include <algorithm>
@@ -354,6 +356,63 @@ cx<R> cdbg_amplitude(int n, const V4r<R>* mom, const V4c<R>* ext, const int8_t* 
     return A;
 }
 
+// ---- CDBG with general external states: the same recursion Eq. 28-32 with arbitrary external
+// polarisation vectors ext[k] and arbitrary external 3x3 colour matrices X[k] (Eq. 14: the
+// colour-helicity sub-amplitude is the amplitude contracted with one polarisation and one colour state per gluon).
+//   |pi|=1: J({k})_{hg} = ext[k] X[k]_{hg};   closure: A = sum_{hg} (ext[n-1] . J({1..n-1})_{hg}) X[n-1]_{gh}
+// Continuous sampling (Eq. 7, 9, 12): ext = cos(phi) e1 + sin(phi) e2, X_{hg} = etabar_h eta_g (the trace part of
+// eta_i T^a_ij etabar_j T^a_hg = eta_g etabar_h - delta_hg (eta.etabar)/3 decouples - pinned).  Discrete colour flow
+// (i_k, j_k) is X = e_{i_k j_k}, which must reproduce cdbg_amplitude - pinned.
+template <class R>
+cx<R> cdbg_amplitude_general(int n, const V4r<R>* mom, const V4c<R>* ext, const cx<R> (*X)[3][3]) {
+    const int m = n - 1;
+    const int nsub = 1 << m;
+    struct Cur { V4c<R> J[3][3]; T6c<R> T[3][3]; V4r<R> P; };
+    std::vector<Cur> cur(nsub);
+    for (int pi = 1; pi < nsub; pi++) {
+        Cur& c = cur[pi];
+        for (int h = 0; h < 3; h++)
+            for (int g = 0; g < 3; g++) {
+                for (int mu = 0; mu < 4; mu++) c.J[h][g].v[mu] = cx<R>(0, 0);
+                for (int a = 0; a < 4; a++) for (int b = 0; b < 4; b++) c.T[h][g].t[a][b] = cx<R>(0, 0);
+            }
+        for (int mu = 0; mu < 4; mu++) c.P.v[mu] = 0;
+        for (int k = 0; k < m; k++)
+            if (pi >> k & 1) for (int mu = 0; mu < 4; mu++) c.P.v[mu] += mom[k].v[mu];
+        if ((pi & (pi - 1)) == 0) {
+            const int k = __builtin_ctz(pi);
+            for (int h = 0; h < 3; h++)
+                for (int g = 0; g < 3; g++)
+                    for (int mu = 0; mu < 4; mu++) c.J[h][g].v[mu] = ext[k].v[mu] * X[k][h][g];
+            continue;
+        }
+        for (int p1 = (pi - 1) & pi; p1 > 0; p1 = (p1 - 1) & pi) {   // ordered splits
+            const int p2 = pi ^ p1;
+            const Cur& c1 = cur[p1];
+            const Cur& c2 = cur[p2];
+            for (int h = 0; h < 3; h++)
+                for (int k = 0; k < 3; k++)
+                    for (int g = 0; g < 3; g++) {
+                        V4c<R> t;
+                        V3(c1.P, c2.P, c1.J[h][k], c2.J[k][g], t);
+                        VT_add(c1.J[h][k], c1.T[h][k], c2.J[k][g], c2.T[k][g], t);
+                        for (int mu = 0; mu < 4; mu++) c.J[h][g].v[mu] += t.v[mu];
+                        tensor_build_add(c1.J[h][k], c2.J[k][g], c.T[h][g]);
+                    }
+        }
+        if (pi != nsub - 1) {
+            const R P2 = mdot(c.P, c.P);
+            for (int h = 0; h < 3; h++)
+                for (int g = 0; g < 3; g++)
+                    for (int mu = 0; mu < 4; mu++) c.J[h][g].v[mu] /= P2;
+        }
+    }
+    cx<R> A(0, 0);
+    for (int h = 0; h < 3; h++)
+        for (int g = 0; g < 3; g++) A += mdot(ext[n - 1], cur[nsub - 1].J[h][g]) * X[n - 1][g][h];
+    return A;
+}
+
 template <class R>
 R cdbg_me2(int n, const V4r<R>* mom, const int8_t* hel, const int8_t* col, long long* live, double* rho) {
     V4c<R> ex[MAXN];
@@ -408,6 +467,22 @@ template <class R> void load_mom(int n, const double* mom, V4r<R>* out) {
 // ======================================= C entry points (ctypes) ==========================================
 // Arrays: mom[N][n][4] doubles (E,px,py,pz), hel[N][n] int8 (+1/-1), col[N][n][2] int8 in {1,2,3}; AoS.
 // prec: 0 = double, 1 = long double.  All return 0 on success, -1 on bad arguments.
+// Batched CDBG amplitude with general external states: ext [N][n][4][2] (re, im), X [N][n][3][3][2]; amp [N][2].
+template <class R>
+static void cdbg_general_one(int n, const double* mom, const double* ext, const double* X, double* amp) {
+    V4r<R> pm[MAXN]; load_mom(n, mom, pm);
+    V4c<R> ex[MAXN];
+    cx<R> Xm[MAXN][3][3];
+    for (int k = 0; k < n; k++) {
+        for (int mu = 0; mu < 4; mu++) ex[k].v[mu] = cx<R>(ext[(k * 4 + mu) * 2], ext[(k * 4 + mu) * 2 + 1]);
+        for (int h = 0; h < 3; h++)
+            for (int g = 0; g < 3; g++) Xm[k][h][g] = cx<R>(X[((k * 3 + h) * 3 + g) * 2], X[((k * 3 + h) * 3 + g) * 2 + 1]);
+    }
+    const cx<R> A = cdbg_amplitude_general<R>(n, pm, ex, Xm);
+    amp[0] = (double)A.real();
+    amp[1] = (double)A.imag();
+}
+
 extern "C" {
 
 int bgo_polarisation(const double* p, int lambda, double* eps_re_im /* [4][2] */) {
@@ -523,6 +598,17 @@ int bgo_colour_flow(int n, long long N, const double* mom, const signed char* he
             out[e] = (double)colour_flow_me2(n, pm, (const int8_t*)hel + (size_t)e * n, (const int8_t*)col + (size_t)e * n * 2, &c, rho ? rho + e : nullptr);
         }
         if (count) count[e] = c;
+    }
+    return 0;
+}
+
+int bgo_cdbg_general(int n, long long N, const double* mom, const double* ext, const double* X, int prec, int threads,
+                     double* amp) {
+    if (n < 3 || n >= MAXN) return -1;
+#pragma omp parallel for schedule(dynamic, 4) num_threads(threads > 0 ? threads : omp_get_max_threads_wrapper())
+    for (long long e = 0; e < N; e++) {
+        if (prec == 0) cdbg_general_one<double>(n, mom + (size_t)e * n * 4, ext + (size_t)e * n * 8, X + (size_t)e * n * 18, amp + 2 * e);
+        else cdbg_general_one<long double>(n, mom + (size_t)e * n * 4, ext + (size_t)e * n * 8, X + (size_t)e * n * 18, amp + 2 * e);
     }
     return 0;
 }

@@ -753,12 +753,14 @@ size_t prog_scratch_bytes(const ProgTable* t, long long N) {
 template <int G, bool SPILL>
 static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched) {
     constexpr int EPW = G >= 32 ? 1 : 32 / G, BLOCK = G > 32 ? G : 32;
-    static bool configured = false;
-    if (!configured) {
+    static int configured_device = -1;   // the attribute is per device
+    int device = 0;
+    cudaGetDevice(&device);
+    if (configured_device != device) {
         cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)(kMaxSlabBytes + (size_t)kRing * BLOCK * 16));
         if (e != cudaSuccess) return e;
-        configured = true;
+        configured_device = device;
     }
     const long long max_tasks = (p.N + EPW - 1) / EPW + kTiers;
     for (int k = 0; k < kTiers; k++) {
@@ -793,11 +795,13 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     const unsigned eb = (unsigned)((N + kPreEvents - 1) / kPreEvents);
     const size_t hist_smem = sizeof(uint32_t) * nbins;
     if (hist_smem <= 160 * 1024) {
-        static bool configured = false;
-        if (!configured) {
+        static int configured_device = -1;
+        int device = 0;
+        cudaGetDevice(&device);
+        if (configured_device != device) {
             cudaFuncSetAttribute(cdbg_classify_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
             cudaFuncSetAttribute(cdbg_scatter_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
-            configured = true;
+            configured_device = device;
         }
         cdbg_classify_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
                                                                       t->d_sortkey, cls, perm, hist);

@@ -393,11 +393,13 @@ template <int NG, int TPE, bool LC>
 static cudaError_t launch_cobg(cudaStream_t s, const CobgParams& p) {
     constexpr int EPB = 128 / TPE, NSUB = 1 << (NG - 1);
     const size_t smem = (size_t)EPB * (p.nslots * 2 * kSlotStride + NSUB * 4 + 8 + p.np * 2 + 8) * sizeof(double);
-    static bool configured = false;
-    if (!configured) {
+    static int configured_device = -1;   // the attribute is per device
+    int device = 0;
+    cudaGetDevice(&device);
+    if (configured_device != device) {
         cudaError_t e = cudaFuncSetAttribute(cobg_shared_kernel<NG, TPE, LC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
-        configured = true;
+        configured_device = device;
     }
     const unsigned blocks = p.helsum ? (unsigned)p.N : (unsigned)((p.N + EPB - 1) / EPB);
     cobg_shared_kernel<NG, TPE, LC><<<blocks, 128, smem, s>>>(p);
