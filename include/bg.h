@@ -48,12 +48,15 @@ enum {
     BG_COL_FULL = 0x100,  /* full-colour sum sum_{s,s'} C_{ss'} A_s A_s'^*, Eq. 15-17; col NULL */
     BG_COL_LC = 0x400,    /* leading-colour approximation N_c^(n-2) (N_c^2-1) sum_{S_(n-1)} |A|^2, Eq. 33
                              without its O(1/N_c^2) remainder; col NULL; COBG, n <= 7 */
+    BG_HEL_CONT = 0x040,  /* continuous polarisation angle phi per gluon, real e(phi) of Eq. 7 */
+    BG_COL_CONT = 0x800,  /* continuous colour states: two real unit 3-vectors (eta, etabar) per gluon, Eq. 9, 12 */
     BG_COL_GIVEN = 0x200, /* one colour-flow assignment (i_k, j_k) per gluon per event in col, Eq. 19 */
 
     BG_COBG_HELSUM_FULLCOLOR = BG_REC_COBG | BG_HEL_SUM | BG_COL_FULL,     /* BASELINE config 1 */
     BG_COBG_HELGIVEN_FULLCOLOR = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_FULL, /* BASELINE config 3 */
     BG_CDBG_GIVEN = BG_REC_CDBG | BG_HEL_GIVEN | BG_COL_GIVEN,             /* BASELINE configs 2, 4, 5 */
     BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN,
+    BG_CDBG_CONTINUOUS = BG_REC_CDBG | BG_HEL_CONT | BG_COL_CONT,          /* the paper's CD_MC sampling */
     BG_COBG_HELSUM_LC = BG_REC_COBG | BG_HEL_SUM | BG_COL_LC,
     BG_COBG_HELGIVEN_LC = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_LC
 };
@@ -97,6 +100,17 @@ int bg_init(bg_ctx** ctx, int n, int mode);
  */
 int bg_eval(bg_ctx* ctx, void* cuda_stream, long long N, const double* mom, const signed char* hel,
             const signed char* col, double* out);
+
+/*
+ * BG_CDBG_CONTINUOUS (n <= 9): |A|^2 of the colour-helicity sub-amplitude of Eq. 14 for continuous
+ * states - the colour-dressed recursion Eq. 28-32 with external currents  e(p_k, phi_k) x X_k,  e = cos(phi) e1 +
+ * sin(phi) e2 (Eq. 7; e1, e2 the unit vectors of the gauge of reading g2) and X_k[h][g] = etabar_k[h] eta_k[g]
+ * (Eq. 12 without its trace part, which decouples).  Summing/averaging over the states with the weights of Eq. 13
+ * is the caller's business.  DEVICE pointers, event-fastest:  phi[k*N + e];  eta[(k*6 + a)*N + e], a = 0..2 eta,
+ * a = 3..5 etabar (unit vectors).  Same stream / allocation rules as bg_eval.
+ */
+int bg_eval_continuous(bg_ctx* ctx, void* cuda_stream, long long N, const double* mom, const double* phi,
+                       const double* eta, double* out);
 
 /*
  * Same computation with HOST buffers (same layouts): copies inputs to the device, runs bg_eval on an internal

@@ -21,11 +21,13 @@ BG_COBG_HELSUM_FULLCOLOR = BG_REC_COBG | BG_HEL_SUM | BG_COL_FULL
 BG_COBG_HELGIVEN_FULLCOLOR = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_FULL
 BG_CDBG_GIVEN = BG_REC_CDBG | BG_HEL_GIVEN | BG_COL_GIVEN
 BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN
+BG_HEL_CONT, BG_COL_CONT = 0x040, 0x800
+BG_CDBG_CONTINUOUS = BG_REC_CDBG | BG_HEL_CONT | BG_COL_CONT
 BG_COBG_HELSUM_LC = BG_REC_COBG | BG_HEL_SUM | BG_COL_LC
 BG_COBG_HELGIVEN_LC = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_LC
 BG_OPT_KERNEL, BG_OPT_SCRATCH_LIMIT, BG_OPT_LANES, BG_OPT_TIMING, BG_OPT_SMEM_LIMIT, BG_OPT_PRECISION = 1, 2, 3, 4, 5, 6
 
-EXPORTS = ("bg_init", "bg_eval", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",
+EXPORTS = ("bg_init", "bg_eval", "bg_eval_continuous", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",
            "bg_set_option", "bg_colour_matrix", "bg_build_colour_matrix", "bg_last_launch_count",
            "bg_last_kernel_name", "bg_last_kernel_ms", "bg_class_program_stats", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe")
 
@@ -51,6 +53,8 @@ def load():
         lib.bg_init.argtypes = [ctypes.POINTER(vp), i, i]
         lib.bg_eval.argtypes = [vp, vp, ll, vp, vp, vp, vp]
         lib.bg_eval_host.argtypes = [vp, ll, vp, vp, vp, vp]
+        lib.bg_eval_continuous.argtypes = [vp, vp, ll, vp, vp, vp, vp]
+        lib.bg_eval_continuous.restype = i
         lib.bg_reserve.argtypes = [vp, ll]
         lib.bg_scratch_bytes.argtypes = [vp, ll]
         lib.bg_scratch_bytes.restype = ctypes.c_size_t
@@ -108,6 +112,12 @@ def bg_eval(ctx, stream, N: int, mom, hel, col, out) -> None:
     """Device pointers (or torch CUDA tensors); ``stream`` is a cudaStream_t as int (0/None = default stream)."""
     s = ctypes.c_void_p(int(stream)) if stream else None
     _check(load().bg_eval(ctx, s, N, _ptr(mom), _ptr(hel), _ptr(col), _ptr(out)), "bg_eval")
+
+
+def bg_eval_continuous(ctx, stream, N: int, mom, phi, eta, out) -> None:
+    """Device pointers; phi[n][N], eta[n][6][N] (eta then etabar), event-fastest."""
+    s = ctypes.c_void_p(int(stream)) if stream else None
+    _check(load().bg_eval_continuous(ctx, s, N, _ptr(mom), _ptr(phi), _ptr(eta), _ptr(out)), "bg_eval_continuous")
 
 
 def bg_eval_host(ctx, N: int, mom, hel, col, out) -> None:

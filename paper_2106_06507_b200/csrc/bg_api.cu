@@ -132,11 +132,16 @@ static int auto_lanes(int n) {
 // shared memory one event's state may take before its top levels spill to global memory (0 = all of it)
 static size_t auto_slab_limit(int n) { return n >= 11 ? (size_t)104 * 1024 : 0; }   // two blocks per SM (with their op rings), measured
 
+extern "C" {
+static int make_prog_table(const bg_ctx* c, int G, size_t limit, bg::ProgTable** t);
+}
+
 static bool mode_supported(int n, int mode) {
     if (n < 4 || n > 12) return false;
     if (mode == BG_COBG_HELSUM_FULLCOLOR || mode == BG_COBG_HELGIVEN_FULLCOLOR) return n <= 8;
     if (mode == BG_COBG_HELSUM_LC || mode == BG_COBG_HELGIVEN_LC) return bg::cobg_shared_supported(n);
     if (mode == BG_CDBG_GIVEN || mode == BG_CDBG_HELSUM_COLGIVEN) return true;
+    if (mode == BG_CDBG_CONTINUOUS) return n <= 9;
     return false;
 }
 
@@ -188,8 +193,8 @@ int bg_init(bg_ctx** out, int n, int mode) {
         const int rc = bg::cobg_table_create(n, &c->cobg);
         if (rc != BG_OK) { cudaFree(c->dC); std::free(c->hC); delete c; return rc; }
     }
-    if (mode == BG_CDBG_GIVEN && n <= kProgMaxN) {
-        const int rc = bg::prog_table_create(n, auto_lanes(n), auto_slab_limit(n), &c->prog);
+    if ((mode == BG_CDBG_GIVEN && n <= kProgMaxN) || mode == BG_CDBG_CONTINUOUS) {
+        const int rc = make_prog_table(c, 0, 0, &c->prog);
         if (rc != BG_OK) { delete c; return rc; }
     }
     bool streams_ok = cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking) == cudaSuccess &&
@@ -249,8 +254,16 @@ static long long dd_chunk(const bg_ctx* c, long long N) {
 }
 
 static bool use_prog(const bg_ctx* c) {
+    if (c->mode == BG_CDBG_CONTINUOUS) return c->prog != nullptr;
     if (c->mode != BG_CDBG_GIVEN || c->kernel_opt == 1 || use_dd(c)) return false;
     return c->prog != nullptr;
+}
+
+// lanes per event of the dense (continuous-state) program, and the table for the context's mode
+static int auto_lanes_dense(int n) { return n <= 4 ? 32 : (n == 5 ? 64 : 128); }
+static int make_prog_table(const bg_ctx* c, int G, size_t limit, bg::ProgTable** t) {
+    if (c->mode == BG_CDBG_CONTINUOUS) return bg::prog_table_create_dense(c->n, G ? G : auto_lanes_dense(c->n), limit, t);
+    return bg::prog_table_create(c->n, G ? G : auto_lanes(c->n), limit ? limit : auto_slab_limit(c->n), t);
 }
 
 // events per generic-CDBG launch under the scratch limit
@@ -325,15 +338,15 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
             c->kernel_opt = (int)value;
             return BG_OK;
         case BG_OPT_LANES: {
-            if (c->mode != BG_CDBG_GIVEN || c->n > kProgMaxN) return BG_EUNSUPPORTED;
+            if ((c->mode != BG_CDBG_GIVEN && c->mode != BG_CDBG_CONTINUOUS) || c->n > kProgMaxN) return BG_EUNSUPPORTED;
             if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32 &&
                 value != 64 && value != 128 && value != 256)
                 return BG_EINVAL;
-            const int G = value ? (int)value : auto_lanes(c->n);
-            if (c->prog && bg::prog_lanes(c->prog) == G) return BG_OK;
+            const int G = (int)value;
+            if (c->prog && G && bg::prog_lanes(c->prog) == G) return BG_OK;
             cudaDeviceSynchronize();
             bg::ProgTable* t = nullptr;
-            const int rc = bg::prog_table_create(c->n, G, c->slab_limit ? c->slab_limit : auto_slab_limit(c->n), &t);
+            const int rc = make_prog_table(c, G, c->slab_limit, &t);
             if (rc != BG_OK) return rc;
             bg::prog_table_destroy(c->prog);
             c->prog = t;
@@ -341,11 +354,11 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
             return BG_OK;
         }
         case BG_OPT_SMEM_LIMIT: {
-            if (c->mode != BG_CDBG_GIVEN || c->n > kProgMaxN || !c->prog) return BG_EUNSUPPORTED;
+            if ((c->mode != BG_CDBG_GIVEN && c->mode != BG_CDBG_CONTINUOUS) || !c->prog) return BG_EUNSUPPORTED;
             if (value != 0 && (value < 16 * 1024 || value > 222 * 1024)) return BG_EINVAL;
             cudaDeviceSynchronize();
             bg::ProgTable* t = nullptr;
-            const int rc = bg::prog_table_create(c->n, bg::prog_lanes(c->prog), value ? (size_t)value : auto_slab_limit(c->n), &t);
+            const int rc = make_prog_table(c, bg::prog_lanes(c->prog), (size_t)value, &t);
             if (rc != BG_OK) return rc;
             bg::prog_table_destroy(c->prog);
             c->prog = t;
@@ -419,7 +432,7 @@ const char* bg_last_kernel_name(const bg_ctx* c) { return c ? c->last_kernel : "
 
 int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const signed char* hel,
             const signed char* col, double* out) {
-    if (!c || N < 0) return BG_EINVAL;
+    if (!c || N < 0 || c->mode == BG_CDBG_CONTINUOUS) return BG_EINVAL;   // continuous states: bg_eval_continuous
     c->last_launches = 0;
     if (N == 0) return BG_OK;
     if (!mom || !out) return BG_EINVAL;
@@ -482,6 +495,23 @@ int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const 
         if (ev1) cudaEventRecord(ev1, s);
         c->last_kernel = "cdbg_generic_kernel";
     }
+    return err == cudaSuccess ? BG_OK : BG_ECUDA;
+}
+
+int bg_eval_continuous(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const double* phi,
+                       const double* eta, double* out) {
+    if (!c || N < 0 || c->mode != BG_CDBG_CONTINUOUS) return BG_EINVAL;
+    c->last_launches = 0;
+    if (N == 0) return BG_OK;
+    if (!mom || !phi || !eta || !out || !c->prog) return BG_EINVAL;
+    int rc = ensure_scratch(c, N);
+    if (rc != BG_OK) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaEvent_t ev0 = c->timing ? c->ev0 : nullptr, ev1 = c->timing ? c->ev1 : nullptr;
+    c->timed = c->timing != 0;
+    const cudaError_t err = bg::cdbg_dense_launch(s, c->prog, c->sm_count, N, mom, phi, eta, out, c->scratch,
+                                                  &c->last_launches, ev0, ev1);
+    c->last_kernel = "cdbg_prog_kernel";
     return err == cudaSuccess ? BG_OK : BG_ECUDA;
 }
 

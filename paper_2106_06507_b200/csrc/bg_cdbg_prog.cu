@@ -68,6 +68,8 @@ struct ProgTable {
     long long num_classes;
     int max_state_cx;
     TierInfo tiers;
+    bool dense;               // continuous colour states: one program, nine colour entries per subset current
+    int rec_bytes;            // bytes of one event record
     bool spill;               // largest state blocks exceed the slab limit: top of the state in global memory
     int spill_blocks_per_sm;  // resident blocks per SM of the spill kernels (each owns one global slab)
     int sm_count;
@@ -86,7 +88,8 @@ struct ProgParams {
     const ClassInfo* info;
     const ProgOp* ops;
     const char* rec;           // [N] event records (header + canonical momenta) grouped by class
-    int rec_bytes;             // 32 + 32 n
+    int rec_bytes;             // 32 + 32 n (discrete states) or 32 + 96 n (continuous states)
+    int rec_gstride;           // doubles per gluon in a record: 4 or 12
     const uint32_t* bounds;    // [kTiers + 1] record positions where the tiers start (bounds[kTiers] = N)
     int tier;
     int slab_cx;               // complex doubles of state per event in the shared-memory slab
@@ -545,11 +548,37 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                         st_.st(offPt, mk(Pt[0], Pt[1]));
                         st_.st(offPt + 1, mk(Pt[2], Pt[3]));
                     }
+                } else if (flags & OPF_EXTD) {
+                    // continuous states (Eq. 7, 9, 12): real polarisation e(phi) times the colour matrix etabar_h eta_g;
+                    // record per gluon: p (4), phi, eta (3), etabar (3), pad
+                    const int k = (int)raw.w;
+                    const double* gr = mrec + k * p.rec_gstride;
+                    double pk[4], ev[4], eta[3], etab[3];
+#pragma unroll
+                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(gr + c);
+                    const double phi = __ldcg(gr + 4);
+#pragma unroll
+                    for (int c = 0; c < 3; c++) { eta[c] = __ldcg(gr + 5 + c); etab[c] = __ldcg(gr + 8 + c); }
+                    polarisation_real(pk, phi, ev);
+                    const bool closure_leg = offPt == 0xFFFF;   // gluon n: no momentum slot; target (h,g) reads X_n[g][h]
+#pragma unroll
+                    for (int h = 0; h < 3; h++)
+#pragma unroll
+                        for (int gg = 0; gg < 3; gg++) {
+                            const double x = etab[h] * eta[gg];
+                            const int at = offDst + 4 * (h * 3 + gg);
+#pragma unroll
+                            for (int c = 0; c < 4; c++) st_.st(at + c, mk(x * ev[c], 0.0));
+                        }
+                    if (!closure_leg) {
+                        st_.st(offPt, mk(pk[0], pk[1]));
+                        st_.st(offPt + 1, mk(pk[2], pk[3]));
+                    }
                 } else if (flags & OPF_EXT) {
                     const int k = (int)raw.w;
                     double pk[4];
 #pragma unroll
-                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + k * 4 + c);   // not through L1: it is kept for the ops
+                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + k * p.rec_gstride + c);   // not through L1: it is kept for the ops
                     cx eps[4];
                     polarisation(pk, ((perm >> (48 + k)) & 1) ? 1 : -1, eps);
 #pragma unroll
@@ -693,6 +722,8 @@ int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out) {
     if (!t) return BG_ENOMEM;
     std::memset(t, 0, sizeof(*t));
     t->n = n; t->G = G; t->num_classes = nc; t->max_state_cx = max_state; t->tiers = tiers;
+    t->dense = false;
+    t->rec_bytes = kRecHeaderBytes + 32 * n;
     t->spill = spill;
     {   // blocks of the largest tier that fit an SM (shared memory and registers)
         const size_t smem0 = (size_t)tiers.slab_cx[0] * 16;
@@ -729,6 +760,87 @@ int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out) {
     return BG_OK;
 }
 
+// ---- continuous colour / polarisation states (Eq. 5-14): one dense program ----------
+int prog_table_create_dense(int n, int G, size_t slab_limit, ProgTable** out) {
+    *out = nullptr;
+    if (slab_limit == 0 || slab_limit > kMaxSlabBytes) slab_limit = kMaxSlabBytes;
+    if (n < 4 || n > kMaxN || G < 32 || G > 256 || (G & (G - 1))) return BG_EINVAL;
+    ClassProgram cp;
+    int code[kMaxN] = {0};
+    build_program(n, G, code, cp, true);
+    if (!cp.valid || cp.state_cx > 65535) return BG_EUNSUPPORTED;
+    const bool spill = (size_t)cp.state_cx * 16 > slab_limit;
+    if (spill && G < 128) return BG_EUNSUPPORTED;
+    ClassInfo ci;
+    std::memset(&ci, 0, sizeof(ci));
+    ci.valid = 1;
+    ci.state_cx = (uint16_t)cp.state_cx;
+    ci.total_steps = (uint32_t)cp.total_steps;
+    ci.n_sync = (uint32_t)cp.n_sync;
+    std::vector<ProgOp> ops = cp.ops;
+    ProgOp nop;
+    std::memset(&nop, 0, sizeof(nop));
+    ops.insert(ops.end(), (size_t)kRing * G, nop);
+    ProgTable* t = new (std::nothrow) ProgTable();
+    if (!t) return BG_ENOMEM;
+    std::memset(t, 0, sizeof(*t));
+    t->n = n; t->G = G; t->num_classes = 1; t->max_state_cx = cp.state_cx;
+    t->dense = true;
+    t->rec_bytes = kRecHeaderBytes + 96 * n;
+    for (int k = 0; k < kTiers; k++) {
+        t->tiers.slab_cx[k] = std::min<int>(cp.state_cx, (int)(slab_limit / 16));
+        t->tiers.first_key[k] = k == 0 ? 0 : 1;
+    }
+    t->tiers.first_key[kTiers] = 1;
+    t->spill = spill;
+    {
+        const size_t smem0 = (size_t)t->tiers.slab_cx[0] * 16;
+        const int block = G > 32 ? G : 32;
+        t->spill_blocks_per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * block), (228 * 1024) / (smem0 + 1024)));
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    }
+    t->ops_bytes = ops.size() * sizeof(ProgOp);
+    bool ok = cudaMalloc(&t->d_info, sizeof(ClassInfo)) == cudaSuccess && cudaMalloc(&t->d_ops, t->ops_bytes) == cudaSuccess;
+    ok = ok && cudaMemcpy(t->d_info, &ci, sizeof(ci), cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(t->d_ops, ops.data(), t->ops_bytes, cudaMemcpyHostToDevice) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        prog_table_destroy(t);
+        return BG_ENOMEM;
+    }
+    *out = t;
+    return BG_OK;
+}
+
+// one record per event, in input order: header | per gluon p (4), phi, eta (3), etabar (3), pad
+__global__ void __launch_bounds__(256)
+cdbg_pack_continuous_kernel(int n, long long N, const double* __restrict__ mom, const double* __restrict__ phi,
+                            const double* __restrict__ eta, char* __restrict__ rec, int rec_bytes,
+                            uint32_t* __restrict__ bounds) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e == 0) {
+        bounds[0] = 0;
+        for (int k = 1; k <= kTiers; k++) bounds[k] = (uint32_t)N;
+    }
+    if (e >= N) return;
+    char* r = rec + (size_t)e * rec_bytes;
+    EventHeader h;
+    h.event = (uint32_t)e; h.cls = 0; h.perm = 0;
+    for (int k = 0; k < n; k++) h.perm |= (uint64_t)k << (4 * k);
+    *reinterpret_cast<EventHeader*>(r) = h;
+    double2* g = reinterpret_cast<double2*>(r + kRecHeaderBytes);
+    for (int k = 0; k < n; k++) {
+        double v[12];
+        for (int c = 0; c < 4; c++) v[c] = mom[(size_t)(k * 4 + c) * N + e];
+        v[4] = phi[(size_t)k * N + e];
+        for (int c = 0; c < 6; c++) v[5 + c] = eta[(size_t)(k * 6 + c) * N + e];
+        v[11] = 0.0;
+        for (int c = 0; c < 6; c++) g[k * 6 + c] = make_double2(v[2 * c], v[2 * c + 1]);
+    }
+}
+
 void prog_table_destroy(ProgTable* t) {
     if (!t) return;
     if (t->d_info) cudaFree(t->d_info);
@@ -742,7 +854,7 @@ int prog_lanes(const ProgTable* t) { return t ? t->G : 0; }
 
 // scratch: records (32 + 32 n) B x N | perm u64[N] | cls u32[N] | hist u32[num_classes + 1] | tier bounds | spill slabs
 static size_t prog_spill_offset(const ProgTable* t, long long N) {
-    return (((size_t)N * (44 + 32 * t->n) + ((size_t)t->num_classes + 1) * 4 + 256) + 255) / 256 * 256;
+    return (((size_t)N * (12 + t->rec_bytes) + ((size_t)t->num_classes + 1) * 4 + 256) + 255) / 256 * 256;
 }
 size_t prog_scratch_bytes(const ProgTable* t, long long N) {
     // spill kernels run one block per SM, each with a slab for the part of the largest state beyond shared memory
@@ -780,10 +892,32 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
     return cudaGetLastError();
 }
 
+static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches) {
+    cudaError_t err;
+    switch (t->G) {
+        case 1: err = launch_interp<1, false>(s, t, sm_count, p, launches); break;
+        case 2: err = launch_interp<2, false>(s, t, sm_count, p, launches); break;
+        case 4: err = launch_interp<4, false>(s, t, sm_count, p, launches); break;
+        case 8: err = launch_interp<8, false>(s, t, sm_count, p, launches); break;
+        case 16: err = launch_interp<16, false>(s, t, sm_count, p, launches); break;
+        case 32: err = launch_interp<32, false>(s, t, sm_count, p, launches); break;
+        case 64: err = launch_interp<64, false>(s, t, sm_count, p, launches); break;
+        case 128:
+            err = t->spill ? launch_interp<128, true>(s, t, sm_count, p, launches)
+                           : launch_interp<128, false>(s, t, sm_count, p, launches);
+            break;
+        default:
+            err = t->spill ? launch_interp<256, true>(s, t, sm_count, p, launches)
+                           : launch_interp<256, false>(s, t, sm_count, p, launches);
+            break;
+    }
+    return err;
+}
+
 cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
                              const signed char* hel, const signed char* col, double* out, void* scratch,
                              int* launches, cudaEvent_t ev0, cudaEvent_t ev1) {
-    const int rec_bytes = kRecHeaderBytes + 32 * t->n;
+    const int rec_bytes = t->rec_bytes;
     char* rec = (char*)scratch;
     uint64_t* perm = (uint64_t*)(rec + (size_t)N * rec_bytes);
     uint32_t* cls = (uint32_t*)(perm + N);
@@ -818,7 +952,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     if ((err = cudaGetLastError()) != cudaSuccess) return err;
     ProgParams p;
     p.n = t->n; p.N = N; p.out = out;
-    p.info = t->d_info; p.ops = t->d_ops; p.rec = rec; p.rec_bytes = rec_bytes;
+    p.info = t->d_info; p.ops = t->d_ops; p.rec = rec; p.rec_bytes = rec_bytes; p.rec_gstride = 4;
     p.bounds = bounds;
     p.spill = t->spill ? (double2*)((char*)scratch + prog_spill_offset(t, N)) : nullptr;
     p.spill_cx = t->max_state_cx;
@@ -826,23 +960,31 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.slab_cx = t->max_state_cx;
     *launches = 3;
     if (ev0) cudaEventRecord(ev0, s);
-    switch (t->G) {
-        case 1: err = launch_interp<1, false>(s, t, sm_count, p, launches); break;
-        case 2: err = launch_interp<2, false>(s, t, sm_count, p, launches); break;
-        case 4: err = launch_interp<4, false>(s, t, sm_count, p, launches); break;
-        case 8: err = launch_interp<8, false>(s, t, sm_count, p, launches); break;
-        case 16: err = launch_interp<16, false>(s, t, sm_count, p, launches); break;
-        case 32: err = launch_interp<32, false>(s, t, sm_count, p, launches); break;
-        case 64: err = launch_interp<64, false>(s, t, sm_count, p, launches); break;
-        case 128:
-            err = t->spill ? launch_interp<128, true>(s, t, sm_count, p, launches)
-                           : launch_interp<128, false>(s, t, sm_count, p, launches);
-            break;
-        default:
-            err = t->spill ? launch_interp<256, true>(s, t, sm_count, p, launches)
-                           : launch_interp<256, false>(s, t, sm_count, p, launches);
-            break;
-    }
+    err = dispatch_interp(s, t, sm_count, p, launches);
+    if (ev1) cudaEventRecord(ev1, s);
+    return err;
+}
+
+cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
+                              const double* phi, const double* eta, double* out, void* scratch, int* launches,
+                              cudaEvent_t ev0, cudaEvent_t ev1) {
+    char* rec = (char*)scratch;
+    // same scratch layout as the discrete path (perm / cls / histogram areas stay unused)
+    uint32_t* bounds = (uint32_t*)(rec + (size_t)N * (t->rec_bytes + 12)) + ((size_t)t->num_classes + 1);
+    cdbg_pack_continuous_kernel<<<(unsigned)((N + 255) / 256), 256, 0, s>>>(t->n, N, mom, phi, eta, rec, t->rec_bytes, bounds);
+    cudaError_t err = cudaGetLastError();
+    if (err != cudaSuccess) return err;
+    ProgParams p;
+    p.n = t->n; p.N = N; p.out = out;
+    p.info = t->d_info; p.ops = t->d_ops; p.rec = rec; p.rec_bytes = t->rec_bytes; p.rec_gstride = 12;
+    p.bounds = bounds;
+    p.spill = t->spill ? (double2*)((char*)scratch + prog_spill_offset(t, N)) : nullptr;
+    p.spill_cx = t->max_state_cx;
+    p.tier = 0;
+    p.slab_cx = t->max_state_cx;
+    *launches = 1;
+    if (ev0) cudaEventRecord(ev0, s);
+    err = dispatch_interp(s, t, sm_count, p, launches);
     if (ev1) cudaEventRecord(ev1, s);
     return err;
 }

@@ -69,6 +69,7 @@ cudaError_t cobg_dd_launch(cudaStream_t s, int n, bool helsum, int nperm, const 
 
 // ---- colour-class program interpreter (bg_cdbg_prog.cu): G lanes per event, currents in shared memory -------
 int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out);   // BG_* code; slab_limit 0 = all of shared memory
+int prog_table_create_dense(int n, int G, size_t slab_limit, ProgTable** out);   // continuous states (one program)
 void prog_table_destroy(ProgTable* t);
 size_t prog_state_bytes(const ProgTable* t);               // largest per-event state block
 int prog_lanes(const ProgTable* t);
@@ -76,6 +77,10 @@ size_t prog_scratch_bytes(const ProgTable* t, long long N);
 cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
                              const signed char* hel, const signed char* col, double* out, void* scratch,
                              int* launches, cudaEvent_t ev0, cudaEvent_t ev1);
+
+cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
+                              const double* phi, const double* eta, double* out, void* scratch, int* launches,
+                              cudaEvent_t ev0, cudaEvent_t ev1);
 
 // ---- shared-current COBG kernel (bg_cobg_shared.cu): one thread group per event, n <= 7 -----------------------
 bool cobg_shared_supported(int n);

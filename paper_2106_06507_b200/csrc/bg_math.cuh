@@ -83,6 +83,30 @@ __device__ __forceinline__ void polarisation(const double* p, int lambda, cx* ep
     eps[3] = mk(l * e1z, 0.0);
 }
 
+// Real polarisation vector of the continuous sampling, Eq. 7: e(p, phi) = cos(phi) e1 + sin(phi) e2
+// with the unit vectors e1, e2 of the same gauge as `polarisation` (eps^lambda = (-lambda e1 - i e2)/sqrt2).
+__device__ __forceinline__ void polarisation_real(const double* p, double phi, double* e) {
+    const double s = p[0] < 0.0 ? -1.0 : 1.0;
+    const double qx = s * p[1], qy = s * p[2], qz = s * p[3];
+    const double qt2 = qx * qx + qy * qy;
+    const double qt = sqrt(qt2), qa = sqrt(qt2 + qz * qz);
+    double e1x, e1y, e1z, e2x, e2y;
+    if (qt < 1e-9 * qa) {
+        e1x = 1.0; e1y = 0.0; e1z = 0.0;
+        e2x = 0.0; e2y = qz < 0.0 ? -1.0 : 1.0;
+    } else {
+        const double inv = 1.0 / (qa * qt), invt = 1.0 / qt;
+        e1x = qx * qz * inv; e1y = qy * qz * inv; e1z = -qt / qa;
+        e2x = -qy * invt; e2y = qx * invt;
+    }
+    double sn, cs;
+    sincos(phi, &sn, &cs);
+    e[0] = 0.0;
+    e[1] = cs * e1x + sn * e2x;
+    e[2] = cs * e1y + sn * e2y;
+    e[3] = cs * e1z;
+}
+
 // acc += sign * sqrt2 * V3(p,q;a,b)   [Eq. 21 first line: (a.b)(p-q) + ((2q+p).a) b - ((2p+q).b) a]
 __device__ __forceinline__ void v3_acc(cx* acc, const double* p, const double* q, const cx* a, const cx* b,
                                        double sign) {

@@ -27,8 +27,10 @@ long long class_rank(int n, const int* m) {
 
 namespace {
 
-// colour type of a subset current: 0x40 dead | 0x80|mask diagonal entries | (h<<2)|g one off-diagonal entry
+// colour type of a subset current: 0x40 dead | 0x80|mask diagonal entries | (h<<2)|g one off-diagonal entry |
+// 0xFF all nine entries (continuous colour states)
 inline bool has_entry(unsigned t, int h, int g) {
+    if (t == 0xFFu) return true;
     if (t & 0x80u) return h == g && ((t >> h) & 1u);
     if (t & 0x40u) return false;
     return t == (unsigned)((h << 2) | g);
@@ -43,19 +45,26 @@ struct Target {
     int pi, h, g;
     bool store_p = false;   // its LAST op also stores P(pi) (one entry per subset whose momentum is read later)
     bool used = false;      // read by a later vertex (dead-code elimination)
-    bool fused = false;     // |pi| = n-2: not stored; its closure contribution is taken from registers
-    VOp fuse;               // the closure vertex X(eps_k, this) of a fused target (pb = this entry)
+    bool fused = false;     // |pi| = n-2: not stored; its closure contributions are taken from registers
+    std::vector<std::pair<VOp, int>> fuses;   // closure vertices X(eps_k, this) (pb = this entry) and their closure entry
     std::vector<VOp> ops;
-    int slot() const { return h == g ? h : 0; }
+    int s = 0;              // slot of the entry inside its subset
+    int slot() const { return s; }
 };
 
 inline int popc(int x) { return __builtin_popcount((unsigned)x); }
 
 }  // namespace
 
-void build_program(int n, int G, const int* code, ClassProgram& out) {
+void build_program(int n, int G, const int* code, ClassProgram& out, bool dense) {
     out = ClassProgram();
     const int m = n - 1, nsub = 1 << m, full = nsub - 1;
+    // dense: every gluon carries a full 3x3 colour matrix (continuous colour states) - all nine entries of every
+    // subset current are live and `code` is ignored; otherwise elementary matrices e_ij and at most 3 live entries
+    const int SL = dense ? 9 : 3;
+    auto slot_of = [&](int h, int g) { return dense ? h * 3 + g : (h == g ? h : 0); };
+    int dummy_code[kMaxN] = {0};
+    if (dense) code = dummy_code;
     int ci[kMaxN], cj[kMaxN], wk[kMaxN];
     for (int k = 0; k < n; k++) {
         ci[k] = code[k] / 3;
@@ -67,18 +76,21 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
     // ---- phase 1: which entries of which subsets are non-zero, and the vertex evaluations that feed them ----
     std::vector<uint8_t> type(nsub, 0x40);
     for (int k = 0; k < m; k++)
-        type[1 << k] = ci[k] == cj[k] ? (uint8_t)(0x80u | (1u << ci[k])) : (uint8_t)((ci[k] << 2) | cj[k]);
+        type[1 << k] = dense ? (uint8_t)0xFF : (ci[k] == cj[k] ? (uint8_t)(0x80u | (1u << ci[k])) : (uint8_t)((ci[k] << 2) | cj[k]));
     std::vector<std::vector<Target>> levels(m + 1);   // by popcount
-    std::vector<int> tindex(nsub * 3, -1);            // (subset, slot) -> index in its level
+    std::vector<int> tindex(nsub * SL, -1);           // (subset, slot) -> index in its level
     for (int pi = 3; pi <= full; pi++) {
         if ((pi & (pi - 1)) == 0) continue;
         const int low = pi & -pi, rest = pi ^ low;
         int D = 0;
         for (int k = 0; k < m; k++)
             if ((pi >> k) & 1) D += wk[k];
-        int cand_h[3], cand_g[3], ncand = 0;
+        int cand_h[9], cand_g[9], ncand = 0;
         bool diag = false;
-        if (D == 0) {
+        if (dense) {
+            for (int h = 0; h < 3; h++)
+                for (int g = 0; g < 3; g++) { cand_h[ncand] = h; cand_g[ncand] = g; ncand++; }
+        } else if (D == 0) {
             diag = true;
             for (int h = 0; h < 3; h++) { cand_h[ncand] = h; cand_g[ncand] = h; ncand++; }
         } else {
@@ -86,7 +98,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
                 for (int g = 0; g < 3; g++)
                     if (h != g && D == (1 << (8 * h)) - (1 << (8 * g))) { cand_h[0] = h; cand_g[0] = g; ncand = 1; }
         }
-        if (pi == full) {
+        if (pi == full && !dense) {
             // closure, Eq. 22: only the entry contracted with X_n = e_{i_n j_n}
             const int h = cj[n - 1], g = ci[n - 1];
             bool ok = false;
@@ -98,11 +110,11 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
         for (int cd = 0; cd < ncand; cd++) {
             const int h = cand_h[cd], g = cand_g[cd];
             Target t;
-            t.pi = pi; t.h = h; t.g = g;
+            t.pi = pi; t.h = h; t.g = g; t.s = slot_of(h, g);
             for (int sub = (rest - 1) & rest;; sub = (sub - 1) & rest) {
                 const int p1 = low | sub, p2 = pi ^ p1;
                 const unsigned t1 = type[p1], t2 = type[p2];
-                if (!((t1 | t2) & 0x40u)) {
+                if (t1 != 0x40u && t2 != 0x40u) {
                     for (int k = 0; k < 3; k++) {
                         const bool fwd = has_entry(t1, h, k) && has_entry(t2, k, g);
                         const bool bwd = has_entry(t2, h, k) && has_entry(t1, k, g);
@@ -112,8 +124,8 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
                             const int ah = dir == 0 ? h : k, ag = dir == 0 ? k : g;   // entry of pi_1
                             const int bh = dir == 0 ? k : h, bg_ = dir == 0 ? g : k;  // entry of pi_2
                             VOp o;
-                            o.pa = p1; o.sa = ah == ag ? ah : 0;
-                            o.pb = p2; o.sb = bh == bg_ ? bh : 0;
+                            o.pa = p1; o.sa = slot_of(ah, ag);
+                            o.pb = p2; o.sb = slot_of(bh, bg_);
                             o.neg = dir == 1;
                             if (popc(o.pa) > popc(o.pb)) {   // X(a,b) = -X(b,a): keep the smaller subset as `a`
                                 std::swap(o.pa, o.pb);
@@ -128,12 +140,12 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
             }
             if (t.ops.empty()) continue;
             livemask |= diag ? (1u << h) : 1u;
-            tindex[pi * 3 + t.slot()] = (int)levels[popc(pi)].size();
+            tindex[pi * SL + t.slot()] = (int)levels[popc(pi)].size();
             levels[popc(pi)].push_back(std::move(t));
         }
         if (pi != full) {
             uint8_t ty = 0x40u;
-            if (livemask) ty = diag ? (uint8_t)(0x80u | livemask) : (uint8_t)((cand_h[0] << 2) | cand_g[0]);
+            if (livemask) ty = dense ? (uint8_t)0xFF : (diag ? (uint8_t)(0x80u | livemask) : (uint8_t)((cand_h[0] << 2) | cand_g[0]));
             type[pi] = ty;
         }
     }
@@ -143,19 +155,19 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
     // that hold the just-finished J(pi), T(pi) ("fused": those currents are never stored), and entries that no
     // later vertex reads are dropped ----
     {
-        Target& clo = levels[m][0];
-        clo.used = true;
-        if (m - 1 >= 2) {
+        for (auto& clo : levels[m]) {
+            clo.used = true;
+            if (m - 1 < 2) continue;
+            // the closure entry (h,g) is contracted with eps_n X_n[g][h]: index of that vector behind off_epsn
+            const int centry = dense ? clo.g * 3 + clo.h : 0;
             std::vector<VOp> keep;
             for (auto& v : clo.ops) {
                 if (popc(v.pa) == 1 && popc(v.pb) == m - 1) {
-                    Target& t = levels[m - 1][tindex[v.pb * 3 + v.sb]];
-                    if (!t.fused) {   // at most one closure vertex reads a given entry
-                        t.fused = true;
-                        t.fuse = v;
-                        t.used = true;
-                        continue;
-                    }
+                    Target& t = levels[m - 1][tindex[v.pb * SL + v.sb]];
+                    t.fused = true;
+                    t.fuses.push_back({v, centry});
+                    t.used = true;
+                    continue;
                 }
                 keep.push_back(v);
             }
@@ -165,8 +177,8 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
             for (auto& t : levels[pc]) {
                 if (!t.used) continue;
                 for (auto& v : t.ops) {
-                    if (popc(v.pa) >= 2) levels[popc(v.pa)][tindex[v.pa * 3 + v.sa]].used = true;
-                    if (popc(v.pb) >= 2) levels[popc(v.pb)][tindex[v.pb * 3 + v.sb]].used = true;
+                    if (popc(v.pa) >= 2) levels[popc(v.pa)][tindex[v.pa * SL + v.sa]].used = true;
+                    if (popc(v.pb) >= 2) levels[popc(v.pb)][tindex[v.pb * SL + v.sb]].used = true;
                 }
             }
         for (int pc = 2; pc < m; pc++) {
@@ -178,25 +190,29 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
     }
 
     // ---- phase 3: state layout (units of one complex double) ----
-    std::vector<int> off(nsub * 3, -1), poff(nsub, -1);
+    std::vector<int> off(nsub * SL, -1), poff(nsub, -1);
     std::vector<char> need_p(nsub, 0);
     for (int pc = 2; pc <= m; pc++)
         for (auto& t : levels[pc])
             for (auto& v : t.ops) { need_p[v.pa] = 1; need_p[v.pb] = 1; }
     int next = 0;
     for (int k = 0; k < m; k++) {
-        off[(1 << k) * 3 + (ci[k] == cj[k] ? ci[k] : 0)] = next;
-        next += 4;
+        if (dense) {
+            for (int hg = 0; hg < 9; hg++) { off[(1 << k) * SL + hg] = next; next += 4; }   // eps_k X_k[h][g], hg = 3h+g
+        } else {
+            off[(1 << k) * SL + slot_of(ci[k], cj[k])] = next;
+            next += 4;
+        }
     }
-    const int off_epsn = next;
-    next += 4;
+    const int off_epsn = next;      // eps_n (dense: the nine vectors eps_n X_n[g][h] at index 3g+h)
+    next += dense ? 36 : 4;
     for (int k = 0; k < m; k++) { poff[1 << k] = next; next += 2; }
     // With fewer than 8 events per warp the bank group of an element depends on its offset: one element of padding
     // after every entry makes the entry starts run through all residues (10 + 2 would only ever give multiples of 4).
     const int pad = G >= 8 ? 1 : 0;
     for (int pc = 2; pc < m; pc++)
         for (auto& t : levels[pc]) {
-            if (!t.fused) { off[t.pi * 3 + t.slot()] = next; next += 10 + pad; }
+            if (!t.fused) { off[t.pi * SL + t.slot()] = next; next += 10 + pad; }
             if (need_p[t.pi] && poff[t.pi] < 0) { poff[t.pi] = next; next += 2; t.store_p = true; }
         }
     out.level_steps.assign(2 * m - 2, 0);   // setup | (main, combine) per popcount 2..n-2 | closure
@@ -269,11 +285,11 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
         for (int k = 0; k < n; k++) {
             ProgOp o;
             std::memset(&o, 0, sizeof(o));
-            o.flags = OPF_EXT;
+            o.flags = OPF_EXT | (dense ? OPF_EXTD : 0);
             o.extra = (uint32_t)k;
             if (k < m) {
                 const int pi = 1 << k;
-                o.offDst = (uint16_t)off[pi * 3 + (ci[k] == cj[k] ? ci[k] : 0)];
+                o.offDst = (uint16_t)off[pi * SL + (dense ? 0 : slot_of(ci[k], cj[k]))];
                 o.offPt = (uint16_t)poff[pi];
             } else {
                 o.offDst = (uint16_t)off_epsn;
@@ -287,15 +303,28 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
     auto make_op = [&](const Target& t, const VOp& v) {
         ProgOp o;
         std::memset(&o, 0, sizeof(o));
-        o.offA = (uint16_t)off[v.pa * 3 + v.sa];
-        o.offB = (uint16_t)off[v.pb * 3 + v.sb];
+        o.offA = (uint16_t)off[v.pa * SL + v.sa];
+        o.offB = (uint16_t)off[v.pb * SL + v.sb];
         o.offP1 = (uint16_t)poff[v.pa];
         o.extra = (uint32_t)poff[v.pb];
         o.offPt = t.store_p ? (uint16_t)poff[t.pi] : (uint16_t)0xFFFF;
-        o.offDst = t.pi == full ? (uint16_t)off_epsn : (t.fused ? (uint16_t)0xFFFF : (uint16_t)off[t.pi * 3 + t.slot()]);
+        o.offDst = t.pi == full ? (uint16_t)(off_epsn + (dense ? 4 * (t.g * 3 + t.h) : 0))
+                                : (t.fused ? (uint16_t)0xFFFF : (uint16_t)off[t.pi * SL + t.slot()]);
         o.flags = OPF_VALID | (v.neg ? OPF_NEG : 0) | (popc(v.pa) >= 2 ? OPF_TENA : 0) |
                   (popc(v.pb) >= 2 ? OPF_TENB : 0) | (t.pi == full ? OPF_CLOSURE : 0);
         return o;
+    };
+    auto push_fuses = [&](std::vector<ProgOp>& lane, const Target& t) {
+        for (auto& fz : t.fuses) {
+            ProgOp o;
+            std::memset(&o, 0, sizeof(o));
+            o.offA = (uint16_t)off[fz.first.pa * SL + fz.first.sa];
+            o.offP1 = (uint16_t)poff[fz.first.pa];
+            o.offDst = (uint16_t)(off_epsn + 4 * fz.second);
+            o.flags = OPF_FUSED | (fz.first.neg ? OPF_NEG : 0);
+            lane.push_back(o);
+            out.n_vertex_ops++;
+        }
     };
     auto push_target = [&](std::vector<ProgOp>& lane, const Target& t) {
         for (size_t i = 0; i < t.ops.size(); i++) {
@@ -306,16 +335,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
             lane.push_back(o);
             out.n_vertex_ops++;
         }
-        if (t.fused) {
-            ProgOp o;
-            std::memset(&o, 0, sizeof(o));
-            o.offA = (uint16_t)off[t.fuse.pa * 3 + t.fuse.sa];
-            o.offP1 = (uint16_t)poff[t.fuse.pa];
-            o.offDst = (uint16_t)off_epsn;
-            o.flags = OPF_FUSED | (t.fuse.neg ? OPF_NEG : 0);
-            lane.push_back(o);
-            out.n_vertex_ops++;
-        }
+        push_fuses(lane, t);
     };
 
     // A unit of work is a run of vertices of one target that one lane accumulates in its registers: the whole
@@ -328,23 +348,34 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
         std::vector<std::vector<ProgOp>> lanes(G), clanes(G);
         auto& tg = levels[pc];
         if (pc == m) {
-            // closure: one target, its remaining vertices dealt round-robin; every lane contracts its partial
-            // sum with eps_n and the lanes' amplitudes are added at the end
-            const Target& t = tg[0];
-            for (size_t i = 0; i < t.ops.size(); i++) {
-                lanes[i % G].push_back(make_op(t, t.ops[i]));
-                out.n_vertex_ops++;
-            }
-            for (auto& l : lanes)
-                if (!l.empty()) { l.front().flags |= OPF_FIRST; l.back().flags |= OPF_LAST; }
+            // closure: every lane contracts the partial sum of its run with the closure vector of that target
+            // (eps_n, or eps_n X_n[g][h]) and the lanes' amplitudes are added at the end, so the closure targets can
+            // be cut into runs of any length without scratch
+            long long total = 0;
+            for (auto& t : tg) total += (long long)t.ops.size();
+            const int chunk = std::max<int>(1, (int)((total + G - 1) / G));
+            std::vector<int> load(G, 0);
+            for (auto& t : tg)
+                for (size_t lo = 0; lo < t.ops.size(); lo += chunk) {
+                    const size_t hi = std::min(t.ops.size(), lo + chunk);
+                    const int l = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+                    load[l] += (int)(hi - lo);
+                    for (size_t i = lo; i < hi; i++) {
+                        ProgOp o = make_op(t, t.ops[i]);
+                        if (i == lo) o.flags |= OPF_FIRST;
+                        if (i + 1 == hi) o.flags |= OPF_LAST;
+                        lanes[l].push_back(o);
+                        out.n_vertex_ops++;
+                    }
+                }
             reduce_bank_conflicts(lanes);
             emit_level(2 * (pc - 2) + 1, lanes);
             break;
         }
         long long total = 0;
-        for (auto& t : tg) total += (long long)t.ops.size() + (t.fused ? 1 : 0);
+        for (auto& t : tg) total += (long long)t.ops.size() + (long long)t.fuses.size();
         const int ideal = (int)((total + G - 1) / G);
-        auto ucost = [&](const Unit& u) { return u.count + (u.part < 0 && tg[u.target].fused ? 1 : 0); };
+        auto ucost = [&](const Unit& u) { return u.count + (u.part < 0 ? (int)tg[u.target].fuses.size() : 0); };
         // Units no larger than chunk_max vertices; the number of steps the level then needs (longest-processing-
         // time rule).  A chunk size equal to the ideal step count often leaves slightly more units than lanes and costs a
         // second round, so slightly larger sizes are tried and the one with the fewest steps (then chunks) is kept.
@@ -358,7 +389,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
             nscratch = 0;
             for (size_t i = 0; i < tg.size(); i++) {
                 const int c = (int)tg[i].ops.size();
-                if (G == 1 || c + (tg[i].fused ? 1 : 0) <= chunk_max || c < 4) {
+                if (G == 1 || c + (int)tg[i].fuses.size() <= chunk_max || c < 4) {
                     units.push_back({(int)i, 0, c, -1});
                     continue;
                 }
@@ -419,16 +450,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out) {
             o.flags = OPF_COMBINE | (t.store_p ? OPF_STOREP : 0) | (t.fused ? OPF_NOSTORE : 0);
             auto& lane = clanes[cl++ % G];
             lane.push_back(o);
-            if (t.fused) {
-                ProgOp f;
-                std::memset(&f, 0, sizeof(f));
-                f.offA = (uint16_t)off[t.fuse.pa * 3 + t.fuse.sa];
-                f.offP1 = (uint16_t)poff[t.fuse.pa];
-                f.offDst = (uint16_t)off_epsn;
-                f.flags = OPF_FUSED | (t.fuse.neg ? OPF_NEG : 0);
-                lane.push_back(f);
-                out.n_vertex_ops++;
-            }
+            push_fuses(lane, t);
         }
         reduce_bank_conflicts(lanes);
         emit_level(2 * (pc - 2) + 1, lanes);

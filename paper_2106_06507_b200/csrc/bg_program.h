@@ -44,6 +44,8 @@ enum : uint16_t {
     OPF_PARTIAL = 2048,// (with LAST) chunk of a split target: raw partial sums -> scratch slot offDst
     OPF_COMBINE = 4096,// add offB partial slots starting at offA, then finish the target like LAST
     OPF_SYNC = 8192,   // barrier among the lanes of the event after this step (end of a level)
+    OPF_EXTD = 16384,  // (with EXT) continuous states: real polarisation e(phi) times the 3x3 colour matrix
+                       // X[h][g] = etabar_h eta_g -> nine entries of 4 cx from offDst, entry 3h+g (closure target (h,g) reads 3g+h)
     OPF_EXT = 128      // setup: external current of gluon `extra` -> offDst, its momentum -> offPt
 };
 
@@ -66,7 +68,7 @@ long long multiset_count(int r, int t);
 // rank of a count vector m[0..8] (sum = n) in the fixed enumeration order used by host and device
 long long class_rank(int n, const int* counts);
 // Build the program for canonical colour codes code[0..n-1] (code[n-1] = closure leg), G lanes per event.
-void build_program(int n, int G, const int* code, ClassProgram& out);
+void build_program(int n, int G, const int* code, ClassProgram& out, bool dense = false);
 // Build the best program (over the choice of closure leg) for a multiset of colour codes.
 void build_class(int n, int G, const int* counts, ClassProgram& out);
 

@@ -91,6 +91,23 @@ def colour_valid(col_one_event: np.ndarray) -> bool:
     return bool(rc)
 
 
+def continuous_states(n: int, N: int, seed: int = 1, stream: int = 0):
+    """Continuous sampling variables of the paper's CD_MC (Eq. 7, 9, 12; L60-107): one polarisation angle
+    phi in [0, 2 pi) per gluon and two unit 3-vectors (eta, etabar), uniform on the sphere, per gluon.
+    Returns phi[N][n], eta[N][n][2][3].  Inputs only (seeded numpy generator, independent of the phase-space draw)."""
+    rng = np.random.default_rng([seed, stream, n, 0xC0])
+    phi = rng.uniform(0.0, 2.0 * np.pi, size=(N, n))
+    eta = rng.normal(size=(N, n, 2, 3))
+    eta /= np.linalg.norm(eta, axis=-1, keepdims=True)
+    return phi, eta
+
+
+def continuous_to_soa(phi, eta):
+    """phi[N][n] -> [n][N]; eta[N][n][2][3] -> [n][6][N] (eta then etabar), as bg_eval_continuous takes them."""
+    N, n = phi.shape
+    return (np.ascontiguousarray(phi.T), np.ascontiguousarray(np.transpose(eta.reshape(N, n, 6), (1, 2, 0))))
+
+
 def to_soa(mom=None, hel=None, col=None):
     """AoS [N][n][...] -> event-fastest storage [n][...][N] (C-contiguous), as include/bg.h specifies."""
     out = []
