@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--kernel", type=int, default=0, help="BG_OPT_KERNEL (0 auto, 1 generic, 2 class programs)")
     ap.add_argument("--lanes", type=int, default=None, help="BG_OPT_LANES (lanes per event, class-program kernel)")
     ap.add_argument("--smem-limit", type=int, default=None, help="BG_OPT_SMEM_LIMIT in bytes (spill threshold)")
+    ap.add_argument("--continuous", action="store_true",
+                    help="CDBG configs with continuous colour / polarisation states (Eq. 5-14, SURVEY NEXT-1)")
     ap.add_argument("--lc", action="store_true", help="configs 0 / 2 in leading-colour mode (Eq. 33, SURVEY NEXT-3)")
     ap.add_argument("--precision", type=int, default=None, help="BG_OPT_PRECISION (1 = double-double reference path)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -208,6 +210,18 @@ def run_b200(args):
     n, N, flop_per_event, name = workload_desc(args)
     ev = make_events(args, n, N, rank)
     mode = mode_for(args.config, args.lc)
+    d_phi = d_eta = None
+    if args.continuous:
+        if args.config in (0, 2):
+            raise SystemExit("--continuous applies to the colour-dressed configs (1, 3, 4)")
+        mode = bg.BG_CDBG_CONTINUOUS
+        phi, eta = wl.continuous_states(n, N, seed=1, stream=rank)
+        sphi, seta = wl.continuous_to_soa(phi, eta)
+        d_phi, d_eta = torch.from_numpy(sphi).to(dev), torch.from_numpy(seta).to(dev)
+        # dense colour: 3^(n-1) - 2^n + 1 ordered splits x 27 colour terms x ~446 flop (SURVEY 8d "dense-colour bound")
+        flop_per_event = (3 ** (n - 1) - 2 ** n + 1) * 27 * 446.0
+        args.no_e2e = True
+        name += " - continuous colour/polarisation states (Eq. 5-14)"
     mom = wl.to_soa(mom=ev.mom)
     hel = None if ev.hel is None else wl.to_soa(hel=ev.hel)
     col = None if ev.col is None else wl.to_soa(col=ev.col)
@@ -240,7 +254,10 @@ def run_b200(args):
         torch.cuda.synchronize()
 
     def step():
-        bg.bg_eval(ctx, sh, N, d_mom, d_hel, d_col, d_out)
+        if args.continuous:
+            bg.bg_eval_continuous(ctx, sh, N, d_mom, d_phi, d_eta, d_out)
+        else:
+            bg.bg_eval(ctx, sh, N, d_mom, d_hel, d_col, d_out)
 
     peak_tf = bg.bg_fp64_peak_probe(1 << 14) if rank == 0 else None
 
@@ -304,7 +321,7 @@ def run_b200(args):
                     "flop_per_event": flop_per_event, "kernel_ms": kernel_ms,
                     "kernel_share_of_step": kernel_ms / (total_ms / args.steps)}
         cpu = None
-        if not args.no_cpu_baseline and not args.lc:    # the oracle has no batched leading-colour entry point
+        if not args.no_cpu_baseline and not args.lc and not args.continuous:    # no batched oracle entry for these
             import oracle
             S = cpu_sample_size(args, n, N)
             sample = ev.head(S)
