@@ -218,8 +218,9 @@ def run_b200(args):
         phi, eta = wl.continuous_states(n, N, seed=1, stream=rank)
         sphi, seta = wl.continuous_to_soa(phi, eta)
         d_phi, d_eta = torch.from_numpy(sphi).to(dev), torch.from_numpy(seta).to(dev)
-        # dense colour: 3^(n-1) - 2^n + 1 ordered splits x 27 colour terms x ~446 flop (SURVEY 8d "dense-colour bound")
-        flop_per_event = (3 ** (n - 1) - 2 ** n + 1) * 27 * 446.0
+        # dense colour: 3^(n-1) - 2^n + 1 ordered splits x 27 colour terms x ~446 flop with complex currents (SURVEY 8d
+        # "dense-colour bound"); real polarisations make every number real: half of that
+        flop_per_event = (3 ** (n - 1) - 2 ** n + 1) * 27 * 223.0
         args.no_e2e = True
         name += " - continuous colour/polarisation states (Eq. 5-14)"
     mom = wl.to_soa(mom=ev.mom)

@@ -260,9 +260,9 @@ static bool use_prog(const bg_ctx* c) {
 }
 
 // lanes per event of the dense (continuous-state) program, and the table for the context's mode
-static int auto_lanes_dense(int n) { return n <= 4 ? 32 : (n == 5 ? 64 : 128); }
+static int auto_lanes_dense(int n) { return n <= 4 ? 32 : (n <= 6 ? 64 : (n == 7 ? 128 : 256)); }
 static int make_prog_table(const bg_ctx* c, int G, size_t limit, bg::ProgTable** t) {
-    if (c->mode == BG_CDBG_CONTINUOUS) return bg::prog_table_create_dense(c->n, G ? G : auto_lanes_dense(c->n), limit, t);
+    if (c->mode == BG_CDBG_CONTINUOUS) return bg::prog_table_create_dense(c->n, G ? G : auto_lanes_dense(c->n), limit, c->kernel_opt != 1, t);
     return bg::prog_table_create(c->n, G ? G : auto_lanes(c->n), limit ? limit : auto_slab_limit(c->n), t);
 }
 
@@ -343,7 +343,7 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
                 value != 64 && value != 128 && value != 256)
                 return BG_EINVAL;
             const int G = (int)value;
-            if (c->prog && G && bg::prog_lanes(c->prog) == G) return BG_OK;
+            if (c->prog && G && bg::prog_lanes(c->prog) == G && c->mode != BG_CDBG_CONTINUOUS) return BG_OK;
             cudaDeviceSynchronize();
             bg::ProgTable* t = nullptr;
             const int rc = make_prog_table(c, G, c->slab_limit, &t);

@@ -69,6 +69,7 @@ struct ProgTable {
     int max_state_cx;
     TierInfo tiers;
     bool dense;               // continuous colour states: one program, nine colour entries per subset current
+    bool real;                // ... evaluated in real arithmetic (state elements are doubles)
     int rec_bytes;            // bytes of one event record
     bool spill;               // largest state blocks exceed the slab limit: top of the state in global memory
     int spill_blocks_per_sm;  // resident blocks per SM of the spill kernels (each owns one global slab)
@@ -288,25 +289,55 @@ cdbg_scatter_kernel(int n, long long N, long long num_classes, const uint32_t* _
 // Per-event state block: offsets below `cap` live in shared memory ([offset][event], event fastest); with SPILL
 // the rest (the highest popcount levels, which are read least often) lives in an L2-resident global slab owned by
 // the block, accessed with .cg loads/stores (no stale L1 lines).
-template <int EPW, bool SPILL>
+// element of the state: one complex double (double2) or, for the all-real arithmetic of the continuous states with
+// real polarisations, one double
+template <class S> struct StateElem;
+template <> struct StateElem<cx> {
+    using T = double2;
+    static __device__ __forceinline__ cx get(double2 v) { return mk(v.x, v.y); }
+    static __device__ __forceinline__ double2 put(cx v) { return make_double2(v.re, v.im); }
+};
+template <> struct StateElem<double> {
+    using T = double;
+    static __device__ __forceinline__ double get(double v) { return v; }
+    static __device__ __forceinline__ double put(double v) { return v; }
+};
+
+template <int EPW, bool SPILL, class S>
 struct StateRef {
-    double2* S;
-    double2* spill;
+    using T = typename StateElem<S>::T;
+    T* base;
+    T* spill;
     int cap;
-    __device__ __forceinline__ cx ld(int o) const {
-        if (SPILL && o >= cap) {
-            const double2 v = __ldcg(spill + (o - cap));
-            return mk(v.x, v.y);
-        }
-        const double2 v = S[o * EPW];
-        return mk(v.x, v.y);
+    __device__ __forceinline__ S ld(int o) const {
+        if (SPILL && o >= cap) return StateElem<S>::get(__ldcg(spill + (o - cap)));
+        return StateElem<S>::get(base[o * EPW]);
     }
-    __device__ __forceinline__ void st(int o, cx v) const {
+    __device__ __forceinline__ void st(int o, S v) const {
         if (SPILL && o >= cap) {
-            __stcg(spill + (o - cap), make_double2(v.re, v.im));
+            __stcg(spill + (o - cap), StateElem<S>::put(v));
             return;
         }
-        S[o * EPW] = make_double2(v.re, v.im);
+        base[o * EPW] = StateElem<S>::put(v);
+    }
+    // a real 4-momentum: two complex elements, or four real ones
+    __device__ __forceinline__ void ldP(int o, double* P) const {
+        if constexpr (sizeof(T) == 16) {
+            const cx p01 = ld(o), p23 = ld(o + 1);
+            P[0] = p01.re; P[1] = p01.im; P[2] = p23.re; P[3] = p23.im;
+        } else {
+#pragma unroll
+            for (int c = 0; c < 4; c++) P[c] = ld(o + c);
+        }
+    }
+    __device__ __forceinline__ void stP(int o, const double* P) const {
+        if constexpr (sizeof(T) == 16) {
+            st(o, mk(P[0], P[1]));
+            st(o + 1, mk(P[2], P[3]));
+        } else {
+#pragma unroll
+            for (int c = 0; c < 4; c++) st(o + c, P[c]);
+        }
     }
 };
 
@@ -318,9 +349,17 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
 }
 
 // v or -v: flips the sign bits when m = 0x80000000 (integer pipe)
+__device__ __forceinline__ double cneg(double v, int m) {
+    return __hiloint2double(__double2hiint(v) ^ m, __double2loint(v));
+}
 __device__ __forceinline__ cx cneg(cx v, int m) {
     return mk(__hiloint2double(__double2hiint(v.re) ^ m, __double2loint(v.re)),
               __hiloint2double(__double2hiint(v.im) ^ m, __double2loint(v.im)));
+}
+
+__device__ __forceinline__ double shfl_xor(double v, int d) { return __shfl_xor_sync(0xFFFFFFFFu, v, d); }
+__device__ __forceinline__ cx shfl_xor(cx v, int d) {
+    return mk(__shfl_xor_sync(0xFFFFFFFFu, v.re, d), __shfl_xor_sync(0xFFFFFFFFu, v.im, d));
 }
 
 __device__ __forceinline__ EventHeader ld_header(const char* h) {
@@ -330,19 +369,23 @@ __device__ __forceinline__ EventHeader ld_header(const char* h) {
     return r;
 }
 
-template <int G, bool SPILL>
+template <int G, bool SPILL, class S>
 __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgParams p) {
     // G <= 32: one warp per block, EPW = 32/G events per warp.  G > 32: one event per block of G threads.
+    // S: complex currents (cx) or, for continuous states with real polarisations, real ones (double).
     constexpr int EPW = G >= 32 ? 1 : 32 / G;
-    extern __shared__ double2 smem[];
+    using T = typename StateElem<S>::T;
+    extern __shared__ double2 smem_raw[];
+    T* const smem = reinterpret_cast<T*>(smem_raw);
     const int lane = threadIdx.x;
     const int q = lane % EPW, g = lane / EPW;
     constexpr int kBlock = G > 32 ? G : 32;
     constexpr bool kUseRing = G >= 8;
-    uint4* const ring = reinterpret_cast<uint4*>(smem + (size_t)p.slab_cx * EPW) + lane;   // [kRing][kBlock] behind the state
-    StateRef<EPW, SPILL> st_;
-    st_.S = smem + q;
-    st_.spill = SPILL ? p.spill + (size_t)blockIdx.x * p.spill_cx : nullptr;
+    // [kRing][kBlock] behind the state slab (rounded up to 16 bytes)
+    uint4* const ring = reinterpret_cast<uint4*>(smem_raw + ((size_t)p.slab_cx * EPW * sizeof(T) + 15) / 16) + lane;
+    StateRef<EPW, SPILL, S> st_;
+    st_.base = smem + q;
+    st_.spill = SPILL ? reinterpret_cast<T*>(p.spill) + (size_t)blockIdx.x * p.spill_cx : nullptr;
     st_.cap = p.slab_cx;
     const long long first = p.bounds[p.tier], end = p.bounds[p.tier + 1];
     const long long ntasks = (end - first + EPW - 1) / EPW;
@@ -383,13 +426,13 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         const int total = valid ? (int)ci.z : 0;
         bool prefetched = false;
 
-        cx amp = mk(0.0, 0.0);
-        cx acc[4], tacc[6];
+        S amp = s_zero<S>();
+        S acc[4], tacc[6];
         double Pt[4];
 #pragma unroll
-        for (int c = 0; c < 4; c++) { acc[c] = mk(0.0, 0.0); Pt[c] = 0.0; }
+        for (int c = 0; c < 4; c++) { acc[c] = s_zero<S>(); Pt[c] = 0.0; }
 #pragma unroll
-        for (int c = 0; c < 6; c++) tacc[c] = mk(0.0, 0.0);
+        for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
 
         // The lane's ops travel global -> shared by cp.async, kRing - 1 steps ahead, into a private ring (no
         // registers are held across the latency and nothing else reads these slots); the table ends with spare rows.
@@ -425,22 +468,21 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                 const int offPt = raw.z & 0xFFFF;
                 const unsigned flags = raw.z >> 16;
                 if (flags & OPF_VALID) {
-                    cx a[4], b[4];
+                    S a[4], b[4];
 #pragma unroll
                     for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); b[c] = st_.ld(offB + c); }
                     double P1[4], P2[4];
-                    {
-                        const cx p01 = st_.ld(offP1), p23 = st_.ld(offP1 + 1);
-                        P1[0] = p01.re; P1[1] = p01.im; P1[2] = p23.re; P1[3] = p23.im;
-                    }
+                    st_.ldP(offP1, P1);
                     if (flags & OPF_FIRST) {
 #pragma unroll
-                        for (int c = 0; c < 4; c++) acc[c] = mk(0.0, 0.0);
+                        for (int c = 0; c < 4; c++) acc[c] = s_zero<S>();
 #pragma unroll
-                        for (int c = 0; c < 6; c++) tacc[c] = mk(0.0, 0.0);
+                        for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
                         const int offP2 = (int)(raw.w & 0xFFFF);
-                        const cx p01 = st_.ld(offP2), p23 = st_.ld(offP2 + 1);
-                        Pt[0] = P1[0] + p01.re; Pt[1] = P1[1] + p01.im; Pt[2] = P1[2] + p23.re; Pt[3] = P1[3] + p23.im;
+                        double Pb[4];
+                        st_.ldP(offP2, Pb);
+#pragma unroll
+                        for (int c = 0; c < 4; c++) Pt[c] = P1[c] + Pb[c];
                     }
 #pragma unroll
                     for (int c = 0; c < 4; c++) P2[c] = Pt[c] - P1[c];
@@ -451,13 +493,13 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
                     v3_acc(acc, P1, P2, a, b, 1.0);
                     if (flags & OPF_TENB) {
-                        cx T[6];
+                        S T[6];
 #pragma unroll
                         for (int c = 0; c < 6; c++) T[c] = st_.ld(offB + 4 + c);
                         tcontract_acc(acc, T, a, 1.0);
                     }
                     if (flags & OPF_TENA) {
-                        cx T[6];
+                        S T[6];
 #pragma unroll
                         for (int c = 0; c < 6; c++) T[c] = cneg(st_.ld(offA + 4 + c), neg);
                         tcontract_acc(acc, T, b, -1.0);
@@ -471,12 +513,10 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                         for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
                     } else if (flags & OPF_LAST) {
                         if (flags & OPF_CLOSURE) {
-                            cx en[4];
+                            S en[4];
 #pragma unroll
                             for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
-                            const cx d = mdot(en, acc);
-                            amp.re = fma(kInvSqrt2, d.re, amp.re);
-                            amp.im = fma(kInvSqrt2, d.im, amp.im);
+                            amp = amp + kInvSqrt2 * mdot(en, acc);
                         } else {
                             const double f = kInvSqrt2 / mdot(Pt, Pt);
 #pragma unroll
@@ -490,21 +530,17 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                                 for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
                             }
                             if (flags & OPF_STOREP) {
-                                st_.st(offPt, mk(Pt[0], Pt[1]));
-                                st_.st(offPt + 1, mk(Pt[2], Pt[3]));
+                                st_.stP(offPt, Pt);
                             }
                         }
                     }
                 } else if (flags & OPF_FUSED) {
                     // closure vertex X(eps_k, J(pi)) . eps_n with J(pi), T(pi) still in acc / tacc, P(pi) in Pt
-                    cx a[4], x[4], en[4];
+                    S a[4], x[4], en[4];
                     double P1[4];
 #pragma unroll
-                    for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); x[c] = mk(0.0, 0.0); }
-                    {
-                        const cx p01 = st_.ld(offP1), p23 = st_.ld(offP1 + 1);
-                        P1[0] = p01.re; P1[1] = p01.im; P1[2] = p23.re; P1[3] = p23.im;
-                    }
+                    for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); x[c] = s_zero<S>(); }
+                    st_.ldP(offP1, P1);
                     const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
 #pragma unroll
                     for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
@@ -512,9 +548,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     tcontract_acc(x, tacc, a, 1.0);
 #pragma unroll
                     for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
-                    const cx d = mdot(en, x);
-                    amp.re = fma(kInvSqrt2, d.re, amp.re);
-                    amp.im = fma(kInvSqrt2, d.im, amp.im);
+                    amp = amp + kInvSqrt2 * mdot(en, x);
                 } else if (flags & OPF_COMBINE) {
                     // add the offB partial sums of a split target and finish it like a LAST op
 #pragma unroll
@@ -529,9 +563,11 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     }
                     {
                         const int offP2 = (int)(raw.w & 0xFFFF);
-                        const cx a01 = st_.ld(offP1), a23 = st_.ld(offP1 + 1);
-                        const cx b01 = st_.ld(offP2), b23 = st_.ld(offP2 + 1);
-                        Pt[0] = a01.re + b01.re; Pt[1] = a01.im + b01.im; Pt[2] = a23.re + b23.re; Pt[3] = a23.im + b23.im;
+                        double Pa[4], Pb[4];
+                        st_.ldP(offP1, Pa);
+                        st_.ldP(offP2, Pb);
+#pragma unroll
+                        for (int c = 0; c < 4; c++) Pt[c] = Pa[c] + Pb[c];
                     }
                     const double f = kInvSqrt2 / mdot(Pt, Pt);
 #pragma unroll
@@ -545,8 +581,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                         for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
                     }
                     if (flags & OPF_STOREP) {
-                        st_.st(offPt, mk(Pt[0], Pt[1]));
-                        st_.st(offPt + 1, mk(Pt[2], Pt[3]));
+                        st_.stP(offPt, Pt);
                     }
                 } else if (flags & OPF_EXTD) {
                     // continuous states (Eq. 7, 9, 12): real polarisation e(phi) times the colour matrix etabar_h eta_g;
@@ -568,25 +603,23 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                             const double x = etab[h] * eta[gg];
                             const int at = offDst + 4 * (h * 3 + gg);
 #pragma unroll
-                            for (int c = 0; c < 4; c++) st_.st(at + c, mk(x * ev[c], 0.0));
+                            for (int c = 0; c < 4; c++) st_.st(at + c, s_real<S>(x * ev[c]));
                         }
                     if (!closure_leg) {
-                        st_.st(offPt, mk(pk[0], pk[1]));
-                        st_.st(offPt + 1, mk(pk[2], pk[3]));
+                        st_.stP(offPt, pk);
                     }
-                } else if (flags & OPF_EXT) {
+                } else if ((flags & OPF_EXT) && sizeof(T) == 16) {
                     const int k = (int)raw.w;
                     double pk[4];
 #pragma unroll
                     for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + k * p.rec_gstride + c);   // not through L1: it is kept for the ops
                     cx eps[4];
                     polarisation(pk, ((perm >> (48 + k)) & 1) ? 1 : -1, eps);
+                    if constexpr (sizeof(T) == 16) {
 #pragma unroll
                     for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
-                    if (offPt != 0xFFFF) {
-                        st_.st(offPt, mk(pk[0], pk[1]));
-                        st_.st(offPt + 1, mk(pk[2], pk[3]));
                     }
+                    if (offPt != 0xFFFF) st_.stP(offPt, pk);
                 }
                 if (flags & OPF_SYNC) {
                     // end of a level: the currents just written become visible to the lanes of the event
@@ -608,19 +641,18 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         // closure amplitude: sum of the G lanes' partial contractions (Eq. 22), then |A|^2
 #pragma unroll
         for (int d = EPW; d < 32; d <<= 1) {
-            amp.re += __shfl_xor_sync(0xFFFFFFFFu, amp.re, d);
-            amp.im += __shfl_xor_sync(0xFFFFFFFFu, amp.im, d);
+            amp = amp + shfl_xor(amp, d);
         }
         if constexpr (G > 32) {
             __shared__ double red_s[2 * (G / 32)];
-            if ((lane & 31) == 0) { red_s[2 * (lane >> 5)] = amp.re; red_s[2 * (lane >> 5) + 1] = amp.im; }
+            if ((lane & 31) == 0) reinterpret_cast<S*>(red_s)[lane >> 5] = amp;
             __syncthreads();
             if (lane == 0) {
-                amp = mk(0.0, 0.0);
-                for (int w = 0; w < G / 32; w++) { amp.re += red_s[2 * w]; amp.im += red_s[2 * w + 1]; }
+                amp = s_zero<S>();
+                for (int w = 0; w < G / 32; w++) amp = amp + reinterpret_cast<S*>(red_s)[w];
             }
         }
-        if (g == 0 && have) p.out[e] = valid ? fma(amp.re, amp.re, amp.im * amp.im) : 0.0;
+        if (g == 0 && have) p.out[e] = valid ? s_norm2(amp) : 0.0;
         if constexpr (G > 32) __syncthreads(); else __syncwarp();
     }
 }
@@ -761,15 +793,16 @@ int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out) {
 }
 
 // ---- continuous colour / polarisation states (Eq. 5-14): one dense program ----------
-int prog_table_create_dense(int n, int G, size_t slab_limit, ProgTable** out) {
+int prog_table_create_dense(int n, int G, size_t slab_limit, bool real, ProgTable** out) {
     *out = nullptr;
     if (slab_limit == 0 || slab_limit > kMaxSlabBytes) slab_limit = kMaxSlabBytes;
     if (n < 4 || n > kMaxN || G < 32 || G > 256 || (G & (G - 1))) return BG_EINVAL;
     ClassProgram cp;
     int code[kMaxN] = {0};
-    build_program(n, G, code, cp, true);
+    build_program(n, G, code, cp, true, real);
     if (!cp.valid || cp.state_cx > 65535) return BG_EUNSUPPORTED;
-    const bool spill = (size_t)cp.state_cx * 16 > slab_limit;
+    const size_t elem = real ? 8 : 16;
+    const bool spill = (size_t)cp.state_cx * elem > slab_limit;
     if (spill && G < 128) return BG_EUNSUPPORTED;
     ClassInfo ci;
     std::memset(&ci, 0, sizeof(ci));
@@ -786,15 +819,16 @@ int prog_table_create_dense(int n, int G, size_t slab_limit, ProgTable** out) {
     std::memset(t, 0, sizeof(*t));
     t->n = n; t->G = G; t->num_classes = 1; t->max_state_cx = cp.state_cx;
     t->dense = true;
+    t->real = real;
     t->rec_bytes = kRecHeaderBytes + 96 * n;
     for (int k = 0; k < kTiers; k++) {
-        t->tiers.slab_cx[k] = std::min<int>(cp.state_cx, (int)(slab_limit / 16));
+        t->tiers.slab_cx[k] = std::min<int>(cp.state_cx, (int)(slab_limit / elem));
         t->tiers.first_key[k] = k == 0 ? 0 : 1;
     }
     t->tiers.first_key[kTiers] = 1;
     t->spill = spill;
     {
-        const size_t smem0 = (size_t)t->tiers.slab_cx[0] * 16;
+        const size_t smem0 = (size_t)t->tiers.slab_cx[0] * elem;
         const int block = G > 32 ? G : 32;
         t->spill_blocks_per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * block), (228 * 1024) / (smem0 + 1024)));
         int dev = 0;
@@ -849,7 +883,7 @@ void prog_table_destroy(ProgTable* t) {
     delete t;
 }
 
-size_t prog_state_bytes(const ProgTable* t) { return t ? (size_t)t->max_state_cx * 16 : 0; }
+size_t prog_state_bytes(const ProgTable* t) { return t ? (size_t)t->max_state_cx * (t->real ? 8 : 16) : 0; }
 int prog_lanes(const ProgTable* t) { return t ? t->G : 0; }
 
 // scratch: records (32 + 32 n) B x N | perm u64[N] | cls u32[N] | hist u32[num_classes + 1] | tier bounds | spill slabs
@@ -862,14 +896,15 @@ size_t prog_scratch_bytes(const ProgTable* t, long long N) {
     return prog_spill_offset(t, N) + spill;
 }
 
-template <int G, bool SPILL>
+template <int G, bool SPILL, class S = cx>
 static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched) {
     constexpr int EPW = G >= 32 ? 1 : 32 / G, BLOCK = G > 32 ? G : 32;
+    constexpr size_t ELEM = sizeof(typename StateElem<S>::T);
     static int configured_device = -1;   // the attribute is per device
     int device = 0;
     cudaGetDevice(&device);
     if (configured_device != device) {
-        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL, S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)(kMaxSlabBytes + (size_t)kRing * BLOCK * 16));
         if (e != cudaSuccess) return e;
         configured_device = device;
@@ -880,13 +915,13 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         p.tier = k;
         p.slab_cx = t->tiers.slab_cx[k];
         const size_t ring_bytes = G >= 8 ? (size_t)kRing * BLOCK * 16 : 0;
-        const size_t smem = (size_t)EPW * p.slab_cx * 16 + ring_bytes;
+        const size_t smem = ((size_t)EPW * p.slab_cx * ELEM + 15) / 16 * 16 + ring_bytes;
         if (smem > kMaxSlabBytes + ring_bytes) return cudaErrorInvalidValue;
         // resident blocks per SM: shared memory (1 KB reserved per block), and 65536 / (160 x BLOCK) registers
         int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * BLOCK), (228 * 1024) / (smem + 1024)));
         if (SPILL) per_sm = std::min(per_sm, t->spill_blocks_per_sm);   // one global slab per resident block
         const unsigned blocks = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
-        cdbg_prog_kernel<G, SPILL><<<blocks, BLOCK, smem, s>>>(p);
+        cdbg_prog_kernel<G, SPILL, S><<<blocks, BLOCK, smem, s>>>(p);
         ++*launched;
     }
     return cudaGetLastError();
@@ -894,6 +929,18 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
 
 static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches) {
     cudaError_t err;
+    if (t->real) {   // continuous states with real polarisations: all-real arithmetic
+        switch (t->G) {
+            case 32: return launch_interp<32, false, double>(s, t, sm_count, p, launches);
+            case 64: return launch_interp<64, false, double>(s, t, sm_count, p, launches);
+            case 128:
+                return t->spill ? launch_interp<128, true, double>(s, t, sm_count, p, launches)
+                                : launch_interp<128, false, double>(s, t, sm_count, p, launches);
+            default:
+                return t->spill ? launch_interp<256, true, double>(s, t, sm_count, p, launches)
+                                : launch_interp<256, false, double>(s, t, sm_count, p, launches);
+        }
+    }
     switch (t->G) {
         case 1: err = launch_interp<1, false>(s, t, sm_count, p, launches); break;
         case 2: err = launch_interp<2, false>(s, t, sm_count, p, launches); break;

@@ -159,4 +159,49 @@ __device__ __forceinline__ void v4_acc(cx* acc, const cx* a, const cx* b, const 
     }
 }
 
+// ---- the same vertex algebra for REAL currents (continuous states with real polarisations, Eq. 7: "real valued
+// amplitudes for the gluon-only case") --------------------------------------------------------
+__device__ __forceinline__ void v3_acc(double* acc, const double* p, const double* q, const double* a, const double* b,
+                                       double sign) {
+    double tqp[4], tpq[4];
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        tqp[mu] = fma(2.0, q[mu], p[mu]);
+        tpq[mu] = fma(2.0, p[mu], q[mu]);
+    }
+    const double ab = sign * mdot(a, b), qa = sign * mdot(tqp, a), pb = sign * mdot(tpq, b);
+#pragma unroll
+    for (int nu = 0; nu < 4; nu++) {
+        acc[nu] = fma(p[nu] - q[nu], ab, acc[nu]);
+        acc[nu] = fma(qa, b[nu], acc[nu]);
+        acc[nu] = fma(-pb, a[nu], acc[nu]);
+    }
+}
+__device__ __forceinline__ void tcontract_acc(double* acc, const double* T, const double* v, double sign) {
+    const double v0 = sign * v[0], v1 = sign * v[1], v2 = sign * v[2], v3 = sign * v[3];
+    acc[0] = fma(-T[0], v1, acc[0]); acc[0] = fma(-T[1], v2, acc[0]); acc[0] = fma(-T[2], v3, acc[0]);
+    acc[1] = fma(-T[0], v0, acc[1]); acc[1] = fma(-T[3], v2, acc[1]); acc[1] = fma(-T[4], v3, acc[1]);
+    acc[2] = fma(-T[1], v0, acc[2]); acc[2] = fma(T[3], v1, acc[2]);  acc[2] = fma(-T[5], v3, acc[2]);
+    acc[3] = fma(-T[2], v0, acc[3]); acc[3] = fma(T[4], v1, acc[3]);  acc[3] = fma(T[5], v2, acc[3]);
+}
+__device__ __forceinline__ void tbuild_acc(double* tacc, const double* a, const double* b, double sign) {
+    const double b0 = sign * b[0], b1 = sign * b[1], b2 = sign * b[2], b3 = sign * b[3];
+    tacc[0] = fma(a[0], b1, tacc[0]); tacc[0] = fma(-a[1], b0, tacc[0]);
+    tacc[1] = fma(a[0], b2, tacc[1]); tacc[1] = fma(-a[2], b0, tacc[1]);
+    tacc[2] = fma(a[0], b3, tacc[2]); tacc[2] = fma(-a[3], b0, tacc[2]);
+    tacc[3] = fma(a[1], b2, tacc[3]); tacc[3] = fma(-a[2], b1, tacc[3]);
+    tacc[4] = fma(a[1], b3, tacc[4]); tacc[4] = fma(-a[3], b1, tacc[4]);
+    tacc[5] = fma(a[2], b3, tacc[5]); tacc[5] = fma(-a[3], b2, tacc[5]);
+}
+
+// scalar-type helpers so that one interpreter body serves complex (cx) and real (double) currents
+template <class S> __device__ __forceinline__ S s_zero();
+template <> __device__ __forceinline__ cx s_zero<cx>() { return mk(0.0, 0.0); }
+template <> __device__ __forceinline__ double s_zero<double>() { return 0.0; }
+template <class S> __device__ __forceinline__ S s_real(double x);
+template <> __device__ __forceinline__ cx s_real<cx>(double x) { return mk(x, 0.0); }
+template <> __device__ __forceinline__ double s_real<double>(double x) { return x; }
+__device__ __forceinline__ double s_norm2(cx a) { return fma(a.re, a.re, a.im * a.im); }
+__device__ __forceinline__ double s_norm2(double a) { return a * a; }
+
 }  // namespace bg

@@ -56,12 +56,13 @@ inline int popc(int x) { return __builtin_popcount((unsigned)x); }
 
 }  // namespace
 
-void build_program(int n, int G, const int* code, ClassProgram& out, bool dense) {
+void build_program(int n, int G, const int* code, ClassProgram& out, bool dense, bool real) {
     out = ClassProgram();
     const int m = n - 1, nsub = 1 << m, full = nsub - 1;
     // dense: every gluon carries a full 3x3 colour matrix (continuous colour states) - all nine entries of every
     // subset current are live and `code` is ignored; otherwise elementary matrices e_ij and at most 3 live entries
     const int SL = dense ? 9 : 3;
+    const int PU = real ? 4 : 2;   // state elements of a 4-momentum: two complex doubles, or four doubles (real currents)
     auto slot_of = [&](int h, int g) { return dense ? h * 3 + g : (h == g ? h : 0); };
     int dummy_code[kMaxN] = {0};
     if (dense) code = dummy_code;
@@ -206,14 +207,14 @@ void build_program(int n, int G, const int* code, ClassProgram& out, bool dense)
     }
     const int off_epsn = next;      // eps_n (dense: the nine vectors eps_n X_n[g][h] at index 3g+h)
     next += dense ? 36 : 4;
-    for (int k = 0; k < m; k++) { poff[1 << k] = next; next += 2; }
+    for (int k = 0; k < m; k++) { poff[1 << k] = next; next += PU; }
     // With fewer than 8 events per warp the bank group of an element depends on its offset: one element of padding
     // after every entry makes the entry starts run through all residues (10 + 2 would only ever give multiples of 4).
     const int pad = G >= 8 ? 1 : 0;
     for (int pc = 2; pc < m; pc++)
         for (auto& t : levels[pc]) {
             if (!t.fused) { off[t.pi * SL + t.slot()] = next; next += 10 + pad; }
-            if (need_p[t.pi] && poff[t.pi] < 0) { poff[t.pi] = next; next += 2; t.store_p = true; }
+            if (need_p[t.pi] && poff[t.pi] < 0) { poff[t.pi] = next; next += PU; t.store_p = true; }
         }
     out.level_steps.assign(2 * m - 2, 0);   // setup | (main, combine) per popcount 2..n-2 | closure
 

@@ -68,7 +68,9 @@ long long multiset_count(int r, int t);
 // rank of a count vector m[0..8] (sum = n) in the fixed enumeration order used by host and device
 long long class_rank(int n, const int* counts);
 // Build the program for canonical colour codes code[0..n-1] (code[n-1] = closure leg), G lanes per event.
-void build_program(int n, int G, const int* code, ClassProgram& out, bool dense = false);
+// dense: continuous colour states (nine live entries per subset, `code` ignored); real: the state elements are
+// doubles instead of complex doubles (a 4-momentum then takes four elements instead of two).
+void build_program(int n, int G, const int* code, ClassProgram& out, bool dense = false, bool real = false);
 // Build the best program (over the choice of closure leg) for a multiset of colour codes.
 void build_class(int n, int G, const int* counts, ClassProgram& out);
 

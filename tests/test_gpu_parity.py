@@ -240,9 +240,10 @@ def test_double_double_reference_path_cobg(bg, oracle, wl, n, N):
         assert rel_err(got, oracle.cobg_full_colour(ev4.mom, prec="long double")).max() <= 1e-11
 
 
+@pytest.mark.parametrize("arith", ["real", "complex"])
 @pytest.mark.parametrize("n,N,lanes", [(4, 300, None), (5, 200, None), (6, 150, None), (6, 33, 32), (6, 33, 256),
                                          (7, 40, None), (8, 9, 256)])
-def test_continuous_colour_and_polarisation_states(bg, oracle, wl, n, N, lanes):
+def test_continuous_colour_and_polarisation_states(bg, oracle, wl, n, N, lanes, arith):
     """SURVEY NEXT-1 (the paper's CD_MC sampling, Eq. 5-14): colour-dressed recursion with a real polarisation e(phi)
     and a full 3x3 colour matrix etabar x eta per gluon, against the oracle's general-state recursion."""
     import torch
@@ -256,7 +257,10 @@ def test_continuous_colour_and_polarisation_states(bg, oracle, wl, n, N, lanes):
     d_out = torch.full((N,), float("nan"), dtype=torch.float64, device=dev)
     ctx = bg.bg_init(n, bg.BG_CDBG_CONTINUOUS)
     try:
-        if lanes:
+        if arith == "complex":      # BG_OPT_KERNEL = 1: the same program in complex arithmetic (rebuilt by LANES)
+            bg.bg_set_option(ctx, bg.BG_OPT_KERNEL, 1)
+            bg.bg_set_option(ctx, bg.BG_OPT_LANES, lanes or 0)
+        elif lanes:
             bg.bg_set_option(ctx, bg.BG_OPT_LANES, lanes)
         bg.bg_reserve(ctx, N)
         bg.bg_eval_continuous(ctx, torch.cuda.current_stream().cuda_stream, N, d_mom, d_phi, d_eta, d_out)
