@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--kernel", type=int, default=0, help="BG_OPT_KERNEL (0 auto, 1 generic, 2 class programs)")
     ap.add_argument("--lanes", type=int, default=None, help="BG_OPT_LANES (lanes per event, class-program kernel)")
     ap.add_argument("--smem-limit", type=int, default=None, help="BG_OPT_SMEM_LIMIT in bytes (spill threshold)")
+    ap.add_argument("--device-gen", action="store_true",
+                    help="also time generate-on-device + evaluate per step (bg_generate, SURVEY NEXT-4; PAPER.md:L259)")
     ap.add_argument("--continuous", action="store_true",
                     help="CDBG configs with continuous colour / polarisation states (Eq. 5-14, SURVEY NEXT-1)")
     ap.add_argument("--lc", action="store_true", help="configs 0 / 2 in leading-colour mode (Eq. 33, SURVEY NEXT-3)")
@@ -290,6 +292,33 @@ def run_b200(args):
     total_ms = max_over_ranks(total_ms, world, dev)
     value = N * world * args.steps / (total_ms * 1e-3)
 
+    # generation on the device inside the timed region (the paper's timings include phase-space generation, L259):
+    # nothing crosses PCIe but the seed
+    devgen = None
+    if args.device_gen and not args.continuous:
+        g_mom = torch.empty_like(d_mom)
+        g_hel = None if d_hel is None or (mode & bg.BG_HEL_SUM) else torch.empty_like(d_hel)
+        g_col = None if d_col is None or not (mode & bg.BG_COL_GIVEN) else torch.empty_like(d_col)
+        cuts = (0.0, 0.0) if args.config == 0 else (wl.PT_MIN, wl.DR_MIN)
+
+        def gen_step(i):
+            bg.bg_generate(sh, n, N, 1, 9000 + args.config, i * N, wl.SQRT_S, cuts[0], cuts[1], True, g_mom, g_hel, g_col)
+            bg.bg_eval(ctx, sh, N, g_mom, g_hel, g_col, d_out)
+        for i in range(3):
+            gen_step(i)
+        barrier()
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record(stream)
+        for i in range(args.steps):
+            gen_step(3 + i)
+        g1.record(stream)
+        barrier()
+        gms = max_over_ranks(g0.elapsed_time(g1), world, dev)
+        devgen = {"value": N * world * args.steps / (gms * 1e-3), "unit": "events/s", "ms_per_step": gms / args.steps,
+                  "note": "bg_generate (RAMBO + cuts + helicity/colour draws on the device) + bg_eval per step; fresh events every step"}
+        step()      # restore d_out of the resident workload for the checks below
+        barrier()   # (bg_eval_host runs on the context's own streams and shares its scratch)
+
     # end-to-end: host buffers through bg_eval_host (H2D of inputs + D2H of results inside the timed region)
     e2e = None
     if not args.no_e2e:
@@ -347,6 +376,8 @@ def run_b200(args):
                            "kernel": kernel_name, "current_bytes_per_event": bg.bg_current_bytes_per_event(ctx)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
                 "roofline": roofline, "cpu_baseline": cpu}
+        if devgen is not None:
+            line["generate_on_device"] = devgen
         print(json.dumps(line), flush=True)
     bg.bg_destroy(ctx)
     if world > 1:

@@ -158,6 +158,25 @@ const char* bg_last_kernel_name(const bg_ctx* ctx);
  */
 int bg_class_program_stats(int n, int lanes, const int* counts, long long* stats);
 
+/*
+ * On-device event generation (the paper's timings include it): RAMBO flat massless
+ * phase space for the n-2 outgoing gluons at sqrt_s, legs 1, 2 = -(sqrt_s/2)(1,0,0,+-1) in the
+ * all-outgoing convention, every outgoing pT > ptmin and pair Delta R > drmin (<= 0 switches a cut
+ * off) with the whole event redrawn on failure; helicities uniform +-1 (redrawn when fewer than two + or two -, if
+ * reject_zero_helicities); colour-flow indices uniform in {1,2,3} redrawn until the assignment can be non-zero
+ * (reading g8).  Counter-based generator: event e of the call is a pure function of (seed, stream_id,
+ * first_event + e) and reproduces paper_2106_06507_b200/workload (same integer draws; momenta equal to a few ulps).
+ * DEVICE pointers in the layouts of bg_eval; any of mom / hel / col may be NULL (skipped).  Asynchronous on
+ * `cuda_stream`; needs no context.
+ */
+int bg_generate(void* cuda_stream, int n, long long N, unsigned long long seed, unsigned long long stream_id,
+                long long first_event, double sqrt_s, double ptmin, double drmin, int reject_zero_helicities, double* mom,
+                signed char* hel, signed char* col);
+
+/* Host-only: rule g8 as bg_generate applies it (balanced colour charges, connected colour graph, not all indices
+ * equal) for col[n][2] in {1,2,3}; returns 1 / 0, or BG_EINVAL. */
+int bg_colour_rule(int n, const signed char* col);
+
 int bg_destroy(bg_ctx* ctx);
 
 const char* bg_strerror(int code);

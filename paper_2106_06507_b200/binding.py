@@ -27,7 +27,7 @@ BG_COBG_HELSUM_LC = BG_REC_COBG | BG_HEL_SUM | BG_COL_LC
 BG_COBG_HELGIVEN_LC = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_LC
 BG_OPT_KERNEL, BG_OPT_SCRATCH_LIMIT, BG_OPT_LANES, BG_OPT_TIMING, BG_OPT_SMEM_LIMIT, BG_OPT_PRECISION = 1, 2, 3, 4, 5, 6
 
-EXPORTS = ("bg_init", "bg_eval", "bg_eval_continuous", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",
+EXPORTS = ("bg_init", "bg_eval", "bg_eval_continuous", "bg_generate", "bg_colour_rule", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",
            "bg_set_option", "bg_colour_matrix", "bg_build_colour_matrix", "bg_last_launch_count",
            "bg_last_kernel_name", "bg_last_kernel_ms", "bg_class_program_stats", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe")
 
@@ -53,6 +53,11 @@ def load():
         lib.bg_init.argtypes = [ctypes.POINTER(vp), i, i]
         lib.bg_eval.argtypes = [vp, vp, ll, vp, vp, vp, vp]
         lib.bg_eval_host.argtypes = [vp, ll, vp, vp, vp, vp]
+        lib.bg_generate.argtypes = [vp, i, ll, ctypes.c_ulonglong, ctypes.c_ulonglong, ll, ctypes.c_double, ctypes.c_double,
+                                    ctypes.c_double, i, vp, vp, vp]
+        lib.bg_generate.restype = i
+        lib.bg_colour_rule.argtypes = [i, vp]
+        lib.bg_colour_rule.restype = i
         lib.bg_eval_continuous.argtypes = [vp, vp, ll, vp, vp, vp, vp]
         lib.bg_eval_continuous.restype = i
         lib.bg_reserve.argtypes = [vp, ll]
@@ -118,6 +123,24 @@ def bg_eval_continuous(ctx, stream, N: int, mom, phi, eta, out) -> None:
     """Device pointers; phi[n][N], eta[n][6][N] (eta then etabar), event-fastest."""
     s = ctypes.c_void_p(int(stream)) if stream else None
     _check(load().bg_eval_continuous(ctx, s, N, _ptr(mom), _ptr(phi), _ptr(eta), _ptr(out)), "bg_eval_continuous")
+
+
+def bg_generate(stream, n: int, N: int, seed: int, stream_id: int, first_event: int, sqrt_s: float, ptmin: float,
+                drmin: float, reject_zero_helicities: bool, mom, hel, col) -> None:
+    """Generate N synthetic events on the device into event-fastest buffers (any of mom / hel / col may be None)."""
+    s = ctypes.c_void_p(int(stream)) if stream else None
+    _check(load().bg_generate(s, n, N, seed, stream_id, first_event, sqrt_s, ptmin, drmin, int(reject_zero_helicities),
+                              _ptr(mom), _ptr(hel), _ptr(col)), "bg_generate")
+
+
+def bg_colour_rule(col) -> bool:
+    """Host-only: rule g8 for one event, col[n][2] in {1,2,3}."""
+    import numpy as np
+    c = np.ascontiguousarray(col, dtype=np.int8)
+    rc = load().bg_colour_rule(c.shape[0], _ptr(c))
+    if rc < 0:
+        raise BgError(rc, "bg_colour_rule")
+    return bool(rc)
 
 
 def bg_eval_host(ctx, N: int, mom, hel, col, out) -> None:

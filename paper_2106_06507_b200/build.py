@@ -7,7 +7,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libbg.so")
-SOURCES = ["bg_api.cu", "bg_generic.cu", "bg_cobg_generic.cu", "bg_cdbg_prog.cu", "bg_program.cpp", "bg_cobg_shared.cu", "bg_cdbg_dd.cu"]
+SOURCES = ["bg_api.cu", "bg_generic.cu", "bg_cobg_generic.cu", "bg_cdbg_prog.cu", "bg_program.cpp", "bg_cobg_shared.cu", "bg_cdbg_dd.cu", "bg_generate.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 

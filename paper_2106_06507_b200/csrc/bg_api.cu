@@ -561,6 +561,24 @@ int bg_eval_host(bg_ctx* c, long long N, const double* mom, const signed char* h
     return BG_OK;
 }
 
+int bg_generate(void* cuda_stream, int n, long long N, unsigned long long seed, unsigned long long stream_id,
+                long long first_event, double sqrt_s, double ptmin, double drmin, int reject_zero_helicities, double* mom,
+                signed char* hel, signed char* col) {
+    if (n < 4 || n > 12 || N < 0 || !(sqrt_s > 0.0) || first_event < 0) return BG_EINVAL;
+    if (N == 0 || (!mom && !hel && !col)) return BG_OK;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return BG_ECUDA;
+    return bg::generate_launch((cudaStream_t)cuda_stream, n, N, seed, stream_id, first_event, sqrt_s, ptmin, drmin,
+                               reject_zero_helicities, mom, hel, col) == cudaSuccess ? BG_OK : BG_ECUDA;
+}
+
+int bg_colour_rule(int n, const signed char* col) {
+    if (n < 3 || n > 16 || !col) return BG_EINVAL;
+    for (int k = 0; k < 2 * n; k++)
+        if (col[k] < 1 || col[k] > 3) return BG_EINVAL;
+    return bg::colour_rule_host(n, col) ? 1 : 0;
+}
+
 int bg_fp64_peak_probe(int iterations, double* tflops) {
     if (!tflops || iterations < 1) return BG_EINVAL;
     int ndev = 0;

@@ -93,6 +93,12 @@ cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, 
 // ---- colour matrix (bg_colour.cpp part of bg_api.cu) ------------------------------------------------------
 int build_colour_matrix(int n, double* C /* (n-2)!^2 */);
 
+// ---- on-device event generation (bg_generate.cu) ---------------------------------------------------------
+cudaError_t generate_launch(cudaStream_t s, int n, long long N, uint64_t seed, uint64_t stream, long long first_event,
+                            double sqrt_s, double ptmin, double drmin, int reject_zero_hel, double* mom, signed char* hel,
+                            signed char* col);
+bool colour_rule_host(int n, const signed char* col);
+
 // ---- FP64 peak probe ----------------------------------------------------------------------------------
 cudaError_t fp64_probe(int iterations, double* tflops);
 

@@ -1,0 +1,93 @@
+"""On-device event generation (bg_generate) against the host workload generator it restates."""
+import itertools
+
+import numpy as np
+import pytest
+
+
+@pytest.fixture(scope="module")
+def bg():
+    import paper_2106_06507_b200 as bg
+    bg.load()
+    return bg
+
+
+@pytest.mark.parametrize("n", [3, 4, 5, 6])
+def test_colour_rule_equals_the_hamiltonian_cycle_rule_exhaustively(bg, wl, n):
+    """bg_generate decides rule g8 by "Eulerian circuit of the colour multigraph" (balanced + connected); the host
+    generator by a Hamiltonian-cycle DP over the gluons.  All 9^n assignments (n <= 5), a 1-in-7 sample at n = 6."""
+    pairs = [(i, j) for i in (1, 2, 3) for j in (1, 2, 3)]
+    checked = 0
+    for idx, combo in enumerate(itertools.product(pairs, repeat=n)):
+        if n == 6 and idx % 7:
+            continue
+        col = np.array(combo, dtype=np.int8)
+        assert bg.bg_colour_rule(col) == wl.colour_valid(col), combo
+        checked += 1
+    assert checked >= 9 ** min(n, 5)
+
+
+def test_colour_rule_rejects_bad_input(bg):
+    with pytest.raises(bg.BgError):
+        bg.bg_colour_rule(np.array([[1, 2], [2, 4], [3, 1]], dtype=np.int8))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("n,N", [(4, 3000), (6, 5000), (9, 2000), (12, 300)])
+def test_device_generator_reproduces_the_host_generator(bg, wl, n, N):
+    import torch
+    dev = torch.device("cuda:0")
+    stream_id, first = 500 + n, 17
+    d_mom = torch.empty((n, 4, N), dtype=torch.float64, device=dev)
+    d_hel = torch.empty((n, N), dtype=torch.int8, device=dev)
+    d_col = torch.empty((n, 2, N), dtype=torch.int8, device=dev)
+    bg.bg_generate(torch.cuda.current_stream().cuda_stream, n, N, 1, stream_id, first, wl.SQRT_S, wl.PT_MIN, wl.DR_MIN,
+                   True, d_mom, d_hel, d_col)
+    torch.cuda.synchronize()
+    mom = np.transpose(d_mom.cpu().numpy(), (2, 0, 1))
+    hel = d_hel.cpu().numpy().T
+    col = np.transpose(d_col.cpu().numpy(), (2, 0, 1))
+    h_mom = wl.rambo(n, N, 1, stream_id, first)
+    h_hel = wl.helicities(n, N, 1, stream_id, first)
+    h_col = wl.colours(n, N, 1, stream_id, first)
+    assert np.array_equal(hel, h_hel)          # integer draws: identical
+    assert np.array_equal(col, h_col)
+    # momenta: same trial accepted unless a cut sits within rounding of its threshold (never seen at these sizes);
+    # values agree to the accuracy of log / sin / cos / atan2 on the two platforms
+    # (nearly collinear RAMBO draws amplify an ulp in log / sin / cos up to ~1e-10 relative, see gen.c's polish step)
+    same = np.all(np.abs(mom - h_mom) <= 1e-10 * wl.SQRT_S, axis=(1, 2))
+    assert same.mean() > 0.999
+    assert np.median(np.max(np.abs(mom - h_mom), axis=(1, 2))) <= 1e-12 * wl.SQRT_S
+    # and every generated event is a valid phase-space point on its own
+    assert np.max(np.abs(mom.sum(axis=1))) < 1e-9
+    m2 = mom[:, :, 0] ** 2 - (mom[:, :, 1:] ** 2).sum(-1)
+    assert np.max(np.abs(m2)) < 1e-7
+    pt = np.hypot(mom[:, 2:, 1], mom[:, 2:, 2])
+    assert pt.min() > wl.PT_MIN
+
+
+@pytest.mark.gpu
+def test_generated_events_feed_the_evaluation(bg, oracle, wl):
+    """generate -> evaluate on the device, compared with the oracle on the same (downloaded) events."""
+    import torch
+    n, N = 6, 4000
+    dev = torch.device("cuda:0")
+    d_mom = torch.empty((n, 4, N), dtype=torch.float64, device=dev)
+    d_hel = torch.empty((n, N), dtype=torch.int8, device=dev)
+    d_col = torch.empty((n, 2, N), dtype=torch.int8, device=dev)
+    d_out = torch.empty(N, dtype=torch.float64, device=dev)
+    s = torch.cuda.current_stream().cuda_stream
+    ctx = bg.bg_init(n, bg.BG_CDBG_GIVEN)
+    try:
+        bg.bg_reserve(ctx, N)
+        bg.bg_generate(s, n, N, 7, 3, 0, wl.SQRT_S, wl.PT_MIN, wl.DR_MIN, True, d_mom, d_hel, d_col)
+        bg.bg_eval(ctx, s, N, d_mom, d_hel, d_col, d_out)
+        torch.cuda.synchronize()
+    finally:
+        bg.bg_destroy(ctx)
+    mom = np.ascontiguousarray(np.transpose(d_mom.cpu().numpy(), (2, 0, 1)))
+    hel = np.ascontiguousarray(d_hel.cpu().numpy().T)
+    col = np.ascontiguousarray(np.transpose(d_col.cpu().numpy(), (2, 0, 1)))
+    truth = oracle.cdbg(mom, hel, col, prec="long double")
+    err = np.abs(d_out.cpu().numpy() - truth) / truth
+    assert np.median(err) < 1e-14 and np.mean(err > 1e-11) < 0.01
