@@ -55,6 +55,20 @@ __host__ __device__ inline bool colour_rule(int n, const signed char* ci, const 
     return true;
 }
 
+// The same rule on packed data without arrays: occ_out / occ_in hold the per-colour edge counts in three 8-bit
+// fields, pairs has bit 0 / 1 / 2 set when an edge joins colours {1,2} / {1,3} / {2,3}.
+__device__ __forceinline__ bool colour_rule_packed(int n, unsigned occ_out, unsigned occ_in, unsigned pairs) {
+    if (occ_out != occ_in) return false;                                  // colour charges balance
+    if (occ_out == (unsigned)n || occ_out == ((unsigned)n << 8) || occ_out == ((unsigned)n << 16)) return false;
+    const unsigned used = ((occ_out & 0xFFu) ? 1u : 0u) | ((occ_out & 0xFF00u) ? 2u : 0u) | ((occ_out & 0xFF0000u) ? 4u : 0u);
+    if (used == 7u) return __popc(pairs) >= 2;                            // three colours: two joining pairs connect them
+    if (used == 3u) return (pairs & 1u) != 0;
+    if (used == 5u) return (pairs & 2u) != 0;
+    if (used == 6u) return (pairs & 4u) != 0;
+    return true;                                                          // one colour only (excluded above when n edges)
+}
+
+template <int MO>   // number of outgoing gluons n - 2 (compile time: the momenta stay in registers)
 __global__ void __launch_bounds__(128)
 generate_kernel(int n, long long N, uint64_t seed, uint64_t stream, long long first_event, double sqrt_s, double ptmin,
                 double drmin, int reject_zero_hel, double* __restrict__ mom, signed char* __restrict__ hel,
@@ -72,20 +86,25 @@ generate_kernel(int n, long long N, uint64_t seed, uint64_t stream, long long fi
         for (int j = 0; j < 32; j++) {
             const long long ej = e0 + j;
             if (ej >= N) break;                      // uniform over the warp
-            signed char ci[12], cj[12];
             for (uint64_t t0 = 0;; t0 += 32) {
                 const uint64_t key = trial_key(seed, cs, (uint64_t)(first_event + ej), t0 + lane);
+                uint64_t packed = 0;                 // 4 bits per gluon: (i-1) | (j-1) << 2
+                unsigned occ_out = 0, occ_in = 0, pairs = 0;
                 for (int k = 0; k < n; k++) {
-                    int a = 1 + (int)(uni(key, 2 * k) * 3.0), b = 1 + (int)(uni(key, 2 * k + 1) * 3.0);
-                    ci[k] = (signed char)(a > 3 ? 3 : a);
-                    cj[k] = (signed char)(b > 3 ? 3 : b);
+                    int a = (int)(uni(key, 2 * k) * 3.0), b = (int)(uni(key, 2 * k + 1) * 3.0);
+                    a = a > 2 ? 2 : a;
+                    b = b > 2 ? 2 : b;
+                    packed |= (uint64_t)(a | (b << 2)) << (4 * k);
+                    occ_out += 1u << (8 * a);
+                    occ_in += 1u << (8 * b);
+                    if (a != b) pairs |= 1u << (a + b - 1);   // {0,1} -> bit 0, {0,2} -> bit 1, {1,2} -> bit 2
                 }
-                const unsigned ok = __ballot_sync(0xFFFFFFFFu, colour_rule(n, ci, cj));
+                const unsigned ok = __ballot_sync(0xFFFFFFFFu, colour_rule_packed(n, occ_out, occ_in, pairs));
                 if (ok) {
                     if (lane == __ffs(ok) - 1)
                         for (int k = 0; k < n; k++) {
-                            col[(size_t)(2 * k) * N + ej] = ci[k];
-                            col[(size_t)(2 * k + 1) * N + ej] = cj[k];
+                            col[(size_t)(2 * k) * N + ej] = (signed char)(1 + ((packed >> (4 * k)) & 3));
+                            col[(size_t)(2 * k + 1) * N + ej] = (signed char)(1 + ((packed >> (4 * k + 2)) & 3));
                         }
                     break;
                 }
@@ -95,14 +114,15 @@ generate_kernel(int n, long long N, uint64_t seed, uint64_t stream, long long fi
     }
     if (e >= N) return;
     const uint64_t ev = (uint64_t)(first_event + e);
-    const int m = n - 2;
+    constexpr int m = MO;
     const double kPi = 3.14159265358979323846;
     if (role == 0 && mom) {
-        double p[10][4];
+        double p[MO][4];
         for (uint64_t t = 0;; t++) {
             // RAMBO: isotropic massless q_i with energies -ln(u u'), boosted and scaled to (sqrt_s, 0, 0, 0)
             const uint64_t key = trial_key(seed, stream, ev, t);
             double Q[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
             for (int i = 0; i < m; i++) {
                 const double c = 2.0 * uni(key, 4 * i + 0) - 1.0;
                 const double phi = 2.0 * kPi * uni(key, 4 * i + 1);
@@ -114,6 +134,7 @@ generate_kernel(int n, long long N, uint64_t seed, uint64_t stream, long long fi
             const double M = sqrt(Q[0] * Q[0] - Q[1] * Q[1] - Q[2] * Q[2] - Q[3] * Q[3]);
             const double b[3] = {-Q[1] / M, -Q[2] / M, -Q[3] / M};
             const double x = sqrt_s / M, gam = Q[0] / M, a = 1.0 / (1.0 + gam);
+#pragma unroll
             for (int i = 0; i < m; i++) {
                 const double q0 = p[i][0], q1 = p[i][1], q2 = p[i][2], q3 = p[i][3];
                 const double bq = b[0] * q1 + b[1] * q2 + b[2] * q3;
@@ -124,34 +145,40 @@ generate_kernel(int n, long long N, uint64_t seed, uint64_t stream, long long fi
             }
             for (int it = 0; it < 2; it++) {   // polish momentum conservation and masslessness (see gen.c)
                 double d[3] = {0.0, 0.0, 0.0};
+#pragma unroll
                 for (int i = 0; i < m; i++)
                     for (int k = 0; k < 3; k++) d[k] += p[i][k + 1];
                 double esum = 0.0;
+#pragma unroll
                 for (int i = 0; i < m; i++) {
                     for (int k = 0; k < 3; k++) p[i][k + 1] -= d[k] / m;
                     p[i][0] = sqrt(p[i][1] * p[i][1] + p[i][2] * p[i][2] + p[i][3] * p[i][3]);
                     esum += p[i][0];
                 }
                 const double sc = sqrt_s / esum;
+#pragma unroll
                 for (int i = 0; i < m; i++)
                     for (int mu = 0; mu < 4; mu++) p[i][mu] *= sc;
             }
             if (ptmin <= 0.0 && drmin <= 0.0) break;
             bool ok = true;
-            double y[10], ph[10];
-            for (int i = 0; i < m && ok; i++) {
+            double y[MO], ph[MO];
+#pragma unroll
+            for (int i = 0; i < m; i++) {
                 const double pt = sqrt(p[i][1] * p[i][1] + p[i][2] * p[i][2]);
-                ok = pt > ptmin;
+                ok = ok && pt > ptmin;
                 y[i] = 0.5 * log((p[i][0] + p[i][3]) / (p[i][0] - p[i][3]));
                 ph[i] = atan2(p[i][2], p[i][1]);
             }
             if (ok && drmin > 0.0)
-                for (int i = 0; i < m && ok; i++)
-                    for (int j = i + 1; j < m && ok; j++) {
+#pragma unroll
+                for (int i = 0; i < m; i++)
+#pragma unroll
+                    for (int j = i + 1; j < m; j++) {
                         double dphi = fabs(ph[i] - ph[j]);
                         if (dphi > kPi) dphi = 2.0 * kPi - dphi;
                         const double dy = y[i] - y[j];
-                        ok = sqrt(dy * dy + dphi * dphi) > drmin;
+                        ok = ok && dy * dy + dphi * dphi > drmin * drmin;
                     }
             if (ok) break;
         }
@@ -160,6 +187,7 @@ generate_kernel(int n, long long N, uint64_t seed, uint64_t stream, long long fi
         for (int c = 0; c < 4; c++) {
             mom[(size_t)(0 * 4 + c) * N + e] = in0[c];
             mom[(size_t)(1 * 4 + c) * N + e] = in1[c];
+#pragma unroll
             for (int i = 0; i < m; i++) mom[(size_t)((i + 2) * 4 + c) * N + e] = p[i][c];
         }
     }
@@ -183,8 +211,17 @@ cudaError_t generate_launch(cudaStream_t s, int n, long long N, uint64_t seed, u
                             double sqrt_s, double ptmin, double drmin, int reject_zero_hel, double* mom, signed char* hel,
                             signed char* col) {
     const int B = (int)((N + 127) / 128);
-    generate_kernel<<<(unsigned)(3 * B), 128, 0, s>>>(n, N, seed, stream, first_event, sqrt_s, ptmin, drmin, reject_zero_hel,
-                                                      mom, hel, col, B);
+#define BG_GEN_CASE(MO)                                                                                              \
+    case MO:                                                                                                         \
+        generate_kernel<MO><<<(unsigned)(3 * B), 128, 0, s>>>(n, N, seed, stream, first_event, sqrt_s, ptmin, drmin, \
+                                                              reject_zero_hel, mom, hel, col, B);                     \
+        break;
+    switch (n - 2) {
+        BG_GEN_CASE(2) BG_GEN_CASE(3) BG_GEN_CASE(4) BG_GEN_CASE(5) BG_GEN_CASE(6) BG_GEN_CASE(7) BG_GEN_CASE(8)
+        BG_GEN_CASE(9) BG_GEN_CASE(10)
+        default: return cudaErrorInvalidValue;
+    }
+#undef BG_GEN_CASE
     return cudaGetLastError();
 }
 
