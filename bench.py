@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--continuous", action="store_true",
                     help="CDBG configs with continuous colour / polarisation states (Eq. 5-14, SURVEY NEXT-1)")
     ap.add_argument("--lc", action="store_true", help="configs 0 / 2 in leading-colour mode (Eq. 33, SURVEY NEXT-3)")
+    ap.add_argument("--comc", action="store_true",
+                    help="colour-dressed configs through BG_COMC_GIVEN (Eq. 19 with colour-ordered currents, SURVEY NEXT-2; n <= 8)")
     ap.add_argument("--precision", type=int, default=None, help="BG_OPT_PRECISION (1 = double-double reference path)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -225,6 +227,11 @@ def run_b200(args):
         flop_per_event = (3 ** (n - 1) - 2 ** n + 1) * 27 * 223.0
         args.no_e2e = True
         name += " - continuous colour/polarisation states (Eq. 5-14)"
+    if args.comc:
+        if args.config in (0, 2) or args.continuous:
+            raise SystemExit("--comc applies to the colour-dressed configs (1, 3, 4) with discrete colours")
+        mode = bg.BG_COMC_GIVEN          # same events, same |M|^2, same algorithmic flop: another recursion
+        name += " - CO_MC (Eq. 19, colour-ordered currents)"
     mom = wl.to_soa(mom=ev.mom)
     hel = None if ev.hel is None else wl.to_soa(hel=ev.hel)
     col = None if ev.col is None else wl.to_soa(col=ev.col)

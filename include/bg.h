@@ -57,6 +57,8 @@ enum {
     BG_CDBG_GIVEN = BG_REC_CDBG | BG_HEL_GIVEN | BG_COL_GIVEN,             /* BASELINE configs 2, 4, 5 */
     BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN,
     BG_CDBG_CONTINUOUS = BG_REC_CDBG | BG_HEL_CONT | BG_COL_CONT,          /* the paper's CD_MC sampling */
+    BG_COMC_GIVEN = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_GIVEN,            /* Eq. 19 with colour-ordered
+                                                                              currents, sampled colour flows (n <= 9) */
     BG_COBG_HELSUM_LC = BG_REC_COBG | BG_HEL_SUM | BG_COL_LC,
     BG_COBG_HELGIVEN_LC = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_LC
 };
@@ -91,6 +93,8 @@ int bg_init(bg_ctx** ctx, int n, int mode);
  *                        helicities in hel, or summed over all 2^n assignments when the mode has BG_HEL_SUM.
  *   COBG + LC          : out[e] = N_c^(n-2) (N_c^2 - 1) sum over all (n-1)! orderings sigma of gluons 2..n of
  *                        |A(1, sigma)|^2 (Eq. 33), helicities given or summed.
+ *   COBG + GIVEN colour: out[e] = |sum over the colour-connected orderings (1, sigma) of A(1, sigma)|^2 - the
+ *                        colour-flow decomposition Eq. 19; the same number as CDBG + GIVEN.
  *   CDBG + GIVEN colour: out[e] = |A_{i1 j1 .. in jn}|^2 from the subset recursion Eq. 29-32 closed with gluon n
  *                        (Eq. 22); assignments whose amplitude vanishes identically return exactly 0.0.
  * External currents are the helicity eigenvectors of Eq. 3 in the light-cone gauge of DESIGN.md reading g2.
@@ -157,6 +161,15 @@ const char* bg_last_kernel_name(const bg_ctx* ctx);
  * stats[3] = bytes of per-event state, stats[4] = colour code of the gluon chosen as closure leg.
  */
 int bg_class_program_stats(int n, int lanes, const int* counts, long long* stats);
+
+/*
+ * The same for the BG_COMC_GIVEN programs (Eq. 19, evaluated with the colour-ordered currents
+ * of Eq. 20-26; 4 <= n <= 8).  stats[0] = 1 if at least one ordering sigma has all its Kronecker deltas equal
+ * to one, stats[1] = vertex evaluations per event (shared between orderings: a sub-sequence current is computed
+ * once), stats[2] = interpreter steps, stats[3] = bytes of per-event state, stats[4] = number of such orderings
+ * (of (n-1)! with the first gluon fixed).  BG_EINVAL for bad arguments.
+ */
+int bg_comc_program_stats(int n, int lanes, const int* counts, long long* stats);
 
 /*
  * On-device event generation (the paper's timings include it): RAMBO flat massless

@@ -23,13 +23,14 @@ BG_CDBG_GIVEN = BG_REC_CDBG | BG_HEL_GIVEN | BG_COL_GIVEN
 BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN
 BG_HEL_CONT, BG_COL_CONT = 0x040, 0x800
 BG_CDBG_CONTINUOUS = BG_REC_CDBG | BG_HEL_CONT | BG_COL_CONT
+BG_COMC_GIVEN = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_GIVEN
 BG_COBG_HELSUM_LC = BG_REC_COBG | BG_HEL_SUM | BG_COL_LC
 BG_COBG_HELGIVEN_LC = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_LC
 BG_OPT_KERNEL, BG_OPT_SCRATCH_LIMIT, BG_OPT_LANES, BG_OPT_TIMING, BG_OPT_SMEM_LIMIT, BG_OPT_PRECISION = 1, 2, 3, 4, 5, 6
 
 EXPORTS = ("bg_init", "bg_eval", "bg_eval_continuous", "bg_generate", "bg_colour_rule", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",
            "bg_set_option", "bg_colour_matrix", "bg_build_colour_matrix", "bg_last_launch_count",
-           "bg_last_kernel_name", "bg_last_kernel_ms", "bg_class_program_stats", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe")
+           "bg_last_kernel_name", "bg_last_kernel_ms", "bg_class_program_stats", "bg_comc_program_stats", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe")
 
 
 class BgError(RuntimeError):
@@ -75,6 +76,8 @@ def load():
         lib.bg_last_kernel_ms.restype = i
         lib.bg_class_program_stats.argtypes = [i, i, vp, vp]
         lib.bg_class_program_stats.restype = i
+        lib.bg_comc_program_stats.argtypes = [i, i, vp, vp]
+        lib.bg_comc_program_stats.restype = i
         lib.bg_destroy.argtypes = [vp]
         lib.bg_strerror.argtypes = [i]
         lib.bg_strerror.restype = ctypes.c_char_p
@@ -204,6 +207,15 @@ def bg_class_program_stats(n: int, lanes: int, counts):
     c = np.ascontiguousarray(counts, dtype=np.int32)
     out = np.zeros(5, dtype=np.int64)
     _check(load().bg_class_program_stats(n, lanes, _ptr(c), _ptr(out)), "bg_class_program_stats")
+    return tuple(int(x) for x in out)
+
+
+def bg_comc_program_stats(n: int, lanes: int, counts):
+    """Host-only: (valid, vertex_ops, steps, state_bytes, orderings) of the CO_MC program for a colour multiset."""
+    import numpy as np
+    c = np.ascontiguousarray(counts, dtype=np.int32)
+    out = np.zeros(5, dtype=np.int64)
+    _check(load().bg_comc_program_stats(n, lanes, _ptr(c), _ptr(out)), "bg_comc_program_stats")
     return tuple(int(x) for x in out)
 
 

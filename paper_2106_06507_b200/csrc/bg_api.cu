@@ -142,6 +142,7 @@ static bool mode_supported(int n, int mode) {
     if (mode == BG_COBG_HELSUM_LC || mode == BG_COBG_HELGIVEN_LC) return bg::cobg_shared_supported(n);
     if (mode == BG_CDBG_GIVEN || mode == BG_CDBG_HELSUM_COLGIVEN) return true;
     if (mode == BG_CDBG_CONTINUOUS) return n <= 9;
+    if (mode == BG_COMC_GIVEN) return n <= 8;   // (n-1)! orderings per class: the state offsets are 16 bit
     return false;
 }
 
@@ -189,11 +190,11 @@ int bg_init(bg_ctx** out, int n, int mode) {
             cudaFree(c->dC); std::free(c->hC); delete c; return BG_ECUDA;
         }
     }
-    if ((mode & BG_REC_COBG) && bg::cobg_shared_supported(n)) {
+    if ((mode & BG_REC_COBG) && mode != BG_COMC_GIVEN && bg::cobg_shared_supported(n)) {
         const int rc = bg::cobg_table_create(n, &c->cobg);
         if (rc != BG_OK) { cudaFree(c->dC); std::free(c->hC); delete c; return rc; }
     }
-    if ((mode == BG_CDBG_GIVEN && n <= kProgMaxN) || mode == BG_CDBG_CONTINUOUS) {
+    if ((mode == BG_CDBG_GIVEN && n <= kProgMaxN) || mode == BG_CDBG_CONTINUOUS || mode == BG_COMC_GIVEN) {
         const int rc = make_prog_table(c, 0, 0, &c->prog);
         if (rc != BG_OK) { delete c; return rc; }
     }
@@ -254,7 +255,7 @@ static long long dd_chunk(const bg_ctx* c, long long N) {
 }
 
 static bool use_prog(const bg_ctx* c) {
-    if (c->mode == BG_CDBG_CONTINUOUS) return c->prog != nullptr;
+    if (c->mode == BG_CDBG_CONTINUOUS || c->mode == BG_COMC_GIVEN) return c->prog != nullptr;
     if (c->mode != BG_CDBG_GIVEN || c->kernel_opt == 1 || use_dd(c)) return false;
     return c->prog != nullptr;
 }
@@ -263,7 +264,8 @@ static bool use_prog(const bg_ctx* c) {
 static int auto_lanes_dense(int n) { return n <= 4 ? 32 : (n <= 6 ? 64 : (n == 7 ? 128 : 256)); }
 static int make_prog_table(const bg_ctx* c, int G, size_t limit, bg::ProgTable** t) {
     if (c->mode == BG_CDBG_CONTINUOUS) return bg::prog_table_create_dense(c->n, G ? G : auto_lanes_dense(c->n), limit, c->kernel_opt != 1, t);
-    return bg::prog_table_create(c->n, G ? G : auto_lanes(c->n), limit ? limit : auto_slab_limit(c->n), t);
+    if (c->mode == BG_COMC_GIVEN) return bg::prog_table_create(c->n, G ? G : (c->n >= 7 ? 128 : auto_lanes(c->n)), limit, true, t);
+    return bg::prog_table_create(c->n, G ? G : auto_lanes(c->n), limit ? limit : auto_slab_limit(c->n), false, t);
 }
 
 // events per generic-CDBG launch under the scratch limit
@@ -278,6 +280,7 @@ static long long generic_chunk(const bg_ctx* c, long long N) {
 size_t bg_scratch_bytes(const bg_ctx* c, long long N) {
     if (!c || N <= 0) return 0;
     if (use_cobg_dd(c)) return bg::cobg_dd_scratch_per_event(c->n, (c->mode & BG_HEL_SUM) != 0) * (size_t)cobg_dd_chunk(c, N);
+    if (c->mode == BG_COMC_GIVEN) return c->prog ? bg::prog_scratch_bytes(c->prog, N) : 0;
     if (!(c->mode & BG_REC_CDBG)) return 0;
     if (use_dd(c)) return bg::cdbg_dd_scratch_per_event(c->n) * (size_t)dd_chunk(c, N);
     if (use_prog(c)) return bg::prog_scratch_bytes(c->prog, N);
@@ -286,6 +289,7 @@ size_t bg_scratch_bytes(const bg_ctx* c, long long N) {
 
 size_t bg_current_bytes_per_event(const bg_ctx* c) {
     if (!c) return 0;
+    if (c->mode == BG_COMC_GIVEN) return c->prog ? bg::prog_state_bytes(c->prog) : 0;
     if ((c->mode & BG_REC_COBG) && c->cobg && c->kernel_opt != 1) return bg::cobg_shared_current_bytes(c->cobg);
     if (c->mode & BG_REC_COBG) return (size_t)(c->n - 1) * c->n / 2 * 64;   // one ordering's current table
     if (use_prog(c)) return bg::prog_state_bytes(c->prog);
@@ -338,7 +342,8 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
             c->kernel_opt = (int)value;
             return BG_OK;
         case BG_OPT_LANES: {
-            if ((c->mode != BG_CDBG_GIVEN && c->mode != BG_CDBG_CONTINUOUS) || c->n > kProgMaxN) return BG_EUNSUPPORTED;
+            if ((c->mode != BG_CDBG_GIVEN && c->mode != BG_CDBG_CONTINUOUS && c->mode != BG_COMC_GIVEN) || c->n > kProgMaxN)
+                return BG_EUNSUPPORTED;
             if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8 && value != 16 && value != 32 &&
                 value != 64 && value != 128 && value != 256)
                 return BG_EINVAL;
@@ -354,7 +359,8 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
             return BG_OK;
         }
         case BG_OPT_SMEM_LIMIT: {
-            if ((c->mode != BG_CDBG_GIVEN && c->mode != BG_CDBG_CONTINUOUS) || !c->prog) return BG_EUNSUPPORTED;
+            if ((c->mode != BG_CDBG_GIVEN && c->mode != BG_CDBG_CONTINUOUS && c->mode != BG_COMC_GIVEN) || !c->prog)
+                return BG_EUNSUPPORTED;
             if (value != 0 && (value < 16 * 1024 || value > 222 * 1024)) return BG_EINVAL;
             cudaDeviceSynchronize();
             bg::ProgTable* t = nullptr;
@@ -418,6 +424,25 @@ int bg_class_program_stats(int n, int lanes, const int* counts, long long* stats
     return BG_OK;
 }
 
+int bg_comc_program_stats(int n, int lanes, const int* counts, long long* stats) {
+    if (n < 4 || n > 8 || !counts || !stats || lanes < 1 || lanes > 256 || (lanes & (lanes - 1))) return BG_EINVAL;
+    int sum = 0, code[bg::kMaxN];
+    for (int c = 0; c < bg::kNumCodes; c++) {
+        if (counts[c] < 0 || sum + counts[c] > n) return BG_EINVAL;
+        for (int q = 0; q < counts[c]; q++) code[sum++] = c;
+    }
+    if (sum != n) return BG_EINVAL;
+    bg::ClassProgram p;
+    bg::build_comc_program(n, lanes, code, p);
+    if (p.state_cx < 0) return BG_EUNSUPPORTED;
+    stats[0] = p.valid ? 1 : 0;
+    stats[1] = p.n_vertex_ops;
+    stats[2] = p.total_steps;
+    stats[3] = (long long)p.state_cx * 16;
+    stats[4] = p.n_orderings;
+    return BG_OK;
+}
+
 int bg_last_launch_count(const bg_ctx* c) { return c ? c->last_launches : 0; }
 
 int bg_last_kernel_ms(bg_ctx* c, double* ms) {
@@ -455,7 +480,7 @@ int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const 
         }
         if (ev1) cudaEventRecord(ev1, s);
         c->last_kernel = "cobg_dd_kernel";
-    } else if (c->mode & BG_REC_COBG) {
+    } else if ((c->mode & BG_REC_COBG) && c->mode != BG_COMC_GIVEN) {
         if (ev0) cudaEventRecord(ev0, s);
         if (c->cobg && (c->kernel_opt != 1 || (c->mode & BG_COL_LC))) {
             err = bg::cobg_shared_launch(s, c->cobg, helsum, (c->mode & BG_COL_LC) != 0, c->dC, N, mom, hel, out);

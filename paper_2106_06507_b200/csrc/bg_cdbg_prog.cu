@@ -672,7 +672,7 @@ static void enumerate_counts(int t, int r, int* counts, std::vector<std::vector<
     }
 }
 
-int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out) {
+int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** out) {
     if (slab_limit == 0 || slab_limit > kMaxSlabBytes) slab_limit = kMaxSlabBytes;
     *out = nullptr;
     if (n < 4 || n > kMaxN || (G != 1 && G != 2 && G != 4 && G != 8 && G != 16 && G != 32 && G != 64 && G != 128 && G != 256)) return BG_EINVAL;
@@ -691,9 +691,27 @@ int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out) {
             if (class_rank(n, all[r].data()) != r) return BG_EINVAL;
         std::vector<ClassProgram> progs(nc);
         std::atomic<long long> next_class{0};
+        std::atomic<bool> overflow{false};   // CO_MC: a class with too many orderings for the 16-bit state offsets
         auto worker = [&]() {
             for (long long r = next_class.fetch_add(1); r < nc; r = next_class.fetch_add(1))
-                build_class(n, G, all[r].data(), progs[r]);
+                if (!comc) {
+                    build_class(n, G, all[r].data(), progs[r]);
+                } else {
+                    // CO_MC: canonical order = codes ascending; only classes with balanced colour charges can be non-zero
+                    const int* cnt = all[r].data();
+                    bool balanced = true;
+                    for (int c = 0; c < 3; c++) {
+                        int ni = 0, nj = 0;
+                        for (int t = 0; t < kNumCodes; t++) { if (t / 3 == c) ni += cnt[t]; if (t % 3 == c) nj += cnt[t]; }
+                        balanced = balanced && ni == nj;
+                    }
+                    if (!balanced) continue;
+                    int code[kMaxN], k = 0;
+                    for (int t = 0; t < kNumCodes; t++)
+                        for (int q = 0; q < cnt[t]; q++) code[k++] = t;
+                    build_comc_program(n, G, code, progs[r]);
+                    if (progs[r].state_cx < 0 || progs[r].state_cx > 65535) overflow = true;
+                }
         };
         unsigned nthreads = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
         if (n <= 8) nthreads = 1;
@@ -701,6 +719,7 @@ int prog_table_create(int n, int G, size_t slab_limit, ProgTable** out) {
         for (unsigned i = 1; i < nthreads; i++) pool.emplace_back(worker);
         worker();
         for (auto& th : pool) th.join();
+        if (overflow) return BG_EUNSUPPORTED;
         size_t total_ops = 0;
         for (auto& cp : progs) total_ops += cp.ops.size();
         ops.reserve(total_ops + G);

@@ -3,6 +3,7 @@
 
 #include <algorithm>
 #include <cstring>
+#include <map>
 
 namespace bg {
 
@@ -491,6 +492,234 @@ void build_class(int n, int G, const int* counts, ClassProgram& out) {
             have = true;
         }
     }
+}
+
+}  // namespace bg
+
+// ---------------------------------------------------------------------------------------------------------
+// CO_MC: the colour-flow decomposition Eq. 19 evaluated with colour-ORDERED
+// currents.  For canonical colour codes the orderings (1, sigma_2 .. sigma_n) whose colour chain closes (the j of each
+// gluon is the i of the next, cyclically) are enumerated by depth-first search; the amplitude is the sum of the
+// colour-ordered amplitudes A(1, sigma) of those orderings.  Each A is the recursion Eq. 24-25 (tensor form) over
+// contiguous sub-sequences; sub-sequences shared by several orderings are computed once.  The vertex
+// X(J(i..k), J(k+1..j)) is the same operation the colour-dressed programs use, so the same interpreter runs it.
+// ---------------------------------------------------------------------------------------------------------
+namespace bg {
+
+namespace {
+struct SeqNode {
+    std::vector<int> seq;   // canonical gluon indices
+    unsigned mask = 0;
+    int off = -1;           // state offset of its current (4 + 6 cx); -1: external or fused
+    bool closure = false;   // first n-1 gluons of an ordering: contracted with eps of the last one
+    int last = -1;          // closure: the gluon that closes
+    std::vector<std::pair<int, int>> fuses;   // (closure node id, split position) read straight from registers
+};
+}  // namespace
+
+void build_comc_program(int n, int G, const int* code, ClassProgram& out, long long max_orderings) {
+    out = ClassProgram();
+    int ci[kMaxN], cj[kMaxN];
+    for (int k = 0; k < n; k++) { ci[k] = code[k] / 3; cj[k] = code[k] % 3; }
+    out.closure_code = code[n - 1];
+    // colour-connected orderings starting with gluon 0 (depth-first; j of the last must be i of gluon 0)
+    std::vector<std::vector<int>> orderings;
+    {
+        std::vector<int> cur{0};
+        unsigned used = 1;
+        bool overflow = false;
+        auto dfs = [&](auto&& self) -> void {
+            if (overflow) return;
+            if ((int)cur.size() == n) {
+                if (cj[cur.back()] == ci[0]) {
+                    orderings.push_back(cur);
+                    if ((long long)orderings.size() > max_orderings) overflow = true;
+                }
+                return;
+            }
+            for (int g = 1; g < n; g++) {
+                if ((used >> g) & 1u) continue;
+                if (cj[cur.back()] != ci[g]) continue;
+                used |= 1u << g;
+                cur.push_back(g);
+                self(self);
+                cur.pop_back();
+                used &= ~(1u << g);
+            }
+        };
+        dfs(dfs);
+        if (overflow) { out.state_cx = -1; return; }   // too many orderings for a tabulated program: unsupported
+    }
+    if (orderings.empty()) return;
+    out.valid = true;
+    out.n_orderings = (long long)orderings.size();
+
+    // nodes: single gluons 0..n-1, then every distinct contiguous sub-sequence (length >= 2) of the first n-1
+    // elements of the orderings
+    std::vector<SeqNode> nodes(n);
+    std::map<std::vector<int>, int> id_of;
+    for (int g = 0; g < n; g++) { nodes[g].seq = {g}; nodes[g].mask = 1u << g; id_of[nodes[g].seq] = g; }
+    const int m = n - 1;
+    std::vector<std::vector<int>> by_len(m + 1);
+    for (auto& o : orderings)
+        for (int L = 2; L <= m; L++)
+            for (int i = 0; i + L <= m; i++) {
+                std::vector<int> s(o.begin() + i, o.begin() + i + L);
+                if (id_of.count(s)) continue;
+                SeqNode nd;
+                nd.seq = s;
+                for (int g : s) nd.mask |= 1u << g;
+                id_of[s] = (int)nodes.size();
+                by_len[L].push_back((int)nodes.size());
+                nodes.push_back(std::move(nd));
+            }
+    for (auto& o : orderings) {
+        SeqNode& c = nodes[id_of[std::vector<int>(o.begin(), o.begin() + m)]];
+        c.closure = true;
+        c.last = o[m];
+    }
+    auto sub = [&](const SeqNode& nd, int i, int j) { return id_of[std::vector<int>(nd.seq.begin() + i, nd.seq.begin() + j)]; };
+    auto len = [&](int id) { return (int)nodes[id].seq.size(); };
+
+    // layout: externals + momenta, then stored currents (length 2 .. n-3) and one momentum per distinct gluon set
+    int next = 0;
+    std::vector<int> ext_off(n), ext_poff(n);
+    for (int g = 0; g < n; g++) { ext_off[g] = next; nodes[g].off = next; next += 4; }
+    std::map<unsigned, int> poff;
+    for (int g = 0; g < n; g++) { poff[1u << g] = next; ext_poff[g] = next; next += 2; }
+    const int pad = G >= 8 ? 1 : 0;
+    // length n-2 sequences are read by closure vertices only: fused, never stored
+    for (int L = 2; L <= m; L++)
+        for (int id : by_len[L]) {
+            if (L <= m - 2 || (L == m - 1 && m - 1 < 2)) { nodes[id].off = next; next += 10 + pad; }
+            if (L <= m - 1 && !poff.count(nodes[id].mask)) { poff[nodes[id].mask] = -1; }
+        }
+    // which momenta are read: P(a) of every vertex and P(b) of first vertices; simply give every set of length <= n-2
+    // that occurs a slot, written by the first node (in emission order) with that set
+    std::map<unsigned, int> p_writer;
+    for (int L = 2; L <= m - 1; L++)
+        for (int id : by_len[L])
+            if (poff[nodes[id].mask] < 0) { poff[nodes[id].mask] = next; next += 2; p_writer[nodes[id].mask] = id; }
+    // closure targets need P(a), P(b) of their vertices only (both of length <= n-2): nothing to store for them
+
+    // fuse: closure vertices whose larger operand has length n-2
+    if (m - 1 >= 2)
+        for (int L = m; L <= m; L++)
+            for (int id : by_len[L]) {
+                if (!nodes[id].closure) continue;
+                nodes[sub(nodes[id], 1, m)].fuses.push_back({id, 1});        // X(gluon seq[0], seq[1..m-1])
+                nodes[sub(nodes[id], 0, m - 1)].fuses.push_back({id, m - 1});  // X(seq[0..m-2], gluon seq[m-1])
+            }
+
+    out.level_steps.assign(2 * m - 2, 0);
+    auto emit_level = [&](int lvl, std::vector<std::vector<ProgOp>>& lanes) {
+        size_t steps = 0;
+        for (auto& l : lanes) steps = std::max(steps, l.size());
+        out.level_steps[lvl] = (uint16_t)steps;
+        ProgOp nop;
+        std::memset(&nop, 0, sizeof(nop));
+        for (size_t s = 0; s < steps; s++)
+            for (int l = 0; l < G; l++) {
+                ProgOp o = s < lanes[l].size() ? lanes[l][s] : nop;
+                if (s + 1 == steps) o.flags |= OPF_SYNC;
+                out.ops.push_back(o);
+            }
+        out.total_steps += (int)steps;
+        if (steps) out.n_sync++;
+    };
+    {   // level 0: all n external currents and momenta
+        std::vector<std::vector<ProgOp>> lanes(G);
+        for (int g = 0; g < n; g++) {
+            ProgOp o;
+            std::memset(&o, 0, sizeof(o));
+            o.flags = OPF_EXT;
+            o.extra = (uint32_t)g;
+            o.offDst = (uint16_t)ext_off[g];
+            o.offPt = (uint16_t)ext_poff[g];
+            lanes[g % G].push_back(o);
+        }
+        emit_level(0, lanes);
+    }
+    // vertex X(seq[0..k), seq[k..L)) of node `id`; the shorter operand goes first (X is antisymmetric)
+    auto make_vertex = [&](int id, int k, bool closure_target) {
+        const SeqNode& nd = nodes[id];
+        const int L = (int)nd.seq.size();
+        int a = sub(nd, 0, k), b = sub(nd, k, L);
+        bool neg = false;
+        if (len(a) > len(b)) { std::swap(a, b); neg = true; }
+        ProgOp o;
+        std::memset(&o, 0, sizeof(o));
+        o.offA = (uint16_t)nodes[a].off;
+        o.offB = (uint16_t)nodes[b].off;
+        o.offP1 = (uint16_t)poff[nodes[a].mask];
+        o.extra = (uint32_t)poff[nodes[b].mask];
+        o.offPt = 0xFFFF;
+        o.flags = OPF_VALID | (neg ? OPF_NEG : 0) | (len(a) >= 2 ? OPF_TENA : 0) | (len(b) >= 2 ? OPF_TENB : 0) |
+                  (closure_target ? OPF_CLOSURE : 0);
+        return o;
+    };
+    for (int L = 2; L <= m; L++) {
+        std::vector<std::vector<ProgOp>> lanes(G), clanes(G);
+        std::vector<int> load(G, 0);
+        auto least = [&]() { return (int)(std::min_element(load.begin(), load.end()) - load.begin()); };
+        if (L == m) {
+            // closure targets: the vertices not fused (2 <= k <= m-2), one run per ordering
+            for (int id : by_len[L]) {
+                if (!nodes[id].closure) continue;
+                std::vector<ProgOp> run;
+                for (int k = (m - 1 >= 2 ? 2 : 1); k <= (m - 1 >= 2 ? m - 2 : m - 1); k++) {
+                    ProgOp o = make_vertex(id, k, true);
+                    o.offDst = (uint16_t)ext_off[nodes[id].last];
+                    run.push_back(o);
+                }
+                if (run.empty()) continue;
+                run.front().flags |= OPF_FIRST;
+                run.back().flags |= OPF_LAST;
+                const int l = least();
+                load[l] += (int)run.size();
+                lanes[l].insert(lanes[l].end(), run.begin(), run.end());
+                out.n_vertex_ops += (int)run.size();
+            }
+            emit_level(2 * (L - 2) + 1, lanes);
+            break;
+        }
+        std::vector<int> order = by_len[L];
+        auto cost = [&](int id) { return L - 1 + (int)nodes[id].fuses.size(); };
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return cost(a) > cost(b); });
+        for (int id : order) {
+            const int l = least();
+            load[l] += cost(id);
+            const bool writes_p = p_writer.count(nodes[id].mask) && p_writer[nodes[id].mask] == id;
+            for (int k = 1; k < L; k++) {
+                ProgOp o = make_vertex(id, k, false);
+                o.offDst = nodes[id].off >= 0 ? (uint16_t)nodes[id].off : (uint16_t)0xFFFF;
+                if (k == 1) o.flags |= OPF_FIRST;
+                if (k == L - 1) {
+                    o.flags |= OPF_LAST | (nodes[id].off < 0 ? OPF_NOSTORE : 0) | (writes_p ? OPF_STOREP : 0);
+                    if (writes_p) o.offPt = (uint16_t)poff[nodes[id].mask];
+                }
+                lanes[l].push_back(o);
+                out.n_vertex_ops++;
+            }
+            for (auto& fz : nodes[id].fuses) {
+                // closure vertex of ordering fz.first: X(single gluon, this sequence), sign by which side the gluon is on
+                const SeqNode& c = nodes[fz.first];
+                const int single = fz.second == 1 ? c.seq[0] : c.seq[m - 1];
+                ProgOp o;
+                std::memset(&o, 0, sizeof(o));
+                o.offA = (uint16_t)ext_off[single];
+                o.offP1 = (uint16_t)ext_poff[single];
+                o.offDst = (uint16_t)ext_off[c.last];
+                // X(prefix, suffix): gluon first (k = 1) is X(single, this); gluon last is X(this, single) = -X(single, this)
+                o.flags = OPF_FUSED | (fz.second == 1 ? 0 : OPF_NEG);
+                lanes[l].push_back(o);
+                out.n_vertex_ops++;
+            }
+        }
+        emit_level(2 * (L - 2) + 1, lanes);
+        emit_level(2 * (L - 2) + 2, clanes);
+    }
+    out.state_cx = next;
 }
 
 }  // namespace bg

@@ -59,6 +59,7 @@ struct ClassProgram {
     int n_vertex_ops = 0;        // number of OPF_VALID ops
     int total_steps = 0;         // sum over levels of max-lane op count
     int n_sync = 0;              // number of steps that end with a barrier (non-empty levels)
+    long long n_orderings = 0;   // CO_MC programs: colour-connected orderings summed (Eq. 19)
     std::vector<uint16_t> level_steps;   // [2n-4]: setup | (main, combine) for popcount 2..n-2 | closure
     std::vector<ProgOp> ops;             // [total_steps][G]
 };
@@ -71,6 +72,9 @@ long long class_rank(int n, const int* counts);
 // dense: continuous colour states (nine live entries per subset, `code` ignored); real: the state elements are
 // doubles instead of complex doubles (a 4-momentum then takes four elements instead of two).
 void build_program(int n, int G, const int* code, ClassProgram& out, bool dense = false, bool real = false);
+// CO_MC (Eq. 19 with colour-ordered currents): program for canonical colour codes; classes with more than
+// max_orderings colour-connected orderings are left invalid with state_cx = -1 (unsupported, not zero).
+void build_comc_program(int n, int G, const int* code, ClassProgram& out, long long max_orderings = 20000);
 // Build the best program (over the choice of closure leg) for a multiset of colour codes.
 void build_class(int n, int G, const int* counts, ClassProgram& out);
 

@@ -39,7 +39,7 @@ def test_strerror_and_modes(bg):
     for code in (-1, -2, -3, -4, -99):
         assert isinstance(bg.bg_strerror(code), str) and bg.bg_strerror(code)
     assert bg.BG_CDBG_GIVEN == 0x222 and bg.BG_COBG_HELSUM_FULLCOLOR == 0x111
-    assert bg.BG_COBG_HELGIVEN_FULLCOLOR == 0x121
+    assert bg.BG_COBG_HELGIVEN_FULLCOLOR == 0x121 and bg.BG_COMC_GIVEN == 0x221
 
 
 def test_init_argument_errors_without_touching_kernels(bg):
@@ -50,7 +50,10 @@ def test_init_argument_errors_without_touching_kernels(bg):
         bg.bg_init(13, bg.BG_CDBG_GIVEN)
     assert e.value.code == bg.BG_EINVAL
     with pytest.raises(bg.BgError) as e:
-        bg.bg_init(6, bg.BG_REC_COBG | bg.BG_HEL_GIVEN | bg.BG_COL_GIVEN)     # CO_MC is not built
+        bg.bg_init(9, bg.BG_COMC_GIVEN)                                        # CO_MC: (n-1)! orderings, n <= 8
+    assert e.value.code == bg.BG_EUNSUPPORTED
+    with pytest.raises(bg.BgError) as e:
+        bg.bg_init(6, bg.BG_REC_COBG | bg.BG_HEL_SUM | bg.BG_COL_GIVEN)       # not a combination the library has
     assert e.value.code == bg.BG_EUNSUPPORTED
     with pytest.raises(bg.BgError) as e:
         bg.bg_init(9, bg.BG_COBG_HELGIVEN_FULLCOLOR)                           # colour matrix too large

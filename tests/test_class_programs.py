@@ -54,3 +54,44 @@ def test_bad_arguments(bg):
         bg.bg_class_program_stats(6, 3, np.array([6, 0, 0, 0, 0, 0, 0, 0, 0]))
     with pytest.raises(bg.BgError):
         bg.bg_class_program_stats(6, 4, np.array([5, 0, 0, 0, 0, 0, 0, 0, 0]))
+
+
+def connected_orderings(codes):
+    """Brute force over the (n-1)! orderings of Eq. 19 with gluon 0 first: those whose deltas are all one."""
+    n = len(codes)
+    ci, cj = [c // 3 for c in codes], [c % 3 for c in codes]
+    cnt = 0
+    for rest in itertools.permutations(range(1, n)):
+        o = (0,) + rest
+        cnt += all(cj[o[k]] == ci[o[(k + 1) % n]] for k in range(n))
+    return cnt
+
+
+@pytest.mark.parametrize("n", [4, 5, 6])
+def test_comc_programs_sum_the_colour_connected_orderings(bg, wl, oracle, n):
+    mom = wl.config_events(4, N=1, n=n).mom
+    hel = np.ones((1, n), dtype=np.int8)
+    for codes in multisets(n):
+        counts = np.bincount(codes, minlength=9)
+        valid, nvert, steps, state, nord = bg.bg_comc_program_stats(n, 4, counts)
+        expect = connected_orderings(codes)
+        assert nord == expect and bool(valid) == (expect > 0), (codes, nord, expect)
+        col = np.array([[[c // 3 + 1, c % 3 + 1] for c in codes]], dtype=np.int8)
+        # rule g8 is stricter: e.g. all gluons in one U(1) colour state connect in every ordering but sum to zero
+        assert bool(valid) or not wl.colour_valid(col[0])
+        if valid:
+            # the oracle's Eq. 19 brute force counts the same orderings
+            assert oracle.colour_flow(mom, hel, col, return_count=True)[1][0] == nord
+            # currents of shared sub-sequences are evaluated once: never more vertices than ordering-by-ordering
+            per_ordering = sum((n - L) * (L - 1) for L in range(2, n))     # splits of all sub-sequences, Eq. 20
+            assert 0 < nvert <= nord * per_ordering and steps * 4 >= nvert
+    same = np.zeros(9, dtype=np.int64)
+    same[0] = n
+    assert bg.bg_comc_program_stats(n, 4, same)[4] == {4: 6, 5: 24, 6: 120}[n]        # (n-1)!
+
+
+def test_comc_bad_arguments(bg):
+    with pytest.raises(bg.BgError):
+        bg.bg_comc_program_stats(9, 4, np.array([9, 0, 0, 0, 0, 0, 0, 0, 0]))
+    with pytest.raises(bg.BgError):
+        bg.bg_comc_program_stats(6, 4, np.array([5, 0, 0, 0, 0, 0, 0, 0, 0]))

@@ -276,6 +276,44 @@ def test_continuous_colour_and_polarisation_states(bg, oracle, wl, n, N, lanes, 
     assert np.mean(err > 1e-11) <= 0.02 and err.max() < 1e-7
 
 
+@pytest.mark.parametrize("n,N", [(4, 500), (5, 700), (6, 2051), (7, 1031), (8, 259)])
+def test_colour_ordered_monte_carlo_mode(bg, oracle, wl, n, N):
+    """CO_MC: Eq. 19 summed over the colour-connected orderings with colour-ordered currents, on
+    the device.  Truth = the colour-dressed oracle in long double (a different algorithm for the same number);
+    for an event over 1e-11 the FP64 floor is what the oracle's own Eq. 19 sum in double precision delivers
+    (cancellations BETWEEN orderings, which the colour-dressed recursion does not have), relabelled 8 ways."""
+    ev = wl.config_events(4, N=N, n=n)
+    got, name = gpu_eval(ev, bg.BG_COMC_GIVEN)
+    assert name == "cdbg_prog_kernel"
+    truth = oracle.cdbg(ev.mom, ev.hel, ev.col, prec="long double")
+    err = rel_err(got, truth)
+    tail = np.nonzero(err > 1e-11)[0]
+    assert len(tail) <= max(3, 0.01 * N) and np.median(err) < 1e-13
+    if len(tail):
+        te = ev.take(tail)
+        floor = rel_err(oracle.colour_flow(te.mom, te.hel, te.col), truth[tail])
+        rng = np.random.default_rng(11)
+        for _ in range(8):
+            perm = rng.permutation(n)
+            floor = np.maximum(floor, rel_err(oracle.colour_flow(te.mom[:, perm], te.hel[:, perm], te.col[:, perm]),
+                                              truth[tail]))
+        floor = np.maximum(floor, fp64_noise_floor(oracle, te, truth[tail], True, reps=8))
+        assert np.all(err[tail] <= 10 * floor), (err[tail], floor)
+    # same events through the colour-dressed interpreter: the two recursions agree
+    dressed, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
+    assert np.mean(rel_err(got, dressed) > 1e-11) <= 0.01
+    # spilled state and more lanes give the same numbers up to summation order
+    if n == 7:
+        other, _ = gpu_eval(ev, bg.BG_COMC_GIVEN, lanes=256, smem_limit=48 * 1024)
+        assert np.mean(rel_err(other, got) > 1e-11) <= 0.01
+
+
+def test_colour_ordered_monte_carlo_rejects_large_n(bg):
+    with pytest.raises(bg.BgError) as e:
+        bg.bg_init(9, bg.BG_COMC_GIVEN)
+    assert e.value.code == bg.BG_EUNSUPPORTED
+
+
 def test_cdbg_helicity_sum_mode(bg, oracle, wl):
     import itertools
     ev = wl.config_events(4, N=40, n=5)
