@@ -225,11 +225,6 @@ void build_program(int n, int G, const int* code, ClassProgram& out, bool dense,
     // offsets that differ modulo 8/EPW.  The order of the vertices inside a unit is free, so every lane picks, step
     // by step, the remaining vertex of its unit that collides least with what its neighbours read at that step.
     auto reduce_bank_conflicts = [&](std::vector<std::vector<ProgOp>>& lanes) {
-        const int EPW = G >= 32 ? 1 : 32 / G;
-        const int M = 8 / EPW, group = 8 / EPW;
-        if (M <= 1 || G < group) return;
-        size_t steps = 0;
-        for (auto& l : lanes) steps = std::max(steps, l.size());
         auto swap_operands = [](ProgOp& x, ProgOp& y) {
             std::swap(x.offA, y.offA); std::swap(x.offB, y.offB); std::swap(x.offP1, y.offP1); std::swap(x.extra, y.extra);
             const uint16_t keep = OPF_NEG | OPF_TENA | OPF_TENB;
@@ -237,6 +232,28 @@ void build_program(int n, int G, const int* code, ClassProgram& out, bool dense,
             x.flags = (uint16_t)((x.flags & ~keep) | fy);
             y.flags = (uint16_t)((y.flags & ~keep) | fx);
         };
+        // Lanes of one warp whose vertices differ in kind (tensor of pi_1 / pi_2 present or not) run the tensor
+        // contractions one kind after the other; inside every unit the vertices are therefore ordered by kind
+        // (both tensors, one, none), which lines the kinds up across the lanes of a level.
+        auto kind = [](const ProgOp& o) { return ((o.flags & OPF_TENA) ? 2 : 0) + ((o.flags & OPF_TENB) ? 1 : 0); };
+        for (auto& ln : lanes)
+            for (size_t s = 0; s < ln.size();) {
+                if (!(ln[s].flags & OPF_VALID)) { s++; continue; }
+                size_t last = s;
+                while (!(ln[last].flags & OPF_LAST)) last++;
+                for (size_t i = s; i <= last; i++) {          // selection sort: units are short
+                    size_t best = i;
+                    for (size_t c = i + 1; c <= last; c++)
+                        if (kind(ln[c]) > kind(ln[best])) best = c;
+                    if (best != i) swap_operands(ln[i], ln[best]);
+                }
+                s = last + 1;
+            }
+        const int EPW = G >= 32 ? 1 : 32 / G;
+        const int M = 8 / EPW, group = 8 / EPW;
+        if (M <= 1 || G < group) return;
+        size_t steps = 0;
+        for (auto& l : lanes) steps = std::max(steps, l.size());
         for (size_t s = 0; s < steps; s++)
             for (int g0 = 0; g0 < G; g0 += group)
                 for (int l = g0 + 1; l < std::min(G, g0 + group); l++) {
@@ -253,6 +270,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out, bool dense,
                             if (o.offA != r.offA && o.offA % M == r.offA % M) c += 10;
                             if (o.offB != r.offB && o.offB % M == r.offB % M) c += 10;
                             if (o.offP1 != r.offP1 && o.offP1 % M == r.offP1 % M) c += 2;
+                            if (kind(o) != kind(r)) c += 1;
                         }
                         return c;
                     };

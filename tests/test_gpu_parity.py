@@ -272,8 +272,18 @@ def test_continuous_colour_and_polarisation_states(bg, oracle, wl, n, N, lanes, 
     err = rel_err(got, truth)
     # all nine colour entries contribute: the sub-amplitude is a dense sum without the single-flow near-zeros, but
     # it is a sum over many colour orderings that can still cancel: same noise-floor rule as everywhere
-    assert np.median(err) < 1e-13
-    assert np.mean(err > 1e-11) <= 0.02 and err.max() < 1e-7
+    assert np.median(err) < 1e-13 and err.max() < 1e-7
+    tail = np.nonzero(err > 1e-11)[0]
+    assert len(tail) <= max(2, 0.02 * N)
+    if len(tail):
+        # FP64 floor of these events: the oracle itself in double precision, gluons relabelled 16 ways
+        rng = np.random.default_rng(7)
+        floor = rel_err(oracle.cdbg_continuous(mom[tail], phi[tail], eta[tail]), truth[tail])
+        for _ in range(16):
+            perm = rng.permutation(n)
+            floor = np.maximum(floor, rel_err(oracle.cdbg_continuous(mom[tail][:, perm], phi[tail][:, perm],
+                                                                     eta[tail][:, perm]), truth[tail]))
+        assert np.all(err[tail] <= 10 * floor), (err[tail], floor)
 
 
 @pytest.mark.parametrize("n,N", [(4, 500), (5, 700), (6, 2051), (7, 1031), (8, 259)])
