@@ -744,11 +744,69 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
     // grouping order: longest programs first (the tail of the grid then runs the short ones), invalid last
     std::vector<uint32_t> by(nc), sortkey(nc);
     std::iota(by.begin(), by.end(), 0u);
-    // tiers by state size (tier 0 = the largest blocks); inside a tier the longest programs come first, classes
-    // whose amplitude vanishes (no state, no steps) end up last
+    // Tiers by state size (tier 0 = the largest blocks); inside a tier the longest programs come first, classes
+    // whose amplitude vanishes (no state, no steps) end up last.  A tier's slab size decides how many blocks an SM
+    // holds, so the (at most kTiers) slab sizes are chosen among the classes' state sizes to minimise
+    //     sum over tiers of work(tier) / rate(resident warps(slab)),
+    // work = steps x the class's share of uniformly drawn colour assignments (n! / prod counts!), rate(w) = w/(w+7)
+    // (fitted to the measured FP64 pipe utilisation against resident warps: 0.29 at 4.6, 0.43 at 10 warps per SM).
     TierInfo tiers;
-    static const double kTierFrac[kTiers] = {1.0, 0.8, 0.64, 0.5};
-    for (int k = 0; k < kTiers; k++) tiers.slab_cx[k] = std::max(16, (int)(max_state * kTierFrac[k] + 0.999));
+    {
+        const int block = G > 32 ? G : 32, epw = G >= 32 ? 1 : 32 / G;
+        const size_t ring_bytes = G >= 8 ? (size_t)kRing * block * 16 : 0;
+        const int cap_cx = (int)(slab_limit / 16 / (size_t)epw);      // larger states spill (or are refused below)
+        const int reg_blocks = std::max(1, 65536 / (168 * block));
+        auto rate = [&](int slab_cx) {
+            const size_t smem = (size_t)slab_cx * epw * 16 + ring_bytes + 1024;
+            const int blocks = (int)std::max<size_t>(1, std::min<size_t>({(size_t)reg_blocks, (size_t)32, (size_t)(228 * 1024) / smem}));
+            const double w = blocks * (block / 32.0);
+            return w / (w + 7.0);
+        };
+        std::vector<std::pair<int, double>> sw;     // (state, work), one entry per distinct state size, ascending
+        {
+            std::vector<std::pair<int, double>> all_sw;
+            for (long long r = 0; r < nc; r++) {
+                if (!info[r].valid) continue;
+                double w = 1.0;
+                int left = n;
+                for (int t = 0; t < kNumCodes; t++)
+                    for (int q = 1; q <= all[r][t]; q++) w *= (double)(left--) / q;
+                all_sw.push_back({std::min<int>(std::max<int>(16, info[r].state_cx), std::max(16, cap_cx)), w * steps[r]});
+            }
+            std::sort(all_sw.begin(), all_sw.end());
+            for (auto& x : all_sw) {
+                if (!sw.empty() && sw.back().first == x.first) sw.back().second += x.second;
+                else sw.push_back(x);
+            }
+        }
+        const int U = (int)sw.size();
+        for (int k = 0; k < kTiers; k++) tiers.slab_cx[k] = std::max(16, std::min(max_state, std::max(16, cap_cx)));
+        if (U > 0) {
+            std::vector<double> pre(U + 1, 0.0);
+            for (int i = 0; i < U; i++) pre[i + 1] = pre[i] + sw[i].second;
+            const double kInf = 1e300;
+            std::vector<std::vector<double>> best(kTiers + 1, std::vector<double>(U, kInf));
+            std::vector<std::vector<int>> from(kTiers + 1, std::vector<int>(U, -1));
+            for (int j = 0; j < U; j++) best[1][j] = pre[j + 1] / rate(sw[j].first);
+            for (int k = 2; k <= kTiers; k++)
+                for (int j = k - 1; j < U; j++) {
+                    const double rj = rate(sw[j].first);
+                    for (int i = k - 2; i < j; i++) {
+                        const double c = best[k - 1][i] + (pre[j + 1] - pre[i + 1]) / rj;
+                        if (c < best[k][j]) { best[k][j] = c; from[k][j] = i; }
+                    }
+                }
+            int kbest = 1;
+            for (int k = 2; k <= std::min(kTiers, U); k++)
+                if (best[k][U - 1] < best[kbest][U - 1] * (1.0 - 1e-3)) kbest = k;   // a tier must pay for its launch
+            int j = U - 1, slot = 0;
+            for (int k = kbest; k >= 1 && j >= 0; k--) {
+                tiers.slab_cx[slot++] = sw[j].first;
+                j = k > 1 ? from[k][j] : -1;
+            }
+            for (; slot < kTiers; slot++) tiers.slab_cx[slot] = tiers.slab_cx[slot - 1];   // unused tiers stay empty
+        }
+    }
     std::vector<int> tier_of(nc);
     for (long long r = 0; r < nc; r++) {
         int k = 0;
