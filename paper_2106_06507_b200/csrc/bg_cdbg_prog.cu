@@ -96,6 +96,7 @@ struct ProgParams {
     int slab_cx;               // complex doubles of state per event in the shared-memory slab
     double2* spill;            // SPILL kernels: global slab, spill_cx complex doubles per block
     int spill_cx;
+    int zero;                  // always 0 (see the op prefetch in the interpreter)
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -361,6 +362,9 @@ __device__ __forceinline__ double shfl_xor(double v, int d) { return __shfl_xor_
 __device__ __forceinline__ cx shfl_xor(cx v, int d) {
     return mk(__shfl_xor_sync(0xFFFFFFFFu, v.re, d), __shfl_xor_sync(0xFFFFFFFFu, v.im, d));
 }
+
+__device__ __forceinline__ int hi_word(cx v) { return __double2hiint(v.re); }
+__device__ __forceinline__ int hi_word(double v) { return __double2hiint(v); }
 
 __device__ __forceinline__ EventHeader ld_header(const char* h) {
     const uint4 v = __ldcg(reinterpret_cast<const uint4*>(h));   // streamed once: not through L1
@@ -633,7 +637,14 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                         }
                     }
                 }
-                if constexpr (!kUseRing) { r0 = r1; r1 = r2; }
+                if constexpr (!kUseRing) {
+                    // The op requested at the top of this step must not be touched before the step ends (the
+                    // compiler would otherwise park it right behind the load with moves that wait for it): its
+                    // first use is tied to the step's last arithmetic results through an always-zero mask.
+                    const unsigned late = (unsigned)(hi_word(acc[0]) ^ hi_word(amp)) & (unsigned)p.zero;
+                    r0 = r1;
+                    r1 = make_uint4(r2.x | late, r2.y | late, r2.z | late, r2.w | late);
+                }
             }
             if constexpr (kUseRing) asm volatile("cp.async.wait_group 0;" ::: "memory");
         }
@@ -1078,6 +1089,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.n = t->n; p.N = N; p.out = out;
     p.info = t->d_info; p.ops = t->d_ops; p.rec = rec; p.rec_bytes = rec_bytes; p.rec_gstride = 4;
     p.bounds = bounds;
+    p.zero = 0;
     p.spill = t->spill ? (double2*)((char*)scratch + prog_spill_offset(t, N)) : nullptr;
     p.spill_cx = t->max_state_cx;
     p.tier = 0;
@@ -1102,6 +1114,7 @@ cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, 
     p.n = t->n; p.N = N; p.out = out;
     p.info = t->d_info; p.ops = t->d_ops; p.rec = rec; p.rec_bytes = t->rec_bytes; p.rec_gstride = 12;
     p.bounds = bounds;
+    p.zero = 0;
     p.spill = t->spill ? (double2*)((char*)scratch + prog_spill_offset(t, N)) : nullptr;
     p.spill_cx = t->max_state_cx;
     p.tier = 0;
