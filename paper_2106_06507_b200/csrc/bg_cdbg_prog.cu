@@ -409,6 +409,10 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         const long long idx = first + (long long)blockIdx.x * EPW + q;
         if (idx < end) hnext = ld_header(p.rec + (size_t)idx * p.rec_bytes);
     }
+    // carried from one task to the next: the class info of the next event, requested at the first barrier of the
+    // current task (one load less in the chain header -> info -> ops -> inputs at the start of a task)
+    uint4 ci_next = make_uint4(0, 0, 0, 0);
+    bool ci_next_ok = false;
     for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
         const long long idx = first + task * EPW + q;
         const bool have = idx < end;
@@ -422,7 +426,9 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         }
         const long long e = h.event;
         const uint32_t cls = have ? h.cls : 0xFFFFFFFFu;
-        const uint4 ci = __ldg(reinterpret_cast<const uint4*>(p.info + (cls == 0xFFFFFFFFu ? 0 : cls)));
+        uint4 ci = ci_next;
+        if (!ci_next_ok) ci = __ldg(reinterpret_cast<const uint4*>(p.info + (cls == 0xFFFFFFFFu ? 0 : cls)));
+        ci_next_ok = false;
         const bool valid = cls != 0xFFFFFFFFu && ((ci.y >> 24) & 0xFF);
         const uint64_t perm = h.perm;
         const double* mrec = reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
@@ -465,7 +471,8 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     raw = ring[(s % kRing) * kBlock];
                 } else {
                     raw = r0;
-                    r2 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)(s + 2) * G));
+                    const ProgOp* src = ops + (size_t)(s + 2) * G;
+                    r2 = __ldg(reinterpret_cast<const uint4*>(src));
                 }
                 const int offA = raw.x & 0xFFFF, offB = raw.x >> 16;
                 const int offP1 = raw.y & 0xFFFF, offDst = raw.y >> 16;
@@ -634,6 +641,10 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                             // the next event's record (a few 128-byte lines) is pulled into L2 meanwhile
                             for (int k = g * 128; k < p.rec_bytes; k += G * 128)
                                 asm volatile("prefetch.global.L2 [%0];" ::"l"(p.rec + (size_t)idx_next * p.rec_bytes + k));
+                            if constexpr (kUseRing) {      // (G <= 4: measured neutral to slightly slower)
+                                ci_next = __ldg(reinterpret_cast<const uint4*>(p.info + hnext.cls));
+                                ci_next_ok = true;
+                            }
                         }
                     }
                 }
