@@ -426,12 +426,20 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         }
         const long long e = h.event;
         const uint32_t cls = have ? h.cls : 0xFFFFFFFFu;
+        const double* mrec = reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
+        // discrete states: the setup level gives gluon k to lane k % G, so the lane's first momentum is requested
+        // here, ahead of the dependent loads class info -> ops that the setup ops themselves wait for
+        const bool discrete = !kUseRing && p.rec_gstride == 4 && sizeof(T) == 16;   // (G >= 8: measured 1-2 % slower)
+        double pk[4] = {0.0, 0.0, 0.0, 0.0};
+        if (discrete && g < n) {
+#pragma unroll
+            for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + g * 4 + c);
+        }
         uint4 ci = ci_next;
         if (!ci_next_ok) ci = __ldg(reinterpret_cast<const uint4*>(p.info + (cls == 0xFFFFFFFFu ? 0 : cls)));
         ci_next_ok = false;
         const bool valid = cls != 0xFFFFFFFFu && ((ci.y >> 24) & 0xFF);
         const uint64_t perm = h.perm;
-        const double* mrec = reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
         const ProgOp* ops = p.ops + ci.x + g;
         const int total = valid ? (int)ci.z : 0;
         bool prefetched = false;
@@ -448,21 +456,67 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         // registers are held across the latency and nothing else reads these slots); the table ends with spare rows.
         // With few lanes per event (G <= 4) the program of a class is small and stays in L1: plain loads, two steps
         // ahead, are cheaper there.
+        auto first_barrier_done = [&]() {
+            prefetched = true;
+            if (hnext.cls != 0xFFFFFFFFu) {
+                // the next event's record (a few 128-byte lines) is pulled into L2 meanwhile
+                for (int k = g * 128; k < p.rec_bytes; k += G * 128)
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(p.rec + (size_t)idx_next * p.rec_bytes + k));
+                if constexpr (kUseRing) {      // (G <= 4: measured neutral to slightly slower)
+                    ci_next = __ldg(reinterpret_cast<const uint4*>(p.info + hnext.cls));
+                    ci_next_ok = true;
+                }
+            }
+        };
+        const int s0 = (discrete && total > 0) ? (n + G - 1) / G : 0;     // steps of the setup level done up front
         uint4 r0 = make_uint4(0, 0, 0, 0), r1 = r0;
         if constexpr (kUseRing) {
             if (total > 0) {
 #pragma unroll
                 for (int i = 0; i < kRing - 1; i++) {
-                    cp_async16(ring + i * kBlock, ops + (size_t)i * G);
+                    cp_async16(ring + ((s0 + i) % kRing) * kBlock, ops + (size_t)(s0 + i) * G);
                     asm volatile("cp.async.commit_group;" ::: "memory");
                 }
             }
         } else {
-            r0 = __ldg(reinterpret_cast<const uint4*>(ops));
-            r1 = __ldg(reinterpret_cast<const uint4*>(ops + G));
+            r0 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s0 * G));
+            r1 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)(s0 + 1) * G));
+        }
+        if constexpr (sizeof(T) == 16) {
+            // setup level (discrete states): external currents eps(p_k, lambda_k) and momenta, Eq. 20 / g1-g5
+            int k = g;
+            for (int s = 0; s < s0; s++) {
+                const uint4 raw = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s * G));
+                const int kn = k + G;
+                double pn[4] = {0.0, 0.0, 0.0, 0.0};
+                if (kn < n) {
+#pragma unroll
+                    for (int c = 0; c < 4; c++) pn[c] = __ldcg(mrec + kn * 4 + c);
+                }
+                if ((raw.z >> 16) & OPF_EXT) {
+                    const int kk = (int)raw.w;
+                    if (kk != k) {      // another dealing of the gluons than k % G: fetch what the op names
+#pragma unroll
+                        for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + kk * 4 + c);
+                    }
+                    cx eps[4];
+                    polarisation(pk, ((perm >> (48 + kk)) & 1) ? 1 : -1, eps);
+                    const int offDst = raw.y >> 16, offPt = raw.z & 0xFFFF;
+#pragma unroll
+                    for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
+                    if (offPt != 0xFFFF) st_.stP(offPt, pk);
+                }
+#pragma unroll
+                for (int c = 0; c < 4; c++) pk[c] = pn[c];
+                k = kn;
+            }
+            if (s0 > 0) {
+                if constexpr (G > 32) __syncthreads(); else __syncwarp(evmask);
+                first_barrier_done();
+            }
         }
         {
-            for (int s = 0; s < total; s++) {
+            for (int s = s0; s < total; s++) {
                 uint4 raw, r2 = r1;
                 if constexpr (kUseRing) {
                     cp_async16(ring + ((s + kRing - 1) % kRing) * kBlock, ops + (size_t)(s + kRing - 1) * G);
@@ -635,18 +689,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                 if (flags & OPF_SYNC) {
                     // end of a level: the currents just written become visible to the lanes of the event
                     if constexpr (G > 32) __syncthreads(); else __syncwarp(evmask);
-                    if (!prefetched) {
-                        prefetched = true;
-                        if (hnext.cls != 0xFFFFFFFFu) {
-                            // the next event's record (a few 128-byte lines) is pulled into L2 meanwhile
-                            for (int k = g * 128; k < p.rec_bytes; k += G * 128)
-                                asm volatile("prefetch.global.L2 [%0];" ::"l"(p.rec + (size_t)idx_next * p.rec_bytes + k));
-                            if constexpr (kUseRing) {      // (G <= 4: measured neutral to slightly slower)
-                                ci_next = __ldg(reinterpret_cast<const uint4*>(p.info + hnext.cls));
-                                ci_next_ok = true;
-                            }
-                        }
-                    }
+                    if (!prefetched) first_barrier_done();
                 }
                 if constexpr (!kUseRing) {
                     // The op requested at the top of this step must not be touched before the step ends (the
