@@ -284,6 +284,63 @@ cdbg_scatter_kernel(int n, long long N, long long num_classes, const uint32_t* _
     }
 }
 
+// 3b. the same with the records of a warp staged in shared memory: a thread writing its own 32(n+1)-byte record
+// touches 32 different lines per store instruction; here each warp builds its 32 records in shared memory
+// (record stride padded by 16 bytes: conflict-free) and copies them out with consecutive lanes on consecutive
+// 16-byte pieces, so a store instruction covers four to five lines.  Blocks of kStageThreads threads; used when
+// histogram + staging fit in shared memory for at least two blocks per SM (n <= 7).
+constexpr int kStageThreads = 256, kStageEvents = kStageThreads * kPrePer;
+__global__ void __launch_bounds__(kStageThreads)
+cdbg_scatter_staged_kernel(int n, long long N, long long num_classes, const uint32_t* __restrict__ cls,
+                           const uint64_t* __restrict__ perm, const uint32_t* __restrict__ sortkey,
+                           const double* __restrict__ mom, const signed char* __restrict__ hel,
+                           uint32_t* __restrict__ cursor, char* __restrict__ rec, int rec_bytes) {
+    extern __shared__ uint32_t sh_hist[];
+    const int nbins = (int)num_classes + 1;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int rs = rec_bytes + 16, pieces = rec_bytes / 16;
+    char* const stage = reinterpret_cast<char*>(sh_hist + ((nbins + 3) & ~3)) + (size_t)warp * (32 * rs + 256);
+    unsigned long long* const dstp = reinterpret_cast<unsigned long long*>(stage + 32 * rs);
+    uint32_t key[kPrePer], rank[kPrePer];
+    for (int i = threadIdx.x; i < nbins; i += kStageThreads) sh_hist[i] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < kPrePer; j++) {
+        const long long e = (long long)blockIdx.x * kStageEvents + j * kStageThreads + threadIdx.x;
+        key[j] = 0xFFFFFFFFu;
+        rank[j] = 0;
+        if (e < N) {
+            const uint32_t c = cls[e];
+            key[j] = c == 0xFFFFFFFFu ? (uint32_t)num_classes : sortkey[c];
+            rank[j] = atomicAdd(&sh_hist[key[j]], 1u);
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < nbins; i += kStageThreads) {
+        const uint32_t c = sh_hist[i];
+        if (c) sh_hist[i] = atomicAdd(&cursor[i], c);
+    }
+    __syncthreads();
+    for (int j = 0; j < kPrePer; j++) {
+        const long long e = (long long)blockIdx.x * kStageEvents + j * kStageThreads + threadIdx.x;
+        char* dst = nullptr;
+        if (key[j] != 0xFFFFFFFFu) {
+            dst = rec + (size_t)(sh_hist[key[j]] + rank[j]) * rec_bytes;
+            char* mine = stage + lane * rs;
+            *reinterpret_cast<uint4*>(mine + 16) = make_uint4(0, 0, 0, 0);      // second half of the header block
+            write_record(n, N, e, cls[e], perm[e], mom, hel, mine);
+        }
+        dstp[lane] = reinterpret_cast<unsigned long long>(dst);
+        __syncwarp();
+        for (int i = lane; i < 32 * pieces; i += 32) {
+            const int r = i / pieces, q = i - r * pieces;
+            char* d = reinterpret_cast<char*>(dstp[r]);
+            if (d) *reinterpret_cast<uint4*>(d + q * 16) = *reinterpret_cast<const uint4*>(stage + r * rs + q * 16);
+        }
+        __syncwarp();
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // 4. interpreter
 // ---------------------------------------------------------------------------------------------------------
@@ -1135,13 +1192,22 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         if (configured_device != device) {
             cudaFuncSetAttribute(cdbg_classify_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
             cudaFuncSetAttribute(cdbg_scatter_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+            cudaFuncSetAttribute(cdbg_scatter_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
             configured_device = device;
         }
         cdbg_classify_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
                                                                       t->d_sortkey, cls, perm, hist);
         cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins, t->tiers, bounds, (uint32_t)N);
-        cdbg_scatter_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, cls, perm, t->d_sortkey, mom, hel,
-                                                                     hist, rec, rec_bytes);
+        const size_t stage_smem = (((size_t)nbins + 3) & ~(size_t)3) * sizeof(uint32_t) +
+                                  (size_t)(kStageThreads / 32) * (32 * (rec_bytes + 16) + 256);
+        if (stage_smem <= 100 * 1024) {
+            const unsigned sb = (unsigned)((N + kStageEvents - 1) / kStageEvents);
+            cdbg_scatter_staged_kernel<<<sb, kStageThreads, stage_smem, s>>>(t->n, N, t->num_classes, cls, perm, t->d_sortkey,
+                                                                            mom, hel, hist, rec, rec_bytes);
+        } else {
+            cdbg_scatter_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, cls, perm, t->d_sortkey, mom,
+                                                                         hel, hist, rec, rec_bytes);
+        }
     } else {
         cdbg_classify_kernel<false><<<eb, kPreThreads, 0, s>>>(t->n, N, t->num_classes, col, t->d_info, t->d_sortkey,
                                                                cls, perm, hist);
