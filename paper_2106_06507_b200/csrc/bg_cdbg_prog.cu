@@ -122,24 +122,25 @@ cdbg_classify_kernel(int n, long long N, long long num_classes, const signed cha
     for (int j = 0; j < kPrePer; j++) {
         const long long e = (long long)blockIdx.x * kPreEvents + j * kPreThreads + threadIdx.x;
         if (e >= N) break;
-        int code[kMaxN], cnt[kNumCodes];
+        // colour codes 3(i-1)+(j-1) of the n gluons, one nibble each (registers; n is a run-time value)
+        int cnt[kNumCodes];
 #pragma unroll
         for (int c = 0; c < kNumCodes; c++) cnt[c] = 0;
         bool ok = true;
+        uint64_t cw = 0;
         for (int k = 0; k < n; k++) {
             const int i = col[(size_t)(2 * k) * N + e] - 1, jj = col[(size_t)(2 * k + 1) * N + e] - 1;
             ok = ok && i >= 0 && i < 3 && jj >= 0 && jj < 3;
-            code[k] = ok ? 3 * i + jj : 0;
+            const int code = ok ? 3 * i + jj : 0;
+            cw |= (uint64_t)code << (4 * k);
+#pragma unroll
+            for (int c = 0; c < kNumCodes; c++) cnt[c] += code == c;
         }
         if (!ok) {
             cls[e] = 0xFFFFFFFFu;
             perm[e] = 0;
             atomicAdd(&h[num_classes], 1u);
             continue;
-        }
-        for (int k = 0; k < n; k++) {
-#pragma unroll
-            for (int c = 0; c < kNumCodes; c++) cnt[c] += code[k] == c;
         }
         unsigned rank = 0;
         int r = n;
@@ -151,13 +152,25 @@ cdbg_classify_kernel(int n, long long N, long long num_classes, const signed cha
         const ClassInfo ci = info[rank];
         uint64_t pm = 0;
         if (ci.valid) {
+            // canonical order: codes ascending, original order inside a code, the last gluon with the closure code
+            // moved to the end.  start[c] (a nibble per code) = canonical position of the next gluon with code c.
+            const int closure = ci.closure_code;
             int lastk = 0;
             for (int k = 0; k < n; k++)
-                if (code[k] == ci.closure_code) lastk = k;
-            int pos = 0;
-            for (int c = 0; c < kNumCodes; c++)
-                for (int k = 0; k < n; k++)
-                    if (code[k] == c && k != lastk) pm |= (uint64_t)k << (4 * pos++);
+                if ((int)((cw >> (4 * k)) & 0xF) == closure) lastk = k;
+            uint64_t start = 0;
+            int before = 0;
+#pragma unroll
+            for (int c = 0; c < kNumCodes; c++) {
+                start |= (uint64_t)before << (4 * c);
+                before += cnt[c] - (c == closure ? 1 : 0);
+            }
+            for (int k = 0; k < n; k++) {
+                if (k == lastk) continue;
+                const int sh = 4 * (int)((cw >> (4 * k)) & 0xF);
+                pm |= (uint64_t)k << (4 * (int)((start >> sh) & 0xF));
+                start += 1ull << sh;
+            }
             pm |= (uint64_t)lastk << (4 * (n - 1));
         }
         cls[e] = rank;
