@@ -175,12 +175,15 @@ def run_reference(args):
     S = cpu_sample_size(args, n, N)
     S = max(64, S // max(1, args.steps + args.warmup) * 2) if args.steps + args.warmup > 4 else S
     ev = make_events(args, n, S, 0)
-    cores = oracle.max_threads()
+    # torchrun exports OMP_NUM_THREADS=1 to every rank; here rank 0 works alone, so it takes the host cores it may
+    # run on (the same count the N=1 launch gets from OpenMP's default)
+    threads = len(os.sched_getaffinity(0)) if int(os.environ.get("WORLD_SIZE", "1")) > 1 else 0
+    cores = threads or oracle.max_threads()
     for _ in range(max(1, min(args.warmup, 3))):
-        oracle_eval(args, ev.head(max(64, S // 8)))
+        oracle_eval(args, ev.head(max(64, S // 8)), threads)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle_eval(args, ev)
+        oracle_eval(args, ev, threads)
     dt = time.perf_counter() - t0
     value = S * args.steps / dt
     line = {"impl": "reference", "metric": "n-gluon |M|^2 events/sec", "value": value, "unit": "events/s",
