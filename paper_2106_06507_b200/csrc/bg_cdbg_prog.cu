@@ -78,6 +78,10 @@ struct ProgTable {
     uint32_t* d_sortkey;      // class id -> position in the order the events are grouped by
     ProgOp* d_ops;
     size_t ops_bytes;
+    // small batches: the tier launches run side by side on these streams (fork / join around the caller's stream)
+    cudaStream_t aux[kTiers - 1];
+    cudaEvent_t fork_ev, join_ev[kTiers - 1];
+    bool has_streams;
 };
 
 __constant__ unsigned c_mscount[kMaxN + 1][kNumCodes];   // multiset_count(r, t) for r <= 12, t <= 8
@@ -1011,6 +1015,15 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
         prog_table_destroy(t);
         return BG_ENOMEM;
     }
+    {   // side streams of the tier launches (small batches, see cdbg_prog_launch); without them: one stream
+        bool sok = cudaEventCreateWithFlags(&t->fork_ev, cudaEventDisableTiming) == cudaSuccess;
+        int made = 0;
+        for (; sok && made < kTiers - 1; made++)
+            sok = cudaStreamCreateWithFlags(&t->aux[made], cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaEventCreateWithFlags(&t->join_ev[made], cudaEventDisableTiming) == cudaSuccess;
+        t->has_streams = sok;
+        if (!sok) cudaGetLastError();
+    }
     *out = t;
     return BG_OK;
 }
@@ -1100,6 +1113,10 @@ cdbg_pack_continuous_kernel(int n, long long N, const double* __restrict__ mom, 
 
 void prog_table_destroy(ProgTable* t) {
     if (!t) return;
+    if (t->has_streams) {
+        for (int i = 0; i < kTiers - 1; i++) { cudaStreamDestroy(t->aux[i]); cudaEventDestroy(t->join_ev[i]); }
+        cudaEventDestroy(t->fork_ev);
+    }
     if (t->d_info) cudaFree(t->d_info);
     if (t->d_sortkey) cudaFree(t->d_sortkey);
     if (t->d_ops) cudaFree(t->d_ops);
@@ -1120,7 +1137,7 @@ size_t prog_scratch_bytes(const ProgTable* t, long long N) {
 }
 
 template <int G, bool SPILL, class S = cx>
-static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched) {
+static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched, bool conc) {
     constexpr int EPW = G >= 32 ? 1 : 32 / G, BLOCK = G > 32 ? G : 32;
     constexpr size_t ELEM = sizeof(typename StateElem<S>::T);
     static int configured_device = -1;   // the attribute is per device
@@ -1133,52 +1150,79 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         configured_device = device;
     }
     const long long max_tasks = (p.N + EPW - 1) / EPW + kTiers;
+    unsigned blocks[kTiers];
+    size_t smem[kTiers];
+    long long resident = 0;
+    int nlaunch = 0;
     for (int k = 0; k < kTiers; k++) {
+        blocks[k] = 0;
         if (t->tiers.first_key[k] == t->tiers.first_key[k + 1] && k + 1 < kTiers) continue;   // no class in this tier
+        const size_t ring_bytes = G >= 8 ? (size_t)kRing * BLOCK * 16 : 0;
+        smem[k] = ((size_t)EPW * t->tiers.slab_cx[k] * ELEM + 15) / 16 * 16 + ring_bytes;
+        if (smem[k] > kMaxSlabBytes + ring_bytes) return cudaErrorInvalidValue;
+        // resident blocks per SM: shared memory (1 KB reserved per block), and 65536 / (160 x BLOCK) registers
+        int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * BLOCK), (228 * 1024) / (smem[k] + 1024)));
+        if (SPILL) per_sm = std::min(per_sm, t->spill_blocks_per_sm);   // one global slab per resident block
+        blocks[k] = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
+        resident += (long long)sm_count * per_sm;
+        nlaunch++;
+    }
+    // Small batches: when the tiers together hold fewer than two tasks per resident block, each launch is mostly
+    // ramp-up and tail, so the tiers run side by side (fork / join around the caller's stream).  Measured at
+    // n = 6: 2^16 events +22 %, 2^18 neutral, 2^20 -5 %; n >= 7: slower at every size.
+    // (spill slabs are indexed by block: one launch at a time)
+    conc = conc && G <= 4 && !SPILL && t->has_streams && nlaunch > 1 && max_tasks <= 2 * resident;
+    if (conc && cudaEventRecord(t->fork_ev, s) != cudaSuccess) return cudaGetLastError();
+    int side = 0;                                 // launches sent to the side streams so far
+    bool first = true;
+    for (int k = 0; k < kTiers; k++) {
+        if (!blocks[k]) continue;
         p.tier = k;
         p.slab_cx = t->tiers.slab_cx[k];
-        const size_t ring_bytes = G >= 8 ? (size_t)kRing * BLOCK * 16 : 0;
-        const size_t smem = ((size_t)EPW * p.slab_cx * ELEM + 15) / 16 * 16 + ring_bytes;
-        if (smem > kMaxSlabBytes + ring_bytes) return cudaErrorInvalidValue;
-        // resident blocks per SM: shared memory (1 KB reserved per block), and 65536 / (160 x BLOCK) registers
-        int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * BLOCK), (228 * 1024) / (smem + 1024)));
-        if (SPILL) per_sm = std::min(per_sm, t->spill_blocks_per_sm);   // one global slab per resident block
-        const unsigned blocks = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
-        cdbg_prog_kernel<G, SPILL, S><<<blocks, BLOCK, smem, s>>>(p);
+        cudaStream_t ls = s;
+        if (conc && !first) {
+            ls = t->aux[side];
+            cudaStreamWaitEvent(ls, t->fork_ev, 0);
+        }
+        cdbg_prog_kernel<G, SPILL, S><<<blocks[k], BLOCK, smem[k], ls>>>(p);
+        if (conc && !first) cudaEventRecord(t->join_ev[side++], ls);
+        first = false;
         ++*launched;
     }
+    for (int i = 0; i < side; i++) cudaStreamWaitEvent(s, t->join_ev[i], 0);
     return cudaGetLastError();
 }
 
-static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches) {
+static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches,
+                                   bool conc = false) {
     cudaError_t err;
     if (t->real) {   // continuous states with real polarisations: all-real arithmetic
         switch (t->G) {
-            case 32: return launch_interp<32, false, double>(s, t, sm_count, p, launches);
-            case 64: return launch_interp<64, false, double>(s, t, sm_count, p, launches);
+            case 32: return launch_interp<32, false, double>(s, t, sm_count, p, launches, conc);
+            case 64: return launch_interp<64, false, double>(s, t, sm_count, p, launches, conc);
             case 128:
-                return t->spill ? launch_interp<128, true, double>(s, t, sm_count, p, launches)
-                                : launch_interp<128, false, double>(s, t, sm_count, p, launches);
+                return t->spill ? launch_interp<128, true, double>(s, t, sm_count, p, launches, conc)
+                                : launch_interp<128, false, double>(s, t, sm_count, p, launches, conc);
             default:
-                return t->spill ? launch_interp<256, true, double>(s, t, sm_count, p, launches)
-                                : launch_interp<256, false, double>(s, t, sm_count, p, launches);
+                return t->spill ? launch_interp<256, true, double>(s, t, sm_count, p, launches, conc)
+                                : launch_interp<256, false, double>(s, t, sm_count, p, launches, conc);
         }
     }
     switch (t->G) {
-        case 1: err = launch_interp<1, false>(s, t, sm_count, p, launches); break;
-        case 2: err = launch_interp<2, false>(s, t, sm_count, p, launches); break;
-        case 4: err = launch_interp<4, false>(s, t, sm_count, p, launches); break;
-        case 8: err = launch_interp<8, false>(s, t, sm_count, p, launches); break;
-        case 16: err = launch_interp<16, false>(s, t, sm_count, p, launches); break;
-        case 32: err = launch_interp<32, false>(s, t, sm_count, p, launches); break;
-        case 64: err = launch_interp<64, false>(s, t, sm_count, p, launches); break;
+        case 1: err = launch_interp<1, false>(s, t, sm_count, p, launches, conc); break;
+        case 2: err = launch_interp<2, false>(s, t, sm_count, p, launches, conc); break;
+        case 4: err = launch_interp<4, false>(s, t, sm_count, p, launches, conc); break;
+        case 8: err = launch_interp<8, false>(s, t, sm_count, p, launches, conc); break;
+        case 16: err = launch_interp<16, false>(s, t, sm_count, p, launches, conc); break;
+        case 32: err = launch_interp<32, false>(s, t, sm_count, p, launches, conc); break;
+        case 64: err = launch_interp<64, false>(s, t, sm_count, p, launches, conc); break;
         case 128:
-            err = t->spill ? launch_interp<128, true>(s, t, sm_count, p, launches)
-                           : launch_interp<128, false>(s, t, sm_count, p, launches);
+            err = t->spill ? launch_interp<128, true>(s, t, sm_count, p, launches, conc)
+                           : launch_interp<128, false>(s, t, sm_count, p, launches, conc);
             break;
         default:
-            err = t->spill ? launch_interp<256, true>(s, t, sm_count, p, launches)
-                           : launch_interp<256, false>(s, t, sm_count, p, launches);
+            err = t->spill ? launch_interp<256, true>(s, t, sm_count, p, launches, conc)
+                           : launch_interp<256, false>(s, t, sm_count, p, launches, conc);
             break;
     }
     return err;
@@ -1240,7 +1284,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.slab_cx = t->max_state_cx;
     *launches = 3;
     if (ev0) cudaEventRecord(ev0, s);
-    err = dispatch_interp(s, t, sm_count, p, launches);
+    err = dispatch_interp(s, t, sm_count, p, launches, true);
     if (ev1) cudaEventRecord(ev1, s);
     return err;
 }
@@ -1265,7 +1309,7 @@ cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, 
     p.slab_cx = t->max_state_cx;
     *launches = 1;
     if (ev0) cudaEventRecord(ev0, s);
-    err = dispatch_interp(s, t, sm_count, p, launches);
+    err = dispatch_interp(s, t, sm_count, p, launches, false);
     if (ev1) cudaEventRecord(ev1, s);
     return err;
 }
