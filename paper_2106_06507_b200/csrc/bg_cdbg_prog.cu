@@ -82,6 +82,7 @@ struct ProgTable {
     cudaStream_t aux[kTiers - 1];
     cudaEvent_t fork_ev, join_ev[kTiers - 1];
     bool has_streams;
+    uint32_t* d_small;        // [2 (num_classes + 1) + 1] zeroed histogram | cursors | ticket of the fused-scan prepass
 };
 
 __constant__ unsigned c_mscount[kMaxN + 1][kNumCodes];   // multiset_count(r, t) for r <= 12, t <= 8
@@ -307,16 +308,55 @@ cdbg_scatter_kernel(int n, long long N, long long num_classes, const uint32_t* _
 // 16-byte pieces, so a store instruction covers four to five lines.  Blocks of kStageThreads threads; used when
 // histogram + staging fit in shared memory for at least two blocks per SM (n <= 7).
 constexpr int kStageThreads = 256, kStageEvents = kStageThreads * kPrePer;
+constexpr int kFusedScanBins = 4096;            // largest histogram the scatter blocks scan for themselves
+constexpr long long kFusedScanEvents = 1 << 18; // ... and largest batch (beyond it the scan launch is cheaper)
+// FUSED (small batches, where a step is a handful of short launches): the exclusive scan of the class histogram
+// is done here, by every block for itself in shared memory (a few thousand bins), instead of by a launch of its
+// own; `counts` is then the finished histogram of the classify kernel and `cursor` a zeroed array of running
+// offsets inside the classes.  Both live in a small buffer of the table that the last block to finish clears
+// for the next call, so no memset launch is needed either.
+struct FusedScan {
+    const uint32_t* counts;   // [nbins] class histogram (classify kernel)
+    uint32_t* ticket;         // blocks finished so far
+    uint32_t* bounds;         // [kTiers + 1] tier starts (written by block 0)
+    uint32_t N;
+    TierInfo tiers;
+};
+template <bool FUSED>
 __global__ void __launch_bounds__(kStageThreads)
 cdbg_scatter_staged_kernel(int n, long long N, long long num_classes, const uint32_t* __restrict__ cls,
                            const uint64_t* __restrict__ perm, const uint32_t* __restrict__ sortkey,
                            const double* __restrict__ mom, const signed char* __restrict__ hel,
-                           uint32_t* __restrict__ cursor, char* __restrict__ rec, int rec_bytes) {
+                           uint32_t* __restrict__ cursor, char* __restrict__ rec, int rec_bytes, const FusedScan fs) {
     extern __shared__ uint32_t sh_hist[];
     const int nbins = (int)num_classes + 1;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int rs = rec_bytes + 16, pieces = rec_bytes / 16;
-    char* const stage = reinterpret_cast<char*>(sh_hist + ((nbins + 3) & ~3)) + (size_t)warp * (32 * rs + 256);
+    const int hist_words = (nbins + 3) & ~3;
+    uint32_t* const sh_start = sh_hist + hist_words;        // FUSED: exclusive scan of the global histogram
+    char* const stage = reinterpret_cast<char*>(sh_hist + (FUSED ? 2 : 1) * hist_words) + (size_t)warp * (32 * rs + 256);
+    if (FUSED) {
+        __shared__ uint32_t warp_tot[kStageThreads / 32];
+        const int per = (nbins + kStageThreads - 1) / kStageThreads;     // contiguous bins per thread
+        const int b0 = threadIdx.x * per, b1 = min(nbins, b0 + per);
+        uint32_t sum = 0;
+        for (int i = b0; i < b1; i++) sum += fs.counts[i];
+        uint32_t x = sum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xFFFFFFFFu, x, d);
+            if (lane >= d) x += y;
+        }
+        if (lane == 31) warp_tot[warp] = x;
+        __syncthreads();
+        uint32_t before = x - sum;
+        for (int w = 0; w < warp; w++) before += warp_tot[w];
+        for (int i = b0; i < b1; i++) {
+            sh_start[i] = before;
+            before += fs.counts[i];
+        }
+        // (the barrier below, before the first use of sh_start, also orders these writes)
+    }
     unsigned long long* const dstp = reinterpret_cast<unsigned long long*>(stage + 32 * rs);
     uint32_t key[kPrePer], rank[kPrePer];
     for (int i = threadIdx.x; i < nbins; i += kStageThreads) sh_hist[i] = 0;
@@ -335,8 +375,10 @@ cdbg_scatter_staged_kernel(int n, long long N, long long num_classes, const uint
     __syncthreads();
     for (int i = threadIdx.x; i < nbins; i += kStageThreads) {
         const uint32_t c = sh_hist[i];
-        if (c) sh_hist[i] = atomicAdd(&cursor[i], c);
+        if (c) sh_hist[i] = atomicAdd(&cursor[i], c) + (FUSED ? sh_start[i] : 0u);
     }
+    if (FUSED && blockIdx.x == 0 && threadIdx.x <= kTiers)
+        fs.bounds[threadIdx.x] = threadIdx.x == kTiers ? fs.N : sh_start[fs.tiers.first_key[threadIdx.x]];
     __syncthreads();
     for (int j = 0; j < kPrePer; j++) {
         const long long e = (long long)blockIdx.x * kStageEvents + j * kStageThreads + threadIdx.x;
@@ -355,6 +397,21 @@ cdbg_scatter_staged_kernel(int n, long long N, long long num_classes, const uint
             if (d) *reinterpret_cast<uint4*>(d + q * 16) = *reinterpret_cast<const uint4*>(stage + r * rs + q * 16);
         }
         __syncwarp();
+    }
+    if (FUSED) {
+        // the last block to get here leaves histogram, cursors and ticket zeroed for the next call
+        __shared__ bool last;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence();
+            last = atomicAdd(fs.ticket, 1u) == gridDim.x - 1;
+        }
+        __syncthreads();
+        if (last) {
+            uint32_t* counts = const_cast<uint32_t*>(fs.counts);
+            for (int i = threadIdx.x; i < nbins; i += kStageThreads) { counts[i] = 0; cursor[i] = 0; }
+            if (threadIdx.x == 0) *fs.ticket = 0;
+        }
     }
 }
 
@@ -1015,6 +1072,14 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
         prog_table_destroy(t);
         return BG_ENOMEM;
     }
+    if (nc + 1 <= kFusedScanBins) {   // fused-scan prepass of small batches (optional: without it, the scan launch)
+        const size_t bytes = sizeof(uint32_t) * (2 * ((size_t)nc + 1) + 1);
+        if (cudaMalloc(&t->d_small, bytes) != cudaSuccess || cudaMemset(t->d_small, 0, bytes) != cudaSuccess) {
+            cudaGetLastError();
+            if (t->d_small) cudaFree(t->d_small);
+            t->d_small = nullptr;
+        }
+    }
     {   // side streams of the tier launches (small batches, see cdbg_prog_launch); without them: one stream
         bool sok = cudaEventCreateWithFlags(&t->fork_ev, cudaEventDisableTiming) == cudaSuccess;
         int made = 0;
@@ -1113,6 +1178,7 @@ cdbg_pack_continuous_kernel(int n, long long N, const double* __restrict__ mom, 
 
 void prog_table_destroy(ProgTable* t) {
     if (!t) return;
+    if (t->d_small) cudaFree(t->d_small);
     if (t->has_streams) {
         for (int i = 0; i < kTiers - 1; i++) { cudaStreamDestroy(t->aux[i]); cudaEventDestroy(t->join_ev[i]); }
         cudaEventDestroy(t->fork_ev);
@@ -1238,18 +1304,38 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     uint32_t* hist = cls + N;
     uint32_t* bounds = hist + ((size_t)t->num_classes + 1);
     const int nbins = (int)t->num_classes + 1;
-    cudaError_t err = cudaMemsetAsync(hist, 0, sizeof(uint32_t) * nbins, s);
-    if (err != cudaSuccess) return err;
+    cudaError_t err = cudaSuccess;
     const unsigned eb = (unsigned)((N + kPreEvents - 1) / kPreEvents);
     const size_t hist_smem = sizeof(uint32_t) * nbins;
-    if (hist_smem <= 160 * 1024) {
+    const size_t stage_bytes = (size_t)(kStageThreads / 32) * (32 * (rec_bytes + 16) + 256);
+    const size_t hist_words = ((size_t)nbins + 3) & ~(size_t)3;
+    const bool fused = t->d_small && N <= kFusedScanEvents && 2 * hist_words * sizeof(uint32_t) + stage_bytes <= 100 * 1024;
+    if (!fused && (err = cudaMemsetAsync(hist, 0, sizeof(uint32_t) * nbins, s)) != cudaSuccess) return err;
+    if (fused) {
+        static int configured_device = -1;
+        int device = 0;
+        cudaGetDevice(&device);
+        if (configured_device != device) {
+            cudaFuncSetAttribute(cdbg_classify_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+            cudaFuncSetAttribute(cdbg_scatter_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+            configured_device = device;
+        }
+        uint32_t* counts = t->d_small;
+        FusedScan fs;
+        fs.counts = counts; fs.ticket = counts + 2 * nbins; fs.bounds = bounds; fs.N = (uint32_t)N; fs.tiers = t->tiers;
+        cdbg_classify_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
+                                                                      t->d_sortkey, cls, perm, counts);
+        const unsigned sb = (unsigned)((N + kStageEvents - 1) / kStageEvents);
+        cdbg_scatter_staged_kernel<true><<<sb, kStageThreads, 2 * hist_words * sizeof(uint32_t) + stage_bytes, s>>>(
+            t->n, N, t->num_classes, cls, perm, t->d_sortkey, mom, hel, counts + nbins, rec, rec_bytes, fs);
+    } else if (hist_smem <= 160 * 1024) {
         static int configured_device = -1;
         int device = 0;
         cudaGetDevice(&device);
         if (configured_device != device) {
             cudaFuncSetAttribute(cdbg_classify_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
             cudaFuncSetAttribute(cdbg_scatter_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
-            cudaFuncSetAttribute(cdbg_scatter_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+            cudaFuncSetAttribute(cdbg_scatter_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
             configured_device = device;
         }
         cdbg_classify_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
@@ -1259,8 +1345,8 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
                                   (size_t)(kStageThreads / 32) * (32 * (rec_bytes + 16) + 256);
         if (stage_smem <= 100 * 1024) {
             const unsigned sb = (unsigned)((N + kStageEvents - 1) / kStageEvents);
-            cdbg_scatter_staged_kernel<<<sb, kStageThreads, stage_smem, s>>>(t->n, N, t->num_classes, cls, perm, t->d_sortkey,
-                                                                            mom, hel, hist, rec, rec_bytes);
+            cdbg_scatter_staged_kernel<false><<<sb, kStageThreads, stage_smem, s>>>(t->n, N, t->num_classes, cls, perm, t->d_sortkey,
+                                                                                   mom, hel, hist, rec, rec_bytes, FusedScan());
         } else {
             cdbg_scatter_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, cls, perm, t->d_sortkey, mom,
                                                                          hel, hist, rec, rec_bytes);
@@ -1282,7 +1368,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.spill_cx = t->max_state_cx;
     p.tier = 0;
     p.slab_cx = t->max_state_cx;
-    *launches = 3;
+    *launches = fused ? 2 : 3;
     if (ev0) cudaEventRecord(ev0, s);
     err = dispatch_interp(s, t, sm_count, p, launches, true);
     if (ev1) cudaEventRecord(ev1, s);
