@@ -193,6 +193,7 @@ int bg_init(bg_ctx** out, int n, int mode) {
     if ((mode & BG_REC_COBG) && mode != BG_COMC_GIVEN && bg::cobg_shared_supported(n)) {
         const int rc = bg::cobg_table_create(n, &c->cobg);
         if (rc != BG_OK) { cudaFree(c->dC); std::free(c->hC); delete c; return rc; }
+        if (c->hC) bg::cobg_table_set_colour(c->cobg, c->hC);   // optional compressed form; the plain one stays valid
     }
     if ((mode == BG_CDBG_GIVEN && n <= kProgMaxN) || mode == BG_CDBG_CONTINUOUS || mode == BG_COMC_GIVEN) {
         const int rc = make_prog_table(c, 0, 0, &c->prog);

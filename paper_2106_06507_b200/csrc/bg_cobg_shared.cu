@@ -27,6 +27,7 @@
 namespace bg {
 
 constexpr int kCobgMaxM = 6;   // n - 1 <= 6: n = 4..7
+constexpr int kCobgMaxVals = 32;   // distinct entries of the colour matrix held in shared memory (16 at n = 7)
 
 struct CobgTable {
     int n, np, nslots;
@@ -34,6 +35,9 @@ struct CobgTable {
     uint16_t* d_slot;                 // [np][m][m] slot of range (i..j) of ordering sigma; 0xFFFF if longer than n-3
     uint8_t* d_ord;                   // [np][m] gluon at position i of (1, sigma)  (0-based labels, position 0 = gluon 0)
     uint32_t* d_lower;                // representatives of the shared sequences: sigma << 8 | i << 4 | j
+    uint32_t* d_cidx4;                // compressed colour matrix: [ceil(np/4)][np] words, byte u = index of C[4q+u][sigma] in cval
+    int nval;                         // number of distinct entries of C (0: no compressed form)
+    double cval[kCobgMaxVals];
 };
 
 struct CobgParams {
@@ -49,6 +53,9 @@ struct CobgParams {
     const uint8_t* ord;
     const uint32_t* lower;
     int level_begin[kCobgMaxM + 2];
+    const uint32_t* cidx4;            // compressed colour matrix (nval > 0), else C is read as doubles
+    int nval;
+    double cval[kCobgMaxVals];
 };
 
 
@@ -149,6 +156,15 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
     double* epsn = P + NSUB * 4;
     double* A = epsn + 8;
     double* red = A + np * 2;
+    // Eq. 17's matrix has few distinct entries (C_ss' = C_{e, s^-1 s'}: those of one row; 16 at n = 7): the form
+    // below reads one byte per entry (four per load, one L1 line per row of C instead of eight) and looks the value
+    // up here - 32 doubles span the 32 banks once, so any mix of indices is conflict-free
+    __shared__ double cv[kCobgMaxVals];
+    if (p.nval) {
+#pragma unroll
+        for (int i = 0; i < kCobgMaxVals; i++)
+            if (threadIdx.x == i) cv[i] = p.cval[i];
+    }
     const long long N = p.N;
     // given helicities: the EPB thread groups of a block take EPB events.  Summed helicities: the block takes one
     // event and its groups share the 2^n assignments (group evl takes hc = evl, evl + EPB, ..)
@@ -268,6 +284,27 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
             double tr[4] = {0.0, 0.0, 0.0, 0.0}, ti[4] = {0.0, 0.0, 0.0, 0.0};
             const double* Ccol = p.C + t;
             int s2 = 0;
+            if (p.nval) {
+                const uint32_t* ci = p.cidx4 + t;
+                for (; s2 + 4 <= np; s2 += 4) {
+                    const uint32_t w4 = __ldg(ci + (size_t)(s2 >> 2) * np);
+#pragma unroll
+                    for (int u = 0; u < 4; u++) {
+                        const double c = cv[(w4 >> (8 * u)) & 0xFF];
+                        const double2 a2 = *reinterpret_cast<const double2*>(A + 2 * (s2 + u));
+                        tr[u] = fma(c, a2.x, tr[u]);
+                        ti[u] = fma(c, a2.y, ti[u]);
+                    }
+                }
+                if (s2 < np) {
+                    const uint32_t w4 = __ldg(ci + (size_t)(s2 >> 2) * np);
+                    for (int u = 0; s2 < np; s2++, u++) {
+                        const double c = cv[(w4 >> (8 * u)) & 0xFF];
+                        tr[0] = fma(c, A[2 * s2], tr[0]);
+                        ti[0] = fma(c, A[2 * s2 + 1], ti[0]);
+                    }
+                }
+            }
             for (; s2 + 4 <= np; s2 += 4) {
 #pragma unroll
                 for (int u = 0; u < 4; u++) {
@@ -379,8 +416,38 @@ int cobg_table_create(int n, CobgTable** out) {
     return BG_OK;
 }
 
+// Compressed form of the colour matrix hC[np][np] for the colour form of the kernel: the list of its distinct entries
+// and one byte per entry.  Optional: with more than kCobgMaxVals distinct entries the kernel reads C itself.
+int cobg_table_set_colour(CobgTable* t, const double* hC) {
+    if (!t || !hC) return BG_EINVAL;
+    const int np = t->np;
+    std::vector<double> vals;
+    std::vector<uint32_t> idx4((size_t)((np + 3) / 4) * np, 0u);
+    for (int s2 = 0; s2 < np; s2++)
+        for (int sg = 0; sg < np; sg++) {
+            const double c = hC[(size_t)s2 * np + sg];
+            size_t k = std::find(vals.begin(), vals.end(), c) - vals.begin();
+            if (k == vals.size()) {
+                if ((int)vals.size() == kCobgMaxVals) return BG_OK;   // too many: keep the plain form
+                vals.push_back(c);
+            }
+            idx4[(size_t)(s2 / 4) * np + sg] |= (uint32_t)k << (8 * (s2 % 4));
+        }
+    if (cudaMalloc(&t->d_cidx4, idx4.size() * 4) != cudaSuccess ||
+        cudaMemcpy(t->d_cidx4, idx4.data(), idx4.size() * 4, cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        if (t->d_cidx4) cudaFree(t->d_cidx4);
+        t->d_cidx4 = nullptr;
+        return BG_ENOMEM;
+    }
+    for (int i = 0; i < kCobgMaxVals; i++) t->cval[i] = i < (int)vals.size() ? vals[i] : 0.0;
+    t->nval = (int)vals.size();
+    return BG_OK;
+}
+
 void cobg_table_destroy(CobgTable* t) {
     if (!t) return;
+    if (t->d_cidx4) cudaFree(t->d_cidx4);
     if (t->d_slot) cudaFree(t->d_slot);
     if (t->d_ord) cudaFree(t->d_ord);
     if (t->d_lower) cudaFree(t->d_lower);
@@ -415,6 +482,9 @@ cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, 
     for (int i = 0; i < t->n - 2; i++) p.lc_factor *= 3.0;
     p.N = N; p.mom = mom; p.hel = hel; p.C = dC; p.out = out;
     p.slot = t->d_slot; p.ord = t->d_ord; p.lower = t->d_lower;
+    p.cidx4 = t->d_cidx4;
+    p.nval = (!lc && dC && t->np >= 24) ? t->nval : 0;   // (n <= 5: two and six orderings, nothing to gain)
+    for (int i = 0; i < kCobgMaxVals; i++) p.cval[i] = t->cval[i];
     for (int i = 0; i < kCobgMaxM + 2; i++) p.level_begin[i] = t->level_begin[i];
     switch (t->n) {
         case 4: return lc ? launch_cobg<4, 8, true>(s, p) : launch_cobg<4, 8, false>(s, p);

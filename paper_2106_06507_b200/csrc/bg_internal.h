@@ -87,6 +87,7 @@ cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, 
 bool cobg_shared_supported(int n);
 int cobg_table_create(int n, CobgTable** out);              // BG_* code
 void cobg_table_destroy(CobgTable* t);
+int cobg_table_set_colour(CobgTable* t, const double* hC);   // optional: compressed colour matrix for the colour form
 size_t cobg_shared_current_bytes(const CobgTable* t);
 cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, bool lc, const double* dC, long long N,
                                const double* mom, const signed char* hel, double* out);
