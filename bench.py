@@ -31,7 +31,7 @@ CDBG_FLOP_PER_EVENT = {4: 2.1e3, 5: 8.4e3, 6: 2.5e4, 7: 7.0e4, 8: 2.2e5, 9: 6.4e
 COBG_FLOP_PER_EVENT = {0: 2.6e4, 2: 1.41e6 + 5.8e4}     # config 0 (n=4 helsum), config 2 (n=7 + colour form)
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the recursion kernel launches of ONE step, from the
 # `ncu --set full` captures summarised in profiles/r01_ncu_summary.md (same command, default event counts).
-NCU_TRAFFIC_BYTES = {("cdbg_prog_kernel", 6): 244.2e6, ("cobg_shared_kernel", 7): 331.1e6, ("cdbg_prog_kernel", 9): 100.2e6}
+NCU_TRAFFIC_BYTES = {("cdbg_prog_kernel", 6): 244.2e6, ("cobg_shared_kernel", 7): 91.4e6, ("cdbg_prog_kernel", 9): 100.2e6}
 CONFIG_N = {0: 4, 1: 6, 2: 7, 3: 9}
 CONFIG_EVENTS = {0: 1024, 1: 1 << 20, 2: 1 << 18, 3: 1 << 18, 4: 1 << 16}
 

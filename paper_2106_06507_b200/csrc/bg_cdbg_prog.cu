@@ -9,6 +9,9 @@
 //   3. cdbg_scatter_kernel    counting sort: every event becomes one contiguous record (header + momenta of the
 //                             canonical gluons) in class order, so that a warp runs equal programs and reads whole
 //                             sectors
+//      Small batches (<= 2^18 events, <= 4096 classes): no scan launch and no memset - every block of the scatter
+//      kernel scans the finished histogram for itself and the last one clears it for the next call; and with
+//      G <= 4 and fewer than two tasks per resident block the tier launches of step 4 run side by side.
 //   4. cdbg_prog_kernel<G,SPILL>, one launch per non-empty tier: G lanes per event run the class program
 //                             (bg_program.h): vertex operations read their operands from the event's state block in
 //                             shared memory, accumulate in registers and write each finished current back once.

@@ -183,6 +183,36 @@ def test_program_interpreter_is_deterministic(bg, wl):
     assert np.array_equal(a[::-1], c)
 
 
+def test_prepass_variants_share_a_context(bg, wl):
+    """One context, batches on both sides of the small-batch rules of the prepass (fused histogram scan up to 2^18
+    events, tier launches side by side for small batches): the table's persistent histogram buffer
+    must come back zeroed after every call, and every event must get the same bits whichever variant ran."""
+    import torch
+    big = wl.config_events(1, N=(1 << 18) + 4097)          # scan launch + memset, tiers one after the other
+    dev = torch.device("cuda:0")
+    stream = torch.cuda.current_stream().cuda_stream
+    ctx = bg.bg_init(6, bg.BG_CDBG_GIVEN)
+    try:
+        outs = {}
+        for N in (3000, big.N, 3000, 70000, 1, 70000, big.N):
+            ev = big.head(N)                               # prefix property of the generator: same events
+            d_mom = torch.from_numpy(wl.to_soa(mom=ev.mom)).to(dev)
+            d_hel = torch.from_numpy(wl.to_soa(hel=ev.hel)).to(dev)
+            d_col = torch.from_numpy(wl.to_soa(col=ev.col)).to(dev)
+            d_out = torch.full((N,), float("nan"), dtype=torch.float64, device=dev)
+            bg.bg_eval(ctx, stream, N, d_mom, d_hel, d_col, d_out)
+            torch.cuda.synchronize()
+            out = d_out.cpu().numpy()
+            assert np.all(np.isfinite(out)) and np.all(out > 0)
+            if N in outs:
+                assert np.array_equal(outs[N], out)
+            outs[N] = out
+        for N, out in outs.items():
+            assert np.array_equal(out, outs[big.N][:N])
+    finally:
+        bg.bg_destroy(ctx)
+
+
 @pytest.mark.parametrize("n,N", [(4, 40), (5, 33), (6, 12), (7, 5)])
 def test_leading_colour_mode(bg, oracle, wl, n, N):
     """Eq. 33: N^(n-2)(N^2-1) sum over all (n-1)! orderings of |A(1,sigma)|^2, against the oracle's
