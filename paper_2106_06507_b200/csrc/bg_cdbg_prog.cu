@@ -115,20 +115,20 @@ struct ProgParams {
 // (histogram larger than shared memory) the counters are updated in global memory directly.
 constexpr int kPreThreads = 512, kPrePer = 2, kPreEvents = kPreThreads * kPrePer;
 
-template <bool BLOCK_HIST>
-__global__ void __launch_bounds__(kPreThreads)
+template <bool BLOCK_HIST, int THREADS = kPreThreads, int PER = kPrePer>
+__global__ void __launch_bounds__(THREADS)
 cdbg_classify_kernel(int n, long long N, long long num_classes, const signed char* __restrict__ col,
                      const ClassInfo* __restrict__ info, const uint32_t* __restrict__ sortkey,
                      uint32_t* __restrict__ cls, uint64_t* __restrict__ perm, uint32_t* __restrict__ hist) {
     extern __shared__ uint32_t sh_hist[];
     const int nbins = (int)num_classes + 1;
     if (BLOCK_HIST) {
-        for (int i = threadIdx.x; i < nbins; i += kPreThreads) sh_hist[i] = 0;
+        for (int i = threadIdx.x; i < nbins; i += THREADS) sh_hist[i] = 0;
         __syncthreads();
     }
     uint32_t* const h = BLOCK_HIST ? sh_hist : hist;
-    for (int j = 0; j < kPrePer; j++) {
-        const long long e = (long long)blockIdx.x * kPreEvents + j * kPreThreads + threadIdx.x;
+    for (int j = 0; j < PER; j++) {
+        const long long e = (long long)blockIdx.x * (THREADS * PER) + j * THREADS + threadIdx.x;
         if (e >= N) break;
         // colour codes 3(i-1)+(j-1) of the n gluons, one nibble each (registers; n is a run-time value)
         int cnt[kNumCodes];
@@ -187,7 +187,7 @@ cdbg_classify_kernel(int n, long long N, long long num_classes, const signed cha
     }
     if (BLOCK_HIST) {
         __syncthreads();
-        for (int i = threadIdx.x; i < nbins; i += kPreThreads) {
+        for (int i = threadIdx.x; i < nbins; i += THREADS) {
             const uint32_t c = sh_hist[i];
             if (c) atomicAdd(&hist[i], c);
         }
@@ -311,6 +311,7 @@ cdbg_scatter_kernel(int n, long long N, long long num_classes, const uint32_t* _
 // 16-byte pieces, so a store instruction covers four to five lines.  Blocks of kStageThreads threads; used when
 // histogram + staging fit in shared memory for at least two blocks per SM (n <= 7).
 constexpr int kStageThreads = 256, kStageEvents = kStageThreads * kPrePer;
+constexpr int kSmallThreads = 256;              // block size of the classify kernel for small batches
 constexpr int kFusedScanBins = 4096;            // largest histogram the scatter blocks scan for themselves
 constexpr long long kFusedScanEvents = 1 << 18; // ... and largest batch (beyond it the scan launch is cheaper)
 // FUSED (small batches, where a step is a handful of short launches): the exclusive scan of the class histogram
@@ -325,7 +326,7 @@ struct FusedScan {
     uint32_t N;
     TierInfo tiers;
 };
-template <bool FUSED>
+template <bool FUSED, int PER = kPrePer>
 __global__ void __launch_bounds__(kStageThreads)
 cdbg_scatter_staged_kernel(int n, long long N, long long num_classes, const uint32_t* __restrict__ cls,
                            const uint64_t* __restrict__ perm, const uint32_t* __restrict__ sortkey,
@@ -361,12 +362,12 @@ cdbg_scatter_staged_kernel(int n, long long N, long long num_classes, const uint
         // (the barrier below, before the first use of sh_start, also orders these writes)
     }
     unsigned long long* const dstp = reinterpret_cast<unsigned long long*>(stage + 32 * rs);
-    uint32_t key[kPrePer], rank[kPrePer];
+    uint32_t key[PER], rank[PER];
     for (int i = threadIdx.x; i < nbins; i += kStageThreads) sh_hist[i] = 0;
     __syncthreads();
 #pragma unroll
-    for (int j = 0; j < kPrePer; j++) {
-        const long long e = (long long)blockIdx.x * kStageEvents + j * kStageThreads + threadIdx.x;
+    for (int j = 0; j < PER; j++) {
+        const long long e = (long long)blockIdx.x * (kStageThreads * PER) + j * kStageThreads + threadIdx.x;
         key[j] = 0xFFFFFFFFu;
         rank[j] = 0;
         if (e < N) {
@@ -383,8 +384,8 @@ cdbg_scatter_staged_kernel(int n, long long N, long long num_classes, const uint
     if (FUSED && blockIdx.x == 0 && threadIdx.x <= kTiers)
         fs.bounds[threadIdx.x] = threadIdx.x == kTiers ? fs.N : sh_start[fs.tiers.first_key[threadIdx.x]];
     __syncthreads();
-    for (int j = 0; j < kPrePer; j++) {
-        const long long e = (long long)blockIdx.x * kStageEvents + j * kStageThreads + threadIdx.x;
+    for (int j = 0; j < PER; j++) {
+        const long long e = (long long)blockIdx.x * (kStageThreads * PER) + j * kStageThreads + threadIdx.x;
         char* dst = nullptr;
         if (key[j] != 0xFFFFFFFFu) {
             dst = rec + (size_t)(sh_hist[key[j]] + rank[j]) * rec_bytes;
@@ -1319,17 +1320,20 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         int device = 0;
         cudaGetDevice(&device);
         if (configured_device != device) {
-            cudaFuncSetAttribute(cdbg_classify_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
-            cudaFuncSetAttribute(cdbg_scatter_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+            cudaFuncSetAttribute(cdbg_classify_kernel<true, kSmallThreads, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+            cudaFuncSetAttribute(cdbg_scatter_staged_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
             configured_device = device;
         }
         uint32_t* counts = t->d_small;
         FusedScan fs;
         fs.counts = counts; fs.ticket = counts + 2 * nbins; fs.bounds = bounds; fs.N = (uint32_t)N; fs.tiers = t->tiers;
-        cdbg_classify_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
-                                                                      t->d_sortkey, cls, perm, counts);
-        const unsigned sb = (unsigned)((N + kStageEvents - 1) / kStageEvents);
-        cdbg_scatter_staged_kernel<true><<<sb, kStageThreads, 2 * hist_words * sizeof(uint32_t) + stage_bytes, s>>>(
+        // one event per thread and 256-thread blocks: a small batch is less than one wave of the 1024-event blocks
+        // of the large-batch kernels, and each thread is a chain of dependent loads and atomics
+        const unsigned cb = (unsigned)((N + kSmallThreads - 1) / kSmallThreads);
+        cdbg_classify_kernel<true, kSmallThreads, 1><<<cb, kSmallThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
+                                                                                     t->d_sortkey, cls, perm, counts);
+        const unsigned sb = (unsigned)((N + kStageThreads - 1) / kStageThreads);
+        cdbg_scatter_staged_kernel<true, 1><<<sb, kStageThreads, 2 * hist_words * sizeof(uint32_t) + stage_bytes, s>>>(
             t->n, N, t->num_classes, cls, perm, t->d_sortkey, mom, hel, counts + nbins, rec, rec_bytes, fs);
     } else if (hist_smem <= 160 * 1024) {
         static int configured_device = -1;
