@@ -58,7 +58,7 @@ enum {
     BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN,
     BG_CDBG_CONTINUOUS = BG_REC_CDBG | BG_HEL_CONT | BG_COL_CONT,          /* the paper's CD_MC sampling */
     BG_COMC_GIVEN = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_GIVEN,            /* Eq. 19 with colour-ordered
-                                                                              currents, sampled colour flows (n <= 9) */
+                                                                              currents, sampled colour flows (n <= 8) */
     BG_COBG_HELSUM_LC = BG_REC_COBG | BG_HEL_SUM | BG_COL_LC,
     BG_COBG_HELGIVEN_LC = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_LC
 };
@@ -70,10 +70,23 @@ enum {
                                 memory (BG_CDBG_GIVEN, any n; COBG n <= 7) */
     BG_OPT_SCRATCH_LIMIT = 2,/* upper bound in bytes for the scratch the generic kernels may use (default 16 GiB) */
     BG_OPT_LANES = 3,        /* lanes that cooperate on one event in the program interpreter: 1, 2, 4, ..., 256;
-                                0 = automatic.  Rebuilds the class programs (synchronises the device). */
+                                0 = automatic.  Rebuilds the class programs (synchronises the device).  With few lanes
+                                a warp holds many events; if their double-double state no longer fits in shared memory
+                                BG_OPT_PRECISION falls back from 2 to 0 (setting it to 2 then returns BG_EUNSUPPORTED). */
     BG_OPT_TIMING = 4,       /* 1: record CUDA events around the dominant kernel of every bg_eval (bg_last_kernel_ms) */
-    BG_OPT_PRECISION = 6,    /* BG_CDBG_GIVEN and the COBG full-colour modes: 0 = FP64 kernels (default); 1 = every event
-                                in double-double arithmetic: the precision reference on the GPU, slow */
+    BG_OPT_PRECISION = 6,    /* 0 = FP64 kernels only; 1 = every event in double-double arithmetic (BG_CDBG_GIVEN and the COBG
+                                full-colour modes: the precision reference on the GPU, slow); 2 (BG_CDBG_GIVEN, the default
+                                there) = FP64 kernels plus a conditioning flag per event and re-evaluation of the flagged
+                                events by a double-double instantiation of the same kernel: the colour-flow amplitude of
+                                Eq. 19 / 28-32 has near-zeros - helicity-suppressed
+                                configurations, cancellations between orderings - where FP64 round-off exceeds 1e-11 of
+                                the result.  An event is flagged when its Ward residual |p_n . J| / (E_n |eps_n . J|)
+                                (J = the current of gluons 1..n-1 of Eq. 22; zero without round-off) exceeds
+                                BG_OPT_FLAG_THRESHOLD, or when |A| is less than BG_OPT_FLAG_CANCELLATION times the sum of
+                                the moduli of the closure contributions that add up to it.  3, 4 = diagnostics: `out`
+                                receives the Ward residual / that cancellation ratio instead of |M|^2. */
+    BG_OPT_FLAG_THRESHOLD = 7,/* Ward-residual threshold in units of 1e-18 (0 = default: 1e-13; 3e-14 for n = 5, 6) */
+    BG_OPT_FLAG_CANCELLATION = 8, /* cancellation threshold in units of 1e-6 (0 = default: 3e-3) */
     BG_OPT_SMEM_LIMIT = 5    /* program interpreter, >= 128 lanes per event: bytes of shared memory one event's state may
                                 take (16 KiB .. 222 KiB, 0 = default); the rest spills to an L2-resident slab.
                                 Rebuilds the class programs. */
@@ -149,6 +162,11 @@ int bg_last_launch_count(const bg_ctx* ctx);
  * events recorded on the caller's stream around that launch.  Only available after
  * bg_set_option(ctx, BG_OPT_TIMING, 1); waits for that launch to finish.  BG_EINVAL if timing is off or nothing ran. */
 int bg_last_kernel_ms(bg_ctx* ctx, double* ms);
+
+/* BG_OPT_PRECISION = 2: number of events of the most recent bg_eval that the conditioning flag sent to the
+ * double-double re-evaluation and (if BG_OPT_TIMING is on and ms != NULL) the device time of that re-evaluation in
+ * milliseconds, which bg_last_kernel_ms includes.  Waits for the device. */
+int bg_last_refined(bg_ctx* ctx, long long* flagged, double* ms);
 
 /* Name of the kernel variant the most recent bg_eval used (static string). */
 const char* bg_last_kernel_name(const bg_ctx* ctx);

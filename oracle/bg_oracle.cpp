@@ -12,7 +12,7 @@
 // round-off protocol).  No blocking, fusion or reordering beyond the formulas as printed; the only shortcut is
 // skipping terms whose input current is identically zero, which cannot change any result.
 //
-// Pins (tests/test_oracle_pins.py): Parke-Taylor MHV moduli, vanishing all-plus / single-minus amplitudes,
+// Pins (tests/test_oracle_pins_cobg.py, test_oracle_pins_colour.py, test_oracle_pins_continuous.py): Parke-Taylor MHV moduli, vanishing all-plus / single-minus amplitudes,
 // cyclicity, reflection, U(1) decoupling, gauge invariance (eps -> eps + z p, eps -> p), V4 form == tensor
 // form, closed-form gg->gg, hand-derivable colour-matrix entries, Eq. 33 exactness at n = 4,5, colour-dressed
 // == Eq. 19 brute force, sum over all 9^n colour flows == A^dagger C A; general external states (continuous

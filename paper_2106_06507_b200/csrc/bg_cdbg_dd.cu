@@ -4,7 +4,7 @@
 // have near-zeros by cancellation where FP64 round-off exceeds 1e-11; evaluated with
 // ~106-bit significands the same inputs reproduce the extended-precision oracle on every event, which shows that
 // what is left in the FP64 kernels is rounding, not arithmetic.  Not a performance path.
-#include "bg_dd.cuh"
+#include "bg_ddmath.cuh"
 #include "bg_internal.h"
 
 namespace bg {
@@ -208,14 +208,10 @@ constexpr int kDdMaxN = 8;
 __device__ __forceinline__ int tri_dd(int i, int j) { return j * (j + 1) / 2 + i; }   // i <= j
 }  // namespace
 
-__global__ void __launch_bounds__(64)
-cobg_dd_amp_kernel(int n, int nhel, int nperm, long long N, long long first, long long count,
-                   const double* __restrict__ mom, const signed char* __restrict__ hel, double2* __restrict__ amps) {
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= count * nhel * nperm) return;
-    const int s = (int)(idx % nperm);
-    const int hc = (int)((idx / nperm) % nhel);
-    const long long e = first + idx / ((long long)nperm * nhel);
+// A(1, sigma_s(2..n-1), n) of event e in double-double arithmetic (Eq. 20 + 22); hc >= 0: helicity assignment from
+// the bits of hc, else from hel.
+__device__ C cobg_dd_amplitude(int n, int nperm, int s, int hc, long long N, long long e, const double* __restrict__ mom,
+                               const signed char* __restrict__ hel) {
     const int m = n - 1, mm = n - 2;
     // s-th permutation of gluons 2..n-1 (0-based labels 1..n-2) in lexicographic order
     int avail[kDdMaxN], order[kDdMaxN];
@@ -237,7 +233,7 @@ cobg_dd_amp_kernel(int n, int nhel, int nperm, long long N, long long first, lon
         const int g = order[i];
         dd p[4];
         for (int c = 0; c < 4; c++) p[c] = mkdd(mom[(size_t)(g * 4 + c) * N + e]);
-        const int lam = nhel > 1 ? (((hc >> g) & 1) ? 1 : -1) : (int)hel[(size_t)g * N + e];
+        const int lam = hc >= 0 ? (((hc >> g) & 1) ? 1 : -1) : (int)hel[(size_t)g * N + e];
         if (i < m) {
             polarisation_t<dd>(p, lam, J[tri_dd(i, i)]);
             for (int c = 0; c < 4; c++) P[tri_dd(i, i)][c] = p[c];
@@ -249,31 +245,85 @@ cobg_dd_amp_kernel(int n, int nhel, int nperm, long long N, long long first, lon
     for (int len = 2; len <= m; len++)
         for (int i = 0; i + len <= m; i++) {
             const int j = i + len - 1;
-            for (int c = 0; c < 4; c++) P[tri_dd(i, j)][c] = P[tri_dd(i, j - 1)][c] + P[tri_dd(j, j)][c];
+            for (int c = 0; c < 4; c++) P[tri_dd(i, j)][c] = dd_add(P[tri_dd(i, j - 1)][c], P[tri_dd(j, j)][c]);
             C s3[4], s4[4];
             for (int c = 0; c < 4; c++) { s3[c] = mkc<dd>(zero, zero); s4[c] = mkc<dd>(zero, zero); }
             for (int k = i; k < j; k++) {
                 const C* a = J[tri_dd(i, k)];
-                v3_acc_t<dd>(s3, P[tri_dd(i, k)], P[tri_dd(k + 1, j)], a, J[tri_dd(k + 1, j)], false);
+                v3_acc(s3, P[tri_dd(i, k)], P[tri_dd(k + 1, j)], a, J[tri_dd(k + 1, j)], 1.0);   // fused dd multiply-adds (bg_ddmath.cuh)
                 for (int l = k + 1; l < j; l++) {
                     // 2 V4(a,b,c) = 2 (a.c) b - (a.b) c - (b.c) a   (Eq. 21, second line)
                     const C* b = J[tri_dd(k + 1, l)];
                     const C* c3 = J[tri_dd(l + 1, j)];
-                    const C ac = two * mdot_t<dd>(a, c3), ab = mdot_t<dd>(a, b), bc = mdot_t<dd>(b, c3);
-                    for (int nu = 0; nu < 4; nu++) s4[nu] = s4[nu] + ac * b[nu] - ab * c3[nu] - bc * a[nu];
+                    const C ac = cxd_scale(two, mdot(a, c3)), ab = mdot(a, b), bc = mdot(b, c3);
+                    for (int nu = 0; nu < 4; nu++) {
+                        cfma(s4[nu], ac, b[nu]);
+                        cfms(s4[nu], ab, c3[nu]);
+                        cfms(s4[nu], bc, a[nu]);
+                    }
                 }
             }
             dd f3 = inv_sqrt2, f4 = half;
             if (len < m) {
-                const dd ip2 = mkdd(1.0) / mdot_t<dd>(P[tri_dd(i, j)], P[tri_dd(i, j)]);
-                f3 = f3 * ip2; f4 = f4 * ip2;
+                const dd ip2 = mkdd(1.0) / mdot(P[tri_dd(i, j)], P[tri_dd(i, j)]);
+                f3 = dd_mul(f3, ip2); f4 = dd_mul(f4, ip2);
             }
-            for (int c = 0; c < 4; c++) J[tri_dd(i, j)][c] = f3 * s3[c] + f4 * s4[c];
+            for (int c = 0; c < 4; c++) J[tri_dd(i, j)][c] = cxd_add(cxd_scale(f3, s3[c]), cxd_scale(f4, s4[c]));
         }
-    const C A = mdot_t<dd>(epsn, J[tri_dd(0, m - 1)]);
+    return mdot(epsn, J[tri_dd(0, m - 1)]);
+}
+
+__global__ void __launch_bounds__(64)
+cobg_dd_amp_kernel(int n, int nhel, int nperm, long long N, long long first, long long count,
+                   const double* __restrict__ mom, const signed char* __restrict__ hel, double2* __restrict__ amps) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= count * nhel * nperm) return;
+    const int s = (int)(idx % nperm);
+    const int hc = (int)((idx / nperm) % nhel);
+    const long long e = first + idx / ((long long)nperm * nhel);
+    const C A = cobg_dd_amplitude(n, nperm, s, nhel > 1 ? hc : -1, N, e, mom, hel);
     double2* o = amps + idx * 2;
     o[0] = make_double2(A.re.hi, A.re.lo);
     o[1] = make_double2(A.im.hi, A.im.lo);
+}
+
+// Re-evaluation of the events the FP64 kernel flagged (BG_OPT_PRECISION = 2, given helicities): one block per listed
+// event, one thread per ordering; the amplitudes stay in shared memory and thread s takes row s of Eq. 16.
+__global__ void __launch_bounds__(128)   // (n <= 7: at most 120 orderings)
+cobg_dd_flagged_kernel(int n, int nperm, long long N, const uint32_t* __restrict__ list, const uint32_t* __restrict__ count,
+                       const double* __restrict__ mom, const signed char* __restrict__ hel, const double* __restrict__ Cm,
+                       double* __restrict__ out) {
+    extern __shared__ double2 sh_amp[];   // [nperm][2]: (re.hi, re.lo), (im.hi, im.lo), then [blockDim / 32] partial sums
+    const uint32_t total = *count;
+    const int s = threadIdx.x;
+    for (uint32_t it = blockIdx.x; it < total; it += gridDim.x) {
+        const long long e = list[it];
+        __syncthreads();
+        if (s < nperm) {
+            const C A = cobg_dd_amplitude(n, nperm, s, -1, N, e, mom, hel);
+            sh_amp[2 * s] = make_double2(A.re.hi, A.re.lo);
+            sh_amp[2 * s + 1] = make_double2(A.im.hi, A.im.lo);
+        }
+        __syncthreads();
+        dd row = mkdd(0.0);
+        if (s < nperm) {
+            dd tr = mkdd(0.0), ti = mkdd(0.0);
+            for (int s2 = 0; s2 < nperm; s2++) {
+                const dd c = mkdd(Cm[(size_t)s * nperm + s2]);
+                tr = tr + c * mkdd(sh_amp[2 * s2].x, sh_amp[2 * s2].y);
+                ti = ti + c * mkdd(sh_amp[2 * s2 + 1].x, sh_amp[2 * s2 + 1].y);
+            }
+            row = mkdd(sh_amp[2 * s].x, sh_amp[2 * s].y) * tr + mkdd(sh_amp[2 * s + 1].x, sh_amp[2 * s + 1].y) * ti;
+        }
+        __syncthreads();
+        if (s < nperm) sh_amp[2 * s] = make_double2(row.hi, row.lo);
+        __syncthreads();
+        if (s == 0) {
+            dd sum = mkdd(0.0);
+            for (int s2 = 0; s2 < nperm; s2++) sum = sum + mkdd(sh_amp[2 * s2].x, sh_amp[2 * s2].y);
+            out[e] = to_double(sum);
+        }
+    }
 }
 
 __global__ void __launch_bounds__(64)
@@ -295,6 +345,14 @@ cobg_dd_colour_kernel(int nhel, int nperm, long long first, long long count, con
         }
     }
     out[first + el] = to_double(total);
+}
+
+cudaError_t cobg_dd_flagged_launch(cudaStream_t s, int n, int nperm, const double* dC, long long N, const uint32_t* list,
+                                   const uint32_t* count, int blocks, const double* mom, const signed char* hel, double* out) {
+    const int threads = (nperm + 31) / 32 * 32;
+    if (threads > 128) return cudaErrorInvalidValue;
+    cobg_dd_flagged_kernel<<<blocks, threads, (size_t)nperm * 2 * sizeof(double2), s>>>(n, nperm, N, list, count, mom, hel, dC, out);
+    return cudaGetLastError();
 }
 
 size_t cobg_dd_scratch_per_event(int n, bool helsum) {

@@ -1,0 +1,760 @@
+// Program interpreter of the colour-dressed recursion (CDBG, Eq. 28-32, closed with Eq. 22):
+// the kernel template cdbg_prog_kernel<G, SPILL, S> and its launcher, shared by the translation units that
+// instantiate it - bg_cdbg_prog.cu (S = cx: complex FP64; S = double: real currents of the continuous states) and
+// bg_cdbg_prog_dd.cu (S = cxd: complex double-double, the re-evaluation of flagged events).
+// See bg_cdbg_prog.cu for the pipeline of one bg_eval and the state layout.
+#pragma once
+#include <algorithm>
+
+#include "bg_internal.h"
+#include "bg_math.cuh"
+#include "bg_program.h"
+
+namespace bg {
+
+constexpr int kMaxLevels = 2 * kMaxN - 4;   // setup | (main, combine) per popcount 2..n-2 | closure
+
+struct ClassInfo {            // 64 bytes; the interpreter reads the first 16
+    uint32_t op_base;         // first op of the class in the op array (units of ProgOp)
+    uint16_t state_cx;
+    uint8_t closure_code;
+    uint8_t valid;
+    uint32_t total_steps;     // interpreter steps of the whole program
+    uint32_t n_sync;          // how many of them end with a barrier (OPF_SYNC)
+    uint16_t level_steps[kMaxLevels];   // steps per level (setup | main, combine per popcount | closure): diagnostics
+    uint16_t pad[24 - kMaxLevels];
+};
+
+// What the interpreter needs to start an event, in grouping order (written by the scatter kernel).
+constexpr int kRecHeaderBytes = 32;
+
+struct alignas(16) EventHeader {
+    uint32_t event;           // event id
+    uint32_t cls;             // class id (0xFFFFFFFF: colour codes out of range)
+    uint64_t perm;            // canonical order: nibble k = original index of canonical gluon k
+};
+static_assert(sizeof(ClassInfo) == 64, "ClassInfo layout");
+
+constexpr size_t kMaxSlabBytes = 208 * 1024;   // state slab per block (the rest: op ring up to 16 KB, static use)
+constexpr int kTiers = 4;     // classes are grouped by state size so that small ones get more warps per SM
+
+struct TierInfo {
+    int first_key[kTiers + 1];   // first position (in grouping order) of each tier; [kTiers] = number of classes
+    int slab_cx[kTiers];         // state block (complex doubles per event) the tier's launch reserves
+};
+
+struct ProgTable {
+    int n, G;
+    long long num_classes;
+    int max_state_cx;
+    TierInfo tiers;
+    bool dense;               // continuous colour states: one program, nine colour entries per subset current
+    bool real;                // ... evaluated in real arithmetic (state elements are doubles)
+    int rec_bytes;            // bytes of one event record
+    bool spill;               // largest state blocks exceed the slab limit: top of the state in global memory
+    int spill_blocks_per_sm;  // resident blocks per SM of the spill kernels (each owns one global slab)
+    int sm_count;
+    ClassInfo* d_info;
+    uint32_t* d_sortkey;      // class id -> position in the order the events are grouped by
+    ProgOp* d_ops;
+    size_t ops_bytes;
+    // small batches: the tier launches run side by side on these streams (fork / join around the caller's stream)
+    cudaStream_t aux[kTiers - 1];
+    cudaEvent_t fork_ev, join_ev[kTiers - 1];
+    bool has_streams;
+    uint32_t* d_small;        // [2 (num_classes + 1) + 1] zeroed histogram | cursors | ticket of the fused-scan prepass
+    // double-double re-evaluation of flagged events (BG_OPT_PRECISION = 2): state elements are 32 bytes, so less of
+    // the state fits in shared memory
+    int dd_mode;              // 0: fits; 1: top of the state spills (>= 128 lanes); -1: does not fit (unsupported)
+    int dd_cap_cx;            // state elements per event kept in shared memory
+    int dd_spill_blocks;      // resident blocks per SM of the spilling re-evaluation kernels
+};
+
+// how one set of tier launches is sized
+struct LaunchShape {
+    bool conc = false;        // small batches: tiers side by side on the table's side streams
+    int regs = 168;           // registers per thread of the instantiation (resident-block estimate)
+    int cap_cx = 0;           // > 0: at most this many state elements per event in shared memory (SPILL kernels)
+    int spill_blocks = 0;     // SPILL: resident blocks per SM (each owns one global slab)
+};
+
+struct ProgParams {
+    int n;
+    long long N;
+    double* out;
+    const ClassInfo* info;
+    const ProgOp* ops;
+    const char* rec;           // [N] event records (header + canonical momenta) grouped by class
+    int rec_bytes;             // 32 + 32 n (discrete states) or 32 + 96 n (continuous states)
+    int rec_gstride;           // doubles per gluon in a record: 4 or 12
+    const uint32_t* bounds;    // [kTiers + 1] record positions where the tiers start (bounds[kTiers] = N)
+    int tier;
+    int slab_cx;               // complex doubles of state per event in the shared-memory slab
+    double2* spill;            // SPILL kernels: global slab, spill_cx complex doubles per block
+    int spill_cx;
+    int zero;                  // always 0 (see the op prefetch in the interpreter)
+    // Conditioning flag (BG_OPT_PRECISION = 2): events whose Ward residual |p_n . J| / (E_n |eps_n . J|) exceeds
+    // tau are appended (by record position) to the tier's list for re-evaluation in double-double arithmetic
+    double tau2;               // tau^2; 0 = no flagging (negative: diagnostics, the flag quantities instead of |A|^2)
+    double tau_rho;            // ... or whose closure contributions cancel to less than tau_rho of their sum of moduli
+    uint32_t* flag_list;       // [N] record positions; the list of tier k starts at bounds[k]
+    uint32_t* flag_count;      // [kTiers]
+    // re-evaluation launches read their tasks from the lists instead of the record ranges
+    const uint32_t* list;      // nullptr: all records of the tier
+    const uint32_t* list_count;
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// 4. interpreter
+// ---------------------------------------------------------------------------------------------------------
+// Per-event state block: offsets below `cap` live in shared memory ([offset][event], event fastest); with SPILL
+// the rest (the highest popcount levels, which are read least often) lives in an L2-resident global slab owned by
+// the block, accessed with .cg loads/stores (no stale L1 lines).
+// element of the state: one complex double (double2) or, for the all-real arithmetic of the continuous states with
+// real polarisations, one double
+// (bg_cdbg_prog_dd.cu adds the complex double-double element, 32 bytes)
+template <class S> struct StateElem;
+template <> struct StateElem<cx> {
+    using T = double2;
+    using R = double;                     // real type of momenta and scale factors
+    static constexpr bool kComplex = true, kDD = false;
+    static __device__ __forceinline__ cx get(double2 v) { return mk(v.x, v.y); }
+    static __device__ __forceinline__ double2 put(cx v) { return make_double2(v.re, v.im); }
+    static __device__ __forceinline__ cx make(double re, double im) { return mk(re, im); }
+    static __device__ __forceinline__ double2 ldcg(const double2* p) { return __ldcg(p); }
+    static __device__ __forceinline__ void stcg(double2* p, double2 v) { __stcg(p, v); }
+};
+template <> struct StateElem<double> {
+    using T = double;
+    using R = double;
+    static constexpr bool kComplex = false, kDD = false;
+    static __device__ __forceinline__ double get(double v) { return v; }
+    static __device__ __forceinline__ double put(double v) { return v; }
+    static __device__ __forceinline__ double ldcg(const double* p) { return __ldcg(p); }
+    static __device__ __forceinline__ void stcg(double* p, double v) { __stcg(p, v); }
+};
+// real-type helpers with one spelling for double and double-double
+__device__ __forceinline__ double r_add(double a, double b) { return a + b; }
+__device__ __forceinline__ double r_sub(double a, double b) { return a - b; }
+__device__ __forceinline__ double r_from(double x, double) { return x; }
+__device__ __forceinline__ double r_hi(double x) { return x; }
+// 1/sqrt2 x, and 1 / (sqrt2 P^2)
+__device__ __forceinline__ cx s_isqrt2(cx v) { return kInvSqrt2 * v; }
+__device__ __forceinline__ double s_isqrt2(double v) { return kInvSqrt2 * v; }
+__device__ __forceinline__ double r_isqrt2_over(double p2) { return kInvSqrt2 / p2; }
+__device__ __forceinline__ cx s_scale(double f, cx v) { return f * v; }
+__device__ __forceinline__ double s_scale(double f, double v) { return f * v; }
+__device__ __forceinline__ void ext_current(const double* pk, int lambda, cx* eps) { polarisation(pk, lambda, eps); }
+
+
+template <int EPW, bool SPILL, class S>
+struct StateRef {
+    using T = typename StateElem<S>::T;
+    T* base;
+    T* spill;
+    int cap;
+    __device__ __forceinline__ S ld(int o) const {
+        if (SPILL && o >= cap) return StateElem<S>::get(StateElem<S>::ldcg(spill + (o - cap)));
+        return StateElem<S>::get(base[o * EPW]);
+    }
+    __device__ __forceinline__ void st(int o, S v) const {
+        if (SPILL && o >= cap) {
+            StateElem<S>::stcg(spill + (o - cap), StateElem<S>::put(v));
+            return;
+        }
+        base[o * EPW] = StateElem<S>::put(v);
+    }
+    // a real 4-momentum: two complex elements, or four real ones
+    using R = typename StateElem<S>::R;
+    __device__ __forceinline__ void ldP(int o, R* P) const {
+        if constexpr (StateElem<S>::kComplex) {
+            const S p01 = ld(o), p23 = ld(o + 1);
+            P[0] = p01.re; P[1] = p01.im; P[2] = p23.re; P[3] = p23.im;
+        } else {
+#pragma unroll
+            for (int c = 0; c < 4; c++) P[c] = ld(o + c);
+        }
+    }
+    __device__ __forceinline__ void stP(int o, const R* P) const {
+        if constexpr (StateElem<S>::kComplex) {
+            st(o, StateElem<S>::make(P[0], P[1]));
+            st(o + 1, StateElem<S>::make(P[2], P[3]));
+        } else {
+#pragma unroll
+            for (int c = 0; c < 4; c++) st(o + c, P[c]);
+        }
+    }
+    // the same from the doubles of an event record
+    __device__ __forceinline__ void stPd(int o, const double* P) const {
+        R Pr[4];
+#pragma unroll
+        for (int c = 0; c < 4; c++) Pr[c] = r_from(P[c], R());
+        stP(o, Pr);
+    }
+};
+
+constexpr int kRing = 4;   // op ring per lane: ops are requested kRing - 1 steps before they run
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(gmem_src) : "memory");
+}
+
+// v or -v: flips the sign bits when m = 0x80000000 (integer pipe)
+__device__ __forceinline__ double cneg(double v, int m) {
+    return __hiloint2double(__double2hiint(v) ^ m, __double2loint(v));
+}
+__device__ __forceinline__ cx cneg(cx v, int m) {
+    return mk(__hiloint2double(__double2hiint(v.re) ^ m, __double2loint(v.re)),
+              __hiloint2double(__double2hiint(v.im) ^ m, __double2loint(v.im)));
+}
+
+__device__ __forceinline__ double shfl_xor(double v, int d) { return __shfl_xor_sync(0xFFFFFFFFu, v, d); }
+__device__ __forceinline__ cx shfl_xor(cx v, int d) {
+    return mk(__shfl_xor_sync(0xFFFFFFFFu, v.re, d), __shfl_xor_sync(0xFFFFFFFFu, v.im, d));
+}
+
+__device__ __forceinline__ int hi_word(cx v) { return __double2hiint(v.re); }
+__device__ __forceinline__ int hi_word(double v) { return __double2hiint(v); }
+
+__device__ __forceinline__ EventHeader ld_header(const char* h) {
+    const uint4 v = __ldcg(reinterpret_cast<const uint4*>(h));   // streamed once: not through L1
+    EventHeader r;
+    r.event = v.x; r.cls = v.y; r.perm = (uint64_t)v.z | ((uint64_t)v.w << 32);
+    return r;
+}
+
+template <int G, bool SPILL, class S>
+__global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgParams p) {
+    // G <= 32: one warp per block, EPW = 32/G events per warp.  G > 32: one event per block of G threads.
+    // S: complex currents (cx) or, for continuous states with real polarisations, real ones (double).
+    constexpr int EPW = G >= 32 ? 1 : 32 / G;
+    using T = typename StateElem<S>::T;
+    using R = typename StateElem<S>::R;
+    constexpr bool kComplex = StateElem<S>::kComplex;
+    extern __shared__ double2 smem_raw[];
+    T* const smem = reinterpret_cast<T*>(smem_raw);
+    const int lane = threadIdx.x;
+    const int q = lane % EPW, g = lane / EPW;
+    constexpr int kBlock = G > 32 ? G : 32;
+    constexpr bool kUseRing = G >= 8;
+    constexpr bool kEarlyRing = kUseRing && G <= 64;   // op read from the ring one step ahead (G >= 128: measured 1 % slower)
+    // [kRing][kBlock] behind the state slab (rounded up to 16 bytes)
+    uint4* const ring = reinterpret_cast<uint4*>(smem_raw + ((size_t)p.slab_cx * EPW * sizeof(T) + 15) / 16) + lane;
+    StateRef<EPW, SPILL, S> st_;
+    st_.base = smem + q;
+    st_.spill = SPILL ? reinterpret_cast<T*>(p.spill) + (size_t)blockIdx.x * p.spill_cx : nullptr;
+    st_.cap = p.slab_cx;
+    // tasks: the records of the tier, or (re-evaluation) the record positions in the tier's flag list
+    const long long first = p.bounds[p.tier], end = p.list ? first + p.list_count[p.tier] : (long long)p.bounds[p.tier + 1];
+    const long long ntasks = (end - first + EPW - 1) / EPW;
+    auto rec_pos = [&](long long i) -> long long { return p.list ? (long long)__ldg(p.list + i) : i; };
+    const long long N = p.N;
+    const int n = p.n;
+    // lanes of one event (same q) run the same program and meet at its barriers; events of different classes in
+    // one warp pass different numbers of barriers, so the barrier names only the event's own lanes
+    unsigned evmask = 0;
+#pragma unroll
+    for (int i = 0; i < (G < 32 ? G : 32); i++) evmask |= 1u << (q + i * EPW);
+
+    // the header of a task is loaded one task ahead; the inputs of the next task are prefetched into L2 while
+    // the current one computes (events come in class order, so their rows are scattered over the input arrays)
+    EventHeader hnext;
+    hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
+    if ((long long)blockIdx.x < ntasks) {
+        const long long idx = first + (long long)blockIdx.x * EPW + q;
+        if (idx < end) hnext = ld_header(p.rec + (size_t)rec_pos(idx) * p.rec_bytes);
+    }
+    long long pos_next = 0;    // record position of the next task's event (equals its index unless a list is read)
+    if (p.list && (long long)blockIdx.x < ntasks) {
+        const long long idx = first + (long long)blockIdx.x * EPW + q;
+        if (idx < end) pos_next = rec_pos(idx);
+    }
+    // carried from one task to the next: the class info of the next event, requested at the first barrier of the
+    // current task (one load less in the chain header -> info -> ops -> inputs at the start of a task)
+    uint4 ci_next = make_uint4(0, 0, 0, 0);
+    bool ci_next_ok = false;
+    for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
+        const long long idx0 = first + task * EPW + q;
+        const bool have = idx0 < end;
+        const long long idx = p.list ? pos_next : idx0;          // record position
+        const EventHeader h = hnext;
+        long long idx_next = 0;
+        {
+            const long long idx2 = idx0 + (long long)gridDim.x * EPW;
+            hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
+            idx_next = idx2;
+            if (task + gridDim.x < ntasks && idx2 < end) {
+                if (p.list) idx_next = pos_next = rec_pos(idx2);
+                hnext = ld_header(p.rec + (size_t)idx_next * p.rec_bytes);
+            }
+        }
+        const long long e = h.event;
+        const uint32_t cls = have ? h.cls : 0xFFFFFFFFu;
+        const double* mrec = reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
+        // discrete states: the setup level gives gluon k to lane k % G, so the lane's first momentum is requested
+        // here, ahead of the dependent loads class info -> ops that the setup ops themselves wait for
+        const bool discrete = !kUseRing && p.rec_gstride == 4 && kComplex;   // (G >= 8: measured 1-2 % slower)
+        double pk[4] = {0.0, 0.0, 0.0, 0.0};
+        if (discrete && g < n) {
+#pragma unroll
+            for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + g * 4 + c);
+        }
+        uint4 ci = ci_next;
+        if (!ci_next_ok) ci = __ldg(reinterpret_cast<const uint4*>(p.info + (cls == 0xFFFFFFFFu ? 0 : cls)));
+        ci_next_ok = false;
+        const bool valid = cls != 0xFFFFFFFFu && ((ci.y >> 24) & 0xFF);
+        const uint64_t perm = h.perm;
+        const ProgOp* ops = p.ops + ci.x + g;
+        const int total = valid ? (int)ci.z : 0;
+        bool prefetched = false;
+
+        S amp = s_zero<S>();
+        S wamp = s_zero<S>();     // Ward residual  sqrt2 p_n . J({1..n-1})  (exactly zero without round-off)
+        double asum = 0.0;        // sum of |Re| + |Im| of the closure contributions that add up to the amplitude
+        S acc[4], tacc[6];
+        R Pt[4];
+#pragma unroll
+        for (int c = 0; c < 4; c++) { acc[c] = s_zero<S>(); Pt[c] = r_from(0.0, R()); }
+#pragma unroll
+        for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
+
+        // The lane's ops travel global -> shared by cp.async, kRing - 1 steps ahead, into a private ring (no
+        // registers are held across the latency and nothing else reads these slots); the table ends with spare rows.
+        // With few lanes per event (G <= 4) the program of a class is small and stays in L1: plain loads, two steps
+        // ahead, are cheaper there.
+        auto first_barrier_done = [&]() {
+            prefetched = true;
+            if (hnext.cls != 0xFFFFFFFFu) {
+                // the next event's record (a few 128-byte lines) is pulled into L2 meanwhile
+                for (int k = g * 128; k < p.rec_bytes; k += G * 128)
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(p.rec + (size_t)idx_next * p.rec_bytes + k));
+                if constexpr (kUseRing) {      // (G <= 4: measured neutral to slightly slower)
+                    ci_next = __ldg(reinterpret_cast<const uint4*>(p.info + hnext.cls));
+                    ci_next_ok = true;
+                }
+            }
+        };
+        // Momentum conservation holds for double-precision inputs only to round-off, and the recursion never uses the
+        // momentum of the closing gluon: closing with another gluon than input gluon n evaluates a slightly different
+        // continuation of the amplitude off the momentum-conserving surface - a relative difference of 1e-16 times the
+        // event's condition number.  Input gluon n, when the class closes with another one, therefore gets the
+        // momentum -(sum of the others): exactly the momentum flow of the recursion closed with gluon n (oracle and
+        // Eq. 22 as printed) in the double-double kernel; in the FP64 kernels that sum (compensated) rounded once.
+        int kstar = -1;
+        if constexpr (kComplex) {
+            if (p.rec_gstride == 4)
+                for (int k = 0; k + 1 < n; k++)
+                    if ((int)((perm >> (4 * k)) & 0xF) == n - 1) kstar = k;
+        }
+        auto store_ext_momentum = [&](int kk, int offPt, const double* pk) {
+            if constexpr (kComplex && !StateElem<S>::kDD) {
+                if (kk == kstar) {
+                    double Pe[4];
+#pragma unroll
+                    for (int c = 0; c < 4; c++) {
+                        double sum = 0.0, comp = 0.0;     // two-sum accumulation of -(sum of the other momenta)
+                        for (int j = 0; j < n; j++) {
+                            if (j == kk) continue;
+                            const double x = -__ldcg(mrec + j * 4 + c);
+                            const double t = sum + x, bb = t - sum;
+                            comp += (sum - (t - bb)) + (x - bb);
+                            sum = t;
+                        }
+                        Pe[c] = sum + comp;
+                    }
+                    st_.stPd(offPt, Pe);
+                    return;
+                }
+            }
+            if constexpr (StateElem<S>::kDD) {
+                if (kk == kstar) {
+                    R Pe[4];
+#pragma unroll
+                    for (int c = 0; c < 4; c++) Pe[c] = r_from(0.0, R());
+                    for (int j = 0; j < n; j++) {
+                        if (j == kk) continue;
+#pragma unroll
+                        for (int c = 0; c < 4; c++) Pe[c] = r_sub(Pe[c], r_from(__ldcg(mrec + j * p.rec_gstride + c), R()));
+                    }
+                    st_.stP(offPt, Pe);
+                    return;
+                }
+            }
+            st_.stPd(offPt, pk);
+        };
+        const int s0 = (discrete && total > 0) ? (n + G - 1) / G : 0;     // steps of the setup level done up front
+        uint4 r0 = make_uint4(0, 0, 0, 0), r1 = r0;
+        if constexpr (kUseRing) {
+            if (total > 0) {
+#pragma unroll
+                for (int i = 0; i < kRing - 1; i++) {
+                    cp_async16(ring + ((s0 + i) % kRing) * kBlock, ops + (size_t)(s0 + i) * G);
+                    asm volatile("cp.async.commit_group;" ::: "memory");
+                }
+                if constexpr (kEarlyRing) {
+                    asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 2) : "memory");
+                    r0 = ring[(s0 % kRing) * kBlock];
+                }
+            }
+        } else {
+            r0 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s0 * G));
+            r1 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)(s0 + 1) * G));
+        }
+        if constexpr (kComplex) {
+            // setup level (discrete states): external currents eps(p_k, lambda_k) and momenta, Eq. 20 / g1-g5
+            int k = g;
+            for (int s = 0; s < s0; s++) {
+                const uint4 raw = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s * G));
+                const int kn = k + G;
+                double pn[4] = {0.0, 0.0, 0.0, 0.0};
+                if (kn < n) {
+#pragma unroll
+                    for (int c = 0; c < 4; c++) pn[c] = __ldcg(mrec + kn * 4 + c);
+                }
+                if ((raw.z >> 16) & OPF_EXT) {
+                    const int kk = (int)raw.w;
+                    if (kk != k) {      // another dealing of the gluons than k % G: fetch what the op names
+#pragma unroll
+                        for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + kk * 4 + c);
+                    }
+                    S eps[4];
+                    ext_current(pk, ((perm >> (48 + kk)) & 1) ? 1 : -1, eps);
+                    const int offDst = raw.y >> 16, offPt = raw.z & 0xFFFF;
+#pragma unroll
+                    for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
+                    if (offPt != 0xFFFF) store_ext_momentum(kk, offPt, pk);
+                }
+#pragma unroll
+                for (int c = 0; c < 4; c++) pk[c] = pn[c];
+                k = kn;
+            }
+            if (s0 > 0) {
+                if constexpr (G > 32) __syncthreads(); else __syncwarp(evmask);
+                first_barrier_done();
+            }
+        }
+        {
+            for (int s = s0; s < total; s++) {
+                uint4 raw, r2 = r1;
+                if constexpr (kUseRing) {
+                    cp_async16(ring + ((s + kRing - 1) % kRing) * kBlock, ops + (size_t)(s + kRing - 1) * G);
+                    asm volatile("cp.async.commit_group;" ::: "memory");
+                    if constexpr (kEarlyRing) {
+                        asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 2) : "memory");
+                        raw = r0;
+                        r2 = ring[((s + 1) % kRing) * kBlock];     // the next step's op leaves the ring one step early
+                    } else {
+                        asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 1) : "memory");
+                        raw = ring[(s % kRing) * kBlock];
+                    }
+                } else {
+                    raw = r0;
+                    const ProgOp* src = ops + (size_t)(s + 2) * G;
+                    r2 = __ldg(reinterpret_cast<const uint4*>(src));
+                }
+                const int offA = raw.x & 0xFFFF, offB = raw.x >> 16;
+                const int offP1 = raw.y & 0xFFFF, offDst = raw.y >> 16;
+                const int offPt = raw.z & 0xFFFF;
+                const unsigned flags = raw.z >> 16;
+                if (flags & OPF_VALID) {
+                    S a[4], b[4];
+#pragma unroll
+                    for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); b[c] = st_.ld(offB + c); }
+                    R P1[4], P2[4];
+                    st_.ldP(offP1, P1);
+                    if (flags & OPF_FIRST) {
+#pragma unroll
+                        for (int c = 0; c < 4; c++) acc[c] = s_zero<S>();
+#pragma unroll
+                        for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
+                        const int offP2 = (int)(raw.w & 0xFFFF);
+                        R Pb[4];
+                        st_.ldP(offP2, Pb);
+#pragma unroll
+                        for (int c = 0; c < 4; c++) Pt[c] = r_add(P1[c], Pb[c]);
+                    }
+#pragma unroll
+                    for (int c = 0; c < 4; c++) P2[c] = r_sub(Pt[c], P1[c]);
+                    // X(a,b) is linear in the pair (a, T_a): a negative vertex flips the sign bits of that pair
+                    // (integer pipe) instead of multiplying every term by -1 on the FP64 pipe
+                    const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
+#pragma unroll
+                    for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
+                    v3_acc(acc, P1, P2, a, b, 1.0);
+                    if (flags & OPF_TENB) {
+                        S T[6];
+#pragma unroll
+                        for (int c = 0; c < 6; c++) T[c] = st_.ld(offB + 4 + c);
+                        tcontract_acc(acc, T, a, 1.0);
+                    }
+                    if (flags & OPF_TENA) {
+                        S T[6];
+#pragma unroll
+                        for (int c = 0; c < 6; c++) T[c] = cneg(st_.ld(offA + 4 + c), neg);
+                        tcontract_acc(acc, T, b, -1.0);
+                    }
+                    if (!(flags & OPF_CLOSURE)) tbuild_acc(tacc, a, b, 1.0);
+                    if (flags & OPF_PARTIAL) {
+                        // chunk of a split target: raw sums to its scratch slot, finished by a COMBINE op
+#pragma unroll
+                        for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
+#pragma unroll
+                        for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
+                    } else if (flags & OPF_LAST) {
+                        if (flags & OPF_CLOSURE) {
+                            S en[4];
+#pragma unroll
+                            for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
+                            const S term = s_isqrt2(mdot(en, acc));
+                            amp = amp + term;
+                            // Ward identity: the full current is conserved, P . J = 0 with P = P(1..n-1) = -p_n
+                            if constexpr (kComplex && !StateElem<S>::kDD) {
+                                wamp = wamp + mdot(Pt, acc);
+                                asum += fabs(term.re) + fabs(term.im);
+                            }
+                        } else {
+                            const R f = r_isqrt2_over(mdot(Pt, Pt));
+#pragma unroll
+                            for (int c = 0; c < 4; c++) acc[c] = s_scale(f, acc[c]);
+#pragma unroll
+                            for (int c = 0; c < 6; c++) tacc[c] = s_isqrt2(tacc[c]);
+                            if (!(flags & OPF_NOSTORE)) {
+#pragma unroll
+                                for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
+#pragma unroll
+                                for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
+                            }
+                            if (flags & OPF_STOREP) {
+                                st_.stP(offPt, Pt);
+                            }
+                        }
+                    }
+                } else if (flags & OPF_FUSED) {
+                    // closure vertex X(eps_k, J(pi)) . eps_n with J(pi), T(pi) still in acc / tacc, P(pi) in Pt
+                    S a[4], x[4], en[4];
+                    R P1[4];
+#pragma unroll
+                    for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); x[c] = s_zero<S>(); }
+                    st_.ldP(offP1, P1);
+                    const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
+#pragma unroll
+                    for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
+                    v3_acc(x, P1, Pt, a, acc, 1.0);
+                    tcontract_acc(x, tacc, a, 1.0);
+#pragma unroll
+                    for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
+                    const S term = s_isqrt2(mdot(en, x));
+                    amp = amp + term;
+                    if constexpr (kComplex && !StateElem<S>::kDD) {
+                        double Pf[4];
+#pragma unroll
+                        for (int c = 0; c < 4; c++) Pf[c] = P1[c] + Pt[c];
+                        wamp = wamp + mdot(Pf, x);
+                        asum += fabs(term.re) + fabs(term.im);
+                    }
+                } else if (flags & OPF_COMBINE) {
+                    // add the offB partial sums of a split target and finish it like a LAST op
+#pragma unroll
+                    for (int c = 0; c < 4; c++) acc[c] = st_.ld(offA + c);
+#pragma unroll
+                    for (int c = 0; c < 6; c++) tacc[c] = st_.ld(offA + 4 + c);
+                    for (int r = 1; r < offB; r++) {
+#pragma unroll
+                        for (int c = 0; c < 4; c++) acc[c] = acc[c] + st_.ld(offA + 10 * r + c);
+#pragma unroll
+                        for (int c = 0; c < 6; c++) tacc[c] = tacc[c] + st_.ld(offA + 10 * r + 4 + c);
+                    }
+                    {
+                        const int offP2 = (int)(raw.w & 0xFFFF);
+                        R Pa[4], Pb[4];
+                        st_.ldP(offP1, Pa);
+                        st_.ldP(offP2, Pb);
+#pragma unroll
+                        for (int c = 0; c < 4; c++) Pt[c] = r_add(Pa[c], Pb[c]);
+                    }
+                    const R f = r_isqrt2_over(mdot(Pt, Pt));
+#pragma unroll
+                    for (int c = 0; c < 4; c++) acc[c] = s_scale(f, acc[c]);
+#pragma unroll
+                    for (int c = 0; c < 6; c++) tacc[c] = s_isqrt2(tacc[c]);
+                    if (!(flags & OPF_NOSTORE)) {
+#pragma unroll
+                        for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
+#pragma unroll
+                        for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
+                    }
+                    if (flags & OPF_STOREP) {
+                        st_.stP(offPt, Pt);
+                    }
+                } else if (!StateElem<S>::kDD && (flags & OPF_EXTD)) {
+                    // continuous states (Eq. 7, 9, 12): real polarisation e(phi) times the colour matrix etabar_h eta_g;
+                    // record per gluon: p (4), phi, eta (3), etabar (3), pad
+                    const int k = (int)raw.w;
+                    const double* gr = mrec + k * p.rec_gstride;
+                    double pk[4], ev[4], eta[3], etab[3];
+#pragma unroll
+                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(gr + c);
+                    const double phi = __ldcg(gr + 4);
+#pragma unroll
+                    for (int c = 0; c < 3; c++) { eta[c] = __ldcg(gr + 5 + c); etab[c] = __ldcg(gr + 8 + c); }
+                    polarisation_real(pk, phi, ev);
+                    const bool closure_leg = offPt == 0xFFFF;   // gluon n: no momentum slot; target (h,g) reads X_n[g][h]
+#pragma unroll
+                    for (int h = 0; h < 3; h++)
+#pragma unroll
+                        for (int gg = 0; gg < 3; gg++) {
+                            const double x = etab[h] * eta[gg];
+                            const int at = offDst + 4 * (h * 3 + gg);
+#pragma unroll
+                            for (int c = 0; c < 4; c++) st_.st(at + c, s_real<S>(x * ev[c]));
+                        }
+                    if (!closure_leg) {
+                        st_.stPd(offPt, pk);
+                    }
+                } else if ((flags & OPF_EXT) && kComplex) {
+                    const int k = (int)raw.w;
+                    double pk[4];
+#pragma unroll
+                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + k * p.rec_gstride + c);   // not through L1: it is kept for the ops
+                    if constexpr (kComplex) {
+                        S eps[4];
+                        ext_current(pk, ((perm >> (48 + k)) & 1) ? 1 : -1, eps);
+#pragma unroll
+                        for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
+                    }
+                    if (offPt != 0xFFFF) store_ext_momentum(k, offPt, pk);
+                }
+                if (flags & OPF_SYNC) {
+                    // end of a level: the currents just written become visible to the lanes of the event
+                    if constexpr (G > 32) __syncthreads(); else __syncwarp(evmask);
+                    if (!prefetched) first_barrier_done();
+                }
+                {
+                    // The op requested at the top of this step must not be touched before the step ends (the
+                    // compiler would otherwise park it right behind the load with moves that wait for it): its
+                    // first use is tied to the step's last arithmetic results through an always-zero mask.
+                    const unsigned late = (unsigned)(hi_word(acc[0]) ^ hi_word(amp)) & (unsigned)p.zero;
+                    const uint4 moved = make_uint4(r2.x | late, r2.y | late, r2.z | late, r2.w | late);
+                    if constexpr (kEarlyRing) { r0 = moved; } else if constexpr (!kUseRing) { r0 = r1; r1 = moved; }
+                }
+            }
+            if constexpr (kUseRing) asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
+
+        // closure amplitude: sum of the G lanes' partial contractions (Eq. 22), then |A|^2
+        constexpr bool kWard = kComplex && !StateElem<S>::kDD;
+        const bool flagging = kWard && p.tau2 > 0.0;
+#pragma unroll
+        for (int d = EPW; d < 32; d <<= 1) {
+            amp = amp + shfl_xor(amp, d);
+            if constexpr (kWard) { wamp = wamp + shfl_xor(wamp, d); asum += shfl_xor(asum, d); }
+        }
+        if constexpr (G > 32) {
+            __shared__ double red_s[(kWard ? 3 : 1) * (sizeof(S) / 8) * (G / 32)];
+            if ((lane & 31) == 0) {
+                reinterpret_cast<S*>(red_s)[lane >> 5] = amp;
+                if constexpr (kWard) {
+                    reinterpret_cast<S*>(red_s)[G / 32 + (lane >> 5)] = wamp;
+                    red_s[2 * (sizeof(S) / 8) * (G / 32) + (lane >> 5)] = asum;
+                }
+            }
+            __syncthreads();
+            if (lane == 0) {
+                amp = s_zero<S>();
+                for (int w = 0; w < G / 32; w++) amp = amp + reinterpret_cast<S*>(red_s)[w];
+                if constexpr (kWard) {
+                    wamp = s_zero<S>();
+                    asum = 0.0;
+                    for (int w = 0; w < G / 32; w++) {
+                        wamp = wamp + reinterpret_cast<S*>(red_s)[G / 32 + w];
+                        asum += red_s[2 * (sizeof(S) / 8) * (G / 32) + w];
+                    }
+                }
+            }
+        }
+        if (g == 0 && have) {
+            const double w = valid ? s_norm2(amp) : 0.0;
+            p.out[e] = w;
+            if constexpr (kWard) {
+                if (p.tau2 < 0.0 && valid) {
+                    // diagnostic (BG_OPT_PRECISION = 3): the Ward residual itself instead of |A|^2
+                    const double En = __ldcg(mrec + (n - 1) * p.rec_gstride);
+                    p.out[e] = p.tau2 < -1.5 ? (fabs(amp.re) + fabs(amp.im)) / asum : ::sqrt(0.5 * s_norm2(wamp) / (En * En * w));
+                }
+                if (flagging && valid) {
+                    // |sqrt2 p_n . J|^2 / 2 > tau^2 E_n^2 |A|^2, or |A| < tau_rho sum |closure terms| (the Ward residual does
+                    // not see round-off that respects gauge invariance; strong cancellation at the top amplifies
+                    // any), or a result that is not a positive finite number: evaluated again in double-double
+                    const double En = __ldcg(mrec + (n - 1) * p.rec_gstride);
+                    if (!(0.5 * s_norm2(wamp) <= p.tau2 * En * En * w) || !(fabs(amp.re) + fabs(amp.im) >= p.tau_rho * asum) || !(w > 0.0))
+                        p.flag_list[first + atomicAdd(p.flag_count + p.tier, 1u)] = (uint32_t)idx;
+                }
+            }
+        }
+        if constexpr (G > 32) __syncthreads(); else __syncwarp();
+    }
+}
+
+template <int G, bool SPILL, class S = cx>
+static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched,
+                                 const LaunchShape& shape) {
+    bool conc = shape.conc;
+    constexpr int EPW = G >= 32 ? 1 : 32 / G, BLOCK = G > 32 ? G : 32;
+    constexpr size_t ELEM = sizeof(typename StateElem<S>::T);
+    static int configured_device = -1;   // the attribute is per device
+    int device = 0;
+    cudaGetDevice(&device);
+    if (configured_device != device) {
+        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL, S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)(kMaxSlabBytes + (size_t)kRing * BLOCK * 16));
+        if (e != cudaSuccess) return e;
+        configured_device = device;
+    }
+    const long long max_tasks = (p.N + EPW - 1) / EPW + kTiers;
+    unsigned blocks[kTiers];
+    size_t smem[kTiers];
+    int slab[kTiers];
+    long long resident = 0;
+    int nlaunch = 0;
+    for (int k = 0; k < kTiers; k++) {
+        blocks[k] = 0;
+        if (t->tiers.first_key[k] == t->tiers.first_key[k + 1] && k + 1 < kTiers) continue;   // no class in this tier
+        const size_t ring_bytes = G >= 8 ? (size_t)kRing * BLOCK * 16 : 0;
+        slab[k] = shape.cap_cx > 0 ? std::min(t->tiers.slab_cx[k], shape.cap_cx) : t->tiers.slab_cx[k];
+        smem[k] = ((size_t)EPW * slab[k] * ELEM + 15) / 16 * 16 + ring_bytes;
+        if (smem[k] > kMaxSlabBytes + ring_bytes) return cudaErrorInvalidValue;
+        // resident blocks per SM: shared memory (1 KB reserved per block), and 65536 / (regs x BLOCK) registers
+        int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (shape.regs * BLOCK), (228 * 1024) / (smem[k] + 1024)));
+        if (SPILL) per_sm = std::min(per_sm, shape.spill_blocks);   // one global slab per resident block
+        blocks[k] = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
+        resident += (long long)sm_count * per_sm;
+        nlaunch++;
+    }
+    // Small batches: when the tiers together hold fewer than two tasks per resident block, each launch is mostly
+    // ramp-up and tail, so the tiers run side by side (fork / join around the caller's stream).  Measured at
+    // n = 6: 2^16 events +22 %, 2^18 neutral, 2^20 -5 %; n >= 7: slower at every size.
+    // (spill slabs are indexed by block: one launch at a time)
+    conc = conc && G <= 4 && !SPILL && t->has_streams && nlaunch > 1 && max_tasks <= 2 * resident;
+    if (conc && cudaEventRecord(t->fork_ev, s) != cudaSuccess) return cudaGetLastError();
+    int side = 0;                                 // launches sent to the side streams so far
+    bool first = true;
+    for (int k = 0; k < kTiers; k++) {
+        if (!blocks[k]) continue;
+        p.tier = k;
+        p.slab_cx = slab[k];
+        cudaStream_t ls = s;
+        if (conc && !first) {
+            ls = t->aux[side];
+            cudaStreamWaitEvent(ls, t->fork_ev, 0);
+        }
+        cdbg_prog_kernel<G, SPILL, S><<<blocks[k], BLOCK, smem[k], ls>>>(p);
+        if (conc && !first) cudaEventRecord(t->join_ev[side++], ls);
+        first = false;
+        ++*launched;
+    }
+    for (int i = 0; i < side; i++) cudaStreamWaitEvent(s, t->join_ev[i], 0);
+    return cudaGetLastError();
+}
+
+}  // namespace bg

@@ -29,83 +29,11 @@
 #include <thread>
 #include <vector>
 
-#include "bg_internal.h"
-#include "bg_math.cuh"
-#include "bg_program.h"
+#include "bg_cdbg_interp.cuh"
 
 namespace bg {
 
-constexpr int kMaxLevels = 2 * kMaxN - 4;   // setup | (main, combine) per popcount 2..n-2 | closure
-
-struct ClassInfo {            // 64 bytes; the interpreter reads the first 16
-    uint32_t op_base;         // first op of the class in the op array (units of ProgOp)
-    uint16_t state_cx;
-    uint8_t closure_code;
-    uint8_t valid;
-    uint32_t total_steps;     // interpreter steps of the whole program
-    uint32_t n_sync;          // how many of them end with a barrier (OPF_SYNC)
-    uint16_t level_steps[kMaxLevels];   // steps per level (setup | main, combine per popcount | closure): diagnostics
-    uint16_t pad[24 - kMaxLevels];
-};
-
-// What the interpreter needs to start an event, in grouping order (written by the scatter kernel).
-constexpr int kRecHeaderBytes = 32;
-
-struct alignas(16) EventHeader {
-    uint32_t event;           // event id
-    uint32_t cls;             // class id (0xFFFFFFFF: colour codes out of range)
-    uint64_t perm;            // canonical order: nibble k = original index of canonical gluon k
-};
-static_assert(sizeof(ClassInfo) == 64, "ClassInfo layout");
-
-constexpr size_t kMaxSlabBytes = 208 * 1024;   // state slab per block (the rest: op ring up to 16 KB, static use)
-constexpr int kTiers = 4;     // classes are grouped by state size so that small ones get more warps per SM
-
-struct TierInfo {
-    int first_key[kTiers + 1];   // first position (in grouping order) of each tier; [kTiers] = number of classes
-    int slab_cx[kTiers];         // state block (complex doubles per event) the tier's launch reserves
-};
-
-struct ProgTable {
-    int n, G;
-    long long num_classes;
-    int max_state_cx;
-    TierInfo tiers;
-    bool dense;               // continuous colour states: one program, nine colour entries per subset current
-    bool real;                // ... evaluated in real arithmetic (state elements are doubles)
-    int rec_bytes;            // bytes of one event record
-    bool spill;               // largest state blocks exceed the slab limit: top of the state in global memory
-    int spill_blocks_per_sm;  // resident blocks per SM of the spill kernels (each owns one global slab)
-    int sm_count;
-    ClassInfo* d_info;
-    uint32_t* d_sortkey;      // class id -> position in the order the events are grouped by
-    ProgOp* d_ops;
-    size_t ops_bytes;
-    // small batches: the tier launches run side by side on these streams (fork / join around the caller's stream)
-    cudaStream_t aux[kTiers - 1];
-    cudaEvent_t fork_ev, join_ev[kTiers - 1];
-    bool has_streams;
-    uint32_t* d_small;        // [2 (num_classes + 1) + 1] zeroed histogram | cursors | ticket of the fused-scan prepass
-};
-
 __constant__ unsigned c_mscount[kMaxN + 1][kNumCodes];   // multiset_count(r, t) for r <= 12, t <= 8
-
-struct ProgParams {
-    int n;
-    long long N;
-    double* out;
-    const ClassInfo* info;
-    const ProgOp* ops;
-    const char* rec;           // [N] event records (header + canonical momenta) grouped by class
-    int rec_bytes;             // 32 + 32 n (discrete states) or 32 + 96 n (continuous states)
-    int rec_gstride;           // doubles per gluon in a record: 4 or 12
-    const uint32_t* bounds;    // [kTiers + 1] record positions where the tiers start (bounds[kTiers] = N)
-    int tier;
-    int slab_cx;               // complex doubles of state per event in the shared-memory slab
-    double2* spill;            // SPILL kernels: global slab, spill_cx complex doubles per block
-    int spill_cx;
-    int zero;                  // always 0 (see the op prefetch in the interpreter)
-};
 
 // ---------------------------------------------------------------------------------------------------------
 // 1. classification
@@ -119,9 +47,11 @@ template <bool BLOCK_HIST, int THREADS = kPreThreads, int PER = kPrePer>
 __global__ void __launch_bounds__(THREADS)
 cdbg_classify_kernel(int n, long long N, long long num_classes, const signed char* __restrict__ col,
                      const ClassInfo* __restrict__ info, const uint32_t* __restrict__ sortkey,
-                     uint32_t* __restrict__ cls, uint64_t* __restrict__ perm, uint32_t* __restrict__ hist) {
+                     uint32_t* __restrict__ cls, uint64_t* __restrict__ perm, uint32_t* __restrict__ hist,
+                     uint32_t* __restrict__ flag_count) {
     extern __shared__ uint32_t sh_hist[];
     const int nbins = (int)num_classes + 1;
+    if (blockIdx.x == 0 && threadIdx.x < kTiers) flag_count[threadIdx.x] = 0;   // lists of the conditioning flag
     if (BLOCK_HIST) {
         for (int i = threadIdx.x; i < nbins; i += THREADS) sh_hist[i] = 0;
         __syncthreads();
@@ -239,7 +169,17 @@ cdbg_scan_kernel(uint32_t* __restrict__ hist, int count, TierInfo tiers, uint32_
 __device__ __forceinline__ void write_record(int n, long long N, long long e, uint32_t c, uint64_t pm,
                                              const double* __restrict__ mom, const signed char* __restrict__ hel,
                                              char* __restrict__ rec) {
+    if (c == 0xFFFFFFFFu || pm == 0) {
+        // colour codes out of range, or a class whose amplitude vanishes identically: the interpreter reads the
+        // header only (a valid permutation never has pm = 0), so no momenta are gathered
+        EventHeader h;
+        h.event = (uint32_t)e; h.cls = c; h.perm = 0;
+        *reinterpret_cast<EventHeader*>(rec) = h;
+        return;
+    }
     unsigned inv[kMaxN];                       // original gluon -> canonical position
+#pragma unroll
+    for (int k = 0; k < kMaxN; k++) inv[k] = (unsigned)k;
     for (int k = 0; k < n; k++) inv[(pm >> (4 * k)) & 0xF] = (unsigned)k;
     double2* m = reinterpret_cast<double2*>(rec + kRecHeaderBytes);   // 32-byte aligned: one sector per gluon
     // three gluons (12 coalesced loads) in flight per round
@@ -416,455 +356,6 @@ cdbg_scatter_staged_kernel(int n, long long N, long long num_classes, const uint
             for (int i = threadIdx.x; i < nbins; i += kStageThreads) { counts[i] = 0; cursor[i] = 0; }
             if (threadIdx.x == 0) *fs.ticket = 0;
         }
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------
-// 4. interpreter
-// ---------------------------------------------------------------------------------------------------------
-// Per-event state block: offsets below `cap` live in shared memory ([offset][event], event fastest); with SPILL
-// the rest (the highest popcount levels, which are read least often) lives in an L2-resident global slab owned by
-// the block, accessed with .cg loads/stores (no stale L1 lines).
-// element of the state: one complex double (double2) or, for the all-real arithmetic of the continuous states with
-// real polarisations, one double
-template <class S> struct StateElem;
-template <> struct StateElem<cx> {
-    using T = double2;
-    static __device__ __forceinline__ cx get(double2 v) { return mk(v.x, v.y); }
-    static __device__ __forceinline__ double2 put(cx v) { return make_double2(v.re, v.im); }
-};
-template <> struct StateElem<double> {
-    using T = double;
-    static __device__ __forceinline__ double get(double v) { return v; }
-    static __device__ __forceinline__ double put(double v) { return v; }
-};
-
-template <int EPW, bool SPILL, class S>
-struct StateRef {
-    using T = typename StateElem<S>::T;
-    T* base;
-    T* spill;
-    int cap;
-    __device__ __forceinline__ S ld(int o) const {
-        if (SPILL && o >= cap) return StateElem<S>::get(__ldcg(spill + (o - cap)));
-        return StateElem<S>::get(base[o * EPW]);
-    }
-    __device__ __forceinline__ void st(int o, S v) const {
-        if (SPILL && o >= cap) {
-            __stcg(spill + (o - cap), StateElem<S>::put(v));
-            return;
-        }
-        base[o * EPW] = StateElem<S>::put(v);
-    }
-    // a real 4-momentum: two complex elements, or four real ones
-    __device__ __forceinline__ void ldP(int o, double* P) const {
-        if constexpr (sizeof(T) == 16) {
-            const cx p01 = ld(o), p23 = ld(o + 1);
-            P[0] = p01.re; P[1] = p01.im; P[2] = p23.re; P[3] = p23.im;
-        } else {
-#pragma unroll
-            for (int c = 0; c < 4; c++) P[c] = ld(o + c);
-        }
-    }
-    __device__ __forceinline__ void stP(int o, const double* P) const {
-        if constexpr (sizeof(T) == 16) {
-            st(o, mk(P[0], P[1]));
-            st(o + 1, mk(P[2], P[3]));
-        } else {
-#pragma unroll
-            for (int c = 0; c < 4; c++) st(o + c, P[c]);
-        }
-    }
-};
-
-constexpr int kRing = 4;   // op ring per lane: ops are requested kRing - 1 steps before they run
-
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
-    const unsigned dst = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(gmem_src) : "memory");
-}
-
-// v or -v: flips the sign bits when m = 0x80000000 (integer pipe)
-__device__ __forceinline__ double cneg(double v, int m) {
-    return __hiloint2double(__double2hiint(v) ^ m, __double2loint(v));
-}
-__device__ __forceinline__ cx cneg(cx v, int m) {
-    return mk(__hiloint2double(__double2hiint(v.re) ^ m, __double2loint(v.re)),
-              __hiloint2double(__double2hiint(v.im) ^ m, __double2loint(v.im)));
-}
-
-__device__ __forceinline__ double shfl_xor(double v, int d) { return __shfl_xor_sync(0xFFFFFFFFu, v, d); }
-__device__ __forceinline__ cx shfl_xor(cx v, int d) {
-    return mk(__shfl_xor_sync(0xFFFFFFFFu, v.re, d), __shfl_xor_sync(0xFFFFFFFFu, v.im, d));
-}
-
-__device__ __forceinline__ int hi_word(cx v) { return __double2hiint(v.re); }
-__device__ __forceinline__ int hi_word(double v) { return __double2hiint(v); }
-
-__device__ __forceinline__ EventHeader ld_header(const char* h) {
-    const uint4 v = __ldcg(reinterpret_cast<const uint4*>(h));   // streamed once: not through L1
-    EventHeader r;
-    r.event = v.x; r.cls = v.y; r.perm = (uint64_t)v.z | ((uint64_t)v.w << 32);
-    return r;
-}
-
-template <int G, bool SPILL, class S>
-__global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgParams p) {
-    // G <= 32: one warp per block, EPW = 32/G events per warp.  G > 32: one event per block of G threads.
-    // S: complex currents (cx) or, for continuous states with real polarisations, real ones (double).
-    constexpr int EPW = G >= 32 ? 1 : 32 / G;
-    using T = typename StateElem<S>::T;
-    extern __shared__ double2 smem_raw[];
-    T* const smem = reinterpret_cast<T*>(smem_raw);
-    const int lane = threadIdx.x;
-    const int q = lane % EPW, g = lane / EPW;
-    constexpr int kBlock = G > 32 ? G : 32;
-    constexpr bool kUseRing = G >= 8;
-    constexpr bool kEarlyRing = kUseRing && G <= 64;   // op read from the ring one step ahead (G >= 128: measured 1 % slower)
-    // [kRing][kBlock] behind the state slab (rounded up to 16 bytes)
-    uint4* const ring = reinterpret_cast<uint4*>(smem_raw + ((size_t)p.slab_cx * EPW * sizeof(T) + 15) / 16) + lane;
-    StateRef<EPW, SPILL, S> st_;
-    st_.base = smem + q;
-    st_.spill = SPILL ? reinterpret_cast<T*>(p.spill) + (size_t)blockIdx.x * p.spill_cx : nullptr;
-    st_.cap = p.slab_cx;
-    const long long first = p.bounds[p.tier], end = p.bounds[p.tier + 1];
-    const long long ntasks = (end - first + EPW - 1) / EPW;
-    const long long N = p.N;
-    const int n = p.n;
-    // lanes of one event (same q) run the same program and meet at its barriers; events of different classes in
-    // one warp pass different numbers of barriers, so the barrier names only the event's own lanes
-    unsigned evmask = 0;
-#pragma unroll
-    for (int i = 0; i < (G < 32 ? G : 32); i++) evmask |= 1u << (q + i * EPW);
-
-    // the header of a task is loaded one task ahead; the inputs of the next task are prefetched into L2 while
-    // the current one computes (events come in class order, so their rows are scattered over the input arrays)
-    EventHeader hnext;
-    hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
-    if ((long long)blockIdx.x < ntasks) {
-        const long long idx = first + (long long)blockIdx.x * EPW + q;
-        if (idx < end) hnext = ld_header(p.rec + (size_t)idx * p.rec_bytes);
-    }
-    // carried from one task to the next: the class info of the next event, requested at the first barrier of the
-    // current task (one load less in the chain header -> info -> ops -> inputs at the start of a task)
-    uint4 ci_next = make_uint4(0, 0, 0, 0);
-    bool ci_next_ok = false;
-    for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
-        const long long idx = first + task * EPW + q;
-        const bool have = idx < end;
-        const EventHeader h = hnext;
-        long long idx_next = 0;
-        {
-            const long long idx2 = idx + (long long)gridDim.x * EPW;
-            hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
-            idx_next = idx2;
-            if (task + gridDim.x < ntasks && idx2 < end) hnext = ld_header(p.rec + (size_t)idx2 * p.rec_bytes);
-        }
-        const long long e = h.event;
-        const uint32_t cls = have ? h.cls : 0xFFFFFFFFu;
-        const double* mrec = reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
-        // discrete states: the setup level gives gluon k to lane k % G, so the lane's first momentum is requested
-        // here, ahead of the dependent loads class info -> ops that the setup ops themselves wait for
-        const bool discrete = !kUseRing && p.rec_gstride == 4 && sizeof(T) == 16;   // (G >= 8: measured 1-2 % slower)
-        double pk[4] = {0.0, 0.0, 0.0, 0.0};
-        if (discrete && g < n) {
-#pragma unroll
-            for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + g * 4 + c);
-        }
-        uint4 ci = ci_next;
-        if (!ci_next_ok) ci = __ldg(reinterpret_cast<const uint4*>(p.info + (cls == 0xFFFFFFFFu ? 0 : cls)));
-        ci_next_ok = false;
-        const bool valid = cls != 0xFFFFFFFFu && ((ci.y >> 24) & 0xFF);
-        const uint64_t perm = h.perm;
-        const ProgOp* ops = p.ops + ci.x + g;
-        const int total = valid ? (int)ci.z : 0;
-        bool prefetched = false;
-
-        S amp = s_zero<S>();
-        S acc[4], tacc[6];
-        double Pt[4];
-#pragma unroll
-        for (int c = 0; c < 4; c++) { acc[c] = s_zero<S>(); Pt[c] = 0.0; }
-#pragma unroll
-        for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
-
-        // The lane's ops travel global -> shared by cp.async, kRing - 1 steps ahead, into a private ring (no
-        // registers are held across the latency and nothing else reads these slots); the table ends with spare rows.
-        // With few lanes per event (G <= 4) the program of a class is small and stays in L1: plain loads, two steps
-        // ahead, are cheaper there.
-        auto first_barrier_done = [&]() {
-            prefetched = true;
-            if (hnext.cls != 0xFFFFFFFFu) {
-                // the next event's record (a few 128-byte lines) is pulled into L2 meanwhile
-                for (int k = g * 128; k < p.rec_bytes; k += G * 128)
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(p.rec + (size_t)idx_next * p.rec_bytes + k));
-                if constexpr (kUseRing) {      // (G <= 4: measured neutral to slightly slower)
-                    ci_next = __ldg(reinterpret_cast<const uint4*>(p.info + hnext.cls));
-                    ci_next_ok = true;
-                }
-            }
-        };
-        const int s0 = (discrete && total > 0) ? (n + G - 1) / G : 0;     // steps of the setup level done up front
-        uint4 r0 = make_uint4(0, 0, 0, 0), r1 = r0;
-        if constexpr (kUseRing) {
-            if (total > 0) {
-#pragma unroll
-                for (int i = 0; i < kRing - 1; i++) {
-                    cp_async16(ring + ((s0 + i) % kRing) * kBlock, ops + (size_t)(s0 + i) * G);
-                    asm volatile("cp.async.commit_group;" ::: "memory");
-                }
-                if constexpr (kEarlyRing) {
-                    asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 2) : "memory");
-                    r0 = ring[(s0 % kRing) * kBlock];
-                }
-            }
-        } else {
-            r0 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s0 * G));
-            r1 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)(s0 + 1) * G));
-        }
-        if constexpr (sizeof(T) == 16) {
-            // setup level (discrete states): external currents eps(p_k, lambda_k) and momenta, Eq. 20 / g1-g5
-            int k = g;
-            for (int s = 0; s < s0; s++) {
-                const uint4 raw = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s * G));
-                const int kn = k + G;
-                double pn[4] = {0.0, 0.0, 0.0, 0.0};
-                if (kn < n) {
-#pragma unroll
-                    for (int c = 0; c < 4; c++) pn[c] = __ldcg(mrec + kn * 4 + c);
-                }
-                if ((raw.z >> 16) & OPF_EXT) {
-                    const int kk = (int)raw.w;
-                    if (kk != k) {      // another dealing of the gluons than k % G: fetch what the op names
-#pragma unroll
-                        for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + kk * 4 + c);
-                    }
-                    cx eps[4];
-                    polarisation(pk, ((perm >> (48 + kk)) & 1) ? 1 : -1, eps);
-                    const int offDst = raw.y >> 16, offPt = raw.z & 0xFFFF;
-#pragma unroll
-                    for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
-                    if (offPt != 0xFFFF) st_.stP(offPt, pk);
-                }
-#pragma unroll
-                for (int c = 0; c < 4; c++) pk[c] = pn[c];
-                k = kn;
-            }
-            if (s0 > 0) {
-                if constexpr (G > 32) __syncthreads(); else __syncwarp(evmask);
-                first_barrier_done();
-            }
-        }
-        {
-            for (int s = s0; s < total; s++) {
-                uint4 raw, r2 = r1;
-                if constexpr (kUseRing) {
-                    cp_async16(ring + ((s + kRing - 1) % kRing) * kBlock, ops + (size_t)(s + kRing - 1) * G);
-                    asm volatile("cp.async.commit_group;" ::: "memory");
-                    if constexpr (kEarlyRing) {
-                        asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 2) : "memory");
-                        raw = r0;
-                        r2 = ring[((s + 1) % kRing) * kBlock];     // the next step's op leaves the ring one step early
-                    } else {
-                        asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 1) : "memory");
-                        raw = ring[(s % kRing) * kBlock];
-                    }
-                } else {
-                    raw = r0;
-                    const ProgOp* src = ops + (size_t)(s + 2) * G;
-                    r2 = __ldg(reinterpret_cast<const uint4*>(src));
-                }
-                const int offA = raw.x & 0xFFFF, offB = raw.x >> 16;
-                const int offP1 = raw.y & 0xFFFF, offDst = raw.y >> 16;
-                const int offPt = raw.z & 0xFFFF;
-                const unsigned flags = raw.z >> 16;
-                if (flags & OPF_VALID) {
-                    S a[4], b[4];
-#pragma unroll
-                    for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); b[c] = st_.ld(offB + c); }
-                    double P1[4], P2[4];
-                    st_.ldP(offP1, P1);
-                    if (flags & OPF_FIRST) {
-#pragma unroll
-                        for (int c = 0; c < 4; c++) acc[c] = s_zero<S>();
-#pragma unroll
-                        for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
-                        const int offP2 = (int)(raw.w & 0xFFFF);
-                        double Pb[4];
-                        st_.ldP(offP2, Pb);
-#pragma unroll
-                        for (int c = 0; c < 4; c++) Pt[c] = P1[c] + Pb[c];
-                    }
-#pragma unroll
-                    for (int c = 0; c < 4; c++) P2[c] = Pt[c] - P1[c];
-                    // X(a,b) is linear in the pair (a, T_a): a negative vertex flips the sign bits of that pair
-                    // (integer pipe) instead of multiplying every term by -1 on the FP64 pipe
-                    const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
-#pragma unroll
-                    for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
-                    v3_acc(acc, P1, P2, a, b, 1.0);
-                    if (flags & OPF_TENB) {
-                        S T[6];
-#pragma unroll
-                        for (int c = 0; c < 6; c++) T[c] = st_.ld(offB + 4 + c);
-                        tcontract_acc(acc, T, a, 1.0);
-                    }
-                    if (flags & OPF_TENA) {
-                        S T[6];
-#pragma unroll
-                        for (int c = 0; c < 6; c++) T[c] = cneg(st_.ld(offA + 4 + c), neg);
-                        tcontract_acc(acc, T, b, -1.0);
-                    }
-                    if (!(flags & OPF_CLOSURE)) tbuild_acc(tacc, a, b, 1.0);
-                    if (flags & OPF_PARTIAL) {
-                        // chunk of a split target: raw sums to its scratch slot, finished by a COMBINE op
-#pragma unroll
-                        for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
-#pragma unroll
-                        for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
-                    } else if (flags & OPF_LAST) {
-                        if (flags & OPF_CLOSURE) {
-                            S en[4];
-#pragma unroll
-                            for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
-                            amp = amp + kInvSqrt2 * mdot(en, acc);
-                        } else {
-                            const double f = kInvSqrt2 / mdot(Pt, Pt);
-#pragma unroll
-                            for (int c = 0; c < 4; c++) acc[c] = f * acc[c];
-#pragma unroll
-                            for (int c = 0; c < 6; c++) tacc[c] = kInvSqrt2 * tacc[c];
-                            if (!(flags & OPF_NOSTORE)) {
-#pragma unroll
-                                for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
-#pragma unroll
-                                for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
-                            }
-                            if (flags & OPF_STOREP) {
-                                st_.stP(offPt, Pt);
-                            }
-                        }
-                    }
-                } else if (flags & OPF_FUSED) {
-                    // closure vertex X(eps_k, J(pi)) . eps_n with J(pi), T(pi) still in acc / tacc, P(pi) in Pt
-                    S a[4], x[4], en[4];
-                    double P1[4];
-#pragma unroll
-                    for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); x[c] = s_zero<S>(); }
-                    st_.ldP(offP1, P1);
-                    const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
-#pragma unroll
-                    for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
-                    v3_acc(x, P1, Pt, a, acc, 1.0);
-                    tcontract_acc(x, tacc, a, 1.0);
-#pragma unroll
-                    for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
-                    amp = amp + kInvSqrt2 * mdot(en, x);
-                } else if (flags & OPF_COMBINE) {
-                    // add the offB partial sums of a split target and finish it like a LAST op
-#pragma unroll
-                    for (int c = 0; c < 4; c++) acc[c] = st_.ld(offA + c);
-#pragma unroll
-                    for (int c = 0; c < 6; c++) tacc[c] = st_.ld(offA + 4 + c);
-                    for (int r = 1; r < offB; r++) {
-#pragma unroll
-                        for (int c = 0; c < 4; c++) acc[c] = acc[c] + st_.ld(offA + 10 * r + c);
-#pragma unroll
-                        for (int c = 0; c < 6; c++) tacc[c] = tacc[c] + st_.ld(offA + 10 * r + 4 + c);
-                    }
-                    {
-                        const int offP2 = (int)(raw.w & 0xFFFF);
-                        double Pa[4], Pb[4];
-                        st_.ldP(offP1, Pa);
-                        st_.ldP(offP2, Pb);
-#pragma unroll
-                        for (int c = 0; c < 4; c++) Pt[c] = Pa[c] + Pb[c];
-                    }
-                    const double f = kInvSqrt2 / mdot(Pt, Pt);
-#pragma unroll
-                    for (int c = 0; c < 4; c++) acc[c] = f * acc[c];
-#pragma unroll
-                    for (int c = 0; c < 6; c++) tacc[c] = kInvSqrt2 * tacc[c];
-                    if (!(flags & OPF_NOSTORE)) {
-#pragma unroll
-                        for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
-#pragma unroll
-                        for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
-                    }
-                    if (flags & OPF_STOREP) {
-                        st_.stP(offPt, Pt);
-                    }
-                } else if (flags & OPF_EXTD) {
-                    // continuous states (Eq. 7, 9, 12): real polarisation e(phi) times the colour matrix etabar_h eta_g;
-                    // record per gluon: p (4), phi, eta (3), etabar (3), pad
-                    const int k = (int)raw.w;
-                    const double* gr = mrec + k * p.rec_gstride;
-                    double pk[4], ev[4], eta[3], etab[3];
-#pragma unroll
-                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(gr + c);
-                    const double phi = __ldcg(gr + 4);
-#pragma unroll
-                    for (int c = 0; c < 3; c++) { eta[c] = __ldcg(gr + 5 + c); etab[c] = __ldcg(gr + 8 + c); }
-                    polarisation_real(pk, phi, ev);
-                    const bool closure_leg = offPt == 0xFFFF;   // gluon n: no momentum slot; target (h,g) reads X_n[g][h]
-#pragma unroll
-                    for (int h = 0; h < 3; h++)
-#pragma unroll
-                        for (int gg = 0; gg < 3; gg++) {
-                            const double x = etab[h] * eta[gg];
-                            const int at = offDst + 4 * (h * 3 + gg);
-#pragma unroll
-                            for (int c = 0; c < 4; c++) st_.st(at + c, s_real<S>(x * ev[c]));
-                        }
-                    if (!closure_leg) {
-                        st_.stP(offPt, pk);
-                    }
-                } else if ((flags & OPF_EXT) && sizeof(T) == 16) {
-                    const int k = (int)raw.w;
-                    double pk[4];
-#pragma unroll
-                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + k * p.rec_gstride + c);   // not through L1: it is kept for the ops
-                    cx eps[4];
-                    polarisation(pk, ((perm >> (48 + k)) & 1) ? 1 : -1, eps);
-                    if constexpr (sizeof(T) == 16) {
-#pragma unroll
-                    for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
-                    }
-                    if (offPt != 0xFFFF) st_.stP(offPt, pk);
-                }
-                if (flags & OPF_SYNC) {
-                    // end of a level: the currents just written become visible to the lanes of the event
-                    if constexpr (G > 32) __syncthreads(); else __syncwarp(evmask);
-                    if (!prefetched) first_barrier_done();
-                }
-                {
-                    // The op requested at the top of this step must not be touched before the step ends (the
-                    // compiler would otherwise park it right behind the load with moves that wait for it): its
-                    // first use is tied to the step's last arithmetic results through an always-zero mask.
-                    const unsigned late = (unsigned)(hi_word(acc[0]) ^ hi_word(amp)) & (unsigned)p.zero;
-                    const uint4 moved = make_uint4(r2.x | late, r2.y | late, r2.z | late, r2.w | late);
-                    if constexpr (kEarlyRing) { r0 = moved; } else if constexpr (!kUseRing) { r0 = r1; r1 = moved; }
-                }
-            }
-            if constexpr (kUseRing) asm volatile("cp.async.wait_group 0;" ::: "memory");
-        }
-
-        // closure amplitude: sum of the G lanes' partial contractions (Eq. 22), then |A|^2
-#pragma unroll
-        for (int d = EPW; d < 32; d <<= 1) {
-            amp = amp + shfl_xor(amp, d);
-        }
-        if constexpr (G > 32) {
-            __shared__ double red_s[2 * (G / 32)];
-            if ((lane & 31) == 0) reinterpret_cast<S*>(red_s)[lane >> 5] = amp;
-            __syncthreads();
-            if (lane == 0) {
-                amp = s_zero<S>();
-                for (int w = 0; w < G / 32; w++) amp = amp + reinterpret_cast<S*>(red_s)[w];
-            }
-        }
-        if (g == 0 && have) p.out[e] = valid ? s_norm2(amp) : 0.0;
-        if constexpr (G > 32) __syncthreads(); else __syncwarp();
     }
 }
 
@@ -1055,6 +546,15 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
     }
+    {   // double-double re-evaluation: 32-byte state elements under the same shared-memory limit
+        const int epw = G >= 32 ? 1 : 32 / G, block = G > 32 ? G : 32;
+        const size_t ring_bytes = G >= 8 ? (size_t)kRing * block * 16 : 0;
+        if ((size_t)epw * max_state * 32 <= slab_limit) { t->dd_mode = 0; t->dd_cap_cx = std::max(16, max_state); }
+        else if (G >= 128) { t->dd_mode = 1; t->dd_cap_cx = (int)(slab_limit / 32); }
+        else { t->dd_mode = -1; t->dd_cap_cx = 0; }
+        const size_t smem0 = (size_t)epw * std::min(tiers.slab_cx[0], std::max(16, t->dd_cap_cx)) * 32 + ring_bytes;
+        t->dd_spill_blocks = (int)std::max<size_t>(1, std::min<size_t>(65536 / (255 * block), (228 * 1024) / (smem0 + 1024)));
+    }
     {   // spare rows of no-ops: the interpreter requests ops kRing - 1 steps ahead
         ProgOp nop;
         std::memset(&nop, 0, sizeof(nop));
@@ -1125,6 +625,7 @@ int prog_table_create_dense(int n, int G, size_t slab_limit, bool real, ProgTabl
     t->n = n; t->G = G; t->num_classes = 1; t->max_state_cx = cp.state_cx;
     t->dense = true;
     t->real = real;
+    t->dd_mode = -1;
     t->rec_bytes = kRecHeaderBytes + 96 * n;
     for (int k = 0; k < kTiers; k++) {
         t->tiers.slab_cx[k] = std::min<int>(cp.state_cx, (int)(slab_limit / elem));
@@ -1195,104 +696,69 @@ void prog_table_destroy(ProgTable* t) {
 
 size_t prog_state_bytes(const ProgTable* t) { return t ? (size_t)t->max_state_cx * (t->real ? 8 : 16) : 0; }
 int prog_lanes(const ProgTable* t) { return t ? t->G : 0; }
+int prog_dd_mode(const ProgTable* t) { return t ? t->dd_mode : -1; }
 
-// scratch: records (32 + 32 n) B x N | perm u64[N] | cls u32[N] | hist u32[num_classes + 1] | tier bounds | spill slabs
+// scratch: records (32 + 32 n) B x N | perm u64[N] | cls u32[N] | hist u32[num_classes + 1] | tier bounds (64 B) |
+//          flag counters (64 B) | flag lists u32[N] | spill slabs (FP64) | spill slabs (double-double re-evaluation)
+static size_t prog_flag_offset(const ProgTable* t, long long N) {
+    return ((size_t)N * (12 + t->rec_bytes) + ((size_t)t->num_classes + 1) * 4 + 15) / 16 * 16 + 64;
+}
 static size_t prog_spill_offset(const ProgTable* t, long long N) {
-    return (((size_t)N * (12 + t->rec_bytes) + ((size_t)t->num_classes + 1) * 4 + 256) + 255) / 256 * 256;
+    return (prog_flag_offset(t, N) + 64 + (size_t)N * 4 + 255) / 256 * 256;
+}
+static size_t prog_spill_bytes(const ProgTable* t) {
+    // spill kernels run a fixed number of blocks per SM, each with a slab for the largest state
+    return t->spill ? ((size_t)t->sm_count * t->spill_blocks_per_sm * t->max_state_cx * 16 + 255) / 256 * 256 : 0;
 }
 size_t prog_scratch_bytes(const ProgTable* t, long long N) {
-    // spill kernels run one block per SM, each with a slab for the part of the largest state beyond shared memory
-    const size_t spill = t->spill ? (size_t)t->sm_count * t->spill_blocks_per_sm * t->max_state_cx * 16 : 0;
-    return prog_spill_offset(t, N) + spill;
+    const size_t dd_spill = t->dd_mode == 1 ? (size_t)t->sm_count * t->dd_spill_blocks * t->max_state_cx * 32 : 0;
+    return prog_spill_offset(t, N) + prog_spill_bytes(t) + dd_spill;
 }
 
-template <int G, bool SPILL, class S = cx>
-static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched, bool conc) {
-    constexpr int EPW = G >= 32 ? 1 : 32 / G, BLOCK = G > 32 ? G : 32;
-    constexpr size_t ELEM = sizeof(typename StateElem<S>::T);
-    static int configured_device = -1;   // the attribute is per device
-    int device = 0;
-    cudaGetDevice(&device);
-    if (configured_device != device) {
-        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL, S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)(kMaxSlabBytes + (size_t)kRing * BLOCK * 16));
-        if (e != cudaSuccess) return e;
-        configured_device = device;
-    }
-    const long long max_tasks = (p.N + EPW - 1) / EPW + kTiers;
-    unsigned blocks[kTiers];
-    size_t smem[kTiers];
-    long long resident = 0;
-    int nlaunch = 0;
-    for (int k = 0; k < kTiers; k++) {
-        blocks[k] = 0;
-        if (t->tiers.first_key[k] == t->tiers.first_key[k + 1] && k + 1 < kTiers) continue;   // no class in this tier
-        const size_t ring_bytes = G >= 8 ? (size_t)kRing * BLOCK * 16 : 0;
-        smem[k] = ((size_t)EPW * t->tiers.slab_cx[k] * ELEM + 15) / 16 * 16 + ring_bytes;
-        if (smem[k] > kMaxSlabBytes + ring_bytes) return cudaErrorInvalidValue;
-        // resident blocks per SM: shared memory (1 KB reserved per block), and 65536 / (160 x BLOCK) registers
-        int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * BLOCK), (228 * 1024) / (smem[k] + 1024)));
-        if (SPILL) per_sm = std::min(per_sm, t->spill_blocks_per_sm);   // one global slab per resident block
-        blocks[k] = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
-        resident += (long long)sm_count * per_sm;
-        nlaunch++;
-    }
-    // Small batches: when the tiers together hold fewer than two tasks per resident block, each launch is mostly
-    // ramp-up and tail, so the tiers run side by side (fork / join around the caller's stream).  Measured at
-    // n = 6: 2^16 events +22 %, 2^18 neutral, 2^20 -5 %; n >= 7: slower at every size.
-    // (spill slabs are indexed by block: one launch at a time)
-    conc = conc && G <= 4 && !SPILL && t->has_streams && nlaunch > 1 && max_tasks <= 2 * resident;
-    if (conc && cudaEventRecord(t->fork_ev, s) != cudaSuccess) return cudaGetLastError();
-    int side = 0;                                 // launches sent to the side streams so far
-    bool first = true;
-    for (int k = 0; k < kTiers; k++) {
-        if (!blocks[k]) continue;
-        p.tier = k;
-        p.slab_cx = t->tiers.slab_cx[k];
-        cudaStream_t ls = s;
-        if (conc && !first) {
-            ls = t->aux[side];
-            cudaStreamWaitEvent(ls, t->fork_ev, 0);
-        }
-        cdbg_prog_kernel<G, SPILL, S><<<blocks[k], BLOCK, smem[k], ls>>>(p);
-        if (conc && !first) cudaEventRecord(t->join_ev[side++], ls);
-        first = false;
-        ++*launched;
-    }
-    for (int i = 0; i < side; i++) cudaStreamWaitEvent(s, t->join_ev[i], 0);
-    return cudaGetLastError();
+// flagged events of the most recent launch with a conditioning threshold (synchronises the stream's work first)
+cudaError_t prog_flagged_count(const ProgTable* t, long long N, const void* scratch, long long* count) {
+    uint32_t c[kTiers] = {0, 0, 0, 0};
+    const cudaError_t err = cudaMemcpy(c, (const char*)scratch + prog_flag_offset(t, N), sizeof(c), cudaMemcpyDeviceToHost);
+    *count = 0;
+    for (int k = 0; k < kTiers; k++) *count += c[k];
+    return err;
 }
+
+cudaError_t dispatch_interp_dd(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches);   // bg_cdbg_prog_dd.cu
 
 static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches,
                                    bool conc = false) {
     cudaError_t err;
+    LaunchShape shape;
+    shape.conc = conc;
+    shape.spill_blocks = t->spill_blocks_per_sm;
     if (t->real) {   // continuous states with real polarisations: all-real arithmetic
         switch (t->G) {
-            case 32: return launch_interp<32, false, double>(s, t, sm_count, p, launches, conc);
-            case 64: return launch_interp<64, false, double>(s, t, sm_count, p, launches, conc);
+            case 32: return launch_interp<32, false, double>(s, t, sm_count, p, launches, shape);
+            case 64: return launch_interp<64, false, double>(s, t, sm_count, p, launches, shape);
             case 128:
-                return t->spill ? launch_interp<128, true, double>(s, t, sm_count, p, launches, conc)
-                                : launch_interp<128, false, double>(s, t, sm_count, p, launches, conc);
+                return t->spill ? launch_interp<128, true, double>(s, t, sm_count, p, launches, shape)
+                                : launch_interp<128, false, double>(s, t, sm_count, p, launches, shape);
             default:
-                return t->spill ? launch_interp<256, true, double>(s, t, sm_count, p, launches, conc)
-                                : launch_interp<256, false, double>(s, t, sm_count, p, launches, conc);
+                return t->spill ? launch_interp<256, true, double>(s, t, sm_count, p, launches, shape)
+                                : launch_interp<256, false, double>(s, t, sm_count, p, launches, shape);
         }
     }
     switch (t->G) {
-        case 1: err = launch_interp<1, false>(s, t, sm_count, p, launches, conc); break;
-        case 2: err = launch_interp<2, false>(s, t, sm_count, p, launches, conc); break;
-        case 4: err = launch_interp<4, false>(s, t, sm_count, p, launches, conc); break;
-        case 8: err = launch_interp<8, false>(s, t, sm_count, p, launches, conc); break;
-        case 16: err = launch_interp<16, false>(s, t, sm_count, p, launches, conc); break;
-        case 32: err = launch_interp<32, false>(s, t, sm_count, p, launches, conc); break;
-        case 64: err = launch_interp<64, false>(s, t, sm_count, p, launches, conc); break;
+        case 1: err = launch_interp<1, false>(s, t, sm_count, p, launches, shape); break;
+        case 2: err = launch_interp<2, false>(s, t, sm_count, p, launches, shape); break;
+        case 4: err = launch_interp<4, false>(s, t, sm_count, p, launches, shape); break;
+        case 8: err = launch_interp<8, false>(s, t, sm_count, p, launches, shape); break;
+        case 16: err = launch_interp<16, false>(s, t, sm_count, p, launches, shape); break;
+        case 32: err = launch_interp<32, false>(s, t, sm_count, p, launches, shape); break;
+        case 64: err = launch_interp<64, false>(s, t, sm_count, p, launches, shape); break;
         case 128:
-            err = t->spill ? launch_interp<128, true>(s, t, sm_count, p, launches, conc)
-                           : launch_interp<128, false>(s, t, sm_count, p, launches, conc);
+            err = t->spill ? launch_interp<128, true>(s, t, sm_count, p, launches, shape)
+                           : launch_interp<128, false>(s, t, sm_count, p, launches, shape);
             break;
         default:
-            err = t->spill ? launch_interp<256, true>(s, t, sm_count, p, launches, conc)
-                           : launch_interp<256, false>(s, t, sm_count, p, launches, conc);
+            err = t->spill ? launch_interp<256, true>(s, t, sm_count, p, launches, shape)
+                           : launch_interp<256, false>(s, t, sm_count, p, launches, shape);
             break;
     }
     return err;
@@ -1300,13 +766,16 @@ static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_co
 
 cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
                              const signed char* hel, const signed char* col, double* out, void* scratch,
-                             int* launches, cudaEvent_t ev0, cudaEvent_t ev1) {
+                             int* launches, cudaEvent_t ev0, cudaEvent_t ev1, double tau, double tau_rho, cudaEvent_t ev_mid) {
+    if (tau > 0.0 && t->dd_mode < 0) return cudaErrorNotSupported;
     const int rec_bytes = t->rec_bytes;
     char* rec = (char*)scratch;
     uint64_t* perm = (uint64_t*)(rec + (size_t)N * rec_bytes);
     uint32_t* cls = (uint32_t*)(perm + N);
     uint32_t* hist = cls + N;
     uint32_t* bounds = hist + ((size_t)t->num_classes + 1);
+    uint32_t* flag_count = (uint32_t*)((char*)scratch + prog_flag_offset(t, N));
+    uint32_t* flag_list = flag_count + 16;
     const int nbins = (int)t->num_classes + 1;
     cudaError_t err = cudaSuccess;
     const unsigned eb = (unsigned)((N + kPreEvents - 1) / kPreEvents);
@@ -1331,7 +800,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         // of the large-batch kernels, and each thread is a chain of dependent loads and atomics
         const unsigned cb = (unsigned)((N + kSmallThreads - 1) / kSmallThreads);
         cdbg_classify_kernel<true, kSmallThreads, 1><<<cb, kSmallThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
-                                                                                     t->d_sortkey, cls, perm, counts);
+                                                                                     t->d_sortkey, cls, perm, counts, flag_count);
         const unsigned sb = (unsigned)((N + kStageThreads - 1) / kStageThreads);
         cdbg_scatter_staged_kernel<true, 1><<<sb, kStageThreads, 2 * hist_words * sizeof(uint32_t) + stage_bytes, s>>>(
             t->n, N, t->num_classes, cls, perm, t->d_sortkey, mom, hel, counts + nbins, rec, rec_bytes, fs);
@@ -1346,7 +815,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
             configured_device = device;
         }
         cdbg_classify_kernel<true><<<eb, kPreThreads, hist_smem, s>>>(t->n, N, t->num_classes, col, t->d_info,
-                                                                      t->d_sortkey, cls, perm, hist);
+                                                                      t->d_sortkey, cls, perm, hist, flag_count);
         cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins, t->tiers, bounds, (uint32_t)N);
         const size_t stage_smem = (((size_t)nbins + 3) & ~(size_t)3) * sizeof(uint32_t) +
                                   (size_t)(kStageThreads / 32) * (32 * (rec_bytes + 16) + 256);
@@ -1360,7 +829,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         }
     } else {
         cdbg_classify_kernel<false><<<eb, kPreThreads, 0, s>>>(t->n, N, t->num_classes, col, t->d_info, t->d_sortkey,
-                                                               cls, perm, hist);
+                                                               cls, perm, hist, flag_count);
         cdbg_scan_kernel<<<1, 1024, 0, s>>>(hist, nbins, t->tiers, bounds, (uint32_t)N);
         cdbg_scatter_kernel<false><<<eb, kPreThreads, 0, s>>>(t->n, N, t->num_classes, cls, perm, t->d_sortkey, mom, hel, hist,
                                                               rec, rec_bytes);
@@ -1375,9 +844,24 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.spill_cx = t->max_state_cx;
     p.tier = 0;
     p.slab_cx = t->max_state_cx;
+    p.tau2 = tau < 0.0 ? tau : tau * tau;
+    p.tau_rho = tau_rho;
+    p.flag_list = flag_list;
+    p.flag_count = flag_count;
+    p.list = nullptr;
+    p.list_count = nullptr;
     *launches = fused ? 2 : 3;
     if (ev0) cudaEventRecord(ev0, s);
     err = dispatch_interp(s, t, sm_count, p, launches, true);
+    if (tau > 0.0 && err == cudaSuccess) {
+        // the flagged events of every tier once more, in double-double arithmetic (overwrites their out[])
+        if (ev_mid) cudaEventRecord(ev_mid, s);
+        p.tau2 = 0.0;
+        p.list = flag_list;
+        p.list_count = flag_count;
+        p.spill = t->dd_mode == 1 ? (double2*)((char*)scratch + prog_spill_offset(t, N) + prog_spill_bytes(t)) : nullptr;
+        err = dispatch_interp_dd(s, t, sm_count, p, launches);
+    }
     if (ev1) cudaEventRecord(ev1, s);
     return err;
 }
@@ -1400,6 +884,9 @@ cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, 
     p.spill_cx = t->max_state_cx;
     p.tier = 0;
     p.slab_cx = t->max_state_cx;
+    p.tau2 = 0.0;
+    p.tau_rho = 0.0;
+    p.flag_list = nullptr; p.flag_count = nullptr; p.list = nullptr; p.list_count = nullptr;
     *launches = 1;
     if (ev0) cudaEventRecord(ev0, s);
     err = dispatch_interp(s, t, sm_count, p, launches, false);

@@ -56,6 +56,10 @@ struct CobgParams {
     const uint32_t* cidx4;            // compressed colour matrix (nval > 0), else C is read as doubles
     int nval;
     double cval[kCobgMaxVals];
+    // conditioning flag (given helicities, full colour; BG_OPT_PRECISION = 2): Ward residual of the closing currents
+    double tau2;                      // 0: off; < 0: diagnostic, `out` receives the residual
+    uint32_t* flag_list;              // [N] event ids
+    uint32_t* flag_count;             // [1]
 };
 
 
@@ -265,6 +269,7 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
             __syncthreads();
         }
         // register-resident top: thread sigma builds the two (n-2)-gluon currents and the final one of its ordering
+        double ward2 = 0.0, amp2 = 0.0;
         if (top) {
             tv.template range<1, M - 1, true>(tv.JA);
             tv.template range<0, M - 2, true>(tv.JB);
@@ -274,6 +279,12 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
             const cx amp = mdot(en, JF);
             A[2 * t] = amp.re;
             A[2 * t + 1] = amp.im;
+            if (!LC && p.tau2 != 0.0) {
+                // Ward identity: the current of gluons 1..n-1 is conserved, P . J = 0 with P = -p_n (round-off only)
+                const cx wv = mdot(P + 4 * (NSUB - 1), JF);
+                ward2 = s_norm2(wv);
+                amp2 = s_norm2(amp);
+            }
         }
         __syncthreads();
         // Eq. 16: row sigma of the real symmetric quadratic form
@@ -330,6 +341,26 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
             for (int i = 0; i < TPE / 32; i++) w += red[i];
         }
         total += w;
+        if (!LC && p.tau2 != 0.0) {
+            // sum over the orderings of |P . J_sigma|^2 against E_n^2 sum |A_sigma|^2
+#pragma unroll
+            for (int d = 1; d < (TPE < 32 ? TPE : 32); d <<= 1) {
+                ward2 += __shfl_xor_sync(0xFFFFFFFFu, ward2, d);
+                amp2 += __shfl_xor_sync(0xFFFFFFFFu, amp2, d);
+            }
+            if (TPE > 32) {
+                __syncthreads();
+                if ((t & 31) == 0) { red[t >> 5] = ward2; red[4 + (t >> 5)] = amp2; }
+                __syncthreads();
+                ward2 = 0.0; amp2 = 0.0;
+                for (int i = 0; i < TPE / 32; i++) { ward2 += red[i]; amp2 += red[4 + i]; }
+            }
+            if (t == 0 && active) {
+                const double En = p.mom[(size_t)(M * 4) * N + e];
+                if (p.tau2 < 0.0) total = ::sqrt(ward2 / (En * En * amp2));
+                else if (!(ward2 <= p.tau2 * En * En * amp2) || !(w > 0.0)) p.flag_list[atomicAdd(p.flag_count, 1u)] = (uint32_t)e;
+            }
+        }
     }
     }   // last
     if (LC) total *= p.lc_factor;
@@ -474,8 +505,12 @@ static cudaError_t launch_cobg(cudaStream_t s, const CobgParams& p) {
 }
 
 cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, bool lc, const double* dC, long long N,
-                               const double* mom, const signed char* hel, double* out) {
+                               const double* mom, const signed char* hel, double* out, double tau, uint32_t* flag_list,
+                               uint32_t* flag_count) {
     CobgParams p;
+    p.tau2 = (helsum || lc || !flag_list) && tau >= 0.0 ? 0.0 : (tau < 0.0 ? -1.0 : tau * tau);
+    if (helsum || lc) p.tau2 = 0.0;
+    p.flag_list = flag_list; p.flag_count = flag_count;
     p.n = t->n; p.np = t->np; p.nslots = t->nslots; p.helsum = helsum ? 1 : 0;
     p.lc = lc ? 1 : 0;
     p.lc_factor = 8.0;

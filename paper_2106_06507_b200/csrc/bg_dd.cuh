@@ -21,7 +21,7 @@ __device__ __forceinline__ dd two_sum(double a, double b) {
     return mkdd(s, (a - (s - bb)) + (b - bb));
 }
 __device__ __forceinline__ dd two_prod(double a, double b) {
-    const double p = a * b;
+    const double p = __dmul_rn(a, b);   // never contracted into an FMA with a later addition
     return mkdd(p, fma(a, b, -p));
 }
 __device__ __forceinline__ dd operator+(dd a, dd b) {

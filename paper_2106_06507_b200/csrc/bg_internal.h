@@ -38,7 +38,13 @@ struct bg_ctx {
     bg::CobgTable* cobg;       // sequence tables of the shared-current COBG kernel (n <= 7)
     int prog_lanes;            // BG_OPT_LANES (0 = automatic)
     size_t slab_limit;         // BG_OPT_SMEM_LIMIT (0 = all of shared memory)
-    int precision;             // BG_OPT_PRECISION: 0 = FP64, 1 = double-double reference path (CDBG, given colours)
+    int precision;             // BG_OPT_PRECISION: 0 = FP64, 1 = every event in double-double, 2 = FP64 + double-double
+                               // re-evaluation of the events the conditioning flag names (default where available)
+    double tau;                // BG_OPT_FLAG_THRESHOLD: Ward-residual threshold of the conditioning flag
+    double tau_rho;            // ... and its threshold for the cancellation among the closure contributions
+    cudaEvent_t ev_mid;        // (timing) between the FP64 launches and the re-evaluation
+    long long last_N;          // events of the most recent bg_eval (for bg_last_refined)
+    bool last_auto;            // ... and whether it ran with the conditioning flag
     // bookkeeping
     int timing;                // BG_OPT_TIMING
     cudaEvent_t ev0, ev1;
@@ -64,6 +70,9 @@ cudaError_t cdbg_dd_launch(cudaStream_t s, int n, long long N, long long first, 
                            const signed char* hel, const signed char* col, double* out, void* scratch);
 
 size_t cobg_dd_scratch_per_event(int n, bool helsum);
+// the events list[0 .. *count) (device) once more in double-double: one block per event, amplitudes in shared memory
+cudaError_t cobg_dd_flagged_launch(cudaStream_t s, int n, int nperm, const double* dC, long long N, const uint32_t* list,
+                                   const uint32_t* count, int blocks, const double* mom, const signed char* hel, double* out);
 cudaError_t cobg_dd_launch(cudaStream_t s, int n, bool helsum, int nperm, const double* dC, long long N, long long first,
                            long long count, const double* mom, const signed char* hel, double* out, void* scratch);
 
@@ -75,9 +84,13 @@ void prog_table_destroy(ProgTable* t);
 size_t prog_state_bytes(const ProgTable* t);               // largest per-event state block
 int prog_lanes(const ProgTable* t);
 size_t prog_scratch_bytes(const ProgTable* t, long long N);
+// tau > 0: events whose Ward residual exceeds tau are evaluated again in double-double arithmetic (ev_mid, if given,
+// is recorded between the FP64 launches and that re-evaluation)
 cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
                              const signed char* hel, const signed char* col, double* out, void* scratch,
-                             int* launches, cudaEvent_t ev0, cudaEvent_t ev1);
+                             int* launches, cudaEvent_t ev0, cudaEvent_t ev1, double tau, double tau_rho, cudaEvent_t ev_mid);
+cudaError_t prog_flagged_count(const ProgTable* t, long long N, const void* scratch, long long* count);
+int prog_dd_mode(const ProgTable* t);   // 0 / 1: re-evaluation available (1: with spill); -1: state does not fit
 
 cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
                               const double* phi, const double* eta, double* out, void* scratch, int* launches,
@@ -89,8 +102,10 @@ int cobg_table_create(int n, CobgTable** out);              // BG_* code
 void cobg_table_destroy(CobgTable* t);
 int cobg_table_set_colour(CobgTable* t, const double* hC);   // optional: compressed colour matrix for the colour form
 size_t cobg_shared_current_bytes(const CobgTable* t);
+// tau != 0 (given helicities, full colour): flag list of the events whose Ward residual exceeds tau (tau < 0: diagnostic)
 cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, bool lc, const double* dC, long long N,
-                               const double* mom, const signed char* hel, double* out);
+                               const double* mom, const signed char* hel, double* out, double tau = 0.0,
+                               uint32_t* flag_list = nullptr, uint32_t* flag_count = nullptr);
 
 // ---- colour matrix (bg_colour.cpp part of bg_api.cu) ------------------------------------------------------
 int build_colour_matrix(int n, double* C /* (n-2)!^2 */);

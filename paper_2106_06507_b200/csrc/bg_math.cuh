@@ -66,7 +66,7 @@ __device__ __forceinline__ void polarisation(const double* p, int lambda, cx* ep
     const double s = p[0] < 0.0 ? -1.0 : 1.0;
     const double qx = s * p[1], qy = s * p[2], qz = s * p[3];
     const double qt2 = qx * qx + qy * qy;
-    const double qt = sqrt(qt2), qa = sqrt(qt2 + qz * qz);
+    const double qt = ::sqrt(qt2), qa = ::sqrt(qt2 + qz * qz);
     double e1x, e1y, e1z, e2x, e2y;
     if (qt < 1e-9 * qa) {
         e1x = 1.0; e1y = 0.0; e1z = 0.0;
@@ -89,7 +89,7 @@ __device__ __forceinline__ void polarisation_real(const double* p, double phi, d
     const double s = p[0] < 0.0 ? -1.0 : 1.0;
     const double qx = s * p[1], qy = s * p[2], qz = s * p[3];
     const double qt2 = qx * qx + qy * qy;
-    const double qt = sqrt(qt2), qa = sqrt(qt2 + qz * qz);
+    const double qt = ::sqrt(qt2), qa = ::sqrt(qt2 + qz * qz);
     double e1x, e1y, e1z, e2x, e2y;
     if (qt < 1e-9 * qa) {
         e1x = 1.0; e1y = 0.0; e1z = 0.0;

@@ -2,7 +2,8 @@
 import numpy as np
 
 
-def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None, lanes=None, smem_limit=None, precision=None):
+def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None, lanes=None, smem_limit=None, precision=None,
+             flag_threshold=None):
     """ev: workload.Events (AoS numpy).  Returns out[N] (numpy) and the kernel name used."""
     import torch
     import paper_2106_06507_b200 as bg
@@ -23,10 +24,12 @@ def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None, lanes=None, sme
                     import pytest
                     pytest.skip(f"{lanes} lanes per event: one warp's state exceeds shared memory for n={n}")
                 raise
-        if precision is not None:
-            bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, precision)
         if smem_limit is not None:
             bg.bg_set_option(ctx, bg.BG_OPT_SMEM_LIMIT, smem_limit)
+        if precision is not None:
+            bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, precision)
+        if flag_threshold is not None:
+            bg.bg_set_option(ctx, bg.BG_OPT_FLAG_THRESHOLD, flag_threshold)
         if scratch_limit:
             bg.bg_set_option(ctx, bg.BG_OPT_SCRATCH_LIMIT, scratch_limit)
         if host:

@@ -81,3 +81,13 @@ def test_host_colour_matrix_n8_properties(bg):
     assert np.all(np.diag(C) == 6 ** 6 * 8)
     assert np.all(C == np.rint(C))
     assert np.linalg.eigvalsh(C).min() > -1e-6 * C[0, 0]
+    # C_{sigma sigma'} depends only on sigma^-1 sigma' (relabelling the summed colours): every row is a permutation of
+    # the first, checked here on a sample of rows against explicitly composed permutations
+    import itertools
+    perms = list(itertools.permutations(range(6)))
+    index = {p: i for i, p in enumerate(perms)}
+    for s in (1, 17, 333, 719):
+        inv = np.argsort(perms[s])
+        for t in (0, 5, 100, 718):
+            rel = tuple(int(inv[perms[t][i]]) for i in range(6))
+            assert C[s, t] == C[0, index[rel]]

@@ -90,4 +90,4 @@ def test_generated_events_feed_the_evaluation(bg, oracle, wl):
     col = np.ascontiguousarray(np.transpose(d_col.cpu().numpy(), (2, 0, 1)))
     truth = oracle.cdbg(mom, hel, col, prec="long double")
     err = np.abs(d_out.cpu().numpy() - truth) / truth
-    assert np.median(err) < 1e-14 and np.mean(err > 1e-11) < 0.01
+    assert np.median(err) < 1e-14 and err.max() <= 1e-11, f"max {err.max():.2e}"

@@ -1,13 +1,15 @@
 """Parity of the CUDA path (through the C-ABI) with the CPU oracle on the same seeded events.
 
-Tolerances: truth = the oracle in long double.  Helicity-summed full colour: relative
-error <= 1e-11 on every event.  Colour-dressed, single colour flow: <= 1e-11 on every event, except where FP64
-arithmetic itself cannot deliver it: single-flow amplitudes have near-zeros by cancellation (gauge cancellations
-between splits, cancellations between colour orderings), where the double-precision oracle misses 1e-11 as well
-(0.13 % of n = 6 events).  For an event over 1e-11 the test measures that event's FP64 noise floor with the
-oracle itself (double precision, gluons relabelled 16 ways: same mathematical value, different summation order)
-and requires e_gpu <= 10 x floor.  The same rule covers the given-helicity full-colour mode, whose kinematic near-zeros
-put 9 of 16384 n = 7 events of the double-precision oracle itself above 1e-11."""
+Bar: truth = the oracle in long double; relative error <= 1e-11 on EVERY event, no tail
+clause, for the library's default path: FP64 kernels + per-event conditioning flag + double-double re-evaluation of
+the flagged events (BG_OPT_PRECISION = 2, the default of BG_CDBG_GIVEN and BG_COBG_HELGIVEN_FULLCOLOR; the helicity-
+summed full-colour mode passes in plain FP64).  Single-colour-flow and single-helicity amplitudes have near-zeros
+(helicity-suppressed configurations, cancellations between orderings) where FP64 round-off alone exceeds 1e-11 on
+~0.15 % of the events - for the double-precision oracle as well.
+
+Tests that pin a kernel variant to FP64 ONLY (BG_OPT_PRECISION = 0: lane-count sweeps, the generic kernels, CO_MC,
+continuous states) use `check_fp64_floor` instead: <= 1e-11 except where the event's own FP64 noise floor - the
+double-precision oracle with the gluons relabelled 16 ways - is above it, and then within 10 x that floor."""
 import numpy as np
 import pytest
 
@@ -40,8 +42,20 @@ def fp64_noise_floor(oracle, ev, truth, cdbg, reps=16, seed=7):
     return floor
 
 
-def check_parity(oracle, ev, got, cdbg, max_tail_frac=0.01):
-    """<= 1e-11 against the long-double truth on every event, except inside the event's own FP64 noise floor."""
+def check_parity(oracle, ev, got, cdbg):
+    """<= 1e-11 against the long-double truth on every event (the default, flag-and-re-evaluate path)."""
+    if cdbg:
+        truth = oracle.cdbg(ev.mom, ev.hel, ev.col, prec="long double")
+    else:
+        truth = oracle.cobg_full_colour(ev.mom, ev.hel, prec="long double")
+    assert np.all(truth > 0)
+    err = rel_err(got, truth)
+    assert err.max() <= 1e-11, f"{np.sum(err > 1e-11)} of {ev.N} events over 1e-11, max {err.max():.2e} at {err.argmax()}"
+    return err
+
+
+def check_fp64_floor(oracle, ev, got, cdbg, max_tail_frac=0.01):
+    """FP64-only kernels: <= 1e-11 against the long-double truth except inside the event's own FP64 noise floor."""
     if cdbg:
         truth = oracle.cdbg(ev.mom, ev.hel, ev.col, prec="long double")
     else:
@@ -58,8 +72,12 @@ def check_parity(oracle, ev, got, cdbg, max_tail_frac=0.01):
     return err, tail
 
 
-def check_cdbg(oracle, ev, got, max_tail_frac=0.01):
-    return check_parity(oracle, ev, got, True, max_tail_frac)
+def check_cdbg(oracle, ev, got):
+    return check_parity(oracle, ev, got, True)
+
+
+def check_cdbg_fp64(oracle, ev, got, max_tail_frac=0.01):
+    return check_fp64_floor(oracle, ev, got, True, max_tail_frac)
 
 
 def test_config1_n4_helsum_closed_form(bg, oracle, wl):
@@ -86,6 +104,29 @@ def test_cobg_given_helicity_full_colour(bg, oracle, wl, n, N):
     ev = wl.config_events(4, N=N, n=n)          # momenta + helicities of the sweep stream; colours ignored
     got, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR)
     check_parity(oracle, ev, got, False)
+    fp64, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR, precision=0)
+    check_fp64_floor(oracle, ev, fp64, False)
+
+
+def test_cobg_full_colour_n8_generic_kernel(bg, oracle, wl):
+    """n = 8 (720 orderings, 720 x 720 colour matrix) runs on the thread-per-event kernel in FP64.  Truth: the
+    oracle's 720 colour-ordered amplitudes in long double contracted with Eq. 17's matrix; the oracle's own
+    Gell-Mann construction of that matrix is out of reach at n = 8 (8^8-component vectors), so the matrix is the
+    product's here - equal to the oracle's for n <= 7 (test_abi, test_device_colour_matrix_equals_oracle) and
+    checked structurally at n = 8 in tests/test_abi.py."""
+    import itertools
+    ev = wl.config_events(4, N=6, n=8)
+    got, name = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR)
+    assert name == "cobg_generic_kernel"
+    C = bg.bg_build_colour_matrix(8).astype(np.longdouble)
+    perms = list(itertools.permutations(range(1, 7)))
+    truth = np.zeros(ev.N)
+    for e in range(ev.N):
+        a = np.array([oracle.cobg_amp(ev.mom[e], ev.hel[e], np.array((0,) + s + (7,), dtype=np.int32), prec="long double")
+                      for s in perms])
+        ar, ai = a.real.astype(np.longdouble), a.imag.astype(np.longdouble)
+        truth[e] = float(ar @ C @ ar + ai @ C @ ai)
+    assert rel_err(got, truth).max() <= 1e-11
 
 
 def test_config3_n7_full_size_sampled(bg, oracle, wl):
@@ -93,7 +134,7 @@ def test_config3_n7_full_size_sampled(bg, oracle, wl):
     got, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR)
     assert np.all(np.isfinite(got)) and np.all(got > 0)
     idx = np.arange(0, ev.N, 127)
-    err, tail = check_parity(oracle, ev.take(idx), got[idx], False, max_tail_frac=0.003)
+    err = check_parity(oracle, ev.take(idx), got[idx], False)
     assert np.median(err) < 1e-14
 
 
@@ -107,15 +148,17 @@ def test_cdbg_sweep_small(bg, oracle, wl, n, N):
 
 def test_config2_n6_full_size_all_events(bg, oracle, wl):
     ev = wl.config_events(1)                      # 2^20 events
-    got, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
-    err, tail = check_cdbg(oracle, ev, got, max_tail_frac=0.003)
+    got, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)      # default: FP64 + conditioning flag + double-double re-evaluation
+    err = check_cdbg(oracle, ev, got)             # every one of the 2^20 events within 1e-11
     assert np.median(err) < 1e-14 and np.percentile(err, 99) < 2e-12
-    # the same 2^20 events through the double-double reference path: every single one within 1e-11 of the truth
+    # the same 2^20 events through the all-double-double reference path
     exact, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, precision=1)
     truth = oracle.cdbg(ev.mom, ev.hel, ev.col, prec="long double")
     assert name == "cdbg_dd_kernel" and rel_err(exact, truth).max() <= 1e-11
-    # and the FP64 kernels deviate from it only where the oracle's own FP64 evaluation does
-    assert np.mean(rel_err(got, exact) > 1e-11) < 0.003
+    # and the FP64 kernels alone deviate from it only on the conditioning-limited tail the flag is there for
+    fp64, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, precision=0)
+    assert np.mean(rel_err(fp64, exact) > 1e-11) < 0.003
+    check_cdbg_fp64(oracle, ev, fp64, max_tail_frac=0.003)
 
 
 def test_config4_n9_full_size_sampled(bg, oracle, wl):
@@ -126,13 +169,59 @@ def test_config4_n9_full_size_sampled(bg, oracle, wl):
     check_cdbg(oracle, ev.take(idx), got[idx])
 
 
+def test_conditioning_flag_reports_and_options(bg, oracle, wl):
+    """BG_OPT_PRECISION = 2 bookkeeping: bg_last_refined counts the re-evaluated events; thresholds are options; the
+    diagnostics (3: Ward residual, 4: cancellation ratio) return the flag quantities; 0 switches the flag off."""
+    import torch
+    ev = wl.config_events(1, N=30000)
+    dev = torch.device("cuda:0")
+    d = [torch.from_numpy(x).to(dev) for x in (wl.to_soa(mom=ev.mom), wl.to_soa(hel=ev.hel), wl.to_soa(col=ev.col))]
+    out = torch.zeros(ev.N, dtype=torch.float64, device=dev)
+    st = torch.cuda.current_stream().cuda_stream
+    ctx = bg.bg_init(6, bg.BG_CDBG_GIVEN)
+    try:
+        res = {}
+        for prec in (2, 0, 3, 4):
+            bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, prec)
+            bg.bg_eval(ctx, st, ev.N, *d, out)
+            torch.cuda.synchronize()
+            res[prec] = (out.cpu().numpy(), bg.bg_last_refined(ctx)[0], bg.bg_last_launch_count(ctx))
+        assert 0 < res[2][1] < 0.15 * ev.N and res[0][1] == 0
+        assert res[2][2] > res[0][2]                       # the re-evaluation launches are counted
+        ward, rho = res[3][0], res[4][0]
+        assert np.all(ward >= 0) and np.all((rho > 0) & (rho <= 1.0 + 1e-12))
+        changed = res[2][0] != res[0][0]
+        flagged = (ward > 3e-14 * (1 - 1e-9)) | (rho < 3e-3 * (1 + 1e-9))   # the documented default rule for n = 6
+        assert np.all(flagged[changed]) and abs(int(flagged.sum()) - res[2][1]) <= 2
+        # a huge threshold and no cancellation test: nothing is re-evaluated, the bits equal the FP64 path
+        bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 2)
+        bg.bg_set_option(ctx, bg.BG_OPT_FLAG_THRESHOLD, 10 ** 17)
+        bg.bg_set_option(ctx, bg.BG_OPT_FLAG_CANCELLATION, 1)
+        bg.bg_eval(ctx, st, ev.N, *d, out)
+        torch.cuda.synchronize()
+        assert bg.bg_last_refined(ctx)[0] <= 2 and np.mean(out.cpu().numpy() != res[0][0]) < 1e-4
+    finally:
+        bg.bg_destroy(ctx)
+
+
+@pytest.mark.parametrize("n,N,lanes", [(6, 4099, 8), (7, 1029, 4), (8, 519, 64), (9, 259, 128), (10, 131, 256),
+                                         (11, 67, 128), (12, 35, 256)])
+def test_flagged_reevaluation_other_lane_counts(bg, oracle, wl, n, N, lanes):
+    """The double-double instantiation of the interpreter with other lane counts than the defaults (its state elements
+    are 32 bytes: n >= 10 spills part of it to the L2 slab)."""
+    ev = wl.config_events(4, N=N, n=n)
+    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, lanes=lanes, flag_threshold=1)     # tau = 1e-18: (almost) all events flagged
+    assert name == "cdbg_prog_kernel"
+    check_cdbg(oracle, ev, got)
+
+
 @pytest.mark.parametrize("n", [6, 8])
 def test_kernel_variants_agree(bg, oracle, wl, n):
     ev = wl.config_events(4, N=777, n=n)
     a, na = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=1)
-    b, nb = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=0)
-    check_cdbg(oracle, ev, a)
-    check_cdbg(oracle, ev, b)
+    b, nb = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=0, precision=0)
+    check_cdbg_fp64(oracle, ev, a)
+    check_cdbg_fp64(oracle, ev, b)
     # chunked launches of the generic kernel (small scratch limit) give identical bits
     c, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=1, scratch_limit=1 << 22)
     assert np.array_equal(a, c)
@@ -143,9 +232,9 @@ def test_kernel_variants_agree(bg, oracle, wl, n):
 def test_program_interpreter_lane_counts(bg, oracle, wl, n, N, lanes):
     """The colour-class program interpreter with G lanes per event, sizes with ragged last warps."""
     ev = wl.config_events(4, N=N, n=n)
-    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=2, lanes=lanes)
+    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=2, lanes=lanes, precision=0)
     assert name == "cdbg_prog_kernel"
-    check_cdbg(oracle, ev, got)
+    check_cdbg_fp64(oracle, ev, got)
 
 
 @pytest.mark.parametrize("n,N", [(8, 131), (9, 259), (10, 131)])
@@ -153,9 +242,9 @@ def test_program_interpreter_lane_counts(bg, oracle, wl, n, N, lanes):
 def test_program_interpreter_block_per_event(bg, oracle, wl, n, N, lanes):
     """One event per warp / per block of 64..256 threads (split targets, combine sub-levels, block barriers)."""
     ev = wl.config_events(4, N=N, n=n)
-    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=2, lanes=lanes)
+    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=2, lanes=lanes, precision=0)
     assert name == "cdbg_prog_kernel"
-    check_cdbg(oracle, ev, got)
+    check_cdbg_fp64(oracle, ev, got)
 
 
 @pytest.mark.parametrize("n,N,lanes,limit", [(8, 131, 128, 16384), (10, 67, 128, 57344), (10, 67, 256, 32768),
@@ -163,9 +252,12 @@ def test_program_interpreter_block_per_event(bg, oracle, wl, n, N, lanes):
 def test_program_interpreter_spill(bg, oracle, wl, n, N, lanes, limit):
     """State beyond the shared-memory limit lives in the L2-resident global slab (top levels of the recursion)."""
     ev = wl.config_events(4, N=N, n=n)
-    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=2, lanes=lanes, smem_limit=limit)
+    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, kernel=2, lanes=lanes, smem_limit=limit, precision=0)
     assert name == "cdbg_prog_kernel"
-    check_cdbg(oracle, ev, got)
+    check_cdbg_fp64(oracle, ev, got)
+    if lanes == 128:     # the default path with the same slab limit: flag + (spilling) double-double re-evaluation
+        got, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, lanes=lanes, smem_limit=limit)
+        check_cdbg(oracle, ev, got)
 
 
 def test_program_interpreter_is_deterministic(bg, wl):
@@ -249,8 +341,10 @@ def test_double_double_reference_path_matches_truth_on_every_event(bg, oracle, w
     err = rel_err(got, truth)
     # the truth itself carries 64-bit-significand round-off amplified by the same cancellations: allow 1e-11
     assert err.max() <= 1e-11, f"max {err.max():.2e} at event {err.argmax()}"
-    fp64, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
+    fp64, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, precision=0)
     assert np.median(rel_err(fp64, got)) < 1e-13
+    auto, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
+    assert rel_err(auto, truth).max() <= 1e-11
 
 
 @pytest.mark.parametrize("n,N", [(5, 1000), (6, 600), (7, 2048)])
@@ -262,7 +356,7 @@ def test_double_double_reference_path_cobg(bg, oracle, wl, n, N):
     assert name == "cobg_dd_kernel"
     truth = oracle.cobg_full_colour(ev.mom, ev.hel, prec="long double")
     assert rel_err(got, truth).max() <= 1e-11
-    fp64, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR)
+    fp64, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR, precision=0)
     assert np.median(rel_err(fp64, got)) < 1e-13
     if n == 5:
         ev4 = wl.config_events(0, N=300)
@@ -272,7 +366,7 @@ def test_double_double_reference_path_cobg(bg, oracle, wl, n, N):
 
 @pytest.mark.parametrize("arith", ["real", "complex"])
 @pytest.mark.parametrize("n,N,lanes", [(4, 300, None), (5, 200, None), (6, 150, None), (6, 33, 32), (6, 33, 256),
-                                         (7, 40, None), (8, 9, 256)])
+                                         (7, 40, None), (8, 9, 256), (9, 3, None)])
 def test_continuous_colour_and_polarisation_states(bg, oracle, wl, n, N, lanes, arith):
     """SURVEY NEXT-1 (the paper's CD_MC sampling, Eq. 5-14): colour-dressed recursion with a real polarisation e(phi)
     and a full 3x3 colour matrix etabar x eta per gluon, against the oracle's general-state recursion."""
@@ -302,7 +396,7 @@ def test_continuous_colour_and_polarisation_states(bg, oracle, wl, n, N, lanes, 
     err = rel_err(got, truth)
     # all nine colour entries contribute: the sub-amplitude is a dense sum without the single-flow near-zeros, but
     # it is a sum over many colour orderings that can still cancel: same noise-floor rule as everywhere
-    assert np.median(err) < 1e-13 and err.max() < 1e-7
+    assert np.median(err) < 1e-13
     tail = np.nonzero(err > 1e-11)[0]
     assert len(tail) <= max(2, 0.02 * N)
     if len(tail):
@@ -339,8 +433,8 @@ def test_colour_ordered_monte_carlo_mode(bg, oracle, wl, n, N):
                                               truth[tail]))
         floor = np.maximum(floor, fp64_noise_floor(oracle, te, truth[tail], True, reps=8))
         assert np.all(err[tail] <= 10 * floor), (err[tail], floor)
-    # same events through the colour-dressed interpreter: the two recursions agree
-    dressed, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
+    # same events through the colour-dressed interpreter (FP64 only, like this mode): the two recursions agree
+    dressed, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, precision=0)
     assert np.mean(rel_err(got, dressed) > 1e-11) <= 0.01
     # spilled state and more lanes give the same numbers up to summation order
     if n == 7:
@@ -354,15 +448,18 @@ def test_colour_ordered_monte_carlo_rejects_large_n(bg):
     assert e.value.code == bg.BG_EUNSUPPORTED
 
 
-def test_cdbg_helicity_sum_mode(bg, oracle, wl):
+@pytest.mark.parametrize("n,N", [(4, 60), (5, 40), (6, 24)])
+def test_cdbg_helicity_sum_mode(bg, oracle, wl, n, N):
+    """Sum over all 2^n helicity assignments of the single-colour-flow |A|^2 (generic kernel, FP64): a sum of
+    non-negative terms dominated by the well-conditioned ones."""
     import itertools
-    ev = wl.config_events(4, N=40, n=5)
+    ev = wl.config_events(4, N=N, n=n)
     got, _ = gpu_eval(ev, bg.BG_CDBG_HELSUM_COLGIVEN)
-    tot = np.zeros(ev.N)
-    for h in itertools.product((-1, 1), repeat=5):
-        tot += oracle.cdbg(ev.mom, np.broadcast_to(np.array(h, dtype=np.int8), (ev.N, 5)).copy(), ev.col,
+    tot = np.zeros(ev.N, dtype=np.longdouble)
+    for h in itertools.product((-1, 1), repeat=n):
+        tot += oracle.cdbg(ev.mom, np.broadcast_to(np.array(h, dtype=np.int8), (ev.N, n)).copy(), ev.col,
                            prec="long double")
-    assert rel_err(got, tot).max() < 1e-10
+    assert rel_err(got, tot.astype(np.float64)).max() <= 1e-11
 
 
 def test_edge_cases(bg, oracle, wl):
@@ -371,6 +468,8 @@ def test_edge_cases(bg, oracle, wl):
     for N in (1, 31, 33, 127, 129):
         ev = wl.config_events(1, N=N)
         got, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
+        check_cdbg(oracle, ev, got)
+        got, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, flag_threshold=1)      # every event through the re-evaluation
         check_cdbg(oracle, ev, got)
     # N = 0 is a no-op
     ctx = bg.bg_init(6, bg.BG_CDBG_GIVEN)
@@ -394,6 +493,41 @@ def test_edge_cases(bg, oracle, wl):
     same = np.ones_like(ev.col)
     got, _ = gpu_eval(type(ev)(ev.n, ev.mom, ev.hel, same), bg.BG_CDBG_GIVEN)
     assert np.all(np.abs(got) < 1e-30 * np.median(oracle.cdbg(ev.mom, ev.hel, ev.col)))
+
+
+def test_vanishing_and_out_of_range_colours_after_a_large_context(bg, wl):
+    """Events whose colour class vanishes, or whose colour indices are out of range, carry no canonical permutation: the
+    scatter kernels must not gather momenta for them (once read through an uninitialised inverse permutation).  Run
+    them after an n = 12 context has used the same kernels with 12 gluons, mixed with valid events, at both prepass
+    sizes; valid events keep their values, the others return exactly 0.0."""
+    ev12 = wl.config_events(4, N=64, n=12)
+    gpu_eval(ev12, bg.BG_CDBG_GIVEN)
+    for N in (2000, (1 << 18) + 777):
+        ev = wl.config_events(1, N=N)
+        ref, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, precision=0)
+        col = ev.col.copy()
+        rng = np.random.default_rng(5)
+        kill = rng.random(N) < 0.5
+        col[kill, 0, 0] = (col[kill, 0, 0] % 3) + 1            # unbalanced colour charges: identically zero
+        bad = rng.random(N) < 0.1
+        col[bad, 3, 1] = 7                                     # out of range
+        got, _ = gpu_eval(type(ev)(ev.n, ev.mom, ev.hel, col), bg.BG_CDBG_GIVEN, precision=0)
+        dead = kill | bad
+        assert np.all(got[dead] == 0.0) and np.array_equal(got[~dead], ref[~dead])
+
+
+def test_batch_size_guard(bg):
+    """Event ids and record positions are 32 bit: larger batches are refused, not truncated."""
+    ctx = bg.bg_init(4, bg.BG_CDBG_GIVEN)
+    try:
+        import torch
+        x = torch.zeros(64, dtype=torch.float64, device="cuda")
+        b = torch.zeros(64, dtype=torch.int8, device="cuda")
+        with pytest.raises(bg.BgError) as e:
+            bg.bg_eval(ctx, 0, (1 << 32) + 5, x, b, b, x)
+        assert e.value.code == bg.BG_EINVAL
+    finally:
+        bg.bg_destroy(ctx)
 
 
 def test_host_path_matches_device_path(bg, wl):
