@@ -29,9 +29,9 @@ sys.path.insert(0, ROOT)
 # mean over sampled colour assignments), and of the colour-ordered configs.
 CDBG_FLOP_PER_EVENT = {4: 2.1e3, 5: 8.4e3, 6: 2.5e4, 7: 7.0e4, 8: 2.2e5, 9: 6.4e5, 10: 1.9e6, 11: 5.1e6, 12: 1.46e7}
 COBG_FLOP_PER_EVENT = {0: 2.6e4, 2: 1.41e6 + 5.8e4}     # config 0 (n=4 helsum), config 2 (n=7 + colour form)
-# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of the recursion kernel launches of ONE step, from the
-# `ncu --set full` captures summarised in profiles/r01_ncu_summary.md (same command, default event counts).
-NCU_TRAFFIC_BYTES = {("cdbg_prog_kernel", 6): 244.2e6, ("cobg_shared_kernel", 7): 91.4e6, ("cdbg_prog_kernel", 9): 100.2e6}
+# DRAM bytes of the dominant kernel's launches of one step are NOT measured here: when profiles/ holds the table
+# written from an `ncu --set full` capture of the same command, the matching row is quoted with the file's name.
+TRAFFIC_CSV = os.path.join("profiles", "r02_dram_traffic.csv")     # kernel,n,events,bytes_per_step,source
 CONFIG_N = {0: 4, 1: 6, 2: 7, 3: 9}
 CONFIG_EVENTS = {0: 1024, 1: 1 << 20, 2: 1 << 18, 3: 1 << 18, 4: 1 << 16}
 
@@ -58,7 +58,126 @@ def parse_args():
     ap.add_argument("--precision", type=int, default=None, help="BG_OPT_PRECISION (1 = double-double reference path)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-configs", action="store_true",
+                    help="skip the compact measurements of the other BASELINE.json configs (C1, C3, C4, C5 n = 4..12)")
     return ap.parse_args()
+
+
+def ncu_traffic(kernel: str, n: int, N: int):
+    """bytes per step of the dominant kernel from the committed ncu table, or (None, None)."""
+    path = os.path.join(ROOT, TRAFFIC_CSV)
+    if not os.path.exists(path):
+        return None, None
+    import csv
+    with open(path) as f:
+        for row in csv.DictReader(f):
+            if row["kernel"] == kernel and int(row["n"]) == n and int(row["events"]) == N:
+                return float(row["bytes_per_step"]), f"{TRAFFIC_CSV}: {row['source']}"
+    return None, None
+
+
+def truth_sample_size(n: int, N: int) -> int:
+    """events of a config compared with the long-double oracle inside the bench (bounded CPU time)."""
+    return min(N, {4: 16384, 5: 16384, 6: 16384, 7: 8192, 8: 4096, 9: 2048, 10: 512, 11: 192, 12: 64}[n])
+
+
+def measure_config(bg, wl, oracle_mod, dev, config: int, n: int, steps: int, peak_tf: float, with_cpu: bool):
+    """Compact measurement of one BASELINE.json config on the current device (N = 1): events/s of the default path,
+    the FP64-only path beside it, the FP64 kernel's roofline fraction, the conditioning flag's cost, the CPU oracle
+    (all cores / one core) and parity against the long-double oracle on a stated sample."""
+    import torch
+    N = CONFIG_EVENTS[config]
+    ev = wl.config_events(config, N=N, n=n if config == 4 else None)
+    mode = mode_for(config)
+    flop = COBG_FLOP_PER_EVENT[config] if config in (0, 2) else CDBG_FLOP_PER_EVENT[n]
+    d_mom = torch.from_numpy(wl.to_soa(mom=ev.mom)).to(dev)
+    d_hel = None if ev.hel is None or (mode & bg.BG_HEL_SUM) else torch.from_numpy(wl.to_soa(hel=ev.hel)).to(dev)
+    d_col = None if not (mode & bg.BG_COL_GIVEN) else torch.from_numpy(wl.to_soa(col=ev.col)).to(dev)
+    d_out = torch.empty(N, dtype=torch.float64, device=dev)
+    stream = torch.cuda.current_stream()
+    sh = stream.cuda_stream
+    ctx = bg.bg_init(n, mode)
+    res = {"workload": {0: "C1", 2: "C3", 3: "C4", 4: "C5"}.get(config, "C2") + f" n={n}", "n": n, "events": N}
+    try:
+        bg.bg_reserve(ctx, N)
+        auto = config != 0
+
+        def timed(precision):
+            if auto:
+                bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, precision)
+            for _ in range(3):
+                bg.bg_eval(ctx, sh, N, d_mom, d_hel, d_col, d_out)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(steps):
+                bg.bg_eval(ctx, sh, N, d_mom, d_hel, d_col, d_out)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / steps
+            bg.bg_set_option(ctx, bg.BG_OPT_TIMING, 1)
+            kms, rms, fl = [], [], 0
+            for _ in range(min(steps, 5)):
+                bg.bg_eval(ctx, sh, N, d_mom, d_hel, d_col, d_out)
+                kms.append(bg.bg_last_kernel_ms(ctx))
+                fl, r = bg.bg_last_refined(ctx)
+                rms.append(r)
+            bg.bg_set_option(ctx, bg.BG_OPT_TIMING, 0)
+            return ms, float(np.mean(kms)), float(np.mean(rms)), fl
+        ms, kms, rms, fl = timed(2)
+        got = d_out.cpu().numpy()
+        res.update({"events_per_s": N / (ms * 1e-3), "ms_per_step": ms, "kernel_ms": kms,
+                    "gpu_launches_per_step": bg.bg_last_launch_count(ctx), "kernel": bg.bg_last_kernel_name(ctx),
+                    "current_bytes_per_event": bg.bg_current_bytes_per_event(ctx)})
+        fp64_kms = kms - rms
+        res["roofline"] = {"bound": "alu", "flop_per_event": flop, "fp64_kernel_ms": fp64_kms,
+                           "achieved": flop * N / (fp64_kms * 1e-3) * 1e-12, "unit": "TFLOP/s",
+                           "frac": flop * N / (fp64_kms * 1e-3) * 1e-12 / peak_tf}
+        if config == 0:
+            res["note"] = "1024 events: one 13 us launch, launch-latency bound (SURVEY 8d); FP64 alone meets 1e-11"
+        if auto:
+            ms0, kms0, _, _ = timed(0)
+            res["precision_auto"] = {"flagged_frac": fl / N, "reevaluation_ms": rms,
+                                     "overhead_pct": 100.0 * (ms / ms0 - 1.0),
+                                     "fp64_only_events_per_s": N / (ms0 * 1e-3), "fp64_only_ms_per_step": ms0}
+            bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 2)
+    finally:
+        bg.bg_destroy(ctx)
+    if with_cpu:
+        S = truth_sample_size(n, N)
+        sub = ev.head(S)
+        if config == 0:
+            truth = oracle_mod.cobg_full_colour(sub.mom, None, prec="long double")
+        elif config == 2:
+            S = min(S, 1024)
+            sub = ev.head(S)
+            truth = oracle_mod.cobg_full_colour(sub.mom, sub.hel, prec="long double")
+        else:
+            truth = oracle_mod.cdbg(sub.mom, sub.hel, sub.col, prec="long double")
+        err = np.abs(got[:S] - truth) / np.abs(truth)
+        res["parity"] = {"max_rel_err_vs_long_double": float(err.max()), "median": float(np.median(err)),
+                         "n_over_1e-11": int(np.sum(err > 1e-11)), "sample": f"first {S} events"}
+
+        class A:
+            pass
+        a = A()
+        a.config = config
+        cpu = {}
+        for label, threads, budget in (("all_cores", 0, 1.0), ("one_core", 1, 1.0)):
+            S2 = max(16, int(cpu_sample_size(a, n, N) * (budget / 15.0) / (1 if threads == 0 else oracle_mod.max_threads())))
+            S2 = min(S2, N)
+            sample = ev.head(S2)
+            t0 = time.perf_counter()
+            reps = 0
+            while reps < 1 or (time.perf_counter() - t0 < 0.5 and reps < 1000):
+                oracle_eval(a, sample, threads)
+                reps += 1
+            dt = time.perf_counter() - t0
+            cpu[label] = {"events_per_s": S2 * reps / dt, "cores": oracle_mod.max_threads() if threads == 0 else 1,
+                          "sample": f"first {S2} events x {reps}"}
+        res["cpu_baseline"] = cpu
+    return res
+
 
 
 def workload_desc(args):
@@ -298,7 +417,14 @@ def run_b200(args):
     total_ms = e0.elapsed_time(e1)
     launches_per_step = bg.bg_last_launch_count(ctx)
     kernel_name = bg.bg_last_kernel_name(ctx)
-    kernel_ms = float(np.mean(kms))      # per step: all launches of the dominant kernel
+    kernel_ms = float(np.mean(kms))      # per step: all launches of the recursion kernels (FP64 + re-evaluation)
+    flagged, refine_ms = (0, 0.0)
+    if not args.continuous:
+        bg.bg_set_option(ctx, bg.BG_OPT_TIMING, 1)
+        step()
+        flagged, refine_ms = bg.bg_last_refined(ctx)
+        bg.bg_set_option(ctx, bg.BG_OPT_TIMING, 0)
+    auto_default = args.precision is None and flagged > 0
     total_ms = max_over_ranks(total_ms, world, dev)
     value = N * world * args.steps / (total_ms * 1e-3)
 
@@ -352,16 +478,21 @@ def run_b200(args):
         out_host = d_out.cpu().numpy()
         if not np.all(np.isfinite(out_host)):
             raise SystemExit("bench.py: non-finite |M|^2 in the output")
-        achieved_tf = flop_per_event * N / (kernel_ms * 1e-3) * 1e-12
-        traffic = NCU_TRAFFIC_BYTES.get((kernel_name, n)) if N == CONFIG_EVENTS.get(args.config) else None
+        # dominant kernel = the FP64 recursion kernel, which evaluates every event; the double-double re-evaluation of
+        # the flagged events is reported beside it (precision_auto) and counted in ms_per_step / value
+        fp64_kernel_ms = kernel_ms - refine_ms
+        achieved_tf = flop_per_event * N / (fp64_kernel_ms * 1e-3) * 1e-12
+        traffic, traffic_src = ncu_traffic(kernel_name, n, N)
         roofline = {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                    "frac": achieved_tf / peak_tf, "traffic": traffic, "traffic_unit": "bytes per step (ncu, "
-                    "profiles/r01_ncu_summary.md)", "kernel": kernel_name,
+                    "frac": achieved_tf / peak_tf, "traffic": traffic, "traffic_source": traffic_src,
+                    "kernel": kernel_name,
                     "peak_source": "bg_fp64_peak_probe (DFMA chains, this run); nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2",
-                    "flop_per_event": flop_per_event, "kernel_ms": kernel_ms,
-                    "kernel_share_of_step": kernel_ms / (total_ms / args.steps)}
+                    "flop_per_event": flop_per_event, "kernel_ms": fp64_kernel_ms,
+                    "kernel_share_of_step": fp64_kernel_ms / (total_ms / args.steps),
+                    "frac_of_whole_step": flop_per_event * N / (total_ms / args.steps * 1e-3) * 1e-12 / peak_tf}
         cpu = None
-        if not args.no_cpu_baseline and not args.lc and not args.continuous:    # no batched oracle entry for these
+        parity = None
+        if not args.no_cpu_baseline and not args.lc and not args.continuous and not args.comc:    # no batched oracle entry for these
             import oracle
             S = cpu_sample_size(args, n, N)
             sample = ev.head(S)
@@ -376,6 +507,23 @@ def run_b200(args):
             cpu = {"value": S * reps / dt, "unit": "events/s", "cores": oracle.max_threads(), "kind": "oracle",
                    "sample": f"first {S} events of the workload x {reps} pass(es), {dt:.2f} s wall",
                    "median_rel_diff_gpu_vs_oracle": float(np.median(err))}
+            S1 = max(64, S // (4 * oracle.max_threads()))
+            t0 = time.perf_counter()
+            oracle_eval(args, ev.head(S1), threads=1)
+            cpu["one_core"] = {"value": S1 / (time.perf_counter() - t0), "unit": "events/s", "sample": f"first {S1} events"}
+            # parity of the default path against the extended-precision oracle on a stated sample
+            St = truth_sample_size(n, N) * 4 if args.config != 2 else 1024
+            St = min(St, N)
+            sub = ev.head(St)
+            if args.config == 0:
+                truth = oracle.cobg_full_colour(sub.mom, None, prec="long double")
+            elif args.config == 2:
+                truth = oracle.cobg_full_colour(sub.mom, sub.hel, prec="long double")
+            else:
+                truth = oracle.cdbg(sub.mom, sub.hel, sub.col, prec="long double")
+            terr = np.abs(out_host[:St] - truth) / np.abs(truth)
+            parity = {"max_rel_err_vs_long_double": float(terr.max()), "median": float(np.median(terr)),
+                      "n_over_1e-11": int(np.sum(terr > 1e-11)), "sample": f"first {St} events"}
         line = {"metric": "n-gluon |M|^2 events/sec", "value": value, "unit": "events/s",
                 "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
                 "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -388,6 +536,39 @@ def run_b200(args):
                 "roofline": roofline, "cpu_baseline": cpu}
         if devgen is not None:
             line["generate_on_device"] = devgen
+        line["parity"] = parity
+        prec_now = 2 if auto_default else (args.precision if args.precision is not None else 0)
+        line["config"]["precision"] = {0: "FP64", 1: "double-double (all events)", 2: "FP64 + conditioning flag + "
+                                       "double-double re-evaluation of the flagged events (default)"}.get(prec_now, str(prec_now))
+        if auto_default:
+            # the FP64-only path (BG_OPT_PRECISION = 0) timed beside the default one, same events
+            bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 0)
+            for _ in range(3):
+                step()
+            torch.cuda.synchronize()
+            f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            f0.record(stream)
+            for _ in range(args.steps):
+                step()
+            f1.record(stream)
+            torch.cuda.synchronize()
+            ms0 = f0.elapsed_time(f1) / args.steps
+            bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 2)
+            line["precision_auto"] = {"flagged_frac": flagged / N, "reevaluation_ms": refine_ms,
+                                      "overhead_pct": 100.0 * (total_ms / args.steps / ms0 - 1.0),
+                                      "fp64_only_events_per_s": N / (ms0 * 1e-3), "fp64_only_ms_per_step": ms0}
+        if world == 1 and args.config == 1 and not args.no_configs and not (args.continuous or args.comc or args.lc) \
+                and args.events is None and args.precision is None and not args.kernel and args.lanes is None:
+            # every BASELINE.json config in the same record: C1, C3, C4 and the C5 sweep n = 4..12 ("events/s vs n")
+            import oracle as oracle_mod
+            ksteps = max(3, min(args.steps, 10))
+            cfgs = {}
+            with_cpu = not args.no_cpu_baseline
+            cfgs["C1"] = measure_config(bg, wl, oracle_mod, dev, 0, 4, max(ksteps, 20), peak_tf, with_cpu)
+            cfgs["C3"] = measure_config(bg, wl, oracle_mod, dev, 2, 7, ksteps, peak_tf, with_cpu)
+            cfgs["C4"] = measure_config(bg, wl, oracle_mod, dev, 3, 9, ksteps, peak_tf, with_cpu)
+            cfgs["C5"] = {str(k): measure_config(bg, wl, oracle_mod, dev, 4, k, ksteps, peak_tf, with_cpu) for k in range(4, 13)}
+            line["configs"] = cfgs
         print(json.dumps(line), flush=True)
     bg.bg_destroy(ctx)
     if world > 1:

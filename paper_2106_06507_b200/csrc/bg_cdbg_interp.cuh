@@ -342,11 +342,13 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         // momentum -(sum of the others): exactly the momentum flow of the recursion closed with gluon n (oracle and
         // Eq. 22 as printed) in the double-double kernel; in the FP64 kernels that sum (compensated) rounded once.
         int kstar = -1;
+#ifndef BG_NO_KSTAR
         if constexpr (kComplex) {
             if (p.rec_gstride == 4)
                 for (int k = 0; k + 1 < n; k++)
                     if ((int)((perm >> (4 * k)) & 0xF) == n - 1) kstar = k;
         }
+#endif
         auto store_ext_momentum = [&](int kk, int offPt, const double* pk) {
             if constexpr (kComplex && !StateElem<S>::kDD) {
                 if (kk == kstar) {
