@@ -65,9 +65,11 @@ struct ProgTable {
     uint32_t* d_small;        // [2 (num_classes + 1) + 1] zeroed histogram | cursors | ticket of the fused-scan prepass
     // double-double re-evaluation of flagged events (BG_OPT_PRECISION = 2): state elements are 32 bytes, so less of
     // the state fits in shared memory
-    int dd_mode;              // 0: fits; 1: top of the state spills (>= 128 lanes); -1: does not fit (unsupported)
-    int dd_cap_cx;            // state elements per event kept in shared memory
-    int dd_spill_blocks;      // resident blocks per SM of the spilling re-evaluation kernels
+    int dd_mode;              // 1: available (state beyond dd_cap_cx elements per event spills to the L2 slab); -1: not (dense tables)
+    int dd_cap_cx;            // state elements per event kept in shared memory: sized so that shared memory allows as many
+                              // resident blocks as the 255 registers per thread do
+    int dd_spill_blocks;      // resident blocks per SM of the re-evaluation kernels
+    long long dd_max_blocks;  // ... and blocks per launch (each owns one global slab; their sum is bounded)
 };
 
 // how one set of tier launches is sized
@@ -76,6 +78,7 @@ struct LaunchShape {
     int regs = 168;           // registers per thread of the instantiation (resident-block estimate)
     int cap_cx = 0;           // > 0: at most this many state elements per event in shared memory (SPILL kernels)
     int spill_blocks = 0;     // SPILL: resident blocks per SM (each owns one global slab)
+    long long max_blocks = 0; // > 0: at most this many blocks per launch
 };
 
 struct ProgParams {
@@ -154,12 +157,12 @@ struct StateRef {
     T* spill;
     int cap;
     __device__ __forceinline__ S ld(int o) const {
-        if (SPILL && o >= cap) return StateElem<S>::get(StateElem<S>::ldcg(spill + (o - cap)));
+        if (SPILL && o >= cap) return StateElem<S>::get(StateElem<S>::ldcg(spill + (size_t)(o - cap) * EPW));
         return StateElem<S>::get(base[o * EPW]);
     }
     __device__ __forceinline__ void st(int o, S v) const {
         if (SPILL && o >= cap) {
-            StateElem<S>::stcg(spill + (o - cap), StateElem<S>::put(v));
+            StateElem<S>::stcg(spill + (size_t)(o - cap) * EPW, StateElem<S>::put(v));
             return;
         }
         base[o * EPW] = StateElem<S>::put(v);
@@ -243,7 +246,8 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     uint4* const ring = reinterpret_cast<uint4*>(smem_raw + ((size_t)p.slab_cx * EPW * sizeof(T) + 15) / 16) + lane;
     StateRef<EPW, SPILL, S> st_;
     st_.base = smem + q;
-    st_.spill = SPILL ? reinterpret_cast<T*>(p.spill) + (size_t)blockIdx.x * p.spill_cx : nullptr;
+    // the block's slab in global memory, [offset - cap][event] like the shared one
+    st_.spill = SPILL ? reinterpret_cast<T*>(p.spill) + (size_t)blockIdx.x * p.spill_cx * EPW + q : nullptr;
     st_.cap = p.slab_cx;
     // tasks: the records of the tier, or (re-evaluation) the record positions in the tier's flag list
     const long long first = p.bounds[p.tier], end = p.list ? first + p.list_count[p.tier] : (long long)p.bounds[p.tier + 1];
@@ -338,37 +342,15 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         // Momentum conservation holds for double-precision inputs only to round-off, and the recursion never uses the
         // momentum of the closing gluon: closing with another gluon than input gluon n evaluates a slightly different
         // continuation of the amplitude off the momentum-conserving surface - a relative difference of 1e-16 times the
-        // event's condition number.  Input gluon n, when the class closes with another one, therefore gets the
-        // momentum -(sum of the others): exactly the momentum flow of the recursion closed with gluon n (oracle and
-        // Eq. 22 as printed) in the double-double kernel; in the FP64 kernels that sum (compensated) rounded once.
+        // event's condition number, inside the FP64 kernels' own round-off but not inside the re-evaluation's.  The
+        // double-double kernel therefore gives input gluon n, when the class closes with another one, the momentum
+        // -(sum of the others): exactly the momentum flow of the recursion closed with gluon n (oracle, Eq. 22).
         int kstar = -1;
-#ifndef BG_NO_KSTAR
-        if constexpr (kComplex) {
-            if (p.rec_gstride == 4)
-                for (int k = 0; k + 1 < n; k++)
-                    if ((int)((perm >> (4 * k)) & 0xF) == n - 1) kstar = k;
+        if constexpr (StateElem<S>::kDD) {
+            for (int k = 0; k + 1 < n; k++)
+                if ((int)((perm >> (4 * k)) & 0xF) == n - 1) kstar = k;
         }
-#endif
         auto store_ext_momentum = [&](int kk, int offPt, const double* pk) {
-            if constexpr (kComplex && !StateElem<S>::kDD) {
-                if (kk == kstar) {
-                    double Pe[4];
-#pragma unroll
-                    for (int c = 0; c < 4; c++) {
-                        double sum = 0.0, comp = 0.0;     // two-sum accumulation of -(sum of the other momenta)
-                        for (int j = 0; j < n; j++) {
-                            if (j == kk) continue;
-                            const double x = -__ldcg(mrec + j * 4 + c);
-                            const double t = sum + x, bb = t - sum;
-                            comp += (sum - (t - bb)) + (x - bb);
-                            sum = t;
-                        }
-                        Pe[c] = sum + comp;
-                    }
-                    st_.stPd(offPt, Pe);
-                    return;
-                }
-            }
             if constexpr (StateElem<S>::kDD) {
                 if (kk == kstar) {
                     R Pe[4];
@@ -730,6 +712,7 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (shape.regs * BLOCK), (228 * 1024) / (smem[k] + 1024)));
         if (SPILL) per_sm = std::min(per_sm, shape.spill_blocks);   // one global slab per resident block
         blocks[k] = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
+        if (shape.max_blocks > 0) blocks[k] = (unsigned)std::min<long long>(blocks[k], shape.max_blocks);
         resident += (long long)sm_count * per_sm;
         nlaunch++;
     }
@@ -737,8 +720,15 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
     // ramp-up and tail, so the tiers run side by side (fork / join around the caller's stream).  Measured at
     // n = 6: 2^16 events +22 %, 2^18 neutral, 2^20 -5 %; n >= 7: slower at every size.
     // (spill slabs are indexed by block: one launch at a time)
-    conc = conc && G <= 4 && !SPILL && t->has_streams && nlaunch > 1 && max_tasks <= 2 * resident;
+    // (spill slabs are indexed by block: concurrent launches each get their own share of the slabs)
+    const bool conc_spill = conc && SPILL && shape.max_blocks > 0 && t->has_streams && nlaunch > 1;
+    const long long share = conc_spill ? std::max<long long>(1, shape.max_blocks / nlaunch) : 0;
+    if (conc_spill)
+        for (int k = 0; k < kTiers; k++) blocks[k] = (unsigned)std::min<long long>(blocks[k], share);
+    conc = conc_spill || (conc && G <= 4 && !SPILL && t->has_streams && nlaunch > 1 && max_tasks <= 2 * resident);
     if (conc && cudaEventRecord(t->fork_ev, s) != cudaSuccess) return cudaGetLastError();
+    double2* const spill0 = p.spill;
+    int li = 0;
     int side = 0;                                 // launches sent to the side streams so far
     bool first = true;
     for (int k = 0; k < kTiers; k++) {
@@ -750,6 +740,8 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
             ls = t->aux[side];
             cudaStreamWaitEvent(ls, t->fork_ev, 0);
         }
+        if (conc_spill) p.spill = reinterpret_cast<double2*>(reinterpret_cast<char*>(spill0) + (size_t)li * share * p.spill_cx * EPW * ELEM);
+        li++;
         cdbg_prog_kernel<G, SPILL, S><<<blocks[k], BLOCK, smem[k], ls>>>(p);
         if (conc && !first) cudaEventRecord(t->join_ev[side++], ls);
         first = false;

@@ -546,14 +546,21 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
     }
-    {   // double-double re-evaluation: 32-byte state elements under the same shared-memory limit
+    {   // double-double re-evaluation: 32-byte state elements and 255 registers per thread.  The registers allow
+        // 65536 / (255 x block) resident blocks per SM; the shared-memory part of the state is capped so that shared
+        // memory allows as many (the kernel is latency-bound: resident warps decide its speed), the rest - the highest
+        // levels - lives in the block's L2-resident slab like the spilled state of the n >= 11 FP64 kernels.
         const int epw = G >= 32 ? 1 : 32 / G, block = G > 32 ? G : 32;
         const size_t ring_bytes = G >= 8 ? (size_t)kRing * block * 16 : 0;
-        if ((size_t)epw * max_state * 32 <= slab_limit) { t->dd_mode = 0; t->dd_cap_cx = std::max(16, max_state); }
-        else if (G >= 128) { t->dd_mode = 1; t->dd_cap_cx = (int)(slab_limit / 32); }
-        else { t->dd_mode = -1; t->dd_cap_cx = 0; }
-        const size_t smem0 = (size_t)epw * std::min(tiers.slab_cx[0], std::max(16, t->dd_cap_cx)) * 32 + ring_bytes;
-        t->dd_spill_blocks = (int)std::max<size_t>(1, std::min<size_t>(65536 / (255 * block), (228 * 1024) / (smem0 + 1024)));
+        const int reg_blocks = std::max(1, 65536 / (256 * block));
+        const size_t per_block = std::min<size_t>(slab_limit, (size_t)(224 * 1024) / reg_blocks - 1024 - ring_bytes);
+        t->dd_mode = 1;
+        t->dd_cap_cx = std::max(16, (int)(per_block / 32 / (size_t)epw));
+        t->dd_spill_blocks = reg_blocks;
+        // one slab of the largest state per block; all slabs together at most 512 MB (fewer blocks otherwise)
+        const size_t slab_bytes = (size_t)epw * max_state * 32;
+        t->dd_max_blocks = std::min<long long>((long long)t->sm_count * reg_blocks, (long long)(((size_t)512 << 20) / std::max<size_t>(1, slab_bytes)));
+        if (t->dd_max_blocks < 8) t->dd_mode = -1;
     }
     {   // spare rows of no-ops: the interpreter requests ops kRing - 1 steps ahead
         ProgOp nop;
@@ -711,7 +718,8 @@ static size_t prog_spill_bytes(const ProgTable* t) {
     return t->spill ? ((size_t)t->sm_count * t->spill_blocks_per_sm * t->max_state_cx * 16 + 255) / 256 * 256 : 0;
 }
 size_t prog_scratch_bytes(const ProgTable* t, long long N) {
-    const size_t dd_spill = t->dd_mode == 1 ? (size_t)t->sm_count * t->dd_spill_blocks * t->max_state_cx * 32 : 0;
+    const size_t epw = t->G >= 32 ? 1 : 32 / t->G;
+    const size_t dd_spill = t->dd_mode == 1 ? (size_t)t->dd_max_blocks * epw * t->max_state_cx * 32 : 0;
     return prog_spill_offset(t, N) + prog_spill_bytes(t) + dd_spill;
 }
 
@@ -724,7 +732,7 @@ cudaError_t prog_flagged_count(const ProgTable* t, long long N, const void* scra
     return err;
 }
 
-cudaError_t dispatch_interp_dd(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches);   // bg_cdbg_prog_dd.cu
+cudaError_t dispatch_interp_dd(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches, bool conc);   // bg_cdbg_prog_dd.cu
 
 static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches,
                                    bool conc = false) {
@@ -860,7 +868,8 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         p.list = flag_list;
         p.list_count = flag_count;
         p.spill = t->dd_mode == 1 ? (double2*)((char*)scratch + prog_spill_offset(t, N) + prog_spill_bytes(t)) : nullptr;
-        err = dispatch_interp_dd(s, t, sm_count, p, launches);
+        // few flagged events per tier for batches up to 2^19: the tier launches overlap their ramp-up and tails
+        err = dispatch_interp_dd(s, t, sm_count, p, launches, N <= (1ll << 19) && t->G < 32);   // (block-per-event lane counts: measured slower)
     }
     if (ev1) cudaEventRecord(ev1, s);
     return err;

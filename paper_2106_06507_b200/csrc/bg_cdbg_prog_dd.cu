@@ -55,27 +55,25 @@ __device__ __forceinline__ cxd shfl_xor(cxd v, int d) {
 }
 __device__ __forceinline__ int hi_word(cxd v) { return __double2hiint(v.re.hi); }
 
-cudaError_t dispatch_interp_dd(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches) {
+cudaError_t dispatch_interp_dd(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches, bool conc) {
     if (t->dd_mode < 0 || t->dense) return cudaErrorInvalidValue;
     LaunchShape shape;
     shape.regs = 255;
+    shape.conc = conc;   // small batches: the tier launches side by side, each with its share of the slabs
     shape.cap_cx = t->dd_cap_cx;
     shape.spill_blocks = t->dd_spill_blocks;
-    const bool spill = t->dd_mode == 1;
+    shape.max_blocks = t->dd_max_blocks;
+    // always the SPILL instantiation: offsets below the cap live in shared memory, the rest in the block's slab
     switch (t->G) {
-        case 1: return launch_interp<1, false, cxd>(s, t, sm_count, p, launches, shape);
-        case 2: return launch_interp<2, false, cxd>(s, t, sm_count, p, launches, shape);
-        case 4: return launch_interp<4, false, cxd>(s, t, sm_count, p, launches, shape);
-        case 8: return launch_interp<8, false, cxd>(s, t, sm_count, p, launches, shape);
-        case 16: return launch_interp<16, false, cxd>(s, t, sm_count, p, launches, shape);
-        case 32: return launch_interp<32, false, cxd>(s, t, sm_count, p, launches, shape);
-        case 64: return launch_interp<64, false, cxd>(s, t, sm_count, p, launches, shape);
-        case 128:
-            return spill ? launch_interp<128, true, cxd>(s, t, sm_count, p, launches, shape)
-                         : launch_interp<128, false, cxd>(s, t, sm_count, p, launches, shape);
-        default:
-            return spill ? launch_interp<256, true, cxd>(s, t, sm_count, p, launches, shape)
-                         : launch_interp<256, false, cxd>(s, t, sm_count, p, launches, shape);
+        case 1: return launch_interp<1, true, cxd>(s, t, sm_count, p, launches, shape);
+        case 2: return launch_interp<2, true, cxd>(s, t, sm_count, p, launches, shape);
+        case 4: return launch_interp<4, true, cxd>(s, t, sm_count, p, launches, shape);
+        case 8: return launch_interp<8, true, cxd>(s, t, sm_count, p, launches, shape);
+        case 16: return launch_interp<16, true, cxd>(s, t, sm_count, p, launches, shape);
+        case 32: return launch_interp<32, true, cxd>(s, t, sm_count, p, launches, shape);
+        case 64: return launch_interp<64, true, cxd>(s, t, sm_count, p, launches, shape);
+        case 128: return launch_interp<128, true, cxd>(s, t, sm_count, p, launches, shape);
+        default: return launch_interp<256, true, cxd>(s, t, sm_count, p, launches, shape);
     }
 }
 

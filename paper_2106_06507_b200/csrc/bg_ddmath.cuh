@@ -17,10 +17,6 @@ using cxd = cxt<dd>;
 // acc += a*b.  (The leading product is formed with __dmul_rn: a plain a.hi * b.hi could be contracted with the
 // following addition into one FMA, and the two-sum below is error-free only for the rounded product.)
 __device__ __forceinline__ void dd_fma(dd& acc, dd a, dd b) {
-#ifdef BG_DD_SLOW
-    acc = acc + a * b;
-    return;
-#endif
     const double p = __dmul_rn(a.hi, b.hi);
     double e = fma(a.hi, b.hi, -p);
     e = fma(a.hi, b.lo, e);
@@ -36,9 +32,6 @@ __device__ __forceinline__ void dd_fma(dd& acc, dd a, dd b) {
 __device__ __forceinline__ dd dd_neg(dd a) { return mkdd(-a.hi, -a.lo); }
 // a + b without the second renormalisation (error 2^-104 relative to |a| + |b|)
 __device__ __forceinline__ dd dd_add(dd a, dd b) {
-#ifdef BG_DD_SLOW
-    return a + b;
-#endif
     const double s = a.hi + b.hi;
     const double bb = s - a.hi;
     const double err = (a.hi - (s - bb)) + (b.hi - bb);
@@ -48,9 +41,6 @@ __device__ __forceinline__ dd dd_add(dd a, dd b) {
 }
 __device__ __forceinline__ dd dd_sub(dd a, dd b) { return dd_add(a, dd_neg(b)); }
 __device__ __forceinline__ dd dd_mul(dd a, dd b) {
-#ifdef BG_DD_SLOW
-    return a * b;
-#endif
     const double p = __dmul_rn(a.hi, b.hi);
     double e = fma(a.hi, b.hi, -p);
     e = fma(a.hi, b.lo, e);
