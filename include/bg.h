@@ -85,7 +85,7 @@ enum {
                                 BG_OPT_FLAG_THRESHOLD, or when |A| is less than BG_OPT_FLAG_CANCELLATION times the sum of
                                 the moduli of the closure contributions that add up to it.  3, 4 = diagnostics: `out`
                                 receives the Ward residual / that cancellation ratio instead of |M|^2. */
-    BG_OPT_FLAG_THRESHOLD = 7,/* Ward-residual threshold in units of 1e-18 (0 = default: 1e-13; 3e-14 for n = 5, 6) */
+    BG_OPT_FLAG_THRESHOLD = 7,/* Ward-residual threshold in units of 1e-18 (0 = default: 1e-13; 3e-14 for n = 5, 2e-14 for n = 6) */
     BG_OPT_FLAG_CANCELLATION = 8, /* cancellation threshold in units of 1e-6 (0 = default: 3e-3) */
     BG_OPT_SMEM_LIMIT = 5    /* program interpreter, >= 128 lanes per event: bytes of shared memory one event's state may
                                 take (16 KiB .. 222 KiB, 0 = default); the rest spills to an L2-resident slab.

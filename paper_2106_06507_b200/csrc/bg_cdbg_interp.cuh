@@ -150,17 +150,28 @@ __device__ __forceinline__ double s_scale(double f, double v) { return f * v; }
 __device__ __forceinline__ void ext_current(const double* pk, int lambda, cx* eps) { polarisation(pk, lambda, eps); }
 
 
+// Debug build (-DBG_BOUNDS_CHECK; compute-sanitizer is not available on every pool): every state access is checked
+// against the slab / spill extents and traps, so that `pytest -m gpu` under this build finds an out-of-range offset.
+#ifdef BG_BOUNDS_CHECK
+#define BG_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define BG_CHECK(cond) do { } while (0)
+#endif
+
 template <int EPW, bool SPILL, class S>
 struct StateRef {
     using T = typename StateElem<S>::T;
     T* base;
     T* spill;
     int cap;
+    int limit;     // (bounds-checked builds) state elements of the largest class
     __device__ __forceinline__ S ld(int o) const {
+        BG_CHECK(o >= 0 && (SPILL ? o < limit : o < cap));
         if (SPILL && o >= cap) return StateElem<S>::get(StateElem<S>::ldcg(spill + (size_t)(o - cap) * EPW));
         return StateElem<S>::get(base[o * EPW]);
     }
     __device__ __forceinline__ void st(int o, S v) const {
+        BG_CHECK(o >= 0 && (SPILL ? o < limit : o < cap));
         if (SPILL && o >= cap) {
             StateElem<S>::stcg(spill + (size_t)(o - cap) * EPW, StateElem<S>::put(v));
             return;
@@ -249,6 +260,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     // the block's slab in global memory, [offset - cap][event] like the shared one
     st_.spill = SPILL ? reinterpret_cast<T*>(p.spill) + (size_t)blockIdx.x * p.spill_cx * EPW + q : nullptr;
     st_.cap = p.slab_cx;
+    st_.limit = p.spill_cx;
     // tasks: the records of the tier, or (re-evaluation) the record positions in the tier's flag list
     const long long first = p.bounds[p.tier], end = p.list ? first + p.list_count[p.tier] : (long long)p.bounds[p.tier + 1];
     const long long ntasks = (end - first + EPW - 1) / EPW;
@@ -672,7 +684,11 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     // any), or a result that is not a positive finite number: evaluated again in double-double
                     const double En = __ldcg(mrec + (n - 1) * p.rec_gstride);
                     if (!(0.5 * s_norm2(wamp) <= p.tau2 * En * En * w) || !(fabs(amp.re) + fabs(amp.im) >= p.tau_rho * asum) || !(w > 0.0))
-                        p.flag_list[first + atomicAdd(p.flag_count + p.tier, 1u)] = (uint32_t)idx;
+                    {
+                        const uint32_t at = atomicAdd(p.flag_count + p.tier, 1u);
+                        BG_CHECK(first + at < end);
+                        p.flag_list[first + at] = (uint32_t)idx;
+                    }
                 }
             }
         }

@@ -191,7 +191,7 @@ def test_conditioning_flag_reports_and_options(bg, oracle, wl):
         ward, rho = res[3][0], res[4][0]
         assert np.all(ward >= 0) and np.all((rho > 0) & (rho <= 1.0 + 1e-12))
         changed = res[2][0] != res[0][0]
-        flagged = (ward > 3e-14 * (1 - 1e-9)) | (rho < 3e-3 * (1 + 1e-9))   # the documented default rule for n = 6
+        flagged = (ward > 2e-14 * (1 - 1e-9)) | (rho < 3e-3 * (1 + 1e-9))   # the documented default rule for n = 6
         assert np.all(flagged[changed]) and abs(int(flagged.sum()) - res[2][1]) <= 2
         # a huge threshold and no cancellation test: nothing is re-evaluated, the bits equal the FP64 path
         bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 2)
