@@ -719,7 +719,9 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
     int nlaunch = 0;
     for (int k = 0; k < kTiers; k++) {
         blocks[k] = 0;
-        if (t->tiers.first_key[k] == t->tiers.first_key[k + 1] && k + 1 < kTiers) continue;   // no class in this tier
+        // no class in this tier (the last tier always runs: events with colour codes out of range are sorted behind
+        // every class and get their 0.0 there)
+        if (t->tiers.first_key[k] == t->tiers.first_key[k + 1] && (k + 1 < kTiers || t->dense)) continue;
         const size_t ring_bytes = G >= 8 ? (size_t)kRing * BLOCK * 16 : 0;
         slab[k] = shape.cap_cx > 0 ? std::min(t->tiers.slab_cx[k], shape.cap_cx) : t->tiers.slab_cx[k];
         smem[k] = ((size_t)EPW * slab[k] * ELEM + 15) / 16 * 16 + ring_bytes;

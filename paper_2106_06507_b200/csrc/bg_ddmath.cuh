@@ -54,6 +54,8 @@ __device__ __forceinline__ dd dd_twice(dd a) { return mkdd(2.0 * a.hi, 2.0 * a.l
 __device__ __forceinline__ cxd mkd(dd re, dd im) { cxd r; r.re = re; r.im = im; return r; }
 __device__ __forceinline__ cxd cxd_add(cxd a, cxd b) { return mkd(dd_add(a.re, b.re), dd_add(a.im, b.im)); }
 __device__ __forceinline__ cxd cxd_neg(cxd a) { return mkd(dd_neg(a.re), dd_neg(a.im)); }
+// (Tried: cfma as a real function to shrink the ~10k-instruction kernel body, which stalls on instruction fetch -
+// the argument moves cost as many instructions as the body saves; 20 % slower.  DESIGN.md 9.)
 __device__ __forceinline__ void cfma(cxd& acc, cxd a, cxd b) {
     dd_fma(acc.re, a.re, b.re);
     dd_fma(acc.re, dd_neg(a.im), b.im);
