@@ -219,6 +219,17 @@ const char* bg_strerror(int code);
  */
 int bg_fp64_peak_probe(int iterations, double* tflops);
 
+/*
+ * Measure step a7 alone - the full-colour quadratic form of Eq. 16 for E synthetic amplitude
+ * vectors of (n-2)! entries, n = 6, 7, 8 - with plain DFMA row dots (the scheme of the COBG kernels) and on the FP64
+ * tensor path (mma.sync.m8n8k4.f64).  Writes the milliseconds per pass of either variant and the largest
+ * relative difference of their results; optionally copies the amplitudes (x_host[E][2][(n-2)!]: real parts, then
+ * imaginary parts of an event) and the tensor-path results (w_host[E]) to host buffers.  Synchronous, allocates its own
+ * device memory.
+ */
+int bg_colour_form_probe(int n, long long E, int iterations, double* ms_dfma, double* ms_dmma, double* max_rel_diff,
+                         double* x_host, double* w_host);
+
 #ifdef __cplusplus
 }
 #endif

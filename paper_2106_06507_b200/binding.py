@@ -31,7 +31,7 @@ BG_OPT_FLAG_THRESHOLD, BG_OPT_FLAG_CANCELLATION = 7, 8
 
 EXPORTS = ("bg_init", "bg_eval", "bg_eval_continuous", "bg_generate", "bg_colour_rule", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",
            "bg_set_option", "bg_colour_matrix", "bg_build_colour_matrix", "bg_last_launch_count",
-           "bg_last_kernel_name", "bg_last_kernel_ms", "bg_last_refined", "bg_class_program_stats", "bg_comc_program_stats", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe")
+           "bg_last_kernel_name", "bg_last_kernel_ms", "bg_last_refined", "bg_class_program_stats", "bg_comc_program_stats", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe", "bg_colour_form_probe")
 
 
 class BgError(RuntimeError):
@@ -85,6 +85,9 @@ def load():
         lib.bg_strerror.argtypes = [i]
         lib.bg_strerror.restype = ctypes.c_char_p
         lib.bg_fp64_peak_probe.argtypes = [i, ctypes.POINTER(ctypes.c_double)]
+        dp = ctypes.POINTER(ctypes.c_double)
+        lib.bg_colour_form_probe.argtypes = [i, ll, i, dp, dp, dp, vp, vp]
+        lib.bg_colour_form_probe.restype = i
         for name in ("bg_init", "bg_eval", "bg_eval_host", "bg_reserve", "bg_set_option", "bg_colour_matrix",
                      "bg_build_colour_matrix", "bg_last_launch_count", "bg_destroy", "bg_fp64_peak_probe"):
             getattr(lib, name).restype = i
@@ -237,3 +240,18 @@ def bg_fp64_peak_probe(iterations: int = 1 << 16) -> float:
     v = ctypes.c_double()
     _check(load().bg_fp64_peak_probe(iterations, ctypes.byref(v)), "bg_fp64_peak_probe")
     return v.value
+
+
+def bg_colour_form_probe(n: int, E: int, iterations: int = 5, return_data: bool = False):
+    """Step a7 alone: (ms per pass with DFMA row dots, ms per pass with mma.sync.m8n8k4.f64, max relative difference)
+    [+ amplitudes x[E][2][(n-2)!] and tensor-path results w[E] when return_data]."""
+    import math
+    import numpy as np
+    a, b, d = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    x = w = None
+    if return_data:
+        x = np.empty((E, 2, math.factorial(n - 2)))
+        w = np.empty(E)
+    _check(load().bg_colour_form_probe(n, E, iterations, ctypes.byref(a), ctypes.byref(b), ctypes.byref(d), _ptr(x), _ptr(w)),
+           "bg_colour_form_probe")
+    return (a.value, b.value, d.value) + ((x, w) if return_data else ())

@@ -299,7 +299,7 @@ static long long generic_chunk(const bg_ctx* c, long long N) {
 size_t bg_scratch_bytes(const bg_ctx* c, long long N) {
     if (!c || N <= 0) return 0;
     if (use_cobg_dd(c)) return bg::cobg_dd_scratch_per_event(c->n, (c->mode & BG_HEL_SUM) != 0) * (size_t)cobg_dd_chunk(c, N);
-    if (use_cobg_auto(c)) return 64 + (size_t)N * 4;   // flag counter | flagged event ids
+    if (use_cobg_auto(c)) return 256 + (size_t)N * 4;   // flag counter | flagged event ids
     if (c->mode == BG_COMC_GIVEN) return c->prog ? bg::prog_scratch_bytes(c->prog, N) : 0;
     if (!(c->mode & BG_REC_CDBG)) return 0;
     if (use_dd(c)) return bg::cdbg_dd_scratch_per_event(c->n) * (size_t)dd_chunk(c, N);
@@ -548,7 +548,7 @@ int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const 
         int rc = ensure_scratch(c, N);
         if (rc != BG_OK) return rc;
         uint32_t* count = (uint32_t*)c->scratch;
-        uint32_t* list = count + 16;
+        uint32_t* list = count + 64;
         const bool flag = c->precision == 2;
         if (cudaMemsetAsync(count, 0, 64, s) != cudaSuccess) return BG_ECUDA;
         if (ev0) cudaEventRecord(ev0, s);
@@ -557,7 +557,7 @@ int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const 
         if (flag && err == cudaSuccess) {
             if (c->timing) cudaEventRecord(c->ev_mid, s);
             err = bg::cobg_dd_flagged_launch(s, c->n, c->nperm, c->dC, N, list, count, c->sm_count * 2, mom, hel, out);
-            c->last_launches = 2;
+            c->last_launches++;
         }
         if (ev1) cudaEventRecord(ev1, s);
         c->last_auto = flag;
@@ -689,6 +689,14 @@ int bg_colour_rule(int n, const signed char* col) {
     for (int k = 0; k < 2 * n; k++)
         if (col[k] < 1 || col[k] > 3) return BG_EINVAL;
     return bg::colour_rule_host(n, col) ? 1 : 0;
+}
+
+int bg_colour_form_probe(int n, long long E, int iterations, double* ms_dfma, double* ms_dmma, double* max_rel_diff,
+                         double* x_host, double* w_host) {
+    if (n < 6 || n > 8 || E < 1 || iterations < 1 || !ms_dfma || !ms_dmma || !max_rel_diff) return BG_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return BG_ECUDA;
+    return bg::colour_form_probe(n, E, iterations, ms_dfma, ms_dmma, max_rel_diff, x_host, w_host) == cudaSuccess ? BG_OK : BG_ECUDA;
 }
 
 int bg_fp64_peak_probe(int iterations, double* tflops) {

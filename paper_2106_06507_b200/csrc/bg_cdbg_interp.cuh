@@ -265,7 +265,6 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     const long long first = p.bounds[p.tier], end = p.list ? first + p.list_count[p.tier] : (long long)p.bounds[p.tier + 1];
     const long long ntasks = (end - first + EPW - 1) / EPW;
     auto rec_pos = [&](long long i) -> long long { return p.list ? (long long)__ldg(p.list + i) : i; };
-    const long long N = p.N;
     const int n = p.n;
     // lanes of one event (same q) run the same program and meet at its barriers; events of different classes in
     // one warp pass different numbers of barriers, so the barrier names only the event's own lanes
@@ -310,7 +309,9 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         const double* mrec = reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
         // discrete states: the setup level gives gluon k to lane k % G, so the lane's first momentum is requested
         // here, ahead of the dependent loads class info -> ops that the setup ops themselves wait for
-        const bool discrete = !kUseRing && p.rec_gstride == 4 && kComplex;   // (G >= 8: measured 1-2 % slower)
+        // (G >= 8: measured 1-2 % slower; double-double: one copy of the polarisation code less in a body that
+        // already overflows the instruction caches)
+        const bool discrete = !kUseRing && p.rec_gstride == 4 && kComplex && !StateElem<S>::kDD;
         double pk[4] = {0.0, 0.0, 0.0, 0.0};
         if (discrete && g < n) {
 #pragma unroll

@@ -116,6 +116,10 @@ cudaError_t generate_launch(cudaStream_t s, int n, long long N, uint64_t seed, u
                             signed char* col);
 bool colour_rule_host(int n, const signed char* col);
 
+// ---- colour-form probe (bg_colour_probe.cu): a7 alone, DFMA row dots against mma.sync.m8n8k4.f64 -------------
+cudaError_t colour_form_probe(int n, long long E, int iters, double* ms_dfma, double* ms_dmma, double* max_rel_diff,
+                              double* x_host, double* w_host);
+
 // ---- FP64 peak probe ----------------------------------------------------------------------------------
 cudaError_t fp64_probe(int iterations, double* tflops);
 

@@ -551,3 +551,15 @@ def test_device_colour_matrix_equals_oracle(bg, oracle):
 def test_fp64_peak_probe_is_sane(bg):
     tf = bg.bg_fp64_peak_probe(1 << 13)
     assert 20.0 < tf < 45.0          # B200: 148 SMs x 64 FP64 lanes x 2 x <= 1.965 GHz = 37.2 TFLOP/s nominal
+
+
+@pytest.mark.parametrize("n,E", [(6, 1000), (7, 333), (8, 37)])
+def test_colour_form_probe_variants_agree(bg, n, E):
+    """Step a7 alone (Eq. 16) with DFMA row dots and on the FP64 tensor path (mma.sync.m8n8k4.f64): same numbers, and
+    equal to the quadratic form evaluated on the host with the same (integer) colour matrix."""
+    ms_dfma, ms_dmma, diff, x, w = bg.bg_colour_form_probe(n, E, 1, return_data=True)
+    assert ms_dfma > 0 and ms_dmma > 0 and diff < 1e-13
+    C = bg.bg_build_colour_matrix(n).astype(np.longdouble)
+    xr, xi = x[:, 0].astype(np.longdouble), x[:, 1].astype(np.longdouble)
+    ref = (np.einsum("ei,ij,ej->e", xr, C, xr) + np.einsum("ei,ij,ej->e", xi, C, xi)).astype(np.float64)
+    assert rel_err(w, ref).max() < 1e-12
