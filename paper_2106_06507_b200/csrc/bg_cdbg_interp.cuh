@@ -309,9 +309,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
         const double* mrec = reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
         // discrete states: the setup level gives gluon k to lane k % G, so the lane's first momentum is requested
         // here, ahead of the dependent loads class info -> ops that the setup ops themselves wait for
-        // (G >= 8: measured 1-2 % slower; double-double: one copy of the polarisation code less in a body that
-        // already overflows the instruction caches)
-        const bool discrete = !kUseRing && p.rec_gstride == 4 && kComplex && !StateElem<S>::kDD;
+        const bool discrete = !kUseRing && p.rec_gstride == 4 && kComplex;   // (G >= 8: measured 1-2 % slower)
         double pk[4] = {0.0, 0.0, 0.0, 0.0};
         if (discrete && g < n) {
 #pragma unroll
@@ -706,10 +704,14 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
     static int configured_device = -1;   // the attribute is per device
     int device = 0;
     cudaGetDevice(&device);
+    static size_t static_smem = 0;       // the kernel's static shared memory (reduction scratch)
     if (configured_device != device) {
         cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL, S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)(kMaxSlabBytes + (size_t)kRing * BLOCK * 16));
         if (e != cudaSuccess) return e;
+        cudaFuncAttributes fa;
+        if ((e = cudaFuncGetAttributes(&fa, cdbg_prog_kernel<G, SPILL, S>)) != cudaSuccess) return e;
+        static_smem = fa.sharedSizeBytes;
         configured_device = device;
     }
     const long long max_tasks = (p.N + EPW - 1) / EPW + kTiers;
@@ -727,8 +729,9 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         slab[k] = shape.cap_cx > 0 ? std::min(t->tiers.slab_cx[k], shape.cap_cx) : t->tiers.slab_cx[k];
         smem[k] = ((size_t)EPW * slab[k] * ELEM + 15) / 16 * 16 + ring_bytes;
         if (smem[k] > kMaxSlabBytes + ring_bytes) return cudaErrorInvalidValue;
-        // resident blocks per SM: shared memory (1 KB reserved per block), and 65536 / (regs x BLOCK) registers
-        int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (shape.regs * BLOCK), (228 * 1024) / (smem[k] + 1024)));
+        // resident blocks per SM: 228 KB of shared memory against dynamic + static + 1 KB reserved per block (a grid
+        // sized for one block more than fits runs a second, nearly empty wave), and 65536 / (regs x BLOCK) registers
+        int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (shape.regs * BLOCK), (228 * 1024) / (smem[k] + 1024 + static_smem)));
         if (SPILL) per_sm = std::min(per_sm, shape.spill_blocks);   // one global slab per resident block
         blocks[k] = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
         if (shape.max_blocks > 0) blocks[k] = (unsigned)std::min<long long>(blocks[k], shape.max_blocks);

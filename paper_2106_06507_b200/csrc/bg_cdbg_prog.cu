@@ -459,7 +459,7 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
         const int cap_cx = (int)(slab_limit / 16 / (size_t)epw);      // larger states spill (or are refused below)
         const int reg_blocks = std::max(1, 65536 / (168 * block));
         auto rate = [&](int slab_cx) {
-            const size_t smem = (size_t)slab_cx * epw * 16 + ring_bytes + 1024;
+            const size_t smem = (size_t)slab_cx * epw * 16 + ring_bytes + 1024 + 512;   // + reserved per block + static (<= 384 B)
             const int blocks = (int)std::max<size_t>(1, std::min<size_t>({(size_t)reg_blocks, (size_t)32, (size_t)(228 * 1024) / smem}));
             const double w = blocks * (block / 32.0);
             return w / (w + 7.0);
@@ -539,7 +539,7 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
     {   // blocks of the largest tier that fit an SM (shared memory and registers)
         const size_t smem0 = (size_t)tiers.slab_cx[0] * 16;
         const int block = G > 32 ? G : 32;
-        t->spill_blocks_per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * block), (228 * 1024) / (smem0 + 1024)));
+        t->spill_blocks_per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * block), (228 * 1024) / (smem0 + 1024 + 512)));
     }
     {
         int dev = 0;
@@ -643,7 +643,7 @@ int prog_table_create_dense(int n, int G, size_t slab_limit, bool real, ProgTabl
     {
         const size_t smem0 = (size_t)t->tiers.slab_cx[0] * elem;
         const int block = G > 32 ? G : 32;
-        t->spill_blocks_per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * block), (228 * 1024) / (smem0 + 1024)));
+        t->spill_blocks_per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (168 * block), (228 * 1024) / (smem0 + 1024 + 512)));
         int dev = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);

@@ -40,9 +40,9 @@ __device__ __forceinline__ double r_hi(dd x) { return x.hi; }
 // 1/sqrt2 to 106 bits
 __device__ __forceinline__ dd dd_isqrt2() { return mkdd(0.70710678118654757, -4.8336466567264567e-17); }
 __device__ __forceinline__ cxd s_isqrt2(cxd v) { return cxd_scale(dd_isqrt2(), v); }
-__device__ __noinline__ dd r_isqrt2_over(dd p2) { return dd_isqrt2() / p2; }   // once per finished current
+__device__ __forceinline__ dd r_isqrt2_over(dd p2) { return dd_isqrt2() / p2; }
 __device__ __forceinline__ cxd s_scale(dd f, cxd v) { return cxd_scale(f, v); }
-__device__ __noinline__ void ext_current(const double* pk, int lambda, cxd* eps) {   // n calls per event: not worth inlining
+__device__ __forceinline__ void ext_current(const double* pk, int lambda, cxd* eps) {
     dd p[4];
 #pragma unroll
     for (int c = 0; c < 4; c++) p[c] = mkdd(pk[c]);

@@ -14,6 +14,7 @@ namespace bg {
 
 using cxd = cxt<dd>;
 
+
 // acc += a*b.  (The leading product is formed with __dmul_rn: a plain a.hi * b.hi could be contracted with the
 // following addition into one FMA, and the two-sum below is error-free only for the rounded product.)
 __device__ __forceinline__ void dd_fma(dd& acc, dd a, dd b) {
