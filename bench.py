@@ -135,6 +135,11 @@ def measure_config(bg, wl, oracle_mod, dev, config: int, n: int, steps: int, pea
                            "frac": flop * N / (fp64_kms * 1e-3) * 1e-12 / peak_tf}
         if config == 0:
             res["note"] = "1024 events: one 13 us launch, launch-latency bound (SURVEY 8d); FP64 alone meets 1e-11"
+        if config == 2:
+            a, b, dmax = bg.bg_colour_form_probe(n, N, 3)
+            res["colour_form_probe"] = {"dfma_row_dots_ms": a, "dmma_m8n8k4_ms": b, "max_rel_diff": dmax,
+                                        "note": "step a7 alone on synthetic amplitudes (bg_colour_form_probe); the production "
+                                                "kernel keeps the fused DFMA form (DESIGN.md 5.2)"}
         if auto:
             ms0, kms0, _, _ = timed(0)
             res["precision_auto"] = {"flagged_frac": fl / N, "reevaluation_ms": rms,
@@ -431,7 +436,9 @@ def run_b200(args):
     # generation on the device inside the timed region (the paper's timings include phase-space generation, L259):
     # nothing crosses PCIe but the seed
     devgen = None
-    if args.device_gen and not args.continuous:
+    default_line = (world == 1 and args.config == 1 and args.events is None and args.precision is None and not args.kernel
+                    and args.lanes is None and not (args.continuous or args.comc or args.lc))
+    if (args.device_gen or default_line) and not args.continuous:
         g_mom = torch.empty_like(d_mom)
         g_hel = None if d_hel is None or (mode & bg.BG_HEL_SUM) else torch.empty_like(d_hel)
         g_col = None if d_col is None or not (mode & bg.BG_COL_GIVEN) else torch.empty_like(d_col)
@@ -557,8 +564,7 @@ def run_b200(args):
             line["precision_auto"] = {"flagged_frac": flagged / N, "reevaluation_ms": refine_ms,
                                       "overhead_pct": 100.0 * (total_ms / args.steps / ms0 - 1.0),
                                       "fp64_only_events_per_s": N / (ms0 * 1e-3), "fp64_only_ms_per_step": ms0}
-        if world == 1 and args.config == 1 and not args.no_configs and not (args.continuous or args.comc or args.lc) \
-                and args.events is None and args.precision is None and not args.kernel and args.lanes is None:
+        if default_line and not args.no_configs:
             # every BASELINE.json config in the same record: C1, C3, C4 and the C5 sweep n = 4..12 ("events/s vs n")
             import oracle as oracle_mod
             ksteps = max(3, min(args.steps, 10))

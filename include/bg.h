@@ -111,6 +111,10 @@ int bg_init(bg_ctx** ctx, int n, int mode);
  *   CDBG + GIVEN colour: out[e] = |A_{i1 j1 .. in jn}|^2 from the subset recursion Eq. 29-32 closed with gluon n
  *                        (Eq. 22); assignments whose amplitude vanishes identically return exactly 0.0.
  * External currents are the helicity eigenvectors of Eq. 3 in the light-cone gauge of DESIGN.md reading g2.
+ * A context serves ONE bg_eval at a time: its scratch (event records, class histogram and ticket buffer of the prepass,
+ * flag lists, spill slabs) and its side streams are per context, so two calls in flight on different streams - or a
+ * call issued while bg_eval_host is running - race.  Use one context per concurrently used stream; calls on the same
+ * stream are ordered by the stream.  N may not exceed 2^32 - 1 (BG_EINVAL).
  * No host synchronisation and no allocation happen here when bg_reserve was called for >= N events; otherwise
  * scratch is (re)allocated first, which synchronises.  Inputs are not validated on the device: non-finite or
  * off-shell momenta give unspecified (possibly NaN) output, never a fault.  N = 0 is a no-op.

@@ -130,7 +130,9 @@ static int auto_lanes(int n) {
 }
 
 // shared memory one event's state may take before its top levels spill to global memory (0 = all of it)
-static size_t auto_slab_limit(int n) { return n >= 11 ? (size_t)104 * 1024 : 0; }   // two blocks per SM (with their op rings), measured
+// measured (2^16 events, FP64): n = 11: 48 / 56 / 64 / 104 KB -> 2.67 / 2.77 / 2.40 / 2.40e6 events/s (three blocks per SM at
+// 56 KB); n = 12: 56 / 80 / 88 / 96 / 104 KB -> 8.1 / 8.6 / 8.8 / 7.4 / 7.7e5 (two blocks per SM)
+static size_t auto_slab_limit(int n) { return n == 11 ? (size_t)56 * 1024 : (n >= 12 ? (size_t)88 * 1024 : 0); }
 
 extern "C" {
 static int make_prog_table(const bg_ctx* c, int G, size_t limit, bg::ProgTable** t);
