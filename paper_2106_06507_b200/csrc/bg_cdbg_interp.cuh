@@ -105,6 +105,7 @@ struct ProgParams {
     // re-evaluation launches read their tasks from the lists instead of the record ranges
     const uint32_t* list;      // nullptr: all records of the tier
     const uint32_t* list_count;
+    uint32_t* ticket;          // [kTiers] next list task of the tier (zeroed with the flag counters)
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -276,30 +277,47 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     // the current one computes (events come in class order, so their rows are scattered over the input arrays)
     EventHeader hnext;
     hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
-    if ((long long)blockIdx.x < ntasks) {
-        const long long idx = first + (long long)blockIdx.x * EPW + q;
-        if (idx < end) hnext = ld_header(p.rec + (size_t)rec_pos(idx) * p.rec_bytes);
-    }
+    // Tasks: record ranges are dealt round-robin (task += gridDim.x: the records are sorted longest program first).
+    // List tasks (re-evaluation) arrive in the random order of the flag appends and take 14 x longer each, so a static
+    // deal leaves a long tail: they are handed out by a ticket counter instead, fetched one task ahead.
+    auto next_ticket = [&]() -> long long {
+        if constexpr (G <= 32) {
+            unsigned v = 0;
+            if (lane == 0) v = atomicAdd(p.ticket + p.tier, 1u);
+            return (long long)__shfl_sync(0xFFFFFFFFu, v, 0);
+        } else {
+            __shared__ unsigned tk;
+            __syncthreads();
+            if (lane == 0) tk = atomicAdd(p.ticket + p.tier, 1u);
+            __syncthreads();
+            return (long long)tk;
+        }
+    };
+    long long task = p.list ? next_ticket() : (long long)blockIdx.x;
+    long long task_next = task < ntasks ? (p.list ? next_ticket() : task + gridDim.x) : ntasks;
     long long pos_next = 0;    // record position of the next task's event (equals its index unless a list is read)
-    if (p.list && (long long)blockIdx.x < ntasks) {
-        const long long idx = first + (long long)blockIdx.x * EPW + q;
-        if (idx < end) pos_next = rec_pos(idx);
+    if (task < ntasks) {
+        const long long idx = first + task * EPW + q;
+        if (idx < end) {
+            pos_next = rec_pos(idx);
+            hnext = ld_header(p.rec + (size_t)pos_next * p.rec_bytes);
+        }
     }
     // carried from one task to the next: the class info of the next event, requested at the first barrier of the
     // current task (one load less in the chain header -> info -> ops -> inputs at the start of a task)
     uint4 ci_next = make_uint4(0, 0, 0, 0);
     bool ci_next_ok = false;
-    for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
+    for (; task < ntasks; task = task_next, task_next = task_next < ntasks ? (p.list ? next_ticket() : task_next + gridDim.x) : ntasks) {
         const long long idx0 = first + task * EPW + q;
         const bool have = idx0 < end;
         const long long idx = p.list ? pos_next : idx0;          // record position
         const EventHeader h = hnext;
         long long idx_next = 0;
         {
-            const long long idx2 = idx0 + (long long)gridDim.x * EPW;
+            const long long idx2 = first + task_next * EPW + q;
             hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
             idx_next = idx2;
-            if (task + gridDim.x < ntasks && idx2 < end) {
+            if (task_next < ntasks && idx2 < end) {
                 if (p.list) idx_next = pos_next = rec_pos(idx2);
                 hnext = ld_header(p.rec + (size_t)idx_next * p.rec_bytes);
             }

@@ -51,7 +51,7 @@ cdbg_classify_kernel(int n, long long N, long long num_classes, const signed cha
                      uint32_t* __restrict__ flag_count) {
     extern __shared__ uint32_t sh_hist[];
     const int nbins = (int)num_classes + 1;
-    if (blockIdx.x == 0 && threadIdx.x < kTiers) flag_count[threadIdx.x] = 0;   // lists of the conditioning flag
+    if (blockIdx.x == 0 && threadIdx.x < 2 * kTiers) flag_count[threadIdx.x] = 0;   // lists of the conditioning flag: counters | tickets
     if (BLOCK_HIST) {
         for (int i = threadIdx.x; i < nbins; i += THREADS) sh_hist[i] = 0;
         __syncthreads();
@@ -858,6 +858,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.flag_count = flag_count;
     p.list = nullptr;
     p.list_count = nullptr;
+    p.ticket = flag_count + kTiers;
     *launches = fused ? 2 : 3;
     if (ev0) cudaEventRecord(ev0, s);
     err = dispatch_interp(s, t, sm_count, p, launches, true);
@@ -895,7 +896,7 @@ cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, 
     p.slab_cx = t->max_state_cx;
     p.tau2 = 0.0;
     p.tau_rho = 0.0;
-    p.flag_list = nullptr; p.flag_count = nullptr; p.list = nullptr; p.list_count = nullptr;
+    p.flag_list = nullptr; p.flag_count = nullptr; p.list = nullptr; p.list_count = nullptr; p.ticket = nullptr;
     *launches = 1;
     if (ev0) cudaEventRecord(ev0, s);
     err = dispatch_interp(s, t, sm_count, p, launches, false);
