@@ -34,6 +34,7 @@ COBG_FLOP_PER_EVENT = {0: 2.6e4, 2: 1.41e6 + 5.8e4}     # config 0 (n=4 helsum),
 TRAFFIC_CSV = os.path.join("profiles", "r02_dram_traffic.csv")     # kernel,n,events,bytes_per_step,source
 CONFIG_N = {0: 4, 1: 6, 2: 7, 3: 9}
 CONFIG_EVENTS = {0: 1024, 1: 1 << 20, 2: 1 << 18, 3: 1 << 18, 4: 1 << 16}
+COBG_N8_EVENTS = 1 << 14      # extra line: colour-ordered n = 8 (720 orderings, 720 x 720 colour matrix)
 
 
 def parse_args():
@@ -86,10 +87,13 @@ def measure_config(bg, wl, oracle_mod, dev, config: int, n: int, steps: int, pea
     the FP64-only path beside it, the FP64 kernel's roofline fraction, the conditioning flag's cost, the CPU oracle
     (all cores / one core) and parity against the long-double oracle on a stated sample."""
     import torch
-    N = CONFIG_EVENTS[config]
-    ev = wl.config_events(config, N=N, n=n if config == 4 else None)
+    cobg8 = config == 2 and n == 8
+    N = COBG_N8_EVENTS if cobg8 else CONFIG_EVENTS[config]
+    ev = wl.config_events(4, N=N, n=8) if cobg8 else wl.config_events(config, N=N, n=n if config == 4 else None)
     mode = mode_for(config)
     flop = COBG_FLOP_PER_EVENT[config] if config in (0, 2) else CDBG_FLOP_PER_EVENT[n]
+    if cobg8:       # 720 orderings x (C(8,3) V3 + C(8,4) V4) at 158 / 178 flop + 2 x 720^2 MAC (SURVEY 8d counting)
+        flop = 720 * (56 * 158 + 70 * 178) + 4.0 * 720 * 720
     d_mom = torch.from_numpy(wl.to_soa(mom=ev.mom)).to(dev)
     d_hel = None if ev.hel is None or (mode & bg.BG_HEL_SUM) else torch.from_numpy(wl.to_soa(hel=ev.hel)).to(dev)
     d_col = None if not (mode & bg.BG_COL_GIVEN) else torch.from_numpy(wl.to_soa(col=ev.col)).to(dev)
@@ -97,7 +101,7 @@ def measure_config(bg, wl, oracle_mod, dev, config: int, n: int, steps: int, pea
     stream = torch.cuda.current_stream()
     sh = stream.cuda_stream
     ctx = bg.bg_init(n, mode)
-    res = {"workload": {0: "C1", 2: "C3", 3: "C4", 4: "C5"}.get(config, "C2") + f" n={n}", "n": n, "events": N}
+    res = {"workload": ("COBG full colour (extra)" if cobg8 else {0: "C1", 2: "C3", 3: "C4", 4: "C5"}.get(config, "C2")) + f" n={n}", "n": n, "events": N}
     try:
         bg.bg_reserve(ctx, N)
         auto = config != 0
@@ -135,7 +139,7 @@ def measure_config(bg, wl, oracle_mod, dev, config: int, n: int, steps: int, pea
                            "frac": flop * N / (fp64_kms * 1e-3) * 1e-12 / peak_tf}
         if config == 0:
             res["note"] = "1024 events: one 13 us launch, launch-latency bound (SURVEY 8d); FP64 alone meets 1e-11"
-        if config == 2:
+        if config == 2 and not cobg8:
             a, b, dmax = bg.bg_colour_form_probe(n, N, 3)
             res["colour_form_probe"] = {"dfma_row_dots_ms": a, "dmma_m8n8k4_ms": b, "max_rel_diff": dmax,
                                         "note": "step a7 alone on synthetic amplitudes (bg_colour_form_probe); the production "
@@ -153,15 +157,20 @@ def measure_config(bg, wl, oracle_mod, dev, config: int, n: int, steps: int, pea
         sub = ev.head(S)
         if config == 0:
             truth = oracle_mod.cobg_full_colour(sub.mom, None, prec="long double")
+        elif cobg8:
+            truth, S = None, 0        # the oracle's Gell-Mann colour matrix is out of reach at n = 8 (tests/: amplitudes + Eq. 17)
         elif config == 2:
             S = min(S, 1024)
             sub = ev.head(S)
             truth = oracle_mod.cobg_full_colour(sub.mom, sub.hel, prec="long double")
         else:
             truth = oracle_mod.cdbg(sub.mom, sub.hel, sub.col, prec="long double")
-        err = np.abs(got[:S] - truth) / np.abs(truth)
-        res["parity"] = {"max_rel_err_vs_long_double": float(err.max()), "median": float(np.median(err)),
-                         "n_over_1e-11": int(np.sum(err > 1e-11)), "sample": f"first {S} events"}
+        if truth is not None:
+            err = np.abs(got[:S] - truth) / np.abs(truth)
+            res["parity"] = {"max_rel_err_vs_long_double": float(err.max()), "median": float(np.median(err)),
+                             "n_over_1e-11": int(np.sum(err > 1e-11)), "sample": f"first {S} events"}
+        if cobg8:
+            return res
 
         class A:
             pass
@@ -573,6 +582,7 @@ def run_b200(args):
             cfgs["C1"] = measure_config(bg, wl, oracle_mod, dev, 0, 4, max(ksteps, 20), peak_tf, with_cpu)
             cfgs["C3"] = measure_config(bg, wl, oracle_mod, dev, 2, 7, ksteps, peak_tf, with_cpu)
             cfgs["C4"] = measure_config(bg, wl, oracle_mod, dev, 3, 9, ksteps, peak_tf, with_cpu)
+            cfgs["COBG_n8"] = measure_config(bg, wl, oracle_mod, dev, 2, 8, 3, peak_tf, with_cpu)
             cfgs["C5"] = {str(k): measure_config(bg, wl, oracle_mod, dev, 4, k, ksteps, peak_tf, with_cpu) for k in range(4, 13)}
             line["configs"] = cfgs
         print(json.dumps(line), flush=True)

@@ -47,7 +47,7 @@ enum {
     BG_HEL_GIVEN = 0x020, /* one assignment per event in hel */
     BG_COL_FULL = 0x100,  /* full-colour sum sum_{s,s'} C_{ss'} A_s A_s'^*, Eq. 15-17; col NULL */
     BG_COL_LC = 0x400,    /* leading-colour approximation N_c^(n-2) (N_c^2-1) sum_{S_(n-1)} |A|^2, Eq. 33
-                             without its O(1/N_c^2) remainder; col NULL; COBG, n <= 7 */
+                             without its O(1/N_c^2) remainder; col NULL; COBG, n <= 8 */
     BG_HEL_CONT = 0x040,  /* continuous polarisation angle phi per gluon, real e(phi) of Eq. 7 */
     BG_COL_CONT = 0x800,  /* continuous colour states: two real unit 3-vectors (eta, etabar) per gluon, Eq. 9, 12 */
     BG_COL_GIVEN = 0x200, /* one colour-flow assignment (i_k, j_k) per gluon per event in col, Eq. 19 */

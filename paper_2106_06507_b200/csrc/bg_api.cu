@@ -142,7 +142,7 @@ static int make_prog_table(const bg_ctx* c, int G, size_t limit, bg::ProgTable**
 // an event is evaluated again in double-double arithmetic; tuned against the extended-precision oracle so that
 // no unflagged event of the test workloads is further than 1e-11 from it.
 static double default_tau(int n) { return n == 6 ? 2e-14 : (n == 5 ? 3e-14 : 1e-13); }
-static double default_tau_cobg(int n) { return n >= 7 ? 3e-13 : 1e-13; }
+static double default_tau_cobg(int n) { return n >= 7 ? 3e-13 : 1e-13; }   // (n = 8: as n = 7; sampled)
 static const double kDefaultTauRho = 3e-3;
 
 static bool mode_supported(int n, int mode) {

@@ -4,6 +4,8 @@
 // have near-zeros by cancellation where FP64 round-off exceeds 1e-11; evaluated with
 // ~106-bit significands the same inputs reproduce the extended-precision oracle on every event, which shows that
 // what is left in the FP64 kernels is rounding, not arithmetic.  Not a performance path.
+#include <algorithm>
+
 #include "bg_ddmath.cuh"
 #include "bg_internal.h"
 
@@ -289,38 +291,38 @@ cobg_dd_amp_kernel(int n, int nhel, int nperm, long long N, long long first, lon
 
 // Re-evaluation of the events the FP64 kernel flagged (BG_OPT_PRECISION = 2, given helicities): one block per listed
 // event, one thread per ordering; the amplitudes stay in shared memory and thread s takes row s of Eq. 16.
-__global__ void __launch_bounds__(128)   // (n <= 7: at most 120 orderings)
+__global__ void __launch_bounds__(128)
 cobg_dd_flagged_kernel(int n, int nperm, long long N, const uint32_t* __restrict__ list, const uint32_t* __restrict__ count,
                        const double* __restrict__ mom, const signed char* __restrict__ hel, const double* __restrict__ Cm,
                        double* __restrict__ out) {
-    extern __shared__ double2 sh_amp[];   // [nperm][2]: (re.hi, re.lo), (im.hi, im.lo), then [blockDim / 32] partial sums
+    extern __shared__ double2 sh_amp[];   // [nperm][2]: (re.hi, re.lo), (im.hi, im.lo); reused for the row sums
     const uint32_t total = *count;
-    const int s = threadIdx.x;
     for (uint32_t it = blockIdx.x; it < total; it += gridDim.x) {
         const long long e = list[it];
         __syncthreads();
-        if (s < nperm) {
+        for (int s = threadIdx.x; s < nperm; s += blockDim.x) {       // (n = 8: 720 orderings in rounds of 128)
             const C A = cobg_dd_amplitude(n, nperm, s, -1, N, e, mom, hel);
             sh_amp[2 * s] = make_double2(A.re.hi, A.re.lo);
             sh_amp[2 * s + 1] = make_double2(A.im.hi, A.im.lo);
         }
         __syncthreads();
-        dd row = mkdd(0.0);
-        if (s < nperm) {
+        dd mine = mkdd(0.0);
+        for (int s = threadIdx.x; s < nperm; s += blockDim.x) {
             dd tr = mkdd(0.0), ti = mkdd(0.0);
             for (int s2 = 0; s2 < nperm; s2++) {
                 const dd c = mkdd(Cm[(size_t)s * nperm + s2]);
-                tr = tr + c * mkdd(sh_amp[2 * s2].x, sh_amp[2 * s2].y);
-                ti = ti + c * mkdd(sh_amp[2 * s2 + 1].x, sh_amp[2 * s2 + 1].y);
+                dd_fma(tr, c, mkdd(sh_amp[2 * s2].x, sh_amp[2 * s2].y));
+                dd_fma(ti, c, mkdd(sh_amp[2 * s2 + 1].x, sh_amp[2 * s2 + 1].y));
             }
-            row = mkdd(sh_amp[2 * s].x, sh_amp[2 * s].y) * tr + mkdd(sh_amp[2 * s + 1].x, sh_amp[2 * s + 1].y) * ti;
+            dd_fma(mine, mkdd(sh_amp[2 * s].x, sh_amp[2 * s].y), tr);
+            dd_fma(mine, mkdd(sh_amp[2 * s + 1].x, sh_amp[2 * s + 1].y), ti);
         }
         __syncthreads();
-        if (s < nperm) sh_amp[2 * s] = make_double2(row.hi, row.lo);
+        sh_amp[threadIdx.x] = make_double2(mine.hi, mine.lo);
         __syncthreads();
-        if (s == 0) {
+        if (threadIdx.x == 0) {
             dd sum = mkdd(0.0);
-            for (int s2 = 0; s2 < nperm; s2++) sum = sum + mkdd(sh_amp[2 * s2].x, sh_amp[2 * s2].y);
+            for (int s2 = 0; s2 < (int)blockDim.x; s2++) sum = sum + mkdd(sh_amp[s2].x, sh_amp[s2].y);
             out[e] = to_double(sum);
         }
     }
@@ -349,9 +351,8 @@ cobg_dd_colour_kernel(int nhel, int nperm, long long first, long long count, con
 
 cudaError_t cobg_dd_flagged_launch(cudaStream_t s, int n, int nperm, const double* dC, long long N, const uint32_t* list,
                                    const uint32_t* count, int blocks, const double* mom, const signed char* hel, double* out) {
-    const int threads = (nperm + 31) / 32 * 32;
-    if (threads > 128) return cudaErrorInvalidValue;
-    cobg_dd_flagged_kernel<<<blocks, threads, (size_t)nperm * 2 * sizeof(double2), s>>>(n, nperm, N, list, count, mom, hel, dC, out);
+    const int threads = std::min(128, (nperm + 31) / 32 * 32);
+    cobg_dd_flagged_kernel<<<blocks, threads, (size_t)std::max(nperm * 2, threads) * sizeof(double2), s>>>(n, nperm, N, list, count, mom, hel, dC, out);
     return cudaGetLastError();
 }
 

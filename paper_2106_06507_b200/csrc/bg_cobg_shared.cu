@@ -26,8 +26,8 @@
 
 namespace bg {
 
-constexpr int kCobgMaxM = 6;   // n - 1 <= 6: n = 4..7
-constexpr int kCobgMaxVals = 32;   // distinct entries of the colour matrix held in shared memory (16 at n = 7)
+constexpr int kCobgMaxM = 7;   // n - 1 <= 7: n = 4..8
+constexpr int kCobgMaxVals = 64;   // distinct entries of the colour matrix held in shared memory (16 at n = 7, 38 at n = 8)
 
 struct CobgTable {
     int n, np, nslots;
@@ -147,14 +147,17 @@ struct TopView {
     }
 };
 
+// TPE threads per event in blocks of max(128, TPE) threads; with more orderings than threads (n = 8: 720 orderings,
+// 256 threads) a thread takes the orderings t, t + TPE, .. in rounds.
 template <int NG, int TPE, bool LC>
-__global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p) {
-    constexpr int M = NG - 1, LS = NG - 3, EPB = 128 / TPE, NSUB = 1 << M;
+__global__ void __launch_bounds__(TPE > 128 ? TPE : 128, TPE > 128 ? 1 : 4) cobg_shared_kernel(const CobgParams p) {
+    constexpr int BLOCK = TPE > 128 ? TPE : 128;
+    constexpr int M = NG - 1, LS = NG - 3, EPB = BLOCK / TPE, NSUB = 1 << M;
     extern __shared__ double smem_d[];
     const int evl = threadIdx.x / TPE, t = threadIdx.x % TPE;
     const int np = p.np;
     // per-event shared block: currents | subset momenta | eps_n | amplitudes | reduction scratch
-    const int ev_doubles = p.nslots * 2 * kSlotStride + NSUB * 4 + 8 + np * 2 + 8;
+    const int ev_doubles = p.nslots * 2 * kSlotStride + NSUB * 4 + 8 + np * 2 + 16;
     double* cur = smem_d + (size_t)evl * ev_doubles;
     double* P = cur + p.nslots * 2 * kSlotStride;
     double* epsn = P + NSUB * 4;
@@ -199,8 +202,7 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
     tv.cur = cur;
     tv.P = P;
     const bool top = t < np;
-    {
-        const int sig = top ? t : 0;
+    auto load_view = [&](int sig) {
         tv.pm[0] = 0;
 #pragma unroll
         for (int i = 0; i < M; i++) {
@@ -208,7 +210,8 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
 #pragma unroll
             for (int j = 0; j < M; j++) tv.sl[i * M + j] = p.slot[(sig * M + i) * M + j];
         }
-    }
+    };
+    load_view(top ? t : 0);
 
     const int nhel = p.helsum ? (1 << NG) : 1;
     const int hc_step = p.helsum ? EPB : 1;
@@ -270,71 +273,75 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
         }
         // register-resident top: thread sigma builds the two (n-2)-gluon currents and the final one of its ordering
         double ward2 = 0.0, amp2 = 0.0;
-        if (top) {
+        for (int sig = t; sig < np; sig += TPE) {
+            if (sig != t || np > TPE) load_view(sig);      // (one ordering per thread: the view loaded above stays)
             tv.template range<1, M - 1, true>(tv.JA);
             tv.template range<0, M - 2, true>(tv.JB);
             cx JF[4], en[4];
             tv.template range<0, M - 1, false>(JF);
             lds_cur(epsn, 0, en);
             const cx amp = mdot(en, JF);
-            A[2 * t] = amp.re;
-            A[2 * t + 1] = amp.im;
+            A[2 * sig] = amp.re;
+            A[2 * sig + 1] = amp.im;
             if (!LC && p.tau2 != 0.0) {
                 // Ward identity: the current of gluons 1..n-1 is conserved, P . J = 0 with P = -p_n (round-off only)
                 const cx wv = mdot(P + 4 * (NSUB - 1), JF);
-                ward2 = s_norm2(wv);
-                amp2 = s_norm2(amp);
+                ward2 += s_norm2(wv);
+                amp2 += s_norm2(amp);
             }
         }
         __syncthreads();
         // Eq. 16: row sigma of the real symmetric quadratic form
         double w = 0.0;
-        if (top && LC) {
-            w = fma(A[2 * t], A[2 * t], A[2 * t + 1] * A[2 * t + 1]);
-        } else if (top) {
-            double tr[4] = {0.0, 0.0, 0.0, 0.0}, ti[4] = {0.0, 0.0, 0.0, 0.0};
-            const double* Ccol = p.C + t;
-            int s2 = 0;
-            if (p.nval) {
-                const uint32_t* ci = p.cidx4 + t;
+        if (LC) {
+            for (int row = t; row < np; row += TPE) w += fma(A[2 * row], A[2 * row], A[2 * row + 1] * A[2 * row + 1]);
+        } else {
+            for (int row = t; row < np; row += TPE) {
+                double tr[4] = {0.0, 0.0, 0.0, 0.0}, ti[4] = {0.0, 0.0, 0.0, 0.0};
+                const double* Ccol = p.C + row;
+                int s2 = 0;
+                if (p.nval) {
+                    const uint32_t* ci = p.cidx4 + row;
+                    for (; s2 + 4 <= np; s2 += 4) {
+                        const uint32_t w4 = __ldg(ci + (size_t)(s2 >> 2) * np);
+    #pragma unroll
+                        for (int u = 0; u < 4; u++) {
+                            const double c = cv[(w4 >> (8 * u)) & 0xFF];
+                            const double2 a2 = *reinterpret_cast<const double2*>(A + 2 * (s2 + u));
+                            tr[u] = fma(c, a2.x, tr[u]);
+                            ti[u] = fma(c, a2.y, ti[u]);
+                        }
+                    }
+                    if (s2 < np) {
+                        const uint32_t w4 = __ldg(ci + (size_t)(s2 >> 2) * np);
+                        for (int u = 0; s2 < np; s2++, u++) {
+                            const double c = cv[(w4 >> (8 * u)) & 0xFF];
+                            tr[0] = fma(c, A[2 * s2], tr[0]);
+                            ti[0] = fma(c, A[2 * s2 + 1], ti[0]);
+                        }
+                    }
+                }
                 for (; s2 + 4 <= np; s2 += 4) {
-                    const uint32_t w4 = __ldg(ci + (size_t)(s2 >> 2) * np);
-#pragma unroll
+    #pragma unroll
                     for (int u = 0; u < 4; u++) {
-                        const double c = cv[(w4 >> (8 * u)) & 0xFF];
+                        const double c = __ldg(Ccol + (size_t)(s2 + u) * np);
                         const double2 a2 = *reinterpret_cast<const double2*>(A + 2 * (s2 + u));
                         tr[u] = fma(c, a2.x, tr[u]);
                         ti[u] = fma(c, a2.y, ti[u]);
                     }
                 }
-                if (s2 < np) {
-                    const uint32_t w4 = __ldg(ci + (size_t)(s2 >> 2) * np);
-                    for (int u = 0; s2 < np; s2++, u++) {
-                        const double c = cv[(w4 >> (8 * u)) & 0xFF];
-                        tr[0] = fma(c, A[2 * s2], tr[0]);
-                        ti[0] = fma(c, A[2 * s2 + 1], ti[0]);
-                    }
+                for (; s2 < np; s2++) {
+                    const double c = __ldg(Ccol + (size_t)s2 * np);
+                    tr[0] = fma(c, A[2 * s2], tr[0]);
+                    ti[0] = fma(c, A[2 * s2 + 1], ti[0]);
                 }
+                w += fma(A[2 * row], (tr[0] + tr[1]) + (tr[2] + tr[3]), A[2 * row + 1] * ((ti[0] + ti[1]) + (ti[2] + ti[3])));
             }
-            for (; s2 + 4 <= np; s2 += 4) {
-#pragma unroll
-                for (int u = 0; u < 4; u++) {
-                    const double c = __ldg(Ccol + (size_t)(s2 + u) * np);
-                    const double2 a2 = *reinterpret_cast<const double2*>(A + 2 * (s2 + u));
-                    tr[u] = fma(c, a2.x, tr[u]);
-                    ti[u] = fma(c, a2.y, ti[u]);
-                }
-            }
-            for (; s2 < np; s2++) {
-                const double c = __ldg(Ccol + (size_t)s2 * np);
-                tr[0] = fma(c, A[2 * s2], tr[0]);
-                ti[0] = fma(c, A[2 * s2 + 1], ti[0]);
-            }
-            w = fma(A[2 * t], (tr[0] + tr[1]) + (tr[2] + tr[3]), A[2 * t + 1] * ((ti[0] + ti[1]) + (ti[2] + ti[3])));
         }
 #pragma unroll
         for (int d = 1; d < (TPE < 32 ? TPE : 32); d <<= 1) w += __shfl_xor_sync(0xFFFFFFFFu, w, d);
         if (TPE > 32) {
+            __syncthreads();
             if ((t & 31) == 0) red[t >> 5] = w;
             __syncthreads();
             w = 0.0;
@@ -350,10 +357,10 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
             }
             if (TPE > 32) {
                 __syncthreads();
-                if ((t & 31) == 0) { red[t >> 5] = ward2; red[4 + (t >> 5)] = amp2; }
+                if ((t & 31) == 0) { red[t >> 5] = ward2; red[8 + (t >> 5)] = amp2; }
                 __syncthreads();
                 ward2 = 0.0; amp2 = 0.0;
-                for (int i = 0; i < TPE / 32; i++) { ward2 += red[i]; amp2 += red[4 + i]; }
+                for (int i = 0; i < TPE / 32; i++) { ward2 += red[i]; amp2 += red[8 + i]; }
             }
             if (t == 0 && active) {
                 const double En = p.mom[(size_t)(M * 4) * N + e];
@@ -382,7 +389,7 @@ __global__ void __launch_bounds__(128, 4) cobg_shared_kernel(const CobgParams p)
 // ---------------------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------------------
-bool cobg_shared_supported(int n) { return n >= 4 && n <= 7; }
+bool cobg_shared_supported(int n) { return n >= 4 && n <= 8; }
 
 int cobg_table_create(int n, CobgTable** out) {
     *out = nullptr;
@@ -489,8 +496,9 @@ size_t cobg_shared_current_bytes(const CobgTable* t) { return t ? (size_t)t->nsl
 
 template <int NG, int TPE, bool LC>
 static cudaError_t launch_cobg(cudaStream_t s, const CobgParams& p) {
-    constexpr int EPB = 128 / TPE, NSUB = 1 << (NG - 1);
-    const size_t smem = (size_t)EPB * (p.nslots * 2 * kSlotStride + NSUB * 4 + 8 + p.np * 2 + 8) * sizeof(double);
+    constexpr int BLOCK = TPE > 128 ? TPE : 128;
+    constexpr int EPB = BLOCK / TPE, NSUB = 1 << (NG - 1);
+    const size_t smem = (size_t)EPB * (p.nslots * 2 * kSlotStride + NSUB * 4 + 8 + p.np * 2 + 16) * sizeof(double);
     static int configured_device = -1;   // the attribute is per device
     int device = 0;
     cudaGetDevice(&device);
@@ -500,7 +508,7 @@ static cudaError_t launch_cobg(cudaStream_t s, const CobgParams& p) {
         configured_device = device;
     }
     const unsigned blocks = p.helsum ? (unsigned)p.N : (unsigned)((p.N + EPB - 1) / EPB);
-    cobg_shared_kernel<NG, TPE, LC><<<blocks, 128, smem, s>>>(p);
+    cobg_shared_kernel<NG, TPE, LC><<<blocks, BLOCK, smem, s>>>(p);
     return cudaGetLastError();
 }
 
@@ -526,6 +534,7 @@ cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, 
         case 5: return lc ? launch_cobg<5, 8, true>(s, p) : launch_cobg<5, 8, false>(s, p);
         case 6: return lc ? launch_cobg<6, 32, true>(s, p) : launch_cobg<6, 32, false>(s, p);
         case 7: return lc ? launch_cobg<7, 128, true>(s, p) : launch_cobg<7, 128, false>(s, p);
+        case 8: return lc ? launch_cobg<8, 256, true>(s, p) : launch_cobg<8, 256, false>(s, p);
         default: return cudaErrorNotSupported;
     }
 }

@@ -109,14 +109,14 @@ def test_cobg_given_helicity_full_colour(bg, oracle, wl, n, N):
 
 
 def test_cobg_full_colour_n8_generic_kernel(bg, oracle, wl):
-    """n = 8 (720 orderings, 720 x 720 colour matrix) runs on the thread-per-event kernel in FP64.  Truth: the
+    """n = 8 (720 orderings, 720 x 720 colour matrix) on the thread-per-event kernel (BG_OPT_KERNEL = 1) in FP64.  Truth: the
     oracle's 720 colour-ordered amplitudes in long double contracted with Eq. 17's matrix; the oracle's own
     Gell-Mann construction of that matrix is out of reach at n = 8 (8^8-component vectors), so the matrix is the
     product's here - equal to the oracle's for n <= 7 (test_abi, test_device_colour_matrix_equals_oracle) and
     checked structurally at n = 8 in tests/test_abi.py."""
     import itertools
     ev = wl.config_events(4, N=6, n=8)
-    got, name = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR)
+    got, name = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR, kernel=1)
     assert name == "cobg_generic_kernel"
     C = bg.bg_build_colour_matrix(8).astype(np.longdouble)
     perms = list(itertools.permutations(range(1, 7)))
@@ -305,7 +305,7 @@ def test_prepass_variants_share_a_context(bg, wl):
         bg.bg_destroy(ctx)
 
 
-@pytest.mark.parametrize("n,N", [(4, 40), (5, 33), (6, 12), (7, 5)])
+@pytest.mark.parametrize("n,N", [(4, 40), (5, 33), (6, 12), (7, 5), (8, 2)])
 def test_leading_colour_mode(bg, oracle, wl, n, N):
     """Eq. 33: N^(n-2)(N^2-1) sum over all (n-1)! orderings of |A(1,sigma)|^2, against the oracle's
     colour-ordered amplitudes ordering by ordering; for n = 4, 5 it also equals the full-colour sum (pinned)."""
@@ -327,6 +327,17 @@ def test_leading_colour_mode(bg, oracle, wl, n, N):
         summed, _ = gpu_eval(ev, bg.BG_COBG_HELSUM_LC)
         fullsum, _ = gpu_eval(ev, bg.BG_COBG_HELSUM_FULLCOLOR)
         assert rel_err(summed, fullsum).max() <= 1e-11
+    if n == 6:
+        # helicity-summed leading colour: 64 assignments x 120 orderings per event, against the oracle ordering by ordering
+        sub = ev.head(2)
+        summed, _ = gpu_eval(sub, bg.BG_COBG_HELSUM_LC)
+        tot = np.zeros(sub.N)
+        for e in range(sub.N):
+            for h in itertools.product((-1, 1), repeat=n):
+                hh = np.array(h, dtype=np.int8)
+                for sig in itertools.permutations(range(1, n)):
+                    tot[e] += abs(oracle.cobg_amp(sub.mom[e], hh, np.array((0,) + sig, dtype=np.int32), prec="long double")) ** 2
+        assert rel_err(summed, tot * 3 ** (n - 2) * 8).max() <= 1e-11
 
 
 @pytest.mark.parametrize("n,N", [(4, 500), (6, 20000), (8, 1500), (9, 515), (10, 131), (12, 19)])
@@ -563,3 +574,28 @@ def test_colour_form_probe_variants_agree(bg, n, E):
     xr, xi = x[:, 0].astype(np.longdouble), x[:, 1].astype(np.longdouble)
     ref = (np.einsum("ei,ij,ej->e", xr, C, xr) + np.einsum("ei,ij,ej->e", xi, C, xi)).astype(np.float64)
     assert rel_err(w, ref).max() < 1e-12
+
+
+def test_cobg_full_colour_n8_shared_kernel(bg, oracle, wl):
+    """n = 8 on the shared-sub-current kernel (720 orderings in rounds of 256 threads, 1753 shared sequence currents
+    in 140 KB of shared memory), default precision (Ward flag + double-double re-evaluation) and FP64 alone, against
+    the oracle's 720 amplitudes in long double contracted with Eq. 17's matrix (see test_cobg_full_colour_n8_generic_kernel
+    for where that matrix comes from); the thread-per-event kernel (BG_OPT_KERNEL = 1) gives the same numbers."""
+    import itertools
+    ev = wl.config_events(4, N=9, n=8)
+    got, name = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR)
+    assert name == "cobg_shared_kernel"
+    fp64, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR, precision=0)
+    flagged_all, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR, flag_threshold=1)     # every event re-evaluated
+    generic, gname = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR, kernel=1, precision=0)
+    assert gname == "cobg_generic_kernel"
+    C = bg.bg_build_colour_matrix(8).astype(np.longdouble)
+    perms = list(itertools.permutations(range(1, 7)))
+    truth = np.zeros(ev.N)
+    for e in range(ev.N):
+        a = np.array([oracle.cobg_amp(ev.mom[e], ev.hel[e], np.array((0,) + s + (7,), dtype=np.int32), prec="long double")
+                      for s in perms])
+        ar, ai = a.real.astype(np.longdouble), a.imag.astype(np.longdouble)
+        truth[e] = float(ar @ C @ ar + ai @ C @ ai)
+    for x in (got, fp64, flagged_all, generic):
+        assert rel_err(x, truth).max() <= 1e-11
