@@ -265,6 +265,7 @@ __device__ C cobg_dd_amplitude(int n, int nperm, int s, int hc, long long N, lon
                     }
                 }
             }
+            for (int nu = 0; nu < 4; nu++) cxd_renorm(s4[nu]);      // (multiply-adds leave their accumulator unnormalised)
             dd f3 = inv_sqrt2, f4 = half;
             if (len < m) {
                 const dd ip2 = mkdd(1.0) / mdot(P[tri_dd(i, j)], P[tri_dd(i, j)]);
@@ -314,9 +315,12 @@ cobg_dd_flagged_kernel(int n, int nperm, long long N, const uint32_t* __restrict
                 dd_fma(tr, c, mkdd(sh_amp[2 * s2].x, sh_amp[2 * s2].y));
                 dd_fma(ti, c, mkdd(sh_amp[2 * s2 + 1].x, sh_amp[2 * s2 + 1].y));
             }
+            dd_renorm(tr);
+            dd_renorm(ti);
             dd_fma(mine, mkdd(sh_amp[2 * s].x, sh_amp[2 * s].y), tr);
             dd_fma(mine, mkdd(sh_amp[2 * s + 1].x, sh_amp[2 * s + 1].y), ti);
         }
+        dd_renorm(mine);
         __syncthreads();
         sh_amp[threadIdx.x] = make_double2(mine.hi, mine.lo);
         __syncthreads();
