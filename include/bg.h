@@ -36,7 +36,8 @@ enum {
     BG_EINVAL = -1,       /* bad argument (n out of range, NULL pointer the mode needs, N < 0, ...) */
     BG_ENOMEM = -2,       /* host or device allocation failed */
     BG_ECUDA = -3,        /* CUDA runtime error (no device, launch failure, ...) */
-    BG_EUNSUPPORTED = -4  /* mode / n combination not implemented */
+    BG_EUNSUPPORTED = -4, /* mode / n combination not implemented */
+    BG_ELIMIT = -5        /* size beyond the fixed maximum of the no-allocation entry point (bg_eval_static) */
 };
 
 /* mode = recursion | helicity treatment | colour treatment */
@@ -233,6 +234,34 @@ int bg_fp64_peak_probe(int iterations, double* tflops);
  */
 int bg_colour_form_probe(int n, long long E, int iterations, double* ms_dfma, double* ms_dmma, double* max_rel_diff,
                          double* x_host, double* w_host);
+
+/*
+ * The no-allocation entry point.  Some callers cannot call cudaMalloc - code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it - and bg_init / bg_reserve / bg_eval allocate tables and scratch.  bg_eval_static
+ * needs no context and calls no cudaMalloc, cudaFree or allocating library routine: it evaluates
+ *     out[e] = |A_{i1 j1 .. in jn}|^2   (colour-dressed recursion Eq. 29-32 closed with gluon n, Eq. 22;
+ *                                         PAPER.md:L187-213)
+ * for given helicities and colour-flow indices with the thread-per-event FP64 kernel (the kernel a BG_CDBG_GIVEN context
+ * runs under BG_OPT_KERNEL = 1; no conditioning flag, no double-double re-evaluation: ill-conditioned events carry
+ * their FP64 round-off), whose per-event scratch - 2^(n-1) x 513 bytes of sub-currents, subset momenta and colour
+ * types - lives in ONE file-scope device array of BG_STATIC_SCRATCH_BYTES that every GPU which loads libbg.so holds
+ * until the process exits.
+ *   Limit: N <= bg_static_max_events(n) = BG_STATIC_SCRATCH_BYTES / (2^(n-1) x 513): 4088 events at n = 5, 2044 at
+ *   n = 6, 511 at n = 8, 31 at n = 12.  Beyond it the call returns BG_ELIMIT and launches nothing; split the batch.
+ *   DEVICE pointers in the layouts of bg_eval (mom[n][4][N], hel[n][N], col[n][2][N] in {1,2,3}, out[N]), all owned by
+ *   the caller; asynchronous on `cuda_stream`, whose device must be current.  N = 0 is a no-op; n outside 4..12, N < 0
+ *   or a NULL pointer with N > 0: BG_EINVAL.
+ *   The array is shared by every call in the process and keeps the last call's contents (nothing in it has to start at
+ *   zero: the kernel writes each entry of an event before reading it).  Calls on one stream are ordered by the stream;
+ *   calls that overlap on the GPU - different streams, or a graph replayed concurrently with itself - RACE.
+ *   bg_static_setup resolves the array's device address for the current device (cudaGetSymbolAddress; once per device,
+ *   thread-safe); bg_eval_static does so itself on first use, but call bg_static_setup before starting a stream capture.
+ */
+#define BG_STATIC_SCRATCH_BYTES (32u << 20)
+int bg_static_setup(void);
+long long bg_static_max_events(int n);     /* host-only; BG_EINVAL for n outside 4..12 */
+int bg_eval_static(void* cuda_stream, int n, long long N, const double* mom, const signed char* hel,
+                   const signed char* col, double* out);
 
 #ifdef __cplusplus
 }

@@ -13,7 +13,8 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libbg.so")
 
-BG_OK, BG_EINVAL, BG_ENOMEM, BG_ECUDA, BG_EUNSUPPORTED = 0, -1, -2, -3, -4
+BG_OK, BG_EINVAL, BG_ENOMEM, BG_ECUDA, BG_EUNSUPPORTED, BG_ELIMIT = 0, -1, -2, -3, -4, -5
+BG_STATIC_SCRATCH_BYTES = 32 << 20
 BG_REC_COBG, BG_REC_CDBG = 0x001, 0x002
 BG_HEL_SUM, BG_HEL_GIVEN = 0x010, 0x020
 BG_COL_FULL, BG_COL_GIVEN, BG_COL_LC = 0x100, 0x200, 0x400
@@ -31,7 +32,8 @@ BG_OPT_FLAG_THRESHOLD, BG_OPT_FLAG_CANCELLATION = 7, 8
 
 EXPORTS = ("bg_init", "bg_eval", "bg_eval_continuous", "bg_generate", "bg_colour_rule", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",
            "bg_set_option", "bg_colour_matrix", "bg_build_colour_matrix", "bg_last_launch_count",
-           "bg_last_kernel_name", "bg_last_kernel_ms", "bg_last_refined", "bg_class_program_stats", "bg_comc_program_stats", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe", "bg_colour_form_probe")
+           "bg_last_kernel_name", "bg_last_kernel_ms", "bg_last_refined", "bg_class_program_stats", "bg_comc_program_stats", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe", "bg_colour_form_probe",
+           "bg_static_setup", "bg_static_max_events", "bg_eval_static")
 
 
 class BgError(RuntimeError):
@@ -88,6 +90,12 @@ def load():
         dp = ctypes.POINTER(ctypes.c_double)
         lib.bg_colour_form_probe.argtypes = [i, ll, i, dp, dp, dp, vp, vp]
         lib.bg_colour_form_probe.restype = i
+        lib.bg_static_setup.argtypes = []
+        lib.bg_static_setup.restype = i
+        lib.bg_static_max_events.argtypes = [i]
+        lib.bg_static_max_events.restype = ll
+        lib.bg_eval_static.argtypes = [vp, i, ll, vp, vp, vp, vp]
+        lib.bg_eval_static.restype = i
         for name in ("bg_init", "bg_eval", "bg_eval_host", "bg_reserve", "bg_set_option", "bg_colour_matrix",
                      "bg_build_colour_matrix", "bg_last_launch_count", "bg_destroy", "bg_fp64_peak_probe"):
             getattr(lib, name).restype = i
@@ -255,3 +263,22 @@ def bg_colour_form_probe(n: int, E: int, iterations: int = 5, return_data: bool 
     _check(load().bg_colour_form_probe(n, E, iterations, ctypes.byref(a), ctypes.byref(b), ctypes.byref(d), _ptr(x), _ptr(w)),
            "bg_colour_form_probe")
     return (a.value, b.value, d.value) + ((x, w) if return_data else ())
+
+
+def bg_static_setup() -> None:
+    """Resolve the device address of the static scratch array for the current device (once per device)."""
+    _check(load().bg_static_setup(), "bg_static_setup")
+
+
+def bg_static_max_events(n: int) -> int:
+    rc = int(load().bg_static_max_events(n))
+    if rc < 0:
+        raise BgError(rc, "bg_static_max_events")
+    return rc
+
+
+def bg_eval_static(stream, n: int, N: int, mom, hel, col, out) -> None:
+    """The no-allocation entry point: CDBG, given helicities and colours, FP64 thread-per-event kernel with its scratch
+    in a fixed device array; N <= bg_static_max_events(n), else BgError(BG_ELIMIT).  Device pointers / CUDA tensors."""
+    s = ctypes.c_void_p(int(stream)) if stream else None
+    _check(load().bg_eval_static(s, n, N, _ptr(mom), _ptr(hel), _ptr(col), _ptr(out)), "bg_eval_static")

@@ -164,6 +164,7 @@ const char* bg_strerror(int code) {
         case BG_ENOMEM: return "out of memory";
         case BG_ECUDA: return "CUDA error (no device, or a runtime/launch failure)";
         case BG_EUNSUPPORTED: return "mode / n combination not supported";
+        case BG_ELIMIT: return "batch larger than the fixed scratch of the no-allocation entry point (bg_static_max_events)";
         default: return "unknown error code";
     }
 }
