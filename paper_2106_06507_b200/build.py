@@ -15,6 +15,7 @@ LIB = os.path.join(_HERE, "libbg.so")
 SOURCES = ["bg_api.cu", "bg_generic.cu", "bg_cobg_generic.cu", "bg_cdbg_prog.cu", "bg_cdbg_prog_dd.cu", "bg_program.cpp",
            "bg_cobg_shared.cu", "bg_cdbg_dd.cu", "bg_generate.cu", "bg_colour_probe.cu", "bg_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
+NVCC_FLAGS += os.environ.get("BG_NVCC_EXTRA", "").split()      # e.g. extra -D switches of an experiment
 if os.environ.get("BG_BOUNDS_CHECK"):      # debug build: every interpreter state access is range-checked (traps)
     NVCC_FLAGS.insert(0, "-DBG_BOUNDS_CHECK")
 

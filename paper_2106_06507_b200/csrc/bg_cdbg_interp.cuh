@@ -63,6 +63,11 @@ struct ProgTable {
     cudaEvent_t fork_ev, join_ev[kTiers - 1];
     bool has_streams;
     uint32_t* d_small;        // [2 (num_classes + 1) + 1] zeroed histogram | cursors | ticket of the fused-scan prepass
+    // FP64 launches of warp-shared lane counts (G <= 8): tiers whose state block exceeds cap_cx keep only the first cap_cx
+    // elements per event in shared memory - as many as let the register-limited number of blocks fit an SM - and the
+    // rest (the highest levels) in the block's L2-resident slab (round 2: n = 6 -6 %, n = 7 -20 %)
+    int cap_cx;               // 0: every tier keeps its whole state in shared memory
+    int cap_blocks;           // resident blocks per SM of the capped launches (each owns one global slab)
     // double-double re-evaluation of flagged events (BG_OPT_PRECISION = 2): state elements are 32 bytes, so less of
     // the state fits in shared memory
     int dd_mode;              // 1: available (state beyond dd_cap_cx elements per event spills to the L2 slab); -1: not (dense tables)
@@ -77,6 +82,8 @@ struct LaunchShape {
     bool conc = false;        // small batches: tiers side by side on the table's side streams
     int regs = 168;           // registers per thread of the instantiation (resident-block estimate)
     int cap_cx = 0;           // > 0: at most this many state elements per event in shared memory (SPILL kernels)
+    bool hybrid = false;      // SPILL kernel only for the tiers whose state exceeds cap_cx, the others keep all of it in
+                              // shared memory (launch_interp<G, false, S> with both kernels instantiated)
     int spill_blocks = 0;     // SPILL: resident blocks per SM (each owns one global slab)
     long long max_blocks = 0; // > 0: at most this many blocks per launch
 };
@@ -713,16 +720,14 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     }
 }
 
-template <int G, bool SPILL, class S = cx>
-static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched,
-                                 const LaunchShape& shape) {
-    bool conc = shape.conc;
-    constexpr int EPW = G >= 32 ? 1 : 32 / G, BLOCK = G > 32 ? G : 32;
-    constexpr size_t ELEM = sizeof(typename StateElem<S>::T);
+// set the dynamic shared-memory limit of one instantiation (once per device); returns its static shared memory
+template <int G, bool SPILL, class S>
+static cudaError_t configure_interp(size_t* static_smem_out) {
+    constexpr int BLOCK = G > 32 ? G : 32;
     static int configured_device = -1;   // the attribute is per device
+    static size_t static_smem = 0;       // the kernel's static shared memory (reduction scratch)
     int device = 0;
     cudaGetDevice(&device);
-    static size_t static_smem = 0;       // the kernel's static shared memory (reduction scratch)
     if (configured_device != device) {
         cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL, S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)(kMaxSlabBytes + (size_t)kRing * BLOCK * 16));
@@ -732,40 +737,78 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         static_smem = fa.sharedSizeBytes;
         configured_device = device;
     }
+    *static_smem_out = static_smem;
+    return cudaSuccess;
+}
+
+// SPILL: every tier runs the spill kernel.  HYBRID (with SPILL = false): shape.hybrid picks it per tier.
+template <int G, bool SPILL, class S = cx, bool HYBRID = false>
+static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched,
+                                 const LaunchShape& shape) {
+    static_assert(!(SPILL && HYBRID), "HYBRID chooses between the two kernels itself");
+    bool conc = shape.conc;
+    constexpr int EPW = G >= 32 ? 1 : 32 / G, BLOCK = G > 32 ? G : 32;
+    constexpr size_t ELEM = sizeof(typename StateElem<S>::T);
+    constexpr bool kHasDirect = !SPILL, kHasSpill = SPILL || HYBRID;
+    size_t static_direct = 0, static_spill = 0;
+    cudaError_t cerr;
+    if constexpr (kHasDirect)
+        if ((cerr = configure_interp<G, false, S>(&static_direct)) != cudaSuccess) return cerr;
+    if constexpr (kHasSpill)
+        if ((cerr = configure_interp<G, true, S>(&static_spill)) != cudaSuccess) return cerr;
+    bool hybrid = HYBRID && shape.hybrid && shape.cap_cx > 0;
     const long long max_tasks = (p.N + EPW - 1) / EPW + kTiers;
+    if (hybrid) {
+        // small batches (fewer than two tasks per block the uncapped launches hold): occupancy is not what limits
+        // them, and the capped kernel's L2 round trips cost more than they hide (n = 6: 2^16 events +7 %, 2^17 equal,
+        // 2^18 and more -2 ... -6 %; n = 7: 2^14 +14 %, 2^16 -8 %, 2^18 -20 %)
+        long long direct = 0;
+        for (int k = 0; k < kTiers; k++) {
+            if (t->tiers.first_key[k] == t->tiers.first_key[k + 1] && k + 1 < kTiers) continue;
+            const size_t sm = ((size_t)EPW * t->tiers.slab_cx[k] * ELEM + 15) / 16 * 16 + (G >= 8 ? (size_t)kRing * BLOCK * 16 : 0);
+            direct += (long long)sm_count * (long long)std::max<size_t>(1, std::min<size_t>(65536 / (shape.regs * BLOCK), (228 * 1024) / (sm + 1024 + static_direct)));
+        }
+        if (max_tasks <= 2 * direct) hybrid = false;
+    }
     unsigned blocks[kTiers];
     size_t smem[kTiers];
     int slab[kTiers];
+    bool sp[kTiers];
     long long resident = 0;
-    int nlaunch = 0;
+    int nlaunch = 0, nspill = 0;
     for (int k = 0; k < kTiers; k++) {
         blocks[k] = 0;
+        sp[k] = false;
         // no class in this tier (the last tier always runs: events with colour codes out of range are sorted behind
         // every class and get their 0.0 there)
         if (t->tiers.first_key[k] == t->tiers.first_key[k + 1] && (k + 1 < kTiers || t->dense)) continue;
         const size_t ring_bytes = G >= 8 ? (size_t)kRing * BLOCK * 16 : 0;
-        slab[k] = shape.cap_cx > 0 ? std::min(t->tiers.slab_cx[k], shape.cap_cx) : t->tiers.slab_cx[k];
+        sp[k] = SPILL || (hybrid && t->tiers.slab_cx[k] > shape.cap_cx);
+        slab[k] = (shape.cap_cx > 0 && (SPILL || sp[k])) ? std::min(t->tiers.slab_cx[k], shape.cap_cx) : t->tiers.slab_cx[k];
         smem[k] = ((size_t)EPW * slab[k] * ELEM + 15) / 16 * 16 + ring_bytes;
         if (smem[k] > kMaxSlabBytes + ring_bytes) return cudaErrorInvalidValue;
         // resident blocks per SM: 228 KB of shared memory against dynamic + static + 1 KB reserved per block (a grid
         // sized for one block more than fits runs a second, nearly empty wave), and 65536 / (regs x BLOCK) registers
+        const size_t static_smem = sp[k] ? static_spill : static_direct;
         int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (shape.regs * BLOCK), (228 * 1024) / (smem[k] + 1024 + static_smem)));
-        if (SPILL) per_sm = std::min(per_sm, shape.spill_blocks);   // one global slab per resident block
+        if (sp[k]) per_sm = std::min(per_sm, shape.spill_blocks);   // one global slab per resident block
         blocks[k] = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
-        if (shape.max_blocks > 0) blocks[k] = (unsigned)std::min<long long>(blocks[k], shape.max_blocks);
+        if (sp[k] && shape.max_blocks > 0) blocks[k] = (unsigned)std::min<long long>(blocks[k], shape.max_blocks);
         resident += (long long)sm_count * per_sm;
         nlaunch++;
+        nspill += sp[k] ? 1 : 0;
     }
     // Small batches: when the tiers together hold fewer than two tasks per resident block, each launch is mostly
     // ramp-up and tail, so the tiers run side by side (fork / join around the caller's stream).  Measured at
     // n = 6: 2^16 events +22 %, 2^18 neutral, 2^20 -5 %; n >= 7: slower at every size.
-    // (spill slabs are indexed by block: one launch at a time)
-    // (spill slabs are indexed by block: concurrent launches each get their own share of the slabs)
-    const bool conc_spill = conc && SPILL && shape.max_blocks > 0 && t->has_streams && nlaunch > 1;
-    const long long share = conc_spill ? std::max<long long>(1, shape.max_blocks / nlaunch) : 0;
-    if (conc_spill)
-        for (int k = 0; k < kTiers; k++) blocks[k] = (unsigned)std::min<long long>(blocks[k], share);
-    conc = conc_spill || (conc && G <= 4 && !SPILL && t->has_streams && nlaunch > 1 && max_tasks <= 2 * resident);
+    // (spill slabs are indexed by block: concurrent spill launches each get their own share of the slabs)
+    if (SPILL) conc = conc && shape.max_blocks > 0 && t->has_streams && nlaunch > 1;
+    else conc = conc && G <= 4 && t->has_streams && nlaunch > 1 && max_tasks <= 2 * resident && (nspill == 0 || shape.max_blocks > 0);
+    const bool share_slabs = conc && nspill > 1;
+    const long long share = share_slabs ? std::max<long long>(1, shape.max_blocks / nspill) : 0;
+    if (share_slabs)
+        for (int k = 0; k < kTiers; k++)
+            if (sp[k]) blocks[k] = (unsigned)std::min<long long>(blocks[k], share);
     if (conc && cudaEventRecord(t->fork_ev, s) != cudaSuccess) return cudaGetLastError();
     double2* const spill0 = p.spill;
     int li = 0;
@@ -780,9 +823,13 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
             ls = t->aux[side];
             cudaStreamWaitEvent(ls, t->fork_ev, 0);
         }
-        if (conc_spill) p.spill = reinterpret_cast<double2*>(reinterpret_cast<char*>(spill0) + (size_t)li * share * p.spill_cx * EPW * ELEM);
-        li++;
-        cdbg_prog_kernel<G, SPILL, S><<<blocks[k], BLOCK, smem[k], ls>>>(p);
+        if (sp[k]) {
+            if (share_slabs) p.spill = reinterpret_cast<double2*>(reinterpret_cast<char*>(spill0) + (size_t)li * share * p.spill_cx * EPW * ELEM);
+            li++;
+            if constexpr (kHasSpill) cdbg_prog_kernel<G, true, S><<<blocks[k], BLOCK, smem[k], ls>>>(p);
+        } else {
+            if constexpr (kHasDirect) cdbg_prog_kernel<G, false, S><<<blocks[k], BLOCK, smem[k], ls>>>(p);
+        }
         if (conc && !first) cudaEventRecord(t->join_ev[side++], ls);
         first = false;
         ++*launched;

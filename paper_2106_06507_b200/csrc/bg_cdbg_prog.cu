@@ -546,6 +546,19 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
     }
+    {   // capped FP64 launches (warp-shared lane counts 4 and 8, the defaults of n = 5, 6 and 7): the 166 registers per
+        // thread allow reg_blocks one-warp blocks per SM, the heavy tiers' slabs (epw events each) far fewer, and the
+        // kernel's FP64 rate follows the resident warps.  Tiers above the cap keep cap_cx elements per event in shared
+        // memory - what lets reg_blocks blocks fit - and the highest levels in an L2 slab.  (Block-per-event lane counts,
+        // n >= 8: measured 13 - 24 % slower, their top levels are the most numerous and the most read.)
+        const int epw = G >= 32 ? 1 : 32 / G, block = G > 32 ? G : 32;
+        const size_t ring_bytes = G >= 8 ? (size_t)kRing * block * 16 : 0;
+        const int reg_blocks = std::max(1, 65536 / (168 * block));
+        const int cap = (int)(((size_t)(228 * 1024) / reg_blocks - 1024 - 128 - ring_bytes) / 16 / (size_t)epw);
+        t->cap_cx = 0;
+        t->cap_blocks = reg_blocks;
+        if ((G == 4 || G == 8) && !spill && cap >= 64 && tiers.slab_cx[0] > cap) t->cap_cx = cap;
+    }
     {   // double-double re-evaluation: 32-byte state elements and 255 registers per thread.  The registers allow
         // 65536 / (255 x block) resident blocks per SM; the shared-memory part of the state is capped so that shared
         // memory allows as many (the kernel is latency-bound: resident warps decide its speed), the rest - the highest
@@ -720,7 +733,9 @@ static size_t prog_spill_bytes(const ProgTable* t) {
 size_t prog_scratch_bytes(const ProgTable* t, long long N) {
     const size_t epw = t->G >= 32 ? 1 : 32 / t->G;
     const size_t dd_spill = t->dd_mode == 1 ? (size_t)t->dd_max_blocks * epw * t->max_state_cx * 32 : 0;
-    return prog_spill_offset(t, N) + prog_spill_bytes(t) + dd_spill;
+    // the slabs of the capped FP64 launches share the region of the re-evaluation's (which runs after them)
+    const size_t cap_spill = t->cap_cx > 0 ? (size_t)t->sm_count * t->cap_blocks * epw * t->max_state_cx * 16 : 0;
+    return prog_spill_offset(t, N) + prog_spill_bytes(t) + std::max(dd_spill, cap_spill);
 }
 
 // flagged events of the most recent launch with a conditioning threshold (synchronises the stream's work first)
@@ -752,11 +767,17 @@ static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_co
                                 : launch_interp<256, false, double>(s, t, sm_count, p, launches, shape);
         }
     }
+    if (t->cap_cx > 0 && p.spill) {     // heavy tiers: capped shared-memory state + L2 slab (see prog_table_create)
+        shape.hybrid = true;
+        shape.cap_cx = t->cap_cx;
+        shape.spill_blocks = t->cap_blocks;
+        shape.max_blocks = (long long)t->sm_count * t->cap_blocks;
+    }
     switch (t->G) {
         case 1: err = launch_interp<1, false>(s, t, sm_count, p, launches, shape); break;
         case 2: err = launch_interp<2, false>(s, t, sm_count, p, launches, shape); break;
-        case 4: err = launch_interp<4, false>(s, t, sm_count, p, launches, shape); break;
-        case 8: err = launch_interp<8, false>(s, t, sm_count, p, launches, shape); break;
+        case 4: err = launch_interp<4, false, cx, true>(s, t, sm_count, p, launches, shape); break;
+        case 8: err = launch_interp<8, false, cx, true>(s, t, sm_count, p, launches, shape); break;
         case 16: err = launch_interp<16, false>(s, t, sm_count, p, launches, shape); break;
         case 32: err = launch_interp<32, false>(s, t, sm_count, p, launches, shape); break;
         case 64: err = launch_interp<64, false>(s, t, sm_count, p, launches, shape); break;
@@ -849,6 +870,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.bounds = bounds;
     p.zero = 0;
     p.spill = t->spill ? (double2*)((char*)scratch + prog_spill_offset(t, N)) : nullptr;
+    if (t->cap_cx > 0) p.spill = (double2*)((char*)scratch + prog_spill_offset(t, N) + prog_spill_bytes(t));
     p.spill_cx = t->max_state_cx;
     p.tier = 0;
     p.slab_cx = t->max_state_cx;
