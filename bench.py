@@ -120,15 +120,16 @@ def measure_config(bg, wl, oracle_mod, dev, config: int, n: int, steps: int, pea
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / steps
             bg.bg_set_option(ctx, bg.BG_OPT_TIMING, 1)
-            kms, rms, fl = [], [], 0
+            kms, rms, fl, tw = [], [], 0, 0
             for _ in range(min(steps, 5)):
                 bg.bg_eval(ctx, sh, N, d_mom, d_hel, d_col, d_out)
                 kms.append(bg.bg_last_kernel_ms(ctx))
                 fl, r = bg.bg_last_refined(ctx)
+                tw = bg.bg_last_twin(ctx)
                 rms.append(r)
             bg.bg_set_option(ctx, bg.BG_OPT_TIMING, 0)
-            return ms, float(np.mean(kms)), float(np.mean(rms)), fl
-        ms, kms, rms, fl = timed(2)
+            return ms, float(np.mean(kms)), float(np.mean(rms)), fl, tw
+        ms, kms, rms, fl, tw = timed(2)
         got = d_out.cpu().numpy()
         res.update({"events_per_s": N / (ms * 1e-3), "ms_per_step": ms, "kernel_ms": kms,
                     "gpu_launches_per_step": bg.bg_last_launch_count(ctx), "kernel": bg.bg_last_kernel_name(ctx),
@@ -145,8 +146,8 @@ def measure_config(bg, wl, oracle_mod, dev, config: int, n: int, steps: int, pea
                                         "note": "step a7 alone on synthetic amplitudes (bg_colour_form_probe); the production "
                                                 "kernel keeps the fused DFMA form (DESIGN.md 5.2)"}
         if auto:
-            ms0, kms0, _, _ = timed(0)
-            res["precision_auto"] = {"flagged_frac": fl / N, "reevaluation_ms": rms,
+            ms0, kms0, _, _, _ = timed(0)
+            res["precision_auto"] = {"flagged_frac": fl / N, "second_fp64_frac": tw / N, "reevaluation_ms": rms,
                                      "overhead_pct": 100.0 * (ms / ms0 - 1.0),
                                      "fp64_only_events_per_s": N / (ms0 * 1e-3), "fp64_only_ms_per_step": ms0}
             bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 2)
@@ -432,11 +433,12 @@ def run_b200(args):
     launches_per_step = bg.bg_last_launch_count(ctx)
     kernel_name = bg.bg_last_kernel_name(ctx)
     kernel_ms = float(np.mean(kms))      # per step: all launches of the recursion kernels (FP64 + re-evaluation)
-    flagged, refine_ms = (0, 0.0)
+    flagged, refine_ms, second = (0, 0.0, 0)
     if not args.continuous:
         bg.bg_set_option(ctx, bg.BG_OPT_TIMING, 1)
         step()
         flagged, refine_ms = bg.bg_last_refined(ctx)
+        second = bg.bg_last_twin(ctx)
         bg.bg_set_option(ctx, bg.BG_OPT_TIMING, 0)
     auto_default = args.precision is None and flagged > 0
     total_ms = max_over_ranks(total_ms, world, dev)
@@ -570,7 +572,7 @@ def run_b200(args):
             torch.cuda.synchronize()
             ms0 = f0.elapsed_time(f1) / args.steps
             bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 2)
-            line["precision_auto"] = {"flagged_frac": flagged / N, "reevaluation_ms": refine_ms,
+            line["precision_auto"] = {"flagged_frac": flagged / N, "second_fp64_frac": second / N, "reevaluation_ms": refine_ms,
                                       "overhead_pct": 100.0 * (total_ms / args.steps / ms0 - 1.0),
                                       "fp64_only_events_per_s": N / (ms0 * 1e-3), "fp64_only_ms_per_step": ms0}
         if default_line and not args.no_configs:

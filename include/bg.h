@@ -76,18 +76,31 @@ enum {
                                 BG_OPT_PRECISION falls back from 2 to 0 (setting it to 2 then returns BG_EUNSUPPORTED). */
     BG_OPT_TIMING = 4,       /* 1: record CUDA events around the dominant kernel of every bg_eval (bg_last_kernel_ms) */
     BG_OPT_PRECISION = 6,    /* 0 = FP64 kernels only; 1 = every event in double-double arithmetic (BG_CDBG_GIVEN and the COBG
-                                full-colour modes: the precision reference on the GPU, slow); 2 (BG_CDBG_GIVEN, the default
-                                there) = FP64 kernels plus a conditioning flag per event and re-evaluation of the flagged
-                                events by a double-double instantiation of the same kernel: the colour-flow amplitude of
-                                Eq. 19 / 28-32 has near-zeros - helicity-suppressed
-                                configurations, cancellations between orderings - where FP64 round-off exceeds 1e-11 of
-                                the result.  An event is flagged when its Ward residual |p_n . J| / (E_n |eps_n . J|)
-                                (J = the current of gluons 1..n-1 of Eq. 22; zero without round-off) exceeds
-                                BG_OPT_FLAG_THRESHOLD, or when |A| is less than BG_OPT_FLAG_CANCELLATION times the sum of
-                                the moduli of the closure contributions that add up to it.  3, 4 = diagnostics: `out`
-                                receives the Ward residual / that cancellation ratio instead of |M|^2. */
-    BG_OPT_FLAG_THRESHOLD = 7,/* Ward-residual threshold in units of 1e-18 (0 = default: 1e-13; 3e-14 for n = 5, 2e-14 for n = 6) */
+                                full-colour modes: the precision reference on the GPU, slow); 2 (the default of BG_CDBG_GIVEN
+                                and BG_COBG_HELGIVEN_FULLCOLOR) = FP64 kernels plus a conditioning flag per event and
+                                re-evaluation of what it names: the colour-flow amplitude of Eq. 19 / 28-32
+                                 has near-zeros - helicity-suppressed configurations,
+                                cancellations between orderings - where FP64 round-off exceeds 1e-11 of the result.
+                                An event is flagged when its Ward residual |p_n . J| / (E_n |eps_n . J|) (J = the current of
+                                gluons 1..n-1 of Eq. 22; zero without round-off) exceeds BG_OPT_FLAG_THRESHOLD, or when |A|
+                                is less than BG_OPT_FLAG_CANCELLATION times the sum of the moduli of the closure
+                                contributions that add up to it.  BG_CDBG_GIVEN then runs a cascade: flagged events whose
+                                residual stays below BG_OPT_FLAG_TWIN are evaluated once more in FP64 in a rotated frame
+                                (the same number with independent round-off); those whose two results agree to
+                                BG_OPT_FLAG_TWIN keep the first one, the others - and the events the first stage did not
+                                send to the second - are evaluated by a double-double instantiation of the same kernel.
+                                3, 4 = diagnostics: `out` receives the Ward residual / the cancellation ratio instead
+                                of |M|^2. */
+    BG_OPT_FLAG_THRESHOLD = 7,/* Ward-residual threshold in units of 1e-18 (0 = default; BG_CDBG_GIVEN: 1e-13 for n = 4 and
+                                n >= 11, 1e-14 for n = 5, 6, 3e-14 for n = 7 .. 10; COBG: 1e-13, 3e-13 for n >= 7) */
     BG_OPT_FLAG_CANCELLATION = 8, /* cancellation threshold in units of 1e-6 (0 = default: 3e-3) */
+    BG_OPT_FLAG_TWIN = 9,    /* BG_CDBG_GIVEN: bound of the second stage in units of 1e-18 (0 = default: 5e-13) on |w - w'| / w
+                                of the two evaluations; the Ward residual of either may not exceed the same number for
+                                n = 6, 0.4 times it otherwise.  With that residual bound at or below BG_OPT_FLAG_THRESHOLD
+                                there is no second stage and every flagged event is evaluated in double-double */
+    BG_OPT_FRAME = 10,       /* BG_CDBG_GIVEN, program interpreter: 1 = evaluate every event in the rotated frame of the
+                                second stage (fixed rotation, axis (1,2,3), 1 rad) - |M|^2 is the same to round-off; a
+                                diagnostic of Lorentz invariance and of the FP64 error */
     BG_OPT_SMEM_LIMIT = 5    /* program interpreter, >= 128 lanes per event: bytes of shared memory one event's state may
                                 take (16 KiB .. 222 KiB, 0 = default); the rest spills to an L2-resident slab.
                                 Rebuilds the class programs. */
@@ -169,12 +182,17 @@ int bg_last_launch_count(const bg_ctx* ctx);
 int bg_last_kernel_ms(bg_ctx* ctx, double* ms);
 
 /* BG_OPT_PRECISION = 2: number of events of the most recent bg_eval that the conditioning flag sent to the
- * double-double re-evaluation and (if BG_OPT_TIMING is on and ms != NULL) the device time of that re-evaluation in
- * milliseconds, which bg_last_kernel_ms includes.  Waits for the device. */
+ * double-double re-evaluation and (if BG_OPT_TIMING is on and ms != NULL) the device time of everything after the first
+ * FP64 pass (second stage of the cascade + double-double re-evaluation) in milliseconds, which bg_last_kernel_ms
+ * includes.  Waits for the device. */
 int bg_last_refined(bg_ctx* ctx, long long* flagged, double* ms);
 
 /* Name of the kernel variant the most recent bg_eval used (static string). */
 const char* bg_last_kernel_name(const bg_ctx* ctx);
+
+/* BG_OPT_PRECISION = 2, BG_CDBG_GIVEN: how many events of the most recent bg_eval went through the second stage of the
+ * cascade (the rotated-frame FP64 evaluation); bg_last_refined counts those evaluated in double-double.  Synchronises. */
+int bg_last_twin(bg_ctx* ctx, long long* count);
 
 /*
  * Host-only introspection of the colour-class program generator behind the BG_CDBG_GIVEN interpreter (no device

@@ -28,11 +28,11 @@ BG_COMC_GIVEN = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_GIVEN
 BG_COBG_HELSUM_LC = BG_REC_COBG | BG_HEL_SUM | BG_COL_LC
 BG_COBG_HELGIVEN_LC = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_LC
 BG_OPT_KERNEL, BG_OPT_SCRATCH_LIMIT, BG_OPT_LANES, BG_OPT_TIMING, BG_OPT_SMEM_LIMIT, BG_OPT_PRECISION = 1, 2, 3, 4, 5, 6
-BG_OPT_FLAG_THRESHOLD, BG_OPT_FLAG_CANCELLATION = 7, 8
+BG_OPT_FLAG_THRESHOLD, BG_OPT_FLAG_CANCELLATION, BG_OPT_FLAG_TWIN, BG_OPT_FRAME = 7, 8, 9, 10
 
 EXPORTS = ("bg_init", "bg_eval", "bg_eval_continuous", "bg_generate", "bg_colour_rule", "bg_eval_host", "bg_reserve", "bg_scratch_bytes", "bg_current_bytes_per_event",
            "bg_set_option", "bg_colour_matrix", "bg_build_colour_matrix", "bg_last_launch_count",
-           "bg_last_kernel_name", "bg_last_kernel_ms", "bg_last_refined", "bg_class_program_stats", "bg_comc_program_stats", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe", "bg_colour_form_probe",
+           "bg_last_kernel_name", "bg_last_kernel_ms", "bg_last_refined", "bg_last_twin", "bg_class_program_stats", "bg_comc_program_stats", "bg_destroy", "bg_strerror", "bg_fp64_peak_probe", "bg_colour_form_probe",
            "bg_static_setup", "bg_static_max_events", "bg_eval_static")
 
 
@@ -79,6 +79,8 @@ def load():
         lib.bg_last_kernel_ms.restype = i
         lib.bg_last_refined.argtypes = [vp, ctypes.POINTER(ll), ctypes.POINTER(ctypes.c_double)]
         lib.bg_last_refined.restype = i
+        lib.bg_last_twin.argtypes = [vp, ctypes.POINTER(ll)]
+        lib.bg_last_twin.restype = i
         lib.bg_class_program_stats.argtypes = [i, i, vp, vp]
         lib.bg_class_program_stats.restype = i
         lib.bg_comc_program_stats.argtypes = [i, i, vp, vp]
@@ -220,6 +222,13 @@ def bg_last_refined(ctx):
     k, ms = ctypes.c_longlong(), ctypes.c_double()
     _check(load().bg_last_refined(ctx, ctypes.byref(k), ctypes.byref(ms)), "bg_last_refined")
     return int(k.value), ms.value
+
+
+def bg_last_twin(ctx) -> int:
+    """Events of the most recent bg_eval that went through the second (rotated-frame FP64) stage of the cascade."""
+    k = ctypes.c_longlong()
+    _check(load().bg_last_twin(ctx, ctypes.byref(k)), "bg_last_twin")
+    return int(k.value)
 
 
 def bg_class_program_stats(n: int, lanes: int, counts):

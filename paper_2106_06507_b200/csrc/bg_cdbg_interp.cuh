@@ -82,6 +82,8 @@ struct LaunchShape {
     bool conc = false;        // small batches: tiers side by side on the table's side streams
     int regs = 168;           // registers per thread of the instantiation (resident-block estimate)
     int cap_cx = 0;           // > 0: at most this many state elements per event in shared memory (SPILL kernels)
+    bool merged = false;      // one launch for all tiers (list launches)
+    long long tasks_hint = 0; // > 0: events this set of launches is expected to process (list launches; default p.N)
     bool hybrid = false;      // SPILL kernel only for the tiers whose state exceeds cap_cx, the others keep all of it in
                               // shared memory (launch_interp<G, false, S> with both kernels instantiated)
     int spill_blocks = 0;     // SPILL: resident blocks per SM (each owns one global slab)
@@ -113,6 +115,16 @@ struct ProgParams {
     const uint32_t* list;      // nullptr: all records of the tier
     const uint32_t* list_count;
     uint32_t* ticket;          // [kTiers] next list task of the tier (zeroed with the flag counters)
+    // Cascade: events whose Ward residual exceeds tau but not tau_twin are first evaluated once more in FP64
+    // in a rotated frame (same value, independent round-off); they go on to the double-double list only if the two
+    // results differ by more than tau_twin or the second evaluation's own flag quantities exceed tau_twin / tau_rho.
+    int merged;                // 1: the launch serves tiers tier .. kTiers - 1 one after the other (list launches)
+    int twin;                  // bit 0: evaluate in the rotated frame (rotate_frame); bit 1: second stage - compare with
+                               // out[e] and append to flag_list on disagreement instead of writing out[e]
+    double tw2;                // tau_twin^2 (<= tau^2: no second stage, every flagged event goes to flag_list)
+    double td;                 // tau_twin as the bound on |w - w'| / w
+    uint32_t* soft_list;       // [N] first stage: events for the second stage, by record position, per tier like flag_list
+    uint32_t* soft_count;      // [kTiers]
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -215,6 +227,17 @@ struct StateRef {
     }
 };
 
+// The same event in another frame: the spatial components of a momentum rotated by a fixed rotation (axis (1,2,3),
+// angle 1 rad).  The polarisation vectors of Eq. 3 in the gauge k = (q0, -q) rotate with the momenta, so every Lorentz
+// product of the recursion keeps its value and |A|^2 is the same number - computed from different components, i.e.
+// with independent round-off: the difference of the two results samples the FP64 error of the event.
+__device__ __forceinline__ void rotate_frame(double* pk) {
+    const double x = pk[1], y = pk[2], z = pk[3];
+    pk[1] = fma(0.5731378554489869, x, fma(-0.6090066421373933, y, 0.5482918096085999 * z));
+    pk[2] = fma(0.740348840460782, x, fma(0.6716445041915284, y, -0.027879282947946255 * z));
+    pk[3] = fma(-0.35127851212351696, x, fma(0.4219058779181122, y, 0.8358222520957642 * z));
+}
+
 constexpr int kRing = 4;   // op ring per lane: ops are requested kRing - 1 steps before they run
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
@@ -254,6 +277,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     using T = typename StateElem<S>::T;
     using R = typename StateElem<S>::R;
     constexpr bool kComplex = StateElem<S>::kComplex;
+    constexpr bool kTwinOk = kComplex && !StateElem<S>::kDD;     // the FP64 discrete-state kernels
     extern __shared__ double2 smem_raw[];
     T* const smem = reinterpret_cast<T*>(smem_raw);
     const int lane = threadIdx.x;
@@ -269,454 +293,476 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     st_.spill = SPILL ? reinterpret_cast<T*>(p.spill) + (size_t)blockIdx.x * p.spill_cx * EPW + q : nullptr;
     st_.cap = p.slab_cx;
     st_.limit = p.spill_cx;
-    // tasks: the records of the tier, or (re-evaluation) the record positions in the tier's flag list
-    const long long first = p.bounds[p.tier], end = p.list ? first + p.list_count[p.tier] : (long long)p.bounds[p.tier + 1];
-    const long long ntasks = (end - first + EPW - 1) / EPW;
-    auto rec_pos = [&](long long i) -> long long { return p.list ? (long long)__ldg(p.list + i) : i; };
-    const int n = p.n;
-    // lanes of one event (same q) run the same program and meet at its barriers; events of different classes in
-    // one warp pass different numbers of barriers, so the barrier names only the event's own lanes
-    unsigned evmask = 0;
-#pragma unroll
-    for (int i = 0; i < (G < 32 ? G : 32); i++) evmask |= 1u << (q + i * EPW);
+    // one launch per tier, or (merged: list launches, whose tiers share one launch shape) this tier and all after it
+    const int tier_end = p.merged ? kTiers : p.tier + 1;
+    for (int tier = p.tier; tier < tier_end; tier++) {
+        // tasks: the records of the tier, or (re-evaluation) the record positions in the tier's flag list
+        const long long first = p.bounds[tier], end = p.list ? first + p.list_count[tier] : (long long)p.bounds[tier + 1];
+        const long long ntasks = (end - first + EPW - 1) / EPW;
+        auto rec_pos = [&](long long i) -> long long { return p.list ? (long long)__ldg(p.list + i) : i; };
+        const int n = p.n;
+        // lanes of one event (same q) run the same program and meet at its barriers; events of different classes in
+        // one warp pass different numbers of barriers, so the barrier names only the event's own lanes
+        unsigned evmask = 0;
+    #pragma unroll
+        for (int i = 0; i < (G < 32 ? G : 32); i++) evmask |= 1u << (q + i * EPW);
 
-    // the header of a task is loaded one task ahead; the inputs of the next task are prefetched into L2 while
-    // the current one computes (events come in class order, so their rows are scattered over the input arrays)
-    EventHeader hnext;
-    hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
-    // Tasks: record ranges are dealt round-robin (task += gridDim.x: the records are sorted longest program first).
-    // List tasks (re-evaluation) arrive in the random order of the flag appends and take 14 x longer each, so a static
-    // deal leaves a long tail: they are handed out by a ticket counter instead, fetched one task ahead.
-    auto next_ticket = [&]() -> long long {
-        if constexpr (G <= 32) {
-            unsigned v = 0;
-            if (lane == 0) v = atomicAdd(p.ticket + p.tier, 1u);
-            return (long long)__shfl_sync(0xFFFFFFFFu, v, 0);
-        } else {
-            __shared__ unsigned tk;
-            __syncthreads();
-            if (lane == 0) tk = atomicAdd(p.ticket + p.tier, 1u);
-            __syncthreads();
-            return (long long)tk;
-        }
-    };
-    long long task = p.list ? next_ticket() : (long long)blockIdx.x;
-    long long task_next = task < ntasks ? (p.list ? next_ticket() : task + gridDim.x) : ntasks;
-    long long pos_next = 0;    // record position of the next task's event (equals its index unless a list is read)
-    if (task < ntasks) {
-        const long long idx = first + task * EPW + q;
-        if (idx < end) {
-            pos_next = rec_pos(idx);
-            hnext = ld_header(p.rec + (size_t)pos_next * p.rec_bytes);
-        }
-    }
-    // carried from one task to the next: the class info of the next event, requested at the first barrier of the
-    // current task (one load less in the chain header -> info -> ops -> inputs at the start of a task)
-    uint4 ci_next = make_uint4(0, 0, 0, 0);
-    bool ci_next_ok = false;
-    for (; task < ntasks; task = task_next, task_next = task_next < ntasks ? (p.list ? next_ticket() : task_next + gridDim.x) : ntasks) {
-        const long long idx0 = first + task * EPW + q;
-        const bool have = idx0 < end;
-        const long long idx = p.list ? pos_next : idx0;          // record position
-        const EventHeader h = hnext;
-        long long idx_next = 0;
-        {
-            const long long idx2 = first + task_next * EPW + q;
-            hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
-            idx_next = idx2;
-            if (task_next < ntasks && idx2 < end) {
-                if (p.list) idx_next = pos_next = rec_pos(idx2);
-                hnext = ld_header(p.rec + (size_t)idx_next * p.rec_bytes);
-            }
-        }
-        const long long e = h.event;
-        const uint32_t cls = have ? h.cls : 0xFFFFFFFFu;
-        const double* mrec = reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
-        // discrete states: the setup level gives gluon k to lane k % G, so the lane's first momentum is requested
-        // here, ahead of the dependent loads class info -> ops that the setup ops themselves wait for
-        const bool discrete = !kUseRing && p.rec_gstride == 4 && kComplex;   // (G >= 8: measured 1-2 % slower)
-        double pk[4] = {0.0, 0.0, 0.0, 0.0};
-        if (discrete && g < n) {
-#pragma unroll
-            for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + g * 4 + c);
-        }
-        uint4 ci = ci_next;
-        if (!ci_next_ok) ci = __ldg(reinterpret_cast<const uint4*>(p.info + (cls == 0xFFFFFFFFu ? 0 : cls)));
-        ci_next_ok = false;
-        const bool valid = cls != 0xFFFFFFFFu && ((ci.y >> 24) & 0xFF);
-        const uint64_t perm = h.perm;
-        const ProgOp* ops = p.ops + ci.x + g;
-        const int total = valid ? (int)ci.z : 0;
-        bool prefetched = false;
-
-        S amp = s_zero<S>();
-        S wamp = s_zero<S>();     // Ward residual  sqrt2 p_n . J({1..n-1})  (exactly zero without round-off)
-        double asum = 0.0;        // sum of |Re| + |Im| of the closure contributions that add up to the amplitude
-        S acc[4], tacc[6];
-        R Pt[4];
-#pragma unroll
-        for (int c = 0; c < 4; c++) { acc[c] = s_zero<S>(); Pt[c] = r_from(0.0, R()); }
-#pragma unroll
-        for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
-
-        // The lane's ops travel global -> shared by cp.async, kRing - 1 steps ahead, into a private ring (no
-        // registers are held across the latency and nothing else reads these slots); the table ends with spare rows.
-        // With few lanes per event (G <= 4) the program of a class is small and stays in L1: plain loads, two steps
-        // ahead, are cheaper there.
-        auto first_barrier_done = [&]() {
-            prefetched = true;
-            if (hnext.cls != 0xFFFFFFFFu) {
-                // the next event's record (a few 128-byte lines) is pulled into L2 meanwhile
-                for (int k = g * 128; k < p.rec_bytes; k += G * 128)
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(p.rec + (size_t)idx_next * p.rec_bytes + k));
-                if constexpr (kUseRing) {      // (G <= 4: measured neutral to slightly slower)
-                    ci_next = __ldg(reinterpret_cast<const uint4*>(p.info + hnext.cls));
-                    ci_next_ok = true;
-                }
+        // the header of a task is loaded one task ahead; the inputs of the next task are prefetched into L2 while
+        // the current one computes (events come in class order, so their rows are scattered over the input arrays)
+        EventHeader hnext;
+        hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
+        // Tasks: record ranges are dealt round-robin (task += gridDim.x: the records are sorted longest program first).
+        // List tasks (re-evaluation) arrive in the random order of the flag appends and take 14 x longer each, so a static
+        // deal leaves a long tail: they are handed out by a ticket counter instead, fetched one task ahead.
+        auto next_ticket = [&]() -> long long {
+            if constexpr (G <= 32) {
+                unsigned v = 0;
+                if (lane == 0) v = atomicAdd(p.ticket + tier, 1u);
+                return (long long)__shfl_sync(0xFFFFFFFFu, v, 0);
+            } else {
+                __shared__ unsigned tk;
+                __syncthreads();
+                if (lane == 0) tk = atomicAdd(p.ticket + tier, 1u);
+                __syncthreads();
+                return (long long)tk;
             }
         };
-        // Momentum conservation holds for double-precision inputs only to round-off, and the recursion never uses the
-        // momentum of the closing gluon: closing with another gluon than input gluon n evaluates a slightly different
-        // continuation of the amplitude off the momentum-conserving surface - a relative difference of 1e-16 times the
-        // event's condition number, inside the FP64 kernels' own round-off but not inside the re-evaluation's.  The
-        // double-double kernel therefore gives input gluon n, when the class closes with another one, the momentum
-        // -(sum of the others): exactly the momentum flow of the recursion closed with gluon n (oracle, Eq. 22).
-        int kstar = -1;
-        if constexpr (StateElem<S>::kDD) {
-            for (int k = 0; k + 1 < n; k++)
-                if ((int)((perm >> (4 * k)) & 0xF) == n - 1) kstar = k;
+        long long task = p.list ? next_ticket() : (long long)blockIdx.x;
+        long long task_next = task < ntasks ? (p.list ? next_ticket() : task + gridDim.x) : ntasks;
+        long long pos_next = 0;    // record position of the next task's event (equals its index unless a list is read)
+        if (task < ntasks) {
+            const long long idx = first + task * EPW + q;
+            if (idx < end) {
+                pos_next = rec_pos(idx);
+                hnext = ld_header(p.rec + (size_t)pos_next * p.rec_bytes);
+            }
         }
-        auto store_ext_momentum = [&](int kk, int offPt, const double* pk) {
+        // carried from one task to the next: the class info of the next event, requested at the first barrier of the
+        // current task (one load less in the chain header -> info -> ops -> inputs at the start of a task)
+        uint4 ci_next = make_uint4(0, 0, 0, 0);
+        bool ci_next_ok = false;
+        for (; task < ntasks; task = task_next, task_next = task_next < ntasks ? (p.list ? next_ticket() : task_next + gridDim.x) : ntasks) {
+            const long long idx0 = first + task * EPW + q;
+            const bool have = idx0 < end;
+            const long long idx = p.list ? pos_next : idx0;          // record position
+            const EventHeader h = hnext;
+            long long idx_next = 0;
+            {
+                const long long idx2 = first + task_next * EPW + q;
+                hnext.event = 0; hnext.cls = 0xFFFFFFFFu; hnext.perm = 0;
+                idx_next = idx2;
+                if (task_next < ntasks && idx2 < end) {
+                    if (p.list) idx_next = pos_next = rec_pos(idx2);
+                    hnext = ld_header(p.rec + (size_t)idx_next * p.rec_bytes);
+                }
+            }
+            const long long e = h.event;
+            const uint32_t cls = have ? h.cls : 0xFFFFFFFFu;
+            const double* mrec = reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
+            // discrete states: the setup level gives gluon k to lane k % G, so the lane's first momentum is requested
+            // here, ahead of the dependent loads class info -> ops that the setup ops themselves wait for
+            const bool discrete = !kUseRing && p.rec_gstride == 4 && kComplex;   // (G >= 8: measured 1-2 % slower)
+            double pk[4] = {0.0, 0.0, 0.0, 0.0};
+            if (discrete && g < n) {
+    #pragma unroll
+                for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + g * 4 + c);
+                if constexpr (kTwinOk) { if (p.twin & 1) rotate_frame(pk); }
+            }
+            uint4 ci = ci_next;
+            if (!ci_next_ok) ci = __ldg(reinterpret_cast<const uint4*>(p.info + (cls == 0xFFFFFFFFu ? 0 : cls)));
+            ci_next_ok = false;
+            const bool valid = cls != 0xFFFFFFFFu && ((ci.y >> 24) & 0xFF);
+            const uint64_t perm = h.perm;
+            const ProgOp* ops = p.ops + ci.x + g;
+            const int total = valid ? (int)ci.z : 0;
+            bool prefetched = false;
+
+            S amp = s_zero<S>();
+            S wamp = s_zero<S>();     // Ward residual  sqrt2 p_n . J({1..n-1})  (exactly zero without round-off)
+            double asum = 0.0;        // sum of |Re| + |Im| of the closure contributions that add up to the amplitude
+            S acc[4], tacc[6];
+            R Pt[4];
+    #pragma unroll
+            for (int c = 0; c < 4; c++) { acc[c] = s_zero<S>(); Pt[c] = r_from(0.0, R()); }
+    #pragma unroll
+            for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
+
+            // The lane's ops travel global -> shared by cp.async, kRing - 1 steps ahead, into a private ring (no
+            // registers are held across the latency and nothing else reads these slots); the table ends with spare rows.
+            // With few lanes per event (G <= 4) the program of a class is small and stays in L1: plain loads, two steps
+            // ahead, are cheaper there.
+            auto first_barrier_done = [&]() {
+                prefetched = true;
+                if (hnext.cls != 0xFFFFFFFFu) {
+                    // the next event's record (a few 128-byte lines) is pulled into L2 meanwhile
+                    for (int k = g * 128; k < p.rec_bytes; k += G * 128)
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(p.rec + (size_t)idx_next * p.rec_bytes + k));
+                    if constexpr (kUseRing) {      // (G <= 4: measured neutral to slightly slower)
+                        ci_next = __ldg(reinterpret_cast<const uint4*>(p.info + hnext.cls));
+                        ci_next_ok = true;
+                    }
+                }
+            };
+            // Momentum conservation holds for double-precision inputs only to round-off, and the recursion never uses the
+            // momentum of the closing gluon: closing with another gluon than input gluon n evaluates a slightly different
+            // continuation of the amplitude off the momentum-conserving surface - a relative difference of 1e-16 times the
+            // event's condition number, inside the FP64 kernels' own round-off but not inside the re-evaluation's.  The
+            // double-double kernel therefore gives input gluon n, when the class closes with another one, the momentum
+            // -(sum of the others): exactly the momentum flow of the recursion closed with gluon n (oracle, Eq. 22).
+            int kstar = -1;
             if constexpr (StateElem<S>::kDD) {
-                if (kk == kstar) {
-                    R Pe[4];
-#pragma unroll
-                    for (int c = 0; c < 4; c++) Pe[c] = r_from(0.0, R());
-                    for (int j = 0; j < n; j++) {
-                        if (j == kk) continue;
-#pragma unroll
-                        for (int c = 0; c < 4; c++) Pe[c] = r_sub(Pe[c], r_from(__ldcg(mrec + j * p.rec_gstride + c), R()));
+                for (int k = 0; k + 1 < n; k++)
+                    if ((int)((perm >> (4 * k)) & 0xF) == n - 1) kstar = k;
+            }
+            auto store_ext_momentum = [&](int kk, int offPt, const double* pk) {
+                if constexpr (StateElem<S>::kDD) {
+                    if (kk == kstar) {
+                        R Pe[4];
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) Pe[c] = r_from(0.0, R());
+                        for (int j = 0; j < n; j++) {
+                            if (j == kk) continue;
+    #pragma unroll
+                            for (int c = 0; c < 4; c++) Pe[c] = r_sub(Pe[c], r_from(__ldcg(mrec + j * p.rec_gstride + c), R()));
+                        }
+                        st_.stP(offPt, Pe);
+                        return;
                     }
-                    st_.stP(offPt, Pe);
-                    return;
                 }
-            }
-            st_.stPd(offPt, pk);
-        };
-        const int s0 = (discrete && total > 0) ? (n + G - 1) / G : 0;     // steps of the setup level done up front
-        uint4 r0 = make_uint4(0, 0, 0, 0), r1 = r0;
-        if constexpr (kUseRing) {
-            if (total > 0) {
-#pragma unroll
-                for (int i = 0; i < kRing - 1; i++) {
-                    cp_async16(ring + ((s0 + i) % kRing) * kBlock, ops + (size_t)(s0 + i) * G);
-                    asm volatile("cp.async.commit_group;" ::: "memory");
-                }
-                if constexpr (kEarlyRing) {
-                    asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 2) : "memory");
-                    r0 = ring[(s0 % kRing) * kBlock];
-                }
-            }
-        } else {
-            r0 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s0 * G));
-            r1 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)(s0 + 1) * G));
-        }
-        if constexpr (kComplex) {
-            // setup level (discrete states): external currents eps(p_k, lambda_k) and momenta, Eq. 20 / g1-g5
-            int k = g;
-            for (int s = 0; s < s0; s++) {
-                const uint4 raw = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s * G));
-                const int kn = k + G;
-                double pn[4] = {0.0, 0.0, 0.0, 0.0};
-                if (kn < n) {
-#pragma unroll
-                    for (int c = 0; c < 4; c++) pn[c] = __ldcg(mrec + kn * 4 + c);
-                }
-                if ((raw.z >> 16) & OPF_EXT) {
-                    const int kk = (int)raw.w;
-                    if (kk != k) {      // another dealing of the gluons than k % G: fetch what the op names
-#pragma unroll
-                        for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + kk * 4 + c);
+                st_.stPd(offPt, pk);
+            };
+            const int s0 = (discrete && total > 0) ? (n + G - 1) / G : 0;     // steps of the setup level done up front
+            uint4 r0 = make_uint4(0, 0, 0, 0), r1 = r0;
+            if constexpr (kUseRing) {
+                if (total > 0) {
+    #pragma unroll
+                    for (int i = 0; i < kRing - 1; i++) {
+                        cp_async16(ring + ((s0 + i) % kRing) * kBlock, ops + (size_t)(s0 + i) * G);
+                        asm volatile("cp.async.commit_group;" ::: "memory");
                     }
-                    S eps[4];
-                    ext_current(pk, ((perm >> (48 + kk)) & 1) ? 1 : -1, eps);
-                    const int offDst = raw.y >> 16, offPt = raw.z & 0xFFFF;
-#pragma unroll
-                    for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
-                    if (offPt != 0xFFFF) store_ext_momentum(kk, offPt, pk);
-                }
-#pragma unroll
-                for (int c = 0; c < 4; c++) pk[c] = pn[c];
-                k = kn;
-            }
-            if (s0 > 0) {
-                if constexpr (G > 32) __syncthreads(); else __syncwarp(evmask);
-                first_barrier_done();
-            }
-        }
-        {
-            for (int s = s0; s < total; s++) {
-                uint4 raw, r2 = r1;
-                if constexpr (kUseRing) {
-                    cp_async16(ring + ((s + kRing - 1) % kRing) * kBlock, ops + (size_t)(s + kRing - 1) * G);
-                    asm volatile("cp.async.commit_group;" ::: "memory");
                     if constexpr (kEarlyRing) {
                         asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 2) : "memory");
-                        raw = r0;
-                        r2 = ring[((s + 1) % kRing) * kBlock];     // the next step's op leaves the ring one step early
-                    } else {
-                        asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 1) : "memory");
-                        raw = ring[(s % kRing) * kBlock];
+                        r0 = ring[(s0 % kRing) * kBlock];
                     }
-                } else {
-                    raw = r0;
-                    const ProgOp* src = ops + (size_t)(s + 2) * G;
-                    r2 = __ldg(reinterpret_cast<const uint4*>(src));
                 }
-                const int offA = raw.x & 0xFFFF, offB = raw.x >> 16;
-                const int offP1 = raw.y & 0xFFFF, offDst = raw.y >> 16;
-                const int offPt = raw.z & 0xFFFF;
-                const unsigned flags = raw.z >> 16;
-                if (flags & OPF_VALID) {
-                    S a[4], b[4];
-#pragma unroll
-                    for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); b[c] = st_.ld(offB + c); }
-                    R P1[4], P2[4];
-                    st_.ldP(offP1, P1);
-                    if (flags & OPF_FIRST) {
-#pragma unroll
-                        for (int c = 0; c < 4; c++) acc[c] = s_zero<S>();
-#pragma unroll
-                        for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
-                        const int offP2 = (int)(raw.w & 0xFFFF);
-                        R Pb[4];
-                        st_.ldP(offP2, Pb);
-#pragma unroll
-                        for (int c = 0; c < 4; c++) Pt[c] = r_add(P1[c], Pb[c]);
+            } else {
+                r0 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s0 * G));
+                r1 = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)(s0 + 1) * G));
+            }
+            if constexpr (kComplex) {
+                // setup level (discrete states): external currents eps(p_k, lambda_k) and momenta, Eq. 20 / g1-g5
+                int k = g;
+                for (int s = 0; s < s0; s++) {
+                    const uint4 raw = __ldg(reinterpret_cast<const uint4*>(ops + (size_t)s * G));
+                    const int kn = k + G;
+                    double pn[4] = {0.0, 0.0, 0.0, 0.0};
+                    if (kn < n) {
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) pn[c] = __ldcg(mrec + kn * 4 + c);
+                        if constexpr (kTwinOk) { if (p.twin & 1) rotate_frame(pn); }
                     }
-#pragma unroll
-                    for (int c = 0; c < 4; c++) P2[c] = r_sub(Pt[c], P1[c]);
-                    // X(a,b) is linear in the pair (a, T_a): a negative vertex flips the sign bits of that pair
-                    // (integer pipe) instead of multiplying every term by -1 on the FP64 pipe
-                    const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
-#pragma unroll
-                    for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
-                    v3_acc(acc, P1, P2, a, b, 1.0);
-                    if (flags & OPF_TENB) {
-                        S T[6];
-#pragma unroll
-                        for (int c = 0; c < 6; c++) T[c] = st_.ld(offB + 4 + c);
-                        tcontract_acc(acc, T, a, 1.0);
-                    }
-                    if (flags & OPF_TENA) {
-                        S T[6];
-#pragma unroll
-                        for (int c = 0; c < 6; c++) T[c] = cneg(st_.ld(offA + 4 + c), neg);
-                        tcontract_acc(acc, T, b, -1.0);
-                    }
-                    if (!(flags & OPF_CLOSURE)) tbuild_acc(tacc, a, b, 1.0);
-                    if (flags & OPF_PARTIAL) {
-                        // chunk of a split target: raw sums to its scratch slot, finished by a COMBINE op
-#pragma unroll
-                        for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
-#pragma unroll
-                        for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
-                    } else if (flags & OPF_LAST) {
-                        if (flags & OPF_CLOSURE) {
-                            S en[4];
-#pragma unroll
-                            for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
-                            const S term = s_isqrt2(mdot(en, acc));
-                            amp = amp + term;
-                            // Ward identity: the full current is conserved, P . J = 0 with P = P(1..n-1) = -p_n
-                            if constexpr (kComplex && !StateElem<S>::kDD) {
-                                wamp = wamp + mdot(Pt, acc);
-                                asum += fabs(term.re) + fabs(term.im);
-                            }
-                        } else {
-                            const R f = r_isqrt2_over(mdot(Pt, Pt));
-#pragma unroll
-                            for (int c = 0; c < 4; c++) acc[c] = s_scale(f, acc[c]);
-#pragma unroll
-                            for (int c = 0; c < 6; c++) tacc[c] = s_isqrt2(tacc[c]);
-                            if (!(flags & OPF_NOSTORE)) {
-#pragma unroll
-                                for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
-#pragma unroll
-                                for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
-                            }
-                            if (flags & OPF_STOREP) {
-                                st_.stP(offPt, Pt);
-                            }
+                    if ((raw.z >> 16) & OPF_EXT) {
+                        const int kk = (int)raw.w;
+                        if (kk != k) {      // another dealing of the gluons than k % G: fetch what the op names
+    #pragma unroll
+                            for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + kk * 4 + c);
+                            if constexpr (kTwinOk) { if (p.twin & 1) rotate_frame(pk); }
                         }
-                    }
-                } else if (flags & OPF_FUSED) {
-                    // closure vertex X(eps_k, J(pi)) . eps_n with J(pi), T(pi) still in acc / tacc, P(pi) in Pt
-                    S a[4], x[4], en[4];
-                    R P1[4];
-#pragma unroll
-                    for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); x[c] = s_zero<S>(); }
-                    st_.ldP(offP1, P1);
-                    const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
-#pragma unroll
-                    for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
-                    v3_acc(x, P1, Pt, a, acc, 1.0);
-                    tcontract_acc(x, tacc, a, 1.0);
-#pragma unroll
-                    for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
-                    const S term = s_isqrt2(mdot(en, x));
-                    amp = amp + term;
-                    if constexpr (kComplex && !StateElem<S>::kDD) {
-                        double Pf[4];
-#pragma unroll
-                        for (int c = 0; c < 4; c++) Pf[c] = P1[c] + Pt[c];
-                        wamp = wamp + mdot(Pf, x);
-                        asum += fabs(term.re) + fabs(term.im);
-                    }
-                } else if (flags & OPF_COMBINE) {
-                    // add the offB partial sums of a split target and finish it like a LAST op
-#pragma unroll
-                    for (int c = 0; c < 4; c++) acc[c] = st_.ld(offA + c);
-#pragma unroll
-                    for (int c = 0; c < 6; c++) tacc[c] = st_.ld(offA + 4 + c);
-                    for (int r = 1; r < offB; r++) {
-#pragma unroll
-                        for (int c = 0; c < 4; c++) acc[c] = acc[c] + st_.ld(offA + 10 * r + c);
-#pragma unroll
-                        for (int c = 0; c < 6; c++) tacc[c] = tacc[c] + st_.ld(offA + 10 * r + 4 + c);
-                    }
-                    {
-                        const int offP2 = (int)(raw.w & 0xFFFF);
-                        R Pa[4], Pb[4];
-                        st_.ldP(offP1, Pa);
-                        st_.ldP(offP2, Pb);
-#pragma unroll
-                        for (int c = 0; c < 4; c++) Pt[c] = r_add(Pa[c], Pb[c]);
-                    }
-                    const R f = r_isqrt2_over(mdot(Pt, Pt));
-#pragma unroll
-                    for (int c = 0; c < 4; c++) acc[c] = s_scale(f, acc[c]);
-#pragma unroll
-                    for (int c = 0; c < 6; c++) tacc[c] = s_isqrt2(tacc[c]);
-                    if (!(flags & OPF_NOSTORE)) {
-#pragma unroll
-                        for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
-#pragma unroll
-                        for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
-                    }
-                    if (flags & OPF_STOREP) {
-                        st_.stP(offPt, Pt);
-                    }
-                } else if (!StateElem<S>::kDD && (flags & OPF_EXTD)) {
-                    // continuous states (Eq. 7, 9, 12): real polarisation e(phi) times the colour matrix etabar_h eta_g;
-                    // record per gluon: p (4), phi, eta (3), etabar (3), pad
-                    const int k = (int)raw.w;
-                    const double* gr = mrec + k * p.rec_gstride;
-                    double pk[4], ev[4], eta[3], etab[3];
-#pragma unroll
-                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(gr + c);
-                    const double phi = __ldcg(gr + 4);
-#pragma unroll
-                    for (int c = 0; c < 3; c++) { eta[c] = __ldcg(gr + 5 + c); etab[c] = __ldcg(gr + 8 + c); }
-                    polarisation_real(pk, phi, ev);
-                    const bool closure_leg = offPt == 0xFFFF;   // gluon n: no momentum slot; target (h,g) reads X_n[g][h]
-#pragma unroll
-                    for (int h = 0; h < 3; h++)
-#pragma unroll
-                        for (int gg = 0; gg < 3; gg++) {
-                            const double x = etab[h] * eta[gg];
-                            const int at = offDst + 4 * (h * 3 + gg);
-#pragma unroll
-                            for (int c = 0; c < 4; c++) st_.st(at + c, s_real<S>(x * ev[c]));
-                        }
-                    if (!closure_leg) {
-                        st_.stPd(offPt, pk);
-                    }
-                } else if ((flags & OPF_EXT) && kComplex) {
-                    const int k = (int)raw.w;
-                    double pk[4];
-#pragma unroll
-                    for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + k * p.rec_gstride + c);   // not through L1: it is kept for the ops
-                    if constexpr (kComplex) {
                         S eps[4];
-                        ext_current(pk, ((perm >> (48 + k)) & 1) ? 1 : -1, eps);
-#pragma unroll
+                        ext_current(pk, ((perm >> (48 + kk)) & 1) ? 1 : -1, eps);
+                        const int offDst = raw.y >> 16, offPt = raw.z & 0xFFFF;
+    #pragma unroll
                         for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
+                        if (offPt != 0xFFFF) store_ext_momentum(kk, offPt, pk);
                     }
-                    if (offPt != 0xFFFF) store_ext_momentum(k, offPt, pk);
+    #pragma unroll
+                    for (int c = 0; c < 4; c++) pk[c] = pn[c];
+                    k = kn;
                 }
-                if (flags & OPF_SYNC) {
-                    // end of a level: the currents just written become visible to the lanes of the event
+                if (s0 > 0) {
                     if constexpr (G > 32) __syncthreads(); else __syncwarp(evmask);
-                    if (!prefetched) first_barrier_done();
-                }
-                {
-                    // The op requested at the top of this step must not be touched before the step ends (the
-                    // compiler would otherwise park it right behind the load with moves that wait for it): its
-                    // first use is tied to the step's last arithmetic results through an always-zero mask.
-                    const unsigned late = (unsigned)(hi_word(acc[0]) ^ hi_word(amp)) & (unsigned)p.zero;
-                    const uint4 moved = make_uint4(r2.x | late, r2.y | late, r2.z | late, r2.w | late);
-                    if constexpr (kEarlyRing) { r0 = moved; } else if constexpr (!kUseRing) { r0 = r1; r1 = moved; }
+                    first_barrier_done();
                 }
             }
-            if constexpr (kUseRing) asm volatile("cp.async.wait_group 0;" ::: "memory");
-        }
-
-        // closure amplitude: sum of the G lanes' partial contractions (Eq. 22), then |A|^2
-        constexpr bool kWard = kComplex && !StateElem<S>::kDD;
-        const bool flagging = kWard && p.tau2 > 0.0;
-#pragma unroll
-        for (int d = EPW; d < 32; d <<= 1) {
-            amp = amp + shfl_xor(amp, d);
-            if constexpr (kWard) { wamp = wamp + shfl_xor(wamp, d); asum += shfl_xor(asum, d); }
-        }
-        if constexpr (G > 32) {
-            __shared__ double red_s[(kWard ? 3 : 1) * (sizeof(S) / 8) * (G / 32)];
-            if ((lane & 31) == 0) {
-                reinterpret_cast<S*>(red_s)[lane >> 5] = amp;
-                if constexpr (kWard) {
-                    reinterpret_cast<S*>(red_s)[G / 32 + (lane >> 5)] = wamp;
-                    red_s[2 * (sizeof(S) / 8) * (G / 32) + (lane >> 5)] = asum;
-                }
-            }
-            __syncthreads();
-            if (lane == 0) {
-                amp = s_zero<S>();
-                for (int w = 0; w < G / 32; w++) amp = amp + reinterpret_cast<S*>(red_s)[w];
-                if constexpr (kWard) {
-                    wamp = s_zero<S>();
-                    asum = 0.0;
-                    for (int w = 0; w < G / 32; w++) {
-                        wamp = wamp + reinterpret_cast<S*>(red_s)[G / 32 + w];
-                        asum += red_s[2 * (sizeof(S) / 8) * (G / 32) + w];
+            {
+                for (int s = s0; s < total; s++) {
+                    uint4 raw, r2 = r1;
+                    if constexpr (kUseRing) {
+                        cp_async16(ring + ((s + kRing - 1) % kRing) * kBlock, ops + (size_t)(s + kRing - 1) * G);
+                        asm volatile("cp.async.commit_group;" ::: "memory");
+                        if constexpr (kEarlyRing) {
+                            asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 2) : "memory");
+                            raw = r0;
+                            r2 = ring[((s + 1) % kRing) * kBlock];     // the next step's op leaves the ring one step early
+                        } else {
+                            asm volatile("cp.async.wait_group %0;" ::"n"(kRing - 1) : "memory");
+                            raw = ring[(s % kRing) * kBlock];
+                        }
+                    } else {
+                        raw = r0;
+                        const ProgOp* src = ops + (size_t)(s + 2) * G;
+                        r2 = __ldg(reinterpret_cast<const uint4*>(src));
                     }
-                }
-            }
-        }
-        if (g == 0 && have) {
-            const double w = valid ? s_norm2(amp) : 0.0;
-            p.out[e] = w;
-            if constexpr (kWard) {
-                if (p.tau2 < 0.0 && valid) {
-                    // diagnostic (BG_OPT_PRECISION = 3): the Ward residual itself instead of |A|^2
-                    const double En = __ldcg(mrec + (n - 1) * p.rec_gstride);
-                    p.out[e] = p.tau2 < -1.5 ? (fabs(amp.re) + fabs(amp.im)) / asum : ::sqrt(0.5 * s_norm2(wamp) / (En * En * w));
-                }
-                if (flagging && valid) {
-                    // |sqrt2 p_n . J|^2 / 2 > tau^2 E_n^2 |A|^2, or |A| < tau_rho sum |closure terms| (the Ward residual does
-                    // not see round-off that respects gauge invariance; strong cancellation at the top amplifies
-                    // any), or a result that is not a positive finite number: evaluated again in double-double
-                    const double En = __ldcg(mrec + (n - 1) * p.rec_gstride);
-                    if (!(0.5 * s_norm2(wamp) <= p.tau2 * En * En * w) || !(fabs(amp.re) + fabs(amp.im) >= p.tau_rho * asum) || !(w > 0.0))
+                    const int offA = raw.x & 0xFFFF, offB = raw.x >> 16;
+                    const int offP1 = raw.y & 0xFFFF, offDst = raw.y >> 16;
+                    const int offPt = raw.z & 0xFFFF;
+                    const unsigned flags = raw.z >> 16;
+                    if (flags & OPF_VALID) {
+                        S a[4], b[4];
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); b[c] = st_.ld(offB + c); }
+                        R P1[4], P2[4];
+                        st_.ldP(offP1, P1);
+                        if (flags & OPF_FIRST) {
+    #pragma unroll
+                            for (int c = 0; c < 4; c++) acc[c] = s_zero<S>();
+    #pragma unroll
+                            for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
+                            const int offP2 = (int)(raw.w & 0xFFFF);
+                            R Pb[4];
+                            st_.ldP(offP2, Pb);
+    #pragma unroll
+                            for (int c = 0; c < 4; c++) Pt[c] = r_add(P1[c], Pb[c]);
+                        }
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) P2[c] = r_sub(Pt[c], P1[c]);
+                        // X(a,b) is linear in the pair (a, T_a): a negative vertex flips the sign bits of that pair
+                        // (integer pipe) instead of multiplying every term by -1 on the FP64 pipe
+                        const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
+                        v3_acc(acc, P1, P2, a, b, 1.0);
+                        if (flags & OPF_TENB) {
+                            S T[6];
+    #pragma unroll
+                            for (int c = 0; c < 6; c++) T[c] = st_.ld(offB + 4 + c);
+                            tcontract_acc(acc, T, a, 1.0);
+                        }
+                        if (flags & OPF_TENA) {
+                            S T[6];
+    #pragma unroll
+                            for (int c = 0; c < 6; c++) T[c] = cneg(st_.ld(offA + 4 + c), neg);
+                            tcontract_acc(acc, T, b, -1.0);
+                        }
+                        if (!(flags & OPF_CLOSURE)) tbuild_acc(tacc, a, b, 1.0);
+                        if (flags & OPF_PARTIAL) {
+                            // chunk of a split target: raw sums to its scratch slot, finished by a COMBINE op
+    #pragma unroll
+                            for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
+    #pragma unroll
+                            for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
+                        } else if (flags & OPF_LAST) {
+                            if (flags & OPF_CLOSURE) {
+                                S en[4];
+    #pragma unroll
+                                for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
+                                const S term = s_isqrt2(mdot(en, acc));
+                                amp = amp + term;
+                                // Ward identity: the full current is conserved, P . J = 0 with P = P(1..n-1) = -p_n
+                                if constexpr (kComplex && !StateElem<S>::kDD) {
+                                    wamp = wamp + mdot(Pt, acc);
+                                    asum += fabs(term.re) + fabs(term.im);
+                                }
+                            } else {
+                                const R f = r_isqrt2_over(mdot(Pt, Pt));
+    #pragma unroll
+                                for (int c = 0; c < 4; c++) acc[c] = s_scale(f, acc[c]);
+    #pragma unroll
+                                for (int c = 0; c < 6; c++) tacc[c] = s_isqrt2(tacc[c]);
+                                if (!(flags & OPF_NOSTORE)) {
+    #pragma unroll
+                                    for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
+    #pragma unroll
+                                    for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
+                                }
+                                if (flags & OPF_STOREP) {
+                                    st_.stP(offPt, Pt);
+                                }
+                            }
+                        }
+                    } else if (flags & OPF_FUSED) {
+                        // closure vertex X(eps_k, J(pi)) . eps_n with J(pi), T(pi) still in acc / tacc, P(pi) in Pt
+                        S a[4], x[4], en[4];
+                        R P1[4];
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); x[c] = s_zero<S>(); }
+                        st_.ldP(offP1, P1);
+                        const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
+                        v3_acc(x, P1, Pt, a, acc, 1.0);
+                        tcontract_acc(x, tacc, a, 1.0);
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
+                        const S term = s_isqrt2(mdot(en, x));
+                        amp = amp + term;
+                        if constexpr (kComplex && !StateElem<S>::kDD) {
+                            double Pf[4];
+    #pragma unroll
+                            for (int c = 0; c < 4; c++) Pf[c] = P1[c] + Pt[c];
+                            wamp = wamp + mdot(Pf, x);
+                            asum += fabs(term.re) + fabs(term.im);
+                        }
+                    } else if (flags & OPF_COMBINE) {
+                        // add the offB partial sums of a split target and finish it like a LAST op
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) acc[c] = st_.ld(offA + c);
+    #pragma unroll
+                        for (int c = 0; c < 6; c++) tacc[c] = st_.ld(offA + 4 + c);
+                        for (int r = 1; r < offB; r++) {
+    #pragma unroll
+                            for (int c = 0; c < 4; c++) acc[c] = acc[c] + st_.ld(offA + 10 * r + c);
+    #pragma unroll
+                            for (int c = 0; c < 6; c++) tacc[c] = tacc[c] + st_.ld(offA + 10 * r + 4 + c);
+                        }
+                        {
+                            const int offP2 = (int)(raw.w & 0xFFFF);
+                            R Pa[4], Pb[4];
+                            st_.ldP(offP1, Pa);
+                            st_.ldP(offP2, Pb);
+    #pragma unroll
+                            for (int c = 0; c < 4; c++) Pt[c] = r_add(Pa[c], Pb[c]);
+                        }
+                        const R f = r_isqrt2_over(mdot(Pt, Pt));
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) acc[c] = s_scale(f, acc[c]);
+    #pragma unroll
+                        for (int c = 0; c < 6; c++) tacc[c] = s_isqrt2(tacc[c]);
+                        if (!(flags & OPF_NOSTORE)) {
+    #pragma unroll
+                            for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
+    #pragma unroll
+                            for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
+                        }
+                        if (flags & OPF_STOREP) {
+                            st_.stP(offPt, Pt);
+                        }
+                    } else if (!StateElem<S>::kDD && (flags & OPF_EXTD)) {
+                        // continuous states (Eq. 7, 9, 12): real polarisation e(phi) times the colour matrix etabar_h eta_g;
+                        // record per gluon: p (4), phi, eta (3), etabar (3), pad
+                        const int k = (int)raw.w;
+                        const double* gr = mrec + k * p.rec_gstride;
+                        double pk[4], ev[4], eta[3], etab[3];
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) pk[c] = __ldcg(gr + c);
+                        const double phi = __ldcg(gr + 4);
+    #pragma unroll
+                        for (int c = 0; c < 3; c++) { eta[c] = __ldcg(gr + 5 + c); etab[c] = __ldcg(gr + 8 + c); }
+                        polarisation_real(pk, phi, ev);
+                        const bool closure_leg = offPt == 0xFFFF;   // gluon n: no momentum slot; target (h,g) reads X_n[g][h]
+    #pragma unroll
+                        for (int h = 0; h < 3; h++)
+    #pragma unroll
+                            for (int gg = 0; gg < 3; gg++) {
+                                const double x = etab[h] * eta[gg];
+                                const int at = offDst + 4 * (h * 3 + gg);
+    #pragma unroll
+                                for (int c = 0; c < 4; c++) st_.st(at + c, s_real<S>(x * ev[c]));
+                            }
+                        if (!closure_leg) {
+                            st_.stPd(offPt, pk);
+                        }
+                    } else if ((flags & OPF_EXT) && kComplex) {
+                        const int k = (int)raw.w;
+                        double pk[4];
+    #pragma unroll
+                        for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + k * p.rec_gstride + c);   // not through L1: it is kept for the ops
+                        if constexpr (kTwinOk) { if (p.twin & 1) rotate_frame(pk); }
+                        if constexpr (kComplex) {
+                            S eps[4];
+                            ext_current(pk, ((perm >> (48 + k)) & 1) ? 1 : -1, eps);
+    #pragma unroll
+                            for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
+                        }
+                        if (offPt != 0xFFFF) store_ext_momentum(k, offPt, pk);
+                    }
+                    if (flags & OPF_SYNC) {
+                        // end of a level: the currents just written become visible to the lanes of the event
+                        if constexpr (G > 32) __syncthreads(); else __syncwarp(evmask);
+                        if (!prefetched) first_barrier_done();
+                    }
                     {
-                        const uint32_t at = atomicAdd(p.flag_count + p.tier, 1u);
-                        BG_CHECK(first + at < end);
-                        p.flag_list[first + at] = (uint32_t)idx;
+                        // The op requested at the top of this step must not be touched before the step ends (the
+                        // compiler would otherwise park it right behind the load with moves that wait for it): its
+                        // first use is tied to the step's last arithmetic results through an always-zero mask.
+                        const unsigned late = (unsigned)(hi_word(acc[0]) ^ hi_word(amp)) & (unsigned)p.zero;
+                        const uint4 moved = make_uint4(r2.x | late, r2.y | late, r2.z | late, r2.w | late);
+                        if constexpr (kEarlyRing) { r0 = moved; } else if constexpr (!kUseRing) { r0 = r1; r1 = moved; }
+                    }
+                }
+                if constexpr (kUseRing) asm volatile("cp.async.wait_group 0;" ::: "memory");
+            }
+
+            // closure amplitude: sum of the G lanes' partial contractions (Eq. 22), then |A|^2
+            constexpr bool kWard = kComplex && !StateElem<S>::kDD;
+            const bool flagging = kWard && p.tau2 > 0.0;
+    #pragma unroll
+            for (int d = EPW; d < 32; d <<= 1) {
+                amp = amp + shfl_xor(amp, d);
+                if constexpr (kWard) { wamp = wamp + shfl_xor(wamp, d); asum += shfl_xor(asum, d); }
+            }
+            if constexpr (G > 32) {
+                __shared__ double red_s[(kWard ? 3 : 1) * (sizeof(S) / 8) * (G / 32)];
+                if ((lane & 31) == 0) {
+                    reinterpret_cast<S*>(red_s)[lane >> 5] = amp;
+                    if constexpr (kWard) {
+                        reinterpret_cast<S*>(red_s)[G / 32 + (lane >> 5)] = wamp;
+                        red_s[2 * (sizeof(S) / 8) * (G / 32) + (lane >> 5)] = asum;
+                    }
+                }
+                __syncthreads();
+                if (lane == 0) {
+                    amp = s_zero<S>();
+                    for (int w = 0; w < G / 32; w++) amp = amp + reinterpret_cast<S*>(red_s)[w];
+                    if constexpr (kWard) {
+                        wamp = s_zero<S>();
+                        asum = 0.0;
+                        for (int w = 0; w < G / 32; w++) {
+                            wamp = wamp + reinterpret_cast<S*>(red_s)[G / 32 + w];
+                            asum += red_s[2 * (sizeof(S) / 8) * (G / 32) + w];
+                        }
                     }
                 }
             }
+            if (g == 0 && have) {
+                const double w = valid ? s_norm2(amp) : 0.0;
+                if (!(kWard && (p.twin & 2))) p.out[e] = w;      // (second stage of the cascade: out[e] keeps the first result)
+                if constexpr (kWard) {
+                    if (p.tau2 < 0.0 && valid) {
+                        // diagnostic (BG_OPT_PRECISION = 3): the Ward residual itself instead of |A|^2
+                        const double En = __ldcg(mrec + (n - 1) * p.rec_gstride);
+                        p.out[e] = p.tau2 < -1.5 ? (fabs(amp.re) + fabs(amp.im)) / asum : ::sqrt(0.5 * s_norm2(wamp) / (En * En * w));
+                    }
+                    if (flagging && valid) {
+                        // |sqrt2 p_n . J|^2 / 2 > tau^2 E_n^2 |A|^2, or |A| < tau_rho sum |closure terms| (the Ward residual does
+                        // not see round-off that respects gauge invariance; strong cancellation at the top amplifies
+                        // any), or a result that is not a positive finite number: not trusted as it stands
+                        const double En = __ldcg(mrec + (n - 1) * p.rec_gstride);
+                        const double ward2 = 0.5 * s_norm2(wamp), scale = En * En * w;
+                        const bool hard = !(ward2 <= fmax(p.tw2, p.tau2) * scale) ||
+                                          !(fabs(amp.re) + fabs(amp.im) >= p.tau_rho * asum) || !(w > 0.0);
+                        bool to_dd = hard, to_twin = false;
+                        if (p.twin & 2) {
+                            // second stage: this frame's result against the first one's
+                            const double w1 = p.out[e];
+                            to_dd = hard || !(fabs(w - w1) <= p.td * w1);
+                        } else if (!hard) {
+                            to_twin = !(ward2 <= p.tau2 * scale);      // (tau_twin <= tau: never - no second stage)
+                        }
+                        if (to_dd) {
+                            const uint32_t at = atomicAdd(p.flag_count + tier, 1u);
+                            BG_CHECK(first + at < (long long)p.bounds[tier + 1]);
+                            p.flag_list[first + at] = (uint32_t)idx;
+                        } else if (to_twin) {
+                            const uint32_t at = atomicAdd(p.soft_count + tier, 1u);
+                            BG_CHECK(first + at < (long long)p.bounds[tier + 1]);
+                            p.soft_list[first + at] = (uint32_t)idx;
+                        }
+                    }
+                }
+            }
+            if constexpr (G > 32) __syncthreads(); else __syncwarp();
         }
-        if constexpr (G > 32) __syncthreads(); else __syncwarp();
     }
 }
 
@@ -757,7 +803,33 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
     if constexpr (kHasSpill)
         if ((cerr = configure_interp<G, true, S>(&static_spill)) != cudaSuccess) return cerr;
     bool hybrid = HYBRID && shape.hybrid && shape.cap_cx > 0;
-    const long long max_tasks = (p.N + EPW - 1) / EPW + kTiers;
+    if (shape.merged) {
+        // list launches (second stage, re-evaluation): few tasks per tier, so one launch walks the tiers' lists one after
+        // the other (heaviest first; tasks by ticket) with the shape of the largest tier
+        int k0 = 0;
+        while (k0 + 1 < kTiers && t->tiers.first_key[k0] == t->tiers.first_key[k0 + 1]) k0++;
+        const size_t ring_bytes = G >= 8 ? (size_t)kRing * BLOCK * 16 : 0;
+        const bool sp = SPILL || (hybrid && t->tiers.slab_cx[k0] > shape.cap_cx);
+        const int slab = (shape.cap_cx > 0 && sp) ? std::min(t->tiers.slab_cx[k0], shape.cap_cx) : t->tiers.slab_cx[k0];
+        const size_t smem = ((size_t)EPW * slab * ELEM + 15) / 16 * 16 + ring_bytes;
+        if (smem > kMaxSlabBytes + ring_bytes) return cudaErrorInvalidValue;
+        int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (shape.regs * BLOCK), (228 * 1024) / (smem + 1024 + (sp ? static_spill : static_direct))));
+        if (sp) per_sm = std::min(per_sm, shape.spill_blocks);
+        const long long tasks = ((shape.tasks_hint > 0 ? shape.tasks_hint : p.N) + EPW - 1) / EPW + kTiers;
+        long long blocks = std::max<long long>(1, std::min<long long>(tasks, (long long)sm_count * per_sm));
+        if (sp && shape.max_blocks > 0) blocks = std::min<long long>(blocks, shape.max_blocks);
+        p.tier = k0;
+        p.merged = 1;
+        p.slab_cx = slab;
+        if (sp) {
+            if constexpr (kHasSpill) cdbg_prog_kernel<G, true, S><<<(unsigned)blocks, BLOCK, smem, s>>>(p);
+        } else {
+            if constexpr (kHasDirect) cdbg_prog_kernel<G, false, S><<<(unsigned)blocks, BLOCK, smem, s>>>(p);
+        }
+        ++*launched;
+        return cudaGetLastError();
+    }
+    const long long max_tasks = ((shape.tasks_hint > 0 ? shape.tasks_hint : p.N) + EPW - 1) / EPW + kTiers;
     if (hybrid) {
         // small batches (fewer than two tasks per block the uncapped launches hold): occupancy is not what limits
         // them, and the capped kernel's L2 round trips cost more than they hide (n = 6: 2^16 events +7 %, 2^17 equal,

@@ -51,7 +51,7 @@ cdbg_classify_kernel(int n, long long N, long long num_classes, const signed cha
                      uint32_t* __restrict__ flag_count) {
     extern __shared__ uint32_t sh_hist[];
     const int nbins = (int)num_classes + 1;
-    if (blockIdx.x == 0 && threadIdx.x < 2 * kTiers) flag_count[threadIdx.x] = 0;   // lists of the conditioning flag: counters | tickets
+    if (blockIdx.x == 0 && threadIdx.x < 4 * kTiers) flag_count[threadIdx.x] = 0;   // lists of the conditioning flag: counters | tickets, twice
     if (BLOCK_HIST) {
         for (int i = threadIdx.x; i < nbins; i += THREADS) sh_hist[i] = 0;
         __syncthreads();
@@ -719,12 +719,14 @@ int prog_lanes(const ProgTable* t) { return t ? t->G : 0; }
 int prog_dd_mode(const ProgTable* t) { return t ? t->dd_mode : -1; }
 
 // scratch: records (32 + 32 n) B x N | perm u64[N] | cls u32[N] | hist u32[num_classes + 1] | tier bounds (64 B) |
-//          flag counters (64 B) | flag lists u32[N] | spill slabs (FP64) | spill slabs (double-double re-evaluation)
+//          flag counters (64 B: double-double list counts | its tickets | second-stage list counts | its tickets) |
+//          double-double list u32[N] | second-stage list u32[N] | spill slabs (FP64) | spill slabs (capped FP64 launches
+//          and double-double re-evaluation)
 static size_t prog_flag_offset(const ProgTable* t, long long N) {
     return ((size_t)N * (12 + t->rec_bytes) + ((size_t)t->num_classes + 1) * 4 + 15) / 16 * 16 + 64;
 }
 static size_t prog_spill_offset(const ProgTable* t, long long N) {
-    return (prog_flag_offset(t, N) + 64 + (size_t)N * 4 + 255) / 256 * 256;
+    return (prog_flag_offset(t, N) + 64 + (size_t)N * 8 + 255) / 256 * 256;
 }
 static size_t prog_spill_bytes(const ProgTable* t) {
     // spill kernels run a fixed number of blocks per SM, each with a slab for the largest state
@@ -746,14 +748,26 @@ cudaError_t prog_flagged_count(const ProgTable* t, long long N, const void* scra
     for (int k = 0; k < kTiers; k++) *count += c[k];
     return err;
 }
+// ... and how many of its events went through the second (rotated-frame FP64) stage
+cudaError_t prog_twin_count(const ProgTable* t, long long N, const void* scratch, long long* count) {
+    uint32_t c[kTiers] = {0, 0, 0, 0};
+    const cudaError_t err = cudaMemcpy(c, (const char*)scratch + prog_flag_offset(t, N) + 2 * kTiers * sizeof(uint32_t), sizeof(c),
+                                       cudaMemcpyDeviceToHost);
+    *count = 0;
+    for (int k = 0; k < kTiers; k++) *count += c[k];
+    return err;
+}
 
-cudaError_t dispatch_interp_dd(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches, bool conc);   // bg_cdbg_prog_dd.cu
+cudaError_t dispatch_interp_dd(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches, bool conc,
+                               bool merged, long long tasks_hint);   // bg_cdbg_prog_dd.cu
 
 static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches,
-                                   bool conc = false) {
+                                   bool conc = false, long long tasks_hint = 0, bool merged = false) {
     cudaError_t err;
     LaunchShape shape;
     shape.conc = conc;
+    shape.tasks_hint = tasks_hint;
+    shape.merged = merged;
     shape.spill_blocks = t->spill_blocks_per_sm;
     if (t->real) {   // continuous states with real polarisations: all-real arithmetic
         switch (t->G) {
@@ -795,7 +809,8 @@ static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_co
 
 cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
                              const signed char* hel, const signed char* col, double* out, void* scratch,
-                             int* launches, cudaEvent_t ev0, cudaEvent_t ev1, double tau, double tau_rho, cudaEvent_t ev_mid) {
+                             int* launches, cudaEvent_t ev0, cudaEvent_t ev1, double tau, double tau_rho, cudaEvent_t ev_mid,
+                             double tau_twin, double tau_twin_ward, bool rotated) {
     if (tau > 0.0 && t->dd_mode < 0) return cudaErrorNotSupported;
     const int rec_bytes = t->rec_bytes;
     char* rec = (char*)scratch;
@@ -873,6 +888,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     if (t->cap_cx > 0) p.spill = (double2*)((char*)scratch + prog_spill_offset(t, N) + prog_spill_bytes(t));
     p.spill_cx = t->max_state_cx;
     p.tier = 0;
+    p.merged = 0;
     p.slab_cx = t->max_state_cx;
     p.tau2 = tau < 0.0 ? tau : tau * tau;
     p.tau_rho = tau_rho;
@@ -881,18 +897,41 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.list = nullptr;
     p.list_count = nullptr;
     p.ticket = flag_count + kTiers;
+    p.twin = rotated ? 1 : 0;
+    const bool cascade = tau > 0.0 && tau_twin_ward > tau;
+    p.tw2 = cascade ? tau_twin_ward * tau_twin_ward : 0.0;
+    p.td = tau_twin;
+    p.soft_count = flag_count + 2 * kTiers;
+    p.soft_list = flag_list + N;
     *launches = fused ? 2 : 3;
     if (ev0) cudaEventRecord(ev0, s);
     err = dispatch_interp(s, t, sm_count, p, launches, true);
+    if (tau > 0.0 && ev_mid) cudaEventRecord(ev_mid, s);
+    if (cascade && err == cudaSuccess) {
+        // second stage: the events between the two thresholds once more in FP64, in the rotated frame; out[] keeps the
+        // first result, and what disagrees joins the double-double list
+        p.twin = rotated ? 2 : 3;
+        p.list = p.soft_list;
+        p.list_count = p.soft_count;
+        p.ticket = flag_count + 3 * kTiers;
+        // One launch for the lists of all tiers where measured faster: 4 lanes per event (n = 5, 6) from 2^18 events
+        // (2^16: +4 %, 2^20: -1 %), 8 - 64 lanes (n = 7 - 9: -2 ... -5 % at 2^16, equal at 2^18) and the spill kernels
+        // (n >= 11: -1 ... -5 %); 128 lanes without spill (n = 10) keep the tiers' own launch shapes (+2 %).
+        const bool merged = t->spill || (t->G <= 4 ? N >= (1ll << 18) : t->G <= 64);
+        err = dispatch_interp(s, t, sm_count, p, launches, true, std::max<long long>(1, N / 16), merged);
+    }
     if (tau > 0.0 && err == cudaSuccess) {
         // the flagged events of every tier once more, in double-double arithmetic (overwrites their out[])
-        if (ev_mid) cudaEventRecord(ev_mid, s);
         p.tau2 = 0.0;
+        p.twin = 0;
+        p.ticket = flag_count + kTiers;
         p.list = flag_list;
         p.list_count = flag_count;
         p.spill = t->dd_mode == 1 ? (double2*)((char*)scratch + prog_spill_offset(t, N) + prog_spill_bytes(t)) : nullptr;
         // few flagged events per tier for batches up to 2^19: the tier launches overlap their ramp-up and tails
-        err = dispatch_interp_dd(s, t, sm_count, p, launches, N <= (1ll << 19) && t->G < 32);   // (block-per-event lane counts: measured slower)
+        // one launch walks the lists of all tiers (their capped shared state has one size): few tasks per tier, each
+        // 14 x an FP64 task, so per-tier launches were mostly tails (n = 6, 2^20 events: 1.15 -> 0.80 ms after the first pass)
+        err = dispatch_interp_dd(s, t, sm_count, p, launches, false, true, std::max<long long>(1, N / 32));
     }
     if (ev1) cudaEventRecord(ev1, s);
     return err;
@@ -915,10 +954,12 @@ cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, 
     p.spill = t->spill ? (double2*)((char*)scratch + prog_spill_offset(t, N)) : nullptr;
     p.spill_cx = t->max_state_cx;
     p.tier = 0;
+    p.merged = 0;
     p.slab_cx = t->max_state_cx;
     p.tau2 = 0.0;
     p.tau_rho = 0.0;
     p.flag_list = nullptr; p.flag_count = nullptr; p.list = nullptr; p.list_count = nullptr; p.ticket = nullptr;
+    p.twin = 0; p.tw2 = 0.0; p.td = 0.0; p.soft_list = nullptr; p.soft_count = nullptr;
     *launches = 1;
     if (ev0) cudaEventRecord(ev0, s);
     err = dispatch_interp(s, t, sm_count, p, launches, false);

@@ -55,14 +55,17 @@ __device__ __forceinline__ cxd shfl_xor(cxd v, int d) {
 }
 __device__ __forceinline__ int hi_word(cxd v) { return __double2hiint(v.re.hi); }
 
-cudaError_t dispatch_interp_dd(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches, bool conc) {
+cudaError_t dispatch_interp_dd(cudaStream_t s, const ProgTable* t, int sm_count, const ProgParams& p, int* launches, bool conc, bool merged,
+                               long long tasks_hint) {
     if (t->dd_mode < 0 || t->dense) return cudaErrorInvalidValue;
     LaunchShape shape;
     shape.regs = 255;
     shape.conc = conc;   // small batches: the tier launches side by side, each with its share of the slabs
+    shape.merged = merged;   // ... or one launch for the lists of all tiers (the capped shared state is the same for all)
     shape.cap_cx = t->dd_cap_cx;
     shape.spill_blocks = t->dd_spill_blocks;
     shape.max_blocks = t->dd_max_blocks;
+    shape.tasks_hint = tasks_hint;
     // always the SPILL instantiation: offsets below the cap live in shared memory, the rest in the block's slab
     switch (t->G) {
         case 1: return launch_interp<1, true, cxd>(s, t, sm_count, p, launches, shape);

@@ -42,6 +42,8 @@ struct bg_ctx {
                                // re-evaluation of the events the conditioning flag names (default where available)
     double tau;                // BG_OPT_FLAG_THRESHOLD: Ward-residual threshold of the conditioning flag
     double tau_rho;            // ... and its threshold for the cancellation among the closure contributions
+    double tau_twin;           // BG_OPT_FLAG_TWIN: what the second (rotated-frame) FP64 evaluation may differ by
+    int frame;                 // BG_OPT_FRAME: 1 = evaluate in the rotated frame (diagnostic)
     cudaEvent_t ev_mid;        // (timing) between the FP64 launches and the re-evaluation
     long long last_N;          // events of the most recent bg_eval (for bg_last_refined)
     bool last_auto;            // ... and whether it ran with the conditioning flag
@@ -88,8 +90,10 @@ size_t prog_scratch_bytes(const ProgTable* t, long long N);
 // is recorded between the FP64 launches and that re-evaluation)
 cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
                              const signed char* hel, const signed char* col, double* out, void* scratch,
-                             int* launches, cudaEvent_t ev0, cudaEvent_t ev1, double tau, double tau_rho, cudaEvent_t ev_mid);
+                             int* launches, cudaEvent_t ev0, cudaEvent_t ev1, double tau, double tau_rho, cudaEvent_t ev_mid,
+                             double tau_twin, double tau_twin_ward, bool rotated);
 cudaError_t prog_flagged_count(const ProgTable* t, long long N, const void* scratch, long long* count);
+cudaError_t prog_twin_count(const ProgTable* t, long long N, const void* scratch, long long* count);
 int prog_dd_mode(const ProgTable* t);   // 0 / 1: re-evaluation available (1: with spill); -1: state does not fit
 
 cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,

@@ -3,7 +3,7 @@ import numpy as np
 
 
 def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None, lanes=None, smem_limit=None, precision=None,
-             flag_threshold=None):
+             flag_threshold=None, flag_twin=None, frame=None):
     """ev: workload.Events (AoS numpy).  Returns out[N] (numpy) and the kernel name used."""
     import torch
     import paper_2106_06507_b200 as bg
@@ -30,6 +30,10 @@ def gpu_eval(ev, mode, kernel=0, host=False, scratch_limit=None, lanes=None, sme
             bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, precision)
         if flag_threshold is not None:
             bg.bg_set_option(ctx, bg.BG_OPT_FLAG_THRESHOLD, flag_threshold)
+        if flag_twin is not None:
+            bg.bg_set_option(ctx, bg.BG_OPT_FLAG_TWIN, flag_twin)
+        if frame is not None:
+            bg.bg_set_option(ctx, bg.BG_OPT_FRAME, frame)
         if scratch_limit:
             bg.bg_set_option(ctx, bg.BG_OPT_SCRATCH_LIMIT, scratch_limit)
         if host:

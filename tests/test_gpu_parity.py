@@ -170,8 +170,9 @@ def test_config4_n9_full_size_sampled(bg, oracle, wl):
 
 
 def test_conditioning_flag_reports_and_options(bg, oracle, wl):
-    """BG_OPT_PRECISION = 2 bookkeeping: bg_last_refined counts the re-evaluated events; thresholds are options; the
-    diagnostics (3: Ward residual, 4: cancellation ratio) return the flag quantities; 0 switches the flag off."""
+    """BG_OPT_PRECISION = 2 bookkeeping: bg_last_twin / bg_last_refined count the events of the second (rotated-frame
+    FP64) and third (double-double) stage; thresholds are options; the diagnostics (3: Ward residual, 4: cancellation
+    ratio) return the flag quantities; 0 switches the flag off."""
     import torch
     ev = wl.config_events(1, N=30000)
     dev = torch.device("cuda:0")
@@ -185,16 +186,30 @@ def test_conditioning_flag_reports_and_options(bg, oracle, wl):
             bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, prec)
             bg.bg_eval(ctx, st, ev.N, *d, out)
             torch.cuda.synchronize()
-            res[prec] = (out.cpu().numpy(), bg.bg_last_refined(ctx)[0], bg.bg_last_launch_count(ctx))
-        assert 0 < res[2][1] < 0.15 * ev.N and res[0][1] == 0
-        assert res[2][2] > res[0][2]                       # the re-evaluation launches are counted
+            res[prec] = (out.cpu().numpy(), bg.bg_last_refined(ctx)[0], bg.bg_last_launch_count(ctx), bg.bg_last_twin(ctx))
+        n_dd, n_twin = res[2][1], res[2][3]
+        assert 0 < n_dd < n_twin < 0.2 * ev.N and res[0][1] == 0 and res[0][3] == 0
+        assert res[2][2] > res[0][2]                       # the launches of the later stages are counted
         ward, rho = res[3][0], res[4][0]
         assert np.all(ward >= 0) and np.all((rho > 0) & (rho <= 1.0 + 1e-12))
+        # the documented default rule for n = 6: Ward residual above 1e-14 -> second stage, above 5e-13 (or strong
+        # cancellation) -> double-double at once; what the second stage rejects joins those
+        hard = (ward > 5e-13 * (1 - 1e-9)) | (rho < 3e-3 * (1 + 1e-9))
+        soft = (ward > 1e-14 * (1 - 1e-9)) & ~hard
+        assert abs(int(soft.sum()) - n_twin) <= 2
+        assert hard.sum() - 2 <= n_dd <= hard.sum() + n_twin
         changed = res[2][0] != res[0][0]
-        flagged = (ward > 2e-14 * (1 - 1e-9)) | (rho < 3e-3 * (1 + 1e-9))   # the documented default rule for n = 6
-        assert np.all(flagged[changed]) and abs(int(flagged.sum()) - res[2][1]) <= 2
-        # a huge threshold and no cancellation test: nothing is re-evaluated, the bits equal the FP64 path
+        assert np.all((hard | soft)[changed]) and changed.sum() <= n_dd
+        # no second stage (its bound at or below the first threshold): every flagged event in double-double
         bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 2)
+        bg.bg_set_option(ctx, bg.BG_OPT_FLAG_TWIN, 1)
+        bg.bg_eval(ctx, st, ev.N, *d, out)
+        torch.cuda.synchronize()
+        assert bg.bg_last_twin(ctx) == 0 and abs(bg.bg_last_refined(ctx)[0] - int((hard | soft).sum())) <= 2   # (n = 6: both bounds 5e-13)
+        both = out.cpu().numpy()
+        assert np.all(rel_err(res[2][0], both) <= 1e-11)
+        # a huge threshold and no cancellation test: nothing is re-evaluated, the bits equal the FP64 path
+        bg.bg_set_option(ctx, bg.BG_OPT_FLAG_TWIN, 0)
         bg.bg_set_option(ctx, bg.BG_OPT_FLAG_THRESHOLD, 10 ** 17)
         bg.bg_set_option(ctx, bg.BG_OPT_FLAG_CANCELLATION, 1)
         bg.bg_eval(ctx, st, ev.N, *d, out)
@@ -204,13 +219,32 @@ def test_conditioning_flag_reports_and_options(bg, oracle, wl):
         bg.bg_destroy(ctx)
 
 
+@pytest.mark.parametrize("n,N", [(5, 4099), (6, 8195), (7, 2051), (9, 515), (11, 67)])
+def test_rotated_frame_gives_the_same_matrix_element(bg, oracle, wl, n, N):
+    """BG_OPT_FRAME = 1, the frame of the cascade's second stage: momenta rotated by a fixed rotation, polarisation
+    vectors of Eq. 3 built from the rotated momenta.  |M|^2 is Lorentz invariant: both evaluations meet the FP64 bar
+    against the oracle (which only knows the original frame) and agree with each other to FP64 round-off."""
+    ev = wl.config_events(4, N=N, n=n)
+    a, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, precision=0)
+    b, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, precision=0, frame=1)
+    assert name == "cdbg_prog_kernel"
+    assert np.any(a != b)                                  # it is another computation ...
+    err_a, tail_a = check_cdbg_fp64(oracle, ev, a)
+    err_b, tail_b = check_cdbg_fp64(oracle, ev, b)         # ... of the same number
+    assert np.median(rel_err(b, a)) < 1e-13
+    # default precision in the rotated frame (the second stage then runs in the original one): the 1e-11 bar
+    c, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, frame=1)
+    check_cdbg(oracle, ev, c)
+
+
 @pytest.mark.parametrize("n,N,lanes", [(6, 4099, 8), (7, 1029, 4), (8, 519, 64), (9, 259, 128), (10, 131, 256),
                                          (11, 67, 128), (12, 35, 256)])
 def test_flagged_reevaluation_other_lane_counts(bg, oracle, wl, n, N, lanes):
     """The double-double instantiation of the interpreter with other lane counts than the defaults (its state elements
     are 32 bytes: n >= 10 spills part of it to the L2 slab)."""
     ev = wl.config_events(4, N=N, n=n)
-    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, lanes=lanes, flag_threshold=1)     # tau = 1e-18: (almost) all events flagged
+    # tau = tau_twin = 1e-18: (almost) all events flagged, no second FP64 stage
+    got, name = gpu_eval(ev, bg.BG_CDBG_GIVEN, lanes=lanes, flag_threshold=1, flag_twin=1)
     assert name == "cdbg_prog_kernel"
     check_cdbg(oracle, ev, got)
 
@@ -480,7 +514,7 @@ def test_edge_cases(bg, oracle, wl):
         ev = wl.config_events(1, N=N)
         got, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
         check_cdbg(oracle, ev, got)
-        got, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, flag_threshold=1)      # every event through the re-evaluation
+        got, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, flag_threshold=1, flag_twin=1)      # every event through the re-evaluation
         check_cdbg(oracle, ev, got)
     # N = 0 is a no-op
     ctx = bg.bg_init(6, bg.BG_CDBG_GIVEN)
