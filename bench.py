@@ -82,6 +82,65 @@ def truth_sample_size(n: int, N: int) -> int:
     return min(N, {4: 16384, 5: 16384, 6: 16384, 7: 8192, 8: 4096, 9: 2048, 10: 512, 11: 192, 12: 64}[n])
 
 
+def measure_next_rows(bg, wl, dev, steps: int = 3):
+    """Sweep lines for the SURVEY 8(f) rows beside the BASELINE configs: events/s (device-resident inputs, FP64 kernels)
+    of the continuous colour / polarisation states (NEXT-1), the colour-ordered Monte Carlo of Eq. 19 (NEXT-2), the
+    leading-colour approximation of Eq. 33 (NEXT-3) and the no-allocation entry point, on small synthetic batches;
+    their parity tests are tests/test_gpu_parity.py and tests/test_zz_no_alloc.py."""
+    import torch
+    stream = torch.cuda.current_stream()
+    sh = stream.cuda_stream
+
+    def rate(call, N):
+        for _ in range(2):
+            call()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            call()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return {"events": N, "events_per_s": N * steps / (e0.elapsed_time(e1) * 1e-3)}
+
+    rows = {"continuous_states": {}, "co_mc": {}, "leading_colour_helgiven": {}, "no_alloc_entry_point": {}}
+    for n in range(4, 11):          # BG_CDBG_CONTINUOUS, real arithmetic
+        N = max(1 << 10, (1 << 17) >> (2 * (n - 4)))
+        mom = wl.rambo(n, N, seed=1, stream=900 + n)
+        phi, eta = wl.continuous_states(n, N, seed=1, stream=900 + n)
+        sphi, seta = wl.continuous_to_soa(phi, eta)
+        d = [torch.from_numpy(x).to(dev) for x in (wl.to_soa(mom=mom), sphi, seta)]
+        out = torch.empty(N, dtype=torch.float64, device=dev)
+        ctx = bg.bg_init(n, bg.BG_CDBG_CONTINUOUS)
+        try:
+            bg.bg_reserve(ctx, N)
+            rows["continuous_states"][str(n)] = rate(lambda: bg.bg_eval_continuous(ctx, sh, N, d[0], d[1], d[2], out), N)
+        finally:
+            bg.bg_destroy(ctx)
+    for mode, key, nmax in ((bg.BG_COMC_GIVEN, "co_mc", 8), (bg.BG_COBG_HELGIVEN_LC, "leading_colour_helgiven", 8)):
+        for n in range(4, nmax + 1):
+            N = max(1 << 10, (1 << 18) >> (2 * (n - 4)))
+            ev = wl.config_events(4, N=N, n=n)
+            d_mom = torch.from_numpy(wl.to_soa(mom=ev.mom)).to(dev)
+            d_hel = torch.from_numpy(wl.to_soa(hel=ev.hel)).to(dev)
+            d_col = torch.from_numpy(wl.to_soa(col=ev.col)).to(dev) if mode & bg.BG_COL_GIVEN else None
+            out = torch.empty(N, dtype=torch.float64, device=dev)
+            ctx = bg.bg_init(n, mode)
+            try:
+                bg.bg_reserve(ctx, N)
+                rows[key][str(n)] = rate(lambda: bg.bg_eval(ctx, sh, N, d_mom, d_hel, d_col, out), N)
+            finally:
+                bg.bg_destroy(ctx)
+    bg.bg_static_setup()
+    for n in (6, 8):                # bg_eval_static: thread-per-event kernel, scratch in the fixed device array
+        N = bg.bg_static_max_events(n)
+        ev = wl.config_events(4, N=N, n=n)
+        d = [torch.from_numpy(x).to(dev) for x in (wl.to_soa(mom=ev.mom), wl.to_soa(hel=ev.hel), wl.to_soa(col=ev.col))]
+        out = torch.empty(N, dtype=torch.float64, device=dev)
+        rows["no_alloc_entry_point"][str(n)] = rate(lambda: bg.bg_eval_static(sh, n, N, d[0], d[1], d[2], out), N)
+    return rows
+
+
 def measure_config(bg, wl, oracle_mod, dev, config: int, n: int, steps: int, peak_tf: float, with_cpu: bool):
     """Compact measurement of one BASELINE.json config on the current device (N = 1): events/s of the default path,
     the FP64-only path beside it, the FP64 kernel's roofline fraction, the conditioning flag's cost, the CPU oracle
@@ -587,6 +646,7 @@ def run_b200(args):
             cfgs["COBG_n8"] = measure_config(bg, wl, oracle_mod, dev, 2, 8, 3, peak_tf, with_cpu)
             cfgs["C5"] = {str(k): measure_config(bg, wl, oracle_mod, dev, 4, k, ksteps, peak_tf, with_cpu) for k in range(4, 13)}
             line["configs"] = cfgs
+            line["next_rows"] = measure_next_rows(bg, wl, dev)
         print(json.dumps(line), flush=True)
     bg.bg_destroy(ctx)
     if world > 1:

@@ -137,7 +137,8 @@ int bg_eval(bg_ctx* ctx, void* cuda_stream, long long N, const double* mom, cons
             const signed char* col, double* out);
 
 /*
- * BG_CDBG_CONTINUOUS (n <= 9): |A|^2 of the colour-helicity sub-amplitude of Eq. 14 for continuous
+ * BG_CDBG_CONTINUOUS (n <= 10: the state offsets of the single dense program are 16 bit; n = 10 keeps the top levels
+ * in the L2 slab): |A|^2 of the colour-helicity sub-amplitude of Eq. 14 for continuous
  * states - the colour-dressed recursion Eq. 28-32 with external currents  e(p_k, phi_k) x X_k,  e = cos(phi) e1 +
  * sin(phi) e2 (Eq. 7; e1, e2 the unit vectors of the gauge of reading g2) and X_k[h][g] = etabar_k[h] eta_k[g]
  * (Eq. 12 without its trace part, which decouples).  Summing/averaging over the states with the weights of Eq. 13

@@ -159,7 +159,7 @@ static bool mode_supported(int n, int mode) {
     if (mode == BG_COBG_HELSUM_FULLCOLOR || mode == BG_COBG_HELGIVEN_FULLCOLOR) return n <= 8;
     if (mode == BG_COBG_HELSUM_LC || mode == BG_COBG_HELGIVEN_LC) return bg::cobg_shared_supported(n);
     if (mode == BG_CDBG_GIVEN || mode == BG_CDBG_HELSUM_COLGIVEN) return true;
-    if (mode == BG_CDBG_CONTINUOUS) return n <= 9;
+    if (mode == BG_CDBG_CONTINUOUS) return n <= 10;   // 16-bit state offsets: 2^(n-1) subsets x 9 colour entries x 10 elements
     if (mode == BG_COMC_GIVEN) return n <= 8;   // (n-1)! orderings per class: the state offsets are 16 bit
     return false;
 }

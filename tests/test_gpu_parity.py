@@ -411,7 +411,7 @@ def test_double_double_reference_path_cobg(bg, oracle, wl, n, N):
 
 @pytest.mark.parametrize("arith", ["real", "complex"])
 @pytest.mark.parametrize("n,N,lanes", [(4, 300, None), (5, 200, None), (6, 150, None), (6, 33, 32), (6, 33, 256),
-                                         (7, 40, None), (8, 9, 256), (9, 3, None)])
+                                         (7, 40, None), (8, 9, 256), (9, 3, None), (10, 2, None)])
 def test_continuous_colour_and_polarisation_states(bg, oracle, wl, n, N, lanes, arith):
     """SURVEY NEXT-1 (the paper's CD_MC sampling, Eq. 5-14): colour-dressed recursion with a real polarisation e(phi)
     and a full 3x3 colour matrix etabar x eta per gluon, against the oracle's general-state recursion."""
