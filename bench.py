@@ -55,7 +55,7 @@ def parse_args():
                     help="CDBG configs with continuous colour / polarisation states (Eq. 5-14, SURVEY NEXT-1)")
     ap.add_argument("--lc", action="store_true", help="configs 0 / 2 in leading-colour mode (Eq. 33, SURVEY NEXT-3)")
     ap.add_argument("--comc", action="store_true",
-                    help="colour-dressed configs through BG_COMC_GIVEN (Eq. 19 with colour-ordered currents, SURVEY NEXT-2; n <= 8)")
+                    help="colour-dressed configs through BG_COMC_GIVEN (Eq. 19 with colour-ordered currents, SURVEY NEXT-2; n <= 9)")
     ap.add_argument("--precision", type=int, default=None, help="BG_OPT_PRECISION (1 = double-double reference path)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -117,7 +117,7 @@ def measure_next_rows(bg, wl, dev, steps: int = 3):
             rows["continuous_states"][str(n)] = rate(lambda: bg.bg_eval_continuous(ctx, sh, N, d[0], d[1], d[2], out), N)
         finally:
             bg.bg_destroy(ctx)
-    for mode, key, nmax in ((bg.BG_COMC_GIVEN, "co_mc", 8), (bg.BG_COBG_HELGIVEN_LC, "leading_colour_helgiven", 8)):
+    for mode, key, nmax in ((bg.BG_COMC_GIVEN, "co_mc", 9), (bg.BG_COBG_HELGIVEN_LC, "leading_colour_helgiven", 8)):
         for n in range(4, nmax + 1):
             N = max(1 << 10, (1 << 18) >> (2 * (n - 4)))
             ev = wl.config_events(4, N=N, n=n)

@@ -59,7 +59,7 @@ enum {
     BG_CDBG_HELSUM_COLGIVEN = BG_REC_CDBG | BG_HEL_SUM | BG_COL_GIVEN,
     BG_CDBG_CONTINUOUS = BG_REC_CDBG | BG_HEL_CONT | BG_COL_CONT,          /* the paper's CD_MC sampling */
     BG_COMC_GIVEN = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_GIVEN,            /* Eq. 19 with colour-ordered
-                                                                              currents, sampled colour flows (n <= 8) */
+                                                                              currents, sampled colour flows (n <= 9) */
     BG_COBG_HELSUM_LC = BG_REC_COBG | BG_HEL_SUM | BG_COL_LC,
     BG_COBG_HELGIVEN_LC = BG_REC_COBG | BG_HEL_GIVEN | BG_COL_LC
 };
@@ -206,10 +206,13 @@ int bg_class_program_stats(int n, int lanes, const int* counts, long long* stats
 
 /*
  * The same for the BG_COMC_GIVEN programs (Eq. 19, evaluated with the colour-ordered currents
- * of Eq. 20-26; 4 <= n <= 8).  stats[0] = 1 if at least one ordering sigma has all its Kronecker deltas equal
+ * of Eq. 20-26; 4 <= n <= 9).  stats[0] = 1 if at least one ordering sigma has all its Kronecker deltas equal
  * to one, stats[1] = vertex evaluations per event (shared between orderings: a sub-sequence current is computed
  * once), stats[2] = interpreter steps, stats[3] = bytes of per-event state, stats[4] = number of such orderings
- * (of (n-1)! with the first gluon fixed).  BG_EINVAL for bad arguments.
+ * (of (n-1)! with the first gluon fixed).  BG_EINVAL for bad arguments; BG_EUNSUPPORTED for a class with more than
+ * 20000 orderings.  (bg_init builds a CO_MC program only where its state fits the 16-bit state offsets - every class
+ * for n <= 8; at n = 9 classes with thousands of orderings, 1e-3 of the classes of uniformly drawn colours, are
+ * evaluated with their colour-dressed program instead: the same number.)
  */
 int bg_comc_program_stats(int n, int lanes, const int* counts, long long* stats);
 

@@ -160,7 +160,7 @@ static bool mode_supported(int n, int mode) {
     if (mode == BG_COBG_HELSUM_LC || mode == BG_COBG_HELGIVEN_LC) return bg::cobg_shared_supported(n);
     if (mode == BG_CDBG_GIVEN || mode == BG_CDBG_HELSUM_COLGIVEN) return true;
     if (mode == BG_CDBG_CONTINUOUS) return n <= 10;   // 16-bit state offsets: 2^(n-1) subsets x 9 colour entries x 10 elements
-    if (mode == BG_COMC_GIVEN) return n <= 8;   // (n-1)! orderings per class: the state offsets are 16 bit
+    if (mode == BG_COMC_GIVEN) return n <= 9;   // (n = 9: classes with thousands of orderings fall back to the dressed program)
     return false;
 }
 
@@ -488,7 +488,7 @@ int bg_class_program_stats(int n, int lanes, const int* counts, long long* stats
 }
 
 int bg_comc_program_stats(int n, int lanes, const int* counts, long long* stats) {
-    if (n < 4 || n > 8 || !counts || !stats || lanes < 1 || lanes > 256 || (lanes & (lanes - 1))) return BG_EINVAL;
+    if (n < 4 || n > 9 || !counts || !stats || lanes < 1 || lanes > 256 || (lanes & (lanes - 1))) return BG_EINVAL;
     int sum = 0, code[bg::kMaxN];
     for (int c = 0; c < bg::kNumCodes; c++) {
         if (counts[c] < 0 || sum + counts[c] > n) return BG_EINVAL;

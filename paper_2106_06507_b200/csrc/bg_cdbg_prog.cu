@@ -393,7 +393,8 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
             if (class_rank(n, all[r].data()) != r) return BG_EINVAL;
         std::vector<ClassProgram> progs(nc);
         std::atomic<long long> next_class{0};
-        std::atomic<bool> overflow{false};   // CO_MC: a class with too many orderings for the 16-bit state offsets
+        std::atomic<bool> overflow{false};   // a class whose state does not fit the 16-bit state offsets
+        std::atomic<long long> dressed_fallbacks{0};
         auto worker = [&]() {
             for (long long r = next_class.fetch_add(1); r < nc; r = next_class.fetch_add(1))
                 if (!comc) {
@@ -411,8 +412,16 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
                     int code[kMaxN], k = 0;
                     for (int t = 0; t < kNumCodes; t++)
                         for (int q = 0; q < cnt[t]; q++) code[k++] = t;
-                    build_comc_program(n, G, code, progs[r]);
-                    if (progs[r].state_cx < 0 || progs[r].state_cx > 65535) overflow = true;
+                    // A class whose shared sequence currents do not fit the 16-bit state offsets (more than a few
+                    // thousand colour-connected orderings: 1e-3 of the classes a uniform colour draw hits at n = 9, none
+                    // for n <= 8) is evaluated with its colour-dressed program instead - the same number (Eq. 19 is
+                    // what Eq. 28-32 compute), same records, same interpreter.
+                    build_comc_program(n, G, code, progs[r], 6000);
+                    if (progs[r].state_cx < 0 || progs[r].state_cx > 65535) {
+                        build_class(n, G, cnt, progs[r]);
+                        if (progs[r].state_cx < 0 || progs[r].state_cx > 65535) overflow = true;
+                        dressed_fallbacks++;
+                    }
                 }
         };
         unsigned nthreads = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));

@@ -455,7 +455,7 @@ def test_continuous_colour_and_polarisation_states(bg, oracle, wl, n, N, lanes, 
         assert np.all(err[tail] <= 10 * floor), (err[tail], floor)
 
 
-@pytest.mark.parametrize("n,N", [(4, 500), (5, 700), (6, 2051), (7, 1031), (8, 259)])
+@pytest.mark.parametrize("n,N", [(4, 500), (5, 700), (6, 2051), (7, 1031), (8, 259), (9, 131)])
 def test_colour_ordered_monte_carlo_mode(bg, oracle, wl, n, N):
     """CO_MC: Eq. 19 summed over the colour-connected orderings with colour-ordered currents, on
     the device.  Truth = the colour-dressed oracle in long double (a different algorithm for the same number);
@@ -489,8 +489,31 @@ def test_colour_ordered_monte_carlo_mode(bg, oracle, wl, n, N):
 
 def test_colour_ordered_monte_carlo_rejects_large_n(bg):
     with pytest.raises(bg.BgError) as e:
-        bg.bg_init(9, bg.BG_COMC_GIVEN)
+        bg.bg_init(10, bg.BG_COMC_GIVEN)
     assert e.value.code == bg.BG_EUNSUPPORTED
+
+
+def test_colour_ordered_monte_carlo_heavy_classes_at_n9(bg, oracle, wl):
+    """n = 9: a class with thousands of colour-connected orderings does not fit the 16-bit state offsets of the CO_MC
+    programs and is evaluated with its colour-dressed program (same number by Eq. 19).  Seven gluons in the U(1)-like
+    state (1,1) between one (1,2) and one (2,1): 7! x 8 orderings."""
+    n, N = 9, 24
+    ev = wl.config_events(4, N=N, n=n)
+    col = np.ones((N, n, 2), dtype=np.int8)
+    rng = np.random.default_rng(5)
+    for e in range(N):
+        a, b = rng.choice(n, size=2, replace=False)
+        col[e, a] = (1, 2)
+        col[e, b] = (2, 1)
+    ev = wl.Events(n, ev.mom, ev.hel, col, "heavy CO_MC classes")
+    try:
+        stats = bg.bg_comc_program_stats(n, 128, np.bincount((col[0, :, 0] - 1) * 3 + col[0, :, 1] - 1, minlength=9))
+        assert stats[3] // 16 > 65535 and stats[4] >= 5040     # a CO_MC program too large for the 16-bit offsets ...
+    except bg.BgError as e:
+        assert e.code == bg.BG_EUNSUPPORTED
+    got, name = gpu_eval(ev, bg.BG_COMC_GIVEN)                 # ... but a result
+    assert name == "cdbg_prog_kernel"
+    check_cdbg_fp64(oracle, ev, got, max_tail_frac=0.2)
 
 
 @pytest.mark.parametrize("n,N", [(4, 60), (5, 40), (6, 24)])
