@@ -5,6 +5,8 @@
 // See bg_cdbg_prog.cu for the pipeline of one bg_eval and the state layout.
 #pragma once
 #include <algorithm>
+#include <cstdio>
+#include <cstdlib>
 
 #include "bg_internal.h"
 #include "bg_math.cuh"
@@ -118,6 +120,11 @@ struct ProgParams {
     // Cascade: events whose Ward residual exceeds tau but not tau_twin are first evaluated once more in FP64
     // in a rotated frame (same value, independent round-off); they go on to the double-double list only if the two
     // results differ by more than tau_twin or the second evaluation's own flag quantities exceed tau_twin / tau_rho.
+    // UNSORTED instantiations (n <= 5: the prepass is more than half of a step there): no records - a lane group
+    // classifies its event itself and reads the caller's arrays; tasks in input order, one tier
+    const double* mom;         // [n][4][N]
+    const signed char* hel;    // [n][N]
+    const signed char* col;    // [n][2][N]
     int merged;                // 1: the launch serves tiers tier .. kTiers - 1 one after the other (list launches)
     int twin;                  // bit 0: evaluate in the rotated frame (rotate_frame); bit 1: second stage - compare with
                                // out[e] and append to flag_list on disagreement instead of writing out[e]
@@ -269,7 +276,74 @@ __device__ __forceinline__ EventHeader ld_header(const char* h) {
     return r;
 }
 
-template <int G, bool SPILL, class S>
+// What the prepass computes for one event, for the UNSORTED instantiations: the class of the colour assignment (rank of
+// the multiset of colour codes, as class_rank / cdbg_classify_kernel), the canonical order (codes ascending, original
+// order inside a code, the last gluon with the class's closure code at the end: nibble k of perm = original index of
+// canonical gluon k) and the helicity bits 48 + k of the canonical gluons.
+static __constant__ unsigned c_multisets[kMaxN + 1][kNumCodes] = {   // c_multisets[r][t] = multisets of size r from t kinds, C(r + t - 1, r)
+    {1, 1, 1, 1, 1, 1, 1, 1, 1},
+    {0, 1, 2, 3, 4, 5, 6, 7, 8},
+    {0, 1, 3, 6, 10, 15, 21, 28, 36},
+    {0, 1, 4, 10, 20, 35, 56, 84, 120},
+    {0, 1, 5, 15, 35, 70, 126, 210, 330},
+    {0, 1, 6, 21, 56, 126, 252, 462, 792},
+    {0, 1, 7, 28, 84, 210, 462, 924, 1716},
+    {0, 1, 8, 36, 120, 330, 792, 1716, 3432},
+    {0, 1, 9, 45, 165, 495, 1287, 3003, 6435},
+    {0, 1, 10, 55, 220, 715, 2002, 5005, 11440},
+    {0, 1, 11, 66, 286, 1001, 3003, 8008, 19448},
+    {0, 1, 12, 78, 364, 1365, 4368, 12376, 31824},
+    {0, 1, 13, 91, 455, 1820, 6188, 18564, 50388}};
+__device__ __forceinline__ EventHeader classify_event(const ProgParams& p, long long e) {
+    const int n = p.n;
+    EventHeader h;
+    h.event = (uint32_t)e; h.cls = 0xFFFFFFFFu; h.perm = 0;
+    int cnt[kNumCodes];
+#pragma unroll
+    for (int c = 0; c < kNumCodes; c++) cnt[c] = 0;
+    bool ok = true;
+    uint64_t cw = 0;
+    for (int k = 0; k < n; k++) {
+        const int i = p.col[(size_t)(2 * k) * p.N + e] - 1, jj = p.col[(size_t)(2 * k + 1) * p.N + e] - 1;
+        ok = ok && i >= 0 && i < 3 && jj >= 0 && jj < 3;
+        const int code = ok ? 3 * i + jj : 0;
+        cw |= (uint64_t)code << (4 * k);
+#pragma unroll
+        for (int c = 0; c < kNumCodes; c++) cnt[c] += code == c;
+    }
+    if (!ok) return h;
+    unsigned rank = 0;
+    int r = n;
+#pragma unroll
+    for (int t = 0; t < kNumCodes - 1; t++) {
+        for (int c = 0; c < cnt[t]; c++) rank += c_multisets[r - c][kNumCodes - 1 - t];
+        r -= cnt[t];
+    }
+    const uint4 ci = __ldg(reinterpret_cast<const uint4*>(p.info + rank));
+    h.cls = rank;
+    if (!((ci.y >> 24) & 0xFF)) return h;          // the amplitude of this class vanishes identically
+    const int closure = (int)((ci.y >> 16) & 0xFF);
+    int lastk = 0;
+    for (int k = 0; k < n; k++)
+        if ((int)((cw >> (4 * k)) & 0xF) == closure) lastk = k;
+    uint64_t start = 0, pm = 0;
+    int before = 0;
+#pragma unroll
+    for (int c = 0; c < kNumCodes; c++) {
+        start |= (uint64_t)before << (4 * c);
+        before += cnt[c] - (c == closure ? 1 : 0);
+    }
+    for (int k = 0; k < n; k++) {
+        const int at = k == lastk ? n - 1 : (int)((start >> (4 * (int)((cw >> (4 * k)) & 0xF))) & 0xF);
+        if (k != lastk) start += 1ull << (4 * (int)((cw >> (4 * k)) & 0xF));
+        pm |= (uint64_t)k << (4 * at);
+        if (p.hel[(size_t)k * p.N + e] > 0) pm |= 1ull << (48 + at);
+    }
+    h.perm = pm;
+    return h;
+}
+
+template <int G, bool SPILL, class S, bool UNSORTED = false>
 __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgParams p) {
     // G <= 32: one warp per block, EPW = 32/G events per warp.  G > 32: one event per block of G threads.
     // S: complex currents (cx) or, for continuous states with real polarisations, real ones (double).
@@ -297,14 +371,20 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
     const int tier_end = p.merged ? kTiers : p.tier + 1;
     for (int tier = p.tier; tier < tier_end; tier++) {
         // tasks: the records of the tier, or (re-evaluation) the record positions in the tier's flag list
-        const long long first = p.bounds[tier], end = p.list ? first + p.list_count[tier] : (long long)p.bounds[tier + 1];
+        const long long first = UNSORTED ? 0 : (long long)p.bounds[tier];
+        const long long end = p.list ? first + p.list_count[tier] : (UNSORTED ? p.N : (long long)p.bounds[tier + 1]);
         const long long ntasks = (end - first + EPW - 1) / EPW;
         auto rec_pos = [&](long long i) -> long long { return p.list ? (long long)__ldg(p.list + i) : i; };
+        // the header of the event at record position pos (UNSORTED: of event pos, worked out here)
+        auto get_header = [&](long long pos) -> EventHeader {
+            if constexpr (UNSORTED) return classify_event(p, pos);
+            else return ld_header(p.rec + (size_t)pos * p.rec_bytes);
+        };
         const int n = p.n;
         // lanes of one event (same q) run the same program and meet at its barriers; events of different classes in
         // one warp pass different numbers of barriers, so the barrier names only the event's own lanes
         unsigned evmask = 0;
-    #pragma unroll
+#pragma unroll
         for (int i = 0; i < (G < 32 ? G : 32); i++) evmask |= 1u << (q + i * EPW);
 
         // the header of a task is loaded one task ahead; the inputs of the next task are prefetched into L2 while
@@ -334,7 +414,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
             const long long idx = first + task * EPW + q;
             if (idx < end) {
                 pos_next = rec_pos(idx);
-                hnext = ld_header(p.rec + (size_t)pos_next * p.rec_bytes);
+                hnext = get_header(pos_next);
             }
         }
         // carried from one task to the next: the class info of the next event, requested at the first barrier of the
@@ -353,26 +433,36 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                 idx_next = idx2;
                 if (task_next < ntasks && idx2 < end) {
                     if (p.list) idx_next = pos_next = rec_pos(idx2);
-                    hnext = ld_header(p.rec + (size_t)idx_next * p.rec_bytes);
+                    hnext = get_header(idx_next);
                 }
             }
             const long long e = h.event;
             const uint32_t cls = have ? h.cls : 0xFFFFFFFFu;
-            const double* mrec = reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
+            const double* mrec = UNSORTED ? nullptr
+                                          : reinterpret_cast<const double*>(p.rec + (size_t)(have ? idx : first) * p.rec_bytes + kRecHeaderBytes);
+            const uint64_t perm = h.perm;
+            // component c of the momentum of canonical gluon k: from the record, or (UNSORTED) from the caller's array
+            auto ldm = [&](int k, int c) -> double {
+                if constexpr (UNSORTED) {
+                    const int orig = (int)((perm >> (4 * k)) & 0xF);
+                    return __ldg(p.mom + (size_t)(orig * 4 + c) * p.N + (have ? e : 0));
+                } else {
+                    return __ldcg(mrec + k * p.rec_gstride + c);
+                }
+            };
             // discrete states: the setup level gives gluon k to lane k % G, so the lane's first momentum is requested
             // here, ahead of the dependent loads class info -> ops that the setup ops themselves wait for
             const bool discrete = !kUseRing && p.rec_gstride == 4 && kComplex;   // (G >= 8: measured 1-2 % slower)
             double pk[4] = {0.0, 0.0, 0.0, 0.0};
             if (discrete && g < n) {
-    #pragma unroll
-                for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + g * 4 + c);
+#pragma unroll
+                for (int c = 0; c < 4; c++) pk[c] = ldm(g, c);
                 if constexpr (kTwinOk) { if (p.twin & 1) rotate_frame(pk); }
             }
             uint4 ci = ci_next;
             if (!ci_next_ok) ci = __ldg(reinterpret_cast<const uint4*>(p.info + (cls == 0xFFFFFFFFu ? 0 : cls)));
             ci_next_ok = false;
             const bool valid = cls != 0xFFFFFFFFu && ((ci.y >> 24) & 0xFF);
-            const uint64_t perm = h.perm;
             const ProgOp* ops = p.ops + ci.x + g;
             const int total = valid ? (int)ci.z : 0;
             bool prefetched = false;
@@ -382,9 +472,9 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
             double asum = 0.0;        // sum of |Re| + |Im| of the closure contributions that add up to the amplitude
             S acc[4], tacc[6];
             R Pt[4];
-    #pragma unroll
+#pragma unroll
             for (int c = 0; c < 4; c++) { acc[c] = s_zero<S>(); Pt[c] = r_from(0.0, R()); }
-    #pragma unroll
+#pragma unroll
             for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
 
             // The lane's ops travel global -> shared by cp.async, kRing - 1 steps ahead, into a private ring (no
@@ -395,8 +485,9 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                 prefetched = true;
                 if (hnext.cls != 0xFFFFFFFFu) {
                     // the next event's record (a few 128-byte lines) is pulled into L2 meanwhile
-                    for (int k = g * 128; k < p.rec_bytes; k += G * 128)
-                        asm volatile("prefetch.global.L2 [%0];" ::"l"(p.rec + (size_t)idx_next * p.rec_bytes + k));
+                    if constexpr (!UNSORTED)
+                        for (int k = g * 128; k < p.rec_bytes; k += G * 128)
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(p.rec + (size_t)idx_next * p.rec_bytes + k));
                     if constexpr (kUseRing) {      // (G <= 4: measured neutral to slightly slower)
                         ci_next = __ldg(reinterpret_cast<const uint4*>(p.info + hnext.cls));
                         ci_next_ok = true;
@@ -418,12 +509,12 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                 if constexpr (StateElem<S>::kDD) {
                     if (kk == kstar) {
                         R Pe[4];
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 4; c++) Pe[c] = r_from(0.0, R());
                         for (int j = 0; j < n; j++) {
                             if (j == kk) continue;
-    #pragma unroll
-                            for (int c = 0; c < 4; c++) Pe[c] = r_sub(Pe[c], r_from(__ldcg(mrec + j * p.rec_gstride + c), R()));
+#pragma unroll
+                            for (int c = 0; c < 4; c++) Pe[c] = r_sub(Pe[c], r_from(ldm(j, c), R()));
                         }
                         st_.stP(offPt, Pe);
                         return;
@@ -435,7 +526,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
             uint4 r0 = make_uint4(0, 0, 0, 0), r1 = r0;
             if constexpr (kUseRing) {
                 if (total > 0) {
-    #pragma unroll
+#pragma unroll
                     for (int i = 0; i < kRing - 1; i++) {
                         cp_async16(ring + ((s0 + i) % kRing) * kBlock, ops + (size_t)(s0 + i) * G);
                         asm volatile("cp.async.commit_group;" ::: "memory");
@@ -457,25 +548,25 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     const int kn = k + G;
                     double pn[4] = {0.0, 0.0, 0.0, 0.0};
                     if (kn < n) {
-    #pragma unroll
-                        for (int c = 0; c < 4; c++) pn[c] = __ldcg(mrec + kn * 4 + c);
+#pragma unroll
+                        for (int c = 0; c < 4; c++) pn[c] = ldm(kn, c);
                         if constexpr (kTwinOk) { if (p.twin & 1) rotate_frame(pn); }
                     }
                     if ((raw.z >> 16) & OPF_EXT) {
                         const int kk = (int)raw.w;
                         if (kk != k) {      // another dealing of the gluons than k % G: fetch what the op names
-    #pragma unroll
-                            for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + kk * 4 + c);
+#pragma unroll
+                            for (int c = 0; c < 4; c++) pk[c] = ldm(kk, c);
                             if constexpr (kTwinOk) { if (p.twin & 1) rotate_frame(pk); }
                         }
                         S eps[4];
                         ext_current(pk, ((perm >> (48 + kk)) & 1) ? 1 : -1, eps);
                         const int offDst = raw.y >> 16, offPt = raw.z & 0xFFFF;
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
                         if (offPt != 0xFFFF) store_ext_momentum(kk, offPt, pk);
                     }
-    #pragma unroll
+#pragma unroll
                     for (int c = 0; c < 4; c++) pk[c] = pn[c];
                     k = kn;
                 }
@@ -509,52 +600,52 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     const unsigned flags = raw.z >> 16;
                     if (flags & OPF_VALID) {
                         S a[4], b[4];
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); b[c] = st_.ld(offB + c); }
                         R P1[4], P2[4];
                         st_.ldP(offP1, P1);
                         if (flags & OPF_FIRST) {
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 4; c++) acc[c] = s_zero<S>();
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 6; c++) tacc[c] = s_zero<S>();
                             const int offP2 = (int)(raw.w & 0xFFFF);
                             R Pb[4];
                             st_.ldP(offP2, Pb);
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 4; c++) Pt[c] = r_add(P1[c], Pb[c]);
                         }
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 4; c++) P2[c] = r_sub(Pt[c], P1[c]);
                         // X(a,b) is linear in the pair (a, T_a): a negative vertex flips the sign bits of that pair
                         // (integer pipe) instead of multiplying every term by -1 on the FP64 pipe
                         const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
                         v3_acc(acc, P1, P2, a, b, 1.0);
                         if (flags & OPF_TENB) {
                             S T[6];
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 6; c++) T[c] = st_.ld(offB + 4 + c);
                             tcontract_acc(acc, T, a, 1.0);
                         }
                         if (flags & OPF_TENA) {
                             S T[6];
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 6; c++) T[c] = cneg(st_.ld(offA + 4 + c), neg);
                             tcontract_acc(acc, T, b, -1.0);
                         }
                         if (!(flags & OPF_CLOSURE)) tbuild_acc(tacc, a, b, 1.0);
                         if (flags & OPF_PARTIAL) {
                             // chunk of a split target: raw sums to its scratch slot, finished by a COMBINE op
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
                         } else if (flags & OPF_LAST) {
                             if (flags & OPF_CLOSURE) {
                                 S en[4];
-    #pragma unroll
+#pragma unroll
                                 for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
                                 const S term = s_isqrt2(mdot(en, acc));
                                 amp = amp + term;
@@ -565,14 +656,14 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                                 }
                             } else {
                                 const R f = r_isqrt2_over(mdot(Pt, Pt));
-    #pragma unroll
+#pragma unroll
                                 for (int c = 0; c < 4; c++) acc[c] = s_scale(f, acc[c]);
-    #pragma unroll
+#pragma unroll
                                 for (int c = 0; c < 6; c++) tacc[c] = s_isqrt2(tacc[c]);
                                 if (!(flags & OPF_NOSTORE)) {
-    #pragma unroll
+#pragma unroll
                                     for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
-    #pragma unroll
+#pragma unroll
                                     for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
                                 }
                                 if (flags & OPF_STOREP) {
@@ -584,35 +675,35 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                         // closure vertex X(eps_k, J(pi)) . eps_n with J(pi), T(pi) still in acc / tacc, P(pi) in Pt
                         S a[4], x[4], en[4];
                         R P1[4];
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 4; c++) { a[c] = st_.ld(offA + c); x[c] = s_zero<S>(); }
                         st_.ldP(offP1, P1);
                         const int neg = (flags & OPF_NEG) ? (int)0x80000000 : 0;
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 4; c++) a[c] = cneg(a[c], neg);
                         v3_acc(x, P1, Pt, a, acc, 1.0);
                         tcontract_acc(x, tacc, a, 1.0);
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 4; c++) en[c] = st_.ld(offDst + c);
                         const S term = s_isqrt2(mdot(en, x));
                         amp = amp + term;
                         if constexpr (kComplex && !StateElem<S>::kDD) {
                             double Pf[4];
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 4; c++) Pf[c] = P1[c] + Pt[c];
                             wamp = wamp + mdot(Pf, x);
                             asum += fabs(term.re) + fabs(term.im);
                         }
                     } else if (flags & OPF_COMBINE) {
                         // add the offB partial sums of a split target and finish it like a LAST op
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 4; c++) acc[c] = st_.ld(offA + c);
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 6; c++) tacc[c] = st_.ld(offA + 4 + c);
                         for (int r = 1; r < offB; r++) {
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 4; c++) acc[c] = acc[c] + st_.ld(offA + 10 * r + c);
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 6; c++) tacc[c] = tacc[c] + st_.ld(offA + 10 * r + 4 + c);
                         }
                         {
@@ -620,18 +711,18 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                             R Pa[4], Pb[4];
                             st_.ldP(offP1, Pa);
                             st_.ldP(offP2, Pb);
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 4; c++) Pt[c] = r_add(Pa[c], Pb[c]);
                         }
                         const R f = r_isqrt2_over(mdot(Pt, Pt));
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 4; c++) acc[c] = s_scale(f, acc[c]);
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 6; c++) tacc[c] = s_isqrt2(tacc[c]);
                         if (!(flags & OPF_NOSTORE)) {
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 4; c++) st_.st(offDst + c, acc[c]);
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 6; c++) st_.st(offDst + 4 + c, tacc[c]);
                         }
                         if (flags & OPF_STOREP) {
@@ -643,20 +734,20 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                         const int k = (int)raw.w;
                         const double* gr = mrec + k * p.rec_gstride;
                         double pk[4], ev[4], eta[3], etab[3];
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 4; c++) pk[c] = __ldcg(gr + c);
                         const double phi = __ldcg(gr + 4);
-    #pragma unroll
+#pragma unroll
                         for (int c = 0; c < 3; c++) { eta[c] = __ldcg(gr + 5 + c); etab[c] = __ldcg(gr + 8 + c); }
                         polarisation_real(pk, phi, ev);
                         const bool closure_leg = offPt == 0xFFFF;   // gluon n: no momentum slot; target (h,g) reads X_n[g][h]
-    #pragma unroll
+#pragma unroll
                         for (int h = 0; h < 3; h++)
-    #pragma unroll
+#pragma unroll
                             for (int gg = 0; gg < 3; gg++) {
                                 const double x = etab[h] * eta[gg];
                                 const int at = offDst + 4 * (h * 3 + gg);
-    #pragma unroll
+#pragma unroll
                                 for (int c = 0; c < 4; c++) st_.st(at + c, s_real<S>(x * ev[c]));
                             }
                         if (!closure_leg) {
@@ -665,13 +756,13 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                     } else if ((flags & OPF_EXT) && kComplex) {
                         const int k = (int)raw.w;
                         double pk[4];
-    #pragma unroll
-                        for (int c = 0; c < 4; c++) pk[c] = __ldcg(mrec + k * p.rec_gstride + c);   // not through L1: it is kept for the ops
+#pragma unroll
+                        for (int c = 0; c < 4; c++) pk[c] = ldm(k, c);   // (records: not through L1, which is kept for the ops)
                         if constexpr (kTwinOk) { if (p.twin & 1) rotate_frame(pk); }
                         if constexpr (kComplex) {
                             S eps[4];
                             ext_current(pk, ((perm >> (48 + k)) & 1) ? 1 : -1, eps);
-    #pragma unroll
+#pragma unroll
                             for (int c = 0; c < 4; c++) st_.st(offDst + c, eps[c]);
                         }
                         if (offPt != 0xFFFF) store_ext_momentum(k, offPt, pk);
@@ -696,7 +787,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
             // closure amplitude: sum of the G lanes' partial contractions (Eq. 22), then |A|^2
             constexpr bool kWard = kComplex && !StateElem<S>::kDD;
             const bool flagging = kWard && p.tau2 > 0.0;
-    #pragma unroll
+#pragma unroll
             for (int d = EPW; d < 32; d <<= 1) {
                 amp = amp + shfl_xor(amp, d);
                 if constexpr (kWard) { wamp = wamp + shfl_xor(wamp, d); asum += shfl_xor(asum, d); }
@@ -730,14 +821,14 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                 if constexpr (kWard) {
                     if (p.tau2 < 0.0 && valid) {
                         // diagnostic (BG_OPT_PRECISION = 3): the Ward residual itself instead of |A|^2
-                        const double En = __ldcg(mrec + (n - 1) * p.rec_gstride);
+                        const double En = ldm(n - 1, 0);
                         p.out[e] = p.tau2 < -1.5 ? (fabs(amp.re) + fabs(amp.im)) / asum : ::sqrt(0.5 * s_norm2(wamp) / (En * En * w));
                     }
                     if (flagging && valid) {
                         // |sqrt2 p_n . J|^2 / 2 > tau^2 E_n^2 |A|^2, or |A| < tau_rho sum |closure terms| (the Ward residual does
                         // not see round-off that respects gauge invariance; strong cancellation at the top amplifies
                         // any), or a result that is not a positive finite number: not trusted as it stands
-                        const double En = __ldcg(mrec + (n - 1) * p.rec_gstride);
+                        const double En = ldm(n - 1, 0);
                         const double ward2 = 0.5 * s_norm2(wamp), scale = En * En * w;
                         const bool hard = !(ward2 <= fmax(p.tw2, p.tau2) * scale) ||
                                           !(fabs(amp.re) + fabs(amp.im) >= p.tau_rho * asum) || !(w > 0.0);
@@ -767,7 +858,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
 }
 
 // set the dynamic shared-memory limit of one instantiation (once per device); returns its static shared memory
-template <int G, bool SPILL, class S>
+template <int G, bool SPILL, class S, bool UNSORTED = false>
 static cudaError_t configure_interp(size_t* static_smem_out) {
     constexpr int BLOCK = G > 32 ? G : 32;
     static int configured_device = -1;   // the attribute is per device
@@ -775,11 +866,11 @@ static cudaError_t configure_interp(size_t* static_smem_out) {
     int device = 0;
     cudaGetDevice(&device);
     if (configured_device != device) {
-        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL, S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(cdbg_prog_kernel<G, SPILL, S, UNSORTED>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)(kMaxSlabBytes + (size_t)kRing * BLOCK * 16));
         if (e != cudaSuccess) return e;
         cudaFuncAttributes fa;
-        if ((e = cudaFuncGetAttributes(&fa, cdbg_prog_kernel<G, SPILL, S>)) != cudaSuccess) return e;
+        if ((e = cudaFuncGetAttributes(&fa, cdbg_prog_kernel<G, SPILL, S, UNSORTED>)) != cudaSuccess) return e;
         static_smem = fa.sharedSizeBytes;
         configured_device = device;
     }
@@ -787,8 +878,23 @@ static cudaError_t configure_interp(size_t* static_smem_out) {
     return cudaSuccess;
 }
 
+// resident blocks per SM of one instantiation at a dynamic shared-memory size, as the runtime's occupancy calculator
+// sees it (registers, allocation granularity of shared memory, the per-block reservation): a grid sized for one block
+// more than fits runs a second, nearly empty wave
+template <int G, bool SPILL, class S, bool UNSORTED = false>
+static int interp_blocks_per_sm(size_t smem) {
+    constexpr int BLOCK = G > 32 ? G : 32;
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, cdbg_prog_kernel<G, SPILL, S, UNSORTED>, BLOCK, smem) != cudaSuccess) {
+        cudaGetLastError();
+        nb = 1;
+    }
+    return std::max(1, nb);
+}
+
 // SPILL: every tier runs the spill kernel.  HYBRID (with SPILL = false): shape.hybrid picks it per tier.
-template <int G, bool SPILL, class S = cx, bool HYBRID = false>
+// UNSORTED: the instantiations that read the caller's arrays (one tier, merged launch shape).
+template <int G, bool SPILL, class S = cx, bool HYBRID = false, bool UNSORTED = false>
 static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_count, ProgParams p, int* launched,
                                  const LaunchShape& shape) {
     static_assert(!(SPILL && HYBRID), "HYBRID chooses between the two kernels itself");
@@ -799,9 +905,9 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
     size_t static_direct = 0, static_spill = 0;
     cudaError_t cerr;
     if constexpr (kHasDirect)
-        if ((cerr = configure_interp<G, false, S>(&static_direct)) != cudaSuccess) return cerr;
+        if ((cerr = configure_interp<G, false, S, UNSORTED>(&static_direct)) != cudaSuccess) return cerr;
     if constexpr (kHasSpill)
-        if ((cerr = configure_interp<G, true, S>(&static_spill)) != cudaSuccess) return cerr;
+        if ((cerr = configure_interp<G, true, S, UNSORTED>(&static_spill)) != cudaSuccess) return cerr;
     bool hybrid = HYBRID && shape.hybrid && shape.cap_cx > 0;
     if (shape.merged) {
         // list launches (second stage, re-evaluation): few tasks per tier, so one launch walks the tiers' lists one after
@@ -813,8 +919,9 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         const int slab = (shape.cap_cx > 0 && sp) ? std::min(t->tiers.slab_cx[k0], shape.cap_cx) : t->tiers.slab_cx[k0];
         const size_t smem = ((size_t)EPW * slab * ELEM + 15) / 16 * 16 + ring_bytes;
         if (smem > kMaxSlabBytes + ring_bytes) return cudaErrorInvalidValue;
-        int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (shape.regs * BLOCK), (228 * 1024) / (smem + 1024 + (sp ? static_spill : static_direct))));
-        if (sp) per_sm = std::min(per_sm, shape.spill_blocks);
+        int per_sm = 1;
+        if (sp) { if constexpr (kHasSpill) per_sm = std::min(interp_blocks_per_sm<G, true, S, UNSORTED>(smem), shape.spill_blocks); }
+        else { if constexpr (kHasDirect) per_sm = interp_blocks_per_sm<G, false, S, UNSORTED>(smem); }
         const long long tasks = ((shape.tasks_hint > 0 ? shape.tasks_hint : p.N) + EPW - 1) / EPW + kTiers;
         long long blocks = std::max<long long>(1, std::min<long long>(tasks, (long long)sm_count * per_sm));
         if (sp && shape.max_blocks > 0) blocks = std::min<long long>(blocks, shape.max_blocks);
@@ -822,9 +929,9 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         p.merged = 1;
         p.slab_cx = slab;
         if (sp) {
-            if constexpr (kHasSpill) cdbg_prog_kernel<G, true, S><<<(unsigned)blocks, BLOCK, smem, s>>>(p);
+            if constexpr (kHasSpill) cdbg_prog_kernel<G, true, S, UNSORTED><<<(unsigned)blocks, BLOCK, smem, s>>>(p);
         } else {
-            if constexpr (kHasDirect) cdbg_prog_kernel<G, false, S><<<(unsigned)blocks, BLOCK, smem, s>>>(p);
+            if constexpr (kHasDirect) cdbg_prog_kernel<G, false, S, UNSORTED><<<(unsigned)blocks, BLOCK, smem, s>>>(p);
         }
         ++*launched;
         return cudaGetLastError();
@@ -838,7 +945,7 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         for (int k = 0; k < kTiers; k++) {
             if (t->tiers.first_key[k] == t->tiers.first_key[k + 1] && k + 1 < kTiers) continue;
             const size_t sm = ((size_t)EPW * t->tiers.slab_cx[k] * ELEM + 15) / 16 * 16 + (G >= 8 ? (size_t)kRing * BLOCK * 16 : 0);
-            direct += (long long)sm_count * (long long)std::max<size_t>(1, std::min<size_t>(65536 / (shape.regs * BLOCK), (228 * 1024) / (sm + 1024 + static_direct)));
+            if constexpr (kHasDirect) direct += (long long)sm_count * interp_blocks_per_sm<G, false, S, UNSORTED>(sm);
         }
         if (max_tasks <= 2 * direct) hybrid = false;
     }
@@ -861,9 +968,9 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         if (smem[k] > kMaxSlabBytes + ring_bytes) return cudaErrorInvalidValue;
         // resident blocks per SM: 228 KB of shared memory against dynamic + static + 1 KB reserved per block (a grid
         // sized for one block more than fits runs a second, nearly empty wave), and 65536 / (regs x BLOCK) registers
-        const size_t static_smem = sp[k] ? static_spill : static_direct;
-        int per_sm = (int)std::max<size_t>(1, std::min<size_t>(65536 / (shape.regs * BLOCK), (228 * 1024) / (smem[k] + 1024 + static_smem)));
-        if (sp[k]) per_sm = std::min(per_sm, shape.spill_blocks);   // one global slab per resident block
+        int per_sm = 1;
+        if (sp[k]) { if constexpr (kHasSpill) per_sm = std::min(interp_blocks_per_sm<G, true, S, UNSORTED>(smem[k]), shape.spill_blocks); }   // one global slab per resident block
+        else { if constexpr (kHasDirect) per_sm = interp_blocks_per_sm<G, false, S, UNSORTED>(smem[k]); }
         blocks[k] = (unsigned)std::max<long long>(1, std::min<long long>(max_tasks, (long long)sm_count * per_sm));
         if (sp[k] && shape.max_blocks > 0) blocks[k] = (unsigned)std::min<long long>(blocks[k], shape.max_blocks);
         resident += (long long)sm_count * per_sm;
@@ -898,9 +1005,9 @@ static cudaError_t launch_interp(cudaStream_t s, const ProgTable* t, int sm_coun
         if (sp[k]) {
             if (share_slabs) p.spill = reinterpret_cast<double2*>(reinterpret_cast<char*>(spill0) + (size_t)li * share * p.spill_cx * EPW * ELEM);
             li++;
-            if constexpr (kHasSpill) cdbg_prog_kernel<G, true, S><<<blocks[k], BLOCK, smem[k], ls>>>(p);
+            if constexpr (kHasSpill) cdbg_prog_kernel<G, true, S, UNSORTED><<<blocks[k], BLOCK, smem[k], ls>>>(p);
         } else {
-            if constexpr (kHasDirect) cdbg_prog_kernel<G, false, S><<<blocks[k], BLOCK, smem[k], ls>>>(p);
+            if constexpr (kHasDirect) cdbg_prog_kernel<G, false, S, UNSORTED><<<blocks[k], BLOCK, smem[k], ls>>>(p);
         }
         if (conc && !first) cudaEventRecord(t->join_ev[side++], ls);
         first = false;

@@ -790,6 +790,15 @@ static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_co
                                 : launch_interp<256, false, double>(s, t, sm_count, p, launches, shape);
         }
     }
+    if (!p.rec) {    // UNSORTED (n <= 5): one launch that classifies its events itself and reads the caller's arrays
+        shape.merged = true;
+        switch (t->G) {
+            case 1: return launch_interp<1, false, cx, false, true>(s, t, sm_count, p, launches, shape);
+            case 2: return launch_interp<2, false, cx, false, true>(s, t, sm_count, p, launches, shape);
+            case 4: return launch_interp<4, false, cx, false, true>(s, t, sm_count, p, launches, shape);
+            default: return cudaErrorInvalidValue;
+        }
+    }
     if (t->cap_cx > 0 && p.spill) {     // heavy tiers: capped shared-memory state + L2 slab (see prog_table_create)
         shape.hybrid = true;
         shape.cap_cx = t->cap_cx;
@@ -816,6 +825,15 @@ static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_co
     return err;
 }
 
+// the UNSORTED path: discrete states, at most 4 lanes per event, every class in the one (last) tier, and a batch small
+// enough for the launches saved to outweigh the divergence of unsorted warps (measured, FP64 kernels: n = 4 2^12 ... 2^17
+// events 32 -> 16, 32 -> 18, 42 -> 35, 56 -> 53 us, 2^18 93 -> 96 us; n = 5 2^10 ... 2^15 36 -> 21, 36 -> 23, 42 -> 35,
+// 52 -> 51 us, 2^16 71 -> 88 us)
+static bool prog_unsorted(const ProgTable* t, long long N) {
+    if (t->dense || t->spill || t->G > 4 || t->n > 5 || t->tiers.first_key[kTiers - 1] != 0) return false;
+    return N <= (t->n == 4 ? (1ll << 17) : (1ll << 15));
+}
+
 cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,
                              const signed char* hel, const signed char* col, double* out, void* scratch,
                              int* launches, cudaEvent_t ev0, cudaEvent_t ev1, double tau, double tau_rho, cudaEvent_t ev_mid,
@@ -831,6 +849,32 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     uint32_t* flag_list = flag_count + 16;
     const int nbins = (int)t->num_classes + 1;
     cudaError_t err = cudaSuccess;
+    // n <= 5, small batches, FP64 kernels alone: classify, sort and scatter take more than half of a step (n = 4, 2^16
+    // events: 27 of 43 us in the kernels alone).  The UNSORTED instantiations skip them - tasks in input order,
+    // classification inside the interpreter: one launch (DESIGN.md 5.1c for what that costs at larger sizes).
+    if (tau <= 0.0 && prog_unsorted(t, N)) {
+        ProgParams p;
+        p.n = t->n; p.N = N; p.out = out;
+        p.info = t->d_info; p.ops = t->d_ops; p.rec = nullptr; p.rec_bytes = rec_bytes; p.rec_gstride = 4;
+        p.mom = mom; p.hel = hel; p.col = col;
+        p.bounds = nullptr;
+        p.zero = 0;
+        p.spill = nullptr;
+        p.spill_cx = t->max_state_cx;
+        p.tier = kTiers - 1;
+        p.merged = 0;
+        p.slab_cx = t->max_state_cx;
+        p.tau2 = tau;              // 0, or a diagnostic code
+        p.tau_rho = 0.0;
+        p.flag_list = nullptr; p.flag_count = nullptr; p.list = nullptr; p.list_count = nullptr; p.ticket = nullptr;
+        p.twin = rotated ? 1 : 0;
+        p.tw2 = 0.0; p.td = 0.0; p.soft_count = nullptr; p.soft_list = nullptr;
+        *launches = 0;
+        if (ev0) cudaEventRecord(ev0, s);
+        err = dispatch_interp(s, t, sm_count, p, launches);
+        if (ev1) cudaEventRecord(ev1, s);
+        return err;
+    }
     const unsigned eb = (unsigned)((N + kPreEvents - 1) / kPreEvents);
     const size_t hist_smem = sizeof(uint32_t) * nbins;
     const size_t stage_bytes = (size_t)(kStageThreads / 32) * (32 * (rec_bytes + 16) + 256);
@@ -892,6 +936,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.n = t->n; p.N = N; p.out = out;
     p.info = t->d_info; p.ops = t->d_ops; p.rec = rec; p.rec_bytes = rec_bytes; p.rec_gstride = 4;
     p.bounds = bounds;
+    p.mom = nullptr; p.hel = nullptr; p.col = nullptr;
     p.zero = 0;
     p.spill = t->spill ? (double2*)((char*)scratch + prog_spill_offset(t, N)) : nullptr;
     if (t->cap_cx > 0) p.spill = (double2*)((char*)scratch + prog_spill_offset(t, N) + prog_spill_bytes(t));
@@ -968,6 +1013,7 @@ cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, 
     p.tau2 = 0.0;
     p.tau_rho = 0.0;
     p.flag_list = nullptr; p.flag_count = nullptr; p.list = nullptr; p.list_count = nullptr; p.ticket = nullptr;
+    p.mom = nullptr; p.hel = nullptr; p.col = nullptr;
     p.twin = 0; p.tw2 = 0.0; p.td = 0.0; p.soft_list = nullptr; p.soft_count = nullptr;
     *launches = 1;
     if (ev0) cudaEventRecord(ev0, s);

@@ -584,6 +584,48 @@ def test_vanishing_and_out_of_range_colours_after_a_large_context(bg, wl):
         assert np.all(got[dead] == 0.0) and np.array_equal(got[~dead], ref[~dead])
 
 
+@pytest.mark.parametrize("n,N", [(4, 1), (4, 4099), (5, 33), (5, 20011)])
+def test_single_launch_path_of_small_batches(bg, oracle, wl, n, N):
+    """n <= 5, FP64 kernels alone, small batches: one launch that classifies each event inside the interpreter and reads
+    the caller's arrays in input order (no prepass, no records).  Same class programs, same arithmetic per event as the
+    sorted path, so the bits agree with it - reached here through the default precision with thresholds that flag
+    nothing - and dead events (vanishing class, colour index out of range) return exactly 0.0."""
+    ev = wl.config_events(4, N=N, n=n)
+    col = ev.col.copy()
+    rng = np.random.default_rng(n * 1000 + N)
+    kill = (rng.random(N) < 0.2) & (N > 4)
+    col[kill, 0, 0] = (col[kill, 0, 0] % 3) + 1                # unbalanced colour charges: identically zero
+    bad = (rng.random(N) < 0.1) & (N > 4)
+    col[bad, 2, 1] = 9                                         # out of range
+    ev2 = type(ev)(ev.n, ev.mom, ev.hel, col)
+    got, name = gpu_eval(ev2, bg.BG_CDBG_GIVEN, precision=0)
+    assert name == "cdbg_prog_kernel"
+    import torch
+    dev = torch.device("cuda:0")
+    d = [torch.from_numpy(x).to(dev) for x in (wl.to_soa(mom=ev2.mom), wl.to_soa(hel=ev2.hel), wl.to_soa(col=ev2.col))]
+    out = torch.full((N,), float("nan"), dtype=torch.float64, device=dev)
+    ctx = bg.bg_init(n, bg.BG_CDBG_GIVEN)
+    try:
+        bg.bg_set_option(ctx, bg.BG_OPT_FLAG_THRESHOLD, 10 ** 17)      # sorted path, nothing flagged
+        bg.bg_set_option(ctx, bg.BG_OPT_FLAG_CANCELLATION, 1)
+        bg.bg_eval(ctx, torch.cuda.current_stream().cuda_stream, N, *d, out)
+        torch.cuda.synchronize()
+        launches_sorted = bg.bg_last_launch_count(ctx)
+        ref = out.cpu().numpy()
+        bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 0)
+        bg.bg_eval(ctx, torch.cuda.current_stream().cuda_stream, N, *d, out)
+        torch.cuda.synchronize()
+        assert bg.bg_last_launch_count(ctx) == 1 < launches_sorted
+    finally:
+        bg.bg_destroy(ctx)
+    dead = kill | bad
+    assert np.all(got[dead] == 0.0)
+    live = ~dead & (ref > 0)
+    assert live.any() and np.array_equal(got[live], ref[live])
+    if live.any():
+        check_cdbg_fp64(oracle, ev2.take(np.nonzero(live)[0]), got[live], max_tail_frac=0.02)
+
+
 def test_batch_size_guard(bg):
     """Event ids and record positions are 32 bit: larger batches are refused, not truncated."""
     ctx = bg.bg_init(4, bg.BG_CDBG_GIVEN)
