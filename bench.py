@@ -163,7 +163,7 @@ def measure_config(bg, wl, oracle_mod, dev, config: int, n: int, steps: int, pea
     res = {"workload": ("COBG full colour (extra)" if cobg8 else {0: "C1", 2: "C3", 3: "C4", 4: "C5"}.get(config, "C2")) + f" n={n}", "n": n, "events": N}
     try:
         bg.bg_reserve(ctx, N)
-        auto = config != 0
+        auto = config != 0 and not (config == 4 and n == 4)     # (n = 4 CDBG: the default is FP64 alone)
 
         def timed(precision):
             if auto:

@@ -77,20 +77,20 @@ enum {
     BG_OPT_TIMING = 4,       /* 1: record CUDA events around the dominant kernel of every bg_eval (bg_last_kernel_ms) */
     BG_OPT_PRECISION = 6,    /* 0 = FP64 kernels only; 1 = every event in double-double arithmetic (BG_CDBG_GIVEN and the COBG
                                 full-colour modes: the precision reference on the GPU, slow); 2 (the default of BG_CDBG_GIVEN
-                                and BG_COBG_HELGIVEN_FULLCOLOR) = FP64 kernels plus a conditioning flag per event and
-                                re-evaluation of what it names: the colour-flow amplitude of Eq. 19 / 28-32
-                                 has near-zeros - helicity-suppressed configurations,
-                                cancellations between orderings - where FP64 round-off exceeds 1e-11 of the result.
-                                An event is flagged when its Ward residual |p_n . J| / (E_n |eps_n . J|) (J = the current of
-                                gluons 1..n-1 of Eq. 22; zero without round-off) exceeds BG_OPT_FLAG_THRESHOLD, or when |A|
-                                is less than BG_OPT_FLAG_CANCELLATION times the sum of the moduli of the closure
-                                contributions that add up to it.  BG_CDBG_GIVEN then runs a cascade: flagged events whose
-                                residual stays below BG_OPT_FLAG_TWIN are evaluated once more in FP64 in a rotated frame
-                                (the same number with independent round-off); those whose two results agree to
-                                BG_OPT_FLAG_TWIN keep the first one, the others - and the events the first stage did not
-                                send to the second - are evaluated by a double-double instantiation of the same kernel.
-                                3, 4 = diagnostics: `out` receives the Ward residual / the cancellation ratio instead
-                                of |M|^2. */
+                                for n >= 5 and of BG_COBG_HELGIVEN_FULLCOLOR; n = 4 meets 1e-11 in FP64 and defaults to 0) =
+                                FP64 kernels plus a conditioning flag per event and re-evaluation of what it names: the
+                                colour-flow amplitude of Eq. 19 / 28-32 has near-zeros -
+                                helicity-suppressed configurations, cancellations between orderings - where FP64
+                                round-off exceeds 1e-11 of the result.  An event is flagged when its Ward residual
+                                |p_n . J| / (E_n |eps_n . J|) (J = the current of gluons 1..n-1 of Eq. 22; zero without
+                                round-off) exceeds BG_OPT_FLAG_THRESHOLD, or when |A| is less than BG_OPT_FLAG_CANCELLATION
+                                times the sum of the moduli of the closure contributions that add up to it.  BG_CDBG_GIVEN
+                                then runs a cascade: flagged events whose residual stays below the bound of
+                                BG_OPT_FLAG_TWIN are evaluated once more in FP64 in a rotated frame (the same number with
+                                independent round-off); those whose two results agree to BG_OPT_FLAG_TWIN keep the first
+                                one, the others - and the events the first stage did not send to the second - are
+                                evaluated by a double-double instantiation of the same kernel.  3, 4 = diagnostics: `out`
+                                receives the Ward residual / the cancellation ratio instead of |M|^2. */
     BG_OPT_FLAG_THRESHOLD = 7,/* Ward-residual threshold in units of 1e-18 (0 = default; BG_CDBG_GIVEN: 1e-13 for n = 4 and
                                 n >= 11, 1e-14 for n = 5, 6, 3e-14 for n = 7 .. 10; COBG: 1e-13, 3e-13 for n >= 7) */
     BG_OPT_FLAG_CANCELLATION = 8, /* cancellation threshold in units of 1e-6 (0 = default: 3e-3) */

@@ -223,7 +223,9 @@ int bg_init(bg_ctx** out, int n, int mode) {
     c->tau_rho = kDefaultTauRho;
     c->tau_twin = kDefaultTauTwin;
     c->frame = 0;
-    if (mode == BG_CDBG_GIVEN && c->prog && bg::prog_dd_mode(c->prog) >= 0) c->precision = 2;
+    // (n = 4: a single colour flow is one Parke-Taylor term per helicity assignment; the FP64 kernels alone stay below
+    // 1.2e-12 on 2^20 + 2^18 events, and any flagged event would cost a 47 us double-double pass: FP64 by default)
+    if (mode == BG_CDBG_GIVEN && c->prog && bg::prog_dd_mode(c->prog) >= 0 && n >= 5) c->precision = 2;
     if (mode == BG_COBG_HELGIVEN_FULLCOLOR && c->cobg) c->precision = 2;
     bool streams_ok = cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking) == cudaSuccess &&
                       cudaStreamCreateWithFlags(&c->cstream, cudaStreamNonBlocking) == cudaSuccess;

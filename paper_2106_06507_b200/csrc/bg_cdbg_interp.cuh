@@ -884,12 +884,23 @@ static cudaError_t configure_interp(size_t* static_smem_out) {
 template <int G, bool SPILL, class S, bool UNSORTED = false>
 static int interp_blocks_per_sm(size_t smem) {
     constexpr int BLOCK = G > 32 ? G : 32;
+    // asked once per shared-memory size and device (a bg_eval sizes up to four launches per stage; the query costs
+    // host time that a small batch has nothing to hide behind)
+    struct Entry { int device; size_t smem; int blocks; };
+    static Entry cache[16];
+    static int used = 0;
+    int device = 0;
+    cudaGetDevice(&device);
+    for (int i = 0; i < used; i++)
+        if (cache[i].device == device && cache[i].smem == smem) return cache[i].blocks;
     int nb = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, cdbg_prog_kernel<G, SPILL, S, UNSORTED>, BLOCK, smem) != cudaSuccess) {
         cudaGetLastError();
         nb = 1;
     }
-    return std::max(1, nb);
+    nb = std::max(1, nb);
+    if (used < 16) cache[used++] = {device, smem, nb};
+    return nb;
 }
 
 // SPILL: every tier runs the spill kernel.  HYBRID (with SPILL = false): shape.hybrid picks it per tier.

@@ -606,6 +606,7 @@ def test_single_launch_path_of_small_batches(bg, oracle, wl, n, N):
     out = torch.full((N,), float("nan"), dtype=torch.float64, device=dev)
     ctx = bg.bg_init(n, bg.BG_CDBG_GIVEN)
     try:
+        bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 2)                  # (the default for n >= 5)
         bg.bg_set_option(ctx, bg.BG_OPT_FLAG_THRESHOLD, 10 ** 17)      # sorted path, nothing flagged
         bg.bg_set_option(ctx, bg.BG_OPT_FLAG_CANCELLATION, 1)
         bg.bg_eval(ctx, torch.cuda.current_stream().cuda_stream, N, *d, out)
