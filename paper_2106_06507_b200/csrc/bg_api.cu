@@ -677,7 +677,10 @@ int bg_eval_host(bg_ctx* c, long long N, const double* mom, const signed char* h
     // Chunked pipeline: the copy stream runs ahead with the host->device copies of chunk k+1 (one strided 2-D copy
     // per array: the arrays are event-fastest) while the compute stream evaluates chunk k and returns its results.
     // Every chunk has its own compact region (event stride = its size) inside the staging buffers.
-    int K = (int)std::min<long long>(kHostChunks, N / 32768);
+    // (default precision of the colour-dressed path: every bg_eval ends with a double-double pass that is at least one
+    // task deep - 0.25 ms at n = 6 - so fewer, larger chunks: n = 6, 2^20 events 1.84e8 events/s with 8 chunks, 2.09e8 with 4)
+    const long long min_chunk = (c->precision == 2 && c->mode == BG_CDBG_GIVEN) ? 262144 : 32768;
+    int K = (int)std::min<long long>(kHostChunks, N / min_chunk);
     if (K < 1) K = 1;
     long long chunk = (N + K - 1) / K;
     chunk = (chunk + 255) / 256 * 256;
