@@ -84,22 +84,24 @@ enum {
                                 round-off exceeds 1e-11 of the result.  An event is flagged when its Ward residual
                                 |p_n . J| / (E_n |eps_n . J|) (J = the current of gluons 1..n-1 of Eq. 22; zero without
                                 round-off) exceeds BG_OPT_FLAG_THRESHOLD, or when |A| is less than BG_OPT_FLAG_CANCELLATION
-                                times the sum of the moduli of the closure contributions that add up to it.  BG_CDBG_GIVEN
-                                then runs a cascade: flagged events whose residual stays below the bound of
+                                times the sum of the moduli of the closure contributions that add up to it (colour-ordered
+                                path: the residual summed over the orderings, no cancellation test).  Then a cascade: flagged events whose residual stays below the bound of
                                 BG_OPT_FLAG_TWIN are evaluated once more in FP64 in a rotated frame (the same number with
                                 independent round-off); those whose two results agree to BG_OPT_FLAG_TWIN keep the first
                                 one, the others - and the events the first stage did not send to the second - are
                                 evaluated by a double-double instantiation of the same kernel.  3, 4 = diagnostics: `out`
                                 receives the Ward residual / the cancellation ratio instead of |M|^2. */
     BG_OPT_FLAG_THRESHOLD = 7,/* Ward-residual threshold in units of 1e-18 (0 = default; BG_CDBG_GIVEN: 1e-13 for n = 4 and
-                                n >= 11, 1e-14 for n = 5, 6, 3e-14 for n = 7 .. 10; COBG: 1e-13, 3e-13 for n >= 7) */
+                                n >= 11, 1e-14 for n = 5, 6, 3e-14 for n = 7 .. 10; COBG: 3e-14 for n <= 5, else 1e-13) */
     BG_OPT_FLAG_CANCELLATION = 8, /* cancellation threshold in units of 1e-6 (0 = default: 3e-3) */
-    BG_OPT_FLAG_TWIN = 9,    /* BG_CDBG_GIVEN: bound of the second stage in units of 1e-18 (0 = default: 5e-13) on |w - w'| / w
-                                of the two evaluations; the Ward residual of either may not exceed the same number for
-                                n = 6, 0.4 times it otherwise.  With that residual bound at or below BG_OPT_FLAG_THRESHOLD
+    BG_OPT_FLAG_TWIN = 9,    /* bound of the second stage in units of 1e-18 on |w - w'| / w of the two evaluations (0 = default:
+                                BG_CDBG_GIVEN 5e-13; COBG 5e-13 for n <= 5, else 1e-12).  The Ward residual of either may not
+                                exceed the same number (BG_CDBG_GIVEN n = 6, COBG n >= 6), 0.4 times it (BG_CDBG_GIVEN, other
+                                n) or twice it (COBG n <= 5).  With that residual bound at or below BG_OPT_FLAG_THRESHOLD
                                 there is no second stage and every flagged event is evaluated in double-double */
-    BG_OPT_FRAME = 10,       /* BG_CDBG_GIVEN, program interpreter: 1 = evaluate every event in the rotated frame of the
-                                second stage (fixed rotation, axis (1,2,3), 1 rad) - |M|^2 is the same to round-off; a
+    BG_OPT_FRAME = 10,       /* BG_CDBG_GIVEN (program interpreter) and the COBG modes (shared-current kernel): 1 = evaluate
+                                every event in the rotated frame of the second stage (fixed rotation, axis (1,2,3), 1 rad) -
+                                |M|^2 is the same to round-off; a
                                 diagnostic of Lorentz invariance and of the FP64 error */
     BG_OPT_SMEM_LIMIT = 5    /* program interpreter, >= 128 lanes per event: bytes of shared memory one event's state may
                                 take (16 KiB .. 222 KiB, 0 = default); the rest spills to an L2-resident slab.
@@ -191,7 +193,7 @@ int bg_last_refined(bg_ctx* ctx, long long* flagged, double* ms);
 /* Name of the kernel variant the most recent bg_eval used (static string). */
 const char* bg_last_kernel_name(const bg_ctx* ctx);
 
-/* BG_OPT_PRECISION = 2, BG_CDBG_GIVEN: how many events of the most recent bg_eval went through the second stage of the
+/* BG_OPT_PRECISION = 2: how many events of the most recent bg_eval went through the second stage of the
  * cascade (the rotated-frame FP64 evaluation); bg_last_refined counts those evaluated in double-double.  Synchronises. */
 int bg_last_twin(bg_ctx* ctx, long long* count);
 

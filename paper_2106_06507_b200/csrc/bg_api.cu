@@ -151,7 +151,12 @@ static const double kDefaultTauTwin = 5e-13;
 // recursion never uses) shows in the residuals, not in the difference.  n = 6: no such event in 6 x 2^20; n = 5, 7: one per
 // 2^19 - 2^20 events at 1.0 - 2.3e-11 with residuals of 2.6 - 2.9e-13.
 static double twin_ward_fraction(int n) { return n == 6 ? 1.0 : 0.4; }
-static double default_tau_cobg(int n) { return n >= 7 ? 3e-13 : 1e-13; }   // (n = 8: as n = 7; sampled)
+// COBG (the colour-summed |M|^2 is better conditioned than a single colour flow): second-stage bound 1e-12 on the
+// difference and on the residuals for n >= 6 (2^19 / 2^18 / 2^13 events at n = 6 / 7 / 8: 0.9 - 1.1 % left for double-double,
+// worst accepted error 4.1 / 5.2 / 0.8e-12), 5e-13 on the difference for n <= 5 (1.0 %, 4.1e-12)
+static double default_tau_twin_cobg(int n) { return n <= 5 ? 5e-13 : 1e-12; }
+static double twin_ward_fraction_cobg(int n) { return n <= 5 ? 2.0 : 1.0; }
+static double default_tau_cobg(int n) { return n <= 5 ? 3e-14 : 1e-13; }
 static const double kDefaultTauRho = 3e-3;
 
 static bool mode_supported(int n, int mode) {
@@ -221,7 +226,7 @@ int bg_init(bg_ctx** out, int n, int mode) {
     // default precision: FP64 with the conditioning flag and double-double re-evaluation of the flagged events
     c->tau = mode == BG_COBG_HELGIVEN_FULLCOLOR ? default_tau_cobg(n) : default_tau(n);
     c->tau_rho = kDefaultTauRho;
-    c->tau_twin = kDefaultTauTwin;
+    c->tau_twin = mode == BG_COBG_HELGIVEN_FULLCOLOR ? default_tau_twin_cobg(n) : kDefaultTauTwin;
     c->frame = 0;
     // (n = 4: a single colour flow is one Parke-Taylor term per helicity assignment; the FP64 kernels alone stay below
     // 1.2e-12 on 2^20 + 2^18 events, and any flagged event would cost a 47 us double-double pass: FP64 by default)
@@ -315,7 +320,7 @@ static long long generic_chunk(const bg_ctx* c, long long N) {
 size_t bg_scratch_bytes(const bg_ctx* c, long long N) {
     if (!c || N <= 0) return 0;
     if (use_cobg_dd(c)) return bg::cobg_dd_scratch_per_event(c->n, (c->mode & BG_HEL_SUM) != 0) * (size_t)cobg_dd_chunk(c, N);
-    if (use_cobg_auto(c)) return 256 + (size_t)N * 4;   // flag counter | flagged event ids
+    if (use_cobg_auto(c)) return 256 + (size_t)N * 8;   // list counters | double-double list | second-stage list
     if (c->mode == BG_COMC_GIVEN) return c->prog ? bg::prog_scratch_bytes(c->prog, N) : 0;
     if (!(c->mode & BG_REC_CDBG)) return 0;
     if (use_dd(c)) return bg::cdbg_dd_scratch_per_event(c->n) * (size_t)dd_chunk(c, N);
@@ -433,11 +438,12 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
             return BG_OK;
         case BG_OPT_FLAG_TWIN:
             if (value < 0) return BG_EINVAL;
-            c->tau_twin = value == 0 ? kDefaultTauTwin : (double)value * 1e-18;
+            c->tau_twin = value != 0 ? (double)value * 1e-18
+                                     : (c->mode == BG_COBG_HELGIVEN_FULLCOLOR ? default_tau_twin_cobg(c->n) : kDefaultTauTwin);
             return BG_OK;
         case BG_OPT_FRAME:
             if (value != 0 && value != 1) return BG_EINVAL;
-            if (!(c->mode == BG_CDBG_GIVEN && c->prog)) return BG_EUNSUPPORTED;
+            if (!(c->mode == BG_CDBG_GIVEN && c->prog) && !((c->mode & BG_REC_COBG) && c->mode != BG_COMC_GIVEN && c->cobg)) return BG_EUNSUPPORTED;
             c->frame = (int)value;
             return BG_OK;
         case BG_OPT_TIMING:
@@ -544,8 +550,15 @@ int bg_last_refined(bg_ctx* c, long long* flagged, double* ms) {
 int bg_last_twin(bg_ctx* c, long long* count) {
     if (!c || !count) return BG_EINVAL;
     *count = 0;
-    if (!c->last_auto || !c->scratch || c->mode != BG_CDBG_GIVEN || !c->prog) return BG_OK;
+    if (!c->last_auto || !c->scratch) return BG_OK;
     if (cudaDeviceSynchronize() != cudaSuccess) return BG_ECUDA;
+    if (c->mode == BG_COBG_HELGIVEN_FULLCOLOR) {
+        uint32_t k = 0;
+        if (cudaMemcpy(&k, (const uint32_t*)c->scratch + 1, sizeof(k), cudaMemcpyDeviceToHost) != cudaSuccess) return BG_ECUDA;
+        *count = k;
+        return BG_OK;
+    }
+    if (c->mode != BG_CDBG_GIVEN || !c->prog) return BG_OK;
     return bg::prog_twin_count(c->prog, c->last_N, c->scratch, count) == cudaSuccess ? BG_OK : BG_ECUDA;
 }
 
@@ -580,15 +593,30 @@ int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const 
     } else if (use_cobg_auto(c)) {
         int rc = ensure_scratch(c, N);
         if (rc != BG_OK) return rc;
-        uint32_t* count = (uint32_t*)c->scratch;
+        uint32_t* count = (uint32_t*)c->scratch;      // [0]: double-double list, [1]: second-stage list
         uint32_t* list = count + 64;
         const bool flag = c->precision == 2;
         if (cudaMemsetAsync(count, 0, 64, s) != cudaSuccess) return BG_ECUDA;
         if (ev0) cudaEventRecord(ev0, s);
-        err = bg::cobg_shared_launch(s, c->cobg, false, false, c->dC, N, mom, hel, out, flag ? c->tau : -1.0, list, count);
+        bg::CobgCascade cas;
+        cas.twin = c->frame ? 1 : 0;
+        cas.tau_twin = c->tau_twin;
+        cas.tau_twin_ward = c->tau_twin * twin_ward_fraction_cobg(c->n);
+        cas.soft_list = list + N; cas.soft_count = count + 1;
+        cas.list = nullptr; cas.list_count = nullptr;
+        const bool cascade = flag && cas.tau_twin_ward > c->tau;
+        if (!cascade) cas.tau_twin_ward = 0.0;
+        err = bg::cobg_shared_launch(s, c->cobg, false, false, c->dC, N, mom, hel, out, flag ? c->tau : -1.0, list, count, &cas);
         c->last_launches = 1;
+        if (flag && c->timing) cudaEventRecord(c->ev_mid, s);
+        if (cascade && err == cudaSuccess) {
+            // second stage: the events between the two bounds once more in FP64 in the rotated frame
+            cas.twin = c->frame ? 2 : 3;
+            cas.list = cas.soft_list; cas.list_count = cas.soft_count;
+            err = bg::cobg_shared_launch(s, c->cobg, false, false, c->dC, N, mom, hel, out, c->tau, list, count, &cas);
+            c->last_launches++;
+        }
         if (flag && err == cudaSuccess) {
-            if (c->timing) cudaEventRecord(c->ev_mid, s);
             err = bg::cobg_dd_flagged_launch(s, c->n, c->nperm, c->dC, N, list, count, c->sm_count * 2, mom, hel, out);
             c->last_launches++;
         }
@@ -598,7 +626,8 @@ int bg_eval(bg_ctx* c, void* cuda_stream, long long N, const double* mom, const 
     } else if ((c->mode & BG_REC_COBG) && c->mode != BG_COMC_GIVEN) {
         if (ev0) cudaEventRecord(ev0, s);
         if (c->cobg && (c->kernel_opt != 1 || (c->mode & BG_COL_LC))) {
-            err = bg::cobg_shared_launch(s, c->cobg, helsum, (c->mode & BG_COL_LC) != 0, c->dC, N, mom, hel, out);
+            bg::CobgCascade cas = {c->frame ? 1 : 0, 0.0, 0.0, nullptr, nullptr, nullptr, nullptr};    // (BG_OPT_FRAME)
+            err = bg::cobg_shared_launch(s, c->cobg, helsum, (c->mode & BG_COL_LC) != 0, c->dC, N, mom, hel, out, 0.0, nullptr, nullptr, &cas);
             c->last_kernel = "cobg_shared_kernel";
         } else {
             err = bg::cobg_generic_launch(s, c->n, helsum, c->nperm, c->dC, N, mom, hel, out);

@@ -234,17 +234,6 @@ struct StateRef {
     }
 };
 
-// The same event in another frame: the spatial components of a momentum rotated by a fixed rotation (axis (1,2,3),
-// angle 1 rad).  The polarisation vectors of Eq. 3 in the gauge k = (q0, -q) rotate with the momenta, so every Lorentz
-// product of the recursion keeps its value and |A|^2 is the same number - computed from different components, i.e.
-// with independent round-off: the difference of the two results samples the FP64 error of the event.
-__device__ __forceinline__ void rotate_frame(double* pk) {
-    const double x = pk[1], y = pk[2], z = pk[3];
-    pk[1] = fma(0.5731378554489869, x, fma(-0.6090066421373933, y, 0.5482918096085999 * z));
-    pk[2] = fma(0.740348840460782, x, fma(0.6716445041915284, y, -0.027879282947946255 * z));
-    pk[3] = fma(-0.35127851212351696, x, fma(0.4219058779181122, y, 0.8358222520957642 * z));
-}
-
 constexpr int kRing = 4;   // op ring per lane: ops are requested kRing - 1 steps before they run
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {

@@ -60,6 +60,14 @@ struct CobgParams {
     double tau2;                      // 0: off; < 0: diagnostic, `out` receives the residual
     uint32_t* flag_list;              // [N] event ids
     uint32_t* flag_count;             // [1]
+    // cascade (as the colour-dressed path): events whose residual lies between tau and tau_twin are evaluated
+    // once more in FP64 in the rotated frame (twin bit 0) and compared with out[e] (twin bit 1)
+    int twin;
+    double tw2, td;                   // tau_twin^2 for the residuals, tau_twin for |w - w'| / w
+    uint32_t* soft_list;              // [N] first stage: events for the second stage
+    uint32_t* soft_count;             // [1]
+    const uint32_t* list;             // second stage: the events to evaluate (nullptr: all N)
+    const uint32_t* list_count;
 };
 
 
@@ -175,9 +183,18 @@ __global__ void __launch_bounds__(TPE > 128 ? TPE : 128, TPE > 128 ? 1 : 4) cobg
     const long long N = p.N;
     // given helicities: the EPB thread groups of a block take EPB events.  Summed helicities: the block takes one
     // event and its groups share the 2^n assignments (group evl takes hc = evl, evl + EPB, ..)
-    const long long e_raw = p.helsum ? (long long)blockIdx.x : (long long)blockIdx.x * EPB + evl;
-    const bool active = e_raw < N;
-    const long long e = active ? e_raw : 0;
+    // (list launches: the grid is sized without knowing the count, a block takes tasks blockIdx.x, + gridDim.x, ..)
+    const long long nev = p.list ? (long long)*p.list_count : N;
+    const long long ntask = p.helsum ? nev : (nev + EPB - 1) / EPB;
+    for (long long task = blockIdx.x; task < ntask; task += gridDim.x) {
+    const long long e_raw = p.helsum ? task : task * EPB + evl;
+    const bool active = e_raw < nev;
+    const long long e = active ? (p.list ? (long long)p.list[e_raw] : e_raw) : 0;
+    auto load_momentum = [&](int g, double* pg) {
+#pragma unroll
+        for (int c = 0; c < 4; c++) pg[c] = p.mom[(size_t)(g * 4 + c) * N + e];
+        if (p.twin & 1) rotate_frame(pg);
+    };
 
     double total = 0.0;
     // Leading colour (Eq. 33) needs A(1, sigma) for all (n-1)! orderings of gluons 2..n: for each
@@ -191,8 +208,10 @@ __global__ void __launch_bounds__(TPE > 128 ? TPE : 128, TPE > 128 ? 1 : 4) cobg
         double ps[4] = {0.0, 0.0, 0.0, 0.0};
         for (int g = 0; g < M; g++)
             if ((mask >> g) & 1) {
+                double pg[4];
+                load_momentum(relabel(g), pg);
 #pragma unroll
-                for (int c = 0; c < 4; c++) ps[c] += p.mom[(size_t)(relabel(g) * 4 + c) * N + e];
+                for (int c = 0; c < 4; c++) ps[c] += pg[c];
             }
 #pragma unroll
         for (int c = 0; c < 4; c++) P[mask * 4 + c] = ps[c];
@@ -228,8 +247,7 @@ __global__ void __launch_bounds__(TPE > 128 ? TPE : 128, TPE > 128 ? 1 : 4) cobg
                 slot = p.slot[(sig * M + i) * M + i];
             }
             double pg[4];
-#pragma unroll
-            for (int c = 0; c < 4; c++) pg[c] = p.mom[(size_t)(relabel(g) * 4 + c) * N + e];
+            load_momentum(relabel(g), pg);
             const int lam = p.helsum ? (((hc >> relabel(g)) & 1) ? 1 : -1) : (int)p.hel[(size_t)relabel(g) * N + e];
             cx eps[4];
             polarisation(pg, lam, eps);
@@ -364,8 +382,21 @@ __global__ void __launch_bounds__(TPE > 128 ? TPE : 128, TPE > 128 ? 1 : 4) cobg
             }
             if (t == 0 && active) {
                 const double En = p.mom[(size_t)(M * 4) * N + e];
-                if (p.tau2 < 0.0) total = ::sqrt(ward2 / (En * En * amp2));
-                else if (!(ward2 <= p.tau2 * En * En * amp2) || !(w > 0.0)) p.flag_list[atomicAdd(p.flag_count, 1u)] = (uint32_t)e;
+                const double scale = En * En * amp2;
+                if (p.tau2 < 0.0) {
+                    total = ::sqrt(ward2 / scale);
+                } else {
+                    const bool hard = !(ward2 <= fmax(p.tw2, p.tau2) * scale) || !(w > 0.0);
+                    bool to_dd = hard, to_twin = false;
+                    if (p.twin & 2) {
+                        const double w1 = p.out[e];
+                        to_dd = hard || !(fabs(w - w1) <= p.td * w1);
+                    } else if (!hard) {
+                        to_twin = !(ward2 <= p.tau2 * scale);      // (tau_twin <= tau: never - no second stage)
+                    }
+                    if (to_dd) p.flag_list[atomicAdd(p.flag_count, 1u)] = (uint32_t)e;
+                    else if (to_twin) p.soft_list[atomicAdd(p.soft_count, 1u)] = (uint32_t)e;
+                }
             }
         }
     }
@@ -381,9 +412,10 @@ __global__ void __launch_bounds__(TPE > 128 ? TPE : 128, TPE > 128 ? 1 : 4) cobg
             for (int i = 0; i < EPB; i++) total += (smem_d + (size_t)i * ev_doubles + p.nslots * 2 * kSlotStride + NSUB * 4 + 8 + np * 2)[0];
         }
         if (threadIdx.x == 0 && active) p.out[e] = total;
-        return;
+    } else if (t == 0 && active && !(p.twin & 2)) {
+        p.out[e] = total;                 // (second stage of the cascade: out[e] keeps the first result)
     }
-    if (t == 0 && active) p.out[e] = total;
+    }   // task
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -507,15 +539,26 @@ static cudaError_t launch_cobg(cudaStream_t s, const CobgParams& p) {
         if (e != cudaSuccess) return e;
         configured_device = device;
     }
-    const unsigned blocks = p.helsum ? (unsigned)p.N : (unsigned)((p.N + EPB - 1) / EPB);
+    unsigned blocks = p.helsum ? (unsigned)p.N : (unsigned)((p.N + EPB - 1) / EPB);
+    if (p.list) {     // about 1/16 of the events, at least a wave of blocks (the kernel loops over what the list holds)
+        int sms = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+        blocks = (unsigned)std::max<long long>(1, std::min<long long>(blocks, std::max<long long>(4ll * sms, (p.N / 16 + EPB - 1) / EPB)));
+    }
     cobg_shared_kernel<NG, TPE, LC><<<blocks, BLOCK, smem, s>>>(p);
     return cudaGetLastError();
 }
 
 cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, bool lc, const double* dC, long long N,
                                const double* mom, const signed char* hel, double* out, double tau, uint32_t* flag_list,
-                               uint32_t* flag_count) {
+                               uint32_t* flag_count, const CobgCascade* cascade) {
     CobgParams p;
+    p.twin = 0; p.tw2 = 0.0; p.td = 0.0; p.soft_list = nullptr; p.soft_count = nullptr; p.list = nullptr; p.list_count = nullptr;
+    if (cascade) {
+        p.twin = cascade->twin; p.tw2 = cascade->tau_twin_ward * cascade->tau_twin_ward; p.td = cascade->tau_twin;
+        p.soft_list = cascade->soft_list; p.soft_count = cascade->soft_count;
+        p.list = cascade->list; p.list_count = cascade->list_count;
+    }
     p.tau2 = (helsum || lc || !flag_list) && tau >= 0.0 ? 0.0 : (tau < 0.0 ? -1.0 : tau * tau);
     if (helsum || lc) p.tau2 = 0.0;
     p.flag_list = flag_list; p.flag_count = flag_count;

@@ -107,9 +107,19 @@ void cobg_table_destroy(CobgTable* t);
 int cobg_table_set_colour(CobgTable* t, const double* hC);   // optional: compressed colour matrix for the colour form
 size_t cobg_shared_current_bytes(const CobgTable* t);
 // tau != 0 (given helicities, full colour): flag list of the events whose Ward residual exceeds tau (tau < 0: diagnostic)
+// cascade (BG_OPT_PRECISION = 2): second-stage lists and bounds, or a second-stage launch over `list`
+struct CobgCascade {
+    int twin;                    // bit 0: rotated frame; bit 1: compare with out[e] instead of writing it
+    double tau_twin, tau_twin_ward;
+    uint32_t* soft_list;         // first stage: receives the events for the second stage
+    uint32_t* soft_count;
+    const uint32_t* list;        // second stage: the events to evaluate
+    const uint32_t* list_count;
+};
 cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, bool lc, const double* dC, long long N,
                                const double* mom, const signed char* hel, double* out, double tau = 0.0,
-                               uint32_t* flag_list = nullptr, uint32_t* flag_count = nullptr);
+                               uint32_t* flag_list = nullptr, uint32_t* flag_count = nullptr,
+                               const CobgCascade* cascade = nullptr);
 
 // ---- colour matrix (bg_colour.cpp part of bg_api.cu) ------------------------------------------------------
 int build_colour_matrix(int n, double* C /* (n-2)!^2 */);

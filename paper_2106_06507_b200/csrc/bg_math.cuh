@@ -83,6 +83,17 @@ __device__ __forceinline__ void polarisation(const double* p, int lambda, cx* ep
     eps[3] = mk(l * e1z, 0.0);
 }
 
+// The same event in another frame: the spatial components of a momentum rotated by a fixed rotation (axis (1,2,3),
+// angle 1 rad).  The polarisation vectors of Eq. 3 in the gauge k = (q0, -q) rotate with the momenta, so every Lorentz
+// product of the recursion keeps its value and |A|^2 is the same number - computed from different components, i.e.
+// with independent round-off: the difference of the two results samples the FP64 error of the event.
+__device__ __forceinline__ void rotate_frame(double* pk) {
+    const double x = pk[1], y = pk[2], z = pk[3];
+    pk[1] = fma(0.5731378554489869, x, fma(-0.6090066421373933, y, 0.5482918096085999 * z));
+    pk[2] = fma(0.740348840460782, x, fma(0.6716445041915284, y, -0.027879282947946255 * z));
+    pk[3] = fma(-0.35127851212351696, x, fma(0.4219058779181122, y, 0.8358222520957642 * z));
+}
+
 // Real polarisation vector of the continuous sampling, Eq. 7: e(p, phi) = cos(phi) e1 + sin(phi) e2
 // with the unit vectors e1, e2 of the same gauge as `polarisation` (eps^lambda = (-lambda e1 - i e2)/sqrt2).
 __device__ __forceinline__ void polarisation_real(const double* p, double phi, double* e) {

@@ -219,6 +219,49 @@ def test_conditioning_flag_reports_and_options(bg, oracle, wl):
         bg.bg_destroy(ctx)
 
 
+@pytest.mark.parametrize("n,N", [(5, 20011), (6, 8195), (7, 2051)])
+def test_cobg_cascade_and_rotated_frame(bg, oracle, wl, n, N):
+    """The colour-ordered path's cascade: Ward flag, second FP64 evaluation in the rotated frame, double-double for what
+    is left.  Counters are consistent, every event meets the 1e-11 bar with and without the second stage, and the
+    rotated frame alone (BG_OPT_FRAME = 1) gives the same colour-summed |M|^2 to FP64 round-off."""
+    import torch
+    ev = wl.config_events(4, N=N, n=n)
+    truth = oracle.cobg_full_colour(ev.mom, ev.hel, prec="long double")
+    dev = torch.device("cuda:0")
+    d = [torch.from_numpy(x).to(dev) for x in (wl.to_soa(mom=ev.mom), wl.to_soa(hel=ev.hel))]
+    out = torch.zeros(ev.N, dtype=torch.float64, device=dev)
+    st = torch.cuda.current_stream().cuda_stream
+    ctx = bg.bg_init(n, bg.BG_COBG_HELGIVEN_FULLCOLOR)
+    try:
+        def run():
+            bg.bg_eval(ctx, st, ev.N, d[0], d[1], None, out)
+            torch.cuda.synchronize()
+            return out.cpu().numpy(), bg.bg_last_refined(ctx)[0], bg.bg_last_twin(ctx)
+        casc, n_dd, n_twin = run()
+        assert rel_err(casc, truth).max() <= 1e-11
+        assert 0 < n_twin < 0.1 * ev.N and 0 < n_dd < 0.05 * ev.N
+        bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 3)
+        ward = run()[0]
+        bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 2)
+        tau = 3e-14 if n <= 5 else 1e-13
+        soft = (ward > tau * (1 - 1e-9)) & (ward <= 1e-12 * (1 + 1e-9))
+        assert abs(int(soft.sum()) - n_twin) <= 2 and n_dd >= int((ward > 1e-12 * (1 + 1e-9)).sum())
+        bg.bg_set_option(ctx, bg.BG_OPT_FLAG_TWIN, 1)                  # no second stage
+        two, n_dd2, n_twin2 = run()
+        assert n_twin2 == 0 and abs(n_dd2 - int((ward > tau).sum())) <= 2 and rel_err(two, truth).max() <= 1e-11
+        bg.bg_set_option(ctx, bg.BG_OPT_FLAG_TWIN, 0)
+        bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 0)
+        plain = run()[0]
+        bg.bg_set_option(ctx, bg.BG_OPT_FRAME, 1)
+        rotated = run()[0]
+        assert np.any(plain != rotated) and np.median(rel_err(rotated, plain)) < 1e-13
+        check_fp64_floor(oracle, ev, rotated, False)
+        bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 2)                  # cascade starting from the rotated frame
+        assert rel_err(run()[0], truth).max() <= 1e-11
+    finally:
+        bg.bg_destroy(ctx)
+
+
 @pytest.mark.parametrize("n,N", [(5, 4099), (6, 8195), (7, 2051), (9, 515), (11, 67)])
 def test_rotated_frame_gives_the_same_matrix_element(bg, oracle, wl, n, N):
     """BG_OPT_FRAME = 1, the frame of the cascade's second stage: momenta rotated by a fixed rotation, polarisation
@@ -686,7 +729,7 @@ def test_cobg_full_colour_n8_shared_kernel(bg, oracle, wl):
     got, name = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR)
     assert name == "cobg_shared_kernel"
     fp64, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR, precision=0)
-    flagged_all, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR, flag_threshold=1)     # every event re-evaluated
+    flagged_all, _ = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR, flag_threshold=1, flag_twin=1)     # every event re-evaluated
     generic, gname = gpu_eval(ev, bg.BG_COBG_HELGIVEN_FULLCOLOR, kernel=1, precision=0)
     assert gname == "cobg_generic_kernel"
     C = bg.bg_build_colour_matrix(8).astype(np.longdouble)
