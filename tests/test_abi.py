@@ -50,7 +50,7 @@ def test_init_argument_errors_without_touching_kernels(bg):
         bg.bg_init(13, bg.BG_CDBG_GIVEN)
     assert e.value.code == bg.BG_EINVAL
     with pytest.raises(bg.BgError) as e:
-        bg.bg_init(9, bg.BG_COMC_GIVEN)                                        # CO_MC: (n-1)! orderings, n <= 8
+        bg.bg_init(10, bg.BG_COMC_GIVEN)                                       # CO_MC: n <= 9
     assert e.value.code == bg.BG_EUNSUPPORTED
     with pytest.raises(bg.BgError) as e:
         bg.bg_init(6, bg.BG_REC_COBG | bg.BG_HEL_SUM | bg.BG_COL_GIVEN)       # not a combination the library has
