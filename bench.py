@@ -475,7 +475,9 @@ def run_b200(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for _ in range(args.steps):
+        torch.cuda.nvtx.range_push("bg_timed_step")      # (for `ncu --nvtx --nvtx-include "bg_timed_step/"`: profiles/*.md)
         step()
+        torch.cuda.nvtx.range_pop()
     e1.record(stream)
     barrier()
     # same steps again with the library's CUDA events around the dominant (recursion) kernel, on the launching
@@ -523,7 +525,9 @@ def run_b200(args):
         g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         g0.record(stream)
         for i in range(args.steps):
+            torch.cuda.nvtx.range_push("bg_gen_step")
             gen_step(3 + i)
+            torch.cuda.nvtx.range_pop()
         g1.record(stream)
         barrier()
         gms = max_over_ranks(g0.elapsed_time(g1), world, dev)
