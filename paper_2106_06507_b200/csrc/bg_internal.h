@@ -33,6 +33,9 @@ struct bg_ctx {
     signed char* d_col;
     double* d_out;
     long long staged_events;
+    bg_ctx* alt;               // bg_eval_host, default precision of the colour-dressed path: a second context (own tables,
+                               // scratch and stream) that takes every other chunk, so that the latency-bound later stages
+                               // of one chunk overlap the first pass of the next
     // colour-class programs (CDBG, given colours)
     bg::ProgTable* prog;
     bg::CobgTable* cobg;       // sequence tables of the shared-current COBG kernel (n <= 7)
