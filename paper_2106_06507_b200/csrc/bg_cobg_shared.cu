@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(TPE > 128 ? TPE : 128, TPE > 128 ? 1 : 4) cobg
     auto load_momentum = [&](int g, double* pg) {
 #pragma unroll
         for (int c = 0; c < 4; c++) pg[c] = p.mom[(size_t)(g * 4 + c) * N + e];
-        if (p.twin & 1) rotate_frame(pg);
+        if (p.twin & 1) boost_frame(pg);
     };
 
     double total = 0.0;
