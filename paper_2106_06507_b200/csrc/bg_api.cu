@@ -142,21 +142,23 @@ static int make_prog_table(const bg_ctx* c, int G, size_t limit, bg::ProgTable**
 // an event is evaluated again in double-double arithmetic; tuned against the extended-precision oracle so that
 // no unflagged event of the test workloads is further than 1e-11 from it.
 // Ward-residual threshold of the first stage (events above it are evaluated a second time in FP64, which is cheap, so it
-// sits well below the residuals at which errors of 1e-11 were seen: DESIGN.md 3) and what the second stage may differ by
+// sits well below the residuals at which errors of 1e-11 were seen: DESIGN.md 3) and what the second stage may differ by.
+// n = 6: 3e-15, a quarter of the events - the residual of the events with an error above 1e-11 that 1e-14 left unflagged
+// (7 of 16.8e6) was 4 - 9.5e-15, and their two frames differ by 1e-11; n = 5 (13 of 8.4e6 with residuals from 8e-16): 1e-15.
 // (n >= 11, where the second evaluation runs the spill kernels: measured 3 % faster at 1e-13, worst unflagged error 8e-12)
-static double default_tau(int n) { return n <= 4 || n >= 11 ? 1e-13 : (n <= 6 ? 1e-14 : 3e-14); }
+static double default_tau(int n) { return n <= 4 || n >= 11 ? 1e-13 : (n == 5 ? 1e-15 : (n == 6 ? 3e-15 : 3e-14)); }
 static const double kDefaultTauTwin = 5e-13;
 // The second stage's bound on the Ward residuals, as a fraction of its bound on the difference of the two results: round-off
 // that both frames share (the inputs conserve momentum only to 1e-16, and the closing gluon's momentum is the one the
-// recursion never uses) shows in the residuals, not in the difference.  n = 6: no such event in 6 x 2^20; n = 5, 7: one per
-// 2^19 - 2^20 events at 1.0 - 2.3e-11 with residuals of 2.6 - 2.9e-13.
-static double twin_ward_fraction(int n) { return n == 6 ? 1.0 : 0.4; }
+// recursion never uses) shows in the residuals, not in the difference: events that passed the second stage with both
+// results off by 1.0 - 2.3e-11 had residuals of 1.2 - 4.3e-13 (n = 5, 6, 7: about one per 10^7 events).
+static double twin_ward_fraction(int n) { (void)n; return 0.4; }
 // COBG (the colour-summed |M|^2 is better conditioned than a single colour flow): second-stage bound 1e-12 on the
 // difference and on the residuals for n >= 6 (2^19 / 2^18 / 2^13 events at n = 6 / 7 / 8: 0.9 - 1.1 % left for double-double,
 // worst accepted error 4.1 / 5.2 / 0.8e-12), 5e-13 on the difference for n <= 5 (1.0 %, 4.1e-12)
 static double default_tau_twin_cobg(int n) { return n <= 5 ? 5e-13 : 1e-12; }
 static double twin_ward_fraction_cobg(int n) { return n <= 5 ? 2.0 : 1.0; }
-static double default_tau_cobg(int n) { return n <= 5 ? 3e-14 : 1e-13; }
+static double default_tau_cobg(int n) { return n <= 5 ? 1e-14 : 1e-13; }
 static const double kDefaultTauRho = 3e-3;
 
 static bool mode_supported(int n, int mode) {

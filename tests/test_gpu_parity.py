@@ -188,14 +188,14 @@ def test_conditioning_flag_reports_and_options(bg, oracle, wl):
             torch.cuda.synchronize()
             res[prec] = (out.cpu().numpy(), bg.bg_last_refined(ctx)[0], bg.bg_last_launch_count(ctx), bg.bg_last_twin(ctx))
         n_dd, n_twin = res[2][1], res[2][3]
-        assert 0 < n_dd < n_twin < 0.2 * ev.N and res[0][1] == 0 and res[0][3] == 0
+        assert 0 < n_dd < n_twin < 0.3 * ev.N and res[0][1] == 0 and res[0][3] == 0
         assert res[2][2] > res[0][2]                       # the launches of the later stages are counted
         ward, rho = res[3][0], res[4][0]
         assert np.all(ward >= 0) and np.all((rho > 0) & (rho <= 1.0 + 1e-12))
-        # the documented default rule for n = 6: Ward residual above 1e-14 -> second stage, above 5e-13 (or strong
+        # the documented default rule for n = 6: Ward residual above 3e-15 -> second stage, above 2e-13 (or strong
         # cancellation) -> double-double at once; what the second stage rejects joins those
-        hard = (ward > 5e-13 * (1 - 1e-9)) | (rho < 3e-3 * (1 + 1e-9))
-        soft = (ward > 1e-14 * (1 - 1e-9)) & ~hard
+        hard = (ward > 2e-13 * (1 - 1e-9)) | (rho < 3e-3 * (1 + 1e-9))
+        soft = (ward > 3e-15 * (1 - 1e-9)) & ~hard
         assert abs(int(soft.sum()) - n_twin) <= 2
         assert hard.sum() - 2 <= n_dd <= hard.sum() + n_twin
         changed = res[2][0] != res[0][0]
@@ -205,7 +205,7 @@ def test_conditioning_flag_reports_and_options(bg, oracle, wl):
         bg.bg_set_option(ctx, bg.BG_OPT_FLAG_TWIN, 1)
         bg.bg_eval(ctx, st, ev.N, *d, out)
         torch.cuda.synchronize()
-        assert bg.bg_last_twin(ctx) == 0 and abs(bg.bg_last_refined(ctx)[0] - int((hard | soft).sum())) <= 2   # (n = 6: both bounds 5e-13)
+        assert bg.bg_last_twin(ctx) == 0 and abs(bg.bg_last_refined(ctx)[0] - int((hard | soft).sum())) <= 2
         both = out.cpu().numpy()
         assert np.all(rel_err(res[2][0], both) <= 1e-11)
         # a huge threshold and no cancellation test: nothing is re-evaluated, the bits equal the FP64 path
@@ -239,11 +239,11 @@ def test_cobg_cascade_and_rotated_frame(bg, oracle, wl, n, N):
             return out.cpu().numpy(), bg.bg_last_refined(ctx)[0], bg.bg_last_twin(ctx)
         casc, n_dd, n_twin = run()
         assert rel_err(casc, truth).max() <= 1e-11
-        assert 0 < n_twin < 0.1 * ev.N and 0 < n_dd < 0.05 * ev.N
+        assert 0 < n_twin < 0.15 * ev.N and 0 < n_dd < 0.05 * ev.N
         bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 3)
         ward = run()[0]
         bg.bg_set_option(ctx, bg.BG_OPT_PRECISION, 2)
-        tau = 3e-14 if n <= 5 else 1e-13
+        tau = 1e-14 if n <= 5 else 1e-13
         soft = (ward > tau * (1 - 1e-9)) & (ward <= 1e-12 * (1 + 1e-9))
         assert abs(int(soft.sum()) - n_twin) <= 2 and n_dd >= int((ward > 1e-12 * (1 + 1e-9)).sum())
         bg.bg_set_option(ctx, bg.BG_OPT_FLAG_TWIN, 1)                  # no second stage

@@ -39,6 +39,9 @@ def campaign(mode, n, logN, seeds):
     for c in (ctx_t, ctx, ctx0): bg.bg_destroy(c)
     print(f"{'CDBG' if cdbg else 'COBG'} n={n}: {tot} events ({len(seeds)} x 2^{logN}); default path: {over} over 1e-11 {over_list}, worst {worst:.2e}; second FP64 {tw/tot*100:.2f} %, double-double {dd/tot*100:.2f} %; FP64 alone: {over0} over 1e-11, worst {worst0:.2e}", flush=True)
 C, O = bg.BG_CDBG_GIVEN, bg.BG_COBG_HELGIVEN_FULLCOLOR
+if len(sys.argv) > 1:         # python tests/validate_precision.py cdbg|cobg n log2N seeds
+    campaign(C if sys.argv[1] == "cdbg" else O, int(sys.argv[2]), int(sys.argv[3]), range(101, 101 + int(sys.argv[4])))
+    sys.exit(0)
 campaign(C, 6, 20, range(101, 117)); campaign(C, 5, 20, range(101, 109)); campaign(C, 7, 19, range(101, 109)); campaign(C, 8, 18, range(101, 109))
 campaign(C, 9, 17, range(101, 109)); campaign(C, 10, 16, range(101, 105)); campaign(C, 11, 14, range(101, 103)); campaign(C, 12, 13, range(101, 103)); campaign(C, 4, 20, range(101, 105))
 campaign(O, 5, 20, range(101, 105)); campaign(O, 6, 19, range(101, 109)); campaign(O, 7, 18, range(101, 109)); campaign(O, 8, 13, range(101, 105))
