@@ -684,6 +684,31 @@ def test_batch_size_guard(bg):
         bg.bg_destroy(ctx)
 
 
+@pytest.mark.parametrize("n,N", [(6, (1 << 17) + 77), (7, 140001)])
+def test_host_path_two_lanes_matches_device_path(bg, wl, n, N):
+    """bg_eval_host under the default precision splits large batches into chunks that two contexts evaluate on two
+    streams (the later stages of one chunk overlap the first pass of the next).  Every stage works event by event, so the
+    result is bitwise that of one bg_eval over the whole batch - also when the same context is used again."""
+    ev = wl.config_events(4, N=N, n=n)
+    a, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
+    b, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN, host=True)
+    assert np.array_equal(a, b)
+    mom, hel, col = wl.to_soa(mom=ev.mom), wl.to_soa(hel=ev.hel), wl.to_soa(col=ev.col)
+    ctx = bg.bg_init(n, bg.BG_CDBG_GIVEN)
+    try:
+        for _ in range(2):
+            out = np.full(N, np.nan)
+            bg.bg_eval_host(ctx, N, mom, hel, col, out)
+            assert np.array_equal(out, a)
+        half = N // 2 + 1                                   # a smaller batch afterwards: one lane, compact views
+        out = np.full(half, np.nan)
+        sub = ev.head(half)
+        bg.bg_eval_host(ctx, half, wl.to_soa(mom=sub.mom), wl.to_soa(hel=sub.hel), wl.to_soa(col=sub.col), out)
+        assert np.array_equal(out, a[:half])
+    finally:
+        bg.bg_destroy(ctx)
+
+
 def test_host_path_matches_device_path(bg, wl):
     ev = wl.config_events(1, N=5000)
     a, _ = gpu_eval(ev, bg.BG_CDBG_GIVEN)
