@@ -132,6 +132,10 @@ struct ProgParams {
     double td;                 // tau_twin as the bound on |w - w'| / w
     uint32_t* soft_list;       // [N] first stage: events for the second stage, by record position, per tier like flag_list
     uint32_t* soft_count;      // [kTiers]
+    // Ordered lists (warp-shared lane counts, large batches): the kernels only mark the events - mark[record position] =
+    // 1 second stage, 2 double-double, 3 rejected by the second stage - and a compaction kernel builds the lists in
+    // record order, i.e. class by class: the events a warp takes from a list then run the same program
+    uint8_t* mark;             // nullptr: the kernels append to the lists themselves (one atomic per flagged event)
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -807,6 +811,7 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
             if (g == 0 && have) {
                 const double w = valid ? s_norm2(amp) : 0.0;
                 if (!(kWard && (p.twin & 2))) p.out[e] = w;      // (second stage of the cascade: out[e] keeps the first result)
+                if (kWard && p.mark && p.tau2 > 0.0 && !(p.twin & 2)) p.mark[idx] = 0;
                 if constexpr (kWard) {
                     if (p.tau2 < 0.0 && valid) {
                         // diagnostic (BG_OPT_PRECISION = 3): the Ward residual itself instead of |A|^2
@@ -829,7 +834,10 @@ __global__ void __launch_bounds__(G > 32 ? G : 32) cdbg_prog_kernel(const ProgPa
                         } else if (!hard) {
                             to_twin = !(ward2 <= p.tau2 * scale);      // (tau_twin <= tau: never - no second stage)
                         }
-                        if (to_dd) {
+                        if (p.mark) {
+                            if (to_dd) p.mark[idx] = (p.twin & 2) ? 3 : 2;
+                            else if (to_twin) p.mark[idx] = 1;
+                        } else if (to_dd) {
                             const uint32_t at = atomicAdd(p.flag_count + tier, 1u);
                             BG_CHECK(first + at < (long long)p.bounds[tier + 1]);
                             p.flag_list[first + at] = (uint32_t)idx;

@@ -22,6 +22,7 @@
 // different 16-byte bank groups when events share a warp.  With SPILL, offsets beyond the slab live in an
 // L2-resident global slab of the block.  For G >= 8 a per-lane ring behind the slab receives the ops by cp.async.
 #include <algorithm>
+#include <cstdio>
 #include <cstring>
 #include <new>
 #include <atomic>
@@ -729,13 +730,15 @@ int prog_dd_mode(const ProgTable* t) { return t ? t->dd_mode : -1; }
 
 // scratch: records (32 + 32 n) B x N | perm u64[N] | cls u32[N] | hist u32[num_classes + 1] | tier bounds (64 B) |
 //          flag counters (64 B: double-double list counts | its tickets | second-stage list counts | its tickets) |
-//          double-double list u32[N] | second-stage list u32[N] | spill slabs (FP64) | spill slabs (capped FP64 launches
+//          double-double list u32[N] | second-stage list u32[N] | marks u8[N] | spill slabs (FP64) | spill slabs (capped FP64 launches
 //          and double-double re-evaluation)
 static size_t prog_flag_offset(const ProgTable* t, long long N) {
     return ((size_t)N * (12 + t->rec_bytes) + ((size_t)t->num_classes + 1) * 4 + 15) / 16 * 16 + 64;
 }
 static size_t prog_spill_offset(const ProgTable* t, long long N) {
-    return (prog_flag_offset(t, N) + 64 + (size_t)N * 8 + 255) / 256 * 256;
+    // counters | two lists | marks | work area of the list compaction
+    const size_t lists_end = (prog_flag_offset(t, N) + 64 + (size_t)N * 9 + 15) / 16 * 16;
+    return (lists_end + 64 + ((size_t)N / 4096 + 8) * 8 + 255) / 256 * 256;
 }
 static size_t prog_spill_bytes(const ProgTable* t) {
     // spill kernels run a fixed number of blocks per SM, each with a slab for the largest state
@@ -825,6 +828,122 @@ static cudaError_t dispatch_interp(cudaStream_t s, const ProgTable* t, int sm_co
     return err;
 }
 
+// Ordered flag lists: the interpreter marked the events (ProgParams::mark); two small kernels append the record
+// positions with mark `want_a` to list_a and those with `want_b` to list_b (nullptr: none) behind what the lists hold, tier
+// by tier, in record order: (1) counts per chunk of kCompactChunk records, (2) every chunk adds up the counts of the
+// chunks before it in its tier and places its entries.  Records are sorted by class, longest programs first, so the
+// events one warp of a list launch takes share a class, and the tickets hand out the longest tasks first.
+constexpr int kCompactThreads = 256, kCompactPer = 16, kCompactChunk = kCompactThreads * kCompactPer;
+struct CompactWork {            // behind the marks in the scratch buffer
+    uint32_t start[2][kTiers];  // list lengths before this compaction
+    uint32_t counts[1][2];      // [chunks][2]: entries of a chunk for list a, b
+};
+__device__ __forceinline__ bool compact_chunk_of_block(const uint32_t* bounds, int* tier_out, uint32_t* chunk_out) {
+    int tier = 0;
+    uint32_t chunk = blockIdx.x;
+    for (; tier < kTiers; tier++) {
+        const uint32_t chunks = (bounds[tier + 1] - bounds[tier] + kCompactChunk - 1) / kCompactChunk;
+        if (chunk < chunks) break;
+        chunk -= chunks;
+    }
+    *tier_out = tier; *chunk_out = chunk;
+    return tier < kTiers;
+}
+__device__ __forceinline__ void compact_bits(const uint8_t* mark, uint32_t begin, uint32_t end, int want_a, int want_b, unsigned* bits_a,
+                                             unsigned* bits_b) {
+    unsigned a = 0, b = 0;
+#pragma unroll
+    for (int i = 0; i < kCompactPer; i++) {
+        const uint32_t pos = begin + i;
+        const int m = pos < end ? (int)mark[pos] : 0;
+        a |= (unsigned)(m == want_a) << i;
+        b |= (unsigned)(want_b >= 0 && m == want_b) << i;
+    }
+    *bits_a = a; *bits_b = b;
+}
+__global__ void __launch_bounds__(kCompactThreads)
+cdbg_compact_count_kernel(const uint8_t* __restrict__ mark, const uint32_t* __restrict__ bounds, int want_a, const uint32_t* __restrict__ count_a,
+                          int want_b, const uint32_t* __restrict__ count_b, CompactWork* __restrict__ work) {
+    if (blockIdx.x == 0 && threadIdx.x < kTiers) {
+        work->start[0][threadIdx.x] = count_a[threadIdx.x];
+        work->start[1][threadIdx.x] = want_b >= 0 ? count_b[threadIdx.x] : 0u;
+    }
+    int tier; uint32_t chunk;
+    if (!compact_chunk_of_block(bounds, &tier, &chunk)) {
+        if (threadIdx.x == 0) { work->counts[blockIdx.x][0] = 0; work->counts[blockIdx.x][1] = 0; }
+        return;
+    }
+    unsigned bits_a, bits_b;
+    compact_bits(mark, bounds[tier] + chunk * kCompactChunk + threadIdx.x * kCompactPer, bounds[tier + 1], want_a, want_b, &bits_a, &bits_b);
+    unsigned x = (unsigned)__popc(bits_a) | ((unsigned)__popc(bits_b) << 16);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) x += __shfl_xor_sync(0xFFFFFFFFu, x, d);
+    __shared__ unsigned warp_tot[kCompactThreads / 32];
+    if ((threadIdx.x & 31) == 0) warp_tot[threadIdx.x >> 5] = x;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned total = 0;
+        for (int w = 0; w < kCompactThreads / 32; w++) total += warp_tot[w];
+        work->counts[blockIdx.x][0] = total & 0xFFFFu;
+        work->counts[blockIdx.x][1] = total >> 16;
+    }
+}
+__global__ void __launch_bounds__(kCompactThreads)
+cdbg_compact_place_kernel(const uint8_t* __restrict__ mark, const uint32_t* __restrict__ bounds, int want_a, uint32_t* __restrict__ list_a,
+                          uint32_t* __restrict__ count_a, int want_b, uint32_t* __restrict__ list_b, uint32_t* __restrict__ count_b,
+                          const CompactWork* __restrict__ work) {
+    int tier; uint32_t chunk;
+    if (!compact_chunk_of_block(bounds, &tier, &chunk)) return;
+    const uint32_t first = bounds[tier], end = bounds[tier + 1];
+    const uint32_t begin = first + chunk * kCompactChunk + threadIdx.x * kCompactPer;
+    unsigned bits_a, bits_b;
+    compact_bits(mark, begin, end, want_a, want_b, &bits_a, &bits_b);
+    // entries of the chunks before this one in the tier (a few hundred chunks at most per 2^20 events)
+    __shared__ unsigned warp_tot[kCompactThreads / 32], base_a, base_b;
+    unsigned pa = 0, pb = 0;
+    for (uint32_t c = threadIdx.x; c < chunk; c += kCompactThreads) {
+        pa += work->counts[blockIdx.x - chunk + c][0];
+        pb += work->counts[blockIdx.x - chunk + c][1];
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) { pa += __shfl_xor_sync(0xFFFFFFFFu, pa, d); pb += __shfl_xor_sync(0xFFFFFFFFu, pb, d); }
+    __shared__ unsigned part_a[kCompactThreads / 32], part_b[kCompactThreads / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) { part_a[warp] = pa; part_b[warp] = pb; }
+    // block-wide exclusive scan of this chunk's own counts (packed: a in the low, b in the high half)
+    const unsigned mine = (unsigned)__popc(bits_a) | ((unsigned)__popc(bits_b) << 16);
+    unsigned x = mine;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned y = __shfl_up_sync(0xFFFFFFFFu, x, d);
+        if (lane >= d) x += y;
+    }
+    if (lane == 31) warp_tot[warp] = x;
+    __syncthreads();
+    unsigned before = x - mine, total = 0;
+    for (int w = 0; w < kCompactThreads / 32; w++) {
+        if (w < warp) before += warp_tot[w];
+        total += warp_tot[w];
+    }
+    if (threadIdx.x == 0) {
+        unsigned a = work->start[0][tier], b = work->start[1][tier];
+        for (int w = 0; w < kCompactThreads / 32; w++) { a += part_a[w]; b += part_b[w]; }
+        base_a = a; base_b = b;
+        const uint32_t chunks = (end - first + kCompactChunk - 1) / kCompactChunk;
+        if (chunk + 1 == chunks) {       // the last chunk of the tier knows the new lengths
+            count_a[tier] = a + (total & 0xFFFFu);
+            if (want_b >= 0) count_b[tier] = b + (total >> 16);
+        }
+    }
+    __syncthreads();
+    uint32_t at_a = first + base_a + (before & 0xFFFFu), at_b = first + base_b + (before >> 16);
+#pragma unroll
+    for (int i = 0; i < kCompactPer; i++) {
+        if ((bits_a >> i) & 1u) list_a[at_a++] = begin + i;
+        if ((bits_b >> i) & 1u) list_b[at_b++] = begin + i;
+    }
+}
+
 // the UNSORTED path: discrete states, at most 4 lanes per event, every class in the one (last) tier, and a batch small
 // enough for the launches saved to outweigh the divergence of unsorted warps (measured, FP64 kernels: n = 4 2^12 ... 2^17
 // events 32 -> 16, 32 -> 18, 42 -> 35, 56 -> 53 us, 2^18 93 -> 96 us; n = 5 2^10 ... 2^15 36 -> 21, 36 -> 23, 42 -> 35,
@@ -868,7 +987,7 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         p.tau_rho = 0.0;
         p.flag_list = nullptr; p.flag_count = nullptr; p.list = nullptr; p.list_count = nullptr; p.ticket = nullptr;
         p.twin = rotated ? 1 : 0;
-        p.tw2 = 0.0; p.td = 0.0; p.soft_count = nullptr; p.soft_list = nullptr;
+        p.tw2 = 0.0; p.td = 0.0; p.soft_count = nullptr; p.soft_list = nullptr; p.mark = nullptr;
         *launches = 0;
         if (ev0) cudaEventRecord(ev0, s);
         err = dispatch_interp(s, t, sm_count, p, launches);
@@ -957,9 +1076,24 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.td = tau_twin;
     p.soft_count = flag_count + 2 * kTiers;
     p.soft_list = flag_list + N;
+    // Ordered lists for warp-shared lane counts (n <= 7) from 2^17 events: the kernels mark, a compaction kernel builds the
+    // lists class by class, and the warps of the later stages run 8 (4) events of ONE class instead of 8 arbitrary ones -
+    // and the tickets hand out the longest programs first: double-double stage 0.76 -> 0.65 ms (n = 6, 2^20 events), 0.93 ->
+    // 0.72 ms (n = 7, 2^18), 0.23 -> 0.20 ms (n = 5, 2^20), four small launches included.
+    // Small batches (later stages one task deep) and block-per-event lane counts keep the atomic appends.
+    const bool ordered = tau > 0.0 && t->G <= 8 && N >= (1ll << 17);
+    uint8_t* const mark = reinterpret_cast<uint8_t*>(flag_list + 2 * N);
+    CompactWork* const work = reinterpret_cast<CompactWork*>(reinterpret_cast<char*>(flag_count) + ((size_t)64 + (size_t)N * 9 + 15) / 16 * 16);
+    p.mark = ordered ? mark : nullptr;
+    const unsigned compact_blocks = (unsigned)((N + kCompactChunk - 1) / kCompactChunk + kTiers);
     *launches = fused ? 2 : 3;
     if (ev0) cudaEventRecord(ev0, s);
     err = dispatch_interp(s, t, sm_count, p, launches, true);
+    if (ordered && err == cudaSuccess) {
+        cdbg_compact_count_kernel<<<compact_blocks, kCompactThreads, 0, s>>>(mark, bounds, 1, p.soft_count, 2, flag_count, work);
+        cdbg_compact_place_kernel<<<compact_blocks, kCompactThreads, 0, s>>>(mark, bounds, 1, p.soft_list, p.soft_count, 2, flag_list, flag_count, work);
+        *launches += 2;
+    }
     if (tau > 0.0 && ev_mid) cudaEventRecord(ev_mid, s);
     if (cascade && err == cudaSuccess) {
         // second stage: the events between the two thresholds once more in FP64, in the rotated frame; out[] keeps the
@@ -973,6 +1107,11 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         // (n >= 11: -1 ... -5 %); 128 lanes without spill (n = 10) keep the tiers' own launch shapes (+2 %).
         const bool merged = t->spill || (t->G <= 4 ? N >= (1ll << 18) : t->G <= 64);
         err = dispatch_interp(s, t, sm_count, p, launches, true, std::max<long long>(1, N / 16), merged);
+        if (ordered && err == cudaSuccess) {     // what the second stage rejected, behind the first stage's own double-double list
+            cdbg_compact_count_kernel<<<compact_blocks, kCompactThreads, 0, s>>>(mark, bounds, 3, flag_count, -1, nullptr, work);
+            cdbg_compact_place_kernel<<<compact_blocks, kCompactThreads, 0, s>>>(mark, bounds, 3, flag_list, flag_count, -1, nullptr, nullptr, work);
+            *launches += 2;
+        }
     }
     if (tau > 0.0 && err == cudaSuccess) {
         // the flagged events of every tier once more, in double-double arithmetic (overwrites their out[])
@@ -1014,7 +1153,7 @@ cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, 
     p.tau_rho = 0.0;
     p.flag_list = nullptr; p.flag_count = nullptr; p.list = nullptr; p.list_count = nullptr; p.ticket = nullptr;
     p.mom = nullptr; p.hel = nullptr; p.col = nullptr;
-    p.twin = 0; p.tw2 = 0.0; p.td = 0.0; p.soft_list = nullptr; p.soft_count = nullptr;
+    p.twin = 0; p.tw2 = 0.0; p.td = 0.0; p.soft_list = nullptr; p.soft_count = nullptr; p.mark = nullptr;
     *launches = 1;
     if (ev0) cudaEventRecord(ev0, s);
     err = dispatch_interp(s, t, sm_count, p, launches, false);
