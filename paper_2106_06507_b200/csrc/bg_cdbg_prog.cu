@@ -1076,12 +1076,13 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     p.td = tau_twin;
     p.soft_count = flag_count + 2 * kTiers;
     p.soft_list = flag_list + N;
-    // Ordered lists for warp-shared lane counts (n <= 7) from 2^17 events: the kernels mark, a compaction kernel builds the
-    // lists class by class, and the warps of the later stages run 8 (4) events of ONE class instead of 8 arbitrary ones -
+    // Ordered lists from 2^16 events: the kernels mark, a compaction kernel builds the lists class by class, and with
+    // warp-shared lane counts (n <= 7) the warps of the later stages run 8 (4) events of ONE class instead of 8 arbitrary ones -
     // and the tickets hand out the longest programs first: double-double stage 0.76 -> 0.65 ms (n = 6, 2^20 events), 0.93 ->
-    // 0.72 ms (n = 7, 2^18), 0.23 -> 0.20 ms (n = 5, 2^20), four small launches included.
-    // Small batches (later stages one task deep) and block-per-event lane counts keep the atomic appends.
-    const bool ordered = tau > 0.0 && t->G <= 8 && N >= (1ll << 17);
+    // 0.72 ms (n = 7, 2^18), 0.23 -> 0.20 ms (n = 5, 2^20), four small launches included; block-per-event lane counts
+    // gain the ticket order only (n = 8, 9: -2 ... -3 % of the step, n >= 10: equal).  Smaller batches (later stages one
+    // task deep) keep the atomic appends.
+    const bool ordered = tau > 0.0 && N >= (1ll << 16);
     uint8_t* const mark = reinterpret_cast<uint8_t*>(flag_list + 2 * N);
     CompactWork* const work = reinterpret_cast<CompactWork*>(reinterpret_cast<char*>(flag_count) + ((size_t)64 + (size_t)N * 9 + 15) / 16 * 16);
     p.mark = ordered ? mark : nullptr;
