@@ -1090,12 +1090,12 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
     *launches = fused ? 2 : 3;
     if (ev0) cudaEventRecord(ev0, s);
     err = dispatch_interp(s, t, sm_count, p, launches, true);
+    if (tau > 0.0 && ev_mid) cudaEventRecord(ev_mid, s);      // (the list building counts as part of the later stages)
     if (ordered && err == cudaSuccess) {
         cdbg_compact_count_kernel<<<compact_blocks, kCompactThreads, 0, s>>>(mark, bounds, 1, p.soft_count, 2, flag_count, work);
         cdbg_compact_place_kernel<<<compact_blocks, kCompactThreads, 0, s>>>(mark, bounds, 1, p.soft_list, p.soft_count, 2, flag_list, flag_count, work);
         *launches += 2;
     }
-    if (tau > 0.0 && ev_mid) cudaEventRecord(ev_mid, s);
     if (cascade && err == cudaSuccess) {
         // second stage: the events between the two thresholds once more in FP64, in the rotated frame; out[] keeps the
         // first result, and what disagrees joins the double-double list
