@@ -23,6 +23,7 @@
 // L2-resident global slab of the block.  For G >= 8 a per-lane ring behind the slab receives the ops by cp.async.
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <atomic>
@@ -375,7 +376,7 @@ static void enumerate_counts(int t, int r, int* counts, std::vector<std::vector<
     }
 }
 
-int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** out) {
+int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** out, const ProgTable* like) {
     if (slab_limit == 0 || slab_limit > kMaxSlabBytes) slab_limit = kMaxSlabBytes;
     *out = nullptr;
     if (n < 4 || n > kMaxN || (G != 1 && G != 2 && G != 4 && G != 8 && G != 16 && G != 32 && G != 64 && G != 128 && G != 256)) return BG_EINVAL;
@@ -399,7 +400,7 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
         auto worker = [&]() {
             for (long long r = next_class.fetch_add(1); r < nc; r = next_class.fetch_add(1))
                 if (!comc) {
-                    build_class(n, G, all[r].data(), progs[r]);
+                    build_class(n, G, all[r].data(), progs[r], like ? (int)like->h_closure[r] : -1);
                 } else {
                     // CO_MC: canonical order = codes ascending; only classes with balanced colour charges can be non-zero
                     const int* cnt = all[r].data();
@@ -543,6 +544,13 @@ int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** ou
     if (!t) return BG_ENOMEM;
     std::memset(t, 0, sizeof(*t));
     t->n = n; t->G = G; t->num_classes = nc; t->max_state_cx = max_state; t->tiers = tiers;
+    if (like) {    // a table for the list launches of another table's records: its tier ranges, one slab size
+        t->tiers = like->tiers;
+        for (int k = 0; k < kTiers; k++) t->tiers.slab_cx[k] = std::max(16, max_state);
+    }
+    t->h_closure = static_cast<uint8_t*>(std::malloc((size_t)nc));
+    if (!t->h_closure) { delete t; return BG_ENOMEM; }
+    for (long long r = 0; r < nc; r++) t->h_closure[r] = info[r].closure_code;
     t->dense = false;
     t->rec_bytes = kRecHeaderBytes + 32 * n;
     t->spill = spill;
@@ -713,6 +721,8 @@ cdbg_pack_continuous_kernel(int n, long long N, const double* __restrict__ mom, 
 
 void prog_table_destroy(ProgTable* t) {
     if (!t) return;
+    if (t->dd_table) prog_table_destroy(t->dd_table);
+    std::free(t->h_closure);
     if (t->d_small) cudaFree(t->d_small);
     if (t->has_streams) {
         for (int i = 0; i < kTiers - 1; i++) { cudaStreamDestroy(t->aux[i]); cudaEventDestroy(t->join_ev[i]); }
@@ -746,7 +756,11 @@ static size_t prog_spill_bytes(const ProgTable* t) {
 }
 size_t prog_scratch_bytes(const ProgTable* t, long long N) {
     const size_t epw = t->G >= 32 ? 1 : 32 / t->G;
-    const size_t dd_spill = t->dd_mode == 1 ? (size_t)t->dd_max_blocks * epw * t->max_state_cx * 32 : 0;
+    size_t dd_spill = t->dd_mode == 1 ? (size_t)t->dd_max_blocks * epw * t->max_state_cx * 32 : 0;
+    if (const ProgTable* d = t->dd_table) {
+        const size_t depw = d->G >= 32 ? 1 : 32 / d->G;
+        if (d->dd_mode == 1) dd_spill = std::max(dd_spill, (size_t)d->dd_max_blocks * depw * d->max_state_cx * 32);
+    }
     // the slabs of the capped FP64 launches share the region of the re-evaluation's (which runs after them)
     const size_t cap_spill = t->cap_cx > 0 ? (size_t)t->sm_count * t->cap_blocks * epw * t->max_state_cx * 16 : 0;
     return prog_spill_offset(t, N) + prog_spill_bytes(t) + std::max(dd_spill, cap_spill);
@@ -1125,10 +1139,17 @@ cudaError_t cdbg_prog_launch(cudaStream_t s, const ProgTable* t, int sm_count, l
         // few flagged events per tier for batches up to 2^19: the tier launches overlap their ramp-up and tails
         // one launch walks the lists of all tiers (their capped shared state has one size): few tasks per tier, each
         // 14 x an FP64 task, so per-tier launches were mostly tails (n = 6, 2^20 events: 1.15 -> 0.80 ms after the first pass)
-        err = dispatch_interp_dd(s, t, sm_count, p, launches, false, true, std::max<long long>(1, N / 32));
+        const ProgTable* d = t->dd_table && t->dd_table->dd_mode == 1 ? t->dd_table : t;     // (n = 8, 9: half the lanes)
+        p.info = d->d_info; p.ops = d->d_ops; p.spill_cx = d->max_state_cx;
+        err = dispatch_interp_dd(s, d, sm_count, p, launches, false, true, std::max<long long>(1, N / 32));
     }
     if (ev1) cudaEventRecord(ev1, s);
     return err;
+}
+
+void prog_table_attach_dd(ProgTable* t, ProgTable* dd) {
+    if (t->dd_table) prog_table_destroy(t->dd_table);
+    t->dd_table = dd;
 }
 
 cudaError_t cdbg_dense_launch(cudaStream_t s, const ProgTable* t, int sm_count, long long N, const double* mom,

@@ -82,10 +82,12 @@ cudaError_t cobg_dd_launch(cudaStream_t s, int n, bool helsum, int nperm, const 
                            long long count, const double* mom, const signed char* hel, double* out, void* scratch);
 
 // ---- colour-class program interpreter (bg_cdbg_prog.cu): G lanes per event, currents in shared memory -------
-int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** out);   // BG_* code; slab_limit 0 = all of
+// `like`: a second table for the list launches of that table's records (same closure legs, its tier ranges)
+int prog_table_create(int n, int G, size_t slab_limit, bool comc, ProgTable** out, const ProgTable* like = nullptr);   // BG_* code; slab_limit 0 = all of
                                                                                        // shared memory; comc: Eq. 19 programs
 int prog_table_create_dense(int n, int G, size_t slab_limit, bool real, ProgTable** out);   // continuous states
 void prog_table_destroy(ProgTable* t);
+void prog_table_attach_dd(ProgTable* t, ProgTable* dd);    // t takes ownership; the double-double stage then runs dd's programs
 size_t prog_state_bytes(const ProgTable* t);               // largest per-event state block
 int prog_lanes(const ProgTable* t);
 size_t prog_scratch_bytes(const ProgTable* t, long long N);

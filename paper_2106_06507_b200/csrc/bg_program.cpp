@@ -479,7 +479,7 @@ void build_program(int n, int G, const int* code, ClassProgram& out, bool dense,
     out.state_cx = next + scratch_max;
 }
 
-void build_class(int n, int G, const int* counts, ClassProgram& out) {
+void build_class(int n, int G, const int* counts, ClassProgram& out, int closure) {
     out = ClassProgram();
     // the colour charges must cancel over all n gluons (as many i = c as j = c for every colour c)
     for (int c = 0; c < 3; c++) {
@@ -495,7 +495,7 @@ void build_class(int n, int G, const int* counts, ClassProgram& out) {
     int trials = 0;
     bool have = false;
     for (int c = 0; c < kNumCodes && trials < max_trials; c++) {
-        if (!counts[c]) continue;
+        if (!counts[c] || (closure >= 0 && c != closure)) continue;
         trials++;
         int code[kMaxN], k = 0;
         for (int t = 0; t < kNumCodes; t++)

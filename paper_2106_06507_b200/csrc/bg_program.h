@@ -75,7 +75,8 @@ void build_program(int n, int G, const int* code, ClassProgram& out, bool dense 
 // CO_MC (Eq. 19 with colour-ordered currents): program for canonical colour codes; classes with more than
 // max_orderings colour-connected orderings are left invalid with state_cx = -1 (unsupported, not zero).
 void build_comc_program(int n, int G, const int* code, ClassProgram& out, long long max_orderings = 20000);
-// Build the best program (over the choice of closure leg) for a multiset of colour codes.
-void build_class(int n, int G, const int* counts, ClassProgram& out);
+// Build the best program (over the choice of closure leg) for a multiset of colour codes; closure >= 0: with the gluon
+// of that colour code as the closure leg (a second table for the same event records).
+void build_class(int n, int G, const int* counts, ClassProgram& out, int closure = -1);
 
 }  // namespace bg
