@@ -68,7 +68,8 @@ enum {
 enum {
     BG_OPT_KERNEL = 1,       /* 0 = automatic choice by n; 1 = generic thread-per-event kernels with currents in
                                 global scratch (any n); 2 = colour-class program interpreter, currents in shared
-                                memory (BG_CDBG_GIVEN, any n; COBG n <= 7) */
+                                memory (BG_CDBG_GIVEN, any n; COBG n <= 8).  BG_CDBG_CONTINUOUS: 1 = the interpreter in
+                                complex instead of real arithmetic (rebuilds the program table, synchronises) */
     BG_OPT_SCRATCH_LIMIT = 2,/* upper bound in bytes for the scratch the generic kernels may use (default 16 GiB) */
     BG_OPT_LANES = 3,        /* lanes that cooperate on one event in the program interpreter: 1, 2, 4, ..., 256;
                                 0 = automatic.  Rebuilds the class programs (synchronises the device).  With few lanes

@@ -390,6 +390,18 @@ int bg_set_option(bg_ctx* c, int key, long long value) {
         case BG_OPT_KERNEL:
             if (value < 0 || value > 2) return BG_EINVAL;
             if (value == 2 && !c->prog && !c->cobg) return BG_EUNSUPPORTED;
+            if (c->mode == BG_CDBG_CONTINUOUS && c->prog && ((int)value == 1) != (c->kernel_opt == 1)) {
+                // continuous states: real or complex arithmetic is a property of the program table (element size, offsets)
+                const int before = c->kernel_opt;
+                c->kernel_opt = (int)value;
+                cudaDeviceSynchronize();
+                bg::ProgTable* t = nullptr;
+                const int rc = make_prog_table(c, c->prog_lanes, c->slab_limit, &t);
+                if (rc != BG_OK) { c->kernel_opt = before; return rc; }
+                bg::prog_table_destroy(c->prog);
+                c->prog = t;
+                return BG_OK;
+            }
             c->kernel_opt = (int)value;
             return BG_OK;
         case BG_OPT_LANES: {

@@ -469,9 +469,10 @@ def test_continuous_colour_and_polarisation_states(bg, oracle, wl, n, N, lanes, 
     d_out = torch.full((N,), float("nan"), dtype=torch.float64, device=dev)
     ctx = bg.bg_init(n, bg.BG_CDBG_CONTINUOUS)
     try:
-        if arith == "complex":      # BG_OPT_KERNEL = 1: the same program in complex arithmetic (rebuilt by LANES)
+        if arith == "complex":      # BG_OPT_KERNEL = 1: the same program in complex arithmetic (the table is rebuilt)
             bg.bg_set_option(ctx, bg.BG_OPT_KERNEL, 1)
-            bg.bg_set_option(ctx, bg.BG_OPT_LANES, lanes or 0)
+            if lanes:
+                bg.bg_set_option(ctx, bg.BG_OPT_LANES, lanes)
         elif lanes:
             bg.bg_set_option(ctx, bg.BG_OPT_LANES, lanes)
         bg.bg_reserve(ctx, N)
