@@ -577,9 +577,9 @@ cudaError_t cobg_shared_launch(cudaStream_t s, const CobgTable* t, bool helsum, 
         // threads per event (full colour), measured on 2^19 / 2^19 / 2^18 events: n = 5: 8 -> 4: 0.71 -> 0.64 ms; n = 6: 32 -> 16 -> 8:
         // 5.69 -> 4.45 -> 4.23 ms; n = 7: 128 -> 64: 16.2 -> 15.4 ms (32: 19.6 ms); n = 8: 256 (128: 6.8 -> 10.7 ms).  Fewer
         // threads take several orderings each in rounds and more events share a block: fewer idle threads at the barriers
-        // of the shared levels.  Summed helicities and leading colour keep the round-1 values.
+        // of the shared levels.  Leading colour, n = 6: 32 -> 8: 2.75 -> 2.27 ms for 2^16 events; summed helicities keep the round-1 values.
         case 5: return lc ? launch_cobg<5, 8, true>(s, p) : (helsum ? launch_cobg<5, 8, false>(s, p) : launch_cobg<5, 4, false>(s, p));
-        case 6: return lc ? launch_cobg<6, 32, true>(s, p) : (helsum ? launch_cobg<6, 32, false>(s, p) : launch_cobg<6, 8, false>(s, p));
+        case 6: return lc ? launch_cobg<6, 8, true>(s, p) : (helsum ? launch_cobg<6, 32, false>(s, p) : launch_cobg<6, 8, false>(s, p));
         case 7: return lc ? launch_cobg<7, 128, true>(s, p) : (helsum ? launch_cobg<7, 128, false>(s, p) : launch_cobg<7, 64, false>(s, p));
         case 8: return lc ? launch_cobg<8, 256, true>(s, p) : launch_cobg<8, 256, false>(s, p);
         default: return cudaErrorNotSupported;
