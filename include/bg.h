@@ -93,12 +93,12 @@ enum {
                                 evaluated by a double-double instantiation of the same kernel.  3, 4 = diagnostics: `out`
                                 receives the Ward residual / the cancellation ratio instead of |M|^2. */
     BG_OPT_FLAG_THRESHOLD = 7,/* Ward-residual threshold in units of 1e-18 (0 = default; BG_CDBG_GIVEN: 1e-13 for n = 4 and
-                                n >= 11, 1e-15 for n = 5, 3e-15 for n = 6, 3e-14 for n = 7 .. 10; COBG: 1e-14 for n <= 5, else 1e-13) */
+                                n >= 11, 1e-15 for n = 5, 3e-15 for n = 6, 1e-14 for n = 7, 8, 3e-14 for n = 9, 10; COBG: 3e-15 for n <= 5,
+                                else 3e-14) */
     BG_OPT_FLAG_CANCELLATION = 8, /* cancellation threshold in units of 1e-6 (0 = default: 3e-3) */
     BG_OPT_FLAG_TWIN = 9,    /* bound of the second stage in units of 1e-18 on |w - w'| / w of the two evaluations (0 = default:
                                 BG_CDBG_GIVEN 5e-13; COBG 5e-13 for n <= 5, else 1e-12).  The Ward residual of either may not
-                                exceed 0.4 times that number (BG_CDBG_GIVEN), the same number (COBG n >= 6) or twice it (COBG
-                                n <= 5).  With that residual bound at or below BG_OPT_FLAG_THRESHOLD
+                                exceed 0.4 times that number (BG_CDBG_GIVEN, COBG n <= 5) or the same number (COBG n >= 6).  With that residual bound at or below BG_OPT_FLAG_THRESHOLD
                                 there is no second stage and every flagged event is evaluated in double-double */
     BG_OPT_FRAME = 10,       /* BG_CDBG_GIVEN (program interpreter) and the COBG modes (shared-current kernel): 1 = evaluate
                                 every event in the rotated frame of the second stage (fixed rotation, axis (1,2,3), 1 rad) -

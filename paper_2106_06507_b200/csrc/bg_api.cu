@@ -146,7 +146,8 @@ static int make_prog_table(const bg_ctx* c, int G, size_t limit, bg::ProgTable**
 // n = 6: 3e-15, a quarter of the events - the residual of the events with an error above 1e-11 that 1e-14 left unflagged
 // (7 of 16.8e6) was 4 - 9.5e-15, and their two frames differ by 1e-11; n = 5 (13 of 8.4e6 with residuals from 8e-16): 1e-15.
 // (n >= 11, where the second evaluation runs the spill kernels: measured 3 % faster at 1e-13, worst unflagged error 8e-12)
-static double default_tau(int n) { return n <= 4 || n >= 11 ? 1e-13 : (n == 5 ? 1e-15 : (n == 6 ? 3e-15 : 3e-14)); }
+// (n = 7, 8: 1e-14 - two unflagged events each in 16.8e6 / 8.4e6 with residuals of 2.4 - 2.9e-14; none at n = 9, 10 in 4.2e6 / 1.0e6)
+static double default_tau(int n) { return n <= 4 || n >= 11 ? 1e-13 : (n == 5 ? 1e-15 : (n == 6 ? 3e-15 : (n <= 8 ? 1e-14 : 3e-14))); }
 static const double kDefaultTauTwin = 5e-13;
 // The second stage's bound on the Ward residuals, as a fraction of its bound on the difference of the two results: round-off
 // that both frames share (the inputs conserve momentum only to 1e-16, and the closing gluon's momentum is the one the
@@ -157,8 +158,10 @@ static double twin_ward_fraction(int n) { (void)n; return 0.4; }
 // difference and on the residuals for n >= 6 (2^19 / 2^18 / 2^13 events at n = 6 / 7 / 8: 0.9 - 1.1 % left for double-double,
 // worst accepted error 4.1 / 5.2 / 0.8e-12), 5e-13 on the difference for n <= 5 (1.0 %, 4.1e-12)
 static double default_tau_twin_cobg(int n) { return n <= 5 ? 5e-13 : 1e-12; }
-static double twin_ward_fraction_cobg(int n) { return n <= 5 ? 2.0 : 1.0; }
-static double default_tau_cobg(int n) { return n <= 5 ? 1e-14 : 1e-13; }
+static double twin_ward_fraction_cobg(int n) { return n <= 5 ? 0.4 : 1.0; }
+// (large campaign, 16.8e6 events each: n = 6 left 7 events with residuals of 4 - 9.6e-14 unflagged at 1e-13, n = 5 two with
+// 3.6 - 5.5e-15 at 1e-14; n = 5 passed four events with residuals of 4 - 6.8e-13 through a second-stage bound of 1e-12)
+static double default_tau_cobg(int n) { return n <= 5 ? 3e-15 : 3e-14; }
 static const double kDefaultTauRho = 3e-3;
 
 static bool mode_supported(int n, int mode) {
